@@ -1,0 +1,143 @@
+/* liblsp -- C ABI of the B200-native (sm_100a) Llama decoder-layer forward+backward.
+ *
+ * The hot path is the one the Litespark report says its optimisations target: "the attention and MLP
+ * blocks" and their "forward and backward pass operations" (section 1) of a Llama layer
+ * built from RMSNorm [34], SwiGLU [35], RoPE [36] and GQA [37]/MHA (section 2.4), trained in
+ * BF16 mixed precision (section 2.5.2).  The paper gives no API; the calls below follow its
+ * statement of the problem -- one training step of one transformer layer -- in the reading fixed in
+ * DESIGN.md (SURVEY.md section 8(b),(c)).
+ *
+ * General contract
+ *  - Every pointer is a DEVICE pointer unless marked (host).  All buffers are caller-owned; the library never
+ *    allocates, frees or synchronises outside lsp_create / lsp_destroy.  All work is enqueued on `stream`
+ *    (a cudaStream_t passed as void*; NULL = legacy default stream).
+ *  - Layouts are row-major.  Tokens are sequence-major: token t = b*seq + s is row t of every [T,*] tensor,
+ *    T = batch*seq; every sequence starts at position 0.
+ *  - Weights are bf16, [out,in] (wq [Nq,H], wk/wv [Nkv,H], wo [H,Nq], w_gate/w_up [F,H], w_down [H,F]);
+ *    gains g_attn/g_mlp bf16 [H].  Nq = n_q_heads*head_dim, Nkv = n_kv_heads*head_dim.
+ *  - Inputs x, a, dy, da are `in_dtype` (bf16 or fp32) at the public entry points; every output activation
+ *    (a, y, dx, da) and every weight/gain gradient is fp32 (DESIGN.md precision plan P-1).
+ *  - `saved` (lsp_saved_bytes) is written by a forward call and read by the matching backward call.
+ *    `ws` (lsp_workspace_bytes) is scratch whose contents are undefined between calls.  Both must be
+ *    256-byte aligned.  All other pointers must be 16-byte aligned.
+ *  - Errors: every call returns an lsp_status; nothing throws or aborts across the ABI.  On error
+ *    lsp_last_error(ctx) returns a ctx-owned message.  There is no CPU fallback.
+ *  - Results are bit-reproducible run to run (no floating-point atomics anywhere).
+ */
+#ifndef LSP_H_
+#define LSP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lsp_ctx lsp_ctx;
+
+typedef enum {
+  LSP_OK = 0,
+  LSP_EINVAL = -1,        /* bad argument / NULL pointer */
+  LSP_EUNSUPPORTED = -2,  /* shape or option not supported (never a silent fallback) */
+  LSP_ENOMEM = -3,
+  LSP_ECUDA = -4,         /* a CUDA call or launch failed; see lsp_last_error */
+  LSP_EALIGN = -5         /* pointer alignment violated */
+} lsp_status;
+
+typedef enum { LSP_BF16 = 0, LSP_F32 = 1 } lsp_dtype;
+
+/* One decoder layer (Table 1 / section 2.4; BASELINE.json configs). */
+typedef struct {
+  int32_t batch, seq, hidden, n_q_heads, n_kv_heads, head_dim, ffn;
+  float rms_eps;            /* inside the sqrt, added to mean(x^2) (reading A-3) */
+  double rope_base;         /* theta_i = pos * base^(-2i/d), no scaling (reading A-5) */
+  int32_t rope_layout;      /* 0 = adjacent pairs (2i,2i+1) as in ref [36]; others: LSP_EUNSUPPORTED */
+  int32_t use_rope;         /* 1 in the layer path; 0 = no rotation */
+  int32_t in_dtype;         /* lsp_dtype of x / a / dy / da inputs */
+  int32_t wgrad_accumulate; /* 0 = overwrite weight gradients; 1: LSP_EUNSUPPORTED in this revision */
+} lsp_layer_desc;
+
+typedef struct {
+  const void *wq, *wk, *wv, *wo, *g_attn, *w_gate, *w_up, *w_down, *g_mlp;   /* bf16 */
+} lsp_layer_weights;
+
+typedef struct {
+  void *wq, *wk, *wv, *wo, *g_attn, *w_gate, *w_up, *w_down, *g_mlp;         /* fp32, same shapes */
+} lsp_layer_wgrads;
+
+/* Create a context for one layer shape on `cuda_device`.  Checks: n_q_heads % n_kv_heads == 0,
+ * head_dim in {64,128}, hidden/ffn/Nq/Nkv multiples of 8, hidden <= 8192.  The only call (with
+ * lsp_destroy) that allocates (RoPE cos/sin table [seq, head_dim/2], angles evaluated in fp64) or syncs. */
+lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device);
+lsp_status lsp_destroy(lsp_ctx* ctx);
+size_t lsp_saved_bytes(const lsp_ctx* ctx);
+size_t lsp_workspace_bytes(const lsp_ctx* ctx);
+const char* lsp_last_error(const lsp_ctx* ctx);
+
+/* Attention block:  a = x + Wo . GQA(RoPE(Wq xn), RoPE(Wk xn), Wv xn), xn = RMSNorm(x; g_attn).
+ *   x [T,H] in_dtype -> a_out [T,H] fp32. */
+lsp_status lsp_attn_fwd(lsp_ctx* ctx, const void* x, const lsp_layer_weights* w, void* a_out, void* saved, void* ws,
+                        void* stream);
+/* Backward of the attention block (B6-B10).  x: the forward input; da [T,H] in_dtype -> dx [T,H] fp32;
+ * writes grads->wq, wk, wv, wo, g_attn. */
+lsp_status lsp_attn_bwd(lsp_ctx* ctx, const void* x, const void* da, const lsp_layer_weights* w, const void* saved,
+                        void* dx, lsp_layer_wgrads* grads, void* ws, void* stream);
+
+/* MLP block (F5-F7):  y = a + Wd . (silu(Wg an) * (Wu an)), an = RMSNorm(a; g_mlp).  a [T,H] in_dtype -> y fp32. */
+lsp_status lsp_mlp_fwd(lsp_ctx* ctx, const void* a, const lsp_layer_weights* w, void* y_out, void* saved, void* ws,
+                       void* stream);
+/* Backward of the MLP block (B1-B5).  a: the forward input; dy in_dtype -> da fp32; writes grads->w_gate,
+ * w_up, w_down, g_mlp. */
+lsp_status lsp_mlp_bwd(lsp_ctx* ctx, const void* a, const void* dy, const lsp_layer_weights* w, const void* saved,
+                       void* da, lsp_layer_wgrads* grads, void* ws, void* stream);
+
+/* Whole layer = mlp o attn.  x in_dtype -> y fp32.  The intermediate `a` (fp32) lives in `saved`. */
+lsp_status lsp_layer_fwd(lsp_ctx* ctx, const void* x, const lsp_layer_weights* w, void* y_out, void* saved, void* ws,
+                         void* stream);
+/* x: the forward input; dy in_dtype -> dx fp32; writes all nine gradients. */
+lsp_status lsp_layer_bwd(lsp_ctx* ctx, const void* x, const void* dy, const lsp_layer_weights* w, const void* saved,
+                         void* dx, lsp_layer_wgrads* grads, void* ws, void* stream);
+
+/* Attention core only (BASELINE.json config 5; no projections, no RoPE):
+ *   q [B,S,nq,d], k,v [B,S,nkv,d], d_o [B,S,nq,d] bf16;  o, dq [B,S,nq,d], dk,dv [B,S,nkv,d] fp32;
+ *   lse [B,nq,S] fp32 = natural log-sum-exp of the scaled causal logits (reading A-6). */
+lsp_status lsp_sdpa_fwd(lsp_ctx* ctx, const void* q, const void* k, const void* v, void* o, float* lse, void* ws,
+                        void* stream);
+lsp_status lsp_sdpa_bwd(lsp_ctx* ctx, const void* q, const void* k, const void* v, const void* o, const float* lse,
+                        const void* d_o, void* dq, void* dk, void* dv, void* ws, void* stream);
+
+/* Embedding gather (config 3):  x0[t,:] = table[ids[t],:]; ids int32 [T], table bf16 [vocab,H] -> x0 fp32 [T,H]. */
+lsp_status lsp_embed_fwd(lsp_ctx* ctx, const int32_t* ids, const void* table, void* x0, void* stream);
+
+/* Building block / test hook: one bias-free linear-layer GEMM on the tcgen05 kernel, bf16 in, fp32 out.
+ *   op 0 (forward): C[M,N] = A[M,K] . B[N,K]^T        A,B row-major as written
+ *   op 1 (dgrad)  : C[M,N] = A[M,K] . B[K,N]          B row-major [K,N]
+ *   op 2 (wgrad)  : C[M,N] = A[K,M]^T . B[K,N]        A row-major [K,M], B row-major [K,N]
+ * lda/ldb/ldc are row pitches in elements (multiples of 8).  Needs no ctx state beyond the device. */
+lsp_status lsp_gemm(lsp_ctx* ctx, int op, int M, int N, int K, const void* A, int64_t lda, const void* B, int64_t ldb,
+                    float* C, int64_t ldc, void* stream);
+
+/* End-to-end step with HOST buffers (bench.py `e2e`): copies x, dy (in_dtype, [T,H]; pinned host memory for
+ * asynchronous copies) to the caller's device staging buffers x_dev / dy_dev, runs lsp_layer_fwd + lsp_layer_bwd,
+ * and copies y and dx (fp32 [T,H]) back to y_host / dx_host, all enqueued on `stream` (no sync).  Weights and
+ * weight gradients stay on the device (DEVICE pointers), as they do in a training step. */
+lsp_status lsp_layer_step_host(lsp_ctx* ctx, const void* x_host, const void* dy_host, const lsp_layer_weights* w,
+                               void* y_host, void* dx_host, lsp_layer_wgrads* grads, void* x_dev, void* dy_dev,
+                               void* y_dev, void* dx_dev, void* saved, void* ws, void* stream);
+
+/* Measurement aids; they change no result.
+ * lsp_launch_count: kernels launched through this context so far.
+ * lsp_timing_enable(n > 0): pre-create n CUDA-event pairs; from then on every pipeline stage records one pair on
+ *   the caller's stream (silently stops recording once the pairs are used up); n = 0 disables and frees them.
+ * lsp_timing_read: synchronises the recorded events, sums elapsed milliseconds and record counts per stage into the
+ *   caller's HOST arrays (names[i] points at a static string), resets the recorder, returns the number of stages
+ *   written (<= max_stages) or -1 on error. */
+long long lsp_launch_count(const lsp_ctx* ctx);
+lsp_status lsp_timing_enable(lsp_ctx* ctx, int max_records);
+int lsp_timing_read(lsp_ctx* ctx, int max_stages, const char** names, float* total_ms, int* records);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LSP_H_ */

@@ -1,0 +1,210 @@
+"""Thin ctypes binding over liblsp.so (include/lsp.h): argument marshalling only.
+
+Every function has the name and argument order of its C entry point; tensors are torch CUDA tensors
+(PyTorch is used for device memory and streams only) passed as raw device pointers.  There is no CPU
+fallback: if liblsp.so is missing or a call fails, this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "liblsp.so")
+
+LSP_BF16, LSP_F32 = 0, 1
+STATUS = {0: "LSP_OK", -1: "LSP_EINVAL", -2: "LSP_EUNSUPPORTED", -3: "LSP_ENOMEM", -4: "LSP_ECUDA", -5: "LSP_EALIGN"}
+WEIGHT_FIELDS = ("wq", "wk", "wv", "wo", "g_attn", "w_gate", "w_up", "w_down", "g_mlp")
+EXPORTS = ("lsp_create", "lsp_destroy", "lsp_saved_bytes", "lsp_workspace_bytes", "lsp_last_error",
+           "lsp_attn_fwd", "lsp_attn_bwd", "lsp_mlp_fwd", "lsp_mlp_bwd", "lsp_layer_fwd", "lsp_layer_bwd",
+           "lsp_sdpa_fwd", "lsp_sdpa_bwd", "lsp_embed_fwd", "lsp_gemm", "lsp_layer_step_host", "lsp_launch_count",
+           "lsp_timing_enable", "lsp_timing_read")
+
+
+class LspError(RuntimeError):
+    pass
+
+
+class lsp_layer_desc(C.Structure):
+    _fields_ = [("batch", C.c_int32), ("seq", C.c_int32), ("hidden", C.c_int32), ("n_q_heads", C.c_int32),
+                ("n_kv_heads", C.c_int32), ("head_dim", C.c_int32), ("ffn", C.c_int32), ("rms_eps", C.c_float),
+                ("rope_base", C.c_double), ("rope_layout", C.c_int32), ("use_rope", C.c_int32),
+                ("in_dtype", C.c_int32), ("wgrad_accumulate", C.c_int32)]
+
+
+class lsp_layer_weights(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in WEIGHT_FIELDS]
+
+
+class lsp_layer_wgrads(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in WEIGHT_FIELDS]
+
+
+_lib = None
+
+
+def lib():
+    """Load liblsp.so (raises if it has not been built: there is no fallback path)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise LspError(f"{LIB_PATH} not found: build it with `python -m paper_2510_02483_b200.build`")
+        L = C.CDLL(LIB_PATH)
+        vp, i32, i64 = C.c_void_p, C.c_int, C.c_int64
+        L.lsp_create.argtypes = [C.POINTER(vp), C.POINTER(lsp_layer_desc), i32]
+        L.lsp_destroy.argtypes = [vp]
+        L.lsp_saved_bytes.argtypes = [vp]; L.lsp_saved_bytes.restype = C.c_size_t
+        L.lsp_workspace_bytes.argtypes = [vp]; L.lsp_workspace_bytes.restype = C.c_size_t
+        L.lsp_last_error.argtypes = [vp]; L.lsp_last_error.restype = C.c_char_p
+        pw, pg = C.POINTER(lsp_layer_weights), C.POINTER(lsp_layer_wgrads)
+        L.lsp_attn_fwd.argtypes = [vp, vp, pw, vp, vp, vp, vp]
+        L.lsp_attn_bwd.argtypes = [vp, vp, vp, pw, vp, vp, pg, vp, vp]
+        L.lsp_mlp_fwd.argtypes = [vp, vp, pw, vp, vp, vp, vp]
+        L.lsp_mlp_bwd.argtypes = [vp, vp, vp, pw, vp, vp, pg, vp, vp]
+        L.lsp_layer_fwd.argtypes = [vp, vp, pw, vp, vp, vp, vp]
+        L.lsp_layer_bwd.argtypes = [vp, vp, vp, pw, vp, vp, pg, vp, vp]
+        L.lsp_sdpa_fwd.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
+        L.lsp_sdpa_bwd.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.lsp_embed_fwd.argtypes = [vp, vp, vp, vp, vp]
+        L.lsp_gemm.argtypes = [vp, i32, i32, i32, i32, vp, i64, vp, i64, vp, i64, vp]
+        L.lsp_layer_step_host.argtypes = [vp, vp, vp, pw, vp, vp, pg, vp, vp, vp, vp, vp, vp, vp]
+        L.lsp_launch_count.argtypes = [vp]; L.lsp_launch_count.restype = C.c_longlong
+        L.lsp_timing_enable.argtypes = [vp, i32]
+        L.lsp_timing_read.argtypes = [vp, i32, C.POINTER(C.c_char_p), C.POINTER(C.c_float), C.POINTER(i32)]
+        for n in EXPORTS:
+            if n not in ("lsp_saved_bytes", "lsp_workspace_bytes", "lsp_last_error", "lsp_launch_count"):
+                getattr(L, n).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return C.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+def _pack(struct_t, tensors: dict):
+    s = struct_t()
+    for n in WEIGHT_FIELDS:
+        t = tensors.get(n)
+        setattr(s, n, None if t is None else t.data_ptr())
+    return s
+
+
+class Ctx:
+    """Owns one lsp_ctx (a layer shape on a device)."""
+
+    def __init__(self, *, batch, seq, hidden, n_q_heads, n_kv_heads, head_dim, ffn, rms_eps=1e-5, rope_base=10000.0,
+                 use_rope=True, in_dtype=LSP_BF16, device=0):
+        self.desc = lsp_layer_desc(batch, seq, hidden, n_q_heads, n_kv_heads, head_dim, ffn, rms_eps, rope_base, 0,
+                                   1 if use_rope else 0, in_dtype, 0)
+        self.handle = C.c_void_p()
+        st = lib().lsp_create(C.byref(self.handle), C.byref(self.desc), device)
+        if st != 0:
+            self.handle = None
+            raise LspError(f"lsp_create failed: {STATUS.get(st, st)}")
+
+    def close(self):
+        if self.handle:
+            lib().lsp_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def check(self, st):
+        if st != 0:
+            raise LspError(f"{STATUS.get(st, st)}: {lib().lsp_last_error(self.handle).decode()}")
+
+    @property
+    def saved_bytes(self):
+        return lib().lsp_saved_bytes(self.handle)
+
+    @property
+    def workspace_bytes(self):
+        return lib().lsp_workspace_bytes(self.handle)
+
+
+def lsp_attn_fwd(ctx, x, weights, a_out, saved, ws, stream=None):
+    w = _pack(lsp_layer_weights, weights)
+    ctx.check(lib().lsp_attn_fwd(ctx.handle, _ptr(x), C.byref(w), _ptr(a_out), _ptr(saved), _ptr(ws), _stream(stream)))
+
+
+def lsp_attn_bwd(ctx, x, da, weights, saved, dx, grads, ws, stream=None):
+    w, g = _pack(lsp_layer_weights, weights), _pack(lsp_layer_wgrads, grads)
+    ctx.check(lib().lsp_attn_bwd(ctx.handle, _ptr(x), _ptr(da), C.byref(w), _ptr(saved), _ptr(dx), C.byref(g), _ptr(ws),
+                                 _stream(stream)))
+
+
+def lsp_mlp_fwd(ctx, a, weights, y_out, saved, ws, stream=None):
+    w = _pack(lsp_layer_weights, weights)
+    ctx.check(lib().lsp_mlp_fwd(ctx.handle, _ptr(a), C.byref(w), _ptr(y_out), _ptr(saved), _ptr(ws), _stream(stream)))
+
+
+def lsp_mlp_bwd(ctx, a, dy, weights, saved, da, grads, ws, stream=None):
+    w, g = _pack(lsp_layer_weights, weights), _pack(lsp_layer_wgrads, grads)
+    ctx.check(lib().lsp_mlp_bwd(ctx.handle, _ptr(a), _ptr(dy), C.byref(w), _ptr(saved), _ptr(da), C.byref(g), _ptr(ws),
+                                _stream(stream)))
+
+
+def lsp_layer_fwd(ctx, x, weights, y_out, saved, ws, stream=None):
+    w = _pack(lsp_layer_weights, weights)
+    ctx.check(lib().lsp_layer_fwd(ctx.handle, _ptr(x), C.byref(w), _ptr(y_out), _ptr(saved), _ptr(ws), _stream(stream)))
+
+
+def lsp_layer_bwd(ctx, x, dy, weights, saved, dx, grads, ws, stream=None):
+    w, g = _pack(lsp_layer_weights, weights), _pack(lsp_layer_wgrads, grads)
+    ctx.check(lib().lsp_layer_bwd(ctx.handle, _ptr(x), _ptr(dy), C.byref(w), _ptr(saved), _ptr(dx), C.byref(g), _ptr(ws),
+                                  _stream(stream)))
+
+
+def lsp_sdpa_fwd(ctx, q, k, v, o, lse, ws, stream=None):
+    ctx.check(lib().lsp_sdpa_fwd(ctx.handle, _ptr(q), _ptr(k), _ptr(v), _ptr(o), _ptr(lse), _ptr(ws), _stream(stream)))
+
+
+def lsp_sdpa_bwd(ctx, q, k, v, o, lse, d_o, dq, dk, dv, ws, stream=None):
+    ctx.check(lib().lsp_sdpa_bwd(ctx.handle, _ptr(q), _ptr(k), _ptr(v), _ptr(o), _ptr(lse), _ptr(d_o), _ptr(dq), _ptr(dk),
+                                 _ptr(dv), _ptr(ws), _stream(stream)))
+
+
+def lsp_embed_fwd(ctx, ids, table, x0, stream=None):
+    ctx.check(lib().lsp_embed_fwd(ctx.handle, _ptr(ids), _ptr(table), _ptr(x0), _stream(stream)))
+
+
+def lsp_gemm(ctx, op, M, N, K, A, lda, B, ldb, Cout, ldc, stream=None):
+    ctx.check(lib().lsp_gemm(ctx.handle, op, M, N, K, _ptr(A), lda, _ptr(B), ldb, _ptr(Cout), ldc, _stream(stream)))
+
+
+def lsp_layer_step_host(ctx, x_host, dy_host, weights, y_host, dx_host, grads, x_dev, dy_dev, y_dev, dx_dev, saved, ws,
+                        stream=None):
+    w, g = _pack(lsp_layer_weights, weights), _pack(lsp_layer_wgrads, grads)
+    ctx.check(lib().lsp_layer_step_host(ctx.handle, _ptr(x_host), _ptr(dy_host), C.byref(w), _ptr(y_host), _ptr(dx_host),
+                                        C.byref(g), _ptr(x_dev), _ptr(dy_dev), _ptr(y_dev), _ptr(dx_dev), _ptr(saved),
+                                        _ptr(ws), _stream(stream)))
+
+
+def lsp_launch_count(ctx) -> int:
+    return int(lib().lsp_launch_count(ctx.handle))
+
+
+def lsp_timing_enable(ctx, max_records: int):
+    ctx.check(lib().lsp_timing_enable(ctx.handle, max_records))
+
+
+def lsp_timing_read(ctx) -> dict:
+    """{stage name: (total_ms, records)} for the stages recorded since the last read."""
+    n = 64
+    names, ms, cnt = (C.c_char_p * n)(), (C.c_float * n)(), (C.c_int * n)()
+    k = lib().lsp_timing_read(ctx.handle, n, names, ms, cnt)
+    if k < 0:
+        raise LspError("lsp_timing_read failed")
+    return {names[i].decode(): (float(ms[i]), int(cnt[i])) for i in range(k) if cnt[i] > 0}

@@ -1,0 +1,451 @@
+// Persistent warp-specialised tcgen05 GEMM for sm_100a with fused epilogues.
+//
+//   C[M,N] = sum over K-segments s of  A_s[M,K_s] * B_s[N,K_s]^T        (fp32 accumulate in TMEM)
+//
+// Operands are 16-bit (bf16), fetched by TMA into 128B-swizzled shared memory in a multi-stage
+// mbarrier ring; either operand may be K-major (row = M/N index, K contiguous) or MN-major
+// (row = K index, M/N contiguous) so that dgrad (dX = dY W) and wgrad (dW = dY^T X) run on the
+// tensors as they lie in HBM -- no transposes.  One elected thread issues tcgen05.mma
+// (128 x BN x 16, cta_group::1); two TMEM accumulator stages let the 4 epilogue warps drain tile i
+// (tcgen05.ld -> registers -> fused epilogue -> global) while the tensor core works on tile i+1.
+//
+// DUAL mode: B tile rows [0,128) come from b[0] and rows [128,256) from b[1] (same 128 output columns);
+// one 128x256 MMA then yields both the gate and the up projection, which the SwiGLU epilogue combines.
+//
+// Warp roles (192 threads): warp 0 = TMA producer, warp 1 = MMA issuer + TMEM owner, warps 2..5 = epilogue.
+#pragma once
+#include "ptx.cuh"
+
+namespace lsp {
+
+enum : int { DT_BF16 = 0, DT_F32 = 1, DT_F16 = 2 };
+
+constexpr int GEMM_BM = 128;
+constexpr int GEMM_BK = 64;          // 64 x 16-bit = one 128-byte swizzle row
+constexpr int GEMM_THREADS = 192;
+constexpr int GEMM_MAX_SEG = 3;
+
+struct GemmMaps {
+  CUtensorMap a[GEMM_MAX_SEG];
+  CUtensorMap b[GEMM_MAX_SEG];
+};
+struct GemmShape {
+  int M, N;                          // output extent (DUAL: N = columns of each of the two outputs)
+  int nseg;                          // number of K segments (non-DUAL); DUAL uses a[0], b[0], b[1]
+  int kblocks[GEMM_MAX_SEG];         // ceil(K_s / 64)
+};
+
+template <int BN> struct GemmCfg {
+  static constexpr int A_BYTES = GEMM_BM * GEMM_BK * 2;
+  static constexpr int B_BYTES = BN * GEMM_BK * 2;
+  static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+  static constexpr int STAGES = (BN == 256) ? 4 : 6;
+  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
+  static constexpr int TMEM_COLS = 2 * BN;   // two accumulator stages (power of two: 256 or 512)
+};
+
+// ------------------------------------------------------------------------------------------- store helpers
+template <int DT> struct OutElem;
+template <> struct OutElem<DT_BF16> { using type = __nv_bfloat16; };
+template <> struct OutElem<DT_F16> { using type = __half; };
+template <> struct OutElem<DT_F32> { using type = float; };
+
+// Write up to 32 consecutive values of one row (nvalid is a multiple of 8; p is 16-byte aligned).
+template <int DT>
+__device__ __forceinline__ void store_row32(void* p, const float (&v)[32], int nvalid) {
+  if constexpr (DT == DT_F32) {
+    float4* q = reinterpret_cast<float4*>(p);
+#pragma unroll
+    for (int j = 0; j < 8; ++j)
+      if (4 * j + 4 <= nvalid) q[j] = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+  } else {
+    uint4* q = reinterpret_cast<uint4*>(p);
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+      if (8 * j + 8 <= nvalid) {
+        uint4 w;
+        if constexpr (DT == DT_BF16) {
+          w.x = pack_bf16(v[8 * j], v[8 * j + 1]); w.y = pack_bf16(v[8 * j + 2], v[8 * j + 3]);
+          w.z = pack_bf16(v[8 * j + 4], v[8 * j + 5]); w.w = pack_bf16(v[8 * j + 6], v[8 * j + 7]);
+        } else {
+          w.x = pack_f16(v[8 * j], v[8 * j + 1]); w.y = pack_f16(v[8 * j + 2], v[8 * j + 3]);
+          w.z = pack_f16(v[8 * j + 4], v[8 * j + 5]); w.w = pack_f16(v[8 * j + 6], v[8 * j + 7]);
+        }
+        q[j] = w;
+      }
+  }
+}
+// Read up to 32 consecutive values of one row into fp32.
+template <int DT>
+__device__ __forceinline__ void load_row32(const void* p, float (&v)[32], int nvalid) {
+  if constexpr (DT == DT_F32) {
+    const float4* q = reinterpret_cast<const float4*>(p);
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      float4 t = (4 * j + 4 <= nvalid) ? __ldg(q + j) : make_float4(0.f, 0.f, 0.f, 0.f);
+      v[4 * j] = t.x; v[4 * j + 1] = t.y; v[4 * j + 2] = t.z; v[4 * j + 3] = t.w;
+    }
+  } else {
+    const uint4* q = reinterpret_cast<const uint4*>(p);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      uint4 t = (8 * j + 8 <= nvalid) ? __ldg(q + j) : make_uint4(0, 0, 0, 0);
+      const uint32_t w[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        if constexpr (DT == DT_BF16) {
+          v[8 * j + 2 * e] = bf16_lo(w[e]); v[8 * j + 2 * e + 1] = bf16_hi(w[e]);
+        } else {
+          const __half2 h = *reinterpret_cast<const __half2*>(&w[e]);
+          v[8 * j + 2 * e] = __low2float(h); v[8 * j + 2 * e + 1] = __high2float(h);
+        }
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------- epilogues
+// Plain store with optional residual add and up to three row-segments of output (wgrad of fused QKV / gate-up).
+template <int ODT, int RDT, bool HAS_RES>
+struct EpiStore {
+  void* out[3];
+  int split1, split2;        // rows [0,split1) -> out[0], [split1,split2) -> out[1], [split2,M) -> out[2]
+  long long ld;              // row pitch (elements) of every output and of the residual
+  const void* res;
+  float alpha;
+  __device__ __forceinline__ void operator()(int m, int n, float (&v)[32], int nvalid) const {
+    using OT = typename OutElem<ODT>::type;
+    int seg = (m >= split1) + (m >= split2);
+    int mr = m - (seg == 0 ? 0 : (seg == 1 ? split1 : split2));
+    if (alpha != 1.0f) {
+#pragma unroll
+      for (int j = 0; j < 32; ++j) v[j] *= alpha;
+    }
+    if constexpr (HAS_RES) {
+      using RT = typename OutElem<RDT>::type;
+      float r[32];
+      load_row32<RDT>(reinterpret_cast<const RT*>(res) + static_cast<long long>(m) * ld + n, r, nvalid);
+#pragma unroll
+      for (int j = 0; j < 32; ++j) v[j] += r[j];
+    }
+    store_row32<ODT>(reinterpret_cast<OT*>(out[seg]) + static_cast<long long>(mr) * ld + n, v, nvalid);
+  }
+};
+
+// Projection output with fused RoPE (adjacent pairs (2i,2i+1), ref [36]); fp16 out.
+// rope table: float2 (cos, sin) [S, d/2], angles computed in fp64 on the host (reading A-5).
+template <bool ROPE>
+struct EpiProjRope {
+  __half* out; long long ld; int col_off;   // output row pitch, first output column of this projection
+  const float2* rope; int S, d;
+  __device__ __forceinline__ void operator()(int m, int n, float (&v)[32], int nvalid) const {
+    if constexpr (ROPE) {
+      const int pos = m % S;
+      const float2* t = rope + static_cast<long long>(pos) * (d >> 1) + ((n % d) >> 1);
+#pragma unroll
+      for (int j = 0; j < 16; ++j) {
+        if (2 * j + 2 <= nvalid) {
+          const float2 cs = __ldg(t + j);
+          const float z0 = v[2 * j], z1 = v[2 * j + 1];
+          v[2 * j] = z0 * cs.x - z1 * cs.y;
+          v[2 * j + 1] = z0 * cs.y + z1 * cs.x;
+        }
+      }
+    }
+    store_row32<DT_F16>(out + static_cast<long long>(m) * ld + col_off + n, v, nvalid);
+  }
+};
+
+// DUAL epilogue: h = silu(g) * u (ref [35]); saves g,u in fp16 for the backward (DESIGN.md precision plan).
+struct EpiSwiGLU {
+  __nv_bfloat16* h; __half* g16; __half* u16; long long ld;
+  __device__ __forceinline__ void operator()(int m, int n, float (&g)[32], float (&u)[32], int nvalid) const {
+    const long long off = static_cast<long long>(m) * ld + n;
+    store_row32<DT_F16>(g16 + off, g, nvalid);
+    store_row32<DT_F16>(u16 + off, u, nvalid);
+    float hv[32];
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+      const float sg = 1.0f / (1.0f + __expf(-g[j]));
+      hv[j] = g[j] * sg * u[j];
+    }
+    store_row32<DT_BF16>(h + off, hv, nvalid);
+  }
+};
+
+// Down-projection dgrad with fused SwiGLU backward: acc = dh; writes [dg | du] (bf16) into one [T, 2F] buffer.
+struct EpiSwiGLUBwd {
+  const __half* g16; const __half* u16; long long ld;      // saved g,u [T,F]
+  __nv_bfloat16* dgu; int F;                               // [T, 2F]
+  __device__ __forceinline__ void operator()(int m, int n, float (&dh)[32], int nvalid) const {
+    float g[32], u[32];
+    const long long off = static_cast<long long>(m) * ld + n;
+    load_row32<DT_F16>(g16 + off, g, nvalid);
+    load_row32<DT_F16>(u16 + off, u, nvalid);
+    float dg[32], du[32];
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+      const float sg = 1.0f / (1.0f + __expf(-g[j]));
+      du[j] = dh[j] * g[j] * sg;
+      dg[j] = dh[j] * u[j] * sg * (1.0f + g[j] * (1.0f - sg));
+    }
+    __nv_bfloat16* row = dgu + static_cast<long long>(m) * (2LL * F);
+    store_row32<DT_BF16>(row + n, dg, nvalid);
+    store_row32<DT_BF16>(row + F + n, du, nvalid);
+  }
+};
+
+// ------------------------------------------------------------------------------------------- the kernel
+template <int BN, bool A_MN, bool B_MN, bool DUAL, class Epi>
+__global__ void __launch_bounds__(GEMM_THREADS, 1)
+gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, const Epi epi) {
+  using Cfg = GemmCfg<BN>;
+  constexpr int STAGES = Cfg::STAGES;
+  constexpr int NOUT = DUAL ? BN / 2 : BN;       // output columns covered by one tile
+  static_assert(!DUAL || (BN == 256 && !A_MN && !B_MN), "DUAL is the forward gate/up GEMM");
+
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bar_base = smem_base + STAGES * Cfg::STAGE_BYTES;
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
+  auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * STAGES + s); };
+  auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * STAGES + 2 + s); };
+  const uint32_t tmem_slot = bar_base + 8u * (2 * STAGES + 4);
+  uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+
+  const int mblocks = (sh.M + GEMM_BM - 1) / GEMM_BM;
+  const int nblocks = (sh.N + NOUT - 1) / NOUT;
+  const int ntiles = mblocks * nblocks;
+  int kb_total = 0;
+  const int nseg = DUAL ? 1 : sh.nseg;
+  for (int s = 0; s < nseg; ++s) kb_total += sh.kblocks[s];
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < nseg; ++s) { tma_prefetch_desc(&maps.a[s]); tma_prefetch_desc(&maps.b[s]); }
+    if (DUAL) tma_prefetch_desc(&maps.b[1]);
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+    for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 4); }
+    fence_barrier_init();
+  }
+  if (warp == 1) {
+    tmem_alloc(tmem_slot, Cfg::TMEM_COLS);
+    tmem_relinquish();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot_ptr;
+
+  if (warp == 0) {
+    // ===================================================================== TMA producer
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int m0 = (tile % mblocks) * GEMM_BM;
+        const int n0 = (tile / mblocks) * NOUT;
+        for (int s = 0; s < nseg; ++s) {
+          for (int kb = 0; kb < sh.kblocks[s]; ++kb) {
+            mbar_wait(empty_bar(stage), phase ^ 1u);
+            const uint32_t sa = smem_base + stage * Cfg::STAGE_BYTES;
+            const uint32_t sb = sa + Cfg::A_BYTES;
+            const uint32_t fb = full_bar(stage);
+            mbar_expect_tx(fb, Cfg::STAGE_BYTES);
+            const int k0 = kb * GEMM_BK;
+            if constexpr (!A_MN) {
+              tma_load_2d(sa, &maps.a[s], fb, k0, m0);                       // box {64 k, 128 rows}
+            } else {
+#pragma unroll
+              for (int c = 0; c < GEMM_BM / 64; ++c)                          // box {64 m, 64 k-rows} per chunk
+                tma_load_2d(sa + c * (GEMM_BK * 128), &maps.a[s], fb, m0 + 64 * c, k0);
+            }
+            if constexpr (DUAL) {
+              tma_load_2d(sb, &maps.b[0], fb, k0, n0);                       // gate rows [0,128)
+              tma_load_2d(sb + 128 * 128, &maps.b[1], fb, k0, n0);           // up   rows [128,256)
+            } else if constexpr (!B_MN) {
+              tma_load_2d(sb, &maps.b[s], fb, k0, n0);                       // box {64 k, BN rows}
+            } else {
+#pragma unroll
+              for (int c = 0; c < BN / 64; ++c)
+                tma_load_2d(sb + c * (GEMM_BK * 128), &maps.b[s], fb, n0 + 64 * c, k0);
+            }
+            if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================================================================== MMA issuer
+    if (lane == 0) {
+      constexpr uint32_t idesc = umma_idesc(GEMM_BM, BN, 1, 1, A_MN ? 1 : 0, B_MN ? 1 : 0);
+      // K-major: atoms of 8 rows x 128 B, SBO = 1024; one UMMA_K (16 elems) = +32 B inside the swizzle row.
+      // MN-major: LBO = bytes between 64-wide M/N chunks (BK*128), SBO = 1024 between 8-k-row atoms;
+      //           one UMMA_K (16 k-rows) = +2048 B.
+      constexpr uint32_t A_LBO = A_MN ? GEMM_BK * 128 : 16, B_LBO = B_MN ? GEMM_BK * 128 : 16;
+      constexpr uint32_t A_KSTEP = A_MN ? 2048 : 32, B_KSTEP = B_MN ? 2048 : 32;
+      int stage = 0; uint32_t phase = 0;
+      int acc = 0; uint32_t acc_phase = 0;
+      for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
+        tc_fence_after();
+        const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(acc * BN);
+        for (int kb = 0; kb < kb_total; ++kb) {
+          mbar_wait(full_bar(stage), phase);
+          tc_fence_after();
+          const uint32_t sa = smem_base + stage * Cfg::STAGE_BYTES;
+          const uint32_t sb = sa + Cfg::A_BYTES;
+#pragma unroll
+          for (int k = 0; k < GEMM_BK / 16; ++k) {
+            const uint64_t ad = umma_smem_desc(sa + k * A_KSTEP, A_LBO, 1024);
+            const uint64_t bd = umma_smem_desc(sb + k * B_KSTEP, B_LBO, 1024);
+            umma_f16(d_tmem, ad, bd, idesc, (kb | k) != 0 ? 1u : 0u);
+          }
+          umma_commit(empty_bar(stage));        // smem slot reusable once these MMAs have read it
+          if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+        }
+        umma_commit(tfull_bar(acc));             // accumulator complete -> epilogue
+        if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+      }
+    }
+  } else {
+    // ===================================================================== epilogue warps (2..5)
+    const int quarter = warp & 3;               // TMEM lanes [32*quarter, 32*quarter+32) are this warp's
+    int acc = 0; uint32_t acc_phase = 0;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+      const int m0 = (tile % mblocks) * GEMM_BM;
+      const int n0 = (tile / mblocks) * NOUT;
+      mbar_wait(tfull_bar(acc), acc_phase);
+      tc_fence_after();
+      const int m = m0 + quarter * 32 + lane;
+      const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + static_cast<uint32_t>(acc * BN);
+#pragma unroll 1
+      for (int c = 0; c < NOUT / 32; ++c) {
+        const int n = n0 + c * 32;
+        if (n >= sh.N) break;                   // warp-uniform
+        const int nvalid = min(32, sh.N - n);
+        uint32_t r0[32];
+        tmem_ld32(t_row + c * 32, r0);
+        if constexpr (DUAL) {
+          uint32_t r1[32];
+          tmem_ld32(t_row + NOUT + c * 32, r1);
+          tmem_ld_wait();
+          if (m < sh.M) epi(m, n, reinterpret_cast<float(&)[32]>(r0), reinterpret_cast<float(&)[32]>(r1), nvalid);
+        } else {
+          tmem_ld_wait();
+          if (m < sh.M) epi(m, n, reinterpret_cast<float(&)[32]>(r0), nvalid);
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(tempty_bar(acc));
+      if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc(tmem_base, Cfg::TMEM_COLS);
+  }
+}
+
+// ------------------------------------------------------------------------------------------- host side
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+inline PFN_encodeTiled get_encode_fn() {
+  static PFN_encodeTiled fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<PFN_encodeTiled>(p);
+  }
+  return fn;
+}
+
+// 2-D tensor map over a row-major 16-bit matrix [rows, cols] with pitch ld (elements):
+// box = {64 contiguous elements, box_rows}, 128-byte swizzle, out-of-bounds reads return zero.
+inline bool make_map_2d(CUtensorMap* m, const void* base, long long rows, long long cols, long long ld, int box_rows,
+                        bool f16 = false) {
+  PFN_encodeTiled fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[2] = {static_cast<cuuint64_t>(cols), static_cast<cuuint64_t>(rows)};
+  cuuint64_t strides[1] = {static_cast<cuuint64_t>(ld) * 2};
+  cuuint32_t box[2] = {64u, static_cast<cuuint32_t>(box_rows)};
+  cuuint32_t estr[2] = {1u, 1u};
+  CUresult r = fn(m, f16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2,
+                  const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS;
+}
+
+// One operand of one K-segment as it lies in memory.
+struct Operand {
+  const void* ptr;
+  long long ld;       // pitch in elements
+  bool mn_major;      // false: [MN, K] row-major (K contiguous); true: [K, MN] row-major (MN contiguous)
+};
+
+// Encode the map of an operand with logical extents (mn, k); rows_box = tile rows for K-major.
+inline bool encode_operand(CUtensorMap* m, const Operand& o, long long mn, long long k, int tile_mn) {
+  if (!o.mn_major) return make_map_2d(m, o.ptr, mn, k, o.ld, tile_mn);
+  return make_map_2d(m, o.ptr, k, mn, o.ld, GEMM_BK);
+}
+
+template <int BN, bool A_MN, bool B_MN, bool DUAL, class Epi>
+cudaError_t launch_gemm(const GemmMaps& maps, const GemmShape& sh, const Epi& epi, int num_sms, cudaStream_t st) {
+  using Cfg = GemmCfg<BN>;
+  auto kern = gemm_tcgen05_kernel<BN, A_MN, B_MN, DUAL, Epi>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  constexpr int NOUT = DUAL ? BN / 2 : BN;
+  const int mblocks = (sh.M + GEMM_BM - 1) / GEMM_BM, nblocks = (sh.N + NOUT - 1) / NOUT;
+  const int ntiles = mblocks * nblocks;
+  if (ntiles == 0) return cudaSuccess;
+  const int grid = ntiles < num_sms ? ntiles : num_sms;
+  kern<<<grid, GEMM_THREADS, Cfg::SMEM_BYTES, st>>>(maps, sh, epi);
+  return cudaGetLastError();
+}
+
+// Generic entry: up to three K-segments (A_s, B_s, K_s); all segments share the operand majors.
+template <int BN, bool A_MN, bool B_MN, class Epi>
+cudaError_t gemm_run(int M, int N, int nseg, const Operand* a, const Operand* b, const int* ks, const Epi& epi,
+                     int num_sms, cudaStream_t st) {
+  GemmMaps maps;
+  GemmShape sh;
+  sh.M = M; sh.N = N; sh.nseg = nseg;
+  for (int s = 0; s < GEMM_MAX_SEG; ++s) sh.kblocks[s] = 0;
+  for (int s = 0; s < nseg; ++s) {
+    sh.kblocks[s] = (ks[s] + GEMM_BK - 1) / GEMM_BK;
+    if (!encode_operand(&maps.a[s], a[s], M, ks[s], GEMM_BM)) return cudaErrorInvalidValue;
+    if (!encode_operand(&maps.b[s], b[s], N, ks[s], BN)) return cudaErrorInvalidValue;
+  }
+  return launch_gemm<BN, A_MN, B_MN, false, Epi>(maps, sh, epi, num_sms, st);
+}
+
+// Forward gate/up GEMM (DUAL): A [M,K], Wg/Wu [N,K] all K-major.
+template <class Epi>
+cudaError_t gemm_run_dual(int M, int N, int K, const Operand& a, const Operand& bg, const Operand& bu, const Epi& epi,
+                          int num_sms, cudaStream_t st) {
+  GemmMaps maps;
+  GemmShape sh;
+  sh.M = M; sh.N = N; sh.nseg = 1;
+  sh.kblocks[0] = (K + GEMM_BK - 1) / GEMM_BK; sh.kblocks[1] = sh.kblocks[2] = 0;
+  if (!encode_operand(&maps.a[0], a, M, K, GEMM_BM)) return cudaErrorInvalidValue;
+  if (!encode_operand(&maps.b[0], bg, N, K, 128)) return cudaErrorInvalidValue;
+  if (!encode_operand(&maps.b[1], bu, N, K, 128)) return cudaErrorInvalidValue;
+  return launch_gemm<256, false, false, true, Epi>(maps, sh, epi, num_sms, st);
+}
+
+}  // namespace lsp

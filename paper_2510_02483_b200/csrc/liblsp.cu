@@ -1,0 +1,708 @@
+// liblsp -- host side of the C ABI declared in include/lsp.h: argument checks, buffer carving and the
+// kernel sequence of one Llama decoder layer forward / backward.
+// Every step of the path runs in the kernels of gemm.cuh / attn.cuh / norm.cuh; nothing is computed on the host
+// except the RoPE angle table (fp64, once, at lsp_create).
+#include "../../include/lsp.h"
+
+#include <math.h>
+#include <stdarg.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "attn.cuh"
+#include "gemm.cuh"
+#include "norm.cuh"
+
+using namespace lsp;
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
+
+// Byte offsets inside `saved` and `ws` (all 256-byte aligned).
+struct SavedLayout {
+  size_t a32, xn, rstd1, qkv16, o32, o16, lse, an, rstd2, g16, u16, h, total;
+};
+struct WsLayout {
+  size_t in16, dgu, dn32, da32, da16, dO16, dvec, dqkv16, dgpart, q16, k16, v16, total;
+};
+
+}  // namespace
+
+// Pipeline stages (for launch counting and the optional per-stage device timing of lsp_timing_*).
+enum Stage : int {
+  ST_CAST = 0, ST_NORM_FWD, ST_QKV, ST_ATTN_FWD, ST_OPROJ, ST_GATEUP, ST_DOWN,
+  ST_WGRAD_DOWN, ST_DGRAD_DOWN, ST_WGRAD_GATEUP, ST_DGRAD_GATEUP, ST_NORM_BWD,
+  ST_WGRAD_O, ST_DGRAD_O, ST_DVEC, ST_ATTN_BWD, ST_WGRAD_QKV, ST_DGRAD_QKV, ST_EMBED, ST_COUNT
+};
+static const char* const STAGE_NAMES[ST_COUNT] = {
+  "cast", "rmsnorm_fwd", "gemm_qkv_rope", "attn_fwd", "gemm_oproj_res", "gemm_gateup_swiglu", "gemm_down_res",
+  "wgrad_down", "dgrad_down_swiglu_bwd", "wgrad_gateup", "dgrad_gateup", "rmsnorm_bwd",
+  "wgrad_oproj", "dgrad_oproj", "attn_dvec", "attn_bwd", "wgrad_qkv", "dgrad_qkv", "embed_gather"};
+
+struct TimingRec { int stage; cudaEvent_t beg, end; };
+
+struct lsp_ctx {
+  long long launches;                 // kernels launched through this context (cumulative)
+  int timing_on;
+  std::vector<TimingRec>* recs;       // pre-created event pairs
+  int recs_used;
+  lsp_layer_desc d;
+  int device, num_sms;
+  int T, Nq, Nkv, Nqkv, G;
+  float2* rope;         // [seq, head_dim/2] (cos, sin), device
+  int norm_blocks;      // persistent grid of the RMSNorm backward
+  SavedLayout sv;
+  WsLayout ws;
+  char err[512];
+};
+
+namespace {
+
+lsp_status fail(lsp_ctx* c, lsp_status s, const char* fmt, ...) {
+  if (c) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(c->err, sizeof(c->err), fmt, ap);
+    va_end(ap);
+  }
+  return s;
+}
+
+#define LSP_CUDA(call)                                                                                   \
+  do {                                                                                                   \
+    cudaError_t e__ = (call);                                                                            \
+    if (e__ != cudaSuccess) return fail(ctx, LSP_ECUDA, "%s failed: %s", #call, cudaGetErrorString(e__)); \
+  } while (0)
+// One pipeline stage: `call` launches `n` kernels on stream `st`.
+#define LSP_STAGE(id, n, call)                                                                            \
+  do {                                                                                                   \
+    TimingRec* r__ = stage_begin(ctx, id, st);                                                           \
+    cudaError_t e__ = (call);                                                                            \
+    if (r__) cudaEventRecord(r__->end, st);                                                              \
+    ctx->launches += (n);                                                                                \
+    if (e__ != cudaSuccess) return fail(ctx, LSP_ECUDA, "%s: %s", STAGE_NAMES[id], cudaGetErrorString(e__)); \
+  } while (0)
+#define LSP_TRY(call)                    \
+  do {                                   \
+    lsp_status s__ = (call);             \
+    if (s__ != LSP_OK) return s__;       \
+  } while (0)
+
+inline TimingRec* stage_begin(lsp_ctx* c, int id, cudaStream_t st) {
+  if (!c->timing_on || !c->recs || c->recs_used >= static_cast<int>(c->recs->size())) return nullptr;
+  TimingRec* r = &(*c->recs)[c->recs_used++];
+  r->stage = id;
+  cudaEventRecord(r->beg, st);
+  return r;
+}
+
+inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+void plan_layout(lsp_ctx* c) {
+  const size_t T = c->T, H = c->d.hidden, F = c->d.ffn, Nq = c->Nq, Nqkv = c->Nqkv;
+  const size_t BnqS = static_cast<size_t>(c->d.batch) * c->d.n_q_heads * c->d.seq;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t r = o; o += align_up(bytes); return r; };
+  SavedLayout& s = c->sv;
+  s.a32 = take(T * H * 4);
+  s.xn = take(T * H * 2);
+  s.rstd1 = take(T * 4);
+  s.qkv16 = take(T * Nqkv * 2);
+  s.o32 = take(T * Nq * 4);
+  s.o16 = take(T * Nq * 2);
+  s.lse = take(BnqS * 4);
+  s.an = take(T * H * 2);
+  s.rstd2 = take(T * 4);
+  s.g16 = take(T * F * 2);
+  s.u16 = take(T * F * 2);
+  s.h = take(T * F * 2);
+  s.total = o;
+
+  o = 0;
+  WsLayout& w = c->ws;
+  w.in16 = take(T * H * 2);
+  w.dgu = take(T * 2 * F * 2);
+  w.dn32 = take(T * H * 4);
+  w.da32 = take(T * H * 4);
+  w.da16 = take(T * H * 2);
+  w.dO16 = take(T * Nq * 2);
+  w.dvec = take(BnqS * 4);
+  w.dqkv16 = take(T * Nqkv * 2);
+  w.dgpart = take(static_cast<size_t>(c->norm_blocks) * H * 4);
+  w.q16 = take(T * Nq * 2);
+  w.k16 = take(T * c->Nkv * 2);
+  w.v16 = take(T * c->Nkv * 2);
+  w.total = o;
+}
+
+template <typename T> T* at(void* base, size_t off) { return reinterpret_cast<T*>(static_cast<uint8_t*>(base) + off); }
+template <typename T> const T* at(const void* base, size_t off) {
+  return reinterpret_cast<const T*>(static_cast<const uint8_t*>(base) + off);
+}
+
+// ------------------------------------------------------------------------------------------- norm dispatch
+template <typename XT>
+cudaError_t norm_fwd_t(const lsp_ctx* c, const void* x, const void* g, __nv_bfloat16* xn, float* rstd, cudaStream_t st) {
+  const int H = c->d.hidden, nv = (H / 4 + NORM_THREADS - 1) / NORM_THREADS;
+  const XT* xp = static_cast<const XT*>(x);
+  const __nv_bfloat16* gp = static_cast<const __nv_bfloat16*>(g);
+#define LSP_NF(NV) case NV: rmsnorm_fwd_kernel<XT, NV><<<c->T, NORM_THREADS, 0, st>>>(xp, gp, xn, rstd, H, c->d.rms_eps); break;
+  switch (nv) { LSP_NF(1) LSP_NF(2) LSP_NF(3) LSP_NF(4) LSP_NF(5) LSP_NF(6) LSP_NF(7) LSP_NF(8) default: return cudaErrorInvalidValue; }
+#undef LSP_NF
+  return cudaGetLastError();
+}
+cudaError_t norm_fwd(const lsp_ctx* c, int dt, const void* x, const void* g, __nv_bfloat16* xn, float* rstd, cudaStream_t st) {
+  return dt == LSP_F32 ? norm_fwd_t<float>(c, x, g, xn, rstd, st) : norm_fwd_t<__nv_bfloat16>(c, x, g, xn, rstd, st);
+}
+
+template <typename XT, typename RT>
+cudaError_t norm_bwd_t(const lsp_ctx* c, const void* x, const float* rstd, const void* g, const float* dxn, const void* dres,
+                       float* dx, __nv_bfloat16* dx16, float* dg_part, float* dg, cudaStream_t st) {
+  const int H = c->d.hidden, nv = (H / 4 + NORM_THREADS - 1) / NORM_THREADS;
+  const XT* xp = static_cast<const XT*>(x);
+  const RT* rp = static_cast<const RT*>(dres);
+  const __nv_bfloat16* gp = static_cast<const __nv_bfloat16*>(g);
+  const int nb = c->norm_blocks < c->T ? c->norm_blocks : c->T;
+#define LSP_NB(NV) case NV: rmsnorm_bwd_kernel<XT, RT, NV><<<nb, NORM_THREADS, 0, st>>>(xp, rstd, gp, dxn, rp, dx, dx16, dg_part, c->T, H); break;
+  switch (nv) { LSP_NB(1) LSP_NB(2) LSP_NB(3) LSP_NB(4) LSP_NB(5) LSP_NB(6) LSP_NB(7) LSP_NB(8) default: return cudaErrorInvalidValue; }
+#undef LSP_NB
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  colsum_kernel<<<(H + 255) / 256, 256, 0, st>>>(dg_part, dg, nb, H);
+  return cudaGetLastError();
+}
+// x: forward input of the norm (XT = x_dt); dres: incoming residual gradient (RT = r_dt)
+cudaError_t norm_bwd(const lsp_ctx* c, int x_dt, int r_dt, const void* x, const float* rstd, const void* g, const float* dxn,
+                     const void* dres, float* dx, __nv_bfloat16* dx16, float* dg_part, float* dg, cudaStream_t st) {
+  if (x_dt == LSP_F32)
+    return r_dt == LSP_F32 ? norm_bwd_t<float, float>(c, x, rstd, g, dxn, dres, dx, dx16, dg_part, dg, st)
+                           : norm_bwd_t<float, __nv_bfloat16>(c, x, rstd, g, dxn, dres, dx, dx16, dg_part, dg, st);
+  return r_dt == LSP_F32 ? norm_bwd_t<__nv_bfloat16, float>(c, x, rstd, g, dxn, dres, dx, dx16, dg_part, dg, st)
+                         : norm_bwd_t<__nv_bfloat16, __nv_bfloat16>(c, x, rstd, g, dxn, dres, dx, dx16, dg_part, dg, st);
+}
+
+cudaError_t cast_f32_bf16(const float* in, __nv_bfloat16* out, long long n, int sms, cudaStream_t st) {
+  const long long n8 = n / 8;
+  long long blocks = (n8 + 255) / 256;
+  if (blocks > sms * 16LL) blocks = sms * 16LL;
+  if (blocks < 1) blocks = 1;
+  cast_f32_bf16_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(in, out, n8);
+  return cudaGetLastError();
+}
+cudaError_t cast_bf16_f16(const __nv_bfloat16* in, __half* out, long long n, int sms, cudaStream_t st) {
+  const long long n8 = n / 8;
+  long long blocks = (n8 + 255) / 256;
+  if (blocks > sms * 16LL) blocks = sms * 16LL;
+  if (blocks < 1) blocks = 1;
+  cast_bf16_f16_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(in, out, n8);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------- GEMM call sites
+namespace {
+
+constexpr int BN_MAIN = 256;
+
+using EpiF32 = EpiStore<DT_F32, DT_F32, false>;
+inline EpiF32 epi_f32(float* out, long long ld) {
+  EpiF32 e;
+  e.out[0] = out; e.out[1] = e.out[2] = nullptr;
+  e.split1 = e.split2 = 0x7fffffff; e.ld = ld; e.res = nullptr; e.alpha = 1.0f;
+  return e;
+}
+
+template <bool A_MN, bool B_MN, class Epi>
+cudaError_t gemm1(const lsp_ctx* c, int M, int N, int K, const Operand& a, const Operand& b, const Epi& epi, cudaStream_t st) {
+  const int ks[1] = {K};
+  return gemm_run<BN_MAIN, A_MN, B_MN, Epi>(M, N, 1, &a, &b, ks, epi, c->num_sms, st);
+}
+
+// out[T,H] fp32 = res + A[T,K] . W[H,K]^T   (O-proj and down-proj forward with the residual epilogue; F4, F7)
+cudaError_t gemm_fwd_residual(const lsp_ctx* c, const __nv_bfloat16* A, int K, const void* W, int res_dt, const void* res,
+                              float* out, cudaStream_t st) {
+  const int T = c->T, H = c->d.hidden;
+  const Operand a{A, K, false}, b{W, K, false};
+  if (res_dt == LSP_F32) {
+    EpiStore<DT_F32, DT_F32, true> e;
+    e.out[0] = out; e.out[1] = e.out[2] = nullptr; e.split1 = e.split2 = 0x7fffffff; e.ld = H; e.res = res; e.alpha = 1.0f;
+    return gemm1<false, false>(c, T, H, K, a, b, e, st);
+  }
+  EpiStore<DT_F32, DT_BF16, true> e;
+  e.out[0] = out; e.out[1] = e.out[2] = nullptr; e.split1 = e.split2 = 0x7fffffff; e.ld = H; e.res = res; e.alpha = 1.0f;
+  return gemm1<false, false>(c, T, H, K, a, b, e, st);
+}
+
+// ------------------------------------------------------------------------------------------- attention block
+// x [T,H] x_dt -> a32 [T,H] fp32.  SURVEY 8(a) F1-F4.
+lsp_status attn_fwd_impl(lsp_ctx* ctx, int x_dt, const void* x, const lsp_layer_weights* w, float* a_out, void* saved,
+                         cudaStream_t st) {
+  const lsp_layer_desc& d = ctx->d;
+  const int T = ctx->T, H = d.hidden, Nq = ctx->Nq, Nkv = ctx->Nkv, Nqkv = ctx->Nqkv;
+  __nv_bfloat16* xn = at<__nv_bfloat16>(saved, ctx->sv.xn);
+  float* rstd1 = at<float>(saved, ctx->sv.rstd1);
+  __half* qkv = at<__half>(saved, ctx->sv.qkv16);
+  float* o32 = at<float>(saved, ctx->sv.o32);
+  __nv_bfloat16* o16 = at<__nv_bfloat16>(saved, ctx->sv.o16);
+  float* lse = at<float>(saved, ctx->sv.lse);
+
+  // F1 RMSNorm-1
+  LSP_STAGE(ST_NORM_FWD, 1, norm_fwd(ctx, x_dt, x, w->g_attn, xn, rstd1, st));
+  // F2 QKV projections with the RoPE epilogue (q, k rotated; v plain) into one [T, Nq+2Nkv] fp16 buffer
+  const Operand a{xn, H, false};
+  {
+    EpiProjRope<true> e{qkv, Nqkv, 0, ctx->rope, d.seq, d.head_dim};
+    EpiProjRope<false> en{qkv, Nqkv, 0, ctx->rope, d.seq, d.head_dim};
+    if (d.use_rope) {
+      LSP_STAGE(ST_QKV, 1, (gemm1<false, false>(ctx, T, Nq, H, a, Operand{w->wq, H, false}, e, st)));
+      e.col_off = Nq;
+      LSP_STAGE(ST_QKV, 1, (gemm1<false, false>(ctx, T, Nkv, H, a, Operand{w->wk, H, false}, e, st)));
+    } else {
+      LSP_STAGE(ST_QKV, 1, (gemm1<false, false>(ctx, T, Nq, H, a, Operand{w->wq, H, false}, en, st)));
+      en.col_off = Nq;
+      LSP_STAGE(ST_QKV, 1, (gemm1<false, false>(ctx, T, Nkv, H, a, Operand{w->wk, H, false}, en, st)));
+    }
+    en.col_off = Nq + Nkv;
+    LSP_STAGE(ST_QKV, 1, (gemm1<false, false>(ctx, T, Nkv, H, a, Operand{w->wv, H, false}, en, st)));
+  }
+  // F3 causal GQA flash forward
+  AttnParams p;
+  memset(&p, 0, sizeof(p));
+  p.q = qkv; p.k = qkv + Nq; p.v = qkv + Nq + Nkv;
+  p.ldq = p.ldk = p.ldv = Nqkv;
+  p.B = d.batch; p.S = d.seq; p.nq = d.n_q_heads; p.nkv = d.n_kv_heads;
+  p.scale = 1.0f / sqrtf(static_cast<float>(d.head_dim));
+  p.scale_log2 = p.scale * 1.4426950408889634f;
+  p.o32 = o32; p.o16 = o16; p.ldo = Nq; p.lse = lse;
+  if (d.head_dim == 128) LSP_STAGE(ST_ATTN_FWD, 1, attn_fwd_launch<128>(p, st));
+  else LSP_STAGE(ST_ATTN_FWD, 1, attn_fwd_launch<64>(p, st));
+  // F4 O-projection + residual
+  LSP_STAGE(ST_OPROJ, 1, gemm_fwd_residual(ctx, o16, Nq, w->wo, x_dt, x, a_out, st));
+  return LSP_OK;
+}
+
+// da (da_dt; da16 = its bf16 copy or itself) -> dx fp32.  SURVEY 8(a) B6-B10.
+lsp_status attn_bwd_impl(lsp_ctx* ctx, int x_dt, const void* x, int da_dt, const void* da, const __nv_bfloat16* da16,
+                         const lsp_layer_weights* w, const void* saved, float* dx, lsp_layer_wgrads* g, void* ws,
+                         cudaStream_t st) {
+  const lsp_layer_desc& d = ctx->d;
+  const int T = ctx->T, H = d.hidden, Nq = ctx->Nq, Nkv = ctx->Nkv, Nqkv = ctx->Nqkv;
+  const __nv_bfloat16* xn = at<__nv_bfloat16>(saved, ctx->sv.xn);
+  const float* rstd1 = at<float>(saved, ctx->sv.rstd1);
+  const __half* qkv = at<__half>(saved, ctx->sv.qkv16);
+  const float* o32 = at<float>(saved, ctx->sv.o32);
+  const __nv_bfloat16* o16 = at<__nv_bfloat16>(saved, ctx->sv.o16);
+  const float* lse = at<float>(saved, ctx->sv.lse);
+  __half* dO16 = at<__half>(ws, ctx->ws.dO16);
+  float* dvec = at<float>(ws, ctx->ws.dvec);
+  __nv_bfloat16* dqkv = at<__nv_bfloat16>(ws, ctx->ws.dqkv16);
+  float* dxn = at<float>(ws, ctx->ws.dn32);
+  float* dgpart = at<float>(ws, ctx->ws.dgpart);
+
+  // B6 dWo = da^T O ; dO = da Wo ; D = rowsum(dO * O32)
+  LSP_STAGE(ST_WGRAD_O, 1, (gemm1<true, true>(ctx, H, Nq, T, Operand{da16, H, true}, Operand{o16, Nq, true},
+                              epi_f32(static_cast<float*>(g->wo), Nq), st)));
+  {
+    EpiStore<DT_F16, DT_F32, false> e;
+    e.out[0] = dO16; e.out[1] = e.out[2] = nullptr; e.split1 = e.split2 = 0x7fffffff; e.ld = Nq; e.res = nullptr; e.alpha = 1.0f;
+    LSP_STAGE(ST_DGRAD_O, 1, (gemm1<false, true>(ctx, T, Nq, H, Operand{da16, H, false}, Operand{w->wo, Nq, true}, e, st)));
+  }
+  if (d.head_dim == 128) LSP_STAGE(ST_DVEC, 1, attn_dvec_launch<128>(dO16, Nq, o32, Nq, dvec, d.batch, d.seq, d.n_q_heads, st));
+  else LSP_STAGE(ST_DVEC, 1, attn_dvec_launch<64>(dO16, Nq, o32, Nq, dvec, d.batch, d.seq, d.n_q_heads, st));
+  // B7 + B8 flash backward with the inverse rotation on store
+  AttnParams p;
+  memset(&p, 0, sizeof(p));
+  p.q = qkv; p.k = qkv + Nq; p.v = qkv + Nq + Nkv; p.dO = dO16;
+  p.ldq = p.ldk = p.ldv = Nqkv; p.lddo = Nq;
+  p.B = d.batch; p.S = d.seq; p.nq = d.n_q_heads; p.nkv = d.n_kv_heads;
+  p.scale = 1.0f / sqrtf(static_cast<float>(d.head_dim));
+  p.scale_log2 = p.scale * 1.4426950408889634f;
+  p.lse = const_cast<float*>(lse); p.dvec = dvec;
+  p.rope = d.use_rope ? ctx->rope : nullptr;
+  p.dq16 = dqkv; p.dk16 = dqkv + Nq; p.dv16 = dqkv + Nq + Nkv; p.ldd16 = Nqkv;
+  if (d.head_dim == 128) LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_launch<128>(p, st));
+  else LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_launch<64>(p, st));
+  // B9 dW{q,k,v} = d{q,k,v}^T xn (one GEMM, rows split over three outputs) ; dxn = dq Wq + dk Wk + dv Wv (3 K-segments)
+  {
+    EpiF32 e = epi_f32(static_cast<float*>(g->wq), H);
+    e.out[1] = g->wk; e.out[2] = g->wv; e.split1 = Nq; e.split2 = Nq + Nkv;
+    LSP_STAGE(ST_WGRAD_QKV, 1, (gemm1<true, true>(ctx, Nqkv, H, T, Operand{dqkv, Nqkv, true}, Operand{xn, H, true}, e, st)));
+  }
+  {
+    const Operand as[3] = {{dqkv, Nqkv, false}, {dqkv + Nq, Nqkv, false}, {dqkv + Nq + Nkv, Nqkv, false}};
+    const Operand bs[3] = {{w->wq, H, true}, {w->wk, H, true}, {w->wv, H, true}};
+    const int ks[3] = {Nq, Nkv, Nkv};
+    LSP_STAGE(ST_DGRAD_QKV, 1, (gemm_run<BN_MAIN, false, true>(T, H, 3, as, bs, ks, epi_f32(dxn, H), ctx->num_sms, st)));
+  }
+  // B10 RMSNorm-1 backward + residual gradient
+  LSP_STAGE(ST_NORM_BWD, 2, norm_bwd(ctx, x_dt, da_dt, x, rstd1, w->g_attn, dxn, da, dx, nullptr, dgpart, static_cast<float*>(g->g_attn), st));
+  return LSP_OK;
+}
+
+// ------------------------------------------------------------------------------------------- MLP block
+// a (a_dt) -> y fp32.  SURVEY 8(a) F5-F7.
+lsp_status mlp_fwd_impl(lsp_ctx* ctx, int a_dt, const void* a, const lsp_layer_weights* w, float* y, void* saved, cudaStream_t st) {
+  const lsp_layer_desc& d = ctx->d;
+  const int T = ctx->T, H = d.hidden, F = d.ffn;
+  __nv_bfloat16* an = at<__nv_bfloat16>(saved, ctx->sv.an);
+  float* rstd2 = at<float>(saved, ctx->sv.rstd2);
+  __half* g16 = at<__half>(saved, ctx->sv.g16);
+  __half* u16 = at<__half>(saved, ctx->sv.u16);
+  __nv_bfloat16* h = at<__nv_bfloat16>(saved, ctx->sv.h);
+  LSP_STAGE(ST_NORM_FWD, 1, norm_fwd(ctx, a_dt, a, w->g_mlp, an, rstd2, st));
+  EpiSwiGLU e{h, g16, u16, F};
+  LSP_STAGE(ST_GATEUP, 1, gemm_run_dual(T, F, H, Operand{an, H, false}, Operand{w->w_gate, H, false}, Operand{w->w_up, H, false}, e,
+                         ctx->num_sms, st));
+  LSP_STAGE(ST_DOWN, 1, gemm_fwd_residual(ctx, h, F, w->w_down, a_dt, a, y, st));
+  return LSP_OK;
+}
+
+// dy (dy_dt; dy16 = bf16 copy or itself) -> da fp32 (+ bf16 copy da16 if non-null).  SURVEY 8(a) B1-B5.
+lsp_status mlp_bwd_impl(lsp_ctx* ctx, int a_dt, const void* a, int dy_dt, const void* dy, const __nv_bfloat16* dy16,
+                        const lsp_layer_weights* w, const void* saved, float* da, __nv_bfloat16* da16, lsp_layer_wgrads* g,
+                        void* ws, cudaStream_t st) {
+  const lsp_layer_desc& d = ctx->d;
+  const int T = ctx->T, H = d.hidden, F = d.ffn;
+  const __nv_bfloat16* an = at<__nv_bfloat16>(saved, ctx->sv.an);
+  const float* rstd2 = at<float>(saved, ctx->sv.rstd2);
+  const __half* g16 = at<__half>(saved, ctx->sv.g16);
+  const __half* u16 = at<__half>(saved, ctx->sv.u16);
+  const __nv_bfloat16* h = at<__nv_bfloat16>(saved, ctx->sv.h);
+  __nv_bfloat16* dgu = at<__nv_bfloat16>(ws, ctx->ws.dgu);
+  float* dan = at<float>(ws, ctx->ws.dn32);
+  float* dgpart = at<float>(ws, ctx->ws.dgpart);
+
+  // B2 dWd = dy^T h
+  LSP_STAGE(ST_WGRAD_DOWN, 1, (gemm1<true, true>(ctx, H, F, T, Operand{dy16, H, true}, Operand{h, F, true}, epi_f32(static_cast<float*>(g->w_down), F), st)));
+  // B1 dh = dy Wd with the SwiGLU-backward epilogue -> [dg | du]
+  {
+    EpiSwiGLUBwd e{g16, u16, F, dgu, F};
+    LSP_STAGE(ST_DGRAD_DOWN, 1, (gemm1<false, true>(ctx, T, F, H, Operand{dy16, H, false}, Operand{w->w_down, F, true}, e, st)));
+  }
+  // B4 dWg = dg^T an, dWu = du^T an (one GEMM over the 2F rows of [dg | du]^T)
+  {
+    EpiF32 e = epi_f32(static_cast<float*>(g->w_gate), H);
+    e.out[1] = g->w_up; e.split1 = F;
+    LSP_STAGE(ST_WGRAD_GATEUP, 1, (gemm1<true, true>(ctx, 2 * F, H, T, Operand{dgu, 2LL * F, true}, Operand{an, H, true}, e, st)));
+  }
+  // B3 dan = dg Wg + du Wu (two K-segments)
+  {
+    const Operand as[2] = {{dgu, 2LL * F, false}, {dgu + F, 2LL * F, false}};
+    const Operand bs[2] = {{w->w_gate, H, true}, {w->w_up, H, true}};
+    const int ks[2] = {F, F};
+    LSP_STAGE(ST_DGRAD_GATEUP, 1, (gemm_run<BN_MAIN, false, true>(T, H, 2, as, bs, ks, epi_f32(dan, H), ctx->num_sms, st)));
+  }
+  // B5 RMSNorm-2 backward + residual gradient
+  LSP_STAGE(ST_NORM_BWD, 2, norm_bwd(ctx, a_dt, dy_dt, a, rstd2, w->g_mlp, dan, dy, da, da16, dgpart, static_cast<float*>(g->g_mlp), st));
+  return LSP_OK;
+}
+
+lsp_status check_common(lsp_ctx* ctx, const void* saved, const void* ws, int n, const void* const* ptrs) {
+  if (!ctx) return LSP_EINVAL;
+  for (int i = 0; i < n; ++i) {
+    if (!ptrs[i]) return fail(ctx, LSP_EINVAL, "NULL pointer argument (#%d)", i);
+    if (!aligned(ptrs[i], 16)) return fail(ctx, LSP_EALIGN, "pointer argument #%d is not 16-byte aligned", i);
+  }
+  if (saved && !aligned(saved, ALIGN)) return fail(ctx, LSP_EALIGN, "`saved` must be 256-byte aligned");
+  if (ws && !aligned(ws, ALIGN)) return fail(ctx, LSP_EALIGN, "`ws` must be 256-byte aligned");
+  return LSP_OK;
+}
+
+// bf16 view of an activation-gradient input: the tensor itself if it is bf16, else a cast into ws.in16
+lsp_status as_bf16(lsp_ctx* ctx, const void* in, void* ws, cudaStream_t st, const __nv_bfloat16** out) {
+  if (ctx->d.in_dtype == LSP_BF16) { *out = static_cast<const __nv_bfloat16*>(in); return LSP_OK; }
+  __nv_bfloat16* t = at<__nv_bfloat16>(ws, ctx->ws.in16);
+  LSP_STAGE(ST_CAST, 1, cast_f32_bf16(static_cast<const float*>(in), t, static_cast<long long>(ctx->T) * ctx->d.hidden, ctx->num_sms, st));
+  *out = t;
+  return LSP_OK;
+}
+
+}  // namespace
+
+// =========================================================================================== C ABI
+extern "C" {
+
+lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device) {
+  if (!out || !desc) return LSP_EINVAL;
+  *out = nullptr;
+  const lsp_layer_desc& d = *desc;
+  if (d.batch <= 0 || d.seq <= 0 || d.hidden <= 0 || d.n_q_heads <= 0 || d.n_kv_heads <= 0 || d.ffn <= 0) return LSP_EINVAL;
+  if (d.n_q_heads % d.n_kv_heads != 0) return LSP_EINVAL;
+  if (d.head_dim != 64 && d.head_dim != 128) return LSP_EUNSUPPORTED;
+  if (d.hidden % 8 || d.ffn % 8 || d.hidden > 8192) return LSP_EUNSUPPORTED;
+  if (d.rope_layout != 0 || d.wgrad_accumulate != 0) return LSP_EUNSUPPORTED;
+  if (d.in_dtype != LSP_BF16 && d.in_dtype != LSP_F32) return LSP_EINVAL;
+  if (!(d.rms_eps >= 0.0f) || !(d.rope_base > 0.0)) return LSP_EINVAL;
+  if (static_cast<long long>(d.batch) * d.seq > 0x7fffffffLL / 4) return LSP_EUNSUPPORTED;
+
+  lsp_ctx* ctx = new (std::nothrow) lsp_ctx;
+  if (!ctx) return LSP_ENOMEM;
+  memset(ctx, 0, sizeof(*ctx));
+  ctx->d = d;
+  ctx->device = cuda_device;
+  ctx->T = d.batch * d.seq;
+  ctx->Nq = d.n_q_heads * d.head_dim;
+  ctx->Nkv = d.n_kv_heads * d.head_dim;
+  ctx->Nqkv = ctx->Nq + 2 * ctx->Nkv;
+  ctx->G = d.n_q_heads / d.n_kv_heads;
+
+  cudaDeviceProp prop;
+  if (cudaSetDevice(cuda_device) != cudaSuccess || cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) {
+    delete ctx;
+    return LSP_ECUDA;
+  }
+  if (prop.major != 10) {          // tcgen05 / TMEM kernels: Blackwell only, no fallback
+    delete ctx;
+    return LSP_EUNSUPPORTED;
+  }
+  ctx->num_sms = prop.multiProcessorCount;
+  ctx->norm_blocks = ctx->num_sms * 4;
+  plan_layout(ctx);
+
+  // RoPE table: theta = pos * base^(-2i/d) in fp64 (reading A-5), stored as fp32 (cos, sin)
+  const int half = d.head_dim / 2;
+  std::vector<float2> tab(static_cast<size_t>(d.seq) * half);
+  for (int p = 0; p < d.seq; ++p)
+    for (int i = 0; i < half; ++i) {
+      const double th = static_cast<double>(p) * pow(d.rope_base, -2.0 * i / d.head_dim);
+      tab[static_cast<size_t>(p) * half + i] = make_float2(static_cast<float>(cos(th)), static_cast<float>(sin(th)));
+    }
+  if (cudaMalloc(&ctx->rope, tab.size() * sizeof(float2)) != cudaSuccess) { delete ctx; return LSP_ENOMEM; }
+  if (cudaMemcpy(ctx->rope, tab.data(), tab.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess) {
+    cudaFree(ctx->rope);
+    delete ctx;
+    return LSP_ECUDA;
+  }
+  if (!get_encode_fn()) { cudaFree(ctx->rope); delete ctx; return LSP_ECUDA; }
+  *out = ctx;
+  return LSP_OK;
+}
+
+lsp_status lsp_destroy(lsp_ctx* ctx) {
+  if (!ctx) return LSP_EINVAL;
+  lsp_timing_enable(ctx, 0);
+  cudaFree(ctx->rope);
+  delete ctx;
+  return LSP_OK;
+}
+
+size_t lsp_saved_bytes(const lsp_ctx* ctx) { return ctx ? ctx->sv.total : 0; }
+size_t lsp_workspace_bytes(const lsp_ctx* ctx) { return ctx ? ctx->ws.total : 0; }
+const char* lsp_last_error(const lsp_ctx* ctx) { return ctx ? ctx->err : "lsp: NULL context"; }
+
+lsp_status lsp_attn_fwd(lsp_ctx* ctx, const void* x, const lsp_layer_weights* w, void* a_out, void* saved, void* ws, void* stream) {
+  if (!ctx || !w) return LSP_EINVAL;
+  const void* ptrs[] = {x, a_out, saved, ws, w->wq, w->wk, w->wv, w->wo, w->g_attn};
+  LSP_TRY(check_common(ctx, saved, ws, 9, ptrs));
+  return attn_fwd_impl(ctx, ctx->d.in_dtype, x, w, static_cast<float*>(a_out), saved, static_cast<cudaStream_t>(stream));
+}
+
+lsp_status lsp_attn_bwd(lsp_ctx* ctx, const void* x, const void* da, const lsp_layer_weights* w, const void* saved, void* dx,
+                        lsp_layer_wgrads* g, void* ws, void* stream) {
+  if (!ctx || !w || !g) return LSP_EINVAL;
+  const void* ptrs[] = {x, da, saved, dx, ws, w->wq, w->wk, w->wv, w->wo, w->g_attn, g->wq, g->wk, g->wv, g->wo, g->g_attn};
+  LSP_TRY(check_common(ctx, saved, ws, 15, ptrs));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const __nv_bfloat16* da16;
+  LSP_TRY(as_bf16(ctx, da, ws, st, &da16));
+  return attn_bwd_impl(ctx, ctx->d.in_dtype, x, ctx->d.in_dtype, da, da16, w, saved, static_cast<float*>(dx), g, ws, st);
+}
+
+lsp_status lsp_mlp_fwd(lsp_ctx* ctx, const void* a, const lsp_layer_weights* w, void* y_out, void* saved, void* ws, void* stream) {
+  if (!ctx || !w) return LSP_EINVAL;
+  const void* ptrs[] = {a, y_out, saved, ws, w->w_gate, w->w_up, w->w_down, w->g_mlp};
+  LSP_TRY(check_common(ctx, saved, ws, 8, ptrs));
+  return mlp_fwd_impl(ctx, ctx->d.in_dtype, a, w, static_cast<float*>(y_out), saved, static_cast<cudaStream_t>(stream));
+}
+
+lsp_status lsp_mlp_bwd(lsp_ctx* ctx, const void* a, const void* dy, const lsp_layer_weights* w, const void* saved, void* da,
+                       lsp_layer_wgrads* g, void* ws, void* stream) {
+  if (!ctx || !w || !g) return LSP_EINVAL;
+  const void* ptrs[] = {a, dy, saved, da, ws, w->w_gate, w->w_up, w->w_down, w->g_mlp, g->w_gate, g->w_up, g->w_down, g->g_mlp};
+  LSP_TRY(check_common(ctx, saved, ws, 13, ptrs));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const __nv_bfloat16* dy16;
+  LSP_TRY(as_bf16(ctx, dy, ws, st, &dy16));
+  return mlp_bwd_impl(ctx, ctx->d.in_dtype, a, ctx->d.in_dtype, dy, dy16, w, saved, static_cast<float*>(da), nullptr, g, ws, st);
+}
+
+lsp_status lsp_layer_fwd(lsp_ctx* ctx, const void* x, const lsp_layer_weights* w, void* y_out, void* saved, void* ws, void* stream) {
+  if (!ctx || !w) return LSP_EINVAL;
+  const void* ptrs[] = {x, y_out, saved, ws, w->wq, w->wk, w->wv, w->wo, w->g_attn, w->w_gate, w->w_up, w->w_down, w->g_mlp};
+  LSP_TRY(check_common(ctx, saved, ws, 13, ptrs));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  float* a32 = at<float>(saved, ctx->sv.a32);
+  LSP_TRY(attn_fwd_impl(ctx, ctx->d.in_dtype, x, w, a32, saved, st));
+  return mlp_fwd_impl(ctx, LSP_F32, a32, w, static_cast<float*>(y_out), saved, st);
+}
+
+lsp_status lsp_layer_bwd(lsp_ctx* ctx, const void* x, const void* dy, const lsp_layer_weights* w, const void* saved, void* dx,
+                         lsp_layer_wgrads* g, void* ws, void* stream) {
+  if (!ctx || !w || !g) return LSP_EINVAL;
+  const void* ptrs[] = {x, dy, saved, dx, ws, w->wq, w->wk, w->wv, w->wo, w->g_attn, w->w_gate, w->w_up, w->w_down, w->g_mlp,
+                        g->wq, g->wk, g->wv, g->wo, g->g_attn, g->w_gate, g->w_up, g->w_down, g->g_mlp};
+  LSP_TRY(check_common(ctx, saved, ws, 23, ptrs));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const __nv_bfloat16* dy16;
+  LSP_TRY(as_bf16(ctx, dy, ws, st, &dy16));
+  const float* a32 = at<float>(saved, ctx->sv.a32);
+  float* da32 = at<float>(ws, ctx->ws.da32);
+  __nv_bfloat16* da16 = at<__nv_bfloat16>(ws, ctx->ws.da16);
+  LSP_TRY(mlp_bwd_impl(ctx, LSP_F32, a32, ctx->d.in_dtype, dy, dy16, w, saved, da32, da16, g, ws, st));
+  return attn_bwd_impl(ctx, ctx->d.in_dtype, x, LSP_F32, da32, da16, w, saved, static_cast<float*>(dx), g, ws, st);
+}
+
+lsp_status lsp_sdpa_fwd(lsp_ctx* ctx, const void* q, const void* k, const void* v, void* o, float* lse, void* ws, void* stream) {
+  if (!ctx) return LSP_EINVAL;
+  const void* ptrs[] = {q, k, v, o, lse, ws};
+  LSP_TRY(check_common(ctx, nullptr, ws, 6, ptrs));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const lsp_layer_desc& d = ctx->d;
+  const long long T = ctx->T;
+  __half* q16 = at<__half>(ws, ctx->ws.q16);
+  __half* k16 = at<__half>(ws, ctx->ws.k16);
+  __half* v16 = at<__half>(ws, ctx->ws.v16);
+  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(q), q16, T * ctx->Nq, ctx->num_sms, st));
+  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(k), k16, T * ctx->Nkv, ctx->num_sms, st));
+  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(v), v16, T * ctx->Nkv, ctx->num_sms, st));
+  AttnParams p;
+  memset(&p, 0, sizeof(p));
+  p.q = q16; p.k = k16; p.v = v16;
+  p.ldq = ctx->Nq; p.ldk = p.ldv = ctx->Nkv;
+  p.B = d.batch; p.S = d.seq; p.nq = d.n_q_heads; p.nkv = d.n_kv_heads;
+  p.scale = 1.0f / sqrtf(static_cast<float>(d.head_dim));
+  p.scale_log2 = p.scale * 1.4426950408889634f;
+  p.o32 = static_cast<float*>(o); p.ldo = ctx->Nq; p.lse = lse;
+  if (d.head_dim == 128) LSP_STAGE(ST_ATTN_FWD, 1, attn_fwd_launch<128>(p, st));
+  else LSP_STAGE(ST_ATTN_FWD, 1, attn_fwd_launch<64>(p, st));
+  return LSP_OK;
+}
+
+lsp_status lsp_sdpa_bwd(lsp_ctx* ctx, const void* q, const void* k, const void* v, const void* o, const float* lse,
+                        const void* d_o, void* dq, void* dk, void* dv, void* ws, void* stream) {
+  if (!ctx) return LSP_EINVAL;
+  const void* ptrs[] = {q, k, v, o, lse, d_o, dq, dk, dv, ws};
+  LSP_TRY(check_common(ctx, nullptr, ws, 10, ptrs));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const lsp_layer_desc& d = ctx->d;
+  const long long T = ctx->T;
+  __half* q16 = at<__half>(ws, ctx->ws.q16);
+  __half* k16 = at<__half>(ws, ctx->ws.k16);
+  __half* v16 = at<__half>(ws, ctx->ws.v16);
+  __half* dO16 = at<__half>(ws, ctx->ws.dO16);
+  float* dvec = at<float>(ws, ctx->ws.dvec);
+  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(q), q16, T * ctx->Nq, ctx->num_sms, st));
+  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(k), k16, T * ctx->Nkv, ctx->num_sms, st));
+  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(v), v16, T * ctx->Nkv, ctx->num_sms, st));
+  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(d_o), dO16, T * ctx->Nq, ctx->num_sms, st));
+  if (d.head_dim == 128) LSP_STAGE(ST_DVEC, 1, attn_dvec_launch<128>(dO16, ctx->Nq, static_cast<const float*>(o), ctx->Nq, dvec, d.batch, d.seq, d.n_q_heads, st));
+  else LSP_STAGE(ST_DVEC, 1, attn_dvec_launch<64>(dO16, ctx->Nq, static_cast<const float*>(o), ctx->Nq, dvec, d.batch, d.seq, d.n_q_heads, st));
+  AttnParams p;
+  memset(&p, 0, sizeof(p));
+  p.q = q16; p.k = k16; p.v = v16; p.dO = dO16;
+  p.ldq = ctx->Nq; p.ldk = p.ldv = ctx->Nkv; p.lddo = ctx->Nq;
+  p.B = d.batch; p.S = d.seq; p.nq = d.n_q_heads; p.nkv = d.n_kv_heads;
+  p.scale = 1.0f / sqrtf(static_cast<float>(d.head_dim));
+  p.scale_log2 = p.scale * 1.4426950408889634f;
+  p.lse = const_cast<float*>(lse); p.dvec = dvec;
+  p.dq32 = static_cast<float*>(dq); p.dk32 = static_cast<float*>(dk); p.dv32 = static_cast<float*>(dv);
+  p.lddq32 = ctx->Nq; p.lddk32 = ctx->Nkv;
+  if (d.head_dim == 128) LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_launch<128>(p, st));
+  else LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_launch<64>(p, st));
+  return LSP_OK;
+}
+
+lsp_status lsp_embed_fwd(lsp_ctx* ctx, const int32_t* ids, const void* table, void* x0, void* stream) {
+  if (!ctx) return LSP_EINVAL;
+  const void* ptrs[] = {ids, table, x0};
+  LSP_TRY(check_common(ctx, nullptr, nullptr, 3, ptrs));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  auto launch = [&]() {
+    embed_gather_kernel<float><<<ctx->T, 256, 0, st>>>(ids, static_cast<const __nv_bfloat16*>(table), static_cast<float*>(x0), ctx->d.hidden);
+    return cudaGetLastError();
+  };
+  LSP_STAGE(ST_EMBED, 1, launch());
+  return LSP_OK;
+}
+
+lsp_status lsp_gemm(lsp_ctx* ctx, int op, int M, int N, int K, const void* A, int64_t lda, const void* B, int64_t ldb,
+                    float* C, int64_t ldc, void* stream) {
+  if (!ctx) return LSP_EINVAL;
+  const void* ptrs[] = {A, B, C};
+  LSP_TRY(check_common(ctx, nullptr, nullptr, 3, ptrs));
+  if (M <= 0 || N <= 0 || K <= 0 || (lda % 8) || (ldb % 8) || (ldc % 8) || (N % 8)) return fail(ctx, LSP_EINVAL, "lsp_gemm: bad extents/pitches");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const EpiF32 e = epi_f32(C, ldc);
+  switch (op) {
+    case 0: LSP_STAGE(ST_OPROJ, 1, (gemm1<false, false>(ctx, M, N, K, Operand{A, lda, false}, Operand{B, ldb, false}, e, st))); break;
+    case 1: LSP_STAGE(ST_DGRAD_O, 1, (gemm1<false, true>(ctx, M, N, K, Operand{A, lda, false}, Operand{B, ldb, true}, e, st))); break;
+    case 2: LSP_STAGE(ST_WGRAD_O, 1, (gemm1<true, true>(ctx, M, N, K, Operand{A, lda, true}, Operand{B, ldb, true}, e, st))); break;
+    default: return fail(ctx, LSP_EINVAL, "lsp_gemm: op must be 0, 1 or 2");
+  }
+  return LSP_OK;
+}
+
+lsp_status lsp_layer_step_host(lsp_ctx* ctx, const void* x_host, const void* dy_host, const lsp_layer_weights* w,
+                               void* y_host, void* dx_host, lsp_layer_wgrads* g, void* x_dev, void* dy_dev, void* y_dev,
+                               void* dx_dev, void* saved, void* ws, void* stream) {
+  if (!ctx || !x_host || !dy_host || !y_host || !dx_host || !x_dev || !dy_dev || !y_dev || !dx_dev) return LSP_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const size_t n = static_cast<size_t>(ctx->T) * ctx->d.hidden;
+  const size_t in_bytes = n * (ctx->d.in_dtype == LSP_F32 ? 4 : 2);
+  LSP_CUDA(cudaMemcpyAsync(x_dev, x_host, in_bytes, cudaMemcpyHostToDevice, st));
+  LSP_CUDA(cudaMemcpyAsync(dy_dev, dy_host, in_bytes, cudaMemcpyHostToDevice, st));
+  LSP_TRY(lsp_layer_fwd(ctx, x_dev, w, y_dev, saved, ws, stream));
+  LSP_CUDA(cudaMemcpyAsync(y_host, y_dev, n * 4, cudaMemcpyDeviceToHost, st));
+  LSP_TRY(lsp_layer_bwd(ctx, x_dev, dy_dev, w, saved, dx_dev, g, ws, stream));
+  LSP_CUDA(cudaMemcpyAsync(dx_host, dx_dev, n * 4, cudaMemcpyDeviceToHost, st));
+  return LSP_OK;
+}
+
+long long lsp_launch_count(const lsp_ctx* ctx) { return ctx ? ctx->launches : -1; }
+
+lsp_status lsp_timing_enable(lsp_ctx* ctx, int max_records) {
+  if (!ctx || max_records < 0) return LSP_EINVAL;
+  if (ctx->recs) {
+    for (TimingRec& r : *ctx->recs) { cudaEventDestroy(r.beg); cudaEventDestroy(r.end); }
+    delete ctx->recs;
+    ctx->recs = nullptr;
+  }
+  ctx->timing_on = 0;
+  ctx->recs_used = 0;
+  if (max_records == 0) return LSP_OK;
+  ctx->recs = new (std::nothrow) std::vector<TimingRec>(max_records);
+  if (!ctx->recs) return LSP_ENOMEM;
+  for (TimingRec& r : *ctx->recs) {
+    r.stage = -1;
+    if (cudaEventCreate(&r.beg) != cudaSuccess || cudaEventCreate(&r.end) != cudaSuccess)
+      return fail(ctx, LSP_ECUDA, "cudaEventCreate failed");
+  }
+  ctx->timing_on = 1;
+  return LSP_OK;
+}
+
+int lsp_timing_read(lsp_ctx* ctx, int max_stages, const char** names, float* total_ms, int* records) {
+  if (!ctx || !names || !total_ms || !records) return -1;
+  const int n = max_stages < ST_COUNT ? max_stages : ST_COUNT;
+  for (int i = 0; i < n; ++i) { names[i] = STAGE_NAMES[i]; total_ms[i] = 0.f; records[i] = 0; }
+  if (ctx->recs) {
+    for (int i = 0; i < ctx->recs_used; ++i) {
+      TimingRec& r = (*ctx->recs)[i];
+      if (r.stage < 0 || r.stage >= n) continue;
+      if (cudaEventSynchronize(r.end) != cudaSuccess) return -1;
+      float ms = 0.f;
+      if (cudaEventElapsedTime(&ms, r.beg, r.end) != cudaSuccess) return -1;
+      total_ms[r.stage] += ms;
+      records[r.stage] += 1;
+    }
+    ctx->recs_used = 0;
+  }
+  return n;
+}
+
+}  // extern "C"

@@ -1,0 +1,162 @@
+// Memory-bound kernels of the layer: RMSNorm forward/backward (ref [34]; SURVEY 8(a) F1,F5,B5,B10),
+// the gain-gradient column reduction, dtype casts and the embedding gather (E0).
+// All are vectorised (16-byte accesses), coalesced, warp-shuffle reduced; HBM is the roofline.
+#pragma once
+#include "ptx.cuh"
+
+namespace lsp {
+
+constexpr int NORM_THREADS = 256;
+constexpr int NORM_MAXV = 8;                 // float4 per thread (template NV <= 8) -> hidden <= 8192
+
+template <typename T> struct Vec4;
+template <> struct Vec4<float> {
+  static __device__ __forceinline__ float4 load(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+};
+template <> struct Vec4<__nv_bfloat16> {
+  static __device__ __forceinline__ float4 load(const __nv_bfloat16* p) {
+    const uint2 u = __ldg(reinterpret_cast<const uint2*>(p));
+    return make_float4(bf16_lo(u.x), bf16_hi(u.x), bf16_lo(u.y), bf16_hi(u.y));
+  }
+};
+__device__ __forceinline__ void store_bf16x4(__nv_bfloat16* p, float4 v) {
+  *reinterpret_cast<uint2*>(p) = make_uint2(pack_bf16(v.x, v.y), pack_bf16(v.z, v.w));
+}
+
+__device__ __forceinline__ float block_sum(float v, float* red) {
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  __syncthreads();                            // protect `red` from the previous use
+  if (lane == 0) red[warp] = v;
+  __syncthreads();
+  float t = (lane < NORM_THREADS / 32) ? red[lane] : 0.f;
+#pragma unroll
+  for (int off = 4; off > 0; off >>= 1) t += __shfl_xor_sync(0xffffffffu, t, off);
+  return __shfl_sync(0xffffffffu, t, 0);
+}
+
+// xn = x * rsqrt(mean(x^2) + eps) * g  (bf16 out), rstd saved in fp32.  One block per token row.
+template <typename XT, int NV>
+__global__ void __launch_bounds__(NORM_THREADS) rmsnorm_fwd_kernel(const XT* __restrict__ x, const __nv_bfloat16* __restrict__ g,
+                                                                   __nv_bfloat16* __restrict__ xn, float* __restrict__ rstd,
+                                                                   int H, float eps) {
+  __shared__ float red[NORM_THREADS / 32];
+  const long long row = blockIdx.x;
+  const XT* xr = x + row * H;
+  float4 v[NV];
+  float ss = 0.f;
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    const int c = (threadIdx.x + i * NORM_THREADS) * 4;
+    if (c < H) {
+      v[i] = Vec4<XT>::load(xr + c);
+      ss += v[i].x * v[i].x + v[i].y * v[i].y + v[i].z * v[i].z + v[i].w * v[i].w;
+    }
+  }
+  ss = block_sum(ss, red);
+  const float r = rsqrtf(ss / static_cast<float>(H) + eps);
+  if (threadIdx.x == 0) rstd[row] = r;
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    const int c = (threadIdx.x + i * NORM_THREADS) * 4;
+    if (c < H) {
+      const float4 gg = Vec4<__nv_bfloat16>::load(g + c);
+      store_bf16x4(xn + row * H + c, make_float4(v[i].x * r * gg.x, v[i].y * r * gg.y, v[i].z * r * gg.z, v[i].w * r * gg.w));
+    }
+  }
+}
+
+// dx = dres + r*(dn - n*mean(dn*n)),  n = x*r, dn = dxn*g ;  dg partial[block][col] = sum_rows dxn*n.
+// Persistent blocks stride over rows so each thread keeps its columns' dg partials in registers.
+template <typename XT, typename RT, int NV>
+__global__ void __launch_bounds__(NORM_THREADS) rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd,
+                                                                   const __nv_bfloat16* __restrict__ g,
+                                                                   const float* __restrict__ dxn, const RT* __restrict__ dres,
+                                                                   float* __restrict__ dx, __nv_bfloat16* __restrict__ dx16,
+                                                                   float* __restrict__ dg_part, int T, int H) {
+  __shared__ float red[NORM_THREADS / 32];
+  float4 gg[NV], acc[NV];
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    const int c = (threadIdx.x + i * NORM_THREADS) * 4;
+    acc[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    gg[i] = (c < H) ? Vec4<__nv_bfloat16>::load(g + c) : make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  const float invH = 1.0f / static_cast<float>(H);
+  for (long long row = blockIdx.x; row < T; row += gridDim.x) {
+    const float r = rstd[row];
+    float4 n[NV], dn[NV];
+    float dot = 0.f;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      const int c = (threadIdx.x + i * NORM_THREADS) * 4;
+      if (c < H) {
+        const float4 xv = Vec4<XT>::load(x + row * H + c);
+        const float4 d = Vec4<float>::load(dxn + row * H + c);
+        n[i] = make_float4(xv.x * r, xv.y * r, xv.z * r, xv.w * r);
+        acc[i].x += d.x * n[i].x; acc[i].y += d.y * n[i].y; acc[i].z += d.z * n[i].z; acc[i].w += d.w * n[i].w;
+        dn[i] = make_float4(d.x * gg[i].x, d.y * gg[i].y, d.z * gg[i].z, d.w * gg[i].w);
+        dot += dn[i].x * n[i].x + dn[i].y * n[i].y + dn[i].z * n[i].z + dn[i].w * n[i].w;
+      }
+    }
+    dot = block_sum(dot, red) * invH;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      const int c = (threadIdx.x + i * NORM_THREADS) * 4;
+      if (c < H) {
+        const float4 rs = Vec4<RT>::load(dres + row * H + c);
+        float4 o;
+        o.x = rs.x + r * (dn[i].x - n[i].x * dot);
+        o.y = rs.y + r * (dn[i].y - n[i].y * dot);
+        o.z = rs.z + r * (dn[i].z - n[i].z * dot);
+        o.w = rs.w + r * (dn[i].w - n[i].w * dot);
+        *reinterpret_cast<float4*>(dx + row * H + c) = o;
+        if (dx16) store_bf16x4(dx16 + row * H + c, o);
+      }
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    const int c = (threadIdx.x + i * NORM_THREADS) * 4;
+    if (c < H) *reinterpret_cast<float4*>(dg_part + static_cast<long long>(blockIdx.x) * H + c) = acc[i];
+  }
+}
+
+// dg[col] = sum over blocks of dg_part[block][col]  (fixed order: deterministic)
+__global__ void colsum_kernel(const float* __restrict__ part, float* __restrict__ out, int nparts, int H) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= H) return;
+  float s = 0.f;
+  for (int b = 0; b < nparts; ++b) s += part[static_cast<long long>(b) * H + c];
+  out[c] = s;
+}
+
+// 8 elements per thread casts (n is a multiple of 8)
+__global__ void cast_f32_bf16_kernel(const float* __restrict__ in, __nv_bfloat16* __restrict__ out, long long n8) {
+  for (long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i < n8; i += static_cast<long long>(gridDim.x) * blockDim.x) {
+    const float4 a = __ldg(reinterpret_cast<const float4*>(in) + 2 * i), b = __ldg(reinterpret_cast<const float4*>(in) + 2 * i + 1);
+    reinterpret_cast<uint4*>(out)[i] = make_uint4(pack_bf16(a.x, a.y), pack_bf16(a.z, a.w), pack_bf16(b.x, b.y), pack_bf16(b.z, b.w));
+  }
+}
+__global__ void cast_bf16_f16_kernel(const __nv_bfloat16* __restrict__ in, __half* __restrict__ out, long long n8) {
+  for (long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i < n8; i += static_cast<long long>(gridDim.x) * blockDim.x) {
+    const uint4 u = __ldg(reinterpret_cast<const uint4*>(in) + i);
+    reinterpret_cast<uint4*>(out)[i] = make_uint4(pack_f16(bf16_lo(u.x), bf16_hi(u.x)), pack_f16(bf16_lo(u.y), bf16_hi(u.y)),
+                                                  pack_f16(bf16_lo(u.z), bf16_hi(u.z)), pack_f16(bf16_lo(u.w), bf16_hi(u.w)));
+  }
+}
+
+// x0[t,:] = E[id_t,:]  (bf16 table row -> fp32 or bf16 stream).  One block per token.
+template <typename OT>
+__global__ void embed_gather_kernel(const int* __restrict__ ids, const __nv_bfloat16* __restrict__ table, OT* __restrict__ out, int H) {
+  const long long t = blockIdx.x;
+  const __nv_bfloat16* src = table + static_cast<long long>(ids[t]) * H;
+  for (int c = threadIdx.x * 4; c < H; c += blockDim.x * 4) {
+    const float4 v = Vec4<__nv_bfloat16>::load(src + c);
+    if constexpr (sizeof(OT) == 4) *reinterpret_cast<float4*>(out + t * H + c) = v;
+    else store_bf16x4(reinterpret_cast<__nv_bfloat16*>(out) + t * H + c, v);
+  }
+}
+
+}  // namespace lsp

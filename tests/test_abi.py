@@ -1,0 +1,60 @@
+"""CPU-side checks of the boundary: liblsp.so builds for sm_100a, loads, and exports every entry point that
+include/lsp.h declares (no compute calls: there is no GPU here), and the binding mirrors the same names."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def libpath():
+    from paper_2510_02483_b200 import build
+    return build.build()           # no-op when the in-tree .so is up to date
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "lsp.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(lsp_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_header_declares_north_star_calls():
+    names = declared_symbols()
+    for n in ("lsp_attn_fwd", "lsp_attn_bwd", "lsp_mlp_fwd", "lsp_mlp_bwd", "lsp_layer_fwd", "lsp_layer_bwd"):
+        assert n in names
+
+
+def test_library_exports_every_declared_symbol(libpath):
+    lib = ctypes.CDLL(libpath)
+    for n in declared_symbols():
+        assert hasattr(lib, n), f"liblsp.so does not export {n}"
+
+
+def test_binding_mirrors_header(libpath):
+    from paper_2510_02483_b200 import binding
+    binding.lib()
+    assert sorted(binding.EXPORTS) == declared_symbols()
+    for n in declared_symbols():
+        if n not in ("lsp_create", "lsp_destroy", "lsp_saved_bytes", "lsp_workspace_bytes", "lsp_last_error"):
+            assert callable(getattr(binding, n)), n
+
+
+def test_null_arguments_are_rejected_without_a_gpu(libpath):
+    lib = ctypes.CDLL(libpath)
+    lib.lsp_create.restype = ctypes.c_int
+    assert lib.lsp_create(None, None, 0) == -1          # LSP_EINVAL
+    lib.lsp_layer_fwd.restype = ctypes.c_int
+    assert lib.lsp_layer_fwd(None, None, None, None, None, None, None) == -1
+
+
+def test_sass_is_blackwell_native(libpath):
+    """The GEMM kernels must contain tcgen05 MMA (UTC*MMA), TMEM loads (LDTM) and TMA loads (UTMALDG)."""
+    import subprocess
+    cuobjdump = "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    sass = subprocess.run([cuobjdump, "-sass", libpath], capture_output=True, text=True).stdout
+    assert re.search(r"UTC[A-Z]*MMA", sass) and "LDTM" in sass and "UTMALDG" in sass

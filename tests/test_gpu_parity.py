@@ -1,0 +1,165 @@
+"""GPU parity: the CUDA path (through the C ABI / binding) against the fp64 oracle, element by element,
+on the same seeded bf16 inputs.  Bar (BASELINE.json north_star): max|gpu - ref| / rms(ref) <= 2e-2 per tensor;
+bit-exact for the integer-indexed embedding gather.
+"""
+import numpy as np
+import pytest
+
+from oracle import lspref as R
+from paper_2510_02483_b200 import synth
+from tests.util import TOL, norm_err
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device")
+    from paper_2510_02483_b200 import binding, harness
+    binding.lib()                      # fail loudly if liblsp.so is missing
+    return harness
+
+
+def oracle_shape(w, use_rope=True):
+    return R.LayerShape(w.batch, w.seq, w.hidden, w.n_q_heads, w.n_kv_heads, w.head_dim, w.ffn, w.rms_eps, w.rope_base,
+                        0, use_rope)
+
+
+def f64(d):
+    return {k: synth.bf16_bits_to_f64(v) for k, v in d.items()}
+
+
+def check(got: dict, ref: dict, names, tol=TOL):
+    errs = {n: norm_err(got[n], ref[n]) for n in names}
+    print("  ".join(f"{n}={e:.2e}" for n, e in errs.items()))
+    bad = {n: e for n, e in errs.items() if not e <= tol}
+    assert not bad, f"normalised error above {tol}: {bad}"
+
+
+ALL = ("y", "dx", "dwq", "dwk", "dwv", "dwo", "dw_gate", "dw_up", "dw_down", "dg_attn", "dg_mlp")
+
+# ------------------------------------------------------------------------------------------- GEMM building block
+GEMM_SHAPES = [(128, 256, 64), (256, 512, 128), (384, 264, 200), (136, 72, 1000), (1000, 1024, 72), (128, 688, 256)]
+
+
+@pytest.mark.parametrize("op", [0, 1, 2])
+@pytest.mark.parametrize("M,N,K", GEMM_SHAPES)
+def test_gemm_vs_fp64(gpu, op, M, N, K):
+    """lsp_gemm (tcgen05) against numpy float64 matmul: all three operand-major variants, ragged M/N/K tails."""
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    rng = np.random.default_rng([op, M, N, K])
+    Kp = (K + 7) // 8 * 8
+    a_shape = (M, Kp) if op < 2 else (K, M)
+    b_shape = (N, Kp) if op == 0 else (K, N)
+    a = synth.f32_to_bf16_bits(rng.standard_normal(a_shape, dtype=np.float32))
+    b = synth.f32_to_bf16_bits(rng.standard_normal(b_shape, dtype=np.float32))
+    A64, B64 = synth.bf16_bits_to_f64(a), synth.bf16_bits_to_f64(b)
+    if op == 0:
+        ref = A64[:, :K] @ B64[:, :K].T
+    elif op == 1:
+        ref = A64[:, :K] @ B64
+    else:
+        ref = A64.T @ B64
+    w = synth.CFG1_TINY
+    ctx = gpu.make_ctx(w)
+    dA, dB = gpu.bf16_to_device(a), gpu.bf16_to_device(b)
+    out = torch.full((M, N), float("nan"), dtype=torch.float32, device=dA.device)
+    B.lsp_gemm(ctx, op, M, N, K, dA, a_shape[1], dB, b_shape[1], out, N)
+    torch.cuda.synchronize()
+    err = norm_err(out.cpu().numpy(), ref)
+    ctx.close()
+    assert err < 1e-5, err            # exact bf16 products, fp32 accumulation
+
+
+# ------------------------------------------------------------------------------------------- whole layer
+MID = synth.Workload("mid", 101, 2, 320, 512, 8, 2, 128, 1376, 1e-5, 500000.0)
+MID64 = synth.Workload("mid64", 102, 3, 200, 384, 6, 6, 64, 1000, 1e-5, 10000.0)
+
+
+@pytest.mark.parametrize("w", [synth.CFG1_TINY, MID, MID64], ids=lambda w: w.name)
+def test_layer_fwd_bwd(gpu, w):
+    """lsp_layer_fwd + lsp_layer_bwd: y, dx and all nine gradients (cfg 1 = BASELINE.json configs[0])."""
+    got = gpu.run_layer(w)
+    inp, wt = f64(synth.layer_inputs(w)), f64(synth.layer_weights(w))
+    ref = R.layer_fwd_bwd(inp["x"], inp["dy"], wt, oracle_shape(w))
+    check(got, ref, ALL)
+
+
+def test_blocks_cfg1(gpu):
+    """lsp_attn_fwd/bwd and lsp_mlp_fwd/bwd called on their own (block-level entry points), bf16 in."""
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    w = synth.CFG1_TINY
+    cfg = oracle_shape(w)
+    inp, wbits = synth.layer_inputs(w), synth.layer_weights(w)
+    x64, dy64, w64 = synth.bf16_bits_to_f64(inp["x"]), synth.bf16_bits_to_f64(inp["dy"]), f64(wbits)
+    ctx = gpu.make_ctx(w)
+    buf = gpu.LayerBuffers(ctx, w)
+    weights = gpu.upload_weights(wbits)
+    x, dy = gpu.bf16_to_device(inp["x"]), gpu.bf16_to_device(inp["dy"])
+    # attention block
+    B.lsp_attn_fwd(ctx, x, weights, buf.y, buf.saved, buf.ws)
+    B.lsp_attn_bwd(ctx, x, dy, weights, buf.saved, buf.dx, buf.grads, buf.ws)
+    torch.cuda.synchronize()
+    a_ref, cache = R.attn_block_fwd(x64, w64, cfg)
+    dx_ref, g_ref = R.attn_block_bwd(dy64, w64, cfg, cache)
+    got = dict(a=buf.y.cpu().numpy(), dx=buf.dx.cpu().numpy(), **{"d" + k: buf.grads[k].cpu().numpy() for k in g_ref})
+    check(got, dict(a=a_ref, dx=dx_ref, **{"d" + k: v for k, v in g_ref.items()}), ["a", "dx"] + ["d" + k for k in g_ref])
+    # MLP block (input = the same bf16 x)
+    B.lsp_mlp_fwd(ctx, x, weights, buf.y, buf.saved, buf.ws)
+    B.lsp_mlp_bwd(ctx, x, dy, weights, buf.saved, buf.dx, buf.grads, buf.ws)
+    torch.cuda.synchronize()
+    y_ref, cache = R.mlp_block_fwd(x64, w64, cfg)
+    da_ref, g_ref = R.mlp_block_bwd(dy64, w64, cfg, cache)
+    got = dict(y=buf.y.cpu().numpy(), da=buf.dx.cpu().numpy(), **{"d" + k: buf.grads[k].cpu().numpy() for k in g_ref})
+    check(got, dict(y=y_ref, da=da_ref, **{"d" + k: v for k, v in g_ref.items()}), ["y", "da"] + ["d" + k for k in g_ref])
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------------- attention core (cfg 5 layout)
+@pytest.mark.parametrize("B_,S,nq,nkv,d", [(2, 256, 24, 8, 128), (1, 200, 4, 4, 64), (1, 1, 2, 1, 128), (3, 65, 6, 2, 128)])
+def test_sdpa_fwd_bwd(gpu, B_, S, nq, nkv, d):
+    """lsp_sdpa_fwd/bwd: O, L, dq, dk, dv on bf16 Q,K,V,dO ~ N(0,1) (no RoPE), incl. ragged S and S = 1."""
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    w = synth.Workload("sdpa", 5, B_, S, nq * d, nq, nkv, d, 64)
+    bits = synth.attn_inputs(w)
+    ctx = gpu.make_ctx(w, use_rope=False)
+    dev = torch.device("cuda")
+    t = {k: gpu.bf16_to_device(v) for k, v in bits.items()}
+    o = torch.empty((B_, S, nq, d), dtype=torch.float32, device=dev)
+    lse = torch.empty((B_, nq, S), dtype=torch.float32, device=dev)
+    dq = torch.empty_like(o)
+    dk = torch.empty((B_, S, nkv, d), dtype=torch.float32, device=dev)
+    dv = torch.empty_like(dk)
+    ws = torch.empty(ctx.workspace_bytes, dtype=torch.uint8, device=dev)
+    B.lsp_sdpa_fwd(ctx, t["q"], t["k"], t["v"], o, lse, ws)
+    B.lsp_sdpa_bwd(ctx, t["q"], t["k"], t["v"], o, lse, t["dO"], dq, dk, dv, ws)
+    torch.cuda.synchronize()
+    i64 = f64(bits)
+    O_ref, L_ref = R.sdpa_fwd(i64["q"], i64["k"], i64["v"])
+    dq_ref, dk_ref, dv_ref = R.sdpa_bwd(i64["q"], i64["k"], i64["v"], i64["dO"])
+    got = dict(O=o.cpu().numpy(), L=lse.cpu().numpy(), dq=dq.cpu().numpy(), dk=dk.cpu().numpy(), dv=dv.cpu().numpy())
+    check(got, dict(O=O_ref, L=L_ref, dq=dq_ref, dk=dk_ref, dv=dv_ref), ["O", "L", "dq", "dk", "dv"])
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------------- embedding gather
+def test_embed_bit_exact(gpu):
+    """lsp_embed_fwd: x0[t,:] = E[id_t,:], integer indexing -> bit-exact against the oracle."""
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    w = synth.Workload("emb", 3, 2, 96, 256, 4, 2, 64, 688, vocab=1000)
+    s = synth.stack_inputs(w)
+    ctx = gpu.make_ctx(w)
+    ids = torch.from_numpy(s["ids"]).cuda()
+    table = gpu.bf16_to_device(s["embedding"])
+    x0 = torch.empty((w.tokens, w.hidden), dtype=torch.float32, device="cuda")
+    B.lsp_embed_fwd(ctx, ids, table, x0)
+    torch.cuda.synchronize()
+    ref = R.embed_fwd(s["ids"], synth.bf16_bits_to_f64(s["embedding"]))
+    assert np.array_equal(x0.cpu().numpy().astype(np.float64), ref)
+    ctx.close()
