@@ -45,7 +45,7 @@ typedef enum {
   LSP_EALIGN = -5         /* pointer alignment violated */
 } lsp_status;
 
-typedef enum { LSP_BF16 = 0, LSP_F32 = 1 } lsp_dtype;
+typedef enum { LSP_BF16 = 0, LSP_F32 = 1, LSP_F16 = 2 } lsp_dtype;
 
 /* One decoder layer (Table 1 / section 2.4; BASELINE.json configs). */
 typedef struct {
@@ -110,13 +110,15 @@ lsp_status lsp_sdpa_bwd(lsp_ctx* ctx, const void* q, const void* k, const void* 
 /* Embedding gather (config 3):  x0[t,:] = table[ids[t],:]; ids int32 [T], table bf16 [vocab,H] -> x0 fp32 [T,H]. */
 lsp_status lsp_embed_fwd(lsp_ctx* ctx, const int32_t* ids, const void* table, void* x0, void* stream);
 
-/* Building block / test hook: one bias-free linear-layer GEMM on the tcgen05 kernel, bf16 in, fp32 out.
+/* Building block / test hook: one bias-free linear-layer GEMM on the tcgen05 kernel, 16-bit in, fp32 out.
+ * a_dtype / b_dtype: both LSP_BF16 or both LSP_F16; a mixed pair returns LSP_EUNSUPPORTED (one
+ * tcgen05.mma.kind::f16 with unequal operand formats faults on sm_100a).
  *   op 0 (forward): C[M,N] = A[M,K] . B[N,K]^T        A,B row-major as written
  *   op 1 (dgrad)  : C[M,N] = A[M,K] . B[K,N]          B row-major [K,N]
  *   op 2 (wgrad)  : C[M,N] = A[K,M]^T . B[K,N]        A row-major [K,M], B row-major [K,N]
  * lda/ldb/ldc are row pitches in elements (multiples of 8).  Needs no ctx state beyond the device. */
-lsp_status lsp_gemm(lsp_ctx* ctx, int op, int M, int N, int K, const void* A, int64_t lda, const void* B, int64_t ldb,
-                    float* C, int64_t ldc, void* stream);
+lsp_status lsp_gemm(lsp_ctx* ctx, int op, int M, int N, int K, const void* A, int64_t lda, int a_dtype, const void* B,
+                    int64_t ldb, int b_dtype, float* C, int64_t ldc, void* stream);
 
 /* End-to-end step with HOST buffers (bench.py `e2e`): copies x, dy (in_dtype, [T,H]; pinned host memory for
  * asynchronous copies) to the caller's device staging buffers x_dev / dy_dev, runs lsp_layer_fwd + lsp_layer_bwd,

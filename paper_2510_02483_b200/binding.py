@@ -12,7 +12,7 @@ import os
 _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "liblsp.so")
 
-LSP_BF16, LSP_F32 = 0, 1
+LSP_BF16, LSP_F32, LSP_F16 = 0, 1, 2
 STATUS = {0: "LSP_OK", -1: "LSP_EINVAL", -2: "LSP_EUNSUPPORTED", -3: "LSP_ENOMEM", -4: "LSP_ECUDA", -5: "LSP_EALIGN"}
 WEIGHT_FIELDS = ("wq", "wk", "wv", "wo", "g_attn", "w_gate", "w_up", "w_down", "g_mlp")
 EXPORTS = ("lsp_create", "lsp_destroy", "lsp_saved_bytes", "lsp_workspace_bytes", "lsp_last_error",
@@ -66,7 +66,7 @@ def lib():
         L.lsp_sdpa_fwd.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
         L.lsp_sdpa_bwd.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.lsp_embed_fwd.argtypes = [vp, vp, vp, vp, vp]
-        L.lsp_gemm.argtypes = [vp, i32, i32, i32, i32, vp, i64, vp, i64, vp, i64, vp]
+        L.lsp_gemm.argtypes = [vp, i32, i32, i32, i32, vp, i64, i32, vp, i64, i32, vp, i64, vp]
         L.lsp_layer_step_host.argtypes = [vp, vp, vp, pw, vp, vp, pg, vp, vp, vp, vp, vp, vp, vp]
         L.lsp_launch_count.argtypes = [vp]; L.lsp_launch_count.restype = C.c_longlong
         L.lsp_timing_enable.argtypes = [vp, i32]
@@ -180,8 +180,9 @@ def lsp_embed_fwd(ctx, ids, table, x0, stream=None):
     ctx.check(lib().lsp_embed_fwd(ctx.handle, _ptr(ids), _ptr(table), _ptr(x0), _stream(stream)))
 
 
-def lsp_gemm(ctx, op, M, N, K, A, lda, B, ldb, Cout, ldc, stream=None):
-    ctx.check(lib().lsp_gemm(ctx.handle, op, M, N, K, _ptr(A), lda, _ptr(B), ldb, _ptr(Cout), ldc, _stream(stream)))
+def lsp_gemm(ctx, op, M, N, K, A, lda, a_dtype, B, ldb, b_dtype, Cout, ldc, stream=None):
+    ctx.check(lib().lsp_gemm(ctx.handle, op, M, N, K, _ptr(A), lda, a_dtype, _ptr(B), ldb, b_dtype, _ptr(Cout), ldc,
+                             _stream(stream)))
 
 
 def lsp_layer_step_host(ctx, x_host, dy_host, weights, y_host, dx_host, grads, x_dev, dy_dev, y_dev, dx_dev, saved, ws,

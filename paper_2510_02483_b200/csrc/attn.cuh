@@ -22,13 +22,13 @@ struct AttnParams {
   float scale_log2;            // (1/sqrt(d)) * log2(e)
   float scale;                 // 1/sqrt(d)
   // forward outputs
-  float* o32; __nv_bfloat16* o16; long long ldo;    // either may be null
+  float* o32; __half* o16; long long ldo;           // either may be null
   float* lse;                  // [B, nq, S]
   // backward inputs/outputs
   const float* dvec;           // D [B, nq, S]
   const float2* rope;          // (cos,sin) [S, d/2] or null: inverse rotation applied to dq, dk on store
   float* dq32; float* dk32; float* dv32; long long lddq32, lddk32;             // fp32 outputs (sdpa API) or null
-  __nv_bfloat16* dq16; __nv_bfloat16* dk16; __nv_bfloat16* dv16; long long ldd16;   // bf16 outputs (layer path) or null
+  __half* dq16; __half* dk16; __half* dv16; long long ldd16;   // fp16 outputs (layer path: GEMM operands) or null
 };
 
 // ------------------------------------------------------------------------------------------- primitives
@@ -220,7 +220,7 @@ __global__ void __launch_bounds__(256, 1) attn_fwd_kernel(const AttnParams p) {
         const int col = h * D + i * 8 + (lane & 3) * 2;
         const float v0 = o[i][2 * r] * inv, v1 = o[i][2 * r + 1] * inv;
         if (p.o32) *reinterpret_cast<float2*>(p.o32 + t * p.ldo + col) = make_float2(v0, v1);
-        if (p.o16) *reinterpret_cast<uint32_t*>(p.o16 + t * p.ldo + col) = pack_bf16(v0, v1);
+        if (p.o16) *reinterpret_cast<uint32_t*>(p.o16 + t * p.ldo + col) = pack_f16(v0, v1);
       }
     }
   }
@@ -252,11 +252,11 @@ __global__ void attn_dvec_kernel(const __half* dO, long long lddo, const float* 
 }
 
 // Store a 16 x D fp32 accumulator tile (mma C layout) of rows s_row0+{0,8}: scale, optional inverse RoPE,
-// to fp32 and/or bf16 destinations.
+// to fp32 and/or fp16 destinations.
 template <int D>
 __device__ __forceinline__ void store_grad_tile(float (&acc)[D / 8][4], float scale, const float2* rope, int S,
                                                 long long tok0, int s_row0, int lane, float* o32, long long ld32,
-                                                __nv_bfloat16* o16, long long ld16, int col_base) {
+                                                __half* o16, long long ld16, int col_base) {
 #pragma unroll
   for (int r = 0; r < 2; ++r) {
     const int s = s_row0 + r * 8;
@@ -273,7 +273,7 @@ __device__ __forceinline__ void store_grad_tile(float (&acc)[D / 8][4], float sc
         v1 = -z0 * cs.y + z1 * cs.x;
       }
       if (o32) *reinterpret_cast<float2*>(o32 + t * ld32 + col_base + c) = make_float2(v0, v1);
-      if (o16) *reinterpret_cast<uint32_t*>(o16 + t * ld16 + col_base + c) = pack_bf16(v0, v1);
+      if (o16) *reinterpret_cast<uint32_t*>(o16 + t * ld16 + col_base + c) = pack_f16(v0, v1);
     }
   }
 }

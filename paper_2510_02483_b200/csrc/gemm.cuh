@@ -2,7 +2,7 @@
 //
 //   C[M,N] = sum over K-segments s of  A_s[M,K_s] * B_s[N,K_s]^T        (fp32 accumulate in TMEM)
 //
-// Operands are 16-bit (bf16), fetched by TMA into 128B-swizzled shared memory in a multi-stage
+// Operands are 16-bit (both fp16 or both bf16), fetched by TMA into 128B-swizzled shared memory in a multi-stage
 // mbarrier ring; either operand may be K-major (row = M/N index, K contiguous) or MN-major
 // (row = K index, M/N contiguous) so that dgrad (dX = dY W) and wgrad (dW = dY^T X) run on the
 // tensors as they lie in HBM -- no transposes.  One elected thread issues tcgen05.mma
@@ -31,6 +31,8 @@ struct GemmMaps {
 };
 struct GemmShape {
   int M, N;                          // output extent (DUAL: N = columns of each of the two outputs)
+  int a_fmt, b_fmt;                  // UMMA operand formats: 0 = fp16, 1 = bf16; must be equal (a mixed pair is an
+                                     // illegal instruction on sm_100a -- measured)
   int nseg;                          // number of K segments (non-DUAL); DUAL uses a[0], b[0], b[1]
   int kblocks[GEMM_MAX_SEG];         // ceil(K_s / 64)
 };
@@ -132,14 +134,16 @@ struct EpiStore {
   }
 };
 
-// Projection output with fused RoPE (adjacent pairs (2i,2i+1), ref [36]); fp16 out.
+// Fused QKV projection output [T, Nq+2Nkv] (fp16) with RoPE on the q and k columns (adjacent pairs (2i,2i+1);
+// SURVEY 8(c) step 3, ref [36]); v columns (n >= rot_cols) pass through.  Nq, Nkv are multiples of d >= 64 and the
+// epilogue works on 32-column chunks, so a chunk never straddles a head or the q|k|v boundaries.
 // rope table: float2 (cos, sin) [S, d/2], angles computed in fp64 on the host (reading A-5).
-template <bool ROPE>
-struct EpiProjRope {
-  __half* out; long long ld; int col_off;   // output row pitch, first output column of this projection
+struct EpiQKVRope {
+  __half* out; long long ld;
   const float2* rope; int S, d;
+  int rot_cols;              // columns [0, rot_cols) are rotated (Nq + Nkv, or 0 when use_rope = 0)
   __device__ __forceinline__ void operator()(int m, int n, float (&v)[32], int nvalid) const {
-    if constexpr (ROPE) {
+    if (n < rot_cols) {
       const int pos = m % S;
       const float2* t = rope + static_cast<long long>(pos) * (d >> 1) + ((n % d) >> 1);
 #pragma unroll
@@ -152,13 +156,13 @@ struct EpiProjRope {
         }
       }
     }
-    store_row32<DT_F16>(out + static_cast<long long>(m) * ld + col_off + n, v, nvalid);
+    store_row32<DT_F16>(out + static_cast<long long>(m) * ld + n, v, nvalid);
   }
 };
 
 // DUAL epilogue: h = silu(g) * u (ref [35]); saves g,u in fp16 for the backward (DESIGN.md precision plan).
 struct EpiSwiGLU {
-  __nv_bfloat16* h; __half* g16; __half* u16; long long ld;
+  __half* h; __half* g16; __half* u16; long long ld;
   __device__ __forceinline__ void operator()(int m, int n, float (&g)[32], float (&u)[32], int nvalid) const {
     const long long off = static_cast<long long>(m) * ld + n;
     store_row32<DT_F16>(g16 + off, g, nvalid);
@@ -169,14 +173,14 @@ struct EpiSwiGLU {
       const float sg = 1.0f / (1.0f + __expf(-g[j]));
       hv[j] = g[j] * sg * u[j];
     }
-    store_row32<DT_BF16>(h + off, hv, nvalid);
+    store_row32<DT_F16>(h + off, hv, nvalid);
   }
 };
 
-// Down-projection dgrad with fused SwiGLU backward: acc = dh; writes [dg | du] (bf16) into one [T, 2F] buffer.
+// Down-projection dgrad with fused SwiGLU backward: acc = dh; writes [dg | du] (fp16) into one [T, 2F] buffer.
 struct EpiSwiGLUBwd {
   const __half* g16; const __half* u16; long long ld;      // saved g,u [T,F]
-  __nv_bfloat16* dgu; int F;                               // [T, 2F]
+  __half* dgu; int F;                                      // [T, 2F]
   __device__ __forceinline__ void operator()(int m, int n, float (&dh)[32], int nvalid) const {
     float g[32], u[32];
     const long long off = static_cast<long long>(m) * ld + n;
@@ -189,9 +193,9 @@ struct EpiSwiGLUBwd {
       du[j] = dh[j] * g[j] * sg;
       dg[j] = dh[j] * u[j] * sg * (1.0f + g[j] * (1.0f - sg));
     }
-    __nv_bfloat16* row = dgu + static_cast<long long>(m) * (2LL * F);
-    store_row32<DT_BF16>(row + n, dg, nvalid);
-    store_row32<DT_BF16>(row + F + n, du, nvalid);
+    __half* row = dgu + static_cast<long long>(m) * (2LL * F);
+    store_row32<DT_F16>(row + n, dg, nvalid);
+    store_row32<DT_F16>(row + F + n, du, nvalid);
   }
 };
 
@@ -280,7 +284,7 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, c
   } else if (warp == 1) {
     // ===================================================================== MMA issuer
     if (lane == 0) {
-      constexpr uint32_t idesc = umma_idesc(GEMM_BM, BN, 1, 1, A_MN ? 1 : 0, B_MN ? 1 : 0);
+      const uint32_t idesc = umma_idesc(GEMM_BM, BN, sh.a_fmt, sh.b_fmt, A_MN ? 1 : 0, B_MN ? 1 : 0);
       // K-major: atoms of 8 rows x 128 B, SBO = 1024; one UMMA_K (16 elems) = +32 B inside the swizzle row.
       // MN-major: LBO = bytes between 64-wide M/N chunks (BK*128), SBO = 1024 between 8-k-row atoms;
       //           one UMMA_K (16 k-rows) = +2048 B.
@@ -391,12 +395,14 @@ struct Operand {
   const void* ptr;
   long long ld;       // pitch in elements
   bool mn_major;      // false: [MN, K] row-major (K contiguous); true: [K, MN] row-major (MN contiguous)
+  int dt = DT_F16;    // DT_F16 (every operand the layer path produces) or DT_BF16; A and B must match
 };
+inline int umma_fmt(int dt) { return dt == DT_F16 ? 0 : 1; }
 
 // Encode the map of an operand with logical extents (mn, k); rows_box = tile rows for K-major.
 inline bool encode_operand(CUtensorMap* m, const Operand& o, long long mn, long long k, int tile_mn) {
-  if (!o.mn_major) return make_map_2d(m, o.ptr, mn, k, o.ld, tile_mn);
-  return make_map_2d(m, o.ptr, k, mn, o.ld, GEMM_BK);
+  if (!o.mn_major) return make_map_2d(m, o.ptr, mn, k, o.ld, tile_mn, o.dt == DT_F16);
+  return make_map_2d(m, o.ptr, k, mn, o.ld, GEMM_BK, o.dt == DT_F16);
 }
 
 template <int BN, bool A_MN, bool B_MN, bool DUAL, class Epi>
@@ -425,6 +431,7 @@ cudaError_t gemm_run(int M, int N, int nseg, const Operand* a, const Operand* b,
   GemmMaps maps;
   GemmShape sh;
   sh.M = M; sh.N = N; sh.nseg = nseg;
+  sh.a_fmt = umma_fmt(a[0].dt); sh.b_fmt = umma_fmt(b[0].dt);      // all segments share the operand formats
   for (int s = 0; s < GEMM_MAX_SEG; ++s) sh.kblocks[s] = 0;
   for (int s = 0; s < nseg; ++s) {
     sh.kblocks[s] = (ks[s] + GEMM_BK - 1) / GEMM_BK;
@@ -441,6 +448,7 @@ cudaError_t gemm_run_dual(int M, int N, int K, const Operand& a, const Operand& 
   GemmMaps maps;
   GemmShape sh;
   sh.M = M; sh.N = N; sh.nseg = 1;
+  sh.a_fmt = umma_fmt(a.dt); sh.b_fmt = umma_fmt(bg.dt);
   sh.kblocks[0] = (K + GEMM_BK - 1) / GEMM_BK; sh.kblocks[1] = sh.kblocks[2] = 0;
   if (!encode_operand(&maps.a[0], a, M, K, GEMM_BM)) return cudaErrorInvalidValue;
   if (!encode_operand(&maps.b[0], bg, N, K, 128)) return cudaErrorInvalidValue;

@@ -24,7 +24,9 @@ inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 // Byte offsets inside `saved` and `ws` (all 256-byte aligned).
 struct SavedLayout {
-  size_t a32, xn, rstd1, qkv16, o32, o16, lse, an, rstd2, g16, u16, h, total;
+  size_t a32, xn, rstd1, qkv16, o32, o16, lse, an, rstd2, g16, u16, h;
+  size_t wqkv16, wo16, wgu16, wd16;      // fp16 copies of the bf16 weights (made by the forward, reused by the backward)
+  size_t total;
 };
 struct WsLayout {
   size_t in16, dgu, dn32, da32, da16, dO16, dvec, dqkv16, dgpart, q16, k16, v16, total;
@@ -120,6 +122,10 @@ void plan_layout(lsp_ctx* c) {
   s.g16 = take(T * F * 2);
   s.u16 = take(T * F * 2);
   s.h = take(T * F * 2);
+  s.wqkv16 = take(Nqkv * H * 2);          // [Wq; Wk; Wv] stacked: one [Nqkv, H] matrix
+  s.wo16 = take(H * Nq * 2);
+  s.wgu16 = take(2 * F * H * 2);          // [Wg; Wu] stacked: one [2F, H] matrix
+  s.wd16 = take(H * F * 2);
   s.total = o;
 
   o = 0;
@@ -146,7 +152,7 @@ template <typename T> const T* at(const void* base, size_t off) {
 
 // ------------------------------------------------------------------------------------------- norm dispatch
 template <typename XT>
-cudaError_t norm_fwd_t(const lsp_ctx* c, const void* x, const void* g, __nv_bfloat16* xn, float* rstd, cudaStream_t st) {
+cudaError_t norm_fwd_t(const lsp_ctx* c, const void* x, const void* g, __half* xn, float* rstd, cudaStream_t st) {
   const int H = c->d.hidden, nv = (H / 4 + NORM_THREADS - 1) / NORM_THREADS;
   const XT* xp = static_cast<const XT*>(x);
   const __nv_bfloat16* gp = static_cast<const __nv_bfloat16*>(g);
@@ -155,13 +161,13 @@ cudaError_t norm_fwd_t(const lsp_ctx* c, const void* x, const void* g, __nv_bflo
 #undef LSP_NF
   return cudaGetLastError();
 }
-cudaError_t norm_fwd(const lsp_ctx* c, int dt, const void* x, const void* g, __nv_bfloat16* xn, float* rstd, cudaStream_t st) {
+cudaError_t norm_fwd(const lsp_ctx* c, int dt, const void* x, const void* g, __half* xn, float* rstd, cudaStream_t st) {
   return dt == LSP_F32 ? norm_fwd_t<float>(c, x, g, xn, rstd, st) : norm_fwd_t<__nv_bfloat16>(c, x, g, xn, rstd, st);
 }
 
 template <typename XT, typename RT>
 cudaError_t norm_bwd_t(const lsp_ctx* c, const void* x, const float* rstd, const void* g, const float* dxn, const void* dres,
-                       float* dx, __nv_bfloat16* dx16, float* dg_part, float* dg, cudaStream_t st) {
+                       float* dx, __half* dx16, float* dg_part, float* dg, cudaStream_t st) {
   const int H = c->d.hidden, nv = (H / 4 + NORM_THREADS - 1) / NORM_THREADS;
   const XT* xp = static_cast<const XT*>(x);
   const RT* rp = static_cast<const RT*>(dres);
@@ -177,7 +183,7 @@ cudaError_t norm_bwd_t(const lsp_ctx* c, const void* x, const float* rstd, const
 }
 // x: forward input of the norm (XT = x_dt); dres: incoming residual gradient (RT = r_dt)
 cudaError_t norm_bwd(const lsp_ctx* c, int x_dt, int r_dt, const void* x, const float* rstd, const void* g, const float* dxn,
-                     const void* dres, float* dx, __nv_bfloat16* dx16, float* dg_part, float* dg, cudaStream_t st) {
+                     const void* dres, float* dx, __half* dx16, float* dg_part, float* dg, cudaStream_t st) {
   if (x_dt == LSP_F32)
     return r_dt == LSP_F32 ? norm_bwd_t<float, float>(c, x, rstd, g, dxn, dres, dx, dx16, dg_part, dg, st)
                            : norm_bwd_t<float, __nv_bfloat16>(c, x, rstd, g, dxn, dres, dx, dx16, dg_part, dg, st);
@@ -185,12 +191,12 @@ cudaError_t norm_bwd(const lsp_ctx* c, int x_dt, int r_dt, const void* x, const 
                          : norm_bwd_t<__nv_bfloat16, __nv_bfloat16>(c, x, rstd, g, dxn, dres, dx, dx16, dg_part, dg, st);
 }
 
-cudaError_t cast_f32_bf16(const float* in, __nv_bfloat16* out, long long n, int sms, cudaStream_t st) {
+cudaError_t cast_f32_f16(const float* in, __half* out, long long n, int sms, cudaStream_t st) {
   const long long n8 = n / 8;
   long long blocks = (n8 + 255) / 256;
   if (blocks > sms * 16LL) blocks = sms * 16LL;
   if (blocks < 1) blocks = 1;
-  cast_f32_bf16_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(in, out, n8);
+  cast_f32_f16_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(in, out, n8);
   return cudaGetLastError();
 }
 cudaError_t cast_bf16_f16(const __nv_bfloat16* in, __half* out, long long n, int sms, cudaStream_t st) {
@@ -224,7 +230,7 @@ cudaError_t gemm1(const lsp_ctx* c, int M, int N, int K, const Operand& a, const
 }
 
 // out[T,H] fp32 = res + A[T,K] . W[H,K]^T   (O-proj and down-proj forward with the residual epilogue; F4, F7)
-cudaError_t gemm_fwd_residual(const lsp_ctx* c, const __nv_bfloat16* A, int K, const void* W, int res_dt, const void* res,
+cudaError_t gemm_fwd_residual(const lsp_ctx* c, const __half* A, int K, const __half* W, int res_dt, const void* res,
                               float* out, cudaStream_t st) {
   const int T = c->T, H = c->d.hidden;
   const Operand a{A, K, false}, b{W, K, false};
@@ -238,37 +244,35 @@ cudaError_t gemm_fwd_residual(const lsp_ctx* c, const __nv_bfloat16* A, int K, c
   return gemm1<false, false>(c, T, H, K, a, b, e, st);
 }
 
+// fp16 copy of a bf16 weight matrix (exact for 2^-17 <= |w| < 65504; DESIGN.md precision plan)
+#define LSP_WCAST(src, dst, n) \
+  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(src), dst, static_cast<long long>(n), ctx->num_sms, st))
+
 // ------------------------------------------------------------------------------------------- attention block
 // x [T,H] x_dt -> a32 [T,H] fp32.  SURVEY 8(a) F1-F4.
 lsp_status attn_fwd_impl(lsp_ctx* ctx, int x_dt, const void* x, const lsp_layer_weights* w, float* a_out, void* saved,
                          cudaStream_t st) {
   const lsp_layer_desc& d = ctx->d;
   const int T = ctx->T, H = d.hidden, Nq = ctx->Nq, Nkv = ctx->Nkv, Nqkv = ctx->Nqkv;
-  __nv_bfloat16* xn = at<__nv_bfloat16>(saved, ctx->sv.xn);
+  __half* xn = at<__half>(saved, ctx->sv.xn);
   float* rstd1 = at<float>(saved, ctx->sv.rstd1);
   __half* qkv = at<__half>(saved, ctx->sv.qkv16);
   float* o32 = at<float>(saved, ctx->sv.o32);
-  __nv_bfloat16* o16 = at<__nv_bfloat16>(saved, ctx->sv.o16);
+  __half* o16 = at<__half>(saved, ctx->sv.o16);
   float* lse = at<float>(saved, ctx->sv.lse);
+  __half* wqkv16 = at<__half>(saved, ctx->sv.wqkv16);
+  __half* wo16 = at<__half>(saved, ctx->sv.wo16);
 
+  LSP_WCAST(w->wq, wqkv16, static_cast<long long>(Nq) * H);
+  LSP_WCAST(w->wk, wqkv16 + static_cast<long long>(Nq) * H, static_cast<long long>(Nkv) * H);
+  LSP_WCAST(w->wv, wqkv16 + static_cast<long long>(Nq + Nkv) * H, static_cast<long long>(Nkv) * H);
+  LSP_WCAST(w->wo, wo16, static_cast<long long>(H) * Nq);
   // F1 RMSNorm-1
   LSP_STAGE(ST_NORM_FWD, 1, norm_fwd(ctx, x_dt, x, w->g_attn, xn, rstd1, st));
-  // F2 QKV projections with the RoPE epilogue (q, k rotated; v plain) into one [T, Nq+2Nkv] fp16 buffer
-  const Operand a{xn, H, false};
+  // F2 fused QKV projection with the RoPE epilogue (q, k rotated; v plain) into one [T, Nq+2Nkv] fp16 buffer
   {
-    EpiProjRope<true> e{qkv, Nqkv, 0, ctx->rope, d.seq, d.head_dim};
-    EpiProjRope<false> en{qkv, Nqkv, 0, ctx->rope, d.seq, d.head_dim};
-    if (d.use_rope) {
-      LSP_STAGE(ST_QKV, 1, (gemm1<false, false>(ctx, T, Nq, H, a, Operand{w->wq, H, false}, e, st)));
-      e.col_off = Nq;
-      LSP_STAGE(ST_QKV, 1, (gemm1<false, false>(ctx, T, Nkv, H, a, Operand{w->wk, H, false}, e, st)));
-    } else {
-      LSP_STAGE(ST_QKV, 1, (gemm1<false, false>(ctx, T, Nq, H, a, Operand{w->wq, H, false}, en, st)));
-      en.col_off = Nq;
-      LSP_STAGE(ST_QKV, 1, (gemm1<false, false>(ctx, T, Nkv, H, a, Operand{w->wk, H, false}, en, st)));
-    }
-    en.col_off = Nq + Nkv;
-    LSP_STAGE(ST_QKV, 1, (gemm1<false, false>(ctx, T, Nkv, H, a, Operand{w->wv, H, false}, en, st)));
+    EpiQKVRope e{qkv, Nqkv, ctx->rope, d.seq, d.head_dim, d.use_rope ? Nq + Nkv : 0};
+    LSP_STAGE(ST_QKV, 1, (gemm1<false, false>(ctx, T, Nqkv, H, Operand{xn, H, false}, Operand{wqkv16, H, false}, e, st)));
   }
   // F3 causal GQA flash forward
   AttnParams p;
@@ -282,25 +286,27 @@ lsp_status attn_fwd_impl(lsp_ctx* ctx, int x_dt, const void* x, const lsp_layer_
   if (d.head_dim == 128) LSP_STAGE(ST_ATTN_FWD, 1, attn_fwd_launch<128>(p, st));
   else LSP_STAGE(ST_ATTN_FWD, 1, attn_fwd_launch<64>(p, st));
   // F4 O-projection + residual
-  LSP_STAGE(ST_OPROJ, 1, gemm_fwd_residual(ctx, o16, Nq, w->wo, x_dt, x, a_out, st));
+  LSP_STAGE(ST_OPROJ, 1, gemm_fwd_residual(ctx, o16, Nq, wo16, x_dt, x, a_out, st));
   return LSP_OK;
 }
 
-// da (da_dt; da16 = its bf16 copy or itself) -> dx fp32.  SURVEY 8(a) B6-B10.
-lsp_status attn_bwd_impl(lsp_ctx* ctx, int x_dt, const void* x, int da_dt, const void* da, const __nv_bfloat16* da16,
+// da (da_dt; da16 = its fp16 copy) -> dx fp32.  SURVEY 8(a) B6-B10.
+lsp_status attn_bwd_impl(lsp_ctx* ctx, int x_dt, const void* x, int da_dt, const void* da, const __half* da16,
                          const lsp_layer_weights* w, const void* saved, float* dx, lsp_layer_wgrads* g, void* ws,
                          cudaStream_t st) {
   const lsp_layer_desc& d = ctx->d;
   const int T = ctx->T, H = d.hidden, Nq = ctx->Nq, Nkv = ctx->Nkv, Nqkv = ctx->Nqkv;
-  const __nv_bfloat16* xn = at<__nv_bfloat16>(saved, ctx->sv.xn);
+  const __half* xn = at<__half>(saved, ctx->sv.xn);
   const float* rstd1 = at<float>(saved, ctx->sv.rstd1);
   const __half* qkv = at<__half>(saved, ctx->sv.qkv16);
   const float* o32 = at<float>(saved, ctx->sv.o32);
-  const __nv_bfloat16* o16 = at<__nv_bfloat16>(saved, ctx->sv.o16);
+  const __half* o16 = at<__half>(saved, ctx->sv.o16);
   const float* lse = at<float>(saved, ctx->sv.lse);
+  const __half* wqkv16 = at<__half>(saved, ctx->sv.wqkv16);
+  const __half* wo16 = at<__half>(saved, ctx->sv.wo16);
   __half* dO16 = at<__half>(ws, ctx->ws.dO16);
   float* dvec = at<float>(ws, ctx->ws.dvec);
-  __nv_bfloat16* dqkv = at<__nv_bfloat16>(ws, ctx->ws.dqkv16);
+  __half* dqkv = at<__half>(ws, ctx->ws.dqkv16);
   float* dxn = at<float>(ws, ctx->ws.dn32);
   float* dgpart = at<float>(ws, ctx->ws.dgpart);
 
@@ -310,7 +316,7 @@ lsp_status attn_bwd_impl(lsp_ctx* ctx, int x_dt, const void* x, int da_dt, const
   {
     EpiStore<DT_F16, DT_F32, false> e;
     e.out[0] = dO16; e.out[1] = e.out[2] = nullptr; e.split1 = e.split2 = 0x7fffffff; e.ld = Nq; e.res = nullptr; e.alpha = 1.0f;
-    LSP_STAGE(ST_DGRAD_O, 1, (gemm1<false, true>(ctx, T, Nq, H, Operand{da16, H, false}, Operand{w->wo, Nq, true}, e, st)));
+    LSP_STAGE(ST_DGRAD_O, 1, (gemm1<false, true>(ctx, T, Nq, H, Operand{da16, H, false}, Operand{wo16, Nq, true}, e, st)));
   }
   if (d.head_dim == 128) LSP_STAGE(ST_DVEC, 1, attn_dvec_launch<128>(dO16, Nq, o32, Nq, dvec, d.batch, d.seq, d.n_q_heads, st));
   else LSP_STAGE(ST_DVEC, 1, attn_dvec_launch<64>(dO16, Nq, o32, Nq, dvec, d.batch, d.seq, d.n_q_heads, st));
@@ -327,18 +333,14 @@ lsp_status attn_bwd_impl(lsp_ctx* ctx, int x_dt, const void* x, int da_dt, const
   p.dq16 = dqkv; p.dk16 = dqkv + Nq; p.dv16 = dqkv + Nq + Nkv; p.ldd16 = Nqkv;
   if (d.head_dim == 128) LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_launch<128>(p, st));
   else LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_launch<64>(p, st));
-  // B9 dW{q,k,v} = d{q,k,v}^T xn (one GEMM, rows split over three outputs) ; dxn = dq Wq + dk Wk + dv Wv (3 K-segments)
+  // B9 dW{q,k,v} = d{q,k,v}^T xn (one GEMM, rows split over three outputs) ; dxn = [dq|dk|dv] [Wq;Wk;Wv] (one GEMM)
   {
     EpiF32 e = epi_f32(static_cast<float*>(g->wq), H);
     e.out[1] = g->wk; e.out[2] = g->wv; e.split1 = Nq; e.split2 = Nq + Nkv;
     LSP_STAGE(ST_WGRAD_QKV, 1, (gemm1<true, true>(ctx, Nqkv, H, T, Operand{dqkv, Nqkv, true}, Operand{xn, H, true}, e, st)));
   }
-  {
-    const Operand as[3] = {{dqkv, Nqkv, false}, {dqkv + Nq, Nqkv, false}, {dqkv + Nq + Nkv, Nqkv, false}};
-    const Operand bs[3] = {{w->wq, H, true}, {w->wk, H, true}, {w->wv, H, true}};
-    const int ks[3] = {Nq, Nkv, Nkv};
-    LSP_STAGE(ST_DGRAD_QKV, 1, (gemm_run<BN_MAIN, false, true>(T, H, 3, as, bs, ks, epi_f32(dxn, H), ctx->num_sms, st)));
-  }
+  LSP_STAGE(ST_DGRAD_QKV, 1, (gemm1<false, true>(ctx, T, H, Nqkv, Operand{dqkv, Nqkv, false}, Operand{wqkv16, H, true},
+                               epi_f32(dxn, H), st)));
   // B10 RMSNorm-1 backward + residual gradient
   LSP_STAGE(ST_NORM_BWD, 2, norm_bwd(ctx, x_dt, da_dt, x, rstd1, w->g_attn, dxn, da, dx, nullptr, dgpart, static_cast<float*>(g->g_attn), st));
   return LSP_OK;
@@ -349,31 +351,39 @@ lsp_status attn_bwd_impl(lsp_ctx* ctx, int x_dt, const void* x, int da_dt, const
 lsp_status mlp_fwd_impl(lsp_ctx* ctx, int a_dt, const void* a, const lsp_layer_weights* w, float* y, void* saved, cudaStream_t st) {
   const lsp_layer_desc& d = ctx->d;
   const int T = ctx->T, H = d.hidden, F = d.ffn;
-  __nv_bfloat16* an = at<__nv_bfloat16>(saved, ctx->sv.an);
+  __half* an = at<__half>(saved, ctx->sv.an);
   float* rstd2 = at<float>(saved, ctx->sv.rstd2);
   __half* g16 = at<__half>(saved, ctx->sv.g16);
   __half* u16 = at<__half>(saved, ctx->sv.u16);
-  __nv_bfloat16* h = at<__nv_bfloat16>(saved, ctx->sv.h);
+  __half* h = at<__half>(saved, ctx->sv.h);
+  __half* wgu16 = at<__half>(saved, ctx->sv.wgu16);
+  __half* wd16 = at<__half>(saved, ctx->sv.wd16);
+  const long long FH = static_cast<long long>(F) * H;
+  LSP_WCAST(w->w_gate, wgu16, FH);
+  LSP_WCAST(w->w_up, wgu16 + FH, FH);
+  LSP_WCAST(w->w_down, wd16, FH);
   LSP_STAGE(ST_NORM_FWD, 1, norm_fwd(ctx, a_dt, a, w->g_mlp, an, rstd2, st));
   EpiSwiGLU e{h, g16, u16, F};
-  LSP_STAGE(ST_GATEUP, 1, gemm_run_dual(T, F, H, Operand{an, H, false}, Operand{w->w_gate, H, false}, Operand{w->w_up, H, false}, e,
+  LSP_STAGE(ST_GATEUP, 1, gemm_run_dual(T, F, H, Operand{an, H, false}, Operand{wgu16, H, false}, Operand{wgu16 + FH, H, false}, e,
                          ctx->num_sms, st));
-  LSP_STAGE(ST_DOWN, 1, gemm_fwd_residual(ctx, h, F, w->w_down, a_dt, a, y, st));
+  LSP_STAGE(ST_DOWN, 1, gemm_fwd_residual(ctx, h, F, wd16, a_dt, a, y, st));
   return LSP_OK;
 }
 
-// dy (dy_dt; dy16 = bf16 copy or itself) -> da fp32 (+ bf16 copy da16 if non-null).  SURVEY 8(a) B1-B5.
-lsp_status mlp_bwd_impl(lsp_ctx* ctx, int a_dt, const void* a, int dy_dt, const void* dy, const __nv_bfloat16* dy16,
-                        const lsp_layer_weights* w, const void* saved, float* da, __nv_bfloat16* da16, lsp_layer_wgrads* g,
+// dy (dy_dt; dy16 = its fp16 copy) -> da fp32 (+ fp16 copy da16 if non-null).  SURVEY 8(a) B1-B5.
+lsp_status mlp_bwd_impl(lsp_ctx* ctx, int a_dt, const void* a, int dy_dt, const void* dy, const __half* dy16,
+                        const lsp_layer_weights* w, const void* saved, float* da, __half* da16, lsp_layer_wgrads* g,
                         void* ws, cudaStream_t st) {
   const lsp_layer_desc& d = ctx->d;
   const int T = ctx->T, H = d.hidden, F = d.ffn;
-  const __nv_bfloat16* an = at<__nv_bfloat16>(saved, ctx->sv.an);
+  const __half* an = at<__half>(saved, ctx->sv.an);
   const float* rstd2 = at<float>(saved, ctx->sv.rstd2);
   const __half* g16 = at<__half>(saved, ctx->sv.g16);
   const __half* u16 = at<__half>(saved, ctx->sv.u16);
-  const __nv_bfloat16* h = at<__nv_bfloat16>(saved, ctx->sv.h);
-  __nv_bfloat16* dgu = at<__nv_bfloat16>(ws, ctx->ws.dgu);
+  const __half* h = at<__half>(saved, ctx->sv.h);
+  const __half* wgu16 = at<__half>(saved, ctx->sv.wgu16);
+  const __half* wd16 = at<__half>(saved, ctx->sv.wd16);
+  __half* dgu = at<__half>(ws, ctx->ws.dgu);
   float* dan = at<float>(ws, ctx->ws.dn32);
   float* dgpart = at<float>(ws, ctx->ws.dgpart);
 
@@ -382,7 +392,7 @@ lsp_status mlp_bwd_impl(lsp_ctx* ctx, int a_dt, const void* a, int dy_dt, const 
   // B1 dh = dy Wd with the SwiGLU-backward epilogue -> [dg | du]
   {
     EpiSwiGLUBwd e{g16, u16, F, dgu, F};
-    LSP_STAGE(ST_DGRAD_DOWN, 1, (gemm1<false, true>(ctx, T, F, H, Operand{dy16, H, false}, Operand{w->w_down, F, true}, e, st)));
+    LSP_STAGE(ST_DGRAD_DOWN, 1, (gemm1<false, true>(ctx, T, F, H, Operand{dy16, H, false}, Operand{wd16, F, true}, e, st)));
   }
   // B4 dWg = dg^T an, dWu = du^T an (one GEMM over the 2F rows of [dg | du]^T)
   {
@@ -390,13 +400,9 @@ lsp_status mlp_bwd_impl(lsp_ctx* ctx, int a_dt, const void* a, int dy_dt, const 
     e.out[1] = g->w_up; e.split1 = F;
     LSP_STAGE(ST_WGRAD_GATEUP, 1, (gemm1<true, true>(ctx, 2 * F, H, T, Operand{dgu, 2LL * F, true}, Operand{an, H, true}, e, st)));
   }
-  // B3 dan = dg Wg + du Wu (two K-segments)
-  {
-    const Operand as[2] = {{dgu, 2LL * F, false}, {dgu + F, 2LL * F, false}};
-    const Operand bs[2] = {{w->w_gate, H, true}, {w->w_up, H, true}};
-    const int ks[2] = {F, F};
-    LSP_STAGE(ST_DGRAD_GATEUP, 1, (gemm_run<BN_MAIN, false, true>(T, H, 2, as, bs, ks, epi_f32(dan, H), ctx->num_sms, st)));
-  }
+  // B3 dan = [dg | du] [Wg; Wu]  (one GEMM, K = 2F)
+  LSP_STAGE(ST_DGRAD_GATEUP, 1, (gemm1<false, true>(ctx, T, H, 2 * F, Operand{dgu, 2LL * F, false}, Operand{wgu16, H, true},
+                                  epi_f32(dan, H), st)));
   // B5 RMSNorm-2 backward + residual gradient
   LSP_STAGE(ST_NORM_BWD, 2, norm_bwd(ctx, a_dt, dy_dt, a, rstd2, w->g_mlp, dan, dy, da, da16, dgpart, static_cast<float*>(g->g_mlp), st));
   return LSP_OK;
@@ -413,11 +419,12 @@ lsp_status check_common(lsp_ctx* ctx, const void* saved, const void* ws, int n, 
   return LSP_OK;
 }
 
-// bf16 view of an activation-gradient input: the tensor itself if it is bf16, else a cast into ws.in16
-lsp_status as_bf16(lsp_ctx* ctx, const void* in, void* ws, cudaStream_t st, const __nv_bfloat16** out) {
-  if (ctx->d.in_dtype == LSP_BF16) { *out = static_cast<const __nv_bfloat16*>(in); return LSP_OK; }
-  __nv_bfloat16* t = at<__nv_bfloat16>(ws, ctx->ws.in16);
-  LSP_STAGE(ST_CAST, 1, cast_f32_bf16(static_cast<const float*>(in), t, static_cast<long long>(ctx->T) * ctx->d.hidden, ctx->num_sms, st));
+// fp16 operand copy of an activation-gradient input (bf16: exact for normal-range values; fp32: rounded), in ws.in16
+lsp_status as_f16(lsp_ctx* ctx, const void* in, void* ws, cudaStream_t st, const __half** out) {
+  __half* t = at<__half>(ws, ctx->ws.in16);
+  const long long n = static_cast<long long>(ctx->T) * ctx->d.hidden;
+  if (ctx->d.in_dtype == LSP_BF16) LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(in), t, n, ctx->num_sms, st));
+  else LSP_STAGE(ST_CAST, 1, cast_f32_f16(static_cast<const float*>(in), t, n, ctx->num_sms, st));
   *out = t;
   return LSP_OK;
 }
@@ -508,8 +515,8 @@ lsp_status lsp_attn_bwd(lsp_ctx* ctx, const void* x, const void* da, const lsp_l
   const void* ptrs[] = {x, da, saved, dx, ws, w->wq, w->wk, w->wv, w->wo, w->g_attn, g->wq, g->wk, g->wv, g->wo, g->g_attn};
   LSP_TRY(check_common(ctx, saved, ws, 15, ptrs));
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  const __nv_bfloat16* da16;
-  LSP_TRY(as_bf16(ctx, da, ws, st, &da16));
+  const __half* da16;
+  LSP_TRY(as_f16(ctx, da, ws, st, &da16));
   return attn_bwd_impl(ctx, ctx->d.in_dtype, x, ctx->d.in_dtype, da, da16, w, saved, static_cast<float*>(dx), g, ws, st);
 }
 
@@ -526,8 +533,8 @@ lsp_status lsp_mlp_bwd(lsp_ctx* ctx, const void* a, const void* dy, const lsp_la
   const void* ptrs[] = {a, dy, saved, da, ws, w->w_gate, w->w_up, w->w_down, w->g_mlp, g->w_gate, g->w_up, g->w_down, g->g_mlp};
   LSP_TRY(check_common(ctx, saved, ws, 13, ptrs));
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  const __nv_bfloat16* dy16;
-  LSP_TRY(as_bf16(ctx, dy, ws, st, &dy16));
+  const __half* dy16;
+  LSP_TRY(as_f16(ctx, dy, ws, st, &dy16));
   return mlp_bwd_impl(ctx, ctx->d.in_dtype, a, ctx->d.in_dtype, dy, dy16, w, saved, static_cast<float*>(da), nullptr, g, ws, st);
 }
 
@@ -548,11 +555,11 @@ lsp_status lsp_layer_bwd(lsp_ctx* ctx, const void* x, const void* dy, const lsp_
                         g->wq, g->wk, g->wv, g->wo, g->g_attn, g->w_gate, g->w_up, g->w_down, g->g_mlp};
   LSP_TRY(check_common(ctx, saved, ws, 23, ptrs));
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  const __nv_bfloat16* dy16;
-  LSP_TRY(as_bf16(ctx, dy, ws, st, &dy16));
+  const __half* dy16;
+  LSP_TRY(as_f16(ctx, dy, ws, st, &dy16));
   const float* a32 = at<float>(saved, ctx->sv.a32);
   float* da32 = at<float>(ws, ctx->ws.da32);
-  __nv_bfloat16* da16 = at<__nv_bfloat16>(ws, ctx->ws.da16);
+  __half* da16 = at<__half>(ws, ctx->ws.da16);
   LSP_TRY(mlp_bwd_impl(ctx, LSP_F32, a32, ctx->d.in_dtype, dy, dy16, w, saved, da32, da16, g, ws, st));
   return attn_bwd_impl(ctx, ctx->d.in_dtype, x, LSP_F32, da32, da16, w, saved, static_cast<float*>(dx), g, ws, st);
 }
@@ -630,18 +637,23 @@ lsp_status lsp_embed_fwd(lsp_ctx* ctx, const int32_t* ids, const void* table, vo
   return LSP_OK;
 }
 
-lsp_status lsp_gemm(lsp_ctx* ctx, int op, int M, int N, int K, const void* A, int64_t lda, const void* B, int64_t ldb,
-                    float* C, int64_t ldc, void* stream) {
+lsp_status lsp_gemm(lsp_ctx* ctx, int op, int M, int N, int K, const void* A, int64_t lda, int a_dtype, const void* B,
+                    int64_t ldb, int b_dtype, float* C, int64_t ldc, void* stream) {
   if (!ctx) return LSP_EINVAL;
   const void* ptrs[] = {A, B, C};
   LSP_TRY(check_common(ctx, nullptr, nullptr, 3, ptrs));
   if (M <= 0 || N <= 0 || K <= 0 || (lda % 8) || (ldb % 8) || (ldc % 8) || (N % 8)) return fail(ctx, LSP_EINVAL, "lsp_gemm: bad extents/pitches");
+  if ((a_dtype != LSP_BF16 && a_dtype != LSP_F16) || (b_dtype != LSP_BF16 && b_dtype != LSP_F16))
+    return fail(ctx, LSP_EINVAL, "lsp_gemm: operand dtype must be LSP_BF16 or LSP_F16");
+  if (a_dtype != b_dtype)       // tcgen05.mma.kind::f16 with unequal A/B formats faults on sm_100a (measured)
+    return fail(ctx, LSP_EUNSUPPORTED, "lsp_gemm: A and B must have the same 16-bit format");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const EpiF32 e = epi_f32(C, ldc);
+  const int adt = a_dtype == LSP_F16 ? DT_F16 : DT_BF16, bdt = b_dtype == LSP_F16 ? DT_F16 : DT_BF16;
   switch (op) {
-    case 0: LSP_STAGE(ST_OPROJ, 1, (gemm1<false, false>(ctx, M, N, K, Operand{A, lda, false}, Operand{B, ldb, false}, e, st))); break;
-    case 1: LSP_STAGE(ST_DGRAD_O, 1, (gemm1<false, true>(ctx, M, N, K, Operand{A, lda, false}, Operand{B, ldb, true}, e, st))); break;
-    case 2: LSP_STAGE(ST_WGRAD_O, 1, (gemm1<true, true>(ctx, M, N, K, Operand{A, lda, true}, Operand{B, ldb, true}, e, st))); break;
+    case 0: LSP_STAGE(ST_OPROJ, 1, (gemm1<false, false>(ctx, M, N, K, Operand{A, lda, false, adt}, Operand{B, ldb, false, bdt}, e, st))); break;
+    case 1: LSP_STAGE(ST_DGRAD_O, 1, (gemm1<false, true>(ctx, M, N, K, Operand{A, lda, false, adt}, Operand{B, ldb, true, bdt}, e, st))); break;
+    case 2: LSP_STAGE(ST_WGRAD_O, 1, (gemm1<true, true>(ctx, M, N, K, Operand{A, lda, true, adt}, Operand{B, ldb, true, bdt}, e, st))); break;
     default: return fail(ctx, LSP_EINVAL, "lsp_gemm: op must be 0, 1 or 2");
   }
   return LSP_OK;

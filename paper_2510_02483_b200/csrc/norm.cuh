@@ -22,6 +22,9 @@ template <> struct Vec4<__nv_bfloat16> {
 __device__ __forceinline__ void store_bf16x4(__nv_bfloat16* p, float4 v) {
   *reinterpret_cast<uint2*>(p) = make_uint2(pack_bf16(v.x, v.y), pack_bf16(v.z, v.w));
 }
+__device__ __forceinline__ void store_f16x4(__half* p, float4 v) {
+  *reinterpret_cast<uint2*>(p) = make_uint2(pack_f16(v.x, v.y), pack_f16(v.z, v.w));
+}
 
 __device__ __forceinline__ float block_sum(float v, float* red) {
 #pragma unroll
@@ -36,10 +39,10 @@ __device__ __forceinline__ float block_sum(float v, float* red) {
   return __shfl_sync(0xffffffffu, t, 0);
 }
 
-// xn = x * rsqrt(mean(x^2) + eps) * g  (bf16 out), rstd saved in fp32.  One block per token row.
+// xn = x * rsqrt(mean(x^2) + eps) * g  (fp16 out: the GEMM operand), rstd saved in fp32.  One block per token row.
 template <typename XT, int NV>
 __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_fwd_kernel(const XT* __restrict__ x, const __nv_bfloat16* __restrict__ g,
-                                                                   __nv_bfloat16* __restrict__ xn, float* __restrict__ rstd,
+                                                                   __half* __restrict__ xn, float* __restrict__ rstd,
                                                                    int H, float eps) {
   __shared__ float red[NORM_THREADS / 32];
   const long long row = blockIdx.x;
@@ -62,7 +65,7 @@ __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_fwd_kernel(const XT* __r
     const int c = (threadIdx.x + i * NORM_THREADS) * 4;
     if (c < H) {
       const float4 gg = Vec4<__nv_bfloat16>::load(g + c);
-      store_bf16x4(xn + row * H + c, make_float4(v[i].x * r * gg.x, v[i].y * r * gg.y, v[i].z * r * gg.z, v[i].w * r * gg.w));
+      store_f16x4(xn + row * H + c, make_float4(v[i].x * r * gg.x, v[i].y * r * gg.y, v[i].z * r * gg.z, v[i].w * r * gg.w));
     }
   }
 }
@@ -73,7 +76,7 @@ template <typename XT, typename RT, int NV>
 __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd,
                                                                    const __nv_bfloat16* __restrict__ g,
                                                                    const float* __restrict__ dxn, const RT* __restrict__ dres,
-                                                                   float* __restrict__ dx, __nv_bfloat16* __restrict__ dx16,
+                                                                   float* __restrict__ dx, __half* __restrict__ dx16,
                                                                    float* __restrict__ dg_part, int T, int H) {
   __shared__ float red[NORM_THREADS / 32];
   float4 gg[NV], acc[NV];
@@ -112,7 +115,7 @@ __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_bwd_kernel(const XT* __r
         o.z = rs.z + r * (dn[i].z - n[i].z * dot);
         o.w = rs.w + r * (dn[i].w - n[i].w * dot);
         *reinterpret_cast<float4*>(dx + row * H + c) = o;
-        if (dx16) store_bf16x4(dx16 + row * H + c, o);
+        if (dx16) store_f16x4(dx16 + row * H + c, o);
       }
     }
   }
@@ -133,10 +136,10 @@ __global__ void colsum_kernel(const float* __restrict__ part, float* __restrict_
 }
 
 // 8 elements per thread casts (n is a multiple of 8)
-__global__ void cast_f32_bf16_kernel(const float* __restrict__ in, __nv_bfloat16* __restrict__ out, long long n8) {
+__global__ void cast_f32_f16_kernel(const float* __restrict__ in, __half* __restrict__ out, long long n8) {
   for (long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i < n8; i += static_cast<long long>(gridDim.x) * blockDim.x) {
     const float4 a = __ldg(reinterpret_cast<const float4*>(in) + 2 * i), b = __ldg(reinterpret_cast<const float4*>(in) + 2 * i + 1);
-    reinterpret_cast<uint4*>(out)[i] = make_uint4(pack_bf16(a.x, a.y), pack_bf16(a.z, a.w), pack_bf16(b.x, b.y), pack_bf16(b.z, b.w));
+    reinterpret_cast<uint4*>(out)[i] = make_uint4(pack_f16(a.x, a.y), pack_f16(a.z, a.w), pack_f16(b.x, b.y), pack_f16(b.z, b.w));
   }
 }
 __global__ void cast_bf16_f16_kernel(const __nv_bfloat16* __restrict__ in, __half* __restrict__ out, long long n8) {
