@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "attn.cuh"
+#include "attn_tc.cuh"
 #include "gemm.cuh"
 #include "norm.cuh"
 
@@ -248,6 +249,17 @@ cudaError_t gemm_fwd_residual(const lsp_ctx* c, const __half* A, int K, const __
 #define LSP_WCAST(src, dst, n) \
   LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(src), dst, static_cast<long long>(n), ctx->num_sms, st))
 
+// F3 dispatch: head_dim 128 runs on tcgen05 (attn_tc.cuh); head_dim 64 on the mma.sync kernel (attn.cuh).
+cudaError_t attn_fwd_dispatch(const lsp_ctx* c, const AttnParams& p, cudaStream_t st) {
+  if (c->d.head_dim == 128) {
+    AttnTcParams t;
+    t.B = p.B; t.S = p.S; t.nq = p.nq; t.nkv = p.nkv; t.scale_log2 = p.scale_log2; t.scale = p.scale;
+    t.o32 = p.o32; t.o16 = p.o16; t.ldo = p.ldo; t.lse = p.lse;
+    return attn_fwd_tc_launch(p.q, p.ldq, p.k, p.ldk, p.v, p.ldv, t, st);
+  }
+  return attn_fwd_launch<64>(p, st);
+}
+
 // ------------------------------------------------------------------------------------------- attention block
 // x [T,H] x_dt -> a32 [T,H] fp32.  SURVEY 8(a) F1-F4.
 lsp_status attn_fwd_impl(lsp_ctx* ctx, int x_dt, const void* x, const lsp_layer_weights* w, float* a_out, void* saved,
@@ -283,8 +295,7 @@ lsp_status attn_fwd_impl(lsp_ctx* ctx, int x_dt, const void* x, const lsp_layer_
   p.scale = 1.0f / sqrtf(static_cast<float>(d.head_dim));
   p.scale_log2 = p.scale * 1.4426950408889634f;
   p.o32 = o32; p.o16 = o16; p.ldo = Nq; p.lse = lse;
-  if (d.head_dim == 128) LSP_STAGE(ST_ATTN_FWD, 1, attn_fwd_launch<128>(p, st));
-  else LSP_STAGE(ST_ATTN_FWD, 1, attn_fwd_launch<64>(p, st));
+  LSP_STAGE(ST_ATTN_FWD, 1, attn_fwd_dispatch(ctx, p, st));
   // F4 O-projection + residual
   LSP_STAGE(ST_OPROJ, 1, gemm_fwd_residual(ctx, o16, Nq, wo16, x_dt, x, a_out, st));
   return LSP_OK;
@@ -585,8 +596,7 @@ lsp_status lsp_sdpa_fwd(lsp_ctx* ctx, const void* q, const void* k, const void* 
   p.scale = 1.0f / sqrtf(static_cast<float>(d.head_dim));
   p.scale_log2 = p.scale * 1.4426950408889634f;
   p.o32 = static_cast<float*>(o); p.ldo = ctx->Nq; p.lse = lse;
-  if (d.head_dim == 128) LSP_STAGE(ST_ATTN_FWD, 1, attn_fwd_launch<128>(p, st));
-  else LSP_STAGE(ST_ATTN_FWD, 1, attn_fwd_launch<64>(p, st));
+  LSP_STAGE(ST_ATTN_FWD, 1, attn_fwd_dispatch(ctx, p, st));
   return LSP_OK;
 }
 
