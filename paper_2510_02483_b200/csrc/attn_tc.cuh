@@ -38,13 +38,13 @@ constexpr int ATC_FWD_THREADS = 320;
 constexpr int ATC_FWD_SMEM = 6 * ATC_TILE_BYTES + 1024 + 256;
 constexpr float ATC_RESCALE_LOG2 = 8.0f;
 
-// 3-D map over a [B*S, ld] fp16 matrix seen as (column, position, batch); box = 64 columns x 128 positions.
-inline bool make_map_attn(CUtensorMap* m, const void* base, int ncols, int S, int B, long long ld) {
+// 3-D map over a [B*S, ld] fp16 matrix seen as (column, position, batch); box = 64 columns x box_rows positions.
+inline bool make_map_attn(CUtensorMap* m, const void* base, int ncols, int S, int B, long long ld, int box_rows = 128) {
   PFN_encodeTiled fn = get_encode_fn();
   if (!fn) return false;
   cuuint64_t dims[3] = {static_cast<cuuint64_t>(ncols), static_cast<cuuint64_t>(S), static_cast<cuuint64_t>(B)};
   cuuint64_t strides[2] = {static_cast<cuuint64_t>(ld) * 2, static_cast<cuuint64_t>(ld) * 2 * static_cast<cuuint64_t>(S)};
-  cuuint32_t box[3] = {64u, 128u, 1u};
+  cuuint32_t box[3] = {64u, static_cast<cuuint32_t>(box_rows), 1u};
   cuuint32_t estr[3] = {1u, 1u, 1u};
   return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -306,6 +306,449 @@ inline cudaError_t attn_fwd_tc_launch(const __half* q, long long ldq, const __ha
   maps.dO = maps.q;
   dim3 grid((p.S + 255) / 256, p.nq, p.B);
   attn_fwd_tc_kernel<<<grid, ATC_FWD_THREADS, ATC_FWD_SMEM, st>>>(maps, p);
+  return cudaGetLastError();
+}
+
+// =========================================================================================== backward
+// SURVEY 8(a) B7 (+B8 on store).  Two deterministic kernels, no atomics (results are bit-reproducible):
+//   dK/dV : one CTA per (128-key block, kv head, batch) walks the G query heads of the group and the 64-query
+//           blocks at / below the diagonal, in the transposed domain (TMEM lane = key):
+//             S^T = K Q^T, dP^T = V dO^T          (A = K, V K-major from smem; B = Q, dO K-major)
+//             P^T = exp2(S^T c - L log2e)         (softmax threads; fp16 -> TMEM over S^T)
+//             dV += P^T dO                        (A = P^T from TMEM; B = dO MN-major: the same smem tile)
+//             dS^T = P^T (dP^T - D)               (fp16 -> TMEM over dP^T)
+//             dK += dS^T Q                        (A = dS^T from TMEM; B = Q MN-major)
+//           dK, dV accumulate in TMEM over the whole walk (the GQA group sum costs nothing).
+//   dQ    : one CTA per (128-query block, head, batch) walks the 64-key blocks up to the diagonal:
+//             S = Q K^T, dP = dO V^T, dS = exp2(S c - L log2e)(dP - D) -> TMEM, dQ += dS K (K MN-major).
+// Both double-buffer the 64-column S / dP accumulators so the tensor core computes block i+1 while the 256
+// softmax threads (8 warps: TMEM lane quarter x column half) work on block i.
+// TMEM: [0,64) [64,128) S buffers, [128,192) [192,256) dP buffers, [256,384) dV or dQ, [384,512) dK.
+// The 16-bit operand written back over a 64-column fp32 buffer keeps each half inside the columns its own warp
+// read (keys/queries 0..31 -> columns 0..15, 32..63 -> columns 32..47), so the two half-warps never race.
+constexpr int ATC_BWD_THREADS = 320;
+constexpr int ATC_NST = 3;                                 // stages of the streamed 64-row tiles
+constexpr int ATC_HALF_TILE = 64 * ATC_D * 2;              // 64 x 128 fp16 = 16 KB (two 8 KB chunks)
+constexpr int ATC_BWD_SMEM = 2 * ATC_TILE_BYTES + 2 * ATC_NST * ATC_HALF_TILE + ATC_NST * 2 * 64 * 4 + 1024 + 256;
+
+struct AttnTcBwdParams {
+  int B, S, nq, nkv;
+  float scale_log2, scale;
+  const float* lse;            // [B, nq, S]
+  const float* dvec;           // [B, nq, S]
+  const float2* rope;          // (cos, sin) [S, 64] or null: inverse rotation of dq, dk on store
+  float* dq32; float* dk32; float* dv32; long long lddq32, lddk32;
+  __half* dq16; __half* dk16; __half* dv16; long long ldd16;
+};
+
+__device__ __forceinline__ void atc_load_half_tile(uint32_t dst, const CUtensorMap* m, uint32_t bar, int col0, int s0, int b) {
+  mbar_expect_tx(bar, ATC_HALF_TILE);
+  tma_load_3d(dst, m, bar, col0, s0, b);
+  tma_load_3d(dst + 64 * 128, m, bar, col0 + 64, s0, b);
+}
+// 64-row tile (two 8 KB chunks) as a K-major B operand (N = 64 rows, K = 128 contiguous): kk-th 16-element K step
+__device__ __forceinline__ uint64_t atc_desc_half_kmajor(uint32_t tile, int kk) {
+  return umma_smem_desc(tile + (kk >> 2) * (64 * 128) + (kk & 3) * 32, 16, 1024);
+}
+// the same tile as an MN-major B operand (K = 64 rows, N = 128 contiguous): kk-th 16-row K step
+__device__ __forceinline__ uint64_t atc_desc_half_mnmajor(uint32_t tile, int kk) {
+  return umma_smem_desc(tile + kk * 2048, 64 * 128, 1024);
+}
+// TMEM column of the kk-th 16-element K step of a 64-wide fp16 operand stored as described above
+__device__ __forceinline__ uint32_t atc_half_operand_col(int kk) { return static_cast<uint32_t>((kk >> 1) * 32 + (kk & 1) * 8); }
+
+// Scale, optionally rotate by -theta (transpose of the forward rotation), and store 32 columns of one row.
+__device__ __forceinline__ void atc_store_grad32(float (&v)[32], float scale, const float2* rope_row, float* o32, __half* o16) {
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    float z0 = v[2 * i] * scale, z1 = v[2 * i + 1] * scale;
+    if (rope_row) {
+      const float2 cs = __ldg(rope_row + i);
+      const float r0 = z0 * cs.x + z1 * cs.y, r1 = -z0 * cs.y + z1 * cs.x;
+      z0 = r0; z1 = r1;
+    }
+    v[2 * i] = z0; v[2 * i + 1] = z1;
+  }
+  if (o32) store_row32<DT_F32>(o32, v, 32);
+  if (o16) store_row32<DT_F16>(o16, v, 32);
+}
+
+// --------------------------------------------------------------------------------------------- dK, dV
+__global__ void __launch_bounds__(ATC_BWD_THREADS, 1)
+attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sK = smem_base, sV = sK + ATC_TILE_BYTES;
+  const uint32_t sQ = sV + ATC_TILE_BYTES;                       // ATC_NST stages of 64 x 128
+  const uint32_t sDO = sQ + ATC_NST * ATC_HALF_TILE;
+  const uint32_t sLD = sDO + ATC_NST * ATC_HALF_TILE;            // [stage][L*log2e (64) | D (64)] fp32
+  const uint32_t bar_base = sLD + ATC_NST * 2 * 64 * 4;
+  float* sLD_ptr = reinterpret_cast<float*>(smem_raw + (sLD - smem_u32(smem_raw)));
+  auto kv_full = [&]() { return bar_base; };
+  auto acc_full = [&]() { return bar_base + 8u; };
+  auto qdo_full = [&](int s) { return bar_base + 8u * (2 + s); };
+  auto qdo_empty = [&](int s) { return bar_base + 8u * (2 + ATC_NST + s); };
+  auto ld_full = [&](int s) { return bar_base + 8u * (2 + 2 * ATC_NST + s); };
+  auto sdp_full = [&](int s) { return bar_base + 8u * (2 + 3 * ATC_NST + s); };
+  auto p_full = [&](int s) { return bar_base + 8u * (4 + 3 * ATC_NST + s); };
+  auto ds_full = [&](int s) { return bar_base + 8u * (6 + 3 * ATC_NST + s); };
+  const uint32_t tmem_slot = bar_base + 8u * (8 + 3 * ATC_NST);
+  uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int kb = blockIdx.x, kvh = blockIdx.y, b = blockIdx.z;
+  const int G = p.nq / p.nkv;
+  const int k0 = kb * 128;
+  const int nq64 = (p.S + 63) / 64;
+  const int per_head = nq64 - 2 * kb;                            // 64-query blocks at / below the diagonal
+  const int iters = per_head * G;
+
+  if (threadIdx.x == 0) {
+    tma_prefetch_desc(&maps.q); tma_prefetch_desc(&maps.k); tma_prefetch_desc(&maps.v); tma_prefetch_desc(&maps.dO);
+    mbar_init(kv_full(), 1); mbar_init(acc_full(), 1);
+    for (int i = 0; i < ATC_NST; ++i) { mbar_init(qdo_full(i), 1); mbar_init(qdo_empty(i), 1); mbar_init(ld_full(i), 32); }
+    for (int i = 0; i < 2; ++i) { mbar_init(sdp_full(i), 1); mbar_init(p_full(i), 8); mbar_init(ds_full(i), 8); }
+    fence_barrier_init();
+  }
+  if (warp == 1) { tmem_alloc(tmem_slot, 512); tmem_relinquish(); }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot_ptr;
+
+  if (warp == 0) {
+    // ===================================================================== producer: TMA tiles + L, D vectors
+    if (lane == 0) {
+      mbar_expect_tx(kv_full(), 2 * ATC_TILE_BYTES);
+      tma_load_3d(sK, &maps.k, kv_full(), kvh * ATC_D, k0, b);
+      tma_load_3d(sK + ATC_CHUNK_BYTES, &maps.k, kv_full(), kvh * ATC_D + 64, k0, b);
+      tma_load_3d(sV, &maps.v, kv_full(), kvh * ATC_D, k0, b);
+      tma_load_3d(sV + ATC_CHUNK_BYTES, &maps.v, kv_full(), kvh * ATC_D + 64, k0, b);
+    }
+    for (int it = 0; it < iters; ++it) {
+      const int st = it % ATC_NST;
+      const int hh = kvh * G + it / per_head;
+      const int s0 = (2 * kb + it % per_head) * 64;
+      mbar_wait(qdo_empty(st), ((it / ATC_NST) & 1) ^ 1u);
+      if (lane == 0) {
+        mbar_expect_tx(qdo_full(st), 2 * ATC_HALF_TILE);
+        tma_load_3d(sQ + st * ATC_HALF_TILE, &maps.q, qdo_full(st), hh * ATC_D, s0, b);
+        tma_load_3d(sQ + st * ATC_HALF_TILE + 64 * 128, &maps.q, qdo_full(st), hh * ATC_D + 64, s0, b);
+        tma_load_3d(sDO + st * ATC_HALF_TILE, &maps.dO, qdo_full(st), hh * ATC_D, s0, b);
+        tma_load_3d(sDO + st * ATC_HALF_TILE + 64 * 128, &maps.dO, qdo_full(st), hh * ATC_D + 64, s0, b);
+      }
+      const long long vbase = (static_cast<long long>(b) * p.nq + hh) * p.S;
+#pragma unroll
+      for (int r = 0; r < 2; ++r) {
+        const int s = s0 + lane + 32 * r;
+        const bool ok = s < p.S;
+        sLD_ptr[st * 128 + lane + 32 * r] = ok ? p.lse[vbase + s] * 1.4426950408889634f : INFINITY;
+        sLD_ptr[st * 128 + 64 + lane + 32 * r] = ok ? p.dvec[vbase + s] : 0.f;
+      }
+      mbar_arrive(ld_full(st));
+    }
+  } else if (warp == 1) {
+    // ===================================================================== MMA issuer
+    if (lane == 0) {
+      const uint32_t idesc_sdp = umma_idesc(128, 64, 0, 0, 0, 0);     // [128 keys x 64 queries] = A(K-major) B(K-major)^T
+      const uint32_t idesc_acc = umma_idesc(128, 128, 0, 0, 0, 1);    // [128 keys x 128 d] += A(TMEM) B(MN-major)
+      auto issue_sdp = [&](int it) {
+        const int st = it % ATC_NST, buf = it & 1;
+        mbar_wait(qdo_full(st), (it / ATC_NST) & 1);
+        tc_fence_after();
+        const uint32_t qa = sQ + st * ATC_HALF_TILE, da = sDO + st * ATC_HALF_TILE;
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk)
+          umma_f16(tmem_base + buf * 64, atc_desc_kmajor(sK, kk), atc_desc_half_kmajor(qa, kk), idesc_sdp, kk != 0 ? 1u : 0u);
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk)
+          umma_f16(tmem_base + 128 + buf * 64, atc_desc_kmajor(sV, kk), atc_desc_half_kmajor(da, kk), idesc_sdp, kk != 0 ? 1u : 0u);
+        umma_commit(sdp_full(buf));
+      };
+      mbar_wait(kv_full(), 0);
+      issue_sdp(0);
+      for (int it = 0; it < iters; ++it) {
+        const int st = it % ATC_NST, buf = it & 1;
+        const uint32_t ph = (it >> 1) & 1;
+        if (it + 1 < iters) issue_sdp(it + 1);
+        const uint32_t qa = sQ + st * ATC_HALF_TILE, da = sDO + st * ATC_HALF_TILE;
+        mbar_wait(p_full(buf), ph);
+        tc_fence_after();
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk)                                // dV += P^T dO
+          umma_f16_ts(tmem_base + 256, tmem_base + buf * 64 + atc_half_operand_col(kk), atc_desc_half_mnmajor(da, kk), idesc_acc,
+                      (it | kk) != 0 ? 1u : 0u);
+        mbar_wait(ds_full(buf), ph);
+        tc_fence_after();
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk)                                // dK += dS^T Q
+          umma_f16_ts(tmem_base + 384, tmem_base + 128 + buf * 64 + atc_half_operand_col(kk), atc_desc_half_mnmajor(qa, kk),
+                      idesc_acc, (it | kk) != 0 ? 1u : 0u);
+        umma_commit(qdo_empty(st));
+      }
+      umma_commit(acc_full());
+    }
+  } else {
+    // ===================================================================== softmax warps (8): lane quarter x column half
+    const int quarter = warp & 3, half = (warp - 2) >> 2;
+    const int row = quarter * 32 + lane;                               // key within the block = TMEM lane
+    const uint32_t lane_off = static_cast<uint32_t>(quarter * 32) << 16;
+    const int col0 = half * 32;
+    const float c = p.scale_log2;
+    for (int it = 0; it < iters; ++it) {
+      const int st = it % ATC_NST, buf = it & 1;
+      const int rel = it % per_head;                                   // 64-query block index relative to the diagonal
+      mbar_wait(ld_full(st), (it / ATC_NST) & 1);
+      mbar_wait(sdp_full(buf), (it >> 1) & 1);
+      tc_fence_after();
+      uint32_t sr[32], dr[32];
+      tmem_ld32(tmem_base + lane_off + buf * 64 + col0, sr);
+      tmem_ld32(tmem_base + lane_off + 128 + buf * 64 + col0, dr);
+      tmem_ld_wait();
+      const float4* l4 = reinterpret_cast<const float4*>(sLD_ptr + st * 128 + col0);
+      const float4* d4 = reinterpret_cast<const float4*>(sLD_ptr + st * 128 + 64 + col0);
+      float pv[32];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const float4 L = l4[i];
+        pv[4 * i] = exp2f(fmaf(__uint_as_float(sr[4 * i]), c, -L.x));
+        pv[4 * i + 1] = exp2f(fmaf(__uint_as_float(sr[4 * i + 1]), c, -L.y));
+        pv[4 * i + 2] = exp2f(fmaf(__uint_as_float(sr[4 * i + 2]), c, -L.z));
+        pv[4 * i + 3] = exp2f(fmaf(__uint_as_float(sr[4 * i + 3]), c, -L.w));
+      }
+      if (rel < 2) {                                                   // diagonal: query (64 rel + col0 + i) < key (row) is masked
+        const int qrel = rel * 64 + col0;
+#pragma unroll
+        for (int i = 0; i < 32; ++i)
+          if (qrel + i < row) pv[i] = 0.f;
+      }
+      uint32_t pk[16];
+#pragma unroll
+      for (int i = 0; i < 16; ++i) pk[i] = pack_f16(pv[2 * i], pv[2 * i + 1]);
+      tmem_st16(tmem_base + lane_off + buf * 64 + col0, pk);
+      tmem_st_wait();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(p_full(buf));
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const float4 Dv = d4[i];
+        pv[4 * i] *= __uint_as_float(dr[4 * i]) - Dv.x;
+        pv[4 * i + 1] *= __uint_as_float(dr[4 * i + 1]) - Dv.y;
+        pv[4 * i + 2] *= __uint_as_float(dr[4 * i + 2]) - Dv.z;
+        pv[4 * i + 3] *= __uint_as_float(dr[4 * i + 3]) - Dv.w;
+      }
+#pragma unroll
+      for (int i = 0; i < 16; ++i) pk[i] = pack_f16(pv[2 * i], pv[2 * i + 1]);
+      tmem_st16(tmem_base + lane_off + 128 + buf * 64 + col0, pk);
+      tmem_st_wait();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(ds_full(buf));
+    }
+    // epilogue: this thread stores columns [64 half, 64 half + 64) of its key row of dV and dK
+    mbar_wait(acc_full(), 0);
+    tc_fence_after();
+    const int key = k0 + row;
+    const bool valid = key < p.S;
+    const long long tok = static_cast<long long>(b) * p.S + key;
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      const int cc = half * 64 + q * 32;
+      uint32_t a[32];
+      tmem_ld32(tmem_base + lane_off + 256 + cc, a);
+      tmem_ld_wait();
+      if (valid)
+        atc_store_grad32(reinterpret_cast<float(&)[32]>(a), 1.0f, nullptr,
+                         p.dv32 ? p.dv32 + tok * p.lddk32 + kvh * ATC_D + cc : nullptr,
+                         p.dv16 ? p.dv16 + tok * p.ldd16 + kvh * ATC_D + cc : nullptr);
+      tmem_ld32(tmem_base + lane_off + 384 + cc, a);
+      tmem_ld_wait();
+      if (valid)
+        atc_store_grad32(reinterpret_cast<float(&)[32]>(a), p.scale, p.rope ? p.rope + static_cast<long long>(key) * 64 + (cc >> 1) : nullptr,
+                         p.dk32 ? p.dk32 + tok * p.lddk32 + kvh * ATC_D + cc : nullptr,
+                         p.dk16 ? p.dk16 + tok * p.ldd16 + kvh * ATC_D + cc : nullptr);
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) { tc_fence_after(); tmem_dealloc(tmem_base, 512); }
+}
+
+// --------------------------------------------------------------------------------------------- dQ
+__global__ void __launch_bounds__(ATC_BWD_THREADS, 1)
+attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t sQ = smem_base, sDO = sQ + ATC_TILE_BYTES;
+  const uint32_t sK = sDO + ATC_TILE_BYTES;                      // ATC_NST stages of 64 keys x 128
+  const uint32_t sV = sK + ATC_NST * ATC_HALF_TILE;
+  const uint32_t bar_base = sV + ATC_NST * ATC_HALF_TILE;
+  auto qdo_full = [&]() { return bar_base; };
+  auto acc_full = [&]() { return bar_base + 8u; };
+  auto kv_full = [&](int s) { return bar_base + 8u * (2 + s); };
+  auto kv_empty = [&](int s) { return bar_base + 8u * (2 + ATC_NST + s); };
+  auto sdp_full = [&](int s) { return bar_base + 8u * (2 + 2 * ATC_NST + s); };
+  auto ds_full = [&](int s) { return bar_base + 8u * (4 + 2 * ATC_NST + s); };
+  const uint32_t tmem_slot = bar_base + 8u * (6 + 2 * ATC_NST);
+  uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int qb = gridDim.x - 1 - blockIdx.x;                     // heavy (late) query blocks first
+  const int h = blockIdx.y, b = blockIdx.z;
+  const int kvh = h / (p.nq / p.nkv);
+  const int q0 = qb * 128;
+  const int kv_end = min(p.S, q0 + 128);
+  const int iters = (kv_end + 63) / 64;                          // 64-key blocks [0, kv_end)
+
+  if (threadIdx.x == 0) {
+    tma_prefetch_desc(&maps.q); tma_prefetch_desc(&maps.k); tma_prefetch_desc(&maps.v); tma_prefetch_desc(&maps.dO);
+    mbar_init(qdo_full(), 1); mbar_init(acc_full(), 1);
+    for (int i = 0; i < ATC_NST; ++i) { mbar_init(kv_full(i), 1); mbar_init(kv_empty(i), 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(sdp_full(i), 1); mbar_init(ds_full(i), 8); }
+    fence_barrier_init();
+  }
+  if (warp == 1) { tmem_alloc(tmem_slot, 512); tmem_relinquish(); }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot_ptr;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      mbar_expect_tx(qdo_full(), 2 * ATC_TILE_BYTES);
+      tma_load_3d(sQ, &maps.q, qdo_full(), h * ATC_D, q0, b);
+      tma_load_3d(sQ + ATC_CHUNK_BYTES, &maps.q, qdo_full(), h * ATC_D + 64, q0, b);
+      tma_load_3d(sDO, &maps.dO, qdo_full(), h * ATC_D, q0, b);
+      tma_load_3d(sDO + ATC_CHUNK_BYTES, &maps.dO, qdo_full(), h * ATC_D + 64, q0, b);
+      for (int it = 0; it < iters; ++it) {
+        const int st = it % ATC_NST;
+        mbar_wait(kv_empty(st), ((it / ATC_NST) & 1) ^ 1u);
+        mbar_expect_tx(kv_full(st), 2 * ATC_HALF_TILE);
+        tma_load_3d(sK + st * ATC_HALF_TILE, &maps.k, kv_full(st), kvh * ATC_D, it * 64, b);
+        tma_load_3d(sK + st * ATC_HALF_TILE + 64 * 128, &maps.k, kv_full(st), kvh * ATC_D + 64, it * 64, b);
+        tma_load_3d(sV + st * ATC_HALF_TILE, &maps.v, kv_full(st), kvh * ATC_D, it * 64, b);
+        tma_load_3d(sV + st * ATC_HALF_TILE + 64 * 128, &maps.v, kv_full(st), kvh * ATC_D + 64, it * 64, b);
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      const uint32_t idesc_sdp = umma_idesc(128, 64, 0, 0, 0, 0);     // [128 queries x 64 keys]
+      const uint32_t idesc_acc = umma_idesc(128, 128, 0, 0, 0, 1);    // dQ [128 x 128] += dS(TMEM) K(MN-major)
+      auto issue_sdp = [&](int it) {
+        const int st = it % ATC_NST, buf = it & 1;
+        mbar_wait(kv_full(st), (it / ATC_NST) & 1);
+        tc_fence_after();
+        const uint32_t ka = sK + st * ATC_HALF_TILE, va = sV + st * ATC_HALF_TILE;
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk)
+          umma_f16(tmem_base + buf * 64, atc_desc_kmajor(sQ, kk), atc_desc_half_kmajor(ka, kk), idesc_sdp, kk != 0 ? 1u : 0u);
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk)
+          umma_f16(tmem_base + 128 + buf * 64, atc_desc_kmajor(sDO, kk), atc_desc_half_kmajor(va, kk), idesc_sdp, kk != 0 ? 1u : 0u);
+        umma_commit(sdp_full(buf));
+      };
+      mbar_wait(qdo_full(), 0);
+      issue_sdp(0);
+      for (int it = 0; it < iters; ++it) {
+        const int st = it % ATC_NST, buf = it & 1;
+        if (it + 1 < iters) issue_sdp(it + 1);
+        mbar_wait(ds_full(buf), (it >> 1) & 1);
+        tc_fence_after();
+        const uint32_t ka = sK + st * ATC_HALF_TILE;
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk)
+          umma_f16_ts(tmem_base + 256, tmem_base + buf * 64 + atc_half_operand_col(kk), atc_desc_half_mnmajor(ka, kk), idesc_acc,
+                      (it | kk) != 0 ? 1u : 0u);
+        umma_commit(kv_empty(st));
+      }
+      umma_commit(acc_full());
+    }
+  } else {
+    const int quarter = warp & 3, half = (warp - 2) >> 2;
+    const int row = quarter * 32 + lane;
+    const uint32_t lane_off = static_cast<uint32_t>(quarter * 32) << 16;
+    const int col0 = half * 32;
+    const float c = p.scale_log2;
+    const int qi = q0 + row;
+    const bool valid = qi < p.S;
+    const long long vidx = (static_cast<long long>(b) * p.nq + h) * p.S + qi;
+    const float L2 = valid ? p.lse[vidx] * 1.4426950408889634f : INFINITY;
+    const float Dr = valid ? p.dvec[vidx] : 0.f;
+    for (int it = 0; it < iters; ++it) {
+      const int buf = it & 1;
+      mbar_wait(sdp_full(buf), (it >> 1) & 1);
+      tc_fence_after();
+      uint32_t sr[32], dr[32];
+      tmem_ld32(tmem_base + lane_off + buf * 64 + col0, sr);
+      tmem_ld32(tmem_base + lane_off + 128 + buf * 64 + col0, dr);
+      tmem_ld_wait();
+      float ds[32];
+#pragma unroll
+      for (int i = 0; i < 32; ++i)
+        ds[i] = exp2f(fmaf(__uint_as_float(sr[i]), c, -L2)) * (__uint_as_float(dr[i]) - Dr);
+      if (it * 64 + 63 > q0) {                                        // diagonal blocks: key > query is masked
+        const int krel = it * 64 + col0 - q0;
+#pragma unroll
+        for (int i = 0; i < 32; ++i)
+          if (krel + i > row) ds[i] = 0.f;
+      }
+      uint32_t pk[16];
+#pragma unroll
+      for (int i = 0; i < 16; ++i) pk[i] = pack_f16(ds[2 * i], ds[2 * i + 1]);
+      tmem_st16(tmem_base + lane_off + buf * 64 + col0, pk);
+      tmem_st_wait();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(ds_full(buf));
+    }
+    mbar_wait(acc_full(), 0);
+    tc_fence_after();
+    const long long tok = static_cast<long long>(b) * p.S + qi;
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      const int cc = half * 64 + q * 32;
+      uint32_t a[32];
+      tmem_ld32(tmem_base + lane_off + 256 + cc, a);
+      tmem_ld_wait();
+      if (valid)
+        atc_store_grad32(reinterpret_cast<float(&)[32]>(a), p.scale, p.rope ? p.rope + static_cast<long long>(qi) * 64 + (cc >> 1) : nullptr,
+                         p.dq32 ? p.dq32 + tok * p.lddq32 + h * ATC_D + cc : nullptr,
+                         p.dq16 ? p.dq16 + tok * p.ldd16 + h * ATC_D + cc : nullptr);
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) { tc_fence_after(); tmem_dealloc(tmem_base, 512); }
+}
+
+inline cudaError_t attn_bwd_tc_launch(const __half* q, long long ldq, const __half* k, long long ldk, const __half* v,
+                                      long long ldv, const __half* dO, long long lddo, const AttnTcBwdParams& p, cudaStream_t st) {
+  static bool set = false;
+  if (!set) {
+    cudaError_t e = cudaFuncSetAttribute(attn_bwd_dkdv_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_BWD_SMEM);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(attn_bwd_dq_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_BWD_SMEM);
+    if (e != cudaSuccess) return e;
+    set = true;
+  }
+  AttnTcMaps m1, m2;
+  // dK/dV: K, V as 128-row tiles; Q, dO streamed as 64-row tiles
+  if (!make_map_attn(&m1.k, k, p.nkv * ATC_D, p.S, p.B, ldk, 128) || !make_map_attn(&m1.v, v, p.nkv * ATC_D, p.S, p.B, ldv, 128) ||
+      !make_map_attn(&m1.q, q, p.nq * ATC_D, p.S, p.B, ldq, 64) || !make_map_attn(&m1.dO, dO, p.nq * ATC_D, p.S, p.B, lddo, 64))
+    return cudaErrorInvalidValue;
+  // dQ: Q, dO as 128-row tiles; K, V streamed as 64-row tiles
+  if (!make_map_attn(&m2.k, k, p.nkv * ATC_D, p.S, p.B, ldk, 64) || !make_map_attn(&m2.v, v, p.nkv * ATC_D, p.S, p.B, ldv, 64) ||
+      !make_map_attn(&m2.q, q, p.nq * ATC_D, p.S, p.B, ldq, 128) || !make_map_attn(&m2.dO, dO, p.nq * ATC_D, p.S, p.B, lddo, 128))
+    return cudaErrorInvalidValue;
+  dim3 g1((p.S + 127) / 128, p.nkv, p.B);
+  attn_bwd_dkdv_tc_kernel<<<g1, ATC_BWD_THREADS, ATC_BWD_SMEM, st>>>(m1, p);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  dim3 g2((p.S + 127) / 128, p.nq, p.B);
+  attn_bwd_dq_tc_kernel<<<g2, ATC_BWD_THREADS, ATC_BWD_SMEM, st>>>(m2, p);
   return cudaGetLastError();
 }
 

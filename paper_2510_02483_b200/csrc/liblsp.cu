@@ -260,6 +260,19 @@ cudaError_t attn_fwd_dispatch(const lsp_ctx* c, const AttnParams& p, cudaStream_
   return attn_fwd_launch<64>(p, st);
 }
 
+// B7 dispatch (two kernels either way: dK/dV, then dQ)
+cudaError_t attn_bwd_dispatch(const lsp_ctx* c, const AttnParams& p, cudaStream_t st) {
+  if (c->d.head_dim == 128) {
+    AttnTcBwdParams t;
+    t.B = p.B; t.S = p.S; t.nq = p.nq; t.nkv = p.nkv; t.scale_log2 = p.scale_log2; t.scale = p.scale;
+    t.lse = p.lse; t.dvec = p.dvec; t.rope = p.rope;
+    t.dq32 = p.dq32; t.dk32 = p.dk32; t.dv32 = p.dv32; t.lddq32 = p.lddq32; t.lddk32 = p.lddk32;
+    t.dq16 = p.dq16; t.dk16 = p.dk16; t.dv16 = p.dv16; t.ldd16 = p.ldd16;
+    return attn_bwd_tc_launch(p.q, p.ldq, p.k, p.ldk, p.v, p.ldv, p.dO, p.lddo, t, st);
+  }
+  return attn_bwd_launch<64>(p, st);
+}
+
 // ------------------------------------------------------------------------------------------- attention block
 // x [T,H] x_dt -> a32 [T,H] fp32.  SURVEY 8(a) F1-F4.
 lsp_status attn_fwd_impl(lsp_ctx* ctx, int x_dt, const void* x, const lsp_layer_weights* w, float* a_out, void* saved,
@@ -342,8 +355,7 @@ lsp_status attn_bwd_impl(lsp_ctx* ctx, int x_dt, const void* x, int da_dt, const
   p.lse = const_cast<float*>(lse); p.dvec = dvec;
   p.rope = d.use_rope ? ctx->rope : nullptr;
   p.dq16 = dqkv; p.dk16 = dqkv + Nq; p.dv16 = dqkv + Nq + Nkv; p.ldd16 = Nqkv;
-  if (d.head_dim == 128) LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_launch<128>(p, st));
-  else LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_launch<64>(p, st));
+  LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_dispatch(ctx, p, st));
   // B9 dW{q,k,v} = d{q,k,v}^T xn (one GEMM, rows split over three outputs) ; dxn = [dq|dk|dv] [Wq;Wk;Wv] (one GEMM)
   {
     EpiF32 e = epi_f32(static_cast<float*>(g->wq), H);
@@ -629,8 +641,7 @@ lsp_status lsp_sdpa_bwd(lsp_ctx* ctx, const void* q, const void* k, const void* 
   p.lse = const_cast<float*>(lse); p.dvec = dvec;
   p.dq32 = static_cast<float*>(dq); p.dk32 = static_cast<float*>(dk); p.dv32 = static_cast<float*>(dv);
   p.lddq32 = ctx->Nq; p.lddk32 = ctx->Nkv;
-  if (d.head_dim == 128) LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_launch<128>(p, st));
-  else LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_launch<64>(p, st));
+  LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_dispatch(ctx, p, st));
   return LSP_OK;
 }
 
