@@ -12,8 +12,17 @@
 // DUAL mode: B tile rows [0,128) come from b[0] and rows [128,256) from b[1] (same 128 output columns);
 // one 128x256 MMA then yields both the gate and the up projection, which the SwiGLU epilogue combines.
 //
-// Warp roles (192 threads): warp 0 = TMA producer, warp 1 = MMA issuer + TMEM owner, warps 2..5 = epilogue.
+// Warp roles (320 threads): warp 0 = TMA producer, warp 1 = MMA issuer + TMEM owner, warps 2..9 = epilogue
+// (TMEM lane quarter = warp & 3; the two warps of a quarter take alternate 32-column chunks).
+//
+// Tile order: persistent CTAs take tiles i, i + grid, ...; tile ids run m-fastest inside bands of `band`
+// m-blocks and sweep all n-blocks before moving to the next band, so the ~148 tiles in flight form a compact
+// band x (148/band) block: each A k-slice is shared by ~148/band CTAs and each B k-slice by `band` CTAs through
+// L2, and the band's A panel stays L2-resident for the sweep (m-fastest over all of M re-read A once per
+// n-block: 4-6 GB of DRAM reads per GEMM at the 3B shape, profiles/r1_gemm_ncu.md).
 #pragma once
+#include <stdlib.h>
+
 #include "ptx.cuh"
 
 namespace lsp {
@@ -22,7 +31,8 @@ enum : int { DT_BF16 = 0, DT_F32 = 1, DT_F16 = 2 };
 
 constexpr int GEMM_BM = 128;
 constexpr int GEMM_BK = 64;          // 64 x 16-bit = one 128-byte swizzle row
-constexpr int GEMM_THREADS = 192;
+constexpr int GEMM_THREADS = 320;         // warp 0 TMA, warp 1 MMA, warps 2..9 epilogue
+constexpr int GEMM_EPI_WARPS = 8;
 constexpr int GEMM_MAX_SEG = 3;
 
 struct GemmMaps {
@@ -34,6 +44,7 @@ struct GemmShape {
   int a_fmt, b_fmt;                  // UMMA operand formats: 0 = fp16, 1 = bf16; must be equal (a mixed pair is an
                                      // illegal instruction on sm_100a -- measured)
   int nseg;                          // number of K segments (non-DUAL); DUAL uses a[0], b[0], b[1]
+  int band;                          // m-blocks per rasterisation band (>= 1)
   int kblocks[GEMM_MAX_SEG];         // ceil(K_s / 64)
 };
 
@@ -200,6 +211,15 @@ struct EpiSwiGLUBwd {
 };
 
 // ------------------------------------------------------------------------------------------- the kernel
+// linear tile id -> (m-block, n-block), banded m-fastest order
+__device__ __forceinline__ void gemm_tile_coord(int tile, int mblocks, int nblocks, int band, int& mb, int& nb) {
+  const int per_band = band * nblocks;
+  const int bid = tile / per_band, r = tile - bid * per_band;
+  const int rows = min(band, mblocks - bid * band);
+  nb = r / rows;
+  mb = bid * band + (r - nb * rows);
+}
+
 template <int BN, bool A_MN, bool B_MN, bool DUAL, class Epi>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
 gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, const Epi epi) {
@@ -232,7 +252,7 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, c
     for (int s = 0; s < nseg; ++s) { tma_prefetch_desc(&maps.a[s]); tma_prefetch_desc(&maps.b[s]); }
     if (DUAL) tma_prefetch_desc(&maps.b[1]);
     for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 4); }
+    for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), GEMM_EPI_WARPS); }
     fence_barrier_init();
   }
   if (warp == 1) {
@@ -249,8 +269,9 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, c
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
       for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int m0 = (tile % mblocks) * GEMM_BM;
-        const int n0 = (tile / mblocks) * NOUT;
+        int mb, nb;
+        gemm_tile_coord(tile, mblocks, nblocks, sh.band, mb, nb);
+        const int m0 = mb * GEMM_BM, n0 = nb * NOUT;
         for (int s = 0; s < nseg; ++s) {
           for (int kb = 0; kb < sh.kblocks[s]; ++kb) {
             mbar_wait(empty_bar(stage), phase ^ 1u);
@@ -315,18 +336,20 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, c
       }
     }
   } else {
-    // ===================================================================== epilogue warps (2..5)
+    // ===================================================================== epilogue warps (2..9)
     const int quarter = warp & 3;               // TMEM lanes [32*quarter, 32*quarter+32) are this warp's
+    const int half = (warp - 2) >> 2;           // which of the two warps of this quarter: chunks half, half+2, ...
     int acc = 0; uint32_t acc_phase = 0;
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-      const int m0 = (tile % mblocks) * GEMM_BM;
-      const int n0 = (tile / mblocks) * NOUT;
+      int mb, nb;
+      gemm_tile_coord(tile, mblocks, nblocks, sh.band, mb, nb);
+      const int m0 = mb * GEMM_BM, n0 = nb * NOUT;
       mbar_wait(tfull_bar(acc), acc_phase);
       tc_fence_after();
       const int m = m0 + quarter * 32 + lane;
       const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + static_cast<uint32_t>(acc * BN);
 #pragma unroll 1
-      for (int c = 0; c < NOUT / 32; ++c) {
+      for (int c = half; c < NOUT / 32; c += 2) {
         const int n = n0 + c * 32;
         if (n >= sh.N) break;                   // warp-uniform
         const int nvalid = min(32, sh.N - n);
@@ -405,8 +428,20 @@ inline bool encode_operand(CUtensorMap* m, const Operand& o, long long mn, long 
   return make_map_2d(m, o.ptr, k, mn, o.ld, GEMM_BK, o.dt == DT_F16);
 }
 
+// m-blocks per rasterisation band (see the header comment).  LSP_GEMM_BAND overrides (tuning aid).
+inline int gemm_band(int mblocks) {
+  static int forced = -1;
+  if (forced < 0) {
+    const char* e = getenv("LSP_GEMM_BAND");
+    forced = e ? atoi(e) : 0;
+  }
+  int b = forced > 0 ? forced : 16;
+  if (b > mblocks) b = mblocks;
+  return b < 1 ? 1 : b;
+}
+
 template <int BN, bool A_MN, bool B_MN, bool DUAL, class Epi>
-cudaError_t launch_gemm(const GemmMaps& maps, const GemmShape& sh, const Epi& epi, int num_sms, cudaStream_t st) {
+cudaError_t launch_gemm(const GemmMaps& maps, GemmShape sh, const Epi& epi, int num_sms, cudaStream_t st) {
   using Cfg = GemmCfg<BN>;
   auto kern = gemm_tcgen05_kernel<BN, A_MN, B_MN, DUAL, Epi>;
   static bool attr_set = false;
@@ -419,6 +454,7 @@ cudaError_t launch_gemm(const GemmMaps& maps, const GemmShape& sh, const Epi& ep
   const int mblocks = (sh.M + GEMM_BM - 1) / GEMM_BM, nblocks = (sh.N + NOUT - 1) / NOUT;
   const int ntiles = mblocks * nblocks;
   if (ntiles == 0) return cudaSuccess;
+  sh.band = gemm_band(mblocks);
   const int grid = ntiles < num_sms ? ntiles : num_sms;
   kern<<<grid, GEMM_THREADS, Cfg::SMEM_BYTES, st>>>(maps, sh, epi);
   return cudaGetLastError();
