@@ -380,6 +380,183 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, c
   }
 }
 
+// ------------------------------------------------------------------------------------------- the CTA-pair kernel
+// Same pipeline on a pair of CTAs (cluster of 2 = two SMs of one TPC) working on one 256 x 256 tile with
+// tcgen05.mma.cta_group::2: CTA r of the pair stages rows [128 r, +128) of the A tile and rows [128 r, +128) of the
+// B tile (32 KB per stage instead of 48 KB, so 6 stages fit), the leader's single MMA thread issues one
+// 256 x 256 x 16 instruction that reads both CTAs' shared memory, and CTA r's TMEM receives output rows [128 r, +128).
+// Halving the B traffic per SM takes the shared-memory port off the critical path (128 x 256 per SM needs
+// 96 B/clk of operand reads + 96 B/clk of TMA writes with cta_group::1, 64 + 64 with the pair).
+//   full[s]   : leader's barrier, armed by the leader's producer for the bytes of BOTH CTAs; every TMA of the pair
+//               (cp.async.bulk.tensor...cta_group::2) reports to it
+//   empty[s]  : one per CTA; the leader's tcgen05.commit multicasts the arrival to both
+//   tfull[a]  : one per CTA (multicast commit); tempty[a]: leader's, 16 arrivals (8 epilogue warps x 2 CTAs, remote)
+// DUAL: CTA 0 stages the gate rows and CTA 1 the up rows of the same 128 output columns, so the pair's N = 256
+// accumulator is [gate | up] exactly as in the single-CTA kernel.
+constexpr int GEMM2_STAGES = 6;
+constexpr int GEMM2_STAGE_BYTES = 2 * GEMM_BM * GEMM_BK * 2;         // A 128 x 64 + B 128 x 64 (fp16) per CTA
+constexpr int GEMM2_SMEM_BYTES = GEMM2_STAGES * GEMM2_STAGE_BYTES + 1024 + 256;
+
+template <bool A_MN, bool B_MN, bool DUAL, class Epi>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEMM_THREADS, 1)
+gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, const Epi epi) {
+  constexpr int STAGES = GEMM2_STAGES;
+  constexpr int BN = 256;                        // MMA N (both CTAs' B halves)
+  constexpr int NOUT = DUAL ? 128 : 256;         // output columns covered by one tile
+  constexpr int A_BYTES = GEMM_BM * GEMM_BK * 2;
+  static_assert(!DUAL || (!A_MN && !B_MN), "DUAL is the forward gate/up GEMM");
+
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bar_base = smem_base + STAGES * GEMM2_STAGE_BYTES;
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
+  auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * STAGES + s); };
+  auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * STAGES + 2 + s); };
+  const uint32_t tmem_slot = bar_base + 8u * (2 * STAGES + 4);
+  uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const int cid = blockIdx.x >> 1, nclusters = gridDim.x >> 1;
+
+  const int mblocks = (sh.M + 2 * GEMM_BM - 1) / (2 * GEMM_BM);      // 256-row blocks
+  const int nblocks = (sh.N + NOUT - 1) / NOUT;
+  const int ntiles = mblocks * nblocks;
+  int kb_total = 0;
+  const int nseg = DUAL ? 1 : sh.nseg;
+  for (int s = 0; s < nseg; ++s) kb_total += sh.kblocks[s];
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < nseg; ++s) { tma_prefetch_desc(&maps.a[s]); tma_prefetch_desc(&maps.b[s]); }
+    if (DUAL) tma_prefetch_desc(&maps.b[1]);
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+    for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 2 * GEMM_EPI_WARPS); }
+    fence_barrier_init();
+  }
+  if (warp == 1) {
+    tmem_alloc_pair(tmem_slot, 512);
+    tmem_relinquish_pair();
+  }
+  tc_fence_before();
+  cluster_sync_all();                            // barriers of both CTAs initialised before any remote arrival / TMA
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot_ptr;
+
+  if (warp == 0) {
+    // ===================================================================== TMA producer (both CTAs)
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      for (int tile = cid; tile < ntiles; tile += nclusters) {
+        int mb, nb;
+        gemm_tile_coord(tile, mblocks, nblocks, sh.band, mb, nb);
+        const int m0 = mb * 2 * GEMM_BM + static_cast<int>(rank) * GEMM_BM;
+        const int n0 = nb * NOUT;
+        const int nb0 = DUAL ? n0 : n0 + static_cast<int>(rank) * 128;         // this CTA's B rows
+        for (int s = 0; s < nseg; ++s) {
+          const CUtensorMap* bmap = DUAL ? &maps.b[rank] : &maps.b[s];
+          for (int kb = 0; kb < sh.kblocks[s]; ++kb) {
+            mbar_wait(empty_bar(stage), phase ^ 1u);
+            const uint32_t sa = smem_base + stage * GEMM2_STAGE_BYTES;
+            const uint32_t sb = sa + A_BYTES;
+            const uint32_t fb = mapa_shared(full_bar(stage), 0);
+            if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * GEMM2_STAGE_BYTES);
+            const int k0 = kb * GEMM_BK;
+            if constexpr (!A_MN) {
+              tma_load_2d_pair(sa, &maps.a[s], fb, k0, m0);
+            } else {
+#pragma unroll
+              for (int c = 0; c < 2; ++c) tma_load_2d_pair(sa + c * (GEMM_BK * 128), &maps.a[s], fb, m0 + 64 * c, k0);
+            }
+            if constexpr (!B_MN) {
+              tma_load_2d_pair(sb, bmap, fb, k0, nb0);
+            } else {
+#pragma unroll
+              for (int c = 0; c < 2; ++c) tma_load_2d_pair(sb + c * (GEMM_BK * 128), bmap, fb, nb0 + 64 * c, k0);
+            }
+            if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================================================================== MMA issuer (leader CTA only)
+    if (lane == 0 && rank == 0) {
+      const uint32_t idesc = umma_idesc(2 * GEMM_BM, BN, sh.a_fmt, sh.b_fmt, A_MN ? 1 : 0, B_MN ? 1 : 0);
+      constexpr uint32_t A_LBO = A_MN ? GEMM_BK * 128 : 16, B_LBO = B_MN ? GEMM_BK * 128 : 16;
+      constexpr uint32_t A_KSTEP = A_MN ? 2048 : 32, B_KSTEP = B_MN ? 2048 : 32;
+      int stage = 0; uint32_t phase = 0;
+      int acc = 0; uint32_t acc_phase = 0;
+      for (int tile = cid; tile < ntiles; tile += nclusters) {
+        mbar_wait_cluster(tempty_bar(acc), acc_phase ^ 1u);
+        tc_fence_after();
+        const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(acc * BN);
+        for (int kb = 0; kb < kb_total; ++kb) {
+          mbar_wait_cluster(full_bar(stage), phase);
+          tc_fence_after();
+          const uint32_t sa = smem_base + stage * GEMM2_STAGE_BYTES;
+          const uint32_t sb = sa + A_BYTES;
+#pragma unroll
+          for (int k = 0; k < GEMM_BK / 16; ++k) {
+            const uint64_t ad = umma_smem_desc(sa + k * A_KSTEP, A_LBO, 1024);
+            const uint64_t bd = umma_smem_desc(sb + k * B_KSTEP, B_LBO, 1024);
+            umma_f16_pair(d_tmem, ad, bd, idesc, (kb | k) != 0 ? 1u : 0u);
+          }
+          umma_commit_pair(empty_bar(stage), 3);
+          if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+        }
+        umma_commit_pair(tfull_bar(acc), 3);
+        if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+      }
+    }
+  } else {
+    // ===================================================================== epilogue warps (2..9, both CTAs)
+    const int quarter = warp & 3;
+    const int half = (warp - 2) >> 2;
+    const uint32_t tempty_leader0 = mapa_shared(tempty_bar(0), 0), tempty_leader1 = mapa_shared(tempty_bar(1), 0);
+    int acc = 0; uint32_t acc_phase = 0;
+    for (int tile = cid; tile < ntiles; tile += nclusters) {
+      int mb, nb;
+      gemm_tile_coord(tile, mblocks, nblocks, sh.band, mb, nb);
+      const int m0 = mb * 2 * GEMM_BM + static_cast<int>(rank) * GEMM_BM;
+      const int n0 = nb * NOUT;
+      mbar_wait_cluster(tfull_bar(acc), acc_phase);
+      tc_fence_after();
+      const int m = m0 + quarter * 32 + lane;
+      const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + static_cast<uint32_t>(acc * BN);
+#pragma unroll 1
+      for (int c = half; c < NOUT / 32; c += 2) {
+        const int n = n0 + c * 32;
+        if (n >= sh.N) break;                   // warp-uniform
+        const int nvalid = min(32, sh.N - n);
+        uint32_t r0[32];
+        tmem_ld32(t_row + c * 32, r0);
+        if constexpr (DUAL) {
+          uint32_t r1[32];
+          tmem_ld32(t_row + NOUT + c * 32, r1);
+          tmem_ld_wait();
+          if (m < sh.M) epi(m, n, reinterpret_cast<float(&)[32]>(r0), reinterpret_cast<float(&)[32]>(r1), nvalid);
+        } else {
+          tmem_ld_wait();
+          if (m < sh.M) epi(m, n, reinterpret_cast<float(&)[32]>(r0), nvalid);
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_cluster(acc == 0 ? tempty_leader0 : tempty_leader1);
+      if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+    }
+  }
+
+  tc_fence_before();
+  cluster_sync_all();                            // nobody leaves while the peer may still signal its barriers / read its smem
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc_pair(tmem_base, 512);
+  }
+}
+
 // ------------------------------------------------------------------------------------------- host side
 typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                     const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -440,6 +617,37 @@ inline int gemm_band(int mblocks) {
   return b < 1 ? 1 : b;
 }
 
+// CTA-pair kernel for every GEMM with more than one 128-row block; LSP_GEMM_PAIR=0 forces the single-CTA kernel.
+inline bool gemm_use_pair(int M) {
+  static int mode = -1;
+  if (mode < 0) {
+    const char* e = getenv("LSP_GEMM_PAIR");
+    mode = e ? atoi(e) : 1;
+  }
+  return mode != 0 && M > GEMM_BM;
+}
+
+template <bool A_MN, bool B_MN, bool DUAL, class Epi>
+cudaError_t launch_gemm_pair(const GemmMaps& maps, GemmShape sh, const Epi& epi, int num_sms, cudaStream_t st) {
+  auto kern = gemm_pair_tcgen05_kernel<A_MN, B_MN, DUAL, Epi>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM2_SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  constexpr int NOUT = DUAL ? 128 : 256;
+  const int mblocks = (sh.M + 2 * GEMM_BM - 1) / (2 * GEMM_BM), nblocks = (sh.N + NOUT - 1) / NOUT;
+  const int ntiles = mblocks * nblocks;
+  if (ntiles == 0) return cudaSuccess;
+  sh.band = gemm_band(2 * mblocks) / 2;
+  if (sh.band < 1) sh.band = 1;
+  const int pairs = num_sms / 2;
+  const int grid = 2 * (ntiles < pairs ? ntiles : pairs);
+  kern<<<grid, GEMM_THREADS, GEMM2_SMEM_BYTES, st>>>(maps, sh, epi);
+  return cudaGetLastError();
+}
+
 template <int BN, bool A_MN, bool B_MN, bool DUAL, class Epi>
 cudaError_t launch_gemm(const GemmMaps& maps, GemmShape sh, const Epi& epi, int num_sms, cudaStream_t st) {
   using Cfg = GemmCfg<BN>;
@@ -469,11 +677,13 @@ cudaError_t gemm_run(int M, int N, int nseg, const Operand* a, const Operand* b,
   sh.M = M; sh.N = N; sh.nseg = nseg;
   sh.a_fmt = umma_fmt(a[0].dt); sh.b_fmt = umma_fmt(b[0].dt);      // all segments share the operand formats
   for (int s = 0; s < GEMM_MAX_SEG; ++s) sh.kblocks[s] = 0;
+  const bool pair = BN == 256 && gemm_use_pair(M);
   for (int s = 0; s < nseg; ++s) {
     sh.kblocks[s] = (ks[s] + GEMM_BK - 1) / GEMM_BK;
     if (!encode_operand(&maps.a[s], a[s], M, ks[s], GEMM_BM)) return cudaErrorInvalidValue;
-    if (!encode_operand(&maps.b[s], b[s], N, ks[s], BN)) return cudaErrorInvalidValue;
+    if (!encode_operand(&maps.b[s], b[s], N, ks[s], pair ? 128 : BN)) return cudaErrorInvalidValue;
   }
+  if (pair) return launch_gemm_pair<A_MN, B_MN, false, Epi>(maps, sh, epi, num_sms, st);
   return launch_gemm<BN, A_MN, B_MN, false, Epi>(maps, sh, epi, num_sms, st);
 }
 
@@ -489,6 +699,7 @@ cudaError_t gemm_run_dual(int M, int N, int K, const Operand& a, const Operand& 
   if (!encode_operand(&maps.a[0], a, M, K, GEMM_BM)) return cudaErrorInvalidValue;
   if (!encode_operand(&maps.b[0], bg, N, K, 128)) return cudaErrorInvalidValue;
   if (!encode_operand(&maps.b[1], bu, N, K, 128)) return cudaErrorInvalidValue;
+  if (gemm_use_pair(M)) return launch_gemm_pair<false, false, true, Epi>(maps, sh, epi, num_sms, st);
   return launch_gemm<256, false, false, true, Epi>(maps, sh, epi, num_sms, st);
 }
 
