@@ -327,6 +327,10 @@ inline cudaError_t attn_fwd_tc_launch(const __half* q, long long ldq, const __ha
 // The 16-bit operand written back over a 64-column fp32 buffer keeps each half inside the columns its own warp
 // read (keys/queries 0..31 -> columns 0..15, 32..63 -> columns 32..47), so the two half-warps never race.
 constexpr int ATC_BWD_THREADS = 320;
+// Query positions below this keep P / dS as a two-term fp16 sum (hi + lo, two MMAs into the same accumulator):
+// early rows are O(1) while the tensor-wide rms the parity metric divides by shrinks like sqrt(ln S / S), so a
+// single fp16 rounding there is what limits dq/dk/dv at long S (P-5/P-6).
+constexpr int ATC_SPLIT_ROWS = 256;
 constexpr int ATC_NST = 3;                                 // stages of the streamed 64-row tiles
 constexpr int ATC_HALF_TILE = 64 * ATC_D * 2;              // 64 x 128 fp16 = 16 KB (two 8 KB chunks)
 constexpr int ATC_BWD_SMEM = 2 * ATC_TILE_BYTES + 2 * ATC_NST * ATC_HALF_TILE + ATC_NST * 2 * 64 * 4 + 1024 + 256;
@@ -356,6 +360,15 @@ __device__ __forceinline__ uint64_t atc_desc_half_mnmajor(uint32_t tile, int kk)
 }
 // TMEM column of the kk-th 16-element K step of a 64-wide fp16 operand stored as described above
 __device__ __forceinline__ uint32_t atc_half_operand_col(int kk) { return static_cast<uint32_t>((kk >> 1) * 32 + (kk & 1) * 8); }
+
+// x = hi + lo with both halves fp16: packs two values' hi parts and lo parts.
+__device__ __forceinline__ void atc_split_pack(float x0, float x1, uint32_t& hi, uint32_t& lo) {
+  const __half2 h = __floats2half2_rn(x0, x1);
+  const float2 hf = __half22float2(h);
+  const __half2 l = __floats2half2_rn(x0 - hf.x, x1 - hf.y);
+  hi = *reinterpret_cast<const uint32_t*>(&h);
+  lo = *reinterpret_cast<const uint32_t*>(&l);
+}
 
 // Scale, optionally rotate by -theta (transpose of the forward rotation), and store 32 columns of one row.
 __device__ __forceinline__ void atc_store_grad32(float (&v)[32], float scale, const float2* rope_row, float* o32, __half* o16) {
@@ -472,18 +485,31 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
         const uint32_t ph = (it >> 1) & 1;
         if (it + 1 < iters) issue_sdp(it + 1);
         const uint32_t qa = sQ + st * ATC_HALF_TILE, da = sDO + st * ATC_HALF_TILE;
+        const bool split = (2 * kb + it % per_head) * 64 < ATC_SPLIT_ROWS;
         mbar_wait(p_full(buf), ph);
         tc_fence_after();
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk)                                // dV += P^T dO
           umma_f16_ts(tmem_base + 256, tmem_base + buf * 64 + atc_half_operand_col(kk), atc_desc_half_mnmajor(da, kk), idesc_acc,
                       (it | kk) != 0 ? 1u : 0u);
+        if (split) {
+#pragma unroll
+          for (int kk = 0; kk < 4; ++kk)                              // ... + (P^T)_lo dO
+            umma_f16_ts(tmem_base + 256, tmem_base + buf * 64 + 16 + atc_half_operand_col(kk), atc_desc_half_mnmajor(da, kk),
+                        idesc_acc, 1u);
+        }
         mbar_wait(ds_full(buf), ph);
         tc_fence_after();
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk)                                // dK += dS^T Q
           umma_f16_ts(tmem_base + 384, tmem_base + 128 + buf * 64 + atc_half_operand_col(kk), atc_desc_half_mnmajor(qa, kk),
                       idesc_acc, (it | kk) != 0 ? 1u : 0u);
+        if (split) {
+#pragma unroll
+          for (int kk = 0; kk < 4; ++kk)
+            umma_f16_ts(tmem_base + 384, tmem_base + 128 + buf * 64 + 16 + atc_half_operand_col(kk), atc_desc_half_mnmajor(qa, kk),
+                        idesc_acc, 1u);
+        }
         umma_commit(qdo_empty(st));
       }
       umma_commit(acc_full());
@@ -522,9 +548,16 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
         for (int i = 0; i < 32; ++i)
           if (qrel + i < row) pv[i] = 0.f;
       }
-      uint32_t pk[16];
+      const bool split = (2 * kb + rel) * 64 < ATC_SPLIT_ROWS;      // early query positions: hi + lo operands
+      uint32_t pk[16], pl[16];
+      if (split) {
 #pragma unroll
-      for (int i = 0; i < 16; ++i) pk[i] = pack_f16(pv[2 * i], pv[2 * i + 1]);
+        for (int i = 0; i < 16; ++i) atc_split_pack(pv[2 * i], pv[2 * i + 1], pk[i], pl[i]);
+        tmem_st16(tmem_base + lane_off + buf * 64 + col0 + 16, pl);
+      } else {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) pk[i] = pack_f16(pv[2 * i], pv[2 * i + 1]);
+      }
       tmem_st16(tmem_base + lane_off + buf * 64 + col0, pk);
       tmem_st_wait();
       tc_fence_before();
@@ -538,8 +571,14 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
         pv[4 * i + 2] *= __uint_as_float(dr[4 * i + 2]) - Dv.z;
         pv[4 * i + 3] *= __uint_as_float(dr[4 * i + 3]) - Dv.w;
       }
+      if (split) {
 #pragma unroll
-      for (int i = 0; i < 16; ++i) pk[i] = pack_f16(pv[2 * i], pv[2 * i + 1]);
+        for (int i = 0; i < 16; ++i) atc_split_pack(pv[2 * i], pv[2 * i + 1], pk[i], pl[i]);
+        tmem_st16(tmem_base + lane_off + 128 + buf * 64 + col0 + 16, pl);
+      } else {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) pk[i] = pack_f16(pv[2 * i], pv[2 * i + 1]);
+      }
       tmem_st16(tmem_base + lane_off + 128 + buf * 64 + col0, pk);
       tmem_st_wait();
       tc_fence_before();
@@ -661,6 +700,12 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
         for (int kk = 0; kk < 4; ++kk)
           umma_f16_ts(tmem_base + 256, tmem_base + buf * 64 + atc_half_operand_col(kk), atc_desc_half_mnmajor(ka, kk), idesc_acc,
                       (it | kk) != 0 ? 1u : 0u);
+        if (q0 < ATC_SPLIT_ROWS) {                                    // early query rows: + dS_lo K
+#pragma unroll
+          for (int kk = 0; kk < 4; ++kk)
+            umma_f16_ts(tmem_base + 256, tmem_base + buf * 64 + 16 + atc_half_operand_col(kk), atc_desc_half_mnmajor(ka, kk),
+                        idesc_acc, 1u);
+        }
         umma_commit(kv_empty(st));
       }
       umma_commit(acc_full());
@@ -695,8 +740,15 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
           if (krel + i > row) ds[i] = 0.f;
       }
       uint32_t pk[16];
+      if (q0 < ATC_SPLIT_ROWS) {
+        uint32_t pl[16];
 #pragma unroll
-      for (int i = 0; i < 16; ++i) pk[i] = pack_f16(ds[2 * i], ds[2 * i + 1]);
+        for (int i = 0; i < 16; ++i) atc_split_pack(ds[2 * i], ds[2 * i + 1], pk[i], pl[i]);
+        tmem_st16(tmem_base + lane_off + buf * 64 + col0 + 16, pl);
+      } else {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) pk[i] = pack_f16(ds[2 * i], ds[2 * i + 1]);
+      }
       tmem_st16(tmem_base + lane_off + buf * 64 + col0, pk);
       tmem_st_wait();
       tc_fence_before();

@@ -73,3 +73,44 @@ def run_layer(w: synth.Workload, layer: int = 0):
     out.update({"d" + k: v.cpu().numpy() for k, v in buf.grads.items()})
     ctx.close()
     return out
+
+
+class StackRunner:
+    """BASELINE.json config 3: embedding gather, then n_layers x lsp_layer_fwd, then n_layers x lsp_layer_bwd in
+    reverse (reading A-11: no final norm / head / loss; the upstream gradient enters at the last layer's output).
+    The residual stream between layers is fp32 (in_dtype = LSP_F32); every layer keeps its own `saved` bundle, the
+    workspace is shared.  Host-side sequencing only -- every step runs in the library's kernels."""
+
+    def __init__(self, w: synth.Workload, n_layers: int, dev=None):
+        self.dev = dev or require_cuda()
+        self.w, self.L = w, n_layers
+        self.ctx = make_ctx(w, in_dtype=B.LSP_F32)
+        T, H = w.tokens, w.hidden
+        f32 = dict(dtype=torch.float32, device=self.dev)
+        self.saved = [torch.empty(self.ctx.saved_bytes, dtype=torch.uint8, device=self.dev) for _ in range(n_layers)]
+        self.ws = torch.empty(self.ctx.workspace_bytes, dtype=torch.uint8, device=self.dev)
+        self.xs = [torch.empty((T, H), **f32) for _ in range(n_layers + 1)]
+        self.d = [torch.empty((T, H), **f32) for _ in range(2)]
+        self.weights = [upload_weights(synth.layer_weights(w, layer), self.dev) for layer in range(n_layers)]
+        self.grads = {k: torch.empty(s, **f32) for k, s in WEIGHT_SHAPES(w).items()}
+
+    def forward(self, ids: torch.Tensor, table: torch.Tensor, stream=None):
+        B.lsp_embed_fwd(self.ctx, ids, table, self.xs[0], stream)
+        for l in range(self.L):
+            B.lsp_layer_fwd(self.ctx, self.xs[l], self.weights[l], self.xs[l + 1], self.saved[l], self.ws, stream)
+        return self.xs[self.L]
+
+    def backward(self, dy32: torch.Tensor, on_layer_grads=None, stream=None):
+        """dy32: fp32 [T,H].  on_layer_grads(layer, grads_dict) is called after each layer's backward (the gradient
+        buffers are reused by the next layer).  Returns dx0 (gradient w.r.t. the gathered embeddings)."""
+        d_in = dy32
+        for i, l in enumerate(range(self.L - 1, -1, -1)):
+            d_out = self.d[i & 1]
+            B.lsp_layer_bwd(self.ctx, self.xs[l], d_in, self.weights[l], self.saved[l], d_out, self.grads, self.ws, stream)
+            if on_layer_grads is not None:
+                on_layer_grads(l, self.grads)
+            d_in = d_out
+        return d_in
+
+    def close(self):
+        self.ctx.close()

@@ -201,3 +201,59 @@ def test_embed_bit_exact(gpu):
     ref = R.embed_fwd(s["ids"], synth.bf16_bits_to_f64(s["embedding"]))
     assert np.array_equal(x0.cpu().numpy().astype(np.float64), ref)
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------------- stack (cfg 3, reduced depth)
+def test_stack_fwd_bwd(gpu):
+    """Embedding gather + 3 decoder layers forward, then backward (BASELINE.json configs[2] at reduced depth/size so the
+    oracle finishes in seconds): final y, dx0 and every layer's nine gradients."""
+    import torch
+    w = synth.Workload("stack_small", 3, 2, 192, 256, 4, 2, 128, 688, 1e-5, 500000.0, 3, 1000)
+    s = synth.stack_inputs(w)
+    run = gpu.StackRunner(w, w.n_layers)
+    ids = torch.from_numpy(s["ids"]).cuda()
+    table = gpu.bf16_to_device(s["embedding"])
+    y = run.forward(ids, table)
+    got_grads = {}
+    dy32 = gpu.bf16_to_device(s["dy"]).float()
+    dx0 = run.backward(dy32, on_layer_grads=lambda l, g: got_grads.__setitem__(l, {k: v.cpu().numpy() for k, v in g.items()}))
+    torch.cuda.synchronize()
+    x0_ref = R.embed_fwd(s["ids"], synth.bf16_bits_to_f64(s["embedding"]))
+    wts = [f64(synth.layer_weights(w, l)) for l in range(w.n_layers)]
+    y_ref, dx0_ref, g_ref = R.stack_fwd_bwd(x0_ref, synth.bf16_bits_to_f64(s["dy"]), wts, oracle_shape(w))
+    check(dict(y=y.cpu().numpy(), dx0=dx0.cpu().numpy()), dict(y=y_ref, dx0=dx0_ref), ["y", "dx0"])
+    for l in range(w.n_layers):
+        check({"d" + k: v for k, v in got_grads[l].items()}, {"d" + k: v for k, v in g_ref[l].items()},
+              ["d" + k for k in synth.WEIGHT_NAMES])
+    run.close()
+
+
+# ------------------------------------------------------------------------------------------- full-size configurations
+def _layer_full(gpu, w):
+    got = gpu.run_layer(w)
+    inp, wt = f64(synth.layer_inputs(w)), f64(synth.layer_weights(w))
+    ref = R.layer_fwd_bwd(inp["x"], inp["dy"], wt, oracle_shape(w))
+    check(got, ref, ALL)
+
+
+@pytest.mark.slow
+def test_layer_cfg2_full_size(gpu):
+    """BASELINE.json configs[1] exactly as bench.py launches it (3B-shape layer, batch 4 x seq 4096): every element of
+    y, dx and the nine gradients against the fp64 oracle run on the host cores (about a minute of CPU time)."""
+    _layer_full(gpu, synth.CFG2_3B_LAYER)
+
+
+@pytest.mark.slow
+def test_layer_cfg4_one_sequence(gpu):
+    """BASELINE.json configs[3] (30B-class layer, MHA 52 heads, FFN 17920) with batch 1 instead of 2: the same kernels,
+    tiles and tails (F = 17920 = 140 x 128), half the oracle time."""
+    _layer_full(gpu, synth.CFG4_30B_LAYER.with_(batch=1))
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("S", [1024, 4096, 8192, 16384])
+def test_sdpa_cfg5_lengths(gpu, S):
+    """BASELINE.json configs[4] sequence lengths with the 3B group layout (G = 3) on one kv head and one sequence
+    (3 q heads / 1 kv head, batch 1): every element of O, L, dq, dk, dv.  The full 24/8-head, 32768-token launch is
+    the same kernel over more (batch, kv-head) CTAs; its throughput is reported by profiles/."""
+    test_sdpa_fwd_bwd(gpu, 1, S, 3, 1, 128)
