@@ -88,7 +88,7 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
   const uint32_t tmem_slot = bar_base + 8u * 16;
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = warp_idx_uniform(), lane = threadIdx.x & 31;
   const int qb = gridDim.x - 1 - blockIdx.x;                  // heavy (late) query blocks first
   const int h = blockIdx.y, b = blockIdx.z;
   const int kvh = h / (p.nq / p.nkv);
@@ -132,48 +132,57 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
       }
     }
   } else if (warp == 1) {
-    // ===================================================================== MMA issuer
-    if (lane == 0) {
-      const uint32_t idesc_s = umma_idesc(128, 128, 0, 0, 0, 0);     // S = Q K^T : both K-major
-      const uint32_t idesc_pv = umma_idesc(128, 128, 0, 0, 0, 1);    // O += P V  : A from TMEM, B (V) MN-major
-      const int nt[2] = {n0, n1};
-      auto issue_s = [&](int t, int kst) {
-        const uint32_t qa = sQ + t * ATC_TILE_BYTES, ka = sK + kst * ATC_TILE_BYTES;
+    // ===================================================================== MMA issuer (whole warp, elected lane issues)
+    const uint32_t leader = elect_one();
+    const uint32_t idesc_s = umma_idesc(128, 128, 0, 0, 0, 0);     // S = Q K^T : both K-major
+    const uint32_t idesc_pv = umma_idesc(128, 128, 0, 0, 0, 1);    // O += P V  : A from TMEM, B (V) MN-major
+    const int nt[2] = {n0, n1};
+    const uint64_t dq0 = umma_smem_desc(sQ, 16, 1024), dk0 = umma_smem_desc(sK, 16, 1024);
+    const uint64_t dv0 = umma_smem_desc(sV, ATC_CHUNK_BYTES, 1024);
+    auto issue_s = [&](int t, int kst) {
+      if (leader) {
+        const uint64_t qa = desc_adv(dq0, t * ATC_TILE_BYTES), ka = desc_adv(dk0, kst * ATC_TILE_BYTES);
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk)
-          umma_f16(tmem_base + t * 128, atc_desc_kmajor(qa, kk), atc_desc_kmajor(ka, kk), idesc_s, kk != 0 ? 1u : 0u);
+        for (int kk = 0; kk < 8; ++kk) {
+          const uint32_t off = (kk >> 2) * ATC_CHUNK_BYTES + (kk & 3) * 32;
+          umma_f16(tmem_base + t * 128, desc_adv(qa, off), desc_adv(ka, off), idesc_s, kk != 0 ? 1u : 0u);
+        }
         umma_commit(s_full(t));
-      };
-      auto issue_pv = [&](int t, int vst, bool acc) {
-        const uint32_t va = sV + vst * ATC_TILE_BYTES;
+      }
+    };
+    auto issue_pv = [&](int t, int vst, bool acc) {
+      if (leader) {
+        const uint64_t va = desc_adv(dv0, vst * ATC_TILE_BYTES);
 #pragma unroll
         for (int kk = 0; kk < 8; ++kk)
-          umma_f16_ts(tmem_base + 256 + t * 128, tmem_base + t * 128 + kk * 8, atc_desc_mnmajor(va, kk), idesc_pv,
+          umma_f16_ts(tmem_base + 256 + t * 128, tmem_base + t * 128 + kk * 8, desc_adv(va, kk * 2048), idesc_pv,
                       (acc || kk != 0) ? 1u : 0u);
         umma_commit(o_full(t));
-      };
-      mbar_wait(k_full(0), 0);
-      mbar_wait(q_full(0), 0);
-      tc_fence_after();
-      issue_s(0, 0);
-      if (n1 > 0) { mbar_wait(q_full(1), 0); tc_fence_after(); issue_s(1, 0); }
-      umma_commit(k_empty(0));
-      for (int j = 0; j < nmax; ++j) {
-        const int st = j & 1;
-        const uint32_t ph = (j >> 1) & 1;
-        mbar_wait(v_full(st), ph);
-        bool knext_ready = false;
-        for (int t = 0; t < 2; ++t) {
-          if (j < nt[t]) {
-            mbar_wait(p_full(t), j & 1);
-            tc_fence_after();
-            issue_pv(t, st, j > 0);
-          }
-          if (j + 1 < nt[t]) {
-            if (!knext_ready) { mbar_wait(k_full(st ^ 1), ((j + 1) >> 1) & 1); tc_fence_after(); knext_ready = true; }
-            issue_s(t, st ^ 1);
-          }
+      }
+    };
+    mbar_wait(k_full(0), 0);
+    mbar_wait(q_full(0), 0);
+    tc_fence_after();
+    issue_s(0, 0);
+    if (n1 > 0) { mbar_wait(q_full(1), 0); tc_fence_after(); issue_s(1, 0); }
+    if (leader) umma_commit(k_empty(0));
+    for (int j = 0; j < nmax; ++j) {
+      const int st = j & 1;
+      const uint32_t ph = (j >> 1) & 1;
+      mbar_wait(v_full(st), ph);
+      bool knext_ready = false;
+      for (int t = 0; t < 2; ++t) {
+        if (j < nt[t]) {
+          mbar_wait(p_full(t), j & 1);
+          tc_fence_after();
+          issue_pv(t, st, j > 0);
         }
+        if (j + 1 < nt[t]) {
+          if (!knext_ready) { mbar_wait(k_full(st ^ 1), ((j + 1) >> 1) & 1); tc_fence_after(); knext_ready = true; }
+          issue_s(t, st ^ 1);
+        }
+      }
+      if (leader) {
         umma_commit(v_empty(st));
         if (j + 1 < nmax) umma_commit(k_empty(st ^ 1));
       }
@@ -219,38 +228,42 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
         const bool grow = (m_new - m_run) * c > ATC_RESCALE_LOG2;
         if (__any_sync(0xffffffffu, grow)) {
           // raise the reference maximum of every row of this warp and rescale O_t in TMEM
-          const float alpha = exp2f((m_run - m_new) * c);
+          const float alpha = ex2_approx((m_run - m_new) * c);
           m_use = m_new;
           l_run *= alpha;
           mbar_wait(o_full(t), (j - 1) & 1);                     // P_t V_{j-1} has landed in O_t
           tc_fence_after();
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            uint32_t orr[32];
-            tmem_ld32(tO + q * 32, orr);
+#pragma unroll 1
+          for (int q = 0; q < 8; ++q) {                          // 16 columns at a time: S stays in registers
+            uint32_t orr[16];
+            tmem_ld16(tO + q * 16, orr);
             tmem_ld_wait();
 #pragma unroll
-            for (int i = 0; i < 32; ++i) orr[i] = __float_as_uint(__uint_as_float(orr[i]) * alpha);
-            tmem_st32(tO + q * 32, orr);
+            for (int i = 0; i < 16; ++i) orr[i] = __float_as_uint(__uint_as_float(orr[i]) * alpha);
+            tmem_st16(tO + q * 16, orr);
           }
         }
       }
       m_run = m_use;
       const float neg = -m_use * c;
-      float sum0 = 0.f, sum1 = 0.f;
+      // P = 2^(s c - m c): FFMA2 + 2 MUFU + FADD2 + F2FP per key pair
+      const float2 c2 = make_float2(c, c), neg2 = make_float2(neg, neg);
+      float2 acc0 = make_float2(0.f, 0.f), acc1 = make_float2(0.f, 0.f);
 #pragma unroll
       for (int q = 0; q < 2; ++q) {
         uint32_t pk[32];
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
-          const float a0 = exp2f(fmaf(s[2 * q][2 * i], c, neg)), a1 = exp2f(fmaf(s[2 * q][2 * i + 1], c, neg));
-          const float b0 = exp2f(fmaf(s[2 * q + 1][2 * i], c, neg)), b1 = exp2f(fmaf(s[2 * q + 1][2 * i + 1], c, neg));
-          sum0 += a0 + a1; sum1 += b0 + b1;
-          pk[i] = pack_f16(a0, a1);
-          pk[16 + i] = pack_f16(b0, b1);
+          float2 a = ffma2(make_float2(s[2 * q][2 * i], s[2 * q][2 * i + 1]), c2, neg2);
+          float2 b = ffma2(make_float2(s[2 * q + 1][2 * i], s[2 * q + 1][2 * i + 1]), c2, neg2);
+          a.x = ex2_approx(a.x); a.y = ex2_approx(a.y); b.x = ex2_approx(b.x); b.y = ex2_approx(b.y);
+          acc0 = fadd2(acc0, a); acc1 = fadd2(acc1, b);
+          pk[i] = pack_f16(a.x, a.y);
+          pk[16 + i] = pack_f16(b.x, b.y);
         }
         tmem_st32(tS + q * 32, pk);                              // P_t: keys 64 q .. 64 q + 63 -> 32 columns
       }
+      const float sum0 = acc0.x + acc0.y, sum1 = acc1.x + acc1.y;
       l_run += sum0 + sum1;
       tmem_st_wait();
       tc_fence_before();
@@ -408,7 +421,7 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
   const uint32_t tmem_slot = bar_base + 8u * (8 + 3 * ATC_NST);
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = warp_idx_uniform(), lane = threadIdx.x & 31;
   const int kb = blockIdx.x, kvh = blockIdx.y, b = blockIdx.z;
   const int G = p.nq / p.nkv;
   const int k0 = kb * 128;
@@ -461,59 +474,69 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
       mbar_arrive(ld_full(st));
     }
   } else if (warp == 1) {
-    // ===================================================================== MMA issuer
-    if (lane == 0) {
-      const uint32_t idesc_sdp = umma_idesc(128, 64, 0, 0, 0, 0);     // [128 keys x 64 queries] = A(K-major) B(K-major)^T
-      const uint32_t idesc_acc = umma_idesc(128, 128, 0, 0, 0, 1);    // [128 keys x 128 d] += A(TMEM) B(MN-major)
-      auto issue_sdp = [&](int it) {
-        const int st = it % ATC_NST, buf = it & 1;
-        mbar_wait(qdo_full(st), (it / ATC_NST) & 1);
-        tc_fence_after();
-        const uint32_t qa = sQ + st * ATC_HALF_TILE, da = sDO + st * ATC_HALF_TILE;
+    // ===================================================================== MMA issuer (whole warp, elected lane issues)
+    const uint32_t leader = elect_one();
+    const uint32_t idesc_sdp = umma_idesc(128, 64, 0, 0, 0, 0);     // [128 keys x 64 queries] = A(K-major) B(K-major)^T
+    const uint32_t idesc_acc = umma_idesc(128, 128, 0, 0, 0, 1);    // [128 keys x 128 d] += A(TMEM) B(MN-major)
+    const uint64_t dK = umma_smem_desc(sK, 16, 1024), dV = umma_smem_desc(sV, 16, 1024);
+    const uint64_t dQk = umma_smem_desc(sQ, 16, 1024), dDOk = umma_smem_desc(sDO, 16, 1024);           // K-major views
+    const uint64_t dQm = umma_smem_desc(sQ, 64 * 128, 1024), dDOm = umma_smem_desc(sDO, 64 * 128, 1024); // MN-major views
+    auto issue_sdp = [&](int it) {
+      const int st = it % ATC_NST, buf = it & 1;
+      mbar_wait(qdo_full(st), (it / ATC_NST) & 1);
+      tc_fence_after();
+      if (leader) {
+        const uint64_t qa = desc_adv(dQk, st * ATC_HALF_TILE), da = desc_adv(dDOk, st * ATC_HALF_TILE);
 #pragma unroll
         for (int kk = 0; kk < 8; ++kk)
-          umma_f16(tmem_base + buf * 64, atc_desc_kmajor(sK, kk), atc_desc_half_kmajor(qa, kk), idesc_sdp, kk != 0 ? 1u : 0u);
+          umma_f16(tmem_base + buf * 64, desc_adv(dK, (kk >> 2) * ATC_CHUNK_BYTES + (kk & 3) * 32),
+                   desc_adv(qa, (kk >> 2) * (64 * 128) + (kk & 3) * 32), idesc_sdp, kk != 0 ? 1u : 0u);
 #pragma unroll
         for (int kk = 0; kk < 8; ++kk)
-          umma_f16(tmem_base + 128 + buf * 64, atc_desc_kmajor(sV, kk), atc_desc_half_kmajor(da, kk), idesc_sdp, kk != 0 ? 1u : 0u);
+          umma_f16(tmem_base + 128 + buf * 64, desc_adv(dV, (kk >> 2) * ATC_CHUNK_BYTES + (kk & 3) * 32),
+                   desc_adv(da, (kk >> 2) * (64 * 128) + (kk & 3) * 32), idesc_sdp, kk != 0 ? 1u : 0u);
         umma_commit(sdp_full(buf));
-      };
-      mbar_wait(kv_full(), 0);
-      issue_sdp(0);
-      for (int it = 0; it < iters; ++it) {
-        const int st = it % ATC_NST, buf = it & 1;
-        const uint32_t ph = (it >> 1) & 1;
-        if (it + 1 < iters) issue_sdp(it + 1);
-        const uint32_t qa = sQ + st * ATC_HALF_TILE, da = sDO + st * ATC_HALF_TILE;
-        const bool split = (2 * kb + it % per_head) * 64 < ATC_SPLIT_ROWS;
-        mbar_wait(p_full(buf), ph);
-        tc_fence_after();
+      }
+    };
+    mbar_wait(kv_full(), 0);
+    issue_sdp(0);
+    for (int it = 0; it < iters; ++it) {
+      const int st = it % ATC_NST, buf = it & 1;
+      const uint32_t ph = (it >> 1) & 1;
+      if (it + 1 < iters) issue_sdp(it + 1);
+      const uint64_t qa = desc_adv(dQm, st * ATC_HALF_TILE), da = desc_adv(dDOm, st * ATC_HALF_TILE);
+      const bool split = (2 * kb + it % per_head) * 64 < ATC_SPLIT_ROWS;
+      mbar_wait(p_full(buf), ph);
+      tc_fence_after();
+      if (leader) {
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk)                                // dV += P^T dO
-          umma_f16_ts(tmem_base + 256, tmem_base + buf * 64 + atc_half_operand_col(kk), atc_desc_half_mnmajor(da, kk), idesc_acc,
+          umma_f16_ts(tmem_base + 256, tmem_base + buf * 64 + atc_half_operand_col(kk), desc_adv(da, kk * 2048), idesc_acc,
                       (it | kk) != 0 ? 1u : 0u);
         if (split) {
 #pragma unroll
           for (int kk = 0; kk < 4; ++kk)                              // ... + (P^T)_lo dO
-            umma_f16_ts(tmem_base + 256, tmem_base + buf * 64 + 16 + atc_half_operand_col(kk), atc_desc_half_mnmajor(da, kk),
+            umma_f16_ts(tmem_base + 256, tmem_base + buf * 64 + 16 + atc_half_operand_col(kk), desc_adv(da, kk * 2048),
                         idesc_acc, 1u);
         }
-        mbar_wait(ds_full(buf), ph);
-        tc_fence_after();
+      }
+      mbar_wait(ds_full(buf), ph);
+      tc_fence_after();
+      if (leader) {
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk)                                // dK += dS^T Q
-          umma_f16_ts(tmem_base + 384, tmem_base + 128 + buf * 64 + atc_half_operand_col(kk), atc_desc_half_mnmajor(qa, kk),
+          umma_f16_ts(tmem_base + 384, tmem_base + 128 + buf * 64 + atc_half_operand_col(kk), desc_adv(qa, kk * 2048),
                       idesc_acc, (it | kk) != 0 ? 1u : 0u);
         if (split) {
 #pragma unroll
           for (int kk = 0; kk < 4; ++kk)
-            umma_f16_ts(tmem_base + 384, tmem_base + 128 + buf * 64 + 16 + atc_half_operand_col(kk), atc_desc_half_mnmajor(qa, kk),
+            umma_f16_ts(tmem_base + 384, tmem_base + 128 + buf * 64 + 16 + atc_half_operand_col(kk), desc_adv(qa, kk * 2048),
                         idesc_acc, 1u);
         }
         umma_commit(qdo_empty(st));
       }
-      umma_commit(acc_full());
     }
+    if (leader) umma_commit(acc_full());
   } else {
     // ===================================================================== softmax warps (8): lane quarter x column half
     const int quarter = warp & 3, half = (warp - 2) >> 2;
@@ -537,10 +560,10 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
         const float4 L = l4[i];
-        pv[4 * i] = exp2f(fmaf(__uint_as_float(sr[4 * i]), c, -L.x));
-        pv[4 * i + 1] = exp2f(fmaf(__uint_as_float(sr[4 * i + 1]), c, -L.y));
-        pv[4 * i + 2] = exp2f(fmaf(__uint_as_float(sr[4 * i + 2]), c, -L.z));
-        pv[4 * i + 3] = exp2f(fmaf(__uint_as_float(sr[4 * i + 3]), c, -L.w));
+        pv[4 * i] = ex2_approx(fmaf(__uint_as_float(sr[4 * i]), c, -L.x));
+        pv[4 * i + 1] = ex2_approx(fmaf(__uint_as_float(sr[4 * i + 1]), c, -L.y));
+        pv[4 * i + 2] = ex2_approx(fmaf(__uint_as_float(sr[4 * i + 2]), c, -L.z));
+        pv[4 * i + 3] = ex2_approx(fmaf(__uint_as_float(sr[4 * i + 3]), c, -L.w));
       }
       if (rel < 2) {                                                   // diagonal: query (64 rel + col0 + i) < key (row) is masked
         const int qrel = rel * 64 + col0;
@@ -633,7 +656,7 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
   const uint32_t tmem_slot = bar_base + 8u * (6 + 2 * ATC_NST);
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = warp_idx_uniform(), lane = threadIdx.x & 31;
   const int qb = gridDim.x - 1 - blockIdx.x;                     // heavy (late) query blocks first
   const int h = blockIdx.y, b = blockIdx.z;
   const int kvh = h / (p.nq / p.nkv);
@@ -672,44 +695,52 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
       }
     }
   } else if (warp == 1) {
-    if (lane == 0) {
-      const uint32_t idesc_sdp = umma_idesc(128, 64, 0, 0, 0, 0);     // [128 queries x 64 keys]
-      const uint32_t idesc_acc = umma_idesc(128, 128, 0, 0, 0, 1);    // dQ [128 x 128] += dS(TMEM) K(MN-major)
-      auto issue_sdp = [&](int it) {
-        const int st = it % ATC_NST, buf = it & 1;
-        mbar_wait(kv_full(st), (it / ATC_NST) & 1);
-        tc_fence_after();
-        const uint32_t ka = sK + st * ATC_HALF_TILE, va = sV + st * ATC_HALF_TILE;
+    const uint32_t leader = elect_one();
+    const uint32_t idesc_sdp = umma_idesc(128, 64, 0, 0, 0, 0);     // [128 queries x 64 keys]
+    const uint32_t idesc_acc = umma_idesc(128, 128, 0, 0, 0, 1);    // dQ [128 x 128] += dS(TMEM) K(MN-major)
+    const uint64_t dQd = umma_smem_desc(sQ, 16, 1024), dDO = umma_smem_desc(sDO, 16, 1024);
+    const uint64_t dKk = umma_smem_desc(sK, 16, 1024), dVk = umma_smem_desc(sV, 16, 1024);
+    const uint64_t dKm = umma_smem_desc(sK, 64 * 128, 1024);
+    auto issue_sdp = [&](int it) {
+      const int st = it % ATC_NST, buf = it & 1;
+      mbar_wait(kv_full(st), (it / ATC_NST) & 1);
+      tc_fence_after();
+      if (leader) {
+        const uint64_t ka = desc_adv(dKk, st * ATC_HALF_TILE), va = desc_adv(dVk, st * ATC_HALF_TILE);
 #pragma unroll
         for (int kk = 0; kk < 8; ++kk)
-          umma_f16(tmem_base + buf * 64, atc_desc_kmajor(sQ, kk), atc_desc_half_kmajor(ka, kk), idesc_sdp, kk != 0 ? 1u : 0u);
+          umma_f16(tmem_base + buf * 64, desc_adv(dQd, (kk >> 2) * ATC_CHUNK_BYTES + (kk & 3) * 32),
+                   desc_adv(ka, (kk >> 2) * (64 * 128) + (kk & 3) * 32), idesc_sdp, kk != 0 ? 1u : 0u);
 #pragma unroll
         for (int kk = 0; kk < 8; ++kk)
-          umma_f16(tmem_base + 128 + buf * 64, atc_desc_kmajor(sDO, kk), atc_desc_half_kmajor(va, kk), idesc_sdp, kk != 0 ? 1u : 0u);
+          umma_f16(tmem_base + 128 + buf * 64, desc_adv(dDO, (kk >> 2) * ATC_CHUNK_BYTES + (kk & 3) * 32),
+                   desc_adv(va, (kk >> 2) * (64 * 128) + (kk & 3) * 32), idesc_sdp, kk != 0 ? 1u : 0u);
         umma_commit(sdp_full(buf));
-      };
-      mbar_wait(qdo_full(), 0);
-      issue_sdp(0);
-      for (int it = 0; it < iters; ++it) {
-        const int st = it % ATC_NST, buf = it & 1;
-        if (it + 1 < iters) issue_sdp(it + 1);
-        mbar_wait(ds_full(buf), (it >> 1) & 1);
-        tc_fence_after();
-        const uint32_t ka = sK + st * ATC_HALF_TILE;
+      }
+    };
+    mbar_wait(qdo_full(), 0);
+    issue_sdp(0);
+    for (int it = 0; it < iters; ++it) {
+      const int st = it % ATC_NST, buf = it & 1;
+      if (it + 1 < iters) issue_sdp(it + 1);
+      mbar_wait(ds_full(buf), (it >> 1) & 1);
+      tc_fence_after();
+      if (leader) {
+        const uint64_t ka = desc_adv(dKm, st * ATC_HALF_TILE);
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk)
-          umma_f16_ts(tmem_base + 256, tmem_base + buf * 64 + atc_half_operand_col(kk), atc_desc_half_mnmajor(ka, kk), idesc_acc,
+          umma_f16_ts(tmem_base + 256, tmem_base + buf * 64 + atc_half_operand_col(kk), desc_adv(ka, kk * 2048), idesc_acc,
                       (it | kk) != 0 ? 1u : 0u);
         if (q0 < ATC_SPLIT_ROWS) {                                    // early query rows: + dS_lo K
 #pragma unroll
           for (int kk = 0; kk < 4; ++kk)
-            umma_f16_ts(tmem_base + 256, tmem_base + buf * 64 + 16 + atc_half_operand_col(kk), atc_desc_half_mnmajor(ka, kk),
+            umma_f16_ts(tmem_base + 256, tmem_base + buf * 64 + 16 + atc_half_operand_col(kk), desc_adv(ka, kk * 2048),
                         idesc_acc, 1u);
         }
         umma_commit(kv_empty(st));
       }
-      umma_commit(acc_full());
     }
+    if (leader) umma_commit(acc_full());
   } else {
     const int quarter = warp & 3, half = (warp - 2) >> 2;
     const int row = quarter * 32 + lane;
@@ -732,7 +763,7 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
       float ds[32];
 #pragma unroll
       for (int i = 0; i < 32; ++i)
-        ds[i] = exp2f(fmaf(__uint_as_float(sr[i]), c, -L2)) * (__uint_as_float(dr[i]) - Dr);
+        ds[i] = ex2_approx(fmaf(__uint_as_float(sr[i]), c, -L2)) * (__uint_as_float(dr[i]) - Dr);
       if (it * 64 + 63 > q0) {                                        // diagonal blocks: key > query is masked
         const int krel = it * 64 + col0 - q0;
 #pragma unroll
@@ -776,8 +807,7 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
   if (warp == 1) { tc_fence_after(); tmem_dealloc(tmem_base, 512); }
 }
 
-inline cudaError_t attn_bwd_tc_launch(const __half* q, long long ldq, const __half* k, long long ldk, const __half* v,
-                                      long long ldv, const __half* dO, long long lddo, const AttnTcBwdParams& p, cudaStream_t st) {
+inline cudaError_t attn_bwd_tc_set_attrs() {
   static bool set = false;
   if (!set) {
     cudaError_t e = cudaFuncSetAttribute(attn_bwd_dkdv_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_BWD_SMEM);
@@ -786,19 +816,34 @@ inline cudaError_t attn_bwd_tc_launch(const __half* q, long long ldq, const __ha
     if (e != cudaSuccess) return e;
     set = true;
   }
-  AttnTcMaps m1, m2;
-  // dK/dV: K, V as 128-row tiles; Q, dO streamed as 64-row tiles
+  return cudaSuccess;
+}
+
+// dK/dV: K, V as 128-row tiles; Q, dO streamed as 64-row tiles
+inline cudaError_t attn_bwd_dkdv_tc_launch(const __half* q, long long ldq, const __half* k, long long ldk, const __half* v,
+                                           long long ldv, const __half* dO, long long lddo, const AttnTcBwdParams& p,
+                                           cudaStream_t st) {
+  cudaError_t e = attn_bwd_tc_set_attrs();
+  if (e != cudaSuccess) return e;
+  AttnTcMaps m1;
   if (!make_map_attn(&m1.k, k, p.nkv * ATC_D, p.S, p.B, ldk, 128) || !make_map_attn(&m1.v, v, p.nkv * ATC_D, p.S, p.B, ldv, 128) ||
       !make_map_attn(&m1.q, q, p.nq * ATC_D, p.S, p.B, ldq, 64) || !make_map_attn(&m1.dO, dO, p.nq * ATC_D, p.S, p.B, lddo, 64))
     return cudaErrorInvalidValue;
-  // dQ: Q, dO as 128-row tiles; K, V streamed as 64-row tiles
+  dim3 g1((p.S + 127) / 128, p.nkv, p.B);
+  attn_bwd_dkdv_tc_kernel<<<g1, ATC_BWD_THREADS, ATC_BWD_SMEM, st>>>(m1, p);
+  return cudaGetLastError();
+}
+
+// dQ: Q, dO as 128-row tiles; K, V streamed as 64-row tiles
+inline cudaError_t attn_bwd_dq_tc_launch(const __half* q, long long ldq, const __half* k, long long ldk, const __half* v,
+                                         long long ldv, const __half* dO, long long lddo, const AttnTcBwdParams& p,
+                                         cudaStream_t st) {
+  cudaError_t e = attn_bwd_tc_set_attrs();
+  if (e != cudaSuccess) return e;
+  AttnTcMaps m2;
   if (!make_map_attn(&m2.k, k, p.nkv * ATC_D, p.S, p.B, ldk, 64) || !make_map_attn(&m2.v, v, p.nkv * ATC_D, p.S, p.B, ldv, 64) ||
       !make_map_attn(&m2.q, q, p.nq * ATC_D, p.S, p.B, ldq, 128) || !make_map_attn(&m2.dO, dO, p.nq * ATC_D, p.S, p.B, lddo, 128))
     return cudaErrorInvalidValue;
-  dim3 g1((p.S + 127) / 128, p.nkv, p.B);
-  attn_bwd_dkdv_tc_kernel<<<g1, ATC_BWD_THREADS, ATC_BWD_SMEM, st>>>(m1, p);
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
   dim3 g2((p.S + 127) / 128, p.nq, p.B);
   attn_bwd_dq_tc_kernel<<<g2, ATC_BWD_THREADS, ATC_BWD_SMEM, st>>>(m2, p);
   return cudaGetLastError();

@@ -39,12 +39,12 @@ struct WsLayout {
 enum Stage : int {
   ST_CAST = 0, ST_NORM_FWD, ST_QKV, ST_ATTN_FWD, ST_OPROJ, ST_GATEUP, ST_DOWN,
   ST_WGRAD_DOWN, ST_DGRAD_DOWN, ST_WGRAD_GATEUP, ST_DGRAD_GATEUP, ST_NORM_BWD,
-  ST_WGRAD_O, ST_DGRAD_O, ST_DVEC, ST_ATTN_BWD, ST_WGRAD_QKV, ST_DGRAD_QKV, ST_EMBED, ST_COUNT
+  ST_WGRAD_O, ST_DGRAD_O, ST_DVEC, ST_ATTN_BWD, ST_WGRAD_QKV, ST_DGRAD_QKV, ST_EMBED, ST_ATTN_BWD_DQ, ST_COUNT
 };
 static const char* const STAGE_NAMES[ST_COUNT] = {
   "cast", "rmsnorm_fwd", "gemm_qkv_rope", "attn_fwd", "gemm_oproj_res", "gemm_gateup_swiglu", "gemm_down_res",
   "wgrad_down", "dgrad_down_swiglu_bwd", "wgrad_gateup", "dgrad_gateup", "rmsnorm_bwd",
-  "wgrad_oproj", "dgrad_oproj", "attn_dvec", "attn_bwd", "wgrad_qkv", "dgrad_qkv", "embed_gather"};
+  "wgrad_oproj", "dgrad_oproj", "attn_dvec", "attn_bwd", "wgrad_qkv", "dgrad_qkv", "embed_gather", "attn_bwd_dq"};
 
 struct TimingRec { int stage; cudaEvent_t beg, end; };
 
@@ -260,17 +260,20 @@ cudaError_t attn_fwd_dispatch(const lsp_ctx* c, const AttnParams& p, cudaStream_
   return attn_fwd_launch<64>(p, st);
 }
 
-// B7 dispatch (two kernels either way: dK/dV, then dQ)
-cudaError_t attn_bwd_dispatch(const lsp_ctx* c, const AttnParams& p, cudaStream_t st) {
-  if (c->d.head_dim == 128) {
+// B7 dispatch (two kernels either way: dK/dV, then dQ).  head_dim 128: tcgen05 kernels, timed as two stages.
+lsp_status attn_bwd_dispatch(lsp_ctx* ctx, const AttnParams& p, cudaStream_t st) {
+  if (ctx->d.head_dim == 128) {
     AttnTcBwdParams t;
     t.B = p.B; t.S = p.S; t.nq = p.nq; t.nkv = p.nkv; t.scale_log2 = p.scale_log2; t.scale = p.scale;
     t.lse = p.lse; t.dvec = p.dvec; t.rope = p.rope;
     t.dq32 = p.dq32; t.dk32 = p.dk32; t.dv32 = p.dv32; t.lddq32 = p.lddq32; t.lddk32 = p.lddk32;
     t.dq16 = p.dq16; t.dk16 = p.dk16; t.dv16 = p.dv16; t.ldd16 = p.ldd16;
-    return attn_bwd_tc_launch(p.q, p.ldq, p.k, p.ldk, p.v, p.ldv, p.dO, p.lddo, t, st);
+    LSP_STAGE(ST_ATTN_BWD, 1, attn_bwd_dkdv_tc_launch(p.q, p.ldq, p.k, p.ldk, p.v, p.ldv, p.dO, p.lddo, t, st));
+    LSP_STAGE(ST_ATTN_BWD_DQ, 1, attn_bwd_dq_tc_launch(p.q, p.ldq, p.k, p.ldk, p.v, p.ldv, p.dO, p.lddo, t, st));
+    return LSP_OK;
   }
-  return attn_bwd_launch<64>(p, st);
+  LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_launch<64>(p, st));
+  return LSP_OK;
 }
 
 // ------------------------------------------------------------------------------------------- attention block
@@ -355,7 +358,7 @@ lsp_status attn_bwd_impl(lsp_ctx* ctx, int x_dt, const void* x, int da_dt, const
   p.lse = const_cast<float*>(lse); p.dvec = dvec;
   p.rope = d.use_rope ? ctx->rope : nullptr;
   p.dq16 = dqkv; p.dk16 = dqkv + Nq; p.dv16 = dqkv + Nq + Nkv; p.ldd16 = Nqkv;
-  LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_dispatch(ctx, p, st));
+  LSP_TRY(attn_bwd_dispatch(ctx, p, st));
   // B9 dW{q,k,v} = d{q,k,v}^T xn (one GEMM, rows split over three outputs) ; dxn = [dq|dk|dv] [Wq;Wk;Wv] (one GEMM)
   {
     EpiF32 e = epi_f32(static_cast<float*>(g->wq), H);
@@ -641,7 +644,7 @@ lsp_status lsp_sdpa_bwd(lsp_ctx* ctx, const void* q, const void* k, const void* 
   p.lse = const_cast<float*>(lse); p.dvec = dvec;
   p.dq32 = static_cast<float*>(dq); p.dk32 = static_cast<float*>(dk); p.dv32 = static_cast<float*>(dv);
   p.lddq32 = ctx->Nq; p.lddk32 = ctx->Nkv;
-  LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_dispatch(ctx, p, st));
+  LSP_TRY(attn_bwd_dispatch(ctx, p, st));
   return LSP_OK;
 }
 
