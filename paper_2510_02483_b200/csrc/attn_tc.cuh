@@ -344,7 +344,7 @@ constexpr int ATC_BWD_THREADS = 320;
 // early rows are O(1) while the tensor-wide rms the parity metric divides by shrinks like sqrt(ln S / S), so a
 // single fp16 rounding there is what limits dq/dk/dv at long S (P-5/P-6).
 constexpr int ATC_SPLIT_ROWS = 256;
-constexpr int ATC_NST = 3;                                 // stages of the streamed 64-row tiles
+constexpr int ATC_NST = 4;                                 // stages of the streamed 64-row tiles
 constexpr int ATC_HALF_TILE = 64 * ATC_D * 2;              // 64 x 128 fp16 = 16 KB (two 8 KB chunks)
 constexpr int ATC_BWD_SMEM = 2 * ATC_TILE_BYTES + 2 * ATC_NST * ATC_HALF_TILE + ATC_NST * 2 * 64 * 4 + 1024 + 256;
 
@@ -488,13 +488,12 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
       if (leader) {
         const uint64_t qa = desc_adv(dQk, st * ATC_HALF_TILE), da = desc_adv(dDOk, st * ATC_HALF_TILE);
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk)
+        for (int kk = 0; kk < 8; ++kk) {                              // two independent accumulation chains, interleaved
           umma_f16(tmem_base + buf * 64, desc_adv(dK, (kk >> 2) * ATC_CHUNK_BYTES + (kk & 3) * 32),
                    desc_adv(qa, (kk >> 2) * (64 * 128) + (kk & 3) * 32), idesc_sdp, kk != 0 ? 1u : 0u);
-#pragma unroll
-        for (int kk = 0; kk < 8; ++kk)
           umma_f16(tmem_base + 128 + buf * 64, desc_adv(dV, (kk >> 2) * ATC_CHUNK_BYTES + (kk & 3) * 32),
                    desc_adv(da, (kk >> 2) * (64 * 128) + (kk & 3) * 32), idesc_sdp, kk != 0 ? 1u : 0u);
+        }
         umma_commit(sdp_full(buf));
       }
     };
@@ -639,21 +638,29 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
 }
 
 // --------------------------------------------------------------------------------------------- dQ
+// Three S / dP accumulator buffers (TMEM: S [0,192), dP [192,384), dQ [384,512)) and four K/V stages: the tensor core
+// works two key blocks ahead of the softmax threads, so the commit -> mbarrier -> tcgen05.ld round trip (~800 cycles
+// measured) is off the critical path.
+constexpr int ATC_DQ_NB = 3;
+constexpr int ATC_DQ_NST = 5;
+constexpr int ATC_DQ_SMEM = 2 * ATC_TILE_BYTES + 2 * ATC_DQ_NST * ATC_HALF_TILE + 1024 + 256;
+constexpr int ATC_DQ_DP = 64 * ATC_DQ_NB;        // first dP column
+constexpr int ATC_DQ_ACC = 2 * 64 * ATC_DQ_NB;   // dQ accumulator column
 __global__ void __launch_bounds__(ATC_BWD_THREADS, 1)
 attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdParams p) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = smem_base, sDO = sQ + ATC_TILE_BYTES;
-  const uint32_t sK = sDO + ATC_TILE_BYTES;                      // ATC_NST stages of 64 keys x 128
-  const uint32_t sV = sK + ATC_NST * ATC_HALF_TILE;
-  const uint32_t bar_base = sV + ATC_NST * ATC_HALF_TILE;
+  const uint32_t sK = sDO + ATC_TILE_BYTES;                      // ATC_DQ_NST stages of 64 keys x 128
+  const uint32_t sV = sK + ATC_DQ_NST * ATC_HALF_TILE;
+  const uint32_t bar_base = sV + ATC_DQ_NST * ATC_HALF_TILE;
   auto qdo_full = [&]() { return bar_base; };
   auto acc_full = [&]() { return bar_base + 8u; };
   auto kv_full = [&](int s) { return bar_base + 8u * (2 + s); };
-  auto kv_empty = [&](int s) { return bar_base + 8u * (2 + ATC_NST + s); };
-  auto sdp_full = [&](int s) { return bar_base + 8u * (2 + 2 * ATC_NST + s); };
-  auto ds_full = [&](int s) { return bar_base + 8u * (4 + 2 * ATC_NST + s); };
-  const uint32_t tmem_slot = bar_base + 8u * (6 + 2 * ATC_NST);
+  auto kv_empty = [&](int s) { return bar_base + 8u * (2 + ATC_DQ_NST + s); };
+  auto sdp_full = [&](int s) { return bar_base + 8u * (2 + 2 * ATC_DQ_NST + s); };
+  auto ds_full = [&](int s) { return bar_base + 8u * (2 + ATC_DQ_NB + 2 * ATC_DQ_NST + s); };
+  const uint32_t tmem_slot = bar_base + 8u * (2 + 2 * ATC_DQ_NB + 2 * ATC_DQ_NST);
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
   const int warp = warp_idx_uniform(), lane = threadIdx.x & 31;
@@ -667,8 +674,8 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
   if (threadIdx.x == 0) {
     tma_prefetch_desc(&maps.q); tma_prefetch_desc(&maps.k); tma_prefetch_desc(&maps.v); tma_prefetch_desc(&maps.dO);
     mbar_init(qdo_full(), 1); mbar_init(acc_full(), 1);
-    for (int i = 0; i < ATC_NST; ++i) { mbar_init(kv_full(i), 1); mbar_init(kv_empty(i), 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(sdp_full(i), 1); mbar_init(ds_full(i), 8); }
+    for (int i = 0; i < ATC_DQ_NST; ++i) { mbar_init(kv_full(i), 1); mbar_init(kv_empty(i), 1); }
+    for (int i = 0; i < ATC_DQ_NB; ++i) { mbar_init(sdp_full(i), 1); mbar_init(ds_full(i), 8); }
     fence_barrier_init();
   }
   if (warp == 1) { tmem_alloc(tmem_slot, 512); tmem_relinquish(); }
@@ -685,8 +692,8 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
       tma_load_3d(sDO, &maps.dO, qdo_full(), h * ATC_D, q0, b);
       tma_load_3d(sDO + ATC_CHUNK_BYTES, &maps.dO, qdo_full(), h * ATC_D + 64, q0, b);
       for (int it = 0; it < iters; ++it) {
-        const int st = it % ATC_NST;
-        mbar_wait(kv_empty(st), ((it / ATC_NST) & 1) ^ 1u);
+        const int st = it % ATC_DQ_NST;
+        mbar_wait(kv_empty(st), ((it / ATC_DQ_NST) & 1) ^ 1u);
         mbar_expect_tx(kv_full(st), 2 * ATC_HALF_TILE);
         tma_load_3d(sK + st * ATC_HALF_TILE, &maps.k, kv_full(st), kvh * ATC_D, it * 64, b);
         tma_load_3d(sK + st * ATC_HALF_TILE + 64 * 128, &maps.k, kv_full(st), kvh * ATC_D + 64, it * 64, b);
@@ -702,39 +709,39 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
     const uint64_t dKk = umma_smem_desc(sK, 16, 1024), dVk = umma_smem_desc(sV, 16, 1024);
     const uint64_t dKm = umma_smem_desc(sK, 64 * 128, 1024);
     auto issue_sdp = [&](int it) {
-      const int st = it % ATC_NST, buf = it & 1;
-      mbar_wait(kv_full(st), (it / ATC_NST) & 1);
+      const int st = it % ATC_DQ_NST, buf = it % ATC_DQ_NB;
+      mbar_wait(kv_full(st), (it / ATC_DQ_NST) & 1);
       tc_fence_after();
       if (leader) {
         const uint64_t ka = desc_adv(dKk, st * ATC_HALF_TILE), va = desc_adv(dVk, st * ATC_HALF_TILE);
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk)
+        for (int kk = 0; kk < 8; ++kk) {                              // two independent accumulation chains, interleaved
           umma_f16(tmem_base + buf * 64, desc_adv(dQd, (kk >> 2) * ATC_CHUNK_BYTES + (kk & 3) * 32),
                    desc_adv(ka, (kk >> 2) * (64 * 128) + (kk & 3) * 32), idesc_sdp, kk != 0 ? 1u : 0u);
-#pragma unroll
-        for (int kk = 0; kk < 8; ++kk)
-          umma_f16(tmem_base + 128 + buf * 64, desc_adv(dDO, (kk >> 2) * ATC_CHUNK_BYTES + (kk & 3) * 32),
+          umma_f16(tmem_base + ATC_DQ_DP + buf * 64, desc_adv(dDO, (kk >> 2) * ATC_CHUNK_BYTES + (kk & 3) * 32),
                    desc_adv(va, (kk >> 2) * (64 * 128) + (kk & 3) * 32), idesc_sdp, kk != 0 ? 1u : 0u);
+        }
         umma_commit(sdp_full(buf));
       }
     };
     mbar_wait(qdo_full(), 0);
     issue_sdp(0);
+    if (iters > 1) issue_sdp(1);
     for (int it = 0; it < iters; ++it) {
-      const int st = it % ATC_NST, buf = it & 1;
-      if (it + 1 < iters) issue_sdp(it + 1);
-      mbar_wait(ds_full(buf), (it >> 1) & 1);
+      const int st = it % ATC_DQ_NST, buf = it % ATC_DQ_NB;
+      if (it + 2 < iters) issue_sdp(it + 2);           // its buffers were released by dQ(it - 1), already issued
+      mbar_wait(ds_full(buf), (it / ATC_DQ_NB) & 1);
       tc_fence_after();
       if (leader) {
         const uint64_t ka = desc_adv(dKm, st * ATC_HALF_TILE);
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk)
-          umma_f16_ts(tmem_base + 256, tmem_base + buf * 64 + atc_half_operand_col(kk), desc_adv(ka, kk * 2048), idesc_acc,
+          umma_f16_ts(tmem_base + ATC_DQ_ACC, tmem_base + buf * 64 + atc_half_operand_col(kk), desc_adv(ka, kk * 2048), idesc_acc,
                       (it | kk) != 0 ? 1u : 0u);
         if (q0 < ATC_SPLIT_ROWS) {                                    // early query rows: + dS_lo K
 #pragma unroll
           for (int kk = 0; kk < 4; ++kk)
-            umma_f16_ts(tmem_base + 256, tmem_base + buf * 64 + 16 + atc_half_operand_col(kk), desc_adv(ka, kk * 2048),
+            umma_f16_ts(tmem_base + ATC_DQ_ACC, tmem_base + buf * 64 + 16 + atc_half_operand_col(kk), desc_adv(ka, kk * 2048),
                         idesc_acc, 1u);
         }
         umma_commit(kv_empty(st));
@@ -753,12 +760,12 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
     const float L2 = valid ? p.lse[vidx] * 1.4426950408889634f : INFINITY;
     const float Dr = valid ? p.dvec[vidx] : 0.f;
     for (int it = 0; it < iters; ++it) {
-      const int buf = it & 1;
-      mbar_wait(sdp_full(buf), (it >> 1) & 1);
+      const int buf = it % ATC_DQ_NB;
+      mbar_wait(sdp_full(buf), (it / ATC_DQ_NB) & 1);
       tc_fence_after();
       uint32_t sr[32], dr[32];
       tmem_ld32(tmem_base + lane_off + buf * 64 + col0, sr);
-      tmem_ld32(tmem_base + lane_off + 128 + buf * 64 + col0, dr);
+      tmem_ld32(tmem_base + lane_off + ATC_DQ_DP + buf * 64 + col0, dr);
       tmem_ld_wait();
       float ds[32];
 #pragma unroll
@@ -793,7 +800,7 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
     for (int q = 0; q < 2; ++q) {
       const int cc = half * 64 + q * 32;
       uint32_t a[32];
-      tmem_ld32(tmem_base + lane_off + 256 + cc, a);
+      tmem_ld32(tmem_base + lane_off + ATC_DQ_ACC + cc, a);
       tmem_ld_wait();
       if (valid)
         atc_store_grad32(reinterpret_cast<float(&)[32]>(a), p.scale, p.rope ? p.rope + static_cast<long long>(qi) * 64 + (cc >> 1) : nullptr,
@@ -812,7 +819,7 @@ inline cudaError_t attn_bwd_tc_set_attrs() {
   if (!set) {
     cudaError_t e = cudaFuncSetAttribute(attn_bwd_dkdv_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_BWD_SMEM);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(attn_bwd_dq_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_BWD_SMEM);
+    e = cudaFuncSetAttribute(attn_bwd_dq_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_DQ_SMEM);
     if (e != cudaSuccess) return e;
     set = true;
   }
@@ -845,7 +852,7 @@ inline cudaError_t attn_bwd_dq_tc_launch(const __half* q, long long ldq, const _
       !make_map_attn(&m2.q, q, p.nq * ATC_D, p.S, p.B, ldq, 128) || !make_map_attn(&m2.dO, dO, p.nq * ATC_D, p.S, p.B, lddo, 128))
     return cudaErrorInvalidValue;
   dim3 g2((p.S + 127) / 128, p.nq, p.B);
-  attn_bwd_dq_tc_kernel<<<g2, ATC_BWD_THREADS, ATC_BWD_SMEM, st>>>(m2, p);
+  attn_bwd_dq_tc_kernel<<<g2, ATC_BWD_THREADS, ATC_DQ_SMEM, st>>>(m2, p);
   return cudaGetLastError();
 }
 
