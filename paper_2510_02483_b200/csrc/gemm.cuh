@@ -46,6 +46,11 @@ struct GemmShape {
   int nseg;                          // number of K segments (non-DUAL); DUAL uses a[0], b[0], b[1]
   int band;                          // m-blocks per rasterisation band (>= 1)
   int kblocks[GEMM_MAX_SEG];         // ceil(K_s / 64)
+  // stream-K tail of the CTA-pair kernel (all zero / null: data-parallel only)
+  int sk_split;                      // s >= 2: the T mod C tiles of the last wave are each cut into s K-slices (0: off)
+  float* sk_partial;                 // [clusters][2 CTAs][8 chunks][128 rows][32] fp32 partial accumulators
+  unsigned int* sk_flags;            // [clusters][2]: epoch of the partial last published by that CTA
+  unsigned int sk_epoch;             // unique per launch on this context, > 0
 };
 
 template <int BN> struct GemmCfg {
@@ -115,6 +120,20 @@ __device__ __forceinline__ void load_row32(const void* p, float (&v)[32], int nv
       }
     }
   }
+}
+
+// 32 fp32 values written by ANOTHER CTA during this kernel (stream-K partials): plain coherent loads, never ld.global.nc
+__device__ __forceinline__ void load_row32_coherent(const float* p, float (&v)[32]) {
+  const volatile float4* q = reinterpret_cast<const volatile float4*>(p);
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    float4 t;
+    asm volatile("ld.global.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(t.x), "=f"(t.y), "=f"(t.z), "=f"(t.w) : "l"(q + j) : "memory");
+    v[4 * j] = t.x; v[4 * j + 1] = t.y; v[4 * j + 2] = t.z; v[4 * j + 3] = t.w;
+  }
+}
+__device__ __forceinline__ void named_bar_sync_gemm(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
 // ------------------------------------------------------------------------------------------- epilogues
@@ -383,7 +402,7 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, c
 // ------------------------------------------------------------------------------------------- the CTA-pair kernel
 // Same pipeline on a pair of CTAs (cluster of 2 = two SMs of one TPC) working on one 256 x 256 tile with
 // tcgen05.mma.cta_group::2: CTA r of the pair stages rows [128 r, +128) of the A tile and rows [128 r, +128) of the
-// B tile (32 KB per stage instead of 48 KB, so 6 stages fit), the leader's single MMA thread issues one
+// B tile (32 KB per stage instead of 48 KB, so 6 stages fit), the leader's MMA warp issues one
 // 256 x 256 x 16 instruction that reads both CTAs' shared memory, and CTA r's TMEM receives output rows [128 r, +128).
 // Halving the B traffic per SM takes the shared-memory port off the critical path (128 x 256 per SM needs
 // 96 B/clk of operand reads + 96 B/clk of TMA writes with cta_group::1, 64 + 64 with the pair).
@@ -393,9 +412,59 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, c
 //   tfull[a]  : one per CTA (multicast commit); tempty[a]: leader's, 16 arrivals (8 epilogue warps x 2 CTAs, remote)
 // DUAL: CTA 0 stages the gate rows and CTA 1 the up rows of the same 128 output columns, so the pair's N = 256
 // accumulator is [gate | up] exactly as in the single-CTA kernel.
+//
+// Split-K tail (deterministic).  With T tiles on C = 74 persistent pairs the last wave is r = T mod C tiles wide:
+// 5-25 % of the machine idles at the layer's shapes (768 tiles = 10.4 waves, 240 = 3.2).  The full waves are walked
+// whole (tile = pair + i C: the tiles in flight form a compact band and advance through K in lockstep, so every
+// operand k-slice is fetched from DRAM once and shared through L2).  Each of the r leftover tiles is cut into
+// s = min(4, floor(C / r)) K-slices, slice j of tile t going to pair j r + t: one round, s r <= C pairs busy for 1/s
+// of a tile time instead of r pairs for a whole one.  Pairs with the same j sweep the same k range at the same time,
+// which keeps the L2 sharing (contiguous per-pair k ranges that wrap across tiles -- classic stream-K -- do not: they
+// ran DRAM-bound, 10 % slower at K = 16384).  Slices j < s - 1 store their raw fp32 accumulator to sk_partial[pair]
+// and publish sk_flags[pair] = epoch; slice s - 1 waits for those flags, adds the partials in the fixed order
+// j = 0 .. s - 2 to its own accumulator and runs the fused epilogue.  Results are bit-reproducible; no atomics on data.
 constexpr int GEMM2_STAGES = 6;
 constexpr int GEMM2_STAGE_BYTES = 2 * GEMM_BM * GEMM_BK * 2;         // A 128 x 64 + B 128 x 64 (fp16) per CTA
 constexpr int GEMM2_SMEM_BYTES = GEMM2_STAGES * GEMM2_STAGE_BYTES + 1024 + 256;
+constexpr int GEMM2_PARTIAL_FLOATS = 2 * GEMM_BM * 256;               // per pair: 256 rows x 256 accumulator columns
+constexpr int GEMM2_MAX_SPLIT = 4;
+
+struct GemmItem { int tile, kb0, kb1, mode; };   // mode 0: whole tile; 1: K-slice that publishes a partial; 2: last K-slice
+
+// Work list of pair `cid` (identical in every role of both CTAs): its data-parallel tiles, then at most one K-slice.
+struct GemmWork {
+  int cid, nclusters, n_dp, has_piece, rem, split;
+  GemmItem piece;
+  __device__ __forceinline__ void init(int cid_, int nclusters_, int ntiles, int split_, int kbt) {
+    cid = cid_; nclusters = nclusters_; split = split_; has_piece = 0;
+    rem = ntiles % nclusters;
+    if (split >= 2 && rem > 0) {
+      const int dp_tiles = ntiles - rem;
+      n_dp = dp_tiles / nclusters;
+      if (cid < split * rem) {
+        const int j = cid / rem, t = cid - j * rem;
+        piece = GemmItem{dp_tiles + t, j * kbt / split, (j + 1) * kbt / split, j == split - 1 ? 2 : 1};
+        has_piece = 1;
+      }
+    } else {
+      n_dp = ntiles > cid ? (ntiles - cid + nclusters - 1) / nclusters : 0;
+    }
+  }
+  __device__ __forceinline__ int count() const { return n_dp + has_piece; }
+  __device__ __forceinline__ GemmItem get(int j) const {
+    if (j < n_dp) return GemmItem{cid + j * nclusters, 0, 0x7fffffff, 0};
+    return piece;
+  }
+};
+
+__device__ __forceinline__ unsigned int ld_acquire_gpu(const unsigned int* p) {
+  unsigned int v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_gpu(unsigned int* p, unsigned int v) {
+  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
 
 template <bool A_MN, bool B_MN, bool DUAL, class Epi>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEMM_THREADS, 1)
@@ -416,7 +485,7 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
   const uint32_t tmem_slot = bar_base + 8u * (2 * STAGES + 4);
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
-  const int warp = threadIdx.x >> 5;
+  const int warp = warp_idx_uniform();
   const int lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
   const int cid = blockIdx.x >> 1, nclusters = gridDim.x >> 1;
@@ -424,12 +493,13 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
   const int mblocks = (sh.M + 2 * GEMM_BM - 1) / (2 * GEMM_BM);      // 256-row blocks
   const int nblocks = (sh.N + NOUT - 1) / NOUT;
   const int ntiles = mblocks * nblocks;
-  int kb_total = 0;
-  const int nseg = DUAL ? 1 : sh.nseg;
-  for (int s = 0; s < nseg; ++s) kb_total += sh.kblocks[s];
+  const int kb_total = sh.kblocks[0];
+  GemmWork work;
+  work.init(cid, nclusters, ntiles, sh.sk_partial ? sh.sk_split : 0, kb_total);
+  const int nitems = work.count();
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < nseg; ++s) { tma_prefetch_desc(&maps.a[s]); tma_prefetch_desc(&maps.b[s]); }
+    tma_prefetch_desc(&maps.a[0]); tma_prefetch_desc(&maps.b[0]);
     if (DUAL) tma_prefetch_desc(&maps.b[1]);
     for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
     for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 2 * GEMM_EPI_WARPS); }
@@ -447,66 +517,68 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
   if (warp == 0) {
     // ===================================================================== TMA producer (both CTAs)
     if (lane == 0) {
+      const CUtensorMap* bmap = DUAL ? &maps.b[rank] : &maps.b[0];
       int stage = 0; uint32_t phase = 0;
-      for (int tile = cid; tile < ntiles; tile += nclusters) {
+      for (int j = 0; j < nitems; ++j) {
+        const GemmItem it = work.get(j);
         int mb, nb;
-        gemm_tile_coord(tile, mblocks, nblocks, sh.band, mb, nb);
+        gemm_tile_coord(it.tile, mblocks, nblocks, sh.band, mb, nb);
         const int m0 = mb * 2 * GEMM_BM + static_cast<int>(rank) * GEMM_BM;
         const int n0 = nb * NOUT;
         const int nb0 = DUAL ? n0 : n0 + static_cast<int>(rank) * 128;         // this CTA's B rows
-        for (int s = 0; s < nseg; ++s) {
-          const CUtensorMap* bmap = DUAL ? &maps.b[rank] : &maps.b[s];
-          for (int kb = 0; kb < sh.kblocks[s]; ++kb) {
-            mbar_wait(empty_bar(stage), phase ^ 1u);
-            const uint32_t sa = smem_base + stage * GEMM2_STAGE_BYTES;
-            const uint32_t sb = sa + A_BYTES;
-            const uint32_t fb = mapa_shared(full_bar(stage), 0);
-            if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * GEMM2_STAGE_BYTES);
-            const int k0 = kb * GEMM_BK;
-            if constexpr (!A_MN) {
-              tma_load_2d_pair(sa, &maps.a[s], fb, k0, m0);
-            } else {
+        const int kb1 = min(it.kb1, kb_total);
+        for (int kb = it.kb0; kb < kb1; ++kb) {
+          mbar_wait(empty_bar(stage), phase ^ 1u);
+          const uint32_t sa = smem_base + stage * GEMM2_STAGE_BYTES;
+          const uint32_t sb = sa + A_BYTES;
+          const uint32_t fb = mapa_shared(full_bar(stage), 0);
+          if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * GEMM2_STAGE_BYTES);
+          const int k0 = kb * GEMM_BK;
+          if constexpr (!A_MN) {
+            tma_load_2d_pair(sa, &maps.a[0], fb, k0, m0);
+          } else {
 #pragma unroll
-              for (int c = 0; c < 2; ++c) tma_load_2d_pair(sa + c * (GEMM_BK * 128), &maps.a[s], fb, m0 + 64 * c, k0);
-            }
-            if constexpr (!B_MN) {
-              tma_load_2d_pair(sb, bmap, fb, k0, nb0);
-            } else {
-#pragma unroll
-              for (int c = 0; c < 2; ++c) tma_load_2d_pair(sb + c * (GEMM_BK * 128), bmap, fb, nb0 + 64 * c, k0);
-            }
-            if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+            for (int c = 0; c < 2; ++c) tma_load_2d_pair(sa + c * (GEMM_BK * 128), &maps.a[0], fb, m0 + 64 * c, k0);
           }
+          if constexpr (!B_MN) {
+            tma_load_2d_pair(sb, bmap, fb, k0, nb0);
+          } else {
+#pragma unroll
+            for (int c = 0; c < 2; ++c) tma_load_2d_pair(sb + c * (GEMM_BK * 128), bmap, fb, nb0 + 64 * c, k0);
+          }
+          if (++stage == STAGES) { stage = 0; phase ^= 1u; }
         }
       }
     }
   } else if (warp == 1) {
-    // ===================================================================== MMA issuer (leader CTA only)
-    if (lane == 0 && rank == 0) {
+    // ===================================================================== MMA issuer (leader CTA; whole warp, elected lane)
+    if (rank == 0) {
+      const uint32_t leader = elect_one();
       const uint32_t idesc = umma_idesc(2 * GEMM_BM, BN, sh.a_fmt, sh.b_fmt, A_MN ? 1 : 0, B_MN ? 1 : 0);
       constexpr uint32_t A_LBO = A_MN ? GEMM_BK * 128 : 16, B_LBO = B_MN ? GEMM_BK * 128 : 16;
       constexpr uint32_t A_KSTEP = A_MN ? 2048 : 32, B_KSTEP = B_MN ? 2048 : 32;
+      const uint64_t da0 = umma_smem_desc(smem_base, A_LBO, 1024), db0 = umma_smem_desc(smem_base + A_BYTES, B_LBO, 1024);
       int stage = 0; uint32_t phase = 0;
       int acc = 0; uint32_t acc_phase = 0;
-      for (int tile = cid; tile < ntiles; tile += nclusters) {
+      for (int j = 0; j < nitems; ++j) {
+        const GemmItem it = work.get(j);
         mbar_wait_cluster(tempty_bar(acc), acc_phase ^ 1u);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(acc * BN);
-        for (int kb = 0; kb < kb_total; ++kb) {
+        const int kb1 = min(it.kb1, kb_total);
+        for (int kb = it.kb0; kb < kb1; ++kb) {
           mbar_wait_cluster(full_bar(stage), phase);
           tc_fence_after();
-          const uint32_t sa = smem_base + stage * GEMM2_STAGE_BYTES;
-          const uint32_t sb = sa + A_BYTES;
+          if (leader) {
+            const uint64_t da = desc_adv(da0, stage * GEMM2_STAGE_BYTES), db = desc_adv(db0, stage * GEMM2_STAGE_BYTES);
 #pragma unroll
-          for (int k = 0; k < GEMM_BK / 16; ++k) {
-            const uint64_t ad = umma_smem_desc(sa + k * A_KSTEP, A_LBO, 1024);
-            const uint64_t bd = umma_smem_desc(sb + k * B_KSTEP, B_LBO, 1024);
-            umma_f16_pair(d_tmem, ad, bd, idesc, (kb | k) != 0 ? 1u : 0u);
+            for (int k = 0; k < GEMM_BK / 16; ++k)
+              umma_f16_pair(d_tmem, desc_adv(da, k * A_KSTEP), desc_adv(db, k * B_KSTEP), idesc, (kb != it.kb0 || k != 0) ? 1u : 0u);
+            umma_commit_pair(empty_bar(stage), 3);
           }
-          umma_commit_pair(empty_bar(stage), 3);
           if (++stage == STAGES) { stage = 0; phase ^= 1u; }
         }
-        umma_commit_pair(tfull_bar(acc), 3);
+        if (leader) umma_commit_pair(tfull_bar(acc), 3);
         if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
       }
     }
@@ -514,16 +586,36 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
     // ===================================================================== epilogue warps (2..9, both CTAs)
     const int quarter = warp & 3;
     const int half = (warp - 2) >> 2;
+    const int row = quarter * 32 + lane;                                  // accumulator row of this thread = TMEM lane
     const uint32_t tempty_leader0 = mapa_shared(tempty_bar(0), 0), tempty_leader1 = mapa_shared(tempty_bar(1), 0);
+    float* const my_partial = sh.sk_partial ? sh.sk_partial + (static_cast<size_t>(cid) * 2 + rank) * (GEMM_BM * 256) : nullptr;
+    // partial of K-slice jj of the tile whose last slice this pair owns: published by pair jj * rem + (cid mod rem)
+    const int t_sk = work.rem > 0 ? cid % work.rem : 0;
+    auto slice_partial = [&](int jj) -> const float* {
+      return sh.sk_partial + (static_cast<size_t>(jj * work.rem + t_sk) * 2 + rank) * (GEMM_BM * 256);
+    };
     int acc = 0; uint32_t acc_phase = 0;
-    for (int tile = cid; tile < ntiles; tile += nclusters) {
+    for (int j = 0; j < nitems; ++j) {
+      const GemmItem it = work.get(j);
       int mb, nb;
-      gemm_tile_coord(tile, mblocks, nblocks, sh.band, mb, nb);
+      gemm_tile_coord(it.tile, mblocks, nblocks, sh.band, mb, nb);
       const int m0 = mb * 2 * GEMM_BM + static_cast<int>(rank) * GEMM_BM;
       const int n0 = nb * NOUT;
+      if (it.mode == 2) {                       // the other slices of this tile run at the same time: wait for their partials
+        for (int jj = 0; jj < work.split - 1; ++jj) {
+          const unsigned int* f = sh.sk_flags + (jj * work.rem + t_sk) * 2 + rank;
+          long long t0 = 0; uint32_t polls = 0;
+          while (ld_acquire_gpu(f) != sh.sk_epoch) {
+            if ((++polls & 0xFFFu) == 0) {
+              const long long t = clock64();
+              if (t0 == 0) t0 = t; else if (t - t0 > LSP_WAIT_LIMIT_CYCLES) __trap();
+            }
+          }
+        }
+      }
       mbar_wait_cluster(tfull_bar(acc), acc_phase);
       tc_fence_after();
-      const int m = m0 + quarter * 32 + lane;
+      const int m = m0 + row;
       const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + static_cast<uint32_t>(acc * BN);
 #pragma unroll 1
       for (int c = half; c < NOUT / 32; c += 2) {
@@ -536,15 +628,62 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
           uint32_t r1[32];
           tmem_ld32(t_row + NOUT + c * 32, r1);
           tmem_ld_wait();
-          if (m < sh.M) epi(m, n, reinterpret_cast<float(&)[32]>(r0), reinterpret_cast<float(&)[32]>(r1), nvalid);
+          float (&v0)[32] = reinterpret_cast<float(&)[32]>(r0);
+          float (&v1)[32] = reinterpret_cast<float(&)[32]>(r1);
+          if (it.mode == 1) {
+            store_row32<DT_F32>(my_partial + (static_cast<size_t>(c) * GEMM_BM + row) * 32, v0, 32);
+            store_row32<DT_F32>(my_partial + (static_cast<size_t>(NOUT / 32 + c) * GEMM_BM + row) * 32, v1, 32);
+          } else {
+            if (it.mode == 2) {
+              float s0[32], s1[32];
+#pragma unroll
+              for (int q = 0; q < 32; ++q) { s0[q] = 0.f; s1[q] = 0.f; }
+              for (int jj = 0; jj < work.split - 1; ++jj) {                    // fixed order: slice 0, 1, ..., then ours
+                float p0[32], p1[32];
+                const float* pp = slice_partial(jj);
+                load_row32_coherent(pp + (static_cast<size_t>(c) * GEMM_BM + row) * 32, p0);
+                load_row32_coherent(pp + (static_cast<size_t>(NOUT / 32 + c) * GEMM_BM + row) * 32, p1);
+#pragma unroll
+                for (int q = 0; q < 32; ++q) { s0[q] += p0[q]; s1[q] += p1[q]; }
+              }
+#pragma unroll
+              for (int q = 0; q < 32; ++q) { v0[q] += s0[q]; v1[q] += s1[q]; }
+            }
+            if (m < sh.M) epi(m, n, v0, v1, nvalid);
+          }
         } else {
           tmem_ld_wait();
-          if (m < sh.M) epi(m, n, reinterpret_cast<float(&)[32]>(r0), nvalid);
+          float (&v0)[32] = reinterpret_cast<float(&)[32]>(r0);
+          if (it.mode == 1) {
+            store_row32<DT_F32>(my_partial + (static_cast<size_t>(c) * GEMM_BM + row) * 32, v0, 32);
+          } else {
+            if (it.mode == 2) {
+              float s0[32];
+#pragma unroll
+              for (int q = 0; q < 32; ++q) s0[q] = 0.f;
+              for (int jj = 0; jj < work.split - 1; ++jj) {                    // fixed order: slice 0, 1, ..., then ours
+                float p0[32];
+                load_row32_coherent(slice_partial(jj) + (static_cast<size_t>(c) * GEMM_BM + row) * 32, p0);
+#pragma unroll
+                for (int q = 0; q < 32; ++q) s0[q] += p0[q];
+              }
+#pragma unroll
+              for (int q = 0; q < 32; ++q) v0[q] += s0[q];
+            }
+            if (m < sh.M) epi(m, n, v0, nvalid);
+          }
         }
       }
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive_cluster(acc == 0 ? tempty_leader0 : tempty_leader1);
+      if (it.mode == 1) {                       // all 8 epilogue warps of this CTA have stored: publish
+        named_bar_sync_gemm(1, GEMM_EPI_WARPS * 32);
+        if (warp == 2 && lane == 0) {
+          __threadfence();
+          st_release_gpu(sh.sk_flags + cid * 2 + rank, sh.sk_epoch);
+        }
+      }
       if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
     }
   }
@@ -556,6 +695,7 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
     tmem_dealloc_pair(tmem_base, 512);
   }
 }
+
 
 // ------------------------------------------------------------------------------------------- host side
 typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -627,8 +767,24 @@ inline bool gemm_use_pair(int M) {
   return mode != 0 && M > GEMM_BM;
 }
 
+// Context-owned resources of the stream-K tail (lsp_create allocates them; null -> data-parallel tiles only).
+struct GemmSKRes {
+  float* partial;            // [num_sms / 2][GEMM2_PARTIAL_FLOATS]
+  unsigned int* flags;       // [num_sms / 2][2], zero-initialised once
+  unsigned int epoch;        // unique (> 0) per launch
+};
+inline bool gemm_use_streamk() {
+  static int mode = -1;
+  if (mode < 0) {
+    const char* e = getenv("LSP_GEMM_STREAMK");
+    mode = e ? atoi(e) : 1;
+  }
+  return mode != 0;
+}
+
 template <bool A_MN, bool B_MN, bool DUAL, class Epi>
-cudaError_t launch_gemm_pair(const GemmMaps& maps, GemmShape sh, const Epi& epi, int num_sms, cudaStream_t st) {
+cudaError_t launch_gemm_pair(const GemmMaps& maps, GemmShape sh, const Epi& epi, int num_sms, cudaStream_t st,
+                             const GemmSKRes* sk) {
   auto kern = gemm_pair_tcgen05_kernel<A_MN, B_MN, DUAL, Epi>;
   static bool attr_set = false;
   if (!attr_set) {
@@ -643,8 +799,17 @@ cudaError_t launch_gemm_pair(const GemmMaps& maps, GemmShape sh, const Epi& epi,
   sh.band = gemm_band(2 * mblocks) / 2;
   if (sh.band < 1) sh.band = 1;
   const int pairs = num_sms / 2;
-  const int grid = 2 * (ntiles < pairs ? ntiles : pairs);
-  kern<<<grid, GEMM_THREADS, GEMM2_SMEM_BYTES, st>>>(maps, sh, epi);
+  const int clusters = ntiles < pairs ? ntiles : pairs;
+  // split-K tail: the r = ntiles mod clusters leftover tiles are cut into s K-slices when s r <= clusters, s >= 2
+  sh.sk_split = 0; sh.sk_partial = nullptr; sh.sk_flags = nullptr; sh.sk_epoch = 0;
+  const int rem = ntiles % clusters;
+  if (sk && sk->partial && gemm_use_streamk() && ntiles > clusters && rem != 0) {
+    int s = clusters / rem;
+    if (s > GEMM2_MAX_SPLIT) s = GEMM2_MAX_SPLIT;
+    while (s >= 2 && sh.kblocks[0] / s < 4) --s;          // at least 4 k-blocks per slice
+    if (s >= 2) { sh.sk_split = s; sh.sk_partial = sk->partial; sh.sk_flags = sk->flags; sh.sk_epoch = sk->epoch; }
+  }
+  kern<<<2 * clusters, GEMM_THREADS, GEMM2_SMEM_BYTES, st>>>(maps, sh, epi);
   return cudaGetLastError();
 }
 
@@ -663,6 +828,7 @@ cudaError_t launch_gemm(const GemmMaps& maps, GemmShape sh, const Epi& epi, int 
   const int ntiles = mblocks * nblocks;
   if (ntiles == 0) return cudaSuccess;
   sh.band = gemm_band(mblocks);
+  sh.sk_split = 0; sh.sk_partial = nullptr; sh.sk_flags = nullptr; sh.sk_epoch = 0;
   const int grid = ntiles < num_sms ? ntiles : num_sms;
   kern<<<grid, GEMM_THREADS, Cfg::SMEM_BYTES, st>>>(maps, sh, epi);
   return cudaGetLastError();
@@ -671,7 +837,7 @@ cudaError_t launch_gemm(const GemmMaps& maps, GemmShape sh, const Epi& epi, int 
 // Generic entry: up to three K-segments (A_s, B_s, K_s); all segments share the operand majors.
 template <int BN, bool A_MN, bool B_MN, class Epi>
 cudaError_t gemm_run(int M, int N, int nseg, const Operand* a, const Operand* b, const int* ks, const Epi& epi,
-                     int num_sms, cudaStream_t st) {
+                     int num_sms, cudaStream_t st, const GemmSKRes* sk = nullptr) {
   GemmMaps maps;
   GemmShape sh;
   sh.M = M; sh.N = N; sh.nseg = nseg;
@@ -683,14 +849,14 @@ cudaError_t gemm_run(int M, int N, int nseg, const Operand* a, const Operand* b,
     if (!encode_operand(&maps.a[s], a[s], M, ks[s], GEMM_BM)) return cudaErrorInvalidValue;
     if (!encode_operand(&maps.b[s], b[s], N, ks[s], pair ? 128 : BN)) return cudaErrorInvalidValue;
   }
-  if (pair) return launch_gemm_pair<A_MN, B_MN, false, Epi>(maps, sh, epi, num_sms, st);
+  if (pair) return launch_gemm_pair<A_MN, B_MN, false, Epi>(maps, sh, epi, num_sms, st, nseg == 1 ? sk : nullptr);
   return launch_gemm<BN, A_MN, B_MN, false, Epi>(maps, sh, epi, num_sms, st);
 }
 
 // Forward gate/up GEMM (DUAL): A [M,K], Wg/Wu [N,K] all K-major.
 template <class Epi>
 cudaError_t gemm_run_dual(int M, int N, int K, const Operand& a, const Operand& bg, const Operand& bu, const Epi& epi,
-                          int num_sms, cudaStream_t st) {
+                          int num_sms, cudaStream_t st, const GemmSKRes* sk = nullptr) {
   GemmMaps maps;
   GemmShape sh;
   sh.M = M; sh.N = N; sh.nseg = 1;
@@ -699,7 +865,7 @@ cudaError_t gemm_run_dual(int M, int N, int K, const Operand& a, const Operand& 
   if (!encode_operand(&maps.a[0], a, M, K, GEMM_BM)) return cudaErrorInvalidValue;
   if (!encode_operand(&maps.b[0], bg, N, K, 128)) return cudaErrorInvalidValue;
   if (!encode_operand(&maps.b[1], bu, N, K, 128)) return cudaErrorInvalidValue;
-  if (gemm_use_pair(M)) return launch_gemm_pair<false, false, true, Epi>(maps, sh, epi, num_sms, st);
+  if (gemm_use_pair(M)) return launch_gemm_pair<false, false, true, Epi>(maps, sh, epi, num_sms, st, sk);
   return launch_gemm<256, false, false, true, Epi>(maps, sh, epi, num_sms, st);
 }
 

@@ -57,6 +57,9 @@ struct lsp_ctx {
   int device, num_sms;
   int T, Nq, Nkv, Nqkv, G;
   float2* rope;         // [seq, head_dim/2] (cos, sin), device
+  float* sk_partial;             // stream-K partial accumulators, [num_sms/2][256 x 256] fp32 (device)
+  unsigned int* sk_flags;        // [num_sms/2][2] publication epochs (device, zeroed at create)
+  unsigned int gemm_seq;         // launches so far: epoch of the next stream-K launch
   int norm_blocks;      // persistent grid of the RMSNorm backward
   SavedLayout sv;
   WsLayout ws;
@@ -169,17 +172,26 @@ cudaError_t norm_fwd(const lsp_ctx* c, int dt, const void* x, const void* g, __h
 template <typename XT, typename RT>
 cudaError_t norm_bwd_t(const lsp_ctx* c, const void* x, const float* rstd, const void* g, const float* dxn, const void* dres,
                        float* dx, __half* dx16, float* dg_part, float* dg, cudaStream_t st) {
-  const int H = c->d.hidden, nv = (H / 4 + NORM_THREADS - 1) / NORM_THREADS;
+  const int H = c->d.hidden, nv = (H / 4 + NORMB_CONSUMERS - 1) / NORMB_CONSUMERS;
   const XT* xp = static_cast<const XT*>(x);
   const RT* rp = static_cast<const RT*>(dres);
   const __nv_bfloat16* gp = static_cast<const __nv_bfloat16*>(g);
   const int nb = c->norm_blocks < c->T ? c->norm_blocks : c->T;
-#define LSP_NB(NV) case NV: rmsnorm_bwd_kernel<XT, RT, NV><<<nb, NORM_THREADS, 0, st>>>(xp, rstd, gp, dxn, rp, dx, dx16, dg_part, c->T, H); break;
+  const size_t stage_bytes = static_cast<size_t>(H) * (sizeof(XT) + 4 + sizeof(RT));
+  int stages = static_cast<int>(NORMB_SMEM_BUDGET / stage_bytes);
+  if (stages > NORMB_MAX_STAGES) stages = NORMB_MAX_STAGES;
+  if (stages < 2) return cudaErrorInvalidValue;
+  const size_t smem = stages * stage_bytes;
+#define LSP_NB(NV) case NV: { \
+    auto kern = rmsnorm_bwd_kernel<XT, RT, NV>; \
+    static bool set = false; \
+    if (!set) { cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, NORMB_SMEM_BUDGET); if (e != cudaSuccess) return e; set = true; } \
+    kern<<<nb, NORMB_THREADS, smem, st>>>(xp, rstd, gp, dxn, rp, dx, dx16, dg_part, c->T, H, stages); } break;
   switch (nv) { LSP_NB(1) LSP_NB(2) LSP_NB(3) LSP_NB(4) LSP_NB(5) LSP_NB(6) LSP_NB(7) LSP_NB(8) default: return cudaErrorInvalidValue; }
 #undef LSP_NB
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  colsum_kernel<<<(H + 255) / 256, 256, 0, st>>>(dg_part, dg, nb, H);
+  colsum_kernel<<<(H + 31) / 32, 256, 0, st>>>(dg_part, dg, nb, H);
   return cudaGetLastError();
 }
 // x: forward input of the norm (XT = x_dt); dres: incoming residual gradient (RT = r_dt)
@@ -227,7 +239,9 @@ inline EpiF32 epi_f32(float* out, long long ld) {
 template <bool A_MN, bool B_MN, class Epi>
 cudaError_t gemm1(const lsp_ctx* c, int M, int N, int K, const Operand& a, const Operand& b, const Epi& epi, cudaStream_t st) {
   const int ks[1] = {K};
-  return gemm_run<BN_MAIN, A_MN, B_MN, Epi>(M, N, 1, &a, &b, ks, epi, c->num_sms, st);
+  lsp_ctx* mc = const_cast<lsp_ctx*>(c);
+  const GemmSKRes sk{c->sk_partial, c->sk_flags, ++mc->gemm_seq};
+  return gemm_run<BN_MAIN, A_MN, B_MN, Epi>(M, N, 1, &a, &b, ks, epi, c->num_sms, st, &sk);
 }
 
 // out[T,H] fp32 = res + A[T,K] . W[H,K]^T   (O-proj and down-proj forward with the residual epilogue; F4, F7)
@@ -390,8 +404,9 @@ lsp_status mlp_fwd_impl(lsp_ctx* ctx, int a_dt, const void* a, const lsp_layer_w
   LSP_WCAST(w->w_down, wd16, FH);
   LSP_STAGE(ST_NORM_FWD, 1, norm_fwd(ctx, a_dt, a, w->g_mlp, an, rstd2, st));
   EpiSwiGLU e{h, g16, u16, F};
+  const GemmSKRes sk{ctx->sk_partial, ctx->sk_flags, ++ctx->gemm_seq};
   LSP_STAGE(ST_GATEUP, 1, gemm_run_dual(T, F, H, Operand{an, H, false}, Operand{wgu16, H, false}, Operand{wgu16 + FH, H, false}, e,
-                         ctx->num_sms, st));
+                         ctx->num_sms, st, &sk));
   LSP_STAGE(ST_DOWN, 1, gemm_fwd_residual(ctx, h, F, wd16, a_dt, a, y, st));
   return LSP_OK;
 }
@@ -494,7 +509,7 @@ lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device
     return LSP_EUNSUPPORTED;
   }
   ctx->num_sms = prop.multiProcessorCount;
-  ctx->norm_blocks = ctx->num_sms * 4;
+  ctx->norm_blocks = ctx->num_sms;         // one persistent CTA per SM (bulk-copy ring of ~200 KB)
   plan_layout(ctx);
 
   // RoPE table: theta = pos * base^(-2i/d) in fp64 (reading A-5), stored as fp32 (cos, sin)
@@ -512,6 +527,15 @@ lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device
     return LSP_ECUDA;
   }
   if (!get_encode_fn()) { cudaFree(ctx->rope); delete ctx; return LSP_ECUDA; }
+  {
+    const size_t pairs = static_cast<size_t>(ctx->num_sms / 2);
+    if (cudaMalloc(&ctx->sk_partial, pairs * GEMM2_PARTIAL_FLOATS * sizeof(float)) != cudaSuccess ||
+        cudaMalloc(&ctx->sk_flags, pairs * 2 * sizeof(unsigned int)) != cudaSuccess ||
+        cudaMemset(ctx->sk_flags, 0, pairs * 2 * sizeof(unsigned int)) != cudaSuccess) {
+      cudaFree(ctx->sk_partial); cudaFree(ctx->sk_flags); cudaFree(ctx->rope); delete ctx;
+      return LSP_ENOMEM;
+    }
+  }
   *out = ctx;
   return LSP_OK;
 }
@@ -520,6 +544,8 @@ lsp_status lsp_destroy(lsp_ctx* ctx) {
   if (!ctx) return LSP_EINVAL;
   lsp_timing_enable(ctx, 0);
   cudaFree(ctx->rope);
+  cudaFree(ctx->sk_partial);
+  cudaFree(ctx->sk_flags);
   delete ctx;
   return LSP_OK;
 }

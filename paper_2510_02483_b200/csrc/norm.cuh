@@ -70,50 +70,129 @@ __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_fwd_kernel(const XT* __r
   }
 }
 
-// dx = dres + r*(dn - n*mean(dn*n)),  n = x*r, dn = dxn*g ;  dg partial[block][col] = sum_rows dxn*n.
-// Persistent blocks stride over rows so each thread keeps its columns' dg partials in registers.
+// RMSNorm backward + residual gradient:
+//   n = x r,  dn = dxn g,  dx = dres + r (dn - n mean_j(dn_j n_j)),  dg partial[block][col] = sum_rows dxn n.
+// HBM-bound (x, dxn, dres read once, dx written once: 43-49 kB per token at H = 3072).  One persistent CTA per SM;
+// a producer warp streams whole rows of the three inputs into a shared-memory ring with 1-D bulk async copies
+// (cp.async.bulk, completion on an mbarrier), so ~150 KB per SM are in flight regardless of what the 8 consumer
+// warps are doing; the consumers read their columns from shared memory, reduce the row dot product, and store dx
+// (and its fp16 copy) straight from registers.  Each thread keeps its columns' dg partials in registers over all
+// rows of the CTA; colsum_kernel adds the per-CTA partials in a fixed order (deterministic, no atomics).
+constexpr int NORMB_CONSUMERS = 256;                       // 8 consumer warps
+constexpr int NORMB_THREADS = NORMB_CONSUMERS + 32;        // + 1 producer warp
+constexpr int NORMB_MAX_STAGES = 6;
+constexpr int NORMB_SMEM_BUDGET = 200 * 1024;
+
+__device__ __forceinline__ void bulk_load_1d(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(reinterpret_cast<uint64_t>(src)), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+template <typename T> __device__ __forceinline__ float4 lds_vec4(const uint8_t* row, int c);
+template <> __device__ __forceinline__ float4 lds_vec4<float>(const uint8_t* row, int c) {
+  return *reinterpret_cast<const float4*>(row + static_cast<size_t>(c) * 4);
+}
+template <> __device__ __forceinline__ float4 lds_vec4<__nv_bfloat16>(const uint8_t* row, int c) {
+  const uint2 u = *reinterpret_cast<const uint2*>(row + static_cast<size_t>(c) * 2);
+  return make_float4(bf16_lo(u.x), bf16_hi(u.x), bf16_lo(u.y), bf16_hi(u.y));
+}
+
+// sum over the 256 consumer threads (named barrier 1; the producer warp never joins it)
+__device__ __forceinline__ float consumer_sum(float v, float* red) {
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  named_bar_sync(1, NORMB_CONSUMERS);         // protect `red` from the previous row
+  if (lane == 0) red[warp] = v;
+  named_bar_sync(1, NORMB_CONSUMERS);
+  float t = (lane < NORMB_CONSUMERS / 32) ? red[lane] : 0.f;
+#pragma unroll
+  for (int off = 4; off > 0; off >>= 1) t += __shfl_xor_sync(0xffffffffu, t, off);
+  return __shfl_sync(0xffffffffu, t, 0);
+}
+
 template <typename XT, typename RT, int NV>
-__global__ void __launch_bounds__(NORM_THREADS) rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd,
-                                                                   const __nv_bfloat16* __restrict__ g,
-                                                                   const float* __restrict__ dxn, const RT* __restrict__ dres,
-                                                                   float* __restrict__ dx, __half* __restrict__ dx16,
-                                                                   float* __restrict__ dg_part, int T, int H) {
-  __shared__ float red[NORM_THREADS / 32];
+__global__ void __launch_bounds__(NORMB_THREADS, 1)
+rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, const __nv_bfloat16* __restrict__ g,
+                   const float* __restrict__ dxn, const RT* __restrict__ dres, float* __restrict__ dx,
+                   __half* __restrict__ dx16, float* __restrict__ dg_part, int T, int H, int stages) {
+  extern __shared__ __align__(128) uint8_t nsm[];
+  __shared__ float red[NORMB_CONSUMERS / 32];
+  __shared__ __align__(8) unsigned long long bars[2 * NORMB_MAX_STAGES];
+  const uint32_t xb = static_cast<uint32_t>(H) * sizeof(XT), db = static_cast<uint32_t>(H) * 4u, rb = static_cast<uint32_t>(H) * sizeof(RT);
+  const uint32_t stage_bytes = xb + db + rb;                 // every part is a multiple of 16 (H % 8 == 0)
+  const uint32_t smem0 = smem_u32(nsm);
+  auto full = [&](int s) { return smem_u32(&bars[s]); };
+  auto empty = [&](int s) { return smem_u32(&bars[NORMB_MAX_STAGES + s]); };
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < stages; ++s) { mbar_init(full(s), 1); mbar_init(empty(s), NORMB_CONSUMERS / 32); }
+    fence_barrier_init();
+  }
+  __syncthreads();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (warp == NORMB_CONSUMERS / 32) {
+    // ------------------------------------------------------------------ producer warp
+    if (lane == 0) {
+      int s = 0; uint32_t ph = 0;
+      for (long long row = blockIdx.x; row < T; row += gridDim.x) {
+        mbar_wait(empty(s), ph ^ 1u);
+        const uint32_t dst = smem0 + s * stage_bytes;
+        mbar_expect_tx(full(s), stage_bytes);
+        bulk_load_1d(dst, x + row * H, xb, full(s));
+        bulk_load_1d(dst + xb, dxn + row * H, db, full(s));
+        bulk_load_1d(dst + xb + db, dres + row * H, rb, full(s));
+        if (++s == stages) { s = 0; ph ^= 1u; }
+      }
+    }
+    return;
+  }
+  // -------------------------------------------------------------------- consumers
   float4 gg[NV], acc[NV];
 #pragma unroll
   for (int i = 0; i < NV; ++i) {
-    const int c = (threadIdx.x + i * NORM_THREADS) * 4;
+    const int c = (threadIdx.x + i * NORMB_CONSUMERS) * 4;
     acc[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     gg[i] = (c < H) ? Vec4<__nv_bfloat16>::load(g + c) : make_float4(0.f, 0.f, 0.f, 0.f);
   }
   const float invH = 1.0f / static_cast<float>(H);
+  int s = 0; uint32_t ph = 0;
   for (long long row = blockIdx.x; row < T; row += gridDim.x) {
     const float r = rstd[row];
-    float4 n[NV], dn[NV];
+    mbar_wait(full(s), ph);
+    const uint8_t* sx = nsm + static_cast<size_t>(s) * stage_bytes;
+    const uint8_t* sd = sx + xb;
+    const uint8_t* sr = sd + db;
+    float4 n[NV], dn[NV], rs[NV];
     float dot = 0.f;
 #pragma unroll
     for (int i = 0; i < NV; ++i) {
-      const int c = (threadIdx.x + i * NORM_THREADS) * 4;
+      const int c = (threadIdx.x + i * NORMB_CONSUMERS) * 4;
       if (c < H) {
-        const float4 xv = Vec4<XT>::load(x + row * H + c);
-        const float4 d = Vec4<float>::load(dxn + row * H + c);
+        const float4 xv = lds_vec4<XT>(sx, c);
+        const float4 d = lds_vec4<float>(sd, c);
+        rs[i] = lds_vec4<RT>(sr, c);
         n[i] = make_float4(xv.x * r, xv.y * r, xv.z * r, xv.w * r);
         acc[i].x += d.x * n[i].x; acc[i].y += d.y * n[i].y; acc[i].z += d.z * n[i].z; acc[i].w += d.w * n[i].w;
         dn[i] = make_float4(d.x * gg[i].x, d.y * gg[i].y, d.z * gg[i].z, d.w * gg[i].w);
         dot += dn[i].x * n[i].x + dn[i].y * n[i].y + dn[i].z * n[i].z + dn[i].w * n[i].w;
       }
     }
-    dot = block_sum(dot, red) * invH;
+    __syncwarp();
+    if (lane == 0) mbar_arrive(empty(s));                    // this warp has read its part of the stage
+    if (++s == stages) { s = 0; ph ^= 1u; }
+    dot = consumer_sum(dot, red) * invH;
 #pragma unroll
     for (int i = 0; i < NV; ++i) {
-      const int c = (threadIdx.x + i * NORM_THREADS) * 4;
+      const int c = (threadIdx.x + i * NORMB_CONSUMERS) * 4;
       if (c < H) {
-        const float4 rs = Vec4<RT>::load(dres + row * H + c);
         float4 o;
-        o.x = rs.x + r * (dn[i].x - n[i].x * dot);
-        o.y = rs.y + r * (dn[i].y - n[i].y * dot);
-        o.z = rs.z + r * (dn[i].z - n[i].z * dot);
-        o.w = rs.w + r * (dn[i].w - n[i].w * dot);
+        o.x = rs[i].x + r * (dn[i].x - n[i].x * dot);
+        o.y = rs[i].y + r * (dn[i].y - n[i].y * dot);
+        o.z = rs[i].z + r * (dn[i].z - n[i].z * dot);
+        o.w = rs[i].w + r * (dn[i].w - n[i].w * dot);
         *reinterpret_cast<float4*>(dx + row * H + c) = o;
         if (dx16) store_f16x4(dx16 + row * H + c, o);
       }
@@ -121,18 +200,27 @@ __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_bwd_kernel(const XT* __r
   }
 #pragma unroll
   for (int i = 0; i < NV; ++i) {
-    const int c = (threadIdx.x + i * NORM_THREADS) * 4;
+    const int c = (threadIdx.x + i * NORMB_CONSUMERS) * 4;
     if (c < H) *reinterpret_cast<float4*>(dg_part + static_cast<long long>(blockIdx.x) * H + c) = acc[i];
   }
 }
 
-// dg[col] = sum over blocks of dg_part[block][col]  (fixed order: deterministic)
-__global__ void colsum_kernel(const float* __restrict__ part, float* __restrict__ out, int nparts, int H) {
-  const int c = blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= H) return;
+// dg[col] = sum over CTAs of dg_part[cta][col], fixed order (deterministic).  Block = 32 columns x 8 partial groups.
+__global__ void __launch_bounds__(256) colsum_kernel(const float* __restrict__ part, float* __restrict__ out, int nparts, int H) {
+  __shared__ float sm[8][33];
+  const int cx = threadIdx.x & 31, gy = threadIdx.x >> 5;
+  const int c = blockIdx.x * 32 + cx;
   float s = 0.f;
-  for (int b = 0; b < nparts; ++b) s += part[static_cast<long long>(b) * H + c];
-  out[c] = s;
+  if (c < H)
+    for (int b = gy; b < nparts; b += 8) s += part[static_cast<long long>(b) * H + c];
+  sm[gy][cx] = s;
+  __syncthreads();
+  if (gy == 0 && c < H) {
+    float t = 0.f;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) t += sm[k][cx];
+    out[c] = t;
+  }
 }
 
 // 8 elements per thread casts (n is a multiple of 8)

@@ -96,6 +96,38 @@ def test_gemm_vs_fp64(gpu, op, M, N, K, fmt):
     assert err < 1e-5, err            # exact 16-bit products, fp32 accumulation
 
 
+# shapes whose tile count (256 x 256 tiles on 74 CTA pairs) leaves a partial last wave, so the split-K tail of the
+# pair kernel runs: 90 tiles (16 leftover, 4 K-slices each), 320 tiles (24 leftover, 2 slices), and a ragged one
+# (11 x 7 = 77 tiles, 3 leftover, 4 slices; M, N, K tails)
+GEMM_SK_SHAPES = [(2560, 2304, 1024), (4096, 5120, 512), (2696, 1704, 1096)]
+
+
+@pytest.mark.parametrize("op", [0, 1, 2])
+@pytest.mark.parametrize("M,N,K", GEMM_SK_SHAPES)
+def test_gemm_streamk_vs_fp64(gpu, op, M, N, K):
+    """The split-K tail (partial accumulators exchanged through global memory, fixed summation order) against
+    numpy float64, and bit-identical results on a second launch (no atomics on data).  Bound 5e-5: fp32 accumulation
+    of K ~ 1000 N(0,1) products rounds at ~sqrt(K) 2^-24 = 2e-6 rms, and the metric takes the max over 6e6 elements."""
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    rng = np.random.default_rng([7, op, M, N, K])
+    a_shape = (M, K) if op < 2 else (K, M)
+    b_shape = (N, K) if op == 0 else (K, N)
+    dA, A64 = _operand(rng, a_shape, B.LSP_F16)
+    dB, B64 = _operand(rng, b_shape, B.LSP_F16)
+    ref = A64 @ B64.T if op == 0 else (A64 @ B64 if op == 1 else A64.T @ B64)
+    ctx = gpu.make_ctx(synth.CFG1_TINY)
+    outs = []
+    for _ in range(2):
+        out = torch.full((M, N), float("nan"), dtype=torch.float32, device=dA.device)
+        B.lsp_gemm(ctx, op, M, N, K, dA, a_shape[1], B.LSP_F16, dB, b_shape[1], B.LSP_F16, out, N)
+        torch.cuda.synchronize()
+        outs.append(out.cpu().numpy())
+    ctx.close()
+    assert norm_err(outs[0], ref) < 5e-5
+    assert np.array_equal(outs[0], outs[1])
+
+
 def test_gemm_mixed_formats_rejected(gpu):
     """A mixed fp16 x bf16 operand pair must be refused (LSP_EUNSUPPORTED), never launched: it faults on sm_100a."""
     import torch
