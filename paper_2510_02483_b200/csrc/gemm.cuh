@@ -58,7 +58,7 @@ template <int BN> struct GemmCfg {
   static constexpr int B_BYTES = BN * GEMM_BK * 2;
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
   static constexpr int STAGES = (BN == 256) ? 4 : 6;
-  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
+  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 8 * 4096 /*staging tiles*/ + 1024 /*align slack*/ + 256 /*barriers*/;
   static constexpr int TMEM_COLS = 2 * BN;   // two accumulator stages (power of two: 256 or 512)
 };
 
@@ -122,13 +122,20 @@ __device__ __forceinline__ void load_row32(const void* p, float (&v)[32], int nv
   }
 }
 
-// 32 fp32 values written by ANOTHER CTA during this kernel (stream-K partials): plain coherent loads, never ld.global.nc
-__device__ __forceinline__ void load_row32_coherent(const float* p, float (&v)[32]) {
-  const volatile float4* q = reinterpret_cast<const volatile float4*>(p);
+// Split-K partial accumulators: chunk layout [unit j = 0..7][row 0..127][4 floats], so that the 32 lanes of a warp
+// (consecutive rows) write / read 512 contiguous bytes per instruction.  Written by ANOTHER CTA during this kernel:
+// plain coherent loads, never ld.global.nc.
+__device__ __forceinline__ void partial_store(float* chunk, int row, const float (&v)[32]) {
+#pragma unroll
+  for (int j = 0; j < 8; ++j)
+    *reinterpret_cast<float4*>(chunk + (j * GEMM_BM + row) * 4) = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+}
+__device__ __forceinline__ void partial_load(const float* chunk, int row, float (&v)[32]) {
 #pragma unroll
   for (int j = 0; j < 8; ++j) {
     float4 t;
-    asm volatile("ld.global.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(t.x), "=f"(t.y), "=f"(t.z), "=f"(t.w) : "l"(q + j) : "memory");
+    asm volatile("ld.global.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(t.x), "=f"(t.y), "=f"(t.z), "=f"(t.w)
+                 : "l"(chunk + (j * GEMM_BM + row) * 4) : "memory");
     v[4 * j] = t.x; v[4 * j + 1] = t.y; v[4 * j + 2] = t.z; v[4 * j + 3] = t.w;
   }
 }
@@ -136,7 +143,138 @@ __device__ __forceinline__ void named_bar_sync_gemm(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
+// ------------------------------------------------------------------------------------------- warp staging tile
+// tcgen05.ld hands every thread one accumulator ROW (32 consecutive columns).  Writing that straight to global memory
+// makes each warp instruction touch 32 rows x 16 B (32 half-filled sectors): the unoverlapped epilogue of a 256 x 256
+// fp32 tile took ~30 k cycles (8.7 B/clk/SM).  Each epilogue warp therefore owns a 4 KB shared-memory tile
+// (32 rows x 128 B, 16-byte units XOR-swizzled so that both access patterns are bank-conflict free): threads exchange
+// rows through it and global memory sees 8 lanes x 16 B = one full 128-byte row segment, 4 rows per instruction
+// (16-bit data: 4 lanes x 16 B = 64 B, 8 rows per instruction).
+constexpr int GEMM_STAGE_TILE_BYTES = 4096;
+struct WarpStage {
+  uint32_t base;      // shared::cta address of this warp's tile
+  int lane;
+  // ---- thread = row view, 32-bit elements: row `lane`, units j = 0..7
+  __device__ __forceinline__ void put_row32(const float (&v)[32]) const {
+#pragma unroll
+    for (int j = 0; j < 8; ++j)
+      asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(base + lane * 128 + ((j ^ (lane & 7)) << 4)),
+                   "f"(v[4 * j]), "f"(v[4 * j + 1]), "f"(v[4 * j + 2]), "f"(v[4 * j + 3]) : "memory");
+  }
+  __device__ __forceinline__ void get_row32(float (&v)[32]) const {
+#pragma unroll
+    for (int j = 0; j < 8; ++j)
+      asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v[4 * j]), "=f"(v[4 * j + 1]), "=f"(v[4 * j + 2]), "=f"(v[4 * j + 3])
+                   : "r"(base + lane * 128 + ((j ^ (lane & 7)) << 4)) : "memory");
+  }
+  // ---- thread = row view, 16-bit elements packed in pairs: row `lane` (64 B), units j = 0..3
+  __device__ __forceinline__ void put_row16(const uint32_t (&w)[16]) const {
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+      asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(base + lane * 64 + ((j ^ ((lane >> 1) & 3)) << 4)),
+                   "r"(w[4 * j]), "r"(w[4 * j + 1]), "r"(w[4 * j + 2]), "r"(w[4 * j + 3]) : "memory");
+  }
+  __device__ __forceinline__ void get_row16(uint32_t (&w)[16]) const {
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+      asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(w[4 * j]), "=r"(w[4 * j + 1]), "=r"(w[4 * j + 2]), "=r"(w[4 * j + 3])
+                   : "r"(base + lane * 64 + ((j ^ ((lane >> 1) & 3)) << 4)) : "memory");
+  }
+  // ---- coalesced view.  rowptr(r) -> pointer to column 0 of the chunk in row r; rows [0, nrows), columns [0, ncols)
+  template <class RowPtr>
+  __device__ __forceinline__ void to_global32(RowPtr rowptr, int nrows, int ncols) const {
+    const int u = lane & 7;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int r = 4 * i + (lane >> 3);
+      if (r < nrows && 4 * u + 4 <= ncols) {
+        uint4 t;
+        asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(t.x), "=r"(t.y), "=r"(t.z), "=r"(t.w)
+                     : "r"(base + r * 128 + ((u ^ (r & 7)) << 4)) : "memory");
+        *reinterpret_cast<uint4*>(rowptr(r) + 4 * u) = t;
+      }
+    }
+  }
+  template <class RowPtr>
+  __device__ __forceinline__ void from_global32(RowPtr rowptr, int nrows, int ncols) const {
+    const int u = lane & 7;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int r = 4 * i + (lane >> 3);
+      uint4 t = make_uint4(0, 0, 0, 0);
+      if (r < nrows && 4 * u + 4 <= ncols) t = __ldg(reinterpret_cast<const uint4*>(rowptr(r) + 4 * u));
+      asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(base + r * 128 + ((u ^ (r & 7)) << 4)),
+                   "r"(t.x), "r"(t.y), "r"(t.z), "r"(t.w) : "memory");
+    }
+  }
+  template <class RowPtr>
+  __device__ __forceinline__ void to_global16(RowPtr rowptr, int nrows, int ncols) const {
+    const int u = lane & 3;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int r = 8 * i + (lane >> 2);
+      if (r < nrows && 8 * u + 8 <= ncols) {
+        uint4 t;
+        asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(t.x), "=r"(t.y), "=r"(t.z), "=r"(t.w)
+                     : "r"(base + r * 64 + ((u ^ ((r >> 1) & 3)) << 4)) : "memory");
+        *reinterpret_cast<uint4*>(rowptr(r) + 8 * u) = t;
+      }
+    }
+  }
+  template <class RowPtr>
+  __device__ __forceinline__ void from_global16(RowPtr rowptr, int nrows, int ncols) const {
+    const int u = lane & 3;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int r = 8 * i + (lane >> 2);
+      uint4 t = make_uint4(0, 0, 0, 0);
+      if (r < nrows && 8 * u + 8 <= ncols) t = __ldg(reinterpret_cast<const uint4*>(rowptr(r) + 8 * u));
+      asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(base + r * 64 + ((u ^ ((r >> 1) & 3)) << 4)),
+                   "r"(t.x), "r"(t.y), "r"(t.z), "r"(t.w) : "memory");
+    }
+  }
+};
+
+// Row I/O of one warp chunk (32 rows starting at m_base, 32 columns starting at n) through the staging tile.
+template <int DT, class RowPtr>
+__device__ __forceinline__ void chunk_store(const WarpStage& st, RowPtr rowptr, const float (&v)[32], int nrows, int ncols) {
+  __syncwarp();                                  // previous readers of the tile are done
+  if constexpr (DT == DT_F32) {
+    st.put_row32(v);
+    __syncwarp();
+    st.to_global32(rowptr, nrows, ncols);
+  } else {
+    uint32_t w[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) w[j] = DT == DT_BF16 ? pack_bf16(v[2 * j], v[2 * j + 1]) : pack_f16(v[2 * j], v[2 * j + 1]);
+    st.put_row16(w);
+    __syncwarp();
+    st.to_global16(rowptr, nrows, ncols);
+  }
+}
+template <int DT, class RowPtr>
+__device__ __forceinline__ void chunk_load(const WarpStage& st, RowPtr rowptr, float (&v)[32], int nrows, int ncols) {
+  __syncwarp();
+  if constexpr (DT == DT_F32) {
+    st.from_global32(rowptr, nrows, ncols);
+    __syncwarp();
+    st.get_row32(v);
+  } else {
+    st.from_global16(rowptr, nrows, ncols);
+    __syncwarp();
+    uint32_t w[16];
+    st.get_row16(w);
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+      if constexpr (DT == DT_BF16) { v[2 * j] = bf16_lo(w[j]); v[2 * j + 1] = bf16_hi(w[j]); }
+      else { const __half2 h = *reinterpret_cast<const __half2*>(&w[j]); v[2 * j] = __low2float(h); v[2 * j + 1] = __high2float(h); }
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------- epilogues
+// Every epilogue works on one warp chunk: rows [m_base, m_base + nrows) (thread `lane` holds row m_base + lane),
+// columns [n, n + nvalid); all global traffic goes through the warp's staging tile.
 // Plain store with optional residual add and up to three row-segments of output (wgrad of fused QKV / gate-up).
 template <int ODT, int RDT, bool HAS_RES>
 struct EpiStore {
@@ -145,10 +283,19 @@ struct EpiStore {
   long long ld;              // row pitch (elements) of every output and of the residual
   const void* res;
   float alpha;
-  __device__ __forceinline__ void operator()(int m, int n, float (&v)[32], int nvalid) const {
+  // L2 prefetch of what the epilogue of rows [m_base, +nrows) x columns [n0, n0 + ncols) will read (issued by the
+  // epilogue warps while the tensor core still works on the tile, so the reads do not pay DRAM latency per chunk)
+  __device__ __forceinline__ void prefetch(int lane, int m_base, int n0, int nrows, int ncols) const {
+    if constexpr (HAS_RES) {
+      using RT = typename OutElem<RDT>::type;
+      if (lane < nrows) {
+        const RT* rp = reinterpret_cast<const RT*>(res) + static_cast<long long>(m_base + lane) * ld + n0;
+        for (int c = 0; c < ncols; c += 128 / static_cast<int>(sizeof(RT))) prefetch_l2(rp + c);
+      }
+    }
+  }
+  __device__ __forceinline__ void operator()(const WarpStage& st, int m_base, int n, float (&v)[32], int nrows, int nvalid) const {
     using OT = typename OutElem<ODT>::type;
-    int seg = (m >= split1) + (m >= split2);
-    int mr = m - (seg == 0 ? 0 : (seg == 1 ? split1 : split2));
     if (alpha != 1.0f) {
 #pragma unroll
       for (int j = 0; j < 32; ++j) v[j] *= alpha;
@@ -156,11 +303,17 @@ struct EpiStore {
     if constexpr (HAS_RES) {
       using RT = typename OutElem<RDT>::type;
       float r[32];
-      load_row32<RDT>(reinterpret_cast<const RT*>(res) + static_cast<long long>(m) * ld + n, r, nvalid);
+      const RT* rbase = reinterpret_cast<const RT*>(res) + static_cast<long long>(m_base) * ld + n;
+      chunk_load<RDT>(st, [&](int rr) { return rbase + rr * ld; }, r, nrows, nvalid);
 #pragma unroll
       for (int j = 0; j < 32; ++j) v[j] += r[j];
     }
-    store_row32<ODT>(reinterpret_cast<OT*>(out[seg]) + static_cast<long long>(mr) * ld + n, v, nvalid);
+    chunk_store<ODT>(st, [&](int rr) {
+      const int m = m_base + rr;
+      const int seg = (m >= split1) + (m >= split2);
+      const int mr = m - (seg == 0 ? 0 : (seg == 1 ? split1 : split2));
+      return reinterpret_cast<OT*>(out[seg]) + static_cast<long long>(mr) * ld + n;
+    }, v, nrows, nvalid);
   }
 };
 
@@ -172,38 +325,42 @@ struct EpiQKVRope {
   __half* out; long long ld;
   const float2* rope; int S, d;
   int rot_cols;              // columns [0, rot_cols) are rotated (Nq + Nkv, or 0 when use_rope = 0)
-  __device__ __forceinline__ void operator()(int m, int n, float (&v)[32], int nvalid) const {
+  __device__ __forceinline__ void prefetch(int, int, int, int, int) const {}      // the rope table stays L2-resident
+  __device__ __forceinline__ void operator()(const WarpStage& st, int m_base, int n, float (&v)[32], int nrows, int nvalid) const {
     if (n < rot_cols) {
-      const int pos = m % S;
-      const float2* t = rope + static_cast<long long>(pos) * (d >> 1) + ((n % d) >> 1);
+      // 16 (cos, sin) pairs = 32 words per row, fetched coalesced like any other row chunk
+      float cs[32];
+      const int half_d = d >> 1, c0 = (n % d) >> 1;
+      chunk_load<DT_F32>(st, [&](int rr) {
+        return reinterpret_cast<const float*>(rope + static_cast<long long>((m_base + rr) % S) * half_d + c0);
+      }, cs, nrows, 32);
 #pragma unroll
       for (int j = 0; j < 16; ++j) {
-        if (2 * j + 2 <= nvalid) {
-          const float2 cs = __ldg(t + j);
-          const float z0 = v[2 * j], z1 = v[2 * j + 1];
-          v[2 * j] = z0 * cs.x - z1 * cs.y;
-          v[2 * j + 1] = z0 * cs.y + z1 * cs.x;
-        }
+        const float z0 = v[2 * j], z1 = v[2 * j + 1];
+        v[2 * j] = z0 * cs[2 * j] - z1 * cs[2 * j + 1];
+        v[2 * j + 1] = z0 * cs[2 * j + 1] + z1 * cs[2 * j];
       }
     }
-    store_row32<DT_F16>(out + static_cast<long long>(m) * ld + n, v, nvalid);
+    __half* obase = out + static_cast<long long>(m_base) * ld + n;
+    chunk_store<DT_F16>(st, [&](int rr) { return obase + rr * ld; }, v, nrows, nvalid);
   }
 };
 
 // DUAL epilogue: h = silu(g) * u (ref [35]); saves g,u in fp16 for the backward (DESIGN.md precision plan).
 struct EpiSwiGLU {
   __half* h; __half* g16; __half* u16; long long ld;
-  __device__ __forceinline__ void operator()(int m, int n, float (&g)[32], float (&u)[32], int nvalid) const {
-    const long long off = static_cast<long long>(m) * ld + n;
-    store_row32<DT_F16>(g16 + off, g, nvalid);
-    store_row32<DT_F16>(u16 + off, u, nvalid);
-    float hv[32];
+  __device__ __forceinline__ void prefetch(int, int, int, int, int) const {}
+  __device__ __forceinline__ void operator()(const WarpStage& st, int m_base, int n, float (&g)[32], float (&u)[32], int nrows,
+                                             int nvalid) const {
+    const long long off = static_cast<long long>(m_base) * ld + n;
+    chunk_store<DT_F16>(st, [&](int rr) { return g16 + off + rr * ld; }, g, nrows, nvalid);
+    chunk_store<DT_F16>(st, [&](int rr) { return u16 + off + rr * ld; }, u, nrows, nvalid);
 #pragma unroll
     for (int j = 0; j < 32; ++j) {
       const float sg = 1.0f / (1.0f + __expf(-g[j]));
-      hv[j] = g[j] * sg * u[j];
+      g[j] = g[j] * sg * u[j];
     }
-    store_row32<DT_F16>(h + off, hv, nvalid);
+    chunk_store<DT_F16>(st, [&](int rr) { return h + off + rr * ld; }, g, nrows, nvalid);
   }
 };
 
@@ -211,21 +368,27 @@ struct EpiSwiGLU {
 struct EpiSwiGLUBwd {
   const __half* g16; const __half* u16; long long ld;      // saved g,u [T,F]
   __half* dgu; int F;                                      // [T, 2F]
-  __device__ __forceinline__ void operator()(int m, int n, float (&dh)[32], int nvalid) const {
+  __device__ __forceinline__ void prefetch(int lane, int m_base, int n0, int nrows, int ncols) const {
+    if (lane < nrows) {
+      const long long off = static_cast<long long>(m_base + lane) * ld + n0;
+      for (int c = 0; c < ncols; c += 64) { prefetch_l2(g16 + off + c); prefetch_l2(u16 + off + c); }
+    }
+  }
+  __device__ __forceinline__ void operator()(const WarpStage& st, int m_base, int n, float (&dh)[32], int nrows, int nvalid) const {
     float g[32], u[32];
-    const long long off = static_cast<long long>(m) * ld + n;
-    load_row32<DT_F16>(g16 + off, g, nvalid);
-    load_row32<DT_F16>(u16 + off, u, nvalid);
-    float dg[32], du[32];
+    const long long off = static_cast<long long>(m_base) * ld + n;
+    chunk_load<DT_F16>(st, [&](int rr) { return g16 + off + rr * ld; }, g, nrows, nvalid);
+    chunk_load<DT_F16>(st, [&](int rr) { return u16 + off + rr * ld; }, u, nrows, nvalid);
 #pragma unroll
     for (int j = 0; j < 32; ++j) {
       const float sg = 1.0f / (1.0f + __expf(-g[j]));
-      du[j] = dh[j] * g[j] * sg;
-      dg[j] = dh[j] * u[j] * sg * (1.0f + g[j] * (1.0f - sg));
+      const float dgv = dh[j] * u[j] * sg * (1.0f + g[j] * (1.0f - sg));
+      u[j] = dh[j] * g[j] * sg;           // du
+      g[j] = dgv;                         // dg
     }
-    __half* row = dgu + static_cast<long long>(m) * (2LL * F);
-    store_row32<DT_F16>(row + n, dg, nvalid);
-    store_row32<DT_F16>(row + F + n, du, nvalid);
+    __half* row0 = dgu + static_cast<long long>(m_base) * (2LL * F) + n;
+    chunk_store<DT_F16>(st, [&](int rr) { return row0 + rr * (2LL * F); }, g, nrows, nvalid);
+    chunk_store<DT_F16>(st, [&](int rr) { return row0 + F + rr * (2LL * F); }, u, nrows, nvalid);
   }
 };
 
@@ -249,7 +412,8 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, c
 
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t bar_base = smem_base + STAGES * Cfg::STAGE_BYTES;
+  const uint32_t stage_tiles = smem_base + STAGES * Cfg::STAGE_BYTES;     // 8 epilogue warps x 4 KB staging tiles
+  const uint32_t bar_base = stage_tiles + GEMM_EPI_WARPS * GEMM_STAGE_TILE_BYTES;
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
   auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
   auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * STAGES + s); };
@@ -365,7 +529,9 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, c
       const int m0 = mb * GEMM_BM, n0 = nb * NOUT;
       mbar_wait(tfull_bar(acc), acc_phase);
       tc_fence_after();
-      const int m = m0 + quarter * 32 + lane;
+      const int m_wbase = m0 + quarter * 32;
+      const int nrows = min(32, sh.M - m_wbase);
+      const WarpStage wst{stage_tiles + static_cast<uint32_t>(warp - 2) * GEMM_STAGE_TILE_BYTES, lane};
       const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + static_cast<uint32_t>(acc * BN);
 #pragma unroll 1
       for (int c = half; c < NOUT / 32; c += 2) {
@@ -378,10 +544,10 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, c
           uint32_t r1[32];
           tmem_ld32(t_row + NOUT + c * 32, r1);
           tmem_ld_wait();
-          if (m < sh.M) epi(m, n, reinterpret_cast<float(&)[32]>(r0), reinterpret_cast<float(&)[32]>(r1), nvalid);
+          if (nrows > 0) epi(wst, m_wbase, n, reinterpret_cast<float(&)[32]>(r0), reinterpret_cast<float(&)[32]>(r1), nrows, nvalid);
         } else {
           tmem_ld_wait();
-          if (m < sh.M) epi(m, n, reinterpret_cast<float(&)[32]>(r0), nvalid);
+          if (nrows > 0) epi(wst, m_wbase, n, reinterpret_cast<float(&)[32]>(r0), nrows, nvalid);
         }
       }
       tc_fence_before();
@@ -423,10 +589,12 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, c
 // ran DRAM-bound, 10 % slower at K = 16384).  Slices j < s - 1 store their raw fp32 accumulator to sk_partial[pair]
 // and publish sk_flags[pair] = epoch; slice s - 1 waits for those flags, adds the partials in the fixed order
 // j = 0 .. s - 2 to its own accumulator and runs the fused epilogue.  Results are bit-reproducible; no atomics on data.
-constexpr int GEMM2_STAGES = 6;
-constexpr int GEMM2_STAGE_BYTES = 2 * GEMM_BM * GEMM_BK * 2;         // A 128 x 64 + B 128 x 64 (fp16) per CTA
-constexpr int GEMM2_SMEM_BYTES = GEMM2_STAGES * GEMM2_STAGE_BYTES + 1024 + 256;
-constexpr int GEMM2_PARTIAL_FLOATS = 2 * GEMM_BM * 256;               // per pair: 256 rows x 256 accumulator columns
+template <int MT> struct Gemm2Cfg {
+  static constexpr int STAGES = MT == 1 ? 6 : 4;
+  static constexpr int STAGE_BYTES = (MT + 1) * GEMM_BM * GEMM_BK * 2;     // A (MT x 128) x 64 + B 128 x 64 (16-bit) per CTA
+  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + GEMM_EPI_WARPS * GEMM_STAGE_TILE_BYTES + 1024 + 256;
+};
+constexpr int GEMM2_PARTIAL_FLOATS = 2 * 2 * GEMM_BM * 256;           // per pair: up to 512 rows x 256 accumulator columns
 constexpr int GEMM2_MAX_SPLIT = 4;
 
 struct GemmItem { int tile, kb0, kb1, mode; };   // mode 0: whole tile; 1: K-slice that publishes a partial; 2: last K-slice
@@ -466,18 +634,29 @@ __device__ __forceinline__ void st_release_gpu(unsigned int* p, unsigned int v) 
   asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-template <bool A_MN, bool B_MN, bool DUAL, class Epi>
+template <bool A_MN, bool B_MN, bool DUAL, int MT, class Epi>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEMM_THREADS, 1)
 gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, const Epi epi) {
-  constexpr int STAGES = GEMM2_STAGES;
+  // MT = 1: 256 x 256 pair tile, two accumulator stages (epilogue of tile i overlaps the MMAs of tile i + 1).
+  // MT = 2: 512 x 256 pair tile (each CTA 256 rows = two 128-row MMAs per k-step sharing the B slice): A 32 KB +
+  //         B 16 KB per CTA and k-block for twice the MACs, i.e. 25 % less shared-memory fill per flop (the quantity
+  //         that limits clock and tensor duty under the power cap); the accumulators take all 512 TMEM columns, so
+  //         the epilogue is not overlapped -- used where K is large enough to make that negligible.
+  using G = Gemm2Cfg<MT>;
+  constexpr int STAGES = G::STAGES;
+  constexpr int STAGE_BYTES = G::STAGE_BYTES;
   constexpr int BN = 256;                        // MMA N (both CTAs' B halves)
   constexpr int NOUT = DUAL ? 128 : 256;         // output columns covered by one tile
-  constexpr int A_BYTES = GEMM_BM * GEMM_BK * 2;
-  static_assert(!DUAL || (!A_MN && !B_MN), "DUAL is the forward gate/up GEMM");
+  constexpr int A_BYTES = MT * GEMM_BM * GEMM_BK * 2;
+  constexpr int NACC = 2 / MT;                   // accumulator stages
+  constexpr int ACC_COLS = BN * MT;
+  constexpr int CTA_ROWS = GEMM_BM * MT;
+  static_assert(!DUAL || (!A_MN && !B_MN && MT == 1), "DUAL is the forward gate/up GEMM");
 
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t bar_base = smem_base + STAGES * GEMM2_STAGE_BYTES;
+  const uint32_t stage_tiles = smem_base + STAGES * STAGE_BYTES;          // 8 epilogue warps x 4 KB staging tiles
+  const uint32_t bar_base = stage_tiles + GEMM_EPI_WARPS * GEMM_STAGE_TILE_BYTES;
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
   auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
   auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * STAGES + s); };
@@ -490,7 +669,7 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
   const uint32_t rank = cluster_ctarank();
   const int cid = blockIdx.x >> 1, nclusters = gridDim.x >> 1;
 
-  const int mblocks = (sh.M + 2 * GEMM_BM - 1) / (2 * GEMM_BM);      // 256-row blocks
+  const int mblocks = (sh.M + 2 * CTA_ROWS - 1) / (2 * CTA_ROWS);      // 256- or 512-row blocks
   const int nblocks = (sh.N + NOUT - 1) / NOUT;
   const int ntiles = mblocks * nblocks;
   const int kb_total = sh.kblocks[0];
@@ -502,7 +681,7 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
     tma_prefetch_desc(&maps.a[0]); tma_prefetch_desc(&maps.b[0]);
     if (DUAL) tma_prefetch_desc(&maps.b[1]);
     for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int s = 0; s < 2; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 2 * GEMM_EPI_WARPS); }
+    for (int s = 0; s < NACC; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 2 * GEMM_EPI_WARPS); }
     fence_barrier_init();
   }
   if (warp == 1) {
@@ -523,22 +702,23 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
         const GemmItem it = work.get(j);
         int mb, nb;
         gemm_tile_coord(it.tile, mblocks, nblocks, sh.band, mb, nb);
-        const int m0 = mb * 2 * GEMM_BM + static_cast<int>(rank) * GEMM_BM;
+        const int m0 = mb * 2 * CTA_ROWS + static_cast<int>(rank) * CTA_ROWS;
         const int n0 = nb * NOUT;
         const int nb0 = DUAL ? n0 : n0 + static_cast<int>(rank) * 128;         // this CTA's B rows
         const int kb1 = min(it.kb1, kb_total);
         for (int kb = it.kb0; kb < kb1; ++kb) {
           mbar_wait(empty_bar(stage), phase ^ 1u);
-          const uint32_t sa = smem_base + stage * GEMM2_STAGE_BYTES;
+          const uint32_t sa = smem_base + stage * STAGE_BYTES;
           const uint32_t sb = sa + A_BYTES;
           const uint32_t fb = mapa_shared(full_bar(stage), 0);
-          if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * GEMM2_STAGE_BYTES);
+          if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * STAGE_BYTES);
           const int k0 = kb * GEMM_BK;
           if constexpr (!A_MN) {
-            tma_load_2d_pair(sa, &maps.a[0], fb, k0, m0);
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) tma_load_2d_pair(sa + mt * (GEMM_BM * 128), &maps.a[0], fb, k0, m0 + mt * GEMM_BM);
           } else {
 #pragma unroll
-            for (int c = 0; c < 2; ++c) tma_load_2d_pair(sa + c * (GEMM_BK * 128), &maps.a[0], fb, m0 + 64 * c, k0);
+            for (int c = 0; c < 2 * MT; ++c) tma_load_2d_pair(sa + c * (GEMM_BK * 128), &maps.a[0], fb, m0 + 64 * c, k0);
           }
           if constexpr (!B_MN) {
             tma_load_2d_pair(sb, bmap, fb, k0, nb0);
@@ -564,22 +744,25 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
         const GemmItem it = work.get(j);
         mbar_wait_cluster(tempty_bar(acc), acc_phase ^ 1u);
         tc_fence_after();
-        const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(acc * BN);
+        const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(acc * ACC_COLS);
         const int kb1 = min(it.kb1, kb_total);
         for (int kb = it.kb0; kb < kb1; ++kb) {
           mbar_wait_cluster(full_bar(stage), phase);
           tc_fence_after();
           if (leader) {
-            const uint64_t da = desc_adv(da0, stage * GEMM2_STAGE_BYTES), db = desc_adv(db0, stage * GEMM2_STAGE_BYTES);
+            const uint64_t da = desc_adv(da0, stage * STAGE_BYTES), db = desc_adv(db0, stage * STAGE_BYTES);
 #pragma unroll
             for (int k = 0; k < GEMM_BK / 16; ++k)
-              umma_f16_pair(d_tmem, desc_adv(da, k * A_KSTEP), desc_adv(db, k * B_KSTEP), idesc, (kb != it.kb0 || k != 0) ? 1u : 0u);
+#pragma unroll
+              for (int mt = 0; mt < MT; ++mt)             // the 128-row halves of this CTA's A slice share the B slice
+                umma_f16_pair(d_tmem + mt * BN, desc_adv(da, mt * (GEMM_BM * 128) + k * A_KSTEP), desc_adv(db, k * B_KSTEP), idesc,
+                              (kb != it.kb0 || k != 0) ? 1u : 0u);
             umma_commit_pair(empty_bar(stage), 3);
           }
           if (++stage == STAGES) { stage = 0; phase ^= 1u; }
         }
         if (leader) umma_commit_pair(tfull_bar(acc), 3);
-        if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+        if (++acc == NACC) { acc = 0; acc_phase ^= 1u; }
       }
     }
   } else {
@@ -587,19 +770,20 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
     const int quarter = warp & 3;
     const int half = (warp - 2) >> 2;
     const int row = quarter * 32 + lane;                                  // accumulator row of this thread = TMEM lane
+    const WarpStage wst{stage_tiles + static_cast<uint32_t>(warp - 2) * GEMM_STAGE_TILE_BYTES, lane};
     const uint32_t tempty_leader0 = mapa_shared(tempty_bar(0), 0), tempty_leader1 = mapa_shared(tempty_bar(1), 0);
-    float* const my_partial = sh.sk_partial ? sh.sk_partial + (static_cast<size_t>(cid) * 2 + rank) * (GEMM_BM * 256) : nullptr;
+    float* const my_partial = sh.sk_partial ? sh.sk_partial + (static_cast<size_t>(cid) * 2 + rank) * (CTA_ROWS * 256) : nullptr;
     // partial of K-slice jj of the tile whose last slice this pair owns: published by pair jj * rem + (cid mod rem)
     const int t_sk = work.rem > 0 ? cid % work.rem : 0;
     auto slice_partial = [&](int jj) -> const float* {
-      return sh.sk_partial + (static_cast<size_t>(jj * work.rem + t_sk) * 2 + rank) * (GEMM_BM * 256);
+      return sh.sk_partial + (static_cast<size_t>(jj * work.rem + t_sk) * 2 + rank) * (CTA_ROWS * 256);
     };
     int acc = 0; uint32_t acc_phase = 0;
     for (int j = 0; j < nitems; ++j) {
       const GemmItem it = work.get(j);
       int mb, nb;
       gemm_tile_coord(it.tile, mblocks, nblocks, sh.band, mb, nb);
-      const int m0 = mb * 2 * GEMM_BM + static_cast<int>(rank) * GEMM_BM;
+      const int m0 = mb * 2 * CTA_ROWS + static_cast<int>(rank) * CTA_ROWS;
       const int n0 = nb * NOUT;
       if (it.mode == 2) {                       // the other slices of this tile run at the same time: wait for their partials
         for (int jj = 0; jj < work.split - 1; ++jj) {
@@ -613,10 +797,22 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
           }
         }
       }
+#ifndef LSP_NO_EPI_PREFETCH
+      if (it.mode != 1) {
+#pragma unroll 1
+        for (int mt = 0; mt < MT; ++mt) {
+          const int mw = m0 + mt * GEMM_BM + quarter * 32;
+          epi.prefetch(lane, mw, n0 + half * (NOUT / 2), min(32, sh.M - mw), min(NOUT / 2, sh.N - n0 - half * (NOUT / 2)));
+        }
+      }
+#endif
       mbar_wait_cluster(tfull_bar(acc), acc_phase);
       tc_fence_after();
-      const int m = m0 + row;
-      const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + static_cast<uint32_t>(acc * BN);
+#pragma unroll 1
+      for (int mt = 0; mt < MT; ++mt) {
+      const int m_wbase = m0 + mt * GEMM_BM + quarter * 32;                // first row of this warp's 32 accumulator rows
+      const int nrows = min(32, sh.M - m_wbase);
+      const uint32_t t_row = tmem_base + (static_cast<uint32_t>(quarter * 32) << 16) + static_cast<uint32_t>(acc * ACC_COLS + mt * BN);
 #pragma unroll 1
       for (int c = half; c < NOUT / 32; c += 2) {
         const int n = n0 + c * 32;
@@ -631,8 +827,8 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
           float (&v0)[32] = reinterpret_cast<float(&)[32]>(r0);
           float (&v1)[32] = reinterpret_cast<float(&)[32]>(r1);
           if (it.mode == 1) {
-            store_row32<DT_F32>(my_partial + (static_cast<size_t>(c) * GEMM_BM + row) * 32, v0, 32);
-            store_row32<DT_F32>(my_partial + (static_cast<size_t>(NOUT / 32 + c) * GEMM_BM + row) * 32, v1, 32);
+            partial_store(my_partial + static_cast<size_t>(mt * 8 + c) * (GEMM_BM * 32), row, v0);
+            partial_store(my_partial + static_cast<size_t>(mt * 8 + NOUT / 32 + c) * (GEMM_BM * 32), row, v1);
           } else {
             if (it.mode == 2) {
               float s0[32], s1[32];
@@ -641,21 +837,21 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
               for (int jj = 0; jj < work.split - 1; ++jj) {                    // fixed order: slice 0, 1, ..., then ours
                 float p0[32], p1[32];
                 const float* pp = slice_partial(jj);
-                load_row32_coherent(pp + (static_cast<size_t>(c) * GEMM_BM + row) * 32, p0);
-                load_row32_coherent(pp + (static_cast<size_t>(NOUT / 32 + c) * GEMM_BM + row) * 32, p1);
+                partial_load(pp + static_cast<size_t>(mt * 8 + c) * (GEMM_BM * 32), row, p0);
+                partial_load(pp + static_cast<size_t>(mt * 8 + NOUT / 32 + c) * (GEMM_BM * 32), row, p1);
 #pragma unroll
                 for (int q = 0; q < 32; ++q) { s0[q] += p0[q]; s1[q] += p1[q]; }
               }
 #pragma unroll
               for (int q = 0; q < 32; ++q) { v0[q] += s0[q]; v1[q] += s1[q]; }
             }
-            if (m < sh.M) epi(m, n, v0, v1, nvalid);
+            if (nrows > 0) epi(wst, m_wbase, n, v0, v1, nrows, nvalid);
           }
         } else {
           tmem_ld_wait();
           float (&v0)[32] = reinterpret_cast<float(&)[32]>(r0);
           if (it.mode == 1) {
-            store_row32<DT_F32>(my_partial + (static_cast<size_t>(c) * GEMM_BM + row) * 32, v0, 32);
+            partial_store(my_partial + static_cast<size_t>(mt * 8 + c) * (GEMM_BM * 32), row, v0);
           } else {
             if (it.mode == 2) {
               float s0[32];
@@ -663,16 +859,17 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
               for (int q = 0; q < 32; ++q) s0[q] = 0.f;
               for (int jj = 0; jj < work.split - 1; ++jj) {                    // fixed order: slice 0, 1, ..., then ours
                 float p0[32];
-                load_row32_coherent(slice_partial(jj) + (static_cast<size_t>(c) * GEMM_BM + row) * 32, p0);
+                partial_load(slice_partial(jj) + static_cast<size_t>(mt * 8 + c) * (GEMM_BM * 32), row, p0);
 #pragma unroll
                 for (int q = 0; q < 32; ++q) s0[q] += p0[q];
               }
 #pragma unroll
               for (int q = 0; q < 32; ++q) v0[q] += s0[q];
             }
-            if (m < sh.M) epi(m, n, v0, nvalid);
+            if (nrows > 0) epi(wst, m_wbase, n, v0, nrows, nvalid);
           }
         }
+      }
       }
       tc_fence_before();
       __syncwarp();
@@ -684,7 +881,7 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
           st_release_gpu(sh.sk_flags + cid * 2 + rank, sh.sk_epoch);
         }
       }
-      if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
+      if (++acc == NACC) { acc = 0; acc_phase ^= 1u; }
     }
   }
 
@@ -782,34 +979,57 @@ inline bool gemm_use_streamk() {
   return mode != 0;
 }
 
-template <bool A_MN, bool B_MN, bool DUAL, class Epi>
+// Leftover-tile split factor of the pair kernel for `ntiles` tiles on `clusters` pairs (0: none).
+inline int gemm_tail_split(int ntiles, int clusters, int kblocks) {
+  const int rem = ntiles % clusters;
+  if (ntiles <= clusters || rem == 0) return 0;
+  int s = clusters / rem;
+  if (s > GEMM2_MAX_SPLIT) s = GEMM2_MAX_SPLIT;
+  while (s >= 2 && kblocks / s < 4) --s;                  // at least 4 k-blocks per slice
+  return s >= 2 ? s : 0;
+}
+
+// Pair tile height (MT x 256 rows).  The 512-row tile (MT = 2) needs 25 % less shared-memory fill per flop and ran
+// 3-4 % faster in a sustained stand-alone loop at K = 16384, but inside the layer step its unoverlapped epilogue and
+// shallower pipeline cost more than that (wgrad_gateup 1.23 vs 1.17 ms, down 0.75 vs 0.60 ms; profiles/r1c notes), so
+// the default is MT = 1; LSP_GEMM_MT=2 selects the tall tile (kept for tuning on other shapes, covered by the tests).
+inline int gemm_pick_mt(int M, int N, int K, int pairs, bool use_sk) {
+  static int forced = -1;
+  if (forced < 0) {
+    const char* e = getenv("LSP_GEMM_MT");
+    forced = e ? atoi(e) : 0;
+  }
+  if (forced == 1 || forced == 2) return forced;
+  (void)M; (void)N; (void)K; (void)pairs; (void)use_sk;
+  return 1;
+}
+
+template <bool A_MN, bool B_MN, bool DUAL, int MT, class Epi>
 cudaError_t launch_gemm_pair(const GemmMaps& maps, GemmShape sh, const Epi& epi, int num_sms, cudaStream_t st,
                              const GemmSKRes* sk) {
-  auto kern = gemm_pair_tcgen05_kernel<A_MN, B_MN, DUAL, Epi>;
+  using G = Gemm2Cfg<MT>;
+  auto kern = gemm_pair_tcgen05_kernel<A_MN, B_MN, DUAL, MT, Epi>;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, GEMM2_SMEM_BYTES);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEM_BYTES);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
   constexpr int NOUT = DUAL ? 128 : 256;
-  const int mblocks = (sh.M + 2 * GEMM_BM - 1) / (2 * GEMM_BM), nblocks = (sh.N + NOUT - 1) / NOUT;
+  const int mblocks = (sh.M + 2 * MT * GEMM_BM - 1) / (2 * MT * GEMM_BM), nblocks = (sh.N + NOUT - 1) / NOUT;
   const int ntiles = mblocks * nblocks;
   if (ntiles == 0) return cudaSuccess;
-  sh.band = gemm_band(2 * mblocks) / 2;
+  sh.band = gemm_band(2 * MT * mblocks) / (2 * MT);       // ~2048-row bands
   if (sh.band < 1) sh.band = 1;
   const int pairs = num_sms / 2;
   const int clusters = ntiles < pairs ? ntiles : pairs;
   // split-K tail: the r = ntiles mod clusters leftover tiles are cut into s K-slices when s r <= clusters, s >= 2
   sh.sk_split = 0; sh.sk_partial = nullptr; sh.sk_flags = nullptr; sh.sk_epoch = 0;
-  const int rem = ntiles % clusters;
-  if (sk && sk->partial && gemm_use_streamk() && ntiles > clusters && rem != 0) {
-    int s = clusters / rem;
-    if (s > GEMM2_MAX_SPLIT) s = GEMM2_MAX_SPLIT;
-    while (s >= 2 && sh.kblocks[0] / s < 4) --s;          // at least 4 k-blocks per slice
+  if (sk && sk->partial && gemm_use_streamk()) {
+    const int s = gemm_tail_split(ntiles, clusters, sh.kblocks[0]);
     if (s >= 2) { sh.sk_split = s; sh.sk_partial = sk->partial; sh.sk_flags = sk->flags; sh.sk_epoch = sk->epoch; }
   }
-  kern<<<2 * clusters, GEMM_THREADS, GEMM2_SMEM_BYTES, st>>>(maps, sh, epi);
+  kern<<<2 * clusters, GEMM_THREADS, G::SMEM_BYTES, st>>>(maps, sh, epi);
   return cudaGetLastError();
 }
 
@@ -843,13 +1063,18 @@ cudaError_t gemm_run(int M, int N, int nseg, const Operand* a, const Operand* b,
   sh.M = M; sh.N = N; sh.nseg = nseg;
   sh.a_fmt = umma_fmt(a[0].dt); sh.b_fmt = umma_fmt(b[0].dt);      // all segments share the operand formats
   for (int s = 0; s < GEMM_MAX_SEG; ++s) sh.kblocks[s] = 0;
-  const bool pair = BN == 256 && gemm_use_pair(M);
+  const bool pair = BN == 256 && nseg == 1 && gemm_use_pair(M);
   for (int s = 0; s < nseg; ++s) {
     sh.kblocks[s] = (ks[s] + GEMM_BK - 1) / GEMM_BK;
     if (!encode_operand(&maps.a[s], a[s], M, ks[s], GEMM_BM)) return cudaErrorInvalidValue;
     if (!encode_operand(&maps.b[s], b[s], N, ks[s], pair ? 128 : BN)) return cudaErrorInvalidValue;
   }
-  if (pair) return launch_gemm_pair<A_MN, B_MN, false, Epi>(maps, sh, epi, num_sms, st, nseg == 1 ? sk : nullptr);
+  if (pair) {
+    const bool use_sk = nseg == 1 && sk && sk->partial && gemm_use_streamk();
+    if (nseg == 1 && gemm_pick_mt(M, N, ks[0], num_sms / 2, use_sk) == 2)
+      return launch_gemm_pair<A_MN, B_MN, false, 2, Epi>(maps, sh, epi, num_sms, st, sk);
+    return launch_gemm_pair<A_MN, B_MN, false, 1, Epi>(maps, sh, epi, num_sms, st, nseg == 1 ? sk : nullptr);
+  }
   return launch_gemm<BN, A_MN, B_MN, false, Epi>(maps, sh, epi, num_sms, st);
 }
 
@@ -865,7 +1090,7 @@ cudaError_t gemm_run_dual(int M, int N, int K, const Operand& a, const Operand& 
   if (!encode_operand(&maps.a[0], a, M, K, GEMM_BM)) return cudaErrorInvalidValue;
   if (!encode_operand(&maps.b[0], bg, N, K, 128)) return cudaErrorInvalidValue;
   if (!encode_operand(&maps.b[1], bu, N, K, 128)) return cudaErrorInvalidValue;
-  if (gemm_use_pair(M)) return launch_gemm_pair<false, false, true, Epi>(maps, sh, epi, num_sms, st, sk);
+  if (gemm_use_pair(M)) return launch_gemm_pair<false, false, true, 1, Epi>(maps, sh, epi, num_sms, st, sk);
   return launch_gemm<256, false, false, true, Epi>(maps, sh, epi, num_sms, st);
 }
 

@@ -307,6 +307,9 @@ __device__ __forceinline__ uint32_t pack_f16(float a, float b) {
   __half2 v = __floats2half2_rn(a, b);
   return *reinterpret_cast<uint32_t*>(&v);
 }
+__device__ __forceinline__ void prefetch_l2(const void* p) {
+  asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
 // 2^x on the SFU (one MUFU.EX2; flushes denormals -- inputs here are <= ~2^8, results feed 16-bit operands)
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
