@@ -1,7 +1,7 @@
 // Causal grouped-query flash attention on the 5th-generation tensor cores (sm_100a), head_dim 128, fp16 operands,
 // fp32 accumulation in TMEM.  SURVEY 8(a) F3 (forward, saves the log-sum-exp) -- refs [23],[24],[26],[27],[37].
 //
-// Forward.  One CTA owns 256 consecutive queries of one (batch, head) as two 128-row tiles t = 0,1 that ping-pong:
+// Forward.  A work item is 256 consecutive queries of one (batch, head) as two 128-row tiles t = 0,1 that ping-pong:
 // while the 128 softmax threads of tile t turn S_t = Q_t K_j^T into P_t, the tensor core works on the other tile.
 //   warp 0      TMA producer: Q_0, Q_1 once, then K_j / V_j (128 keys x 128) through two-stage mbarrier rings
 //   warp 1      tcgen05.mma issuer (one thread) and TMEM owner
@@ -14,6 +14,8 @@
 // more than 2^8 for some row of the warp, so the TMEM round trip of O is rare after the first blocks; P <= 2^8 fits
 // fp16 with the same relative precision.  Key blocks above the diagonal are never visited; only the diagonal block
 // is masked.  Rows past the end of a sequence are zero-filled by TMA (3-D maps: column, position, batch).
+// O leaves through per-warp swizzled staging tiles and 32 x 32 TMA stores: per-thread st.global of a row-per-thread
+// fp32 tile stalled the softmax warps ~12 k cycles per item (measured with a clock64 trace), the bulk stores ~1 k.
 #pragma once
 #include "gemm.cuh"
 
@@ -21,6 +23,7 @@ namespace lsp {
 
 struct AttnTcMaps {
   CUtensorMap q, k, v, dO;
+  CUtensorMap o32, o16;          // forward outputs (TMA stores of 32 x 32 chunks out of the swizzled staging tiles)
 };
 
 struct AttnTcParams {
@@ -29,13 +32,14 @@ struct AttnTcParams {
   float scale;
   float* o32; __half* o16; long long ldo;        // [T, ldo] outputs (either may be null)
   float* lse;                                    // [B, nq, S]
+  unsigned int* sched;                           // [2] work-item counter and finished-CTA counter (zero between launches)
 };
 
 constexpr int ATC_D = 128;
 constexpr int ATC_TILE_BYTES = 128 * ATC_D * 2;          // one 128 x 128 fp16 tile = 32 KB (two 64-wide swizzled chunks)
 constexpr int ATC_CHUNK_BYTES = 128 * 128;               // one 64-column chunk of 128 rows
 constexpr int ATC_FWD_THREADS = 320;
-constexpr int ATC_FWD_SMEM = 6 * ATC_TILE_BYTES + 1024 + 256;
+constexpr int ATC_FWD_SMEM = 6 * ATC_TILE_BYTES + 8 * GEMM_STAGE_TILE_BYTES + 1024 + 256;
 constexpr float ATC_RESCALE_LOG2 = 8.0f;
 
 // 3-D map over a [B*S, ld] fp16 matrix seen as (column, position, batch); box = 64 columns x box_rows positions.
@@ -49,6 +53,22 @@ inline bool make_map_attn(CUtensorMap* m, const void* base, int ncols, int S, in
   return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// 3-D map (column, position, batch) over a [B*S, ld] matrix of 4- or 2-byte elements for 32-column x 32-row chunk
+// stores out of a staging tile: 128-byte rows with the 128B swizzle (fp32), 64-byte rows with the 64B swizzle (16-bit)
+// -- exactly the XOR patterns of WarpStage::put_row32 / put_row16.
+inline bool make_map_store(CUtensorMap* m, const void* base, int ncols, int S, int B, long long ld, bool f32) {
+  PFN_encodeTiled fn = get_encode_fn();
+  if (!fn) return false;
+  const cuuint64_t es = f32 ? 4 : 2;
+  cuuint64_t dims[3] = {static_cast<cuuint64_t>(ncols), static_cast<cuuint64_t>(S), static_cast<cuuint64_t>(B)};
+  cuuint64_t strides[2] = {static_cast<cuuint64_t>(ld) * es, static_cast<cuuint64_t>(ld) * es * static_cast<cuuint64_t>(S)};
+  cuuint32_t box[3] = {32u, 32u, 1u};
+  cuuint32_t estr[3] = {1u, 1u, 1u};
+  return fn(m, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, const_cast<void*>(base), dims, strides,
+            box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, f32 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B,
+            CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 // A 128-row x 128-column fp16 tile lands as two chunks of [128 rows x 128 B].
@@ -69,6 +89,28 @@ __device__ __forceinline__ uint64_t atc_desc_mnmajor(uint32_t tile, int kk) {
   return umma_smem_desc(tile + kk * 2048, ATC_CHUNK_BYTES, 1024);
 }
 
+// Persistent: one CTA per SM walks work items (256-query block, head, batch) handed out heaviest-first by a global
+// atomic counter (p.sched).  Items are pipelined inside the CTA: the next item's Q tiles are fetched as soon as the
+// last S MMA of the current one has read them (q_empty), its first S = Q K^T is issued right after the current item's
+// last P V, and the O epilogue of a tile (TMEM -> registers -> staging tile -> coalesced global stores) overlaps the
+// other tile's and the next item's MMAs (o_free tells the MMA warp when O_t may be overwritten).  The ~19 k cycles of
+// fill / drain / launch that every one of the 1536 one-shot CTAs paid before are gone (profiles/r1c_attn_notes.md).
+struct AttnItem { int q0, h, b, kvh, n0, n1, nmax; };
+__device__ __forceinline__ AttnItem attn_fwd_item(uint32_t i, const AttnTcParams& p, int nqb) {
+  const int per_lvl = p.nq * p.B;
+  const int lvl = static_cast<int>(i) / per_lvl, r = static_cast<int>(i) - lvl * per_lvl;
+  AttnItem it;
+  it.q0 = (nqb - 1 - lvl) * 256;                               // heavy (late) query blocks first
+  it.b = r / p.nq; it.h = r - it.b * p.nq;
+  it.kvh = it.h / (p.nq / p.nkv);
+  // key blocks per tile: tile t covers queries [q0 + 128 t, +128); causal => keys [0, q0 + 128 t + 128)
+  it.n0 = it.q0 / 128 + 1;
+  it.n1 = (it.q0 + 128 < p.S) ? it.n0 + 1 : 0;
+  it.nmax = it.n1 > it.n0 ? it.n1 : it.n0;
+  return it;
+}
+constexpr int ATC_ITEM_RING = 4;
+
 __global__ void __launch_bounds__(ATC_FWD_THREADS, 1)
 attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p) {
   extern __shared__ uint8_t smem_raw[];
@@ -76,7 +118,8 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
   const uint32_t sQ = smem_base;                              // 2 tiles
   const uint32_t sK = sQ + 2 * ATC_TILE_BYTES;                // 2 stages
   const uint32_t sV = sK + 2 * ATC_TILE_BYTES;                // 2 stages
-  const uint32_t bar_base = sV + 2 * ATC_TILE_BYTES;
+  const uint32_t stage_tiles = sV + 2 * ATC_TILE_BYTES;       // 8 softmax warps x 4 KB staging tiles (epilogue)
+  const uint32_t bar_base = stage_tiles + 8 * GEMM_STAGE_TILE_BYTES;
   auto q_full = [&](int t) { return bar_base + 8u * t; };
   auto k_full = [&](int s) { return bar_base + 8u * (2 + s); };
   auto k_empty = [&](int s) { return bar_base + 8u * (4 + s); };
@@ -85,27 +128,28 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
   auto s_full = [&](int t) { return bar_base + 8u * (10 + t); };
   auto p_full = [&](int t) { return bar_base + 8u * (12 + t); };
   auto o_full = [&](int t) { return bar_base + 8u * (14 + t); };
-  const uint32_t tmem_slot = bar_base + 8u * 16;
+  auto q_empty = [&](int t) { return bar_base + 8u * (16 + t); };
+  auto o_free = [&](int t) { return bar_base + 8u * (18 + t); };
+  auto item_bar = [&](int s) { return bar_base + 8u * (20 + s); };
+  const uint32_t item_slots = bar_base + 8u * (20 + ATC_ITEM_RING);
+  const uint32_t tmem_slot = item_slots + 4u * ATC_ITEM_RING;
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+  volatile uint32_t* item_slot_ptr = reinterpret_cast<volatile uint32_t*>(smem_raw + (item_slots - smem_u32(smem_raw)));
 
   const int warp = warp_idx_uniform(), lane = threadIdx.x & 31;
-  const int qb = gridDim.x - 1 - blockIdx.x;                  // heavy (late) query blocks first
-  const int h = blockIdx.y, b = blockIdx.z;
-  const int kvh = h / (p.nq / p.nkv);
-  const int q0 = qb * 256;
-  // key blocks per tile: tile t covers queries [q0 + 128 t, +128); causal => keys [0, q0 + 128 t + 128)
-  const int n0 = q0 / 128 + 1;
-  const int n1 = (q0 + 128 < p.S) ? n0 + 1 : 0;
-  const int nmax = n1 > n0 ? n1 : n0;
+  const int nqb = (p.S + 255) / 256;
+  const uint32_t nitems = static_cast<uint32_t>(nqb * p.nq * p.B);
 
   if (threadIdx.x == 0) {
     tma_prefetch_desc(&maps.q); tma_prefetch_desc(&maps.k); tma_prefetch_desc(&maps.v);
+    tma_prefetch_desc(&maps.o32); tma_prefetch_desc(&maps.o16);
     for (int i = 0; i < 2; ++i) {
-      mbar_init(q_full(i), 1);
+      mbar_init(q_full(i), 1); mbar_init(q_empty(i), 1);
       mbar_init(k_full(i), 1); mbar_init(k_empty(i), 1);
       mbar_init(v_full(i), 1); mbar_init(v_empty(i), 1);
-      mbar_init(s_full(i), 1); mbar_init(p_full(i), 4); mbar_init(o_full(i), 1);
+      mbar_init(s_full(i), 1); mbar_init(p_full(i), 4); mbar_init(o_full(i), 1); mbar_init(o_free(i), 4);
     }
+    for (int i = 0; i < ATC_ITEM_RING; ++i) mbar_init(item_bar(i), 1);
     fence_barrier_init();
   }
   if (warp == 1) {
@@ -117,26 +161,54 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
 
+  // item `it` of this CTA: published by the producer thread in slot it % ATC_ITEM_RING (slot reuse is safe: the
+  // producer can be at most two items ahead of the slowest reader, see the q_empty / o_free dependencies)
+  auto get_item = [&](uint32_t it) -> uint32_t {
+    mbar_wait(item_bar(it % ATC_ITEM_RING), (it / ATC_ITEM_RING) & 1u);
+    return item_slot_ptr[it % ATC_ITEM_RING];
+  };
+
   if (warp == 0) {
-    // ===================================================================== TMA producer
+    // ===================================================================== scheduler + TMA producer
     if (lane == 0) {
-      atc_load_tile(sQ, &maps.q, q_full(0), h * ATC_D, q0, b);
-      if (n1 > 0) atc_load_tile(sQ + ATC_TILE_BYTES, &maps.q, q_full(1), h * ATC_D, q0 + 128, b);
-      for (int j = 0; j < nmax; ++j) {
-        const int st = j & 1;
-        const uint32_t ph = ((j >> 1) & 1) ^ 1u;
-        mbar_wait(k_empty(st), ph);
-        atc_load_tile(sK + st * ATC_TILE_BYTES, &maps.k, k_full(st), kvh * ATC_D, j * 128, b);
-        mbar_wait(v_empty(st), ph);
-        atc_load_tile(sV + st * ATC_TILE_BYTES, &maps.v, v_full(st), kvh * ATC_D, j * 128, b);
+      auto publish = [&](uint32_t it, uint32_t item) {
+        item_slot_ptr[it % ATC_ITEM_RING] = item;
+        mbar_arrive(item_bar(it % ATC_ITEM_RING));             // release: the slot write is visible to the waiters
+      };
+      uint32_t kvc = 0, qc0 = 0, qc1 = 0;                      // K/V blocks and Q tiles loaded so far
+      uint32_t item = atomicAdd(p.sched, 1u);
+      publish(0, item);
+      for (uint32_t it = 0; item < nitems; ++it) {
+        const AttnItem w = attn_fwd_item(item, p, nqb);
+        mbar_wait(q_empty(0), (qc0 & 1u) ^ 1u);
+        atc_load_tile(sQ, &maps.q, q_full(0), w.h * ATC_D, w.q0, w.b);
+        ++qc0;
+        if (w.n1 > 0) {
+          mbar_wait(q_empty(1), (qc1 & 1u) ^ 1u);
+          atc_load_tile(sQ + ATC_TILE_BYTES, &maps.q, q_full(1), w.h * ATC_D, w.q0 + 128, w.b);
+          ++qc1;
+        }
+        const uint32_t next = atomicAdd(p.sched, 1u);          // latency hidden behind this item's K/V stream
+        for (int j = 0; j < w.nmax; ++j, ++kvc) {
+          const int st = kvc & 1;
+          const uint32_t ph = ((kvc >> 1) & 1u) ^ 1u;
+          mbar_wait(k_empty(st), ph);
+          atc_load_tile(sK + st * ATC_TILE_BYTES, &maps.k, k_full(st), w.kvh * ATC_D, j * 128, w.b);
+          mbar_wait(v_empty(st), ph);
+          atc_load_tile(sV + st * ATC_TILE_BYTES, &maps.v, v_full(st), w.kvh * ATC_D, j * 128, w.b);
+        }
+        publish(it + 1, next);
+        item = next;
       }
+      // the grid's last CTA re-arms the counters for the next launch on this context
+      __threadfence();
+      if (atomicAdd(p.sched + 1, 1u) == gridDim.x - 1) { p.sched[0] = 0; p.sched[1] = 0; __threadfence(); }
     }
   } else if (warp == 1) {
     // ===================================================================== MMA issuer (whole warp, elected lane issues)
     const uint32_t leader = elect_one();
     const uint32_t idesc_s = umma_idesc(128, 128, 0, 0, 0, 0);     // S = Q K^T : both K-major
     const uint32_t idesc_pv = umma_idesc(128, 128, 0, 0, 0, 1);    // O += P V  : A from TMEM, B (V) MN-major
-    const int nt[2] = {n0, n1};
     const uint64_t dq0 = umma_smem_desc(sQ, 16, 1024), dk0 = umma_smem_desc(sK, 16, 1024);
     const uint64_t dv0 = umma_smem_desc(sV, ATC_CHUNK_BYTES, 1024);
     auto issue_s = [&](int t, int kst) {
@@ -160,139 +232,194 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
         umma_commit(o_full(t));
       }
     };
-    mbar_wait(k_full(0), 0);
-    mbar_wait(q_full(0), 0);
-    tc_fence_after();
-    issue_s(0, 0);
-    if (n1 > 0) { mbar_wait(q_full(1), 0); tc_fence_after(); issue_s(1, 0); }
-    if (leader) umma_commit(k_empty(0));
-    for (int j = 0; j < nmax; ++j) {
-      const int st = j & 1;
-      const uint32_t ph = (j >> 1) & 1;
-      mbar_wait(v_full(st), ph);
-      bool knext_ready = false;
-      for (int t = 0; t < 2; ++t) {
-        if (j < nt[t]) {
-          mbar_wait(p_full(t), j & 1);
-          tc_fence_after();
-          issue_pv(t, st, j > 0);
+    uint32_t kvc = 0;                          // K/V blocks consumed so far (ring position of this item's block 0)
+    uint32_t qc[2] = {0, 0};                   // items seen per tile (q_full / o_free phases)
+    uint32_t pc[2] = {0, 0};                   // P blocks consumed per tile (p_full phase)
+    for (uint32_t it = 0;; ++it) {
+      const uint32_t item = get_item(it);
+      if (item >= nitems) break;
+      const AttnItem w = attn_fwd_item(item, p, nqb);
+      const int nt[2] = {w.n0, w.n1};
+      // first S of both tiles (for the second and later items this overlaps the previous item's epilogues)
+      {
+        const int st0 = kvc & 1;
+        mbar_wait(k_full(st0), (kvc >> 1) & 1u);
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+          if (nt[t] > 0) {
+            mbar_wait(q_full(t), qc[t] & 1u);
+            tc_fence_after();
+            issue_s(t, st0);
+            if (nt[t] == 1 && leader) umma_commit(q_empty(t));       // that was this tile's last S of the item
+          }
         }
-        if (j + 1 < nt[t]) {
-          if (!knext_ready) { mbar_wait(k_full(st ^ 1), ((j + 1) >> 1) & 1); tc_fence_after(); knext_ready = true; }
-          issue_s(t, st ^ 1);
+        if (leader) umma_commit(k_empty(st0));
+      }
+      for (int j = 0; j < w.nmax; ++j) {
+        const uint32_t kc = kvc + j;
+        const int st = kc & 1;
+        mbar_wait(v_full(st), (kc >> 1) & 1u);
+        bool knext_ready = false;
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+          if (j < nt[t]) {
+            mbar_wait(p_full(t), pc[t] & 1u);
+            ++pc[t];
+            if (j == 0 && qc[t] > 0) mbar_wait(o_free(t), (qc[t] - 1u) & 1u);   // previous item's O_t has been read out
+            tc_fence_after();
+            issue_pv(t, st, j > 0);
+          }
+          if (j + 1 < nt[t]) {
+            if (!knext_ready) { mbar_wait(k_full(st ^ 1), ((kc + 1) >> 1) & 1u); tc_fence_after(); knext_ready = true; }
+            issue_s(t, st ^ 1);
+            if (j + 2 == nt[t] && leader) umma_commit(q_empty(t));   // last S of this tile: Q_t may be refilled
+          }
+        }
+        if (leader) {
+          umma_commit(v_empty(st));
+          if (j + 1 < w.nmax) umma_commit(k_empty(st ^ 1));
         }
       }
-      if (leader) {
-        umma_commit(v_empty(st));
-        if (j + 1 < nmax) umma_commit(k_empty(st ^ 1));
-      }
+      kvc += w.nmax;
+      if (nt[0] > 0) ++qc[0];
+      if (nt[1] > 0) ++qc[1];
     }
   } else {
     // ===================================================================== softmax warps: tile t, TMEM lane quarter
     const int t = (warp - 2) >> 2;
     const int quarter = warp & 3;
-    const int nblk = t == 0 ? n0 : n1;
     const int row = quarter * 32 + lane;                         // query row within the tile = TMEM lane
-    const int qi = q0 + t * 128 + row;                           // position in the sequence
     const uint32_t lane_off = static_cast<uint32_t>(quarter * 32) << 16;
     const uint32_t tS = tmem_base + lane_off + t * 128;
     const uint32_t tO = tmem_base + lane_off + 256 + t * 128;
+    const WarpStage wst{stage_tiles + static_cast<uint32_t>(warp - 2) * GEMM_STAGE_TILE_BYTES, lane};
     const float c = p.scale_log2;
-    float m_run = -INFINITY, l_run = 0.f;
+    uint32_t cnt = 0;                                            // key blocks this tile has processed (all items)
 
-    for (int j = 0; j < nblk; ++j) {
-      mbar_wait(s_full(t), j & 1);
-      tc_fence_after();
-      uint32_t sr[4][32];
+    for (uint32_t it = 0;; ++it) {
+      const uint32_t item = get_item(it);
+      if (item >= nitems) break;
+      const AttnItem w = attn_fwd_item(item, p, nqb);
+      const int nblk = t == 0 ? w.n0 : w.n1;
+      if (nblk == 0) continue;
+      const int qi = w.q0 + t * 128 + row;                       // position in the sequence
+      float m_run = -INFINITY, l_run = 0.f;
+
+      for (int j = 0; j < nblk; ++j, ++cnt) {
+        mbar_wait(s_full(t), cnt & 1u);
+        tc_fence_after();
+        uint32_t sr[4][32];
 #pragma unroll
-      for (int q = 0; q < 4; ++q) tmem_ld32(tS + q * 32, sr[q]);
-      tmem_ld_wait();
-      float (&s)[4][32] = reinterpret_cast<float(&)[4][32]>(sr);
-      if (j == nblk - 1) {                                       // diagonal block: key 128 j + cidx > query <=> cidx > row
+        for (int q = 0; q < 4; ++q) tmem_ld32(tS + q * 32, sr[q]);
+        tmem_ld_wait();
+        float (&s)[4][32] = reinterpret_cast<float(&)[4][32]>(sr);
+        if (j == nblk - 1) {                                     // diagonal block: key 128 j + cidx > query <=> cidx > row
 #pragma unroll
-        for (int q = 0; q < 4; ++q)
+          for (int q = 0; q < 4; ++q)
 #pragma unroll
-          for (int i = 0; i < 32; ++i)
-            if (q * 32 + i > row) s[q][i] = -INFINITY;
-      }
-      float mx0 = s[0][0], mx1 = s[1][0], mx2 = s[2][0], mx3 = s[3][0];
+            for (int i = 0; i < 32; ++i)
+              if (q * 32 + i > row) s[q][i] = -INFINITY;
+        }
+        float mx0 = s[0][0], mx1 = s[1][0], mx2 = s[2][0], mx3 = s[3][0];
 #pragma unroll
-      for (int i = 1; i < 32; ++i) {
-        mx0 = fmaxf(mx0, s[0][i]); mx1 = fmaxf(mx1, s[1][i]); mx2 = fmaxf(mx2, s[2][i]); mx3 = fmaxf(mx3, s[3][i]);
-      }
-      const float m_new = fmaxf(m_run, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)));
-      float m_use = m_run;
-      if (j == 0) {
-        m_use = m_new;
-      } else {
-        const bool grow = (m_new - m_run) * c > ATC_RESCALE_LOG2;
-        if (__any_sync(0xffffffffu, grow)) {
-          // raise the reference maximum of every row of this warp and rescale O_t in TMEM
-          const float alpha = ex2_approx((m_run - m_new) * c);
+        for (int i = 1; i < 32; ++i) {
+          mx0 = fmaxf(mx0, s[0][i]); mx1 = fmaxf(mx1, s[1][i]); mx2 = fmaxf(mx2, s[2][i]); mx3 = fmaxf(mx3, s[3][i]);
+        }
+        const float m_new = fmaxf(m_run, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)));
+        float m_use = m_run;
+        if (j == 0) {
           m_use = m_new;
-          l_run *= alpha;
-          mbar_wait(o_full(t), (j - 1) & 1);                     // P_t V_{j-1} has landed in O_t
-          tc_fence_after();
+        } else {
+          const bool grow = (m_new - m_run) * c > ATC_RESCALE_LOG2;
+          if (__any_sync(0xffffffffu, grow)) {
+            // raise the reference maximum of every row of this warp and rescale O_t in TMEM
+            const float alpha = ex2_approx((m_run - m_new) * c);
+            m_use = m_new;
+            l_run *= alpha;
+            mbar_wait(o_full(t), (cnt - 1u) & 1u);               // P_t V_{j-1} has landed in O_t
+            tc_fence_after();
 #pragma unroll 1
-          for (int q = 0; q < 8; ++q) {                          // 16 columns at a time: S stays in registers
-            uint32_t orr[16];
-            tmem_ld16(tO + q * 16, orr);
-            tmem_ld_wait();
+            for (int q = 0; q < 8; ++q) {                        // 16 columns at a time: S stays in registers
+              uint32_t orr[16];
+              tmem_ld16(tO + q * 16, orr);
+              tmem_ld_wait();
 #pragma unroll
-            for (int i = 0; i < 16; ++i) orr[i] = __float_as_uint(__uint_as_float(orr[i]) * alpha);
-            tmem_st16(tO + q * 16, orr);
+              for (int i = 0; i < 16; ++i) orr[i] = __float_as_uint(__uint_as_float(orr[i]) * alpha);
+              tmem_st16(tO + q * 16, orr);
+            }
           }
         }
-      }
-      m_run = m_use;
-      const float neg = -m_use * c;
-      // P = 2^(s c - m c): FFMA2 + 2 MUFU + FADD2 + F2FP per key pair
-      const float2 c2 = make_float2(c, c), neg2 = make_float2(neg, neg);
-      float2 acc0 = make_float2(0.f, 0.f), acc1 = make_float2(0.f, 0.f);
+        m_run = m_use;
+        const float neg = -m_use * c;
+        // P = 2^(s c - m c): FFMA2 + 2 MUFU + FADD2 + F2FP per key pair
+        const float2 c2 = make_float2(c, c), neg2 = make_float2(neg, neg);
+        float2 acc0 = make_float2(0.f, 0.f), acc1 = make_float2(0.f, 0.f);
 #pragma unroll
-      for (int q = 0; q < 2; ++q) {
-        uint32_t pk[32];
+        for (int q = 0; q < 2; ++q) {
+          uint32_t pk[32];
 #pragma unroll
-        for (int i = 0; i < 16; ++i) {
-          float2 a = ffma2(make_float2(s[2 * q][2 * i], s[2 * q][2 * i + 1]), c2, neg2);
-          float2 b = ffma2(make_float2(s[2 * q + 1][2 * i], s[2 * q + 1][2 * i + 1]), c2, neg2);
-          a.x = ex2_approx(a.x); a.y = ex2_approx(a.y); b.x = ex2_approx(b.x); b.y = ex2_approx(b.y);
-          acc0 = fadd2(acc0, a); acc1 = fadd2(acc1, b);
-          pk[i] = pack_f16(a.x, a.y);
-          pk[16 + i] = pack_f16(b.x, b.y);
+          for (int i = 0; i < 16; ++i) {
+            float2 a = ffma2(make_float2(s[2 * q][2 * i], s[2 * q][2 * i + 1]), c2, neg2);
+            float2 b2 = ffma2(make_float2(s[2 * q + 1][2 * i], s[2 * q + 1][2 * i + 1]), c2, neg2);
+            a.x = ex2_approx(a.x); a.y = ex2_approx(a.y); b2.x = ex2_approx(b2.x); b2.y = ex2_approx(b2.y);
+            acc0 = fadd2(acc0, a); acc1 = fadd2(acc1, b2);
+            pk[i] = pack_f16(a.x, a.y);
+            pk[16 + i] = pack_f16(b2.x, b2.y);
+          }
+          tmem_st32(tS + q * 32, pk);                            // P_t: keys 64 q .. 64 q + 63 -> 32 columns
         }
-        tmem_st32(tS + q * 32, pk);                              // P_t: keys 64 q .. 64 q + 63 -> 32 columns
+        l_run += (acc0.x + acc0.y) + (acc1.x + acc1.y);
+        tmem_st_wait();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(p_full(t));
       }
-      const float sum0 = acc0.x + acc0.y, sum1 = acc1.x + acc1.y;
-      l_run += sum0 + sum1;
-      tmem_st_wait();
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(p_full(t));
-    }
 
-    if (nblk > 0) {
-      mbar_wait(o_full(t), (nblk - 1) & 1);
+      // epilogue of this tile: O_t / l -> o32, o16 (coalesced through the staging tile), LSE; then release O_t
+      mbar_wait(o_full(t), (cnt - 1u) & 1u);
       tc_fence_after();
       const bool valid = qi < p.S;
       const float inv = 1.0f / l_run;
-      const long long tok = static_cast<long long>(b) * p.S + qi;
-      if (valid) p.lse[(static_cast<long long>(b) * p.nq + h) * p.S + qi] = (m_run * c + log2f(l_run)) * 0.6931471805599453f;
-#pragma unroll
+      if (valid) p.lse[(static_cast<long long>(w.b) * p.nq + w.h) * p.S + qi] = (m_run * c + log2f(l_run)) * 0.6931471805599453f;
+      const int r_base = w.q0 + t * 128 + quarter * 32;          // first row of this warp
+      const int nrows = min(32, p.S - r_base);
+#pragma unroll 1
       for (int q = 0; q < 4; ++q) {
         uint32_t orr[32];
         tmem_ld32(tO + q * 32, orr);
         tmem_ld_wait();
+        if (q == 3) {                                            // O_t is in registers: the next item's P V may overwrite it
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(o_free(t));
+        }
         float (&o)[32] = reinterpret_cast<float(&)[32]>(orr);
 #pragma unroll
         for (int i = 0; i < 32; ++i) o[i] *= inv;
-        if (valid) {
-          const long long off = tok * p.ldo + h * ATC_D + q * 32;
-          if (p.o32) store_row32<DT_F32>(p.o32 + off, o, 32);
-          if (p.o16) store_row32<DT_F16>(p.o16 + off, o, 32);
+        if (nrows > 0) {                                         // rows past the sequence end are clipped by the map
+          if (p.o32) {
+            if (lane == 0) tma_store_wait_read<0>();             // the previous store has read the tile
+            __syncwarp();
+            wst.put_row32(o);
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) { tma_store_3d(&maps.o32, wst.base, w.h * ATC_D + q * 32, r_base, w.b); tma_store_commit(); }
+          }
+          if (p.o16) {
+            uint32_t wv[16];
+#pragma unroll
+            for (int i = 0; i < 16; ++i) wv[i] = pack_f16(o[2 * i], o[2 * i + 1]);
+            if (lane == 0) tma_store_wait_read<0>();
+            __syncwarp();
+            wst.put_row16(wv);
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) { tma_store_3d(&maps.o16, wst.base, w.h * ATC_D + q * 32, r_base, w.b); tma_store_commit(); }
+          }
         }
       }
     }
+    if (lane == 0) tma_store_wait_all<0>();                      // this thread's bulk stores have been written
   }
 
   tc_fence_before();
@@ -305,7 +432,7 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
 
 // q [B*S, ldq] (head h at columns h*128), k, v [B*S, ldk/ldv] (kv head at columns kvh*128), all fp16.
 inline cudaError_t attn_fwd_tc_launch(const __half* q, long long ldq, const __half* k, long long ldk, const __half* v,
-                                      long long ldv, const AttnTcParams& p, cudaStream_t st) {
+                                      long long ldv, const AttnTcParams& p, int num_sms, cudaStream_t st) {
   static bool set = false;
   if (!set) {
     cudaError_t e = cudaFuncSetAttribute(attn_fwd_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_FWD_SMEM);
@@ -317,7 +444,11 @@ inline cudaError_t attn_fwd_tc_launch(const __half* q, long long ldq, const __ha
       !make_map_attn(&maps.v, v, p.nkv * ATC_D, p.S, p.B, ldv))
     return cudaErrorInvalidValue;
   maps.dO = maps.q;
-  dim3 grid((p.S + 255) / 256, p.nq, p.B);
+  maps.o32 = maps.q; maps.o16 = maps.q;
+  if (p.o32 && !make_map_store(&maps.o32, p.o32, p.nq * ATC_D, p.S, p.B, p.ldo, true)) return cudaErrorInvalidValue;
+  if (p.o16 && !make_map_store(&maps.o16, p.o16, p.nq * ATC_D, p.S, p.B, p.ldo, false)) return cudaErrorInvalidValue;
+  const int nitems = ((p.S + 255) / 256) * p.nq * p.B;
+  const int grid = nitems < num_sms ? nitems : num_sms;        // persistent: one CTA per SM
   attn_fwd_tc_kernel<<<grid, ATC_FWD_THREADS, ATC_FWD_SMEM, st>>>(maps, p);
   return cudaGetLastError();
 }

@@ -60,6 +60,7 @@ struct lsp_ctx {
   float* sk_partial;             // stream-K partial accumulators, [num_sms/2][256 x 256] fp32 (device)
   unsigned int* sk_flags;        // [num_sms/2][2] publication epochs (device, zeroed at create)
   unsigned int gemm_seq;         // launches so far: epoch of the next stream-K launch
+  unsigned int* attn_sched;      // work-item counters of the persistent attention kernels (device, zero between launches)
   int norm_blocks;      // persistent grid of the RMSNorm backward
   SavedLayout sv;
   WsLayout ws;
@@ -268,8 +269,8 @@ cudaError_t attn_fwd_dispatch(const lsp_ctx* c, const AttnParams& p, cudaStream_
   if (c->d.head_dim == 128) {
     AttnTcParams t;
     t.B = p.B; t.S = p.S; t.nq = p.nq; t.nkv = p.nkv; t.scale_log2 = p.scale_log2; t.scale = p.scale;
-    t.o32 = p.o32; t.o16 = p.o16; t.ldo = p.ldo; t.lse = p.lse;
-    return attn_fwd_tc_launch(p.q, p.ldq, p.k, p.ldk, p.v, p.ldv, t, st);
+    t.o32 = p.o32; t.o16 = p.o16; t.ldo = p.ldo; t.lse = p.lse; t.sched = c->attn_sched;
+    return attn_fwd_tc_launch(p.q, p.ldq, p.k, p.ldk, p.v, p.ldv, t, c->num_sms, st);
   }
   return attn_fwd_launch<64>(p, st);
 }
@@ -531,8 +532,10 @@ lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device
     const size_t pairs = static_cast<size_t>(ctx->num_sms / 2);
     if (cudaMalloc(&ctx->sk_partial, pairs * GEMM2_PARTIAL_FLOATS * sizeof(float)) != cudaSuccess ||
         cudaMalloc(&ctx->sk_flags, pairs * 2 * sizeof(unsigned int)) != cudaSuccess ||
-        cudaMemset(ctx->sk_flags, 0, pairs * 2 * sizeof(unsigned int)) != cudaSuccess) {
-      cudaFree(ctx->sk_partial); cudaFree(ctx->sk_flags); cudaFree(ctx->rope); delete ctx;
+        cudaMemset(ctx->sk_flags, 0, pairs * 2 * sizeof(unsigned int)) != cudaSuccess ||
+        cudaMalloc(&ctx->attn_sched, 16 * sizeof(unsigned int)) != cudaSuccess ||
+        cudaMemset(ctx->attn_sched, 0, 16 * sizeof(unsigned int)) != cudaSuccess) {
+      cudaFree(ctx->sk_partial); cudaFree(ctx->sk_flags); cudaFree(ctx->attn_sched); cudaFree(ctx->rope); delete ctx;
       return LSP_ENOMEM;
     }
   }
@@ -546,6 +549,7 @@ lsp_status lsp_destroy(lsp_ctx* ctx) {
   cudaFree(ctx->rope);
   cudaFree(ctx->sk_partial);
   cudaFree(ctx->sk_flags);
+  cudaFree(ctx->attn_sched);
   delete ctx;
   return LSP_OK;
 }
