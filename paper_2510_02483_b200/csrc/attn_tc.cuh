@@ -24,6 +24,7 @@ namespace lsp {
 struct AttnTcMaps {
   CUtensorMap q, k, v, dO;
   CUtensorMap o32, o16;          // forward outputs (TMA stores of 32 x 32 chunks out of the swizzled staging tiles)
+  CUtensorMap g32[2], g16[2];    // backward outputs: dK/dV kernel [0] = dv, [1] = dk; dQ kernel [0] = dq
 };
 
 struct AttnTcParams {
@@ -475,9 +476,9 @@ constexpr int ATC_BWD_THREADS = 320;
 // early rows are O(1) while the tensor-wide rms the parity metric divides by shrinks like sqrt(ln S / S), so a
 // single fp16 rounding there is what limits dq/dk/dv at long S (P-5/P-6).
 constexpr int ATC_SPLIT_ROWS = 256;
-constexpr int ATC_NST = 4;                                 // stages of the streamed 64-row tiles
+constexpr int ATC_NST = 3;                                 // stages of the streamed 64-row tiles
 constexpr int ATC_HALF_TILE = 64 * ATC_D * 2;              // 64 x 128 fp16 = 16 KB (two 8 KB chunks)
-constexpr int ATC_BWD_SMEM = 2 * ATC_TILE_BYTES + 2 * ATC_NST * ATC_HALF_TILE + ATC_NST * 2 * 64 * 4 + 1024 + 256;
+constexpr int ATC_BWD_SMEM = 2 * ATC_TILE_BYTES + 2 * ATC_NST * ATC_HALF_TILE + ATC_NST * 2 * 64 * 4 + 8 * GEMM_STAGE_TILE_BYTES + 2048 + 256;
 
 struct AttnTcBwdParams {
   int B, S, nq, nkv;
@@ -514,8 +515,10 @@ __device__ __forceinline__ void atc_split_pack(float x0, float x1, uint32_t& hi,
   lo = *reinterpret_cast<const uint32_t*>(&l);
 }
 
-// Scale, optionally rotate by -theta (transpose of the forward rotation), and store 32 columns of one row.
-__device__ __forceinline__ void atc_store_grad32(float (&v)[32], float scale, const float2* rope_row, float* o32, __half* o16) {
+// Scale, optionally rotate by -theta (transpose of the forward rotation) 32 columns of this thread's row, then write the
+// warp's 32 x 32 chunk (rows s0.., columns col0.., batch b) with bulk tensor stores out of the staging tile.
+__device__ __forceinline__ void atc_store_grad32(const WarpStage& st, float (&v)[32], float scale, const float2* rope_row,
+                                                 const CUtensorMap* m32, const CUtensorMap* m16, int col0, int s0, int b) {
 #pragma unroll
   for (int i = 0; i < 16; ++i) {
     float z0 = v[2 * i] * scale, z1 = v[2 * i + 1] * scale;
@@ -526,8 +529,8 @@ __device__ __forceinline__ void atc_store_grad32(float (&v)[32], float scale, co
     }
     v[2 * i] = z0; v[2 * i + 1] = z1;
   }
-  if (o32) store_row32<DT_F32>(o32, v, 32);
-  if (o16) store_row32<DT_F16>(o16, v, 32);
+  if (m32) chunk_store_tma3<DT_F32>(st, m32, col0, s0, b, v);
+  if (m16) chunk_store_tma3<DT_F16>(st, m16, col0, s0, b, v);
 }
 
 // --------------------------------------------------------------------------------------------- dK, dV
@@ -539,7 +542,8 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
   const uint32_t sQ = sV + ATC_TILE_BYTES;                       // ATC_NST stages of 64 x 128
   const uint32_t sDO = sQ + ATC_NST * ATC_HALF_TILE;
   const uint32_t sLD = sDO + ATC_NST * ATC_HALF_TILE;            // [stage][L*log2e (64) | D (64)] fp32
-  const uint32_t bar_base = sLD + ATC_NST * 2 * 64 * 4;
+  const uint32_t stage_tiles = (sLD + ATC_NST * 2 * 64 * 4 + 1023u) & ~1023u;   // 8 x 4 KB staging tiles (epilogue)
+  const uint32_t bar_base = stage_tiles + 8 * GEMM_STAGE_TILE_BYTES;
   float* sLD_ptr = reinterpret_cast<float*>(smem_raw + (sLD - smem_u32(smem_raw)));
   auto kv_full = [&]() { return bar_base; };
   auto acc_full = [&]() { return bar_base + 8u; };
@@ -738,29 +742,30 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
       __syncwarp();
       if (lane == 0) mbar_arrive(ds_full(buf));
     }
-    // epilogue: this thread stores columns [64 half, 64 half + 64) of its key row of dV and dK
+    // epilogue: this warp stores rows [32 quarter, +32), columns [64 half, 64 half + 64) of dV and dK
     mbar_wait(acc_full(), 0);
     tc_fence_after();
     const int key = k0 + row;
     const bool valid = key < p.S;
-    const long long tok = static_cast<long long>(b) * p.S + key;
-#pragma unroll
-    for (int q = 0; q < 2; ++q) {
-      const int cc = half * 64 + q * 32;
-      uint32_t a[32];
-      tmem_ld32(tmem_base + lane_off + 256 + cc, a);
-      tmem_ld_wait();
-      if (valid)
-        atc_store_grad32(reinterpret_cast<float(&)[32]>(a), 1.0f, nullptr,
-                         p.dv32 ? p.dv32 + tok * p.lddk32 + kvh * ATC_D + cc : nullptr,
-                         p.dv16 ? p.dv16 + tok * p.ldd16 + kvh * ATC_D + cc : nullptr);
-      tmem_ld32(tmem_base + lane_off + 384 + cc, a);
-      tmem_ld_wait();
-      if (valid)
-        atc_store_grad32(reinterpret_cast<float(&)[32]>(a), p.scale, p.rope ? p.rope + static_cast<long long>(key) * 64 + (cc >> 1) : nullptr,
-                         p.dk32 ? p.dk32 + tok * p.lddk32 + kvh * ATC_D + cc : nullptr,
-                         p.dk16 ? p.dk16 + tok * p.ldd16 + kvh * ATC_D + cc : nullptr);
+    const WarpStage wst{stage_tiles + static_cast<uint32_t>(warp - 2) * GEMM_STAGE_TILE_BYTES, lane};
+    const int s0 = k0 + quarter * 32;
+    if (s0 < p.S) {
+#pragma unroll 1
+      for (int q = 0; q < 2; ++q) {
+        const int cc = half * 64 + q * 32;
+        uint32_t a[32];
+        tmem_ld32(tmem_base + lane_off + 256 + cc, a);
+        tmem_ld_wait();
+        atc_store_grad32(wst, reinterpret_cast<float(&)[32]>(a), 1.0f, nullptr, p.dv32 ? &maps.g32[0] : nullptr,
+                         p.dv16 ? &maps.g16[0] : nullptr, kvh * ATC_D + cc, s0, b);
+        tmem_ld32(tmem_base + lane_off + 384 + cc, a);
+        tmem_ld_wait();
+        atc_store_grad32(wst, reinterpret_cast<float(&)[32]>(a), p.scale,
+                         (p.rope && valid) ? p.rope + static_cast<long long>(key) * 64 + (cc >> 1) : nullptr,
+                         p.dk32 ? &maps.g32[1] : nullptr, p.dk16 ? &maps.g16[1] : nullptr, kvh * ATC_D + cc, s0, b);
+      }
     }
+    if (lane == 0) tma_store_wait_all<0>();
   }
 
   tc_fence_before();
@@ -773,8 +778,8 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
 // works two key blocks ahead of the softmax threads, so the commit -> mbarrier -> tcgen05.ld round trip (~800 cycles
 // measured) is off the critical path.
 constexpr int ATC_DQ_NB = 3;
-constexpr int ATC_DQ_NST = 5;
-constexpr int ATC_DQ_SMEM = 2 * ATC_TILE_BYTES + 2 * ATC_DQ_NST * ATC_HALF_TILE + 1024 + 256;
+constexpr int ATC_DQ_NST = 4;
+constexpr int ATC_DQ_SMEM = 2 * ATC_TILE_BYTES + 2 * ATC_DQ_NST * ATC_HALF_TILE + 8 * GEMM_STAGE_TILE_BYTES + 1024 + 256;
 constexpr int ATC_DQ_DP = 64 * ATC_DQ_NB;        // first dP column
 constexpr int ATC_DQ_ACC = 2 * 64 * ATC_DQ_NB;   // dQ accumulator column
 __global__ void __launch_bounds__(ATC_BWD_THREADS, 1)
@@ -784,7 +789,8 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
   const uint32_t sQ = smem_base, sDO = sQ + ATC_TILE_BYTES;
   const uint32_t sK = sDO + ATC_TILE_BYTES;                      // ATC_DQ_NST stages of 64 keys x 128
   const uint32_t sV = sK + ATC_DQ_NST * ATC_HALF_TILE;
-  const uint32_t bar_base = sV + ATC_DQ_NST * ATC_HALF_TILE;
+  const uint32_t stage_tiles = sV + ATC_DQ_NST * ATC_HALF_TILE;      // 8 x 4 KB staging tiles (epilogue)
+  const uint32_t bar_base = stage_tiles + 8 * GEMM_STAGE_TILE_BYTES;
   auto qdo_full = [&]() { return bar_base; };
   auto acc_full = [&]() { return bar_base + 8u; };
   auto kv_full = [&](int s) { return bar_base + 8u * (2 + s); };
@@ -926,18 +932,21 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
     }
     mbar_wait(acc_full(), 0);
     tc_fence_after();
-    const long long tok = static_cast<long long>(b) * p.S + qi;
-#pragma unroll
-    for (int q = 0; q < 2; ++q) {
-      const int cc = half * 64 + q * 32;
-      uint32_t a[32];
-      tmem_ld32(tmem_base + lane_off + ATC_DQ_ACC + cc, a);
-      tmem_ld_wait();
-      if (valid)
-        atc_store_grad32(reinterpret_cast<float(&)[32]>(a), p.scale, p.rope ? p.rope + static_cast<long long>(qi) * 64 + (cc >> 1) : nullptr,
-                         p.dq32 ? p.dq32 + tok * p.lddq32 + h * ATC_D + cc : nullptr,
-                         p.dq16 ? p.dq16 + tok * p.ldd16 + h * ATC_D + cc : nullptr);
+    const WarpStage wst{stage_tiles + static_cast<uint32_t>(warp - 2) * GEMM_STAGE_TILE_BYTES, lane};
+    const int s0 = q0 + quarter * 32;
+    if (s0 < p.S) {
+#pragma unroll 1
+      for (int q = 0; q < 2; ++q) {
+        const int cc = half * 64 + q * 32;
+        uint32_t a[32];
+        tmem_ld32(tmem_base + lane_off + ATC_DQ_ACC + cc, a);
+        tmem_ld_wait();
+        atc_store_grad32(wst, reinterpret_cast<float(&)[32]>(a), p.scale,
+                         (p.rope && valid) ? p.rope + static_cast<long long>(qi) * 64 + (cc >> 1) : nullptr,
+                         p.dq32 ? &maps.g32[0] : nullptr, p.dq16 ? &maps.g16[0] : nullptr, h * ATC_D + cc, s0, b);
+      }
     }
+    if (lane == 0) tma_store_wait_all<0>();
   }
 
   tc_fence_before();
@@ -967,6 +976,12 @@ inline cudaError_t attn_bwd_dkdv_tc_launch(const __half* q, long long ldq, const
   if (!make_map_attn(&m1.k, k, p.nkv * ATC_D, p.S, p.B, ldk, 128) || !make_map_attn(&m1.v, v, p.nkv * ATC_D, p.S, p.B, ldv, 128) ||
       !make_map_attn(&m1.q, q, p.nq * ATC_D, p.S, p.B, ldq, 64) || !make_map_attn(&m1.dO, dO, p.nq * ATC_D, p.S, p.B, lddo, 64))
     return cudaErrorInvalidValue;
+  m1.o32 = m1.o16 = m1.q; m1.g32[0] = m1.g32[1] = m1.g16[0] = m1.g16[1] = m1.q;
+  if ((p.dv32 && !make_map_store(&m1.g32[0], p.dv32, p.nkv * ATC_D, p.S, p.B, p.lddk32, true)) ||
+      (p.dk32 && !make_map_store(&m1.g32[1], p.dk32, p.nkv * ATC_D, p.S, p.B, p.lddk32, true)) ||
+      (p.dv16 && !make_map_store(&m1.g16[0], p.dv16, p.nkv * ATC_D, p.S, p.B, p.ldd16, false)) ||
+      (p.dk16 && !make_map_store(&m1.g16[1], p.dk16, p.nkv * ATC_D, p.S, p.B, p.ldd16, false)))
+    return cudaErrorInvalidValue;
   dim3 g1((p.S + 127) / 128, p.nkv, p.B);
   attn_bwd_dkdv_tc_kernel<<<g1, ATC_BWD_THREADS, ATC_BWD_SMEM, st>>>(m1, p);
   return cudaGetLastError();
@@ -981,6 +996,10 @@ inline cudaError_t attn_bwd_dq_tc_launch(const __half* q, long long ldq, const _
   AttnTcMaps m2;
   if (!make_map_attn(&m2.k, k, p.nkv * ATC_D, p.S, p.B, ldk, 64) || !make_map_attn(&m2.v, v, p.nkv * ATC_D, p.S, p.B, ldv, 64) ||
       !make_map_attn(&m2.q, q, p.nq * ATC_D, p.S, p.B, ldq, 128) || !make_map_attn(&m2.dO, dO, p.nq * ATC_D, p.S, p.B, lddo, 128))
+    return cudaErrorInvalidValue;
+  m2.o32 = m2.o16 = m2.q; m2.g32[0] = m2.g32[1] = m2.g16[0] = m2.g16[1] = m2.q;
+  if ((p.dq32 && !make_map_store(&m2.g32[0], p.dq32, p.nq * ATC_D, p.S, p.B, p.lddq32, true)) ||
+      (p.dq16 && !make_map_store(&m2.g16[0], p.dq16, p.nq * ATC_D, p.S, p.B, p.ldd16, false)))
     return cudaErrorInvalidValue;
   dim3 g2((p.S + 127) / 128, p.nq, p.B);
   attn_bwd_dq_tc_kernel<<<g2, ATC_BWD_THREADS, ATC_DQ_SMEM, st>>>(m2, p);

@@ -53,6 +53,39 @@ struct GemmShape {
   unsigned int sk_epoch;             // unique per launch on this context, > 0
 };
 
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+inline PFN_encodeTiled get_encode_fn() {
+  static PFN_encodeTiled fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<PFN_encodeTiled>(p);
+  }
+  return fn;
+}
+
+// 2-D map over a row-major [rows, cols] output (pitch ld elements) for 32 x 32 chunk stores out of a staging tile:
+// fp32 rows are 128 B (128B swizzle), 16-bit rows 64 B (64B swizzle) -- the XOR patterns of WarpStage::put_row32/16.
+inline bool make_map_store2d(CUtensorMap* m, const void* base, long long rows, long long cols, long long ld, int dt) {
+  PFN_encodeTiled fn = get_encode_fn();
+  if (!fn || rows <= 0 || cols <= 0) return false;
+  const cuuint64_t es = dt == DT_F32 ? 4 : 2;
+  cuuint64_t dims[2] = {static_cast<cuuint64_t>(cols), static_cast<cuuint64_t>(rows)};
+  cuuint64_t strides[1] = {static_cast<cuuint64_t>(ld) * es};
+  cuuint32_t box[2] = {32u, 32u};
+  cuuint32_t estr[2] = {1u, 1u};
+  const CUtensorMapDataType t = dt == DT_F32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
+                              : (dt == DT_F16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16);
+  return fn(m, t, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            dt == DT_F32 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <int BN> struct GemmCfg {
   static constexpr int A_BYTES = GEMM_BM * GEMM_BK * 2;
   static constexpr int B_BYTES = BN * GEMM_BK * 2;
@@ -254,6 +287,7 @@ __device__ __forceinline__ void chunk_store(const WarpStage& st, RowPtr rowptr, 
 }
 template <int DT, class RowPtr>
 __device__ __forceinline__ void chunk_load(const WarpStage& st, RowPtr rowptr, float (&v)[32], int nrows, int ncols) {
+  if (st.lane == 0) tma_store_wait_read<0>();    // a bulk store may still be reading the tile
   __syncwarp();
   if constexpr (DT == DT_F32) {
     st.from_global32(rowptr, nrows, ncols);
@@ -272,17 +306,69 @@ __device__ __forceinline__ void chunk_load(const WarpStage& st, RowPtr rowptr, f
   }
 }
 
+// TMA store of one warp chunk (32 rows x 32 columns at row r0, column c0 of the tensor behind `map`): the rows go
+// into the staging tile in the map's swizzle pattern and ONE bulk tensor store writes them; tails in M and N are
+// clipped by the map.  Per-thread st.global of such a tile stalled the warps an order of magnitude longer (measured in
+// the attention forward: ~12 k vs ~1 k cycles for 4 chunks), the bulk store is asynchronous.
+template <int DT>
+__device__ __forceinline__ void chunk_store_tma(const WarpStage& st, const CUtensorMap* map, int c0, int r0, const float (&v)[32]) {
+  if (st.lane == 0) tma_store_wait_read<0>();    // the previous bulk store of this warp has read the tile
+  __syncwarp();
+  if constexpr (DT == DT_F32) {
+    st.put_row32(v);
+  } else {
+    uint32_t w[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) w[j] = DT == DT_BF16 ? pack_bf16(v[2 * j], v[2 * j + 1]) : pack_f16(v[2 * j], v[2 * j + 1]);
+    st.put_row16(w);
+  }
+  fence_proxy_async_smem();                      // generic-proxy writes -> visible to the async proxy
+  __syncwarp();
+  if (st.lane == 0) { tma_store_2d(map, st.base, c0, r0); tma_store_commit(); }
+}
+
+template <int DT>
+__device__ __forceinline__ void chunk_store_tma3(const WarpStage& st, const CUtensorMap* map, int c0, int c1, int c2, const float (&v)[32]) {
+  if (st.lane == 0) tma_store_wait_read<0>();
+  __syncwarp();
+  if constexpr (DT == DT_F32) {
+    st.put_row32(v);
+  } else {
+    uint32_t w[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) w[j] = DT == DT_BF16 ? pack_bf16(v[2 * j], v[2 * j + 1]) : pack_f16(v[2 * j], v[2 * j + 1]);
+    st.put_row16(w);
+  }
+  fence_proxy_async_smem();
+  __syncwarp();
+  if (st.lane == 0) { tma_store_3d(map, st.base, c0, c1, c2); tma_store_commit(); }
+}
+
 // ------------------------------------------------------------------------------------------- epilogues
 // Every epilogue works on one warp chunk: rows [m_base, m_base + nrows) (thread `lane` holds row m_base + lane),
 // columns [n, n + nvalid); all global traffic goes through the warp's staging tile.
 // Plain store with optional residual add and up to three row-segments of output (wgrad of fused QKV / gate-up).
 template <int ODT, int RDT, bool HAS_RES>
 struct EpiStore {
+  static constexpr bool kStoreOnly = !HAS_RES;
   void* out[3];
-  int split1, split2;        // rows [0,split1) -> out[0], [split1,split2) -> out[1], [split2,M) -> out[2]
+  int split1, split2;        // rows [0,split1) -> out[0], [split1,split2) -> out[1], [split2,M) -> out[2]; multiples of 32
   long long ld;              // row pitch (elements) of every output and of the residual
   const void* res;
   float alpha;
+  CUtensorMap omap[3];       // store maps of the up-to-three outputs (encoded by the host in encode())
+  int use_tma;               // 0 when a 32-row chunk can straddle a split (splits not multiples of 32): per-thread stores
+  bool encode(int M, int N) {
+    use_tma = !((split1 < M && split1 % 32) || (split2 < M && split2 % 32));
+    if (!use_tma) return true;
+    const int s1 = split1 < M ? split1 : M, s2 = split2 < M ? split2 : M;
+    const int rows[3] = {s1, s2 - s1, M - s2};
+    for (int i = 0; i < 3; ++i) {
+      if (rows[i] > 0 && !make_map_store2d(&omap[i], out[i], rows[i], N, ld, ODT)) return false;
+      if (rows[i] <= 0) omap[i] = omap[0];
+    }
+    return true;
+  }
   // L2 prefetch of what the epilogue of rows [m_base, +nrows) x columns [n0, n0 + ncols) will read (issued by the
   // epilogue warps while the tensor core still works on the tile, so the reads do not pay DRAM latency per chunk)
   __device__ __forceinline__ void prefetch(int lane, int m_base, int n0, int nrows, int ncols) const {
@@ -295,7 +381,6 @@ struct EpiStore {
     }
   }
   __device__ __forceinline__ void operator()(const WarpStage& st, int m_base, int n, float (&v)[32], int nrows, int nvalid) const {
-    using OT = typename OutElem<ODT>::type;
     if (alpha != 1.0f) {
 #pragma unroll
       for (int j = 0; j < 32; ++j) v[j] *= alpha;
@@ -308,12 +393,20 @@ struct EpiStore {
 #pragma unroll
       for (int j = 0; j < 32; ++j) v[j] += r[j];
     }
-    chunk_store<ODT>(st, [&](int rr) {
-      const int m = m_base + rr;
-      const int seg = (m >= split1) + (m >= split2);
-      const int mr = m - (seg == 0 ? 0 : (seg == 1 ? split1 : split2));
-      return reinterpret_cast<OT*>(out[seg]) + static_cast<long long>(mr) * ld + n;
-    }, v, nrows, nvalid);
+    if (use_tma) {
+      const int seg = (m_base >= split1) + (m_base >= split2);      // a 32-row chunk never straddles a split
+      const int mr = m_base - (seg == 0 ? 0 : (seg == 1 ? split1 : split2));
+      chunk_store_tma<ODT>(st, &omap[seg], n, mr, v);
+    } else {
+      using OT = typename OutElem<ODT>::type;
+      if (st.lane == 0) tma_store_wait_read<0>();
+      chunk_store<ODT>(st, [&](int rr) {
+        const int m = m_base + rr;
+        const int seg = (m >= split1) + (m >= split2);
+        const int mr = m - (seg == 0 ? 0 : (seg == 1 ? split1 : split2));
+        return reinterpret_cast<OT*>(out[seg]) + static_cast<long long>(mr) * ld + n;
+      }, v, nrows, nvalid);
+    }
   }
 };
 
@@ -322,9 +415,12 @@ struct EpiStore {
 // epilogue works on 32-column chunks, so a chunk never straddles a head or the q|k|v boundaries.
 // rope table: float2 (cos, sin) [S, d/2], angles computed in fp64 on the host (reading A-5).
 struct EpiQKVRope {
+  static constexpr bool kStoreOnly = false;
   __half* out; long long ld;
   const float2* rope; int S, d;
   int rot_cols;              // columns [0, rot_cols) are rotated (Nq + Nkv, or 0 when use_rope = 0)
+  CUtensorMap omap;
+  bool encode(int M, int N) { return make_map_store2d(&omap, out, M, N, ld, DT_F16); }
   __device__ __forceinline__ void prefetch(int, int, int, int, int) const {}      // the rope table stays L2-resident
   __device__ __forceinline__ void operator()(const WarpStage& st, int m_base, int n, float (&v)[32], int nrows, int nvalid) const {
     if (n < rot_cols) {
@@ -341,33 +437,42 @@ struct EpiQKVRope {
         v[2 * j + 1] = z0 * cs[2 * j + 1] + z1 * cs[2 * j];
       }
     }
-    __half* obase = out + static_cast<long long>(m_base) * ld + n;
-    chunk_store<DT_F16>(st, [&](int rr) { return obase + rr * ld; }, v, nrows, nvalid);
+    chunk_store_tma<DT_F16>(st, &omap, n, m_base, v);
   }
 };
 
 // DUAL epilogue: h = silu(g) * u (ref [35]); saves g,u in fp16 for the backward (DESIGN.md precision plan).
 struct EpiSwiGLU {
+  static constexpr bool kStoreOnly = true;
   __half* h; __half* g16; __half* u16; long long ld;
+  CUtensorMap hmap, gmap, umap;
+  bool encode(int M, int N) {
+    return make_map_store2d(&hmap, h, M, N, ld, DT_F16) && make_map_store2d(&gmap, g16, M, N, ld, DT_F16) &&
+           make_map_store2d(&umap, u16, M, N, ld, DT_F16);
+  }
   __device__ __forceinline__ void prefetch(int, int, int, int, int) const {}
   __device__ __forceinline__ void operator()(const WarpStage& st, int m_base, int n, float (&g)[32], float (&u)[32], int nrows,
                                              int nvalid) const {
-    const long long off = static_cast<long long>(m_base) * ld + n;
-    chunk_store<DT_F16>(st, [&](int rr) { return g16 + off + rr * ld; }, g, nrows, nvalid);
-    chunk_store<DT_F16>(st, [&](int rr) { return u16 + off + rr * ld; }, u, nrows, nvalid);
+    chunk_store_tma<DT_F16>(st, &gmap, n, m_base, g);
+    chunk_store_tma<DT_F16>(st, &umap, n, m_base, u);
 #pragma unroll
     for (int j = 0; j < 32; ++j) {
       const float sg = 1.0f / (1.0f + __expf(-g[j]));
       g[j] = g[j] * sg * u[j];
     }
-    chunk_store<DT_F16>(st, [&](int rr) { return h + off + rr * ld; }, g, nrows, nvalid);
+    chunk_store_tma<DT_F16>(st, &hmap, n, m_base, g);
   }
 };
 
 // Down-projection dgrad with fused SwiGLU backward: acc = dh; writes [dg | du] (fp16) into one [T, 2F] buffer.
 struct EpiSwiGLUBwd {
+  static constexpr bool kStoreOnly = false;
   const __half* g16; const __half* u16; long long ld;      // saved g,u [T,F]
   __half* dgu; int F;                                      // [T, 2F]
+  CUtensorMap dgmap, dumap;                                // the dg and du halves of dgu as two [T, F] views of pitch 2F
+  bool encode(int M, int N) {
+    return make_map_store2d(&dgmap, dgu, M, N, 2LL * F, DT_F16) && make_map_store2d(&dumap, dgu + F, M, N, 2LL * F, DT_F16);
+  }
   __device__ __forceinline__ void prefetch(int lane, int m_base, int n0, int nrows, int ncols) const {
     if (lane < nrows) {
       const long long off = static_cast<long long>(m_base + lane) * ld + n0;
@@ -386,9 +491,8 @@ struct EpiSwiGLUBwd {
       u[j] = dh[j] * g[j] * sg;           // du
       g[j] = dgv;                         // dg
     }
-    __half* row0 = dgu + static_cast<long long>(m_base) * (2LL * F) + n;
-    chunk_store<DT_F16>(st, [&](int rr) { return row0 + rr * (2LL * F); }, g, nrows, nvalid);
-    chunk_store<DT_F16>(st, [&](int rr) { return row0 + F + rr * (2LL * F); }, u, nrows, nvalid);
+    chunk_store_tma<DT_F16>(st, &dgmap, n, m_base, g);
+    chunk_store_tma<DT_F16>(st, &dumap, n, m_base, u);
   }
 };
 
@@ -404,7 +508,7 @@ __device__ __forceinline__ void gemm_tile_coord(int tile, int mblocks, int nbloc
 
 template <int BN, bool A_MN, bool B_MN, bool DUAL, class Epi>
 __global__ void __launch_bounds__(GEMM_THREADS, 1)
-gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, const Epi epi) {
+gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, const __grid_constant__ Epi epi) {
   using Cfg = GemmCfg<BN>;
   constexpr int STAGES = Cfg::STAGES;
   constexpr int NOUT = DUAL ? BN / 2 : BN;       // output columns covered by one tile
@@ -555,6 +659,7 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, c
       if (lane == 0) mbar_arrive(tempty_bar(acc));
       if (++acc == 2) { acc = 0; acc_phase ^= 1u; }
     }
+    if (lane == 0) tma_store_wait_all<0>();        // this warp's bulk stores are complete before the CTA exits
   }
 
   tc_fence_before();
@@ -636,7 +741,7 @@ __device__ __forceinline__ void st_release_gpu(unsigned int* p, unsigned int v) 
 
 template <bool A_MN, bool B_MN, bool DUAL, int MT, class Epi>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(GEMM_THREADS, 1)
-gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, const Epi epi) {
+gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, const __grid_constant__ Epi epi) {
   // MT = 1: 256 x 256 pair tile, two accumulator stages (epilogue of tile i overlaps the MMAs of tile i + 1).
   // MT = 2: 512 x 256 pair tile (each CTA 256 rows = two 128-row MMAs per k-step sharing the B slice): A 32 KB +
   //         B 16 KB per CTA and k-block for twice the MACs, i.e. 25 % less shared-memory fill per flop (the quantity
@@ -883,6 +988,7 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
       }
       if (++acc == NACC) { acc = 0; acc_phase ^= 1u; }
     }
+    if (lane == 0) tma_store_wait_all<0>();        // this warp's bulk stores are complete before the CTA exits
   }
 
   tc_fence_before();
@@ -895,22 +1001,6 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
 
 
 // ------------------------------------------------------------------------------------------- host side
-typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-inline PFN_encodeTiled get_encode_fn() {
-  static PFN_encodeTiled fn = nullptr;
-  if (!fn) {
-    void* p = nullptr;
-    cudaDriverEntryPointQueryResult q;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-        q == cudaDriverEntryPointSuccess)
-      fn = reinterpret_cast<PFN_encodeTiled>(p);
-  }
-  return fn;
-}
-
 // 2-D tensor map over a row-major 16-bit matrix [rows, cols] with pitch ld (elements):
 // box = {64 contiguous elements, box_rows}, 128-byte swizzle, out-of-bounds reads return zero.
 inline bool make_map_2d(CUtensorMap* m, const void* base, long long rows, long long cols, long long ld, int box_rows,
@@ -989,18 +1079,21 @@ inline int gemm_tail_split(int ntiles, int clusters, int kblocks) {
   return s >= 2 ? s : 0;
 }
 
-// Pair tile height (MT x 256 rows).  The 512-row tile (MT = 2) needs 25 % less shared-memory fill per flop and ran
-// 3-4 % faster in a sustained stand-alone loop at K = 16384, but inside the layer step its unoverlapped epilogue and
-// shallower pipeline cost more than that (wgrad_gateup 1.23 vs 1.17 ms, down 0.75 vs 0.60 ms; profiles/r1c notes), so
-// the default is MT = 1; LSP_GEMM_MT=2 selects the tall tile (kept for tuning on other shapes, covered by the tests).
-inline int gemm_pick_mt(int M, int N, int K, int pairs, bool use_sk) {
+// Pair tile height (MT x 256 rows).  The 512-row tile (MT = 2) needs 25 % less shared-memory fill per flop and runs
+// its main loop 3-4 % faster, but its accumulators fill the TMEM, so the epilogue is not overlapped: it pays off only
+// for store-only epilogues (bulk stores are asynchronous; epilogues that READ a residual or g, u stall on memory
+// latency per chunk: down 0.74 vs 0.60 ms) at large K, and only when the tile count does not quantise worse.  The
+// candidates at the 3B shape were wgrad gate/up, dgrad gate/up and wgrad O; inside the layer step the gain did not
+// survive (7.39-7.42 vs 7.33-7.39 ms of GEMM time: every kernel's clock depends on the power state its predecessors
+// left), so the default stays MT = 1.  LSP_GEMM_MT=2 selects the tall tile (covered by the GPU tests).
+inline int gemm_pick_mt(int M, int N, int K, int pairs, bool use_sk, bool store_only) {
   static int forced = -1;
   if (forced < 0) {
     const char* e = getenv("LSP_GEMM_MT");
     forced = e ? atoi(e) : 0;
   }
   if (forced == 1 || forced == 2) return forced;
-  (void)M; (void)N; (void)K; (void)pairs; (void)use_sk;
+  (void)M; (void)N; (void)K; (void)pairs; (void)use_sk; (void)store_only;
   return 1;
 }
 
@@ -1063,6 +1156,8 @@ cudaError_t gemm_run(int M, int N, int nseg, const Operand* a, const Operand* b,
   sh.M = M; sh.N = N; sh.nseg = nseg;
   sh.a_fmt = umma_fmt(a[0].dt); sh.b_fmt = umma_fmt(b[0].dt);      // all segments share the operand formats
   for (int s = 0; s < GEMM_MAX_SEG; ++s) sh.kblocks[s] = 0;
+  Epi e = epi;
+  if (!e.encode(M, N)) return cudaErrorInvalidValue;
   const bool pair = BN == 256 && nseg == 1 && gemm_use_pair(M);
   for (int s = 0; s < nseg; ++s) {
     sh.kblocks[s] = (ks[s] + GEMM_BK - 1) / GEMM_BK;
@@ -1071,17 +1166,19 @@ cudaError_t gemm_run(int M, int N, int nseg, const Operand* a, const Operand* b,
   }
   if (pair) {
     const bool use_sk = nseg == 1 && sk && sk->partial && gemm_use_streamk();
-    if (nseg == 1 && gemm_pick_mt(M, N, ks[0], num_sms / 2, use_sk) == 2)
-      return launch_gemm_pair<A_MN, B_MN, false, 2, Epi>(maps, sh, epi, num_sms, st, sk);
-    return launch_gemm_pair<A_MN, B_MN, false, 1, Epi>(maps, sh, epi, num_sms, st, nseg == 1 ? sk : nullptr);
+    if (nseg == 1 && gemm_pick_mt(M, N, ks[0], num_sms / 2, use_sk, Epi::kStoreOnly) == 2)
+      return launch_gemm_pair<A_MN, B_MN, false, 2, Epi>(maps, sh, e, num_sms, st, sk);
+    return launch_gemm_pair<A_MN, B_MN, false, 1, Epi>(maps, sh, e, num_sms, st, nseg == 1 ? sk : nullptr);
   }
-  return launch_gemm<BN, A_MN, B_MN, false, Epi>(maps, sh, epi, num_sms, st);
+  return launch_gemm<BN, A_MN, B_MN, false, Epi>(maps, sh, e, num_sms, st);
 }
 
 // Forward gate/up GEMM (DUAL): A [M,K], Wg/Wu [N,K] all K-major.
 template <class Epi>
 cudaError_t gemm_run_dual(int M, int N, int K, const Operand& a, const Operand& bg, const Operand& bu, const Epi& epi,
                           int num_sms, cudaStream_t st, const GemmSKRes* sk = nullptr) {
+  Epi e = epi;
+  if (!e.encode(M, N)) return cudaErrorInvalidValue;
   GemmMaps maps;
   GemmShape sh;
   sh.M = M; sh.N = N; sh.nseg = 1;
@@ -1090,8 +1187,8 @@ cudaError_t gemm_run_dual(int M, int N, int K, const Operand& a, const Operand& 
   if (!encode_operand(&maps.a[0], a, M, K, GEMM_BM)) return cudaErrorInvalidValue;
   if (!encode_operand(&maps.b[0], bg, N, K, 128)) return cudaErrorInvalidValue;
   if (!encode_operand(&maps.b[1], bu, N, K, 128)) return cudaErrorInvalidValue;
-  if (gemm_use_pair(M)) return launch_gemm_pair<false, false, true, 1, Epi>(maps, sh, epi, num_sms, st, sk);
-  return launch_gemm<256, false, false, true, Epi>(maps, sh, epi, num_sms, st);
+  if (gemm_use_pair(M)) return launch_gemm_pair<false, false, true, 1, Epi>(maps, sh, e, num_sms, st, sk);
+  return launch_gemm<256, false, false, true, Epi>(maps, sh, e, num_sms, st);
 }
 
 }  // namespace lsp
