@@ -488,6 +488,7 @@ struct AttnTcBwdParams {
   const float2* rope;          // (cos, sin) [S, 64] or null: inverse rotation of dq, dk on store
   float* dq32; float* dk32; float* dv32; long long lddq32, lddk32;
   __half* dq16; __half* dk16; __half* dv16; long long ldd16;
+  unsigned int* sched;         // work-item counters of the persistent kernels ([4], [5]: dQ kernel), zero between launches
 };
 
 __device__ __forceinline__ void atc_load_half_tile(uint32_t dst, const CUtensorMap* m, uint32_t bar, int col0, int s0, int b) {
@@ -782,6 +783,22 @@ constexpr int ATC_DQ_NST = 4;
 constexpr int ATC_DQ_SMEM = 2 * ATC_TILE_BYTES + 2 * ATC_DQ_NST * ATC_HALF_TILE + 8 * GEMM_STAGE_TILE_BYTES + 1024 + 256;
 constexpr int ATC_DQ_DP = 64 * ATC_DQ_NB;        // first dP column
 constexpr int ATC_DQ_ACC = 2 * 64 * ATC_DQ_NB;   // dQ accumulator column
+// Persistent like the forward: work items (128-query block, head, batch) come heaviest-first from an atomic counter
+// (p.sched + 4); Q / dO of the next item are fetched as soon as the item's last S / dP MMA has been issued (qdo_empty),
+// the dQ epilogue (TMEM -> staging tile -> bulk stores) overlaps the first S / dP MMAs of the next item, and acc_free
+// tells the MMA warp when the dQ accumulator may be overwritten.
+struct AttnDqItem { int q0, h, b, kvh, iters; };
+__device__ __forceinline__ AttnDqItem attn_dq_item(uint32_t i, const AttnTcBwdParams& p, int nqb) {
+  const int per_lvl = p.nq * p.B;
+  const int lvl = static_cast<int>(i) / per_lvl, r = static_cast<int>(i) - lvl * per_lvl;
+  AttnDqItem it;
+  it.q0 = (nqb - 1 - lvl) * 128;                                 // heavy (late) query blocks first
+  it.b = r / p.nq; it.h = r - it.b * p.nq;
+  it.kvh = it.h / (p.nq / p.nkv);
+  it.iters = (min(p.S, it.q0 + 128) + 63) / 64;                  // 64-key blocks [0, kv_end)
+  return it;
+}
+
 __global__ void __launch_bounds__(ATC_BWD_THREADS, 1)
 attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdParams p) {
   extern __shared__ uint8_t smem_raw[];
@@ -793,26 +810,30 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
   const uint32_t bar_base = stage_tiles + 8 * GEMM_STAGE_TILE_BYTES;
   auto qdo_full = [&]() { return bar_base; };
   auto acc_full = [&]() { return bar_base + 8u; };
-  auto kv_full = [&](int s) { return bar_base + 8u * (2 + s); };
-  auto kv_empty = [&](int s) { return bar_base + 8u * (2 + ATC_DQ_NST + s); };
-  auto sdp_full = [&](int s) { return bar_base + 8u * (2 + 2 * ATC_DQ_NST + s); };
-  auto ds_full = [&](int s) { return bar_base + 8u * (2 + ATC_DQ_NB + 2 * ATC_DQ_NST + s); };
-  const uint32_t tmem_slot = bar_base + 8u * (2 + 2 * ATC_DQ_NB + 2 * ATC_DQ_NST);
+  auto qdo_empty = [&]() { return bar_base + 16u; };
+  auto acc_free = [&]() { return bar_base + 24u; };
+  auto kv_full = [&](int s) { return bar_base + 8u * (4 + s); };
+  auto kv_empty = [&](int s) { return bar_base + 8u * (4 + ATC_DQ_NST + s); };
+  auto sdp_full = [&](int s) { return bar_base + 8u * (4 + 2 * ATC_DQ_NST + s); };
+  auto ds_full = [&](int s) { return bar_base + 8u * (4 + ATC_DQ_NB + 2 * ATC_DQ_NST + s); };
+  auto item_bar = [&](int s) { return bar_base + 8u * (4 + 2 * ATC_DQ_NB + 2 * ATC_DQ_NST + s); };
+  const uint32_t item_slots = bar_base + 8u * (4 + 2 * ATC_DQ_NB + 2 * ATC_DQ_NST + ATC_ITEM_RING);
+  const uint32_t tmem_slot = item_slots + 4u * ATC_ITEM_RING;
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+  volatile uint32_t* item_slot_ptr = reinterpret_cast<volatile uint32_t*>(smem_raw + (item_slots - smem_u32(smem_raw)));
 
   const int warp = warp_idx_uniform(), lane = threadIdx.x & 31;
-  const int qb = gridDim.x - 1 - blockIdx.x;                     // heavy (late) query blocks first
-  const int h = blockIdx.y, b = blockIdx.z;
-  const int kvh = h / (p.nq / p.nkv);
-  const int q0 = qb * 128;
-  const int kv_end = min(p.S, q0 + 128);
-  const int iters = (kv_end + 63) / 64;                          // 64-key blocks [0, kv_end)
+  const int nqb = (p.S + 127) / 128;
+  const uint32_t nitems = static_cast<uint32_t>(nqb * p.nq * p.B);
+  unsigned int* const sched = p.sched + 4;
 
   if (threadIdx.x == 0) {
     tma_prefetch_desc(&maps.q); tma_prefetch_desc(&maps.k); tma_prefetch_desc(&maps.v); tma_prefetch_desc(&maps.dO);
-    mbar_init(qdo_full(), 1); mbar_init(acc_full(), 1);
+    tma_prefetch_desc(&maps.g32[0]); tma_prefetch_desc(&maps.g16[0]);
+    mbar_init(qdo_full(), 1); mbar_init(acc_full(), 1); mbar_init(qdo_empty(), 1); mbar_init(acc_free(), 8);
     for (int i = 0; i < ATC_DQ_NST; ++i) { mbar_init(kv_full(i), 1); mbar_init(kv_empty(i), 1); }
     for (int i = 0; i < ATC_DQ_NB; ++i) { mbar_init(sdp_full(i), 1); mbar_init(ds_full(i), 8); }
+    for (int i = 0; i < ATC_ITEM_RING; ++i) mbar_init(item_bar(i), 1);
     fence_barrier_init();
   }
   if (warp == 1) { tmem_alloc(tmem_slot, 512); tmem_relinquish(); }
@@ -821,33 +842,56 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
 
+  auto get_item = [&](uint32_t it) -> uint32_t {
+    mbar_wait(item_bar(it % ATC_ITEM_RING), (it / ATC_ITEM_RING) & 1u);
+    return item_slot_ptr[it % ATC_ITEM_RING];
+  };
+
   if (warp == 0) {
+    // ===================================================================== scheduler + TMA producer
     if (lane == 0) {
-      mbar_expect_tx(qdo_full(), 2 * ATC_TILE_BYTES);
-      tma_load_3d(sQ, &maps.q, qdo_full(), h * ATC_D, q0, b);
-      tma_load_3d(sQ + ATC_CHUNK_BYTES, &maps.q, qdo_full(), h * ATC_D + 64, q0, b);
-      tma_load_3d(sDO, &maps.dO, qdo_full(), h * ATC_D, q0, b);
-      tma_load_3d(sDO + ATC_CHUNK_BYTES, &maps.dO, qdo_full(), h * ATC_D + 64, q0, b);
-      for (int it = 0; it < iters; ++it) {
-        const int st = it % ATC_DQ_NST;
-        mbar_wait(kv_empty(st), ((it / ATC_DQ_NST) & 1) ^ 1u);
-        mbar_expect_tx(kv_full(st), 2 * ATC_HALF_TILE);
-        tma_load_3d(sK + st * ATC_HALF_TILE, &maps.k, kv_full(st), kvh * ATC_D, it * 64, b);
-        tma_load_3d(sK + st * ATC_HALF_TILE + 64 * 128, &maps.k, kv_full(st), kvh * ATC_D + 64, it * 64, b);
-        tma_load_3d(sV + st * ATC_HALF_TILE, &maps.v, kv_full(st), kvh * ATC_D, it * 64, b);
-        tma_load_3d(sV + st * ATC_HALF_TILE + 64 * 128, &maps.v, kv_full(st), kvh * ATC_D + 64, it * 64, b);
+      auto publish = [&](uint32_t it, uint32_t item) {
+        item_slot_ptr[it % ATC_ITEM_RING] = item;
+        mbar_arrive(item_bar(it % ATC_ITEM_RING));
+      };
+      uint32_t g = 0;                                            // K/V blocks loaded so far (ring position)
+      uint32_t item = atomicAdd(sched, 1u);
+      publish(0, item);
+      for (uint32_t it = 0; item < nitems; ++it) {
+        const AttnDqItem w = attn_dq_item(item, p, nqb);
+        mbar_wait(qdo_empty(), (it & 1u) ^ 1u);                  // the previous item's S / dP MMAs have read Q, dO
+        mbar_expect_tx(qdo_full(), 2 * ATC_TILE_BYTES);
+        tma_load_3d(sQ, &maps.q, qdo_full(), w.h * ATC_D, w.q0, w.b);
+        tma_load_3d(sQ + ATC_CHUNK_BYTES, &maps.q, qdo_full(), w.h * ATC_D + 64, w.q0, w.b);
+        tma_load_3d(sDO, &maps.dO, qdo_full(), w.h * ATC_D, w.q0, w.b);
+        tma_load_3d(sDO + ATC_CHUNK_BYTES, &maps.dO, qdo_full(), w.h * ATC_D + 64, w.q0, w.b);
+        const uint32_t next = atomicAdd(sched, 1u);              // latency hidden behind this item's K/V stream
+        for (int j = 0; j < w.iters; ++j, ++g) {
+          const int st = g % ATC_DQ_NST;
+          mbar_wait(kv_empty(st), ((g / ATC_DQ_NST) & 1u) ^ 1u);
+          mbar_expect_tx(kv_full(st), 2 * ATC_HALF_TILE);
+          tma_load_3d(sK + st * ATC_HALF_TILE, &maps.k, kv_full(st), w.kvh * ATC_D, j * 64, w.b);
+          tma_load_3d(sK + st * ATC_HALF_TILE + 64 * 128, &maps.k, kv_full(st), w.kvh * ATC_D + 64, j * 64, w.b);
+          tma_load_3d(sV + st * ATC_HALF_TILE, &maps.v, kv_full(st), w.kvh * ATC_D, j * 64, w.b);
+          tma_load_3d(sV + st * ATC_HALF_TILE + 64 * 128, &maps.v, kv_full(st), w.kvh * ATC_D + 64, j * 64, w.b);
+        }
+        publish(it + 1, next);
+        item = next;
       }
+      __threadfence();
+      if (atomicAdd(sched + 1, 1u) == gridDim.x - 1) { sched[0] = 0; sched[1] = 0; __threadfence(); }
     }
   } else if (warp == 1) {
+    // ===================================================================== MMA issuer (whole warp, elected lane issues)
     const uint32_t leader = elect_one();
     const uint32_t idesc_sdp = umma_idesc(128, 64, 0, 0, 0, 0);     // [128 queries x 64 keys]
     const uint32_t idesc_acc = umma_idesc(128, 128, 0, 0, 0, 1);    // dQ [128 x 128] += dS(TMEM) K(MN-major)
     const uint64_t dQd = umma_smem_desc(sQ, 16, 1024), dDO = umma_smem_desc(sDO, 16, 1024);
     const uint64_t dKk = umma_smem_desc(sK, 16, 1024), dVk = umma_smem_desc(sV, 16, 1024);
     const uint64_t dKm = umma_smem_desc(sK, 64 * 128, 1024);
-    auto issue_sdp = [&](int it) {
-      const int st = it % ATC_DQ_NST, buf = it % ATC_DQ_NB;
-      mbar_wait(kv_full(st), (it / ATC_DQ_NST) & 1);
+    auto issue_sdp = [&](uint32_t g) {                               // g: global block index (ring positions)
+      const int st = g % ATC_DQ_NST, buf = g % ATC_DQ_NB;
+      mbar_wait(kv_full(st), (g / ATC_DQ_NST) & 1u);
       tc_fence_after();
       if (leader) {
         const uint64_t ka = desc_adv(dKk, st * ATC_HALF_TILE), va = desc_adv(dVk, st * ATC_HALF_TILE);
@@ -861,89 +905,113 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
         umma_commit(sdp_full(buf));
       }
     };
-    mbar_wait(qdo_full(), 0);
-    issue_sdp(0);
-    if (iters > 1) issue_sdp(1);
-    for (int it = 0; it < iters; ++it) {
-      const int st = it % ATC_DQ_NST, buf = it % ATC_DQ_NB;
-      if (it + 2 < iters) issue_sdp(it + 2);           // its buffers were released by dQ(it - 1), already issued
-      mbar_wait(ds_full(buf), (it / ATC_DQ_NB) & 1);
-      tc_fence_after();
-      if (leader) {
-        const uint64_t ka = desc_adv(dKm, st * ATC_HALF_TILE);
-#pragma unroll
-        for (int kk = 0; kk < 4; ++kk)
-          umma_f16_ts(tmem_base + ATC_DQ_ACC, tmem_base + buf * 64 + atc_half_operand_col(kk), desc_adv(ka, kk * 2048), idesc_acc,
-                      (it | kk) != 0 ? 1u : 0u);
-        if (q0 < ATC_SPLIT_ROWS) {                                    // early query rows: + dS_lo K
+    uint32_t g0 = 0;                                                 // global index of this item's block 0
+    for (uint32_t it = 0;; ++it) {
+      const uint32_t item = get_item(it);
+      if (item >= nitems) break;
+      const AttnDqItem w = attn_dq_item(item, p, nqb);
+      const int iters = w.iters;
+      mbar_wait(qdo_full(), it & 1u);
+      issue_sdp(g0);
+      if (iters > 1) issue_sdp(g0 + 1);
+      if (iters <= 2 && leader) umma_commit(qdo_empty());            // those were the item's last S / dP MMAs
+      for (int j = 0; j < iters; ++j) {
+        const uint32_t g = g0 + j;
+        const int st = g % ATC_DQ_NST, buf = g % ATC_DQ_NB;
+        if (j + 2 < iters) {
+          issue_sdp(g + 2);                                          // its buffers were released by dQ(j - 1), already issued
+          if (j + 3 == iters && leader) umma_commit(qdo_empty());
+        }
+        mbar_wait(ds_full(buf), (g / ATC_DQ_NB) & 1u);
+        if (j == 0 && it > 0) mbar_wait(acc_free(), (it - 1u) & 1u); // the previous item's dQ has been read out
+        tc_fence_after();
+        if (leader) {
+          const uint64_t ka = desc_adv(dKm, st * ATC_HALF_TILE);
 #pragma unroll
           for (int kk = 0; kk < 4; ++kk)
-            umma_f16_ts(tmem_base + ATC_DQ_ACC, tmem_base + buf * 64 + 16 + atc_half_operand_col(kk), desc_adv(ka, kk * 2048),
-                        idesc_acc, 1u);
+            umma_f16_ts(tmem_base + ATC_DQ_ACC, tmem_base + buf * 64 + atc_half_operand_col(kk), desc_adv(ka, kk * 2048), idesc_acc,
+                        (j | kk) != 0 ? 1u : 0u);
+          if (w.q0 < ATC_SPLIT_ROWS) {                                // early query rows: + dS_lo K
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk)
+              umma_f16_ts(tmem_base + ATC_DQ_ACC, tmem_base + buf * 64 + 16 + atc_half_operand_col(kk), desc_adv(ka, kk * 2048),
+                          idesc_acc, 1u);
+          }
+          umma_commit(kv_empty(st));
         }
-        umma_commit(kv_empty(st));
       }
+      if (leader) umma_commit(acc_full());
+      g0 += iters;
     }
-    if (leader) umma_commit(acc_full());
   } else {
+    // ===================================================================== softmax warps: TMEM lane quarter x column half
     const int quarter = warp & 3, half = (warp - 2) >> 2;
     const int row = quarter * 32 + lane;
     const uint32_t lane_off = static_cast<uint32_t>(quarter * 32) << 16;
     const int col0 = half * 32;
     const float c = p.scale_log2;
-    const int qi = q0 + row;
-    const bool valid = qi < p.S;
-    const long long vidx = (static_cast<long long>(b) * p.nq + h) * p.S + qi;
-    const float L2 = valid ? p.lse[vidx] * 1.4426950408889634f : INFINITY;
-    const float Dr = valid ? p.dvec[vidx] : 0.f;
-    for (int it = 0; it < iters; ++it) {
-      const int buf = it % ATC_DQ_NB;
-      mbar_wait(sdp_full(buf), (it / ATC_DQ_NB) & 1);
-      tc_fence_after();
-      uint32_t sr[32], dr[32];
-      tmem_ld32(tmem_base + lane_off + buf * 64 + col0, sr);
-      tmem_ld32(tmem_base + lane_off + ATC_DQ_DP + buf * 64 + col0, dr);
-      tmem_ld_wait();
-      float ds[32];
-#pragma unroll
-      for (int i = 0; i < 32; ++i)
-        ds[i] = ex2_approx(fmaf(__uint_as_float(sr[i]), c, -L2)) * (__uint_as_float(dr[i]) - Dr);
-      if (it * 64 + 63 > q0) {                                        // diagonal blocks: key > query is masked
-        const int krel = it * 64 + col0 - q0;
+    const WarpStage wst{stage_tiles + static_cast<uint32_t>(warp - 2) * GEMM_STAGE_TILE_BYTES, lane};
+    uint32_t g = 0;                                                  // global block index
+    for (uint32_t it = 0;; ++it) {
+      const uint32_t item = get_item(it);
+      if (item >= nitems) break;
+      const AttnDqItem w = attn_dq_item(item, p, nqb);
+      const int q0 = w.q0, qi = q0 + row;
+      const bool valid = qi < p.S;
+      const long long vidx = (static_cast<long long>(w.b) * p.nq + w.h) * p.S + qi;
+      const float L2 = valid ? p.lse[vidx] * 1.4426950408889634f : INFINITY;
+      const float Dr = valid ? p.dvec[vidx] : 0.f;
+      for (int j = 0; j < w.iters; ++j, ++g) {
+        const int buf = g % ATC_DQ_NB;
+        mbar_wait(sdp_full(buf), (g / ATC_DQ_NB) & 1u);
+        tc_fence_after();
+        uint32_t sr[32], dr[32];
+        tmem_ld32(tmem_base + lane_off + buf * 64 + col0, sr);
+        tmem_ld32(tmem_base + lane_off + ATC_DQ_DP + buf * 64 + col0, dr);
+        tmem_ld_wait();
+        float ds[32];
 #pragma unroll
         for (int i = 0; i < 32; ++i)
-          if (krel + i > row) ds[i] = 0.f;
-      }
-      uint32_t pk[16];
-      if (q0 < ATC_SPLIT_ROWS) {
-        uint32_t pl[16];
+          ds[i] = ex2_approx(fmaf(__uint_as_float(sr[i]), c, -L2)) * (__uint_as_float(dr[i]) - Dr);
+        if (j * 64 + 63 > q0) {                                      // diagonal blocks: key > query is masked
+          const int krel = j * 64 + col0 - q0;
 #pragma unroll
-        for (int i = 0; i < 16; ++i) atc_split_pack(ds[2 * i], ds[2 * i + 1], pk[i], pl[i]);
-        tmem_st16(tmem_base + lane_off + buf * 64 + col0 + 16, pl);
-      } else {
+          for (int i = 0; i < 32; ++i)
+            if (krel + i > row) ds[i] = 0.f;
+        }
+        uint32_t pk[16];
+        if (q0 < ATC_SPLIT_ROWS) {
+          uint32_t pl[16];
 #pragma unroll
-        for (int i = 0; i < 16; ++i) pk[i] = pack_f16(ds[2 * i], ds[2 * i + 1]);
+          for (int i = 0; i < 16; ++i) atc_split_pack(ds[2 * i], ds[2 * i + 1], pk[i], pl[i]);
+          tmem_st16(tmem_base + lane_off + buf * 64 + col0 + 16, pl);
+        } else {
+#pragma unroll
+          for (int i = 0; i < 16; ++i) pk[i] = pack_f16(ds[2 * i], ds[2 * i + 1]);
+        }
+        tmem_st16(tmem_base + lane_off + buf * 64 + col0, pk);
+        tmem_st_wait();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(ds_full(buf));
       }
-      tmem_st16(tmem_base + lane_off + buf * 64 + col0, pk);
-      tmem_st_wait();
+      // epilogue: this warp stores rows [32 quarter, +32), columns [64 half, +64) of dQ, then releases the accumulator
+      mbar_wait(acc_full(), it & 1u);
+      tc_fence_after();
+      const int s0 = q0 + quarter * 32;
+      uint32_t a0[32], a1[32];
+      tmem_ld32(tmem_base + lane_off + ATC_DQ_ACC + half * 64, a0);
+      tmem_ld32(tmem_base + lane_off + ATC_DQ_ACC + half * 64 + 32, a1);
+      tmem_ld_wait();
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(ds_full(buf));
-    }
-    mbar_wait(acc_full(), 0);
-    tc_fence_after();
-    const WarpStage wst{stage_tiles + static_cast<uint32_t>(warp - 2) * GEMM_STAGE_TILE_BYTES, lane};
-    const int s0 = q0 + quarter * 32;
-    if (s0 < p.S) {
-#pragma unroll 1
-      for (int q = 0; q < 2; ++q) {
-        const int cc = half * 64 + q * 32;
-        uint32_t a[32];
-        tmem_ld32(tmem_base + lane_off + ATC_DQ_ACC + cc, a);
-        tmem_ld_wait();
-        atc_store_grad32(wst, reinterpret_cast<float(&)[32]>(a), p.scale,
-                         (p.rope && valid) ? p.rope + static_cast<long long>(qi) * 64 + (cc >> 1) : nullptr,
-                         p.dq32 ? &maps.g32[0] : nullptr, p.dq16 ? &maps.g16[0] : nullptr, h * ATC_D + cc, s0, b);
+      if (lane == 0) mbar_arrive(acc_free());
+      if (s0 < p.S) {
+        const float2* rr = (p.rope && valid) ? p.rope + static_cast<long long>(qi) * 64 + half * 32 : nullptr;
+        atc_store_grad32(wst, reinterpret_cast<float(&)[32]>(a0), p.scale, rr, p.dq32 ? &maps.g32[0] : nullptr,
+                         p.dq16 ? &maps.g16[0] : nullptr, w.h * ATC_D + half * 64, s0, w.b);
+        atc_store_grad32(wst, reinterpret_cast<float(&)[32]>(a1), p.scale, rr ? rr + 16 : nullptr, p.dq32 ? &maps.g32[0] : nullptr,
+                         p.dq16 ? &maps.g16[0] : nullptr, w.h * ATC_D + half * 64 + 32, s0, w.b);
       }
     }
     if (lane == 0) tma_store_wait_all<0>();
@@ -990,7 +1058,7 @@ inline cudaError_t attn_bwd_dkdv_tc_launch(const __half* q, long long ldq, const
 // dQ: Q, dO as 128-row tiles; K, V streamed as 64-row tiles
 inline cudaError_t attn_bwd_dq_tc_launch(const __half* q, long long ldq, const __half* k, long long ldk, const __half* v,
                                          long long ldv, const __half* dO, long long lddo, const AttnTcBwdParams& p,
-                                         cudaStream_t st) {
+                                         int num_sms, cudaStream_t st) {
   cudaError_t e = attn_bwd_tc_set_attrs();
   if (e != cudaSuccess) return e;
   AttnTcMaps m2;
@@ -1001,8 +1069,9 @@ inline cudaError_t attn_bwd_dq_tc_launch(const __half* q, long long ldq, const _
   if ((p.dq32 && !make_map_store(&m2.g32[0], p.dq32, p.nq * ATC_D, p.S, p.B, p.lddq32, true)) ||
       (p.dq16 && !make_map_store(&m2.g16[0], p.dq16, p.nq * ATC_D, p.S, p.B, p.ldd16, false)))
     return cudaErrorInvalidValue;
-  dim3 g2((p.S + 127) / 128, p.nq, p.B);
-  attn_bwd_dq_tc_kernel<<<g2, ATC_BWD_THREADS, ATC_DQ_SMEM, st>>>(m2, p);
+  const int nitems = ((p.S + 127) / 128) * p.nq * p.B;
+  const int grid = nitems < num_sms ? nitems : num_sms;        // persistent: one CTA per SM
+  attn_bwd_dq_tc_kernel<<<grid, ATC_BWD_THREADS, ATC_DQ_SMEM, st>>>(m2, p);
   return cudaGetLastError();
 }
 

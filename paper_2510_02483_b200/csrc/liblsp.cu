@@ -282,9 +282,9 @@ lsp_status attn_bwd_dispatch(lsp_ctx* ctx, const AttnParams& p, cudaStream_t st)
     t.B = p.B; t.S = p.S; t.nq = p.nq; t.nkv = p.nkv; t.scale_log2 = p.scale_log2; t.scale = p.scale;
     t.lse = p.lse; t.dvec = p.dvec; t.rope = p.rope;
     t.dq32 = p.dq32; t.dk32 = p.dk32; t.dv32 = p.dv32; t.lddq32 = p.lddq32; t.lddk32 = p.lddk32;
-    t.dq16 = p.dq16; t.dk16 = p.dk16; t.dv16 = p.dv16; t.ldd16 = p.ldd16;
+    t.dq16 = p.dq16; t.dk16 = p.dk16; t.dv16 = p.dv16; t.ldd16 = p.ldd16; t.sched = ctx->attn_sched;
     LSP_STAGE(ST_ATTN_BWD, 1, attn_bwd_dkdv_tc_launch(p.q, p.ldq, p.k, p.ldk, p.v, p.ldv, p.dO, p.lddo, t, st));
-    LSP_STAGE(ST_ATTN_BWD_DQ, 1, attn_bwd_dq_tc_launch(p.q, p.ldq, p.k, p.ldk, p.v, p.ldv, p.dO, p.lddo, t, st));
+    LSP_STAGE(ST_ATTN_BWD_DQ, 1, attn_bwd_dq_tc_launch(p.q, p.ldq, p.k, p.ldk, p.v, p.ldv, p.dO, p.lddo, t, ctx->num_sms, st));
     return LSP_OK;
   }
   LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_launch<64>(p, st));
