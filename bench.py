@@ -275,7 +275,7 @@ def run_ours(args):
             traffic = json.load(open(tpath)).get(w.name)
         except Exception:
             traffic = None
-    roofline = {"bound": "tensor", "kernel": "gemm_tcgen05_kernel (12 GEMM launches of the step)",
+    roofline = {"bound": "tensor", "kernel": "gemm_pair_tcgen05_kernel (12 GEMM launches of the step)",
                 "achieved": gemm_tf, "peak": peak_t, "unit": "TFLOP/s", "frac": gemm_tf / peak_t,
                 "peak_source": f"{peak_src} sustained cuBLAS bf16 (kernel timed inside a long step)",
                 "traffic": traffic, "flops_per_step": gemm_flops, "ms_per_step": gemm_ms,

@@ -68,7 +68,11 @@ typedef struct {
 
 /* Create a context for one layer shape on `cuda_device`.  Checks: n_q_heads % n_kv_heads == 0,
  * head_dim in {64,128}, hidden/ffn/Nq/Nkv multiples of 8, hidden <= 8192.  The only call (with
- * lsp_destroy) that allocates (RoPE cos/sin table [seq, head_dim/2], angles evaluated in fp64) or syncs. */
+ * lsp_destroy) that allocates or syncs.  Context-owned device memory: the RoPE cos/sin table [seq, head_dim/2]
+ * (angles evaluated in fp64), the split-K partial-accumulator slots of the GEMM tail (one 512 x 256 fp32 slot per SM
+ * pair, ~39 MB on a B200) with their publication flags, and the work-queue counters of the persistent attention
+ * kernels.  Because those are shared by every call on the context, calls on ONE context must be issued on one
+ * stream at a time (use one context per concurrent stream). */
 lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device);
 lsp_status lsp_destroy(lsp_ctx* ctx);
 size_t lsp_saved_bytes(const lsp_ctx* ctx);

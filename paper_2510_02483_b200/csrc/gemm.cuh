@@ -457,7 +457,7 @@ struct EpiSwiGLU {
     chunk_store_tma<DT_F16>(st, &umap, n, m_base, u);
 #pragma unroll
     for (int j = 0; j < 32; ++j) {
-      const float sg = 1.0f / (1.0f + __expf(-g[j]));
+      const float sg = __fdividef(1.0f, 1.0f + __expf(-g[j]));   // MUFU.EX2 + MUFU.RCP: 2 ulp, far below the 16-bit outputs
       g[j] = g[j] * sg * u[j];
     }
     chunk_store_tma<DT_F16>(st, &hmap, n, m_base, g);
@@ -486,7 +486,7 @@ struct EpiSwiGLUBwd {
     chunk_load<DT_F16>(st, [&](int rr) { return u16 + off + rr * ld; }, u, nrows, nvalid);
 #pragma unroll
     for (int j = 0; j < 32; ++j) {
-      const float sg = 1.0f / (1.0f + __expf(-g[j]));
+      const float sg = __fdividef(1.0f, 1.0f + __expf(-g[j]));   // MUFU.EX2 + MUFU.RCP: 2 ulp, far below the 16-bit outputs
       const float dgv = dh[j] * u[j] * sg * (1.0f + g[j] * (1.0f - sg));
       u[j] = dh[j] * g[j] * sg;           // du
       g[j] = dgv;                         // dg
