@@ -126,7 +126,9 @@ lsp_status lsp_gemm(lsp_ctx* ctx, int op, int M, int N, int K, const void* A, in
 
 /* End-to-end step with HOST buffers (bench.py `e2e`): copies x, dy (in_dtype, [T,H]; pinned host memory for
  * asynchronous copies) to the caller's device staging buffers x_dev / dy_dev, runs lsp_layer_fwd + lsp_layer_bwd,
- * and copies y and dx (fp32 [T,H]) back to y_host / dx_host, all enqueued on `stream` (no sync).  Weights and
+ * and copies y and dx (fp32 [T,H]) back to y_host / dx_host (no sync).  The copies run on two context-owned streams
+ * ordered against `stream` with events, so the upload of dy overlaps the forward pass and the download of y the
+ * backward pass; `stream` completes after the last copy.  Weights and
  * weight gradients stay on the device (DEVICE pointers), as they do in a training step. */
 lsp_status lsp_layer_step_host(lsp_ctx* ctx, const void* x_host, const void* dy_host, const lsp_layer_weights* w,
                                void* y_host, void* dx_host, lsp_layer_wgrads* grads, void* x_dev, void* dy_dev,

@@ -61,6 +61,8 @@ struct lsp_ctx {
   unsigned int* sk_flags;        // [num_sms/2][2] publication epochs (device, zeroed at create)
   unsigned int gemm_seq;         // launches so far: epoch of the next stream-K launch
   unsigned int* attn_sched;      // work-item counters of the persistent attention kernels (device, zero between launches)
+  cudaStream_t s_in, s_out;      // copy streams of lsp_layer_step_host (H2D / D2H overlap the compute stream)
+  cudaEvent_t ev[6];             // start, x in, dy in, fwd done, bwd done, copies out
   int norm_blocks;      // persistent grid of the RMSNorm backward
   SavedLayout sv;
   WsLayout ws;
@@ -539,6 +541,13 @@ lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device
       return LSP_ENOMEM;
     }
   }
+  if (cudaStreamCreateWithFlags(&ctx->s_in, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&ctx->s_out, cudaStreamNonBlocking) != cudaSuccess) {
+    lsp_destroy(ctx);
+    return LSP_ECUDA;
+  }
+  for (int i = 0; i < 6; ++i)
+    if (cudaEventCreateWithFlags(&ctx->ev[i], cudaEventDisableTiming) != cudaSuccess) { lsp_destroy(ctx); return LSP_ECUDA; }
   *out = ctx;
   return LSP_OK;
 }
@@ -550,6 +559,10 @@ lsp_status lsp_destroy(lsp_ctx* ctx) {
   cudaFree(ctx->sk_partial);
   cudaFree(ctx->sk_flags);
   cudaFree(ctx->attn_sched);
+  if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
+  if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
+  for (int i = 0; i < 6; ++i)
+    if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
   delete ctx;
   return LSP_OK;
 }
@@ -720,12 +733,28 @@ lsp_status lsp_layer_step_host(lsp_ctx* ctx, const void* x_host, const void* dy_
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const size_t n = static_cast<size_t>(ctx->T) * ctx->d.hidden;
   const size_t in_bytes = n * (ctx->d.in_dtype == LSP_F32 ? 4 : 2);
-  LSP_CUDA(cudaMemcpyAsync(x_dev, x_host, in_bytes, cudaMemcpyHostToDevice, st));
-  LSP_CUDA(cudaMemcpyAsync(dy_dev, dy_host, in_bytes, cudaMemcpyHostToDevice, st));
+  // Copies run on two context-owned streams so that the upload of dy overlaps the forward pass and the download of y
+  // overlaps the backward pass; everything is ordered after what `st` held before and `st` ends after the last copy.
+  cudaEvent_t* ev = ctx->ev;
+  LSP_CUDA(cudaEventRecord(ev[0], st));
+  LSP_CUDA(cudaStreamWaitEvent(ctx->s_in, ev[0], 0));
+  LSP_CUDA(cudaStreamWaitEvent(ctx->s_out, ev[0], 0));
+  LSP_CUDA(cudaMemcpyAsync(x_dev, x_host, in_bytes, cudaMemcpyHostToDevice, ctx->s_in));
+  LSP_CUDA(cudaEventRecord(ev[1], ctx->s_in));
+  LSP_CUDA(cudaMemcpyAsync(dy_dev, dy_host, in_bytes, cudaMemcpyHostToDevice, ctx->s_in));
+  LSP_CUDA(cudaEventRecord(ev[2], ctx->s_in));
+  LSP_CUDA(cudaStreamWaitEvent(st, ev[1], 0));
   LSP_TRY(lsp_layer_fwd(ctx, x_dev, w, y_dev, saved, ws, stream));
-  LSP_CUDA(cudaMemcpyAsync(y_host, y_dev, n * 4, cudaMemcpyDeviceToHost, st));
+  LSP_CUDA(cudaEventRecord(ev[3], st));
+  LSP_CUDA(cudaStreamWaitEvent(ctx->s_out, ev[3], 0));
+  LSP_CUDA(cudaMemcpyAsync(y_host, y_dev, n * 4, cudaMemcpyDeviceToHost, ctx->s_out));
+  LSP_CUDA(cudaStreamWaitEvent(st, ev[2], 0));
   LSP_TRY(lsp_layer_bwd(ctx, x_dev, dy_dev, w, saved, dx_dev, g, ws, stream));
-  LSP_CUDA(cudaMemcpyAsync(dx_host, dx_dev, n * 4, cudaMemcpyDeviceToHost, st));
+  LSP_CUDA(cudaEventRecord(ev[4], st));
+  LSP_CUDA(cudaStreamWaitEvent(ctx->s_out, ev[4], 0));
+  LSP_CUDA(cudaMemcpyAsync(dx_host, dx_dev, n * 4, cudaMemcpyDeviceToHost, ctx->s_out));
+  LSP_CUDA(cudaEventRecord(ev[5], ctx->s_out));
+  LSP_CUDA(cudaStreamWaitEvent(st, ev[5], 0));
   return LSP_OK;
 }
 

@@ -156,6 +156,44 @@ def test_layer_fwd_bwd(gpu, w):
     check(got, ref, ALL)
 
 
+def test_layer_bit_reproducible(gpu):
+    """Two runs of the same step give bit-identical outputs and gradients (reading A-14): the attention work queues are
+    dynamic (atomic item counters) and the GEMM tails exchange partials through global memory, but every output
+    element has one fixed summation order."""
+    a = gpu.run_layer(MID)
+    b = gpu.run_layer(MID)
+    for n in ALL:
+        assert np.array_equal(a[n], b[n]), n
+
+
+def test_layer_step_host_matches_device_path(gpu):
+    """lsp_layer_step_host (pinned HOST x, dy in; y, dx out; copies on context-owned streams overlapping the compute
+    stream) returns exactly what lsp_layer_fwd + lsp_layer_bwd produce from device-resident inputs."""
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    w = MID
+    ref = gpu.run_layer(w)
+    dev = gpu.require_cuda()
+    ctx = gpu.make_ctx(w)
+    buf = gpu.LayerBuffers(ctx, w, dev)
+    weights = gpu.upload_weights(synth.layer_weights(w, 0), dev)
+    inp = synth.layer_inputs(w)
+    hx, hdy = gpu.bf16_pinned(inp["x"]), gpu.bf16_pinned(inp["dy"])
+    T, H = w.tokens, w.hidden
+    hy = torch.empty((T, H), dtype=torch.float32).pin_memory()
+    hdx = torch.empty((T, H), dtype=torch.float32).pin_memory()
+    x_dev = torch.empty((T, H), dtype=torch.bfloat16, device=dev)
+    dy_dev = torch.empty((T, H), dtype=torch.bfloat16, device=dev)
+    for _ in range(2):                         # twice: the event / stream plumbing must be reusable
+        hy.fill_(float("nan")); hdx.fill_(float("nan"))
+        B.lsp_layer_step_host(ctx, hx, hdy, weights, hy, hdx, buf.grads, x_dev, dy_dev, buf.y, buf.dx, buf.saved, buf.ws)
+        torch.cuda.current_stream().synchronize()
+        assert np.array_equal(hy.numpy(), ref["y"]) and np.array_equal(hdx.numpy(), ref["dx"])
+        for k, v in buf.grads.items():
+            assert np.array_equal(v.cpu().numpy(), ref["d" + k]), k
+    ctx.close()
+
+
 def test_blocks_cfg1(gpu):
     """lsp_attn_fwd/bwd and lsp_mlp_fwd/bwd called on their own (block-level entry points), bf16 in."""
     import torch
@@ -188,7 +226,8 @@ def test_blocks_cfg1(gpu):
 
 
 # ------------------------------------------------------------------------------------------- attention core (cfg 5 layout)
-@pytest.mark.parametrize("B_,S,nq,nkv,d", [(2, 256, 24, 8, 128), (1, 200, 4, 4, 64), (1, 1, 2, 1, 128), (3, 65, 6, 2, 128)])
+@pytest.mark.parametrize("B_,S,nq,nkv,d", [(2, 256, 24, 8, 128), (1, 200, 4, 4, 64), (1, 1, 2, 1, 128), (3, 65, 6, 2, 128),
+                                            (2, 640, 6, 2, 128), (1, 300, 4, 2, 128)])
 def test_sdpa_fwd_bwd(gpu, B_, S, nq, nkv, d):
     """lsp_sdpa_fwd/bwd: O, L, dq, dk, dv on bf16 Q,K,V,dO ~ N(0,1) (no RoPE), incl. ragged S and S = 1."""
     import torch
