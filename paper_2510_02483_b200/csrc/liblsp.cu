@@ -224,6 +224,23 @@ cudaError_t cast_bf16_f16(const __nv_bfloat16* in, __half* out, long long n, int
   return cudaGetLastError();
 }
 
+// up to CAST_MAX_SEGS bf16 -> fp16 weight casts in one launch (element counts are multiples of 8)
+cudaError_t cast_weights(const lsp_ctx* c, int nseg, const void* const* src, __half* const* dst, const long long* n, cudaStream_t st) {
+  CastSegs segs;
+  segs.nseg = nseg;
+  segs.start[0] = 0;
+  for (int i = 0; i < CAST_MAX_SEGS; ++i) {
+    segs.src[i] = i < nseg ? static_cast<const __nv_bfloat16*>(src[i]) : nullptr;
+    segs.dst[i] = i < nseg ? dst[i] : nullptr;
+    segs.start[i + 1] = segs.start[i] + (i < nseg ? n[i] / 8 : 0);
+  }
+  long long blocks = (segs.start[nseg] + 255) / 256;
+  if (blocks > c->num_sms * 16LL) blocks = c->num_sms * 16LL;
+  if (blocks < 1) blocks = 1;
+  cast_multi_bf16_f16_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(segs);
+  return cudaGetLastError();
+}
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------------- GEMM call sites
@@ -261,10 +278,6 @@ cudaError_t gemm_fwd_residual(const lsp_ctx* c, const __half* A, int K, const __
   e.out[0] = out; e.out[1] = e.out[2] = nullptr; e.split1 = e.split2 = 0x7fffffff; e.ld = H; e.res = res; e.alpha = 1.0f;
   return gemm1<false, false>(c, T, H, K, a, b, e, st);
 }
-
-// fp16 copy of a bf16 weight matrix (exact for 2^-17 <= |w| < 65504; DESIGN.md precision plan)
-#define LSP_WCAST(src, dst, n) \
-  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(src), dst, static_cast<long long>(n), ctx->num_sms, st))
 
 // F3 dispatch: head_dim 128 runs on tcgen05 (attn_tc.cuh); head_dim 64 on the mma.sync kernel (attn.cuh).
 cudaError_t attn_fwd_dispatch(const lsp_ctx* c, const AttnParams& p, cudaStream_t st) {
@@ -308,10 +321,13 @@ lsp_status attn_fwd_impl(lsp_ctx* ctx, int x_dt, const void* x, const lsp_layer_
   __half* wqkv16 = at<__half>(saved, ctx->sv.wqkv16);
   __half* wo16 = at<__half>(saved, ctx->sv.wo16);
 
-  LSP_WCAST(w->wq, wqkv16, static_cast<long long>(Nq) * H);
-  LSP_WCAST(w->wk, wqkv16 + static_cast<long long>(Nq) * H, static_cast<long long>(Nkv) * H);
-  LSP_WCAST(w->wv, wqkv16 + static_cast<long long>(Nq + Nkv) * H, static_cast<long long>(Nkv) * H);
-  LSP_WCAST(w->wo, wo16, static_cast<long long>(H) * Nq);
+  {
+    const void* src[4] = {w->wq, w->wk, w->wv, w->wo};
+    __half* dst[4] = {wqkv16, wqkv16 + static_cast<long long>(Nq) * H, wqkv16 + static_cast<long long>(Nq + Nkv) * H, wo16};
+    const long long cnt[4] = {static_cast<long long>(Nq) * H, static_cast<long long>(Nkv) * H, static_cast<long long>(Nkv) * H,
+                              static_cast<long long>(H) * Nq};
+    LSP_STAGE(ST_CAST, 1, cast_weights(ctx, 4, src, dst, cnt, st));
+  }
   // F1 RMSNorm-1
   LSP_STAGE(ST_NORM_FWD, 1, norm_fwd(ctx, x_dt, x, w->g_attn, xn, rstd1, st));
   // F2 fused QKV projection with the RoPE epilogue (q, k rotated; v plain) into one [T, Nq+2Nkv] fp16 buffer
@@ -402,9 +418,12 @@ lsp_status mlp_fwd_impl(lsp_ctx* ctx, int a_dt, const void* a, const lsp_layer_w
   __half* wgu16 = at<__half>(saved, ctx->sv.wgu16);
   __half* wd16 = at<__half>(saved, ctx->sv.wd16);
   const long long FH = static_cast<long long>(F) * H;
-  LSP_WCAST(w->w_gate, wgu16, FH);
-  LSP_WCAST(w->w_up, wgu16 + FH, FH);
-  LSP_WCAST(w->w_down, wd16, FH);
+  {
+    const void* src[3] = {w->w_gate, w->w_up, w->w_down};
+    __half* dst[3] = {wgu16, wgu16 + FH, wd16};
+    const long long cnt[3] = {FH, FH, FH};
+    LSP_STAGE(ST_CAST, 1, cast_weights(ctx, 3, src, dst, cnt, st));
+  }
   LSP_STAGE(ST_NORM_FWD, 1, norm_fwd(ctx, a_dt, a, w->g_mlp, an, rstd2, st));
   EpiSwiGLU e{h, g16, u16, F};
   const GemmSKRes sk{ctx->sk_partial, ctx->sk_flags, ++ctx->gemm_seq};

@@ -238,6 +238,28 @@ __global__ void cast_bf16_f16_kernel(const __nv_bfloat16* __restrict__ in, __hal
   }
 }
 
+// Several bf16 -> fp16 casts in one launch (the weight tensors of a block): segment s covers 8-element groups
+// [start[s], start[s + 1]) of the concatenated index space.
+constexpr int CAST_MAX_SEGS = 4;
+struct CastSegs {
+  const __nv_bfloat16* src[CAST_MAX_SEGS];
+  __half* dst[CAST_MAX_SEGS];
+  long long start[CAST_MAX_SEGS + 1];
+  int nseg;
+};
+__global__ void cast_multi_bf16_f16_kernel(const CastSegs segs) {
+  const long long total = segs.start[segs.nseg];
+  for (long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i < total; i += static_cast<long long>(gridDim.x) * blockDim.x) {
+    int s = 0;
+#pragma unroll
+    for (int k = 1; k < CAST_MAX_SEGS; ++k) s += (k < segs.nseg && i >= segs.start[k]) ? 1 : 0;
+    const long long j = i - segs.start[s];
+    const uint4 u = __ldg(reinterpret_cast<const uint4*>(segs.src[s]) + j);
+    reinterpret_cast<uint4*>(segs.dst[s])[j] = make_uint4(pack_f16(bf16_lo(u.x), bf16_hi(u.x)), pack_f16(bf16_lo(u.y), bf16_hi(u.y)),
+                                                         pack_f16(bf16_lo(u.z), bf16_hi(u.z)), pack_f16(bf16_lo(u.w), bf16_hi(u.w)));
+  }
+}
+
 // x0[t,:] = E[id_t,:]  (bf16 table row -> fp32 or bf16 stream).  One block per token.
 template <typename OT>
 __global__ void embed_gather_kernel(const int* __restrict__ ids, const __nv_bfloat16* __restrict__ table, OT* __restrict__ out, int H) {
