@@ -1,0 +1,113 @@
+"""Device-side timing of every BASELINE.json configuration (bench.py covers the headline config 2 only).
+
+    python -m paper_2510_02483_b200.configs_bench [--steps K] [--only cfg2,cfg3,cfg4,cfg5]
+
+Prints one JSON line per configuration: ms per fwd+bwd step (CUDA events on the launching stream, after warm-up),
+tokens/s and executed TFLOP/s (causal attention FLOPs, SURVEY.md 8(d) convention).  Inputs are the seeded synthetic
+tensors of synth.py, resident in HBM.  Every step runs through the C ABI (binding.py); nothing here imports the oracle.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+
+import torch
+
+from . import binding as B
+from . import harness, synth
+
+
+def _time(fn, steps, warmup=3):
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / steps
+
+
+def bench_layer(w, steps):
+    dev = harness.require_cuda()
+    ctx = harness.make_ctx(w)
+    buf = harness.LayerBuffers(ctx, w, dev)
+    weights = harness.upload_weights(synth.layer_weights(w), dev)
+    inp = synth.layer_inputs(w)
+    x, dy = harness.bf16_to_device(inp["x"], dev), harness.bf16_to_device(inp["dy"], dev)
+
+    def step():
+        B.lsp_layer_fwd(ctx, x, weights, buf.y, buf.saved, buf.ws)
+        B.lsp_layer_bwd(ctx, x, dy, weights, buf.saved, buf.dx, buf.grads, buf.ws)
+    ms = _time(step, steps)
+    ctx.close()
+    return ms, synth.layer_flops(w, causal=True)
+
+
+def bench_stack(w, steps):
+    """Config 3: embedding gather + n_layers x (fwd) + n_layers x (bwd); every layer has its own seeded weights."""
+    dev = harness.require_cuda()
+    run = harness.StackRunner(w, w.n_layers, dev)
+    s = synth.stack_inputs(w)
+    ids = torch.from_numpy(s["ids"]).to(dev)
+    table = harness.bf16_to_device(s["embedding"], dev)
+    dy = harness.bf16_to_device(synth.layer_inputs(w)["dy"], dev).float()
+
+    def step():
+        run.forward(ids, table)
+        run.backward(dy)
+    ms = _time(step, steps, warmup=2)
+    run.close()
+    return ms, w.n_layers * synth.layer_flops(w, causal=True)
+
+
+def bench_sdpa(w, steps):
+    dev = harness.require_cuda()
+    ctx = harness.make_ctx(w, use_rope=False)
+    t = {k: harness.bf16_to_device(v, dev) for k, v in synth.attn_inputs(w).items()}
+    Bz, S, nq, nkv, d = w.batch, w.seq, w.n_q_heads, w.n_kv_heads, w.head_dim
+    o = torch.empty((Bz, S, nq, d), dtype=torch.float32, device=dev)
+    lse = torch.empty((Bz, nq, S), dtype=torch.float32, device=dev)
+    dq = torch.empty_like(o)
+    dk = torch.empty((Bz, S, nkv, d), dtype=torch.float32, device=dev)
+    dv = torch.empty_like(dk)
+    ws = torch.empty(ctx.workspace_bytes, dtype=torch.uint8, device=dev)
+
+    def step():
+        B.lsp_sdpa_fwd(ctx, t["q"], t["k"], t["v"], o, lse, ws)
+        B.lsp_sdpa_bwd(ctx, t["q"], t["k"], t["v"], o, lse, t["dO"], dq, dk, dv, ws)
+    ms = _time(step, steps)
+    ctx.close()
+    fwd = 4.0 * d * nq * Bz * S * (S + 1) / 2.0
+    return ms, 3.5 * fwd
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--only", default="cfg2,cfg3,cfg4,cfg5")
+    args = ap.parse_args(argv)
+    B.lib()
+    only = set(args.only.split(","))
+    jobs = []
+    if "cfg2" in only:
+        jobs.append((synth.CFG2_3B_LAYER, bench_layer))
+    if "cfg4" in only:
+        jobs.append((synth.CFG4_30B_LAYER, bench_layer))
+    if "cfg3" in only:
+        jobs.append((synth.CFG3_3B_STACK, bench_stack))
+    if "cfg5" in only:
+        jobs += [(w, bench_sdpa) for w in synth.CFG5_ATTN]
+    for w, fn in jobs:
+        ms, flops = fn(w, max(2, args.steps if fn is not bench_stack else min(args.steps, 3)))
+        print(json.dumps({"config": w.name, "batch": w.batch, "seq": w.seq, "tokens": w.tokens, "ms_per_step": round(ms, 4),
+                          "tokens_per_s": round(w.tokens / (ms * 1e-3), 1), "tflops_executed": round(flops / (ms * 1e-3) / 1e12, 1)}),
+              flush=True)
+        torch.cuda.empty_cache()
+    return 0
+
+
+if __name__ == "__main__":
+    raise SystemExit(main())
