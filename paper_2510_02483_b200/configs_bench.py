@@ -1,6 +1,6 @@
 """Device-side timing of every BASELINE.json configuration (bench.py covers the headline config 2 only).
 
-    python -m paper_2510_02483_b200.configs_bench [--steps K] [--only cfg2,cfg3,cfg4,cfg5]
+    python -m paper_2510_02483_b200.configs_bench [--steps K] [--only cfg2,cfg3,cfg4,cfg5,table1]
 
 Prints one JSON line per configuration: ms per fwd+bwd step (CUDA events on the launching stream, after warm-up),
 tokens/s and executed TFLOP/s (causal attention FLOPs, SURVEY.md 8(d) convention).  Inputs are the seeded synthetic
@@ -87,7 +87,7 @@ def bench_sdpa(w, steps):
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--only", default="cfg2,cfg3,cfg4,cfg5")
+    ap.add_argument("--only", default="cfg2,cfg3,cfg4,cfg5,table1")
     args = ap.parse_args(argv)
     B.lib()
     only = set(args.only.split(","))
@@ -96,6 +96,8 @@ def main(argv=None):
         jobs.append((synth.CFG2_3B_LAYER, bench_layer))
     if "cfg4" in only:
         jobs.append((synth.CFG4_30B_LAYER, bench_layer))
+    if "table1" in only:      # the paper's own Table-1 3B layer shape: hidden 2048, 16q / 2kv, FFN 11008
+        jobs.append((synth.Workload("table1_3b_layer", 6, 4, 4096, 2048, 16, 2, 128, 11008, 1e-5, 10000.0), bench_layer))
     if "cfg3" in only:
         jobs.append((synth.CFG3_3B_STACK, bench_stack))
     if "cfg5" in only:

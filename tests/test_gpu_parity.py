@@ -145,9 +145,11 @@ def test_gemm_mixed_formats_rejected(gpu):
 # ------------------------------------------------------------------------------------------- whole layer
 MID = synth.Workload("mid", 101, 2, 320, 512, 8, 2, 128, 1376, 1e-5, 500000.0)
 MID64 = synth.Workload("mid64", 102, 3, 200, 384, 6, 6, 64, 1000, 1e-5, 10000.0)
+# the paper's own 3B shape (Table 1: hidden 2048, 16 query / 2 KV heads -> G = 8, FFN 11008), one short sequence
+T1_3B = synth.Workload("table1_3b", 103, 1, 512, 2048, 16, 2, 128, 11008, 1e-5, 10000.0)
 
 
-@pytest.mark.parametrize("w", [synth.CFG1_TINY, MID, MID64], ids=lambda w: w.name)
+@pytest.mark.parametrize("w", [synth.CFG1_TINY, MID, MID64, T1_3B], ids=lambda w: w.name)
 def test_layer_fwd_bwd(gpu, w):
     """lsp_layer_fwd + lsp_layer_bwd: y, dx and all nine gradients (cfg 1 = BASELINE.json configs[0])."""
     got = gpu.run_layer(w)
