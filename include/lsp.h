@@ -134,6 +134,26 @@ lsp_status lsp_layer_step_host(lsp_ctx* ctx, const void* x_host, const void* dy_
                                void* y_host, void* dx_host, lsp_layer_wgrads* grads, void* x_dev, void* dy_dev,
                                void* y_dev, void* dx_dev, void* saved, void* ws, void* stream);
 
+/* Optimizer step after the backward (Table 2): AdamW with decoupled weight decay
+ * and bias-corrected moments (ref [40]), preceded by clipping of the GLOBAL l2 gradient norm over all tensors of the
+ * call (readings O-1 .. O-5 in DESIGN.md section 12).  Per tensor i of `n` elements (n % 4 == 0, pointers 16-byte
+ * aligned): grad fp32 (read), master / m / v fp32 (updated in place), weight_bf16 (written: round-to-nearest-even of
+ * the new master weight; may be NULL), decay = 1 if weight decay applies.  `tensors` is a HOST array of
+ * 1 <= ntensors <= 16 entries.  gnorm_out: DEVICE float[2], receives {global norm, clip coefficient} (no host sync).
+ * Everything is enqueued on `stream`; results are bit-reproducible. */
+typedef struct {
+  const void* grad; float* master; float* m; float* v; void* weight_bf16; int64_t n; int32_t decay;
+} lsp_adamw_tensor;
+typedef struct {
+  float lr, beta1, beta2, eps, weight_decay, clip_norm;   /* paper: lr from lsp_lr_cosine, 0.90, 0.95, 1e-8, 0.01, 1.0 */
+  int32_t step;                                            /* 1-based optimizer step t (bias correction 1 - beta^t) */
+} lsp_adamw_desc;
+lsp_status lsp_adamw_step(lsp_ctx* ctx, int ntensors, const lsp_adamw_tensor* tensors, const lsp_adamw_desc* desc,
+                          float* gnorm_out, void* stream);
+/* Host helper (no GPU): the paper's schedule: linear warm-up from 0 to lr_max over `warmup` steps, then
+ * cosine decay to lr_min at step `total`, lr_min afterwards (reading O-3).  step is 1-based. */
+double lsp_lr_cosine(int step, double lr_max, double lr_min, int warmup, int total);
+
 /* Measurement aids; they change no result.
  * lsp_launch_count: kernels launched through this context so far.
  * lsp_timing_enable(n > 0): pre-create n CUDA-event pairs; from then on every pipeline stage records one pair on

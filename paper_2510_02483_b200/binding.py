@@ -18,7 +18,7 @@ WEIGHT_FIELDS = ("wq", "wk", "wv", "wo", "g_attn", "w_gate", "w_up", "w_down", "
 EXPORTS = ("lsp_create", "lsp_destroy", "lsp_saved_bytes", "lsp_workspace_bytes", "lsp_last_error",
            "lsp_attn_fwd", "lsp_attn_bwd", "lsp_mlp_fwd", "lsp_mlp_bwd", "lsp_layer_fwd", "lsp_layer_bwd",
            "lsp_sdpa_fwd", "lsp_sdpa_bwd", "lsp_embed_fwd", "lsp_gemm", "lsp_layer_step_host", "lsp_launch_count",
-           "lsp_timing_enable", "lsp_timing_read")
+           "lsp_timing_enable", "lsp_timing_read", "lsp_adamw_step", "lsp_lr_cosine")
 
 
 class LspError(RuntimeError):
@@ -34,6 +34,16 @@ class lsp_layer_desc(C.Structure):
 
 class lsp_layer_weights(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in WEIGHT_FIELDS]
+
+
+class lsp_adamw_tensor(C.Structure):
+    _fields_ = [("grad", C.c_void_p), ("master", C.c_void_p), ("m", C.c_void_p), ("v", C.c_void_p),
+                ("weight_bf16", C.c_void_p), ("n", C.c_int64), ("decay", C.c_int32)]
+
+
+class lsp_adamw_desc(C.Structure):
+    _fields_ = [("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float),
+                ("weight_decay", C.c_float), ("clip_norm", C.c_float), ("step", C.c_int32)]
 
 
 class lsp_layer_wgrads(C.Structure):
@@ -71,8 +81,11 @@ def lib():
         L.lsp_launch_count.argtypes = [vp]; L.lsp_launch_count.restype = C.c_longlong
         L.lsp_timing_enable.argtypes = [vp, i32]
         L.lsp_timing_read.argtypes = [vp, i32, C.POINTER(C.c_char_p), C.POINTER(C.c_float), C.POINTER(i32)]
+        L.lsp_adamw_step.argtypes = [vp, i32, C.POINTER(lsp_adamw_tensor), C.POINTER(lsp_adamw_desc), vp, vp]
+        L.lsp_lr_cosine.argtypes = [i32, C.c_double, C.c_double, i32, i32]
+        L.lsp_lr_cosine.restype = C.c_double
         for n in EXPORTS:
-            if n not in ("lsp_saved_bytes", "lsp_workspace_bytes", "lsp_last_error", "lsp_launch_count"):
+            if n not in ("lsp_saved_bytes", "lsp_workspace_bytes", "lsp_last_error", "lsp_launch_count", "lsp_lr_cosine"):
                 getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -191,6 +204,22 @@ def lsp_layer_step_host(ctx, x_host, dy_host, weights, y_host, dx_host, grads, x
     ctx.check(lib().lsp_layer_step_host(ctx.handle, _ptr(x_host), _ptr(dy_host), C.byref(w), _ptr(y_host), _ptr(dx_host),
                                         C.byref(g), _ptr(x_dev), _ptr(dy_dev), _ptr(y_dev), _ptr(dx_dev), _ptr(saved),
                                         _ptr(ws), _stream(stream)))
+
+
+def lsp_adamw_step(ctx, tensors, *, lr, step, gnorm_out, beta1=0.90, beta2=0.95, eps=1e-8, weight_decay=0.01, clip_norm=1.0,
+                   stream=None):
+    """tensors: list of dicts {grad, master, m, v, weight (bf16 or None), decay (bool)} of torch CUDA tensors."""
+    arr = (lsp_adamw_tensor * len(tensors))()
+    for i, t in enumerate(tensors):
+        w = t.get("weight")
+        arr[i] = lsp_adamw_tensor(t["grad"].data_ptr(), t["master"].data_ptr(), t["m"].data_ptr(), t["v"].data_ptr(),
+                                  None if w is None else w.data_ptr(), t["master"].numel(), 1 if t.get("decay", True) else 0)
+    d = lsp_adamw_desc(lr, beta1, beta2, eps, weight_decay, clip_norm, step)
+    ctx.check(lib().lsp_adamw_step(ctx.handle, len(tensors), arr, C.byref(d), _ptr(gnorm_out), _stream(stream)))
+
+
+def lsp_lr_cosine(step: int, lr_max: float = 1.2e-3, lr_min: float = 1.0e-5, warmup: int = 2000, total: int = 100000) -> float:
+    return float(lib().lsp_lr_cosine(step, lr_max, lr_min, warmup, total))
 
 
 def lsp_launch_count(ctx) -> int:

@@ -1,6 +1,6 @@
 """Device-side timing of every BASELINE.json configuration (bench.py covers the headline config 2 only).
 
-    python -m paper_2510_02483_b200.configs_bench [--steps K] [--only cfg2,cfg3,cfg4,cfg5,table1]
+    python -m paper_2510_02483_b200.configs_bench [--steps K] [--only cfg2,cfg3,cfg4,cfg5,table1,adamw]
 
 Prints one JSON line per configuration: ms per fwd+bwd step (CUDA events on the launching stream, after warm-up),
 tokens/s and executed TFLOP/s (causal attention FLOPs, SURVEY.md 8(d) convention).  Inputs are the seeded synthetic
@@ -84,10 +84,33 @@ def bench_sdpa(w, steps):
     return ms, 3.5 * fwd
 
 
+def bench_adamw(w, steps):
+    """Optimizer step (lsp_adamw_step) on the nine tensors of one layer of workload `w`: HBM-bound, 34 algorithmic bytes
+    per parameter (norm pass 4 B; update reads g, p, m, v 16 B, writes p, m, v and the bf16 weight 14 B)."""
+    dev = harness.require_cuda()
+    ctx = harness.make_ctx(synth.CFG1_TINY)
+    tensors = []
+    for k, shape in harness.WEIGHT_SHAPES(w).items():
+        f = lambda: torch.randn(shape, dtype=torch.float32, device=dev) * 0.02
+        tensors.append(dict(grad=f(), master=f(), m=torch.zeros(shape, dtype=torch.float32, device=dev),
+                            v=torch.zeros(shape, dtype=torch.float32, device=dev),
+                            weight=torch.empty(shape, dtype=torch.bfloat16, device=dev), decay=len(shape) == 2))
+    gn = torch.zeros(2, dtype=torch.float32, device=dev)
+    state = {"t": 0}
+
+    def step():
+        state["t"] += 1
+        B.lsp_adamw_step(ctx, tensors, lr=B.lsp_lr_cosine(state["t"]), step=state["t"], gnorm_out=gn)
+    ms = _time(step, steps)
+    ctx.close()
+    nparam = sum(t["master"].numel() for t in tensors)
+    return ms, nparam
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--only", default="cfg2,cfg3,cfg4,cfg5,table1")
+    ap.add_argument("--only", default="cfg2,cfg3,cfg4,cfg5,table1,adamw")
     args = ap.parse_args(argv)
     B.lib()
     only = set(args.only.split(","))
@@ -102,6 +125,12 @@ def main(argv=None):
         jobs.append((synth.CFG3_3B_STACK, bench_stack))
     if "cfg5" in only:
         jobs += [(w, bench_sdpa) for w in synth.CFG5_ATTN]
+    if "adamw" in only:
+        for w in (synth.CFG2_3B_LAYER, synth.CFG4_30B_LAYER):
+            ms, nparam = bench_adamw(w, args.steps)
+            print(json.dumps({"config": "adamw_" + w.name, "params": nparam, "ms_per_step": round(ms, 4),
+                              "algorithmic_GB_per_s": round(34.0 * nparam / (ms * 1e-3) / 1e9, 1)}), flush=True)
+            torch.cuda.empty_cache()
     for w, fn in jobs:
         ms, flops = fn(w, max(2, args.steps if fn is not bench_stack else min(args.steps, 3)))
         print(json.dumps({"config": w.name, "batch": w.batch, "seq": w.seq, "tokens": w.tokens, "ms_per_step": round(ms, 4),

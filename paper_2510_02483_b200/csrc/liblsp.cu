@@ -15,6 +15,7 @@
 #include "attn_tc.cuh"
 #include "gemm.cuh"
 #include "norm.cuh"
+#include "optim.cuh"
 
 using namespace lsp;
 
@@ -39,12 +40,12 @@ struct WsLayout {
 enum Stage : int {
   ST_CAST = 0, ST_NORM_FWD, ST_QKV, ST_ATTN_FWD, ST_OPROJ, ST_GATEUP, ST_DOWN,
   ST_WGRAD_DOWN, ST_DGRAD_DOWN, ST_WGRAD_GATEUP, ST_DGRAD_GATEUP, ST_NORM_BWD,
-  ST_WGRAD_O, ST_DGRAD_O, ST_DVEC, ST_ATTN_BWD, ST_WGRAD_QKV, ST_DGRAD_QKV, ST_EMBED, ST_ATTN_BWD_DQ, ST_COUNT
+  ST_WGRAD_O, ST_DGRAD_O, ST_DVEC, ST_ATTN_BWD, ST_WGRAD_QKV, ST_DGRAD_QKV, ST_EMBED, ST_ATTN_BWD_DQ, ST_ADAMW, ST_COUNT
 };
 static const char* const STAGE_NAMES[ST_COUNT] = {
   "cast", "rmsnorm_fwd", "gemm_qkv_rope", "attn_fwd", "gemm_oproj_res", "gemm_gateup_swiglu", "gemm_down_res",
   "wgrad_down", "dgrad_down_swiglu_bwd", "wgrad_gateup", "dgrad_gateup", "rmsnorm_bwd",
-  "wgrad_oproj", "dgrad_oproj", "attn_dvec", "attn_bwd", "wgrad_qkv", "dgrad_qkv", "embed_gather", "attn_bwd_dq"};
+  "wgrad_oproj", "dgrad_oproj", "attn_dvec", "attn_bwd", "wgrad_qkv", "dgrad_qkv", "embed_gather", "attn_bwd_dq", "adamw"};
 
 struct TimingRec { int stage; cudaEvent_t beg, end; };
 
@@ -61,6 +62,7 @@ struct lsp_ctx {
   unsigned int* sk_flags;        // [num_sms/2][2] publication epochs (device, zeroed at create)
   unsigned int gemm_seq;         // launches so far: epoch of the next stream-K launch
   unsigned int* attn_sched;      // work-item counters of the persistent attention kernels (device, zero between launches)
+  float* opt_partial;            // per-block partial sums of the gradient-norm pass (device)
   cudaStream_t s_in, s_out;      // copy streams of lsp_layer_step_host (H2D / D2H overlap the compute stream)
   cudaEvent_t ev[6];             // start, x in, dy in, fwd done, bwd done, copies out
   int norm_blocks;      // persistent grid of the RMSNorm backward
@@ -554,9 +556,10 @@ lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device
     if (cudaMalloc(&ctx->sk_partial, pairs * GEMM2_PARTIAL_FLOATS * sizeof(float)) != cudaSuccess ||
         cudaMalloc(&ctx->sk_flags, pairs * 2 * sizeof(unsigned int)) != cudaSuccess ||
         cudaMemset(ctx->sk_flags, 0, pairs * 2 * sizeof(unsigned int)) != cudaSuccess ||
+        cudaMalloc(&ctx->opt_partial, 4096 * sizeof(float)) != cudaSuccess ||
         cudaMalloc(&ctx->attn_sched, 16 * sizeof(unsigned int)) != cudaSuccess ||
         cudaMemset(ctx->attn_sched, 0, 16 * sizeof(unsigned int)) != cudaSuccess) {
-      cudaFree(ctx->sk_partial); cudaFree(ctx->sk_flags); cudaFree(ctx->attn_sched); cudaFree(ctx->rope); delete ctx;
+      cudaFree(ctx->sk_partial); cudaFree(ctx->sk_flags); cudaFree(ctx->attn_sched); cudaFree(ctx->opt_partial); cudaFree(ctx->rope); delete ctx;
       return LSP_ENOMEM;
     }
   }
@@ -578,6 +581,7 @@ lsp_status lsp_destroy(lsp_ctx* ctx) {
   cudaFree(ctx->sk_partial);
   cudaFree(ctx->sk_flags);
   cudaFree(ctx->attn_sched);
+  cudaFree(ctx->opt_partial);
   if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
   if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
   for (int i = 0; i < 6; ++i)
@@ -775,6 +779,51 @@ lsp_status lsp_layer_step_host(lsp_ctx* ctx, const void* x_host, const void* dy_
   LSP_CUDA(cudaEventRecord(ev[5], ctx->s_out));
   LSP_CUDA(cudaStreamWaitEvent(st, ev[5], 0));
   return LSP_OK;
+}
+
+lsp_status lsp_adamw_step(lsp_ctx* ctx, int ntensors, const lsp_adamw_tensor* tensors, const lsp_adamw_desc* desc,
+                          float* gnorm_out, void* stream) {
+  if (!ctx || !tensors || !desc || !gnorm_out) return LSP_EINVAL;
+  if (ntensors < 1 || ntensors > OPT_MAX_TENSORS) return fail(ctx, LSP_EINVAL, "lsp_adamw_step: 1 <= ntensors <= %d", OPT_MAX_TENSORS);
+  if (desc->step < 1 || !(desc->beta1 >= 0.f && desc->beta1 < 1.f) || !(desc->beta2 >= 0.f && desc->beta2 < 1.f) || !(desc->clip_norm > 0.f))
+    return fail(ctx, LSP_EINVAL, "lsp_adamw_step: bad hyper-parameters");
+  OptTensors t;
+  memset(&t, 0, sizeof(t));
+  t.n = ntensors;
+  for (int i = 0; i < ntensors; ++i) {
+    const lsp_adamw_tensor& x = tensors[i];
+    if (!x.grad || !x.master || !x.m || !x.v || x.n <= 0 || (x.n % 4)) return fail(ctx, LSP_EINVAL, "lsp_adamw_step: tensor %d: NULL pointer or n %% 4 != 0", i);
+    if (!aligned(x.grad, 16) || !aligned(x.master, 16) || !aligned(x.m, 16) || !aligned(x.v, 16) || (x.weight_bf16 && !aligned(x.weight_bf16, 8)))
+      return fail(ctx, LSP_EALIGN, "lsp_adamw_step: tensor %d is not 16-byte aligned", i);
+    t.g[i] = static_cast<const float*>(x.grad); t.p[i] = x.master; t.m[i] = x.m; t.v[i] = x.v;
+    t.w[i] = static_cast<__nv_bfloat16*>(x.weight_bf16);
+    t.start[i + 1] = t.start[i] + x.n / 4;
+    if (x.decay) t.decay_mask |= 1u << i;
+  }
+  for (int i = ntensors; i < OPT_MAX_TENSORS; ++i) t.start[i + 1] = t.start[ntensors];
+  OptHyper h;
+  h.lr = desc->lr; h.beta1 = desc->beta1; h.beta2 = desc->beta2; h.eps = desc->eps; h.weight_decay = desc->weight_decay;
+  h.inv_bc1 = static_cast<float>(1.0 / (1.0 - pow(static_cast<double>(desc->beta1), desc->step)));
+  h.inv_bc2 = static_cast<float>(1.0 / (1.0 - pow(static_cast<double>(desc->beta2), desc->step)));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  long long blocks = (t.start[ntensors] + OPT_THREADS - 1) / OPT_THREADS;
+  const long long cap = ctx->num_sms * 8LL < 4096 ? ctx->num_sms * 8LL : 4096;
+  if (blocks > cap) blocks = cap;
+  const int nb = static_cast<int>(blocks);
+  auto launch = [&]() {
+    opt_gradsq_kernel<<<nb, OPT_THREADS, 0, st>>>(t, ctx->opt_partial);
+    opt_norm_final_kernel<<<1, 32, 0, st>>>(ctx->opt_partial, nb, desc->clip_norm, gnorm_out);
+    opt_adamw_kernel<<<nb, OPT_THREADS, 0, st>>>(t, h, gnorm_out);
+    return cudaGetLastError();
+  };
+  LSP_STAGE(ST_ADAMW, 3, launch());
+  return LSP_OK;
+}
+
+double lsp_lr_cosine(int step, double lr_max, double lr_min, int warmup, int total) {
+  if (warmup > 0 && step <= warmup) return lr_max * step / warmup;
+  if (step >= total) return lr_min;
+  return lr_min + 0.5 * (lr_max - lr_min) * (1.0 + cos(3.14159265358979323846 * (step - warmup) / (total - warmup)));
 }
 
 long long lsp_launch_count(const lsp_ctx* ctx) { return ctx ? ctx->launches : -1; }

@@ -1,0 +1,98 @@
+// Optimizer step after the layer backward (Table 2): AdamW [40] with
+// global-norm gradient clipping, fp32 master weights and moments, bf16 model weights (BF16 mixed precision).
+// HBM-bound multi-tensor kernels: the squared-norm pass reads 4 B per parameter, the update reads 16 B and writes
+// 14 B per parameter (g, p, m, v in; p, m, v, bf16 w out).  The clip coefficient stays on the device (no host sync);
+// all reductions run in a fixed order (bit-reproducible).
+#pragma once
+#include "ptx.cuh"
+
+namespace lsp {
+
+constexpr int OPT_MAX_TENSORS = 16;
+constexpr int OPT_THREADS = 256;
+
+struct OptTensors {
+  const float* g[OPT_MAX_TENSORS];
+  float* p[OPT_MAX_TENSORS];
+  float* m[OPT_MAX_TENSORS];
+  float* v[OPT_MAX_TENSORS];
+  __nv_bfloat16* w[OPT_MAX_TENSORS];
+  long long start[OPT_MAX_TENSORS + 1];      // prefix sums of the tensor sizes in float4 units
+  unsigned int decay_mask;                   // bit i: weight decay applies to tensor i
+  int n;
+};
+struct OptHyper {
+  float lr, beta1, beta2, eps, weight_decay;
+  float inv_bc1, inv_bc2;                    // 1 / (1 - beta^t), evaluated in fp64 on the host
+};
+
+__device__ __forceinline__ int opt_segment(const OptTensors& t, long long i) {
+  int s = 0;
+#pragma unroll
+  for (int k = 1; k < OPT_MAX_TENSORS; ++k) s += (k < t.n && i >= t.start[k]) ? 1 : 0;
+  return s;
+}
+
+// partial[block] = sum of g^2 over the float4 units this block visits (grid-stride: a fixed assignment)
+__global__ void __launch_bounds__(OPT_THREADS) opt_gradsq_kernel(const OptTensors t, float* __restrict__ partial) {
+  __shared__ float red[OPT_THREADS / 32];
+  const long long total = t.start[t.n];
+  float acc = 0.f;
+  for (long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i < total; i += static_cast<long long>(gridDim.x) * blockDim.x) {
+    const int s = opt_segment(t, i);
+    const float4 g = __ldg(reinterpret_cast<const float4*>(t.g[s]) + (i - t.start[s]));
+    acc += g.x * g.x + g.y * g.y + g.z * g.z + g.w * g.w;
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    float b = 0.f;
+#pragma unroll
+    for (int k = 0; k < OPT_THREADS / 32; ++k) b += red[k];
+    partial[blockIdx.x] = b;
+  }
+}
+
+// out[0] = global l2 norm, out[1] = min(1, clip / (norm + 1e-6)); one thread, fixed order, fp64 accumulation
+__global__ void opt_norm_final_kernel(const float* __restrict__ partial, int nparts, float clip, float* __restrict__ out) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) {
+    double s = 0.0;
+    for (int i = 0; i < nparts; ++i) s += static_cast<double>(partial[i]);
+    const double norm = sqrt(s);
+    out[0] = static_cast<float>(norm);
+    const double c = static_cast<double>(clip) / (norm + 1e-6);
+    out[1] = static_cast<float>(c < 1.0 ? c : 1.0);
+  }
+}
+
+// m <- b1 m + (1 - b1) g ; v <- b2 v + (1 - b2) g^2 ; p <- p - lr (m_hat / (sqrt(v_hat) + eps) + wd p) ; w = bf16(p)
+__global__ void __launch_bounds__(OPT_THREADS) opt_adamw_kernel(const OptTensors t, const OptHyper h, const float* __restrict__ norm_coef) {
+  const long long total = t.start[t.n];
+  const float c = norm_coef[1];
+  for (long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i < total; i += static_cast<long long>(gridDim.x) * blockDim.x) {
+    const int s = opt_segment(t, i);
+    const long long j = i - t.start[s];
+    const float4 g4 = __ldg(reinterpret_cast<const float4*>(t.g[s]) + j);
+    float4 p4 = reinterpret_cast<float4*>(t.p[s])[j];
+    float4 m4 = reinterpret_cast<float4*>(t.m[s])[j];
+    float4 v4 = reinterpret_cast<float4*>(t.v[s])[j];
+    const float wd = ((t.decay_mask >> s) & 1u) ? h.weight_decay : 0.f;
+    const float g[4] = {g4.x * c, g4.y * c, g4.z * c, g4.w * c};
+    float p[4] = {p4.x, p4.y, p4.z, p4.w}, m[4] = {m4.x, m4.y, m4.z, m4.w}, v[4] = {v4.x, v4.y, v4.z, v4.w};
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      m[e] = h.beta1 * m[e] + (1.0f - h.beta1) * g[e];
+      v[e] = h.beta2 * v[e] + (1.0f - h.beta2) * g[e] * g[e];
+      const float m_hat = m[e] * h.inv_bc1, v_hat = v[e] * h.inv_bc2;
+      p[e] = p[e] - h.lr * (m_hat / (sqrtf(v_hat) + h.eps) + wd * p[e]);
+    }
+    reinterpret_cast<float4*>(t.p[s])[j] = make_float4(p[0], p[1], p[2], p[3]);
+    reinterpret_cast<float4*>(t.m[s])[j] = make_float4(m[0], m[1], m[2], m[3]);
+    reinterpret_cast<float4*>(t.v[s])[j] = make_float4(v[0], v[1], v[2], v[3]);
+    if (t.w[s]) reinterpret_cast<uint2*>(t.w[s])[j] = make_uint2(pack_bf16(p[0], p[1]), pack_bf16(p[2], p[3]));
+  }
+}
+
+}  // namespace lsp

@@ -58,3 +58,12 @@ def test_sass_is_blackwell_native(libpath):
         pytest.skip("cuobjdump not available")
     sass = subprocess.run([cuobjdump, "-sass", libpath], capture_output=True, text=True).stdout
     assert re.search(r"UTC[A-Z]*MMA", sass) and "LDTM" in sass and "UTMALDG" in sass
+
+
+def test_lr_cosine_host_helper_matches_oracle(libpath):
+    """lsp_lr_cosine is host-only arithmetic (PAPER.md:77 schedule, reading O-3): identical to the oracle's schedule."""
+    from oracle import adamw_ref as A
+    from paper_2510_02483_b200 import binding
+    for total in (5000, 100000):
+        for step in (1, 2, 999, 2000, 2001, 2500, total // 2, total - 1, total, total + 7):
+            assert binding.lsp_lr_cosine(step, 1.2e-3, 1.0e-5, 2000, total) == pytest.approx(A.lr_cosine(step, total=total), rel=1e-14)

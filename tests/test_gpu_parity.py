@@ -330,3 +330,55 @@ def test_sdpa_cfg5_lengths(gpu, S):
     (3 q heads / 1 kv head, batch 1): every element of O, L, dq, dk, dv.  The full 24/8-head, 32768-token launch is
     the same kernel over more (batch, kv-head) CTAs; its throughput is reported by profiles/."""
     test_sdpa_fwd_bwd(gpu, 1, S, 3, 1, 128)
+
+
+# ------------------------------------------------------------------------------------------- optimizer step (NEXT #2)
+def test_adamw_step_vs_oracle(gpu):
+    """lsp_adamw_step (global-norm clip + AdamW on fp32 master weights, bf16 weights out) against oracle/adamw_ref.py over
+    four steps, gradients alternately above and below the clipping threshold; ragged tensor sizes (multiples of 4).
+    Every step starts the oracle from the GPU's own fp32 state (p, m, v are exactly representable), so each comparison
+    is one step of fp32 arithmetic against fp64.  Bars: global norm 1e-6 relative; m, v and the weight UPDATE
+    (p_new - p_old: one fp32 rounding of p, 2^-24 |p| ~ 3e-9, against an update of rms ~ lr) 2e-5 normalised; the bf16
+    weight must be the round-to-nearest-even of the GPU's master weight and within half a bf16 ulp of the oracle's."""
+    import torch
+    from oracle import adamw_ref as A
+    from paper_2510_02483_b200 import binding as B
+    shapes = [(1000, 64), (512,), (36, 100), (4,), (300, 300)]
+    decay = [True, False, True, False, True]
+    rng = np.random.default_rng([2510, 2483, 77])
+    p = [rng.standard_normal(s) * 0.02 for s in shapes]
+    p = [x.astype(np.float32).astype(np.float64) for x in p]
+    m = [np.zeros(s) for s in shapes]; v = [np.zeros(s) for s in shapes]
+    dev = torch.device("cuda")
+    ctx = gpu.make_ctx(synth.CFG1_TINY)
+    tp = [torch.tensor(x, dtype=torch.float32, device=dev) for x in p]
+    tm = [torch.zeros(s, dtype=torch.float32, device=dev) for s in shapes]
+    tv = [torch.zeros(s, dtype=torch.float32, device=dev) for s in shapes]
+    tw = [torch.empty(s, dtype=torch.bfloat16, device=dev) for s in shapes]
+    gn = torch.zeros(2, dtype=torch.float32, device=dev)
+    for step in range(1, 5):
+        scale = 0.5 if step % 2 else 1e-3
+        g = [(rng.standard_normal(s) * scale).astype(np.float32).astype(np.float64) for s in shapes]
+        tg = [torch.tensor(x, dtype=torch.float32, device=dev) for x in g]
+        lr = A.lr_cosine(step * 600, total=4000)
+        tensors = [dict(grad=a, master=b, m=c, v=d, weight=e, decay=f) for a, b, c, d, e, f in zip(tg, tp, tm, tv, tw, decay)]
+        B.lsp_adamw_step(ctx, tensors, lr=lr, step=step, gnorm_out=gn)
+        torch.cuda.synchronize()
+        p_old = p
+        p, m, v, norm = A.adamw_step(p, g, m, v, decay, step, lr)
+        ref_p, ref_m, ref_v = p, m, v
+        got_n, got_c = [float(x) for x in gn.cpu().numpy()]
+        assert abs(got_n - norm) <= 1e-6 * norm and abs(got_c - A.clip_coefficient(norm)) <= 2e-6
+        for i in range(len(shapes)):
+            gp = tp[i].cpu().numpy().astype(np.float64)
+            assert norm_err(tm[i].cpu().numpy(), m[i]) < 2e-5 and norm_err(tv[i].cpu().numpy(), v[i]) < 2e-5, (step, i)
+            assert norm_err(gp - p_old[i], p[i] - p_old[i]) < 2e-5, (step, i)
+            w = tw[i].float().cpu().numpy().astype(np.float64)
+            # half a bf16 ulp of the oracle's weight plus fp32 round-off of the master weight
+            assert np.all(np.abs(w - p[i]) <= np.abs(p[i]) * 2.0 ** -8 * 1.001 + 1e-9), (step, i)
+            assert np.array_equal(w, A.bf16_rne(gp)), (step, i)           # exactly the rounding of the GPU's own master weight
+        # next step: the oracle continues from the GPU's state
+        p = [t.cpu().numpy().astype(np.float64) for t in tp]
+        m = [t.cpu().numpy().astype(np.float64) for t in tm]
+        v = [t.cpu().numpy().astype(np.float64) for t in tv]
+    ctx.close()
