@@ -134,6 +134,21 @@ lsp_status lsp_layer_step_host(lsp_ctx* ctx, const void* x_host, const void* dy_
                                void* y_host, void* dx_host, lsp_layer_wgrads* grads, void* x_dev, void* dy_dev,
                                void* y_dev, void* dx_dev, void* saved, void* ws, void* stream);
 
+/* Model head (readings H-1 .. H-3 in DESIGN.md section 13): final RMSNorm (gain g_final, the
+ * context's rms_eps), bias-free LM head w_head bf16 [vocab, H] ([out,in]), mean next-token cross-entropy, and all their
+ * gradients, in one call:  xn = RMSNorm(x; g_final); z = xn w_head^T; loss = mean_t (lse_t - z[t, targets[t]]).
+ *   x [T,H] in_dtype (the stack output), targets int32 [T] in [0, vocab), vocab % 8 == 0.
+ *   Outputs: loss DEVICE float[1]; lse fp32 [T] (natural log-sum-exp of the logits); dx fp32 [T,H]; dg_final fp32 [H];
+ *   dw_head fp32 [vocab, H].  ws: lsp_head_workspace_bytes(ctx, vocab) bytes of scratch (256-byte aligned); it holds the
+ *   fp32 logits [T, vocab] and their fp16 gradient -- 6 bytes per (token, class). */
+size_t lsp_head_workspace_bytes(const lsp_ctx* ctx, int32_t vocab);
+lsp_status lsp_head_fwd_bwd(lsp_ctx* ctx, const void* x, const void* g_final, const void* w_head, const int32_t* targets,
+                            int32_t vocab, float* loss, float* lse, void* dx, float* dg_final, float* dw_head, void* ws,
+                            void* stream);
+/* Embedding backward (H-3): d_table [vocab, H] fp32 (fully written: zero for ids that do not occur) =
+ * scatter-add of dx0 fp32 [T,H] by ids int32 [T]; duplicates are added in increasing token order (bit-reproducible). */
+lsp_status lsp_embed_bwd(lsp_ctx* ctx, const int32_t* ids, const void* dx0, int32_t vocab, float* d_table, void* stream);
+
 /* Optimizer step after the backward (Table 2): AdamW with decoupled weight decay
  * and bias-corrected moments (ref [40]), preceded by clipping of the GLOBAL l2 gradient norm over all tensors of the
  * call (readings O-1 .. O-5 in DESIGN.md section 12).  Per tensor i of `n` elements (n % 4 == 0, pointers 16-byte

@@ -18,7 +18,8 @@ WEIGHT_FIELDS = ("wq", "wk", "wv", "wo", "g_attn", "w_gate", "w_up", "w_down", "
 EXPORTS = ("lsp_create", "lsp_destroy", "lsp_saved_bytes", "lsp_workspace_bytes", "lsp_last_error",
            "lsp_attn_fwd", "lsp_attn_bwd", "lsp_mlp_fwd", "lsp_mlp_bwd", "lsp_layer_fwd", "lsp_layer_bwd",
            "lsp_sdpa_fwd", "lsp_sdpa_bwd", "lsp_embed_fwd", "lsp_gemm", "lsp_layer_step_host", "lsp_launch_count",
-           "lsp_timing_enable", "lsp_timing_read", "lsp_adamw_step", "lsp_lr_cosine")
+           "lsp_timing_enable", "lsp_timing_read", "lsp_adamw_step", "lsp_lr_cosine", "lsp_head_workspace_bytes",
+           "lsp_head_fwd_bwd", "lsp_embed_bwd")
 
 
 class LspError(RuntimeError):
@@ -84,8 +85,13 @@ def lib():
         L.lsp_adamw_step.argtypes = [vp, i32, C.POINTER(lsp_adamw_tensor), C.POINTER(lsp_adamw_desc), vp, vp]
         L.lsp_lr_cosine.argtypes = [i32, C.c_double, C.c_double, i32, i32]
         L.lsp_lr_cosine.restype = C.c_double
+        L.lsp_head_workspace_bytes.argtypes = [vp, i32]
+        L.lsp_head_workspace_bytes.restype = C.c_size_t
+        L.lsp_head_fwd_bwd.argtypes = [vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp]
+        L.lsp_embed_bwd.argtypes = [vp, vp, vp, i32, vp, vp]
         for n in EXPORTS:
-            if n not in ("lsp_saved_bytes", "lsp_workspace_bytes", "lsp_last_error", "lsp_launch_count", "lsp_lr_cosine"):
+            if n not in ("lsp_saved_bytes", "lsp_workspace_bytes", "lsp_last_error", "lsp_launch_count", "lsp_lr_cosine",
+                         "lsp_head_workspace_bytes"):
                 getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -220,6 +226,19 @@ def lsp_adamw_step(ctx, tensors, *, lr, step, gnorm_out, beta1=0.90, beta2=0.95,
 
 def lsp_lr_cosine(step: int, lr_max: float = 1.2e-3, lr_min: float = 1.0e-5, warmup: int = 2000, total: int = 100000) -> float:
     return float(lib().lsp_lr_cosine(step, lr_max, lr_min, warmup, total))
+
+
+def lsp_head_workspace_bytes(ctx, vocab: int) -> int:
+    return int(lib().lsp_head_workspace_bytes(ctx.handle, vocab))
+
+
+def lsp_head_fwd_bwd(ctx, x, g_final, w_head, targets, vocab, loss, lse, dx, dg_final, dw_head, ws, stream=None):
+    ctx.check(lib().lsp_head_fwd_bwd(ctx.handle, _ptr(x), _ptr(g_final), _ptr(w_head), _ptr(targets), vocab, _ptr(loss), _ptr(lse),
+                                     _ptr(dx), _ptr(dg_final), _ptr(dw_head), _ptr(ws), _stream(stream)))
+
+
+def lsp_embed_bwd(ctx, ids, dx0, vocab, d_table, stream=None):
+    ctx.check(lib().lsp_embed_bwd(ctx.handle, _ptr(ids), _ptr(dx0), vocab, _ptr(d_table), _stream(stream)))
 
 
 def lsp_launch_count(ctx) -> int:

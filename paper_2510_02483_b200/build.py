@@ -14,7 +14,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "liblsp.so")
 SOURCES = [os.path.join(CSRC, "liblsp.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("ptx.cuh", "gemm.cuh", "attn.cuh", "norm.cuh", "attn_tc.cuh", "optim.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("ptx.cuh", "gemm.cuh", "attn.cuh", "norm.cuh", "attn_tc.cuh", "optim.cuh", "head.cuh")] + [
     os.path.join(os.path.dirname(PKG), "include", "lsp.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-shared",
               "-Xcompiler", "-fPIC"]

@@ -16,6 +16,7 @@
 #include "gemm.cuh"
 #include "norm.cuh"
 #include "optim.cuh"
+#include "head.cuh"
 
 using namespace lsp;
 
@@ -40,12 +41,12 @@ struct WsLayout {
 enum Stage : int {
   ST_CAST = 0, ST_NORM_FWD, ST_QKV, ST_ATTN_FWD, ST_OPROJ, ST_GATEUP, ST_DOWN,
   ST_WGRAD_DOWN, ST_DGRAD_DOWN, ST_WGRAD_GATEUP, ST_DGRAD_GATEUP, ST_NORM_BWD,
-  ST_WGRAD_O, ST_DGRAD_O, ST_DVEC, ST_ATTN_BWD, ST_WGRAD_QKV, ST_DGRAD_QKV, ST_EMBED, ST_ATTN_BWD_DQ, ST_ADAMW, ST_COUNT
+  ST_WGRAD_O, ST_DGRAD_O, ST_DVEC, ST_ATTN_BWD, ST_WGRAD_QKV, ST_DGRAD_QKV, ST_EMBED, ST_ATTN_BWD_DQ, ST_ADAMW, ST_HEAD_GEMM, ST_CE, ST_EMBED_BWD, ST_COUNT
 };
 static const char* const STAGE_NAMES[ST_COUNT] = {
   "cast", "rmsnorm_fwd", "gemm_qkv_rope", "attn_fwd", "gemm_oproj_res", "gemm_gateup_swiglu", "gemm_down_res",
   "wgrad_down", "dgrad_down_swiglu_bwd", "wgrad_gateup", "dgrad_gateup", "rmsnorm_bwd",
-  "wgrad_oproj", "dgrad_oproj", "attn_dvec", "attn_bwd", "wgrad_qkv", "dgrad_qkv", "embed_gather", "attn_bwd_dq", "adamw"};
+  "wgrad_oproj", "dgrad_oproj", "attn_dvec", "attn_bwd", "wgrad_qkv", "dgrad_qkv", "embed_gather", "attn_bwd_dq", "adamw", "head_gemm", "cross_entropy", "embed_bwd"};
 
 struct TimingRec { int stage; cudaEvent_t beg, end; };
 
@@ -182,7 +183,7 @@ cudaError_t norm_bwd_t(const lsp_ctx* c, const void* x, const float* rstd, const
   const RT* rp = static_cast<const RT*>(dres);
   const __nv_bfloat16* gp = static_cast<const __nv_bfloat16*>(g);
   const int nb = c->norm_blocks < c->T ? c->norm_blocks : c->T;
-  const size_t stage_bytes = static_cast<size_t>(H) * (sizeof(XT) + 4 + sizeof(RT));
+  const size_t stage_bytes = static_cast<size_t>(H) * (sizeof(XT) + 4 + (dres ? sizeof(RT) : 0));
   int stages = static_cast<int>(NORMB_SMEM_BUDGET / stage_bytes);
   if (stages > NORMB_MAX_STAGES) stages = NORMB_MAX_STAGES;
   if (stages < 2) return cudaErrorInvalidValue;
@@ -778,6 +779,95 @@ lsp_status lsp_layer_step_host(lsp_ctx* ctx, const void* x_host, const void* dy_
   LSP_CUDA(cudaMemcpyAsync(dx_host, dx_dev, n * 4, cudaMemcpyDeviceToHost, ctx->s_out));
   LSP_CUDA(cudaEventRecord(ev[5], ctx->s_out));
   LSP_CUDA(cudaStreamWaitEvent(st, ev[5], 0));
+  return LSP_OK;
+}
+
+namespace {
+struct HeadLayout { size_t xn16, rstd, w16, logits, dz16, dxn32, loss_row, dgpart, total; };
+HeadLayout head_layout(const lsp_ctx* c, int vocab) {
+  const size_t T = c->T, H = c->d.hidden, V = vocab;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t r = o; o += align_up(bytes); return r; };
+  HeadLayout h;
+  h.xn16 = take(T * H * 2); h.rstd = take(T * 4); h.w16 = take(V * H * 2); h.logits = take(T * V * 4);
+  h.dz16 = take(T * V * 2); h.dxn32 = take(T * H * 4); h.loss_row = take(T * 4);
+  h.dgpart = take(static_cast<size_t>(c->norm_blocks) * H * 4);
+  h.total = o;
+  return h;
+}
+}  // namespace
+
+size_t lsp_head_workspace_bytes(const lsp_ctx* ctx, int32_t vocab) { return (ctx && vocab > 0) ? head_layout(ctx, vocab).total : 0; }
+
+lsp_status lsp_head_fwd_bwd(lsp_ctx* ctx, const void* x, const void* g_final, const void* w_head, const int32_t* targets,
+                            int32_t vocab, float* loss, float* lse, void* dx, float* dg_final, float* dw_head, void* ws,
+                            void* stream) {
+  if (!ctx) return LSP_EINVAL;
+  const void* ptrs[] = {x, g_final, w_head, targets, loss, lse, dx, dg_final, dw_head, ws};
+  LSP_TRY(check_common(ctx, nullptr, ws, 10, ptrs));
+  if (vocab <= 0 || vocab % 8) return fail(ctx, LSP_EINVAL, "lsp_head_fwd_bwd: vocab must be a positive multiple of 8");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int T = ctx->T, H = ctx->d.hidden, V = vocab;
+  const HeadLayout L = head_layout(ctx, V);
+  __half* xn16 = at<__half>(ws, L.xn16);
+  float* rstd = at<float>(ws, L.rstd);
+  __half* w16 = at<__half>(ws, L.w16);
+  float* logits = at<float>(ws, L.logits);
+  __half* dz16 = at<__half>(ws, L.dz16);
+  float* dxn32 = at<float>(ws, L.dxn32);
+  float* loss_row = at<float>(ws, L.loss_row);
+  float* dgpart = at<float>(ws, L.dgpart);
+  // final RMSNorm, fp16 copy of the head weights
+  LSP_STAGE(ST_NORM_FWD, 1, norm_fwd(ctx, ctx->d.in_dtype, x, g_final, xn16, rstd, st));
+  {
+    const void* src[1] = {w_head};
+    __half* dst[1] = {w16};
+    const long long cnt[1] = {static_cast<long long>(V) * H};
+    LSP_STAGE(ST_CAST, 1, cast_weights(ctx, 1, src, dst, cnt, st));
+  }
+  // logits = xn W_head^T (fp32 out)
+  LSP_STAGE(ST_HEAD_GEMM, 1, (gemm1<false, false>(ctx, T, V, H, Operand{xn16, H, false}, Operand{w16, H, false}, epi_f32(logits, V), st)));
+  // cross-entropy: lse, per-token loss, dz = (softmax - onehot) * 2^12 in fp16
+  {
+    int blocks = ctx->num_sms < T ? ctx->num_sms : T;
+    auto launch = [&]() {
+      ce_fwd_bwd_kernel<<<blocks, CE_THREADS, 0, st>>>(logits, targets, T, V, lse, loss_row, dz16);
+      ce_loss_mean_kernel<<<1, 32, 0, st>>>(loss_row, T, loss);
+      return cudaGetLastError();
+    };
+    LSP_STAGE(ST_CE, 2, launch());
+  }
+  const float alpha = 1.0f / (CE_DZ_SCALE * static_cast<float>(T));      // undo the fp16 scaling, apply the 1/T of the mean
+  // dW_head = dz^T xn ; dxn = dz W_head
+  {
+    EpiF32 e = epi_f32(dw_head, H);
+    e.alpha = alpha;
+    LSP_STAGE(ST_HEAD_GEMM, 1, (gemm1<true, true>(ctx, V, H, T, Operand{dz16, V, true}, Operand{xn16, H, true}, e, st)));
+  }
+  {
+    EpiF32 e = epi_f32(dxn32, H);
+    e.alpha = alpha;
+    LSP_STAGE(ST_HEAD_GEMM, 1, (gemm1<false, true>(ctx, T, H, V, Operand{dz16, V, false}, Operand{w16, H, true}, e, st)));
+  }
+  // final RMSNorm backward (no residual gradient)
+  LSP_STAGE(ST_NORM_BWD, 2, norm_bwd(ctx, ctx->d.in_dtype, LSP_F32, x, rstd, g_final, dxn32, nullptr, static_cast<float*>(dx), nullptr,
+                                      dgpart, dg_final, st));
+  return LSP_OK;
+}
+
+lsp_status lsp_embed_bwd(lsp_ctx* ctx, const int32_t* ids, const void* dx0, int32_t vocab, float* d_table, void* stream) {
+  if (!ctx) return LSP_EINVAL;
+  const void* ptrs[] = {ids, dx0, d_table};
+  LSP_TRY(check_common(ctx, nullptr, nullptr, 3, ptrs));
+  if (vocab <= 0) return fail(ctx, LSP_EINVAL, "lsp_embed_bwd: vocab must be positive");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int T = ctx->T, H = ctx->d.hidden;
+  LSP_CUDA(cudaMemsetAsync(d_table, 0, static_cast<size_t>(vocab) * H * sizeof(float), st));
+  auto launch = [&]() {
+    embed_bwd_kernel<<<T, 256, 0, st>>>(ids, static_cast<const float*>(dx0), T, H, d_table);
+    return cudaGetLastError();
+  };
+  LSP_STAGE(ST_EMBED_BWD, 1, launch());
   return LSP_OK;
 }
 

@@ -121,7 +121,9 @@ rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, con
   extern __shared__ __align__(128) uint8_t nsm[];
   __shared__ float red[NORMB_CONSUMERS / 32];
   __shared__ __align__(8) unsigned long long bars[2 * NORMB_MAX_STAGES];
-  const uint32_t xb = static_cast<uint32_t>(H) * sizeof(XT), db = static_cast<uint32_t>(H) * 4u, rb = static_cast<uint32_t>(H) * sizeof(RT);
+  // dres may be null (no residual gradient: the final norm before the LM head)
+  const uint32_t xb = static_cast<uint32_t>(H) * sizeof(XT), db = static_cast<uint32_t>(H) * 4u,
+                 rb = dres ? static_cast<uint32_t>(H) * sizeof(RT) : 0u;
   const uint32_t stage_bytes = xb + db + rb;                 // every part is a multiple of 16 (H % 8 == 0)
   const uint32_t smem0 = smem_u32(nsm);
   auto full = [&](int s) { return smem_u32(&bars[s]); };
@@ -143,7 +145,7 @@ rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, con
         mbar_expect_tx(full(s), stage_bytes);
         bulk_load_1d(dst, x + row * H, xb, full(s));
         bulk_load_1d(dst + xb, dxn + row * H, db, full(s));
-        bulk_load_1d(dst + xb + db, dres + row * H, rb, full(s));
+        if (rb) bulk_load_1d(dst + xb + db, dres + row * H, rb, full(s));
         if (++s == stages) { s = 0; ph ^= 1u; }
       }
     }
@@ -173,7 +175,7 @@ rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, con
       if (c < H) {
         const float4 xv = lds_vec4<XT>(sx, c);
         const float4 d = lds_vec4<float>(sd, c);
-        rs[i] = lds_vec4<RT>(sr, c);
+        rs[i] = rb ? lds_vec4<RT>(sr, c) : make_float4(0.f, 0.f, 0.f, 0.f);
         n[i] = make_float4(xv.x * r, xv.y * r, xv.z * r, xv.w * r);
         acc[i].x += d.x * n[i].x; acc[i].y += d.y * n[i].y; acc[i].z += d.z * n[i].z; acc[i].w += d.w * n[i].w;
         dn[i] = make_float4(d.x * gg[i].x, d.y * gg[i].y, d.z * gg[i].z, d.w * gg[i].w);

@@ -382,3 +382,63 @@ def test_adamw_step_vs_oracle(gpu):
         m = [t.cpu().numpy().astype(np.float64) for t in tm]
         v = [t.cpu().numpy().astype(np.float64) for t in tv]
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------------- model head + embedding backward (NEXT #1)
+@pytest.mark.parametrize("Bz,S,H,V", [(1, 256, 256, 1000), (2, 192, 384, 4104)])
+def test_head_fwd_bwd_vs_oracle(gpu, Bz, S, H, V):
+    """lsp_head_fwd_bwd (final RMSNorm + LM head + mean cross-entropy, all gradients) against oracle/head_ref.py.
+    Bars: loss and lse 1e-4 absolute-relative (fp16 operands, fp32 accumulation over H terms); gradients at the layer's
+    bar, max|gpu - ref| / rms(ref) <= 2e-2."""
+    import torch
+    from oracle import head_ref as Hd
+    from paper_2510_02483_b200 import binding as B
+    w = synth.Workload("head", 7, Bz, S, H, 4, 2, 64, 256, 1e-5, 10000.0)
+    T = w.tokens
+    x_bits = synth.normal_bf16(7, 0, "x", (T, H), 1.0)
+    g_bits = synth.normal_bf16(7, 0, "g_attn", (H,), 0.1, offset=1.0)
+    rng = np.random.default_rng([2510, 2483, 7, V])
+    wh_bits = synth.normal_bf16(7, 0, "embedding", (V, H), 0.02)
+    y = rng.integers(0, V, size=T, dtype=np.int32)
+    ctx = gpu.make_ctx(w)
+    dev = torch.device("cuda")
+    x = gpu.bf16_to_device(x_bits); g = gpu.bf16_to_device(g_bits); wh = gpu.bf16_to_device(wh_bits)
+    ty = torch.from_numpy(y).to(dev)
+    loss = torch.zeros(1, dtype=torch.float32, device=dev); lse = torch.empty(T, dtype=torch.float32, device=dev)
+    dx = torch.empty((T, H), dtype=torch.float32, device=dev); dg = torch.empty(H, dtype=torch.float32, device=dev)
+    dw = torch.empty((V, H), dtype=torch.float32, device=dev)
+    ws = torch.empty(B.lsp_head_workspace_bytes(ctx, V), dtype=torch.uint8, device=dev)
+    B.lsp_head_fwd_bwd(ctx, x, g, wh, ty, V, loss, lse, dx, dg, dw, ws)
+    torch.cuda.synchronize()
+    ref = Hd.head_loss_fwd_bwd(synth.bf16_bits_to_f64(x_bits), synth.bf16_bits_to_f64(g_bits), synth.bf16_bits_to_f64(wh_bits), y, 1e-5)
+    assert abs(float(loss.cpu()) - ref["loss"]) <= 1e-4 * abs(ref["loss"])
+    assert np.max(np.abs(lse.cpu().numpy() - ref["lse"])) <= 1e-4 * np.max(np.abs(ref["lse"]))
+    check(dict(dx=dx.cpu().numpy(), dg_final=dg.cpu().numpy(), dw_head=dw.cpu().numpy()), ref, ["dx", "dg_final", "dw_head"])
+    ctx.close()
+
+
+def test_embed_bwd_vs_oracle(gpu):
+    """lsp_embed_bwd: deterministic scatter-add with many duplicate ids; rows of absent ids are exactly zero; fp32 sums in
+    increasing token order against the fp64 oracle (1e-6 normalised); bit-identical on a second launch."""
+    import torch
+    from oracle import head_ref as Hd
+    from paper_2510_02483_b200 import binding as B
+    w = synth.Workload("embb", 8, 2, 160, 384, 4, 2, 64, 256, 1e-5, 10000.0)
+    T, H, V = w.tokens, w.hidden, 97
+    rng = np.random.default_rng([2510, 2483, 8])
+    ids = rng.integers(0, V, size=T, dtype=np.int32)
+    ids[ids == 5] = 6                                  # id 5 never occurs
+    d = rng.standard_normal((T, H)).astype(np.float32)
+    ctx = gpu.make_ctx(w)
+    dev = torch.device("cuda")
+    tid = torch.from_numpy(ids).to(dev); td = torch.from_numpy(d).to(dev)
+    outs = []
+    for _ in range(2):
+        dE = torch.full((V, H), float("nan"), dtype=torch.float32, device=dev)
+        B.lsp_embed_bwd(ctx, tid, td, V, dE)
+        torch.cuda.synchronize()
+        outs.append(dE.cpu().numpy())
+    ref = Hd.embed_bwd(ids, d.astype(np.float64), V)
+    assert not np.any(outs[0][5]) and np.array_equal(outs[0], outs[1])
+    assert norm_err(outs[0], ref) < 1e-6
+    ctx.close()
