@@ -1,6 +1,6 @@
 """Device-side timing of every BASELINE.json configuration (bench.py covers the headline config 2 only).
 
-    python -m paper_2510_02483_b200.configs_bench [--steps K] [--only cfg2,cfg3,cfg4,cfg5,table1,adamw]
+    python -m paper_2510_02483_b200.configs_bench [--steps K] [--only cfg2,cfg3,cfg4,cfg5,table1,adamw,head]
 
 Prints one JSON line per configuration: ms per fwd+bwd step (CUDA events on the launching stream, after warm-up),
 tokens/s and executed TFLOP/s (causal attention FLOPs, SURVEY.md 8(d) convention).  Inputs are the seeded synthetic
@@ -10,6 +10,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 
 import torch
 
@@ -107,10 +108,32 @@ def bench_adamw(w, steps):
     return ms, nparam
 
 
+def bench_head(w, steps):
+    """Model head of config 3 (lsp_head_fwd_bwd: final RMSNorm + LM head [T,H] x [H,V] + cross-entropy, fwd and bwd) and
+    the embedding backward (lsp_embed_bwd), T = batch * seq tokens, V = the workload's vocabulary."""
+    dev = harness.require_cuda()
+    ctx = harness.make_ctx(w, in_dtype=B.LSP_F32)
+    T, H, V = w.tokens, w.hidden, w.vocab
+    s = synth.stack_inputs(w)
+    ids = torch.from_numpy(s["ids"]).to(dev)
+    x = torch.randn((T, H), dtype=torch.float32, device=dev)
+    g = torch.ones(H, dtype=torch.bfloat16, device=dev)
+    wh = harness.bf16_to_device(s["embedding"], dev)            # an untied head of the embedding's shape and distribution
+    loss = torch.zeros(1, dtype=torch.float32, device=dev); lse = torch.empty(T, dtype=torch.float32, device=dev)
+    dx = torch.empty((T, H), dtype=torch.float32, device=dev); dg = torch.empty(H, dtype=torch.float32, device=dev)
+    dw = torch.empty((V, H), dtype=torch.float32, device=dev)
+    ws = torch.empty(B.lsp_head_workspace_bytes(ctx, V), dtype=torch.uint8, device=dev)
+    ms_head = _time(lambda: B.lsp_head_fwd_bwd(ctx, x, g, wh, ids, V, loss, lse, dx, dg, dw, ws), steps)
+    ms_emb = _time(lambda: B.lsp_embed_bwd(ctx, ids, dx, V, dw), steps)
+    out = dict(ms_head=ms_head, ms_embed_bwd=ms_emb, loss=float(loss.cpu()), flops=3 * 2.0 * T * V * H)
+    ctx.close()
+    return out
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--only", default="cfg2,cfg3,cfg4,cfg5,table1,adamw")
+    ap.add_argument("--only", default="cfg2,cfg3,cfg4,cfg5,table1,adamw,head")
     args = ap.parse_args(argv)
     B.lib()
     only = set(args.only.split(","))
@@ -131,6 +154,13 @@ def main(argv=None):
             print(json.dumps({"config": "adamw_" + w.name, "params": nparam, "ms_per_step": round(ms, 4),
                               "algorithmic_GB_per_s": round(34.0 * nparam / (ms * 1e-3) / 1e9, 1)}), flush=True)
             torch.cuda.empty_cache()
+    if "head" in only:
+        w = synth.CFG3_3B_STACK
+        r = bench_head(w, min(args.steps, 5))
+        print(json.dumps({"config": "head_" + w.name, "tokens": w.tokens, "vocab": w.vocab, "ms_head_fwd_bwd": round(r["ms_head"], 4),
+                          "gemm_tflops": round(r["flops"] / (r["ms_head"] * 1e-3) / 1e12, 1), "loss": round(r["loss"], 4),
+                          "ln_vocab": round(math.log(w.vocab), 4), "ms_embed_bwd": round(r["ms_embed_bwd"], 4)}), flush=True)
+        torch.cuda.empty_cache()
     for w, fn in jobs:
         ms, flops = fn(w, max(2, args.steps if fn is not bench_stack else min(args.steps, 3)))
         print(json.dumps({"config": w.name, "batch": w.batch, "seq": w.seq, "tokens": w.tokens, "ms_per_step": round(ms, 4),

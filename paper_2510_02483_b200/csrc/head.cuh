@@ -76,7 +76,7 @@ __global__ void ce_loss_mean_kernel(const float* __restrict__ loss_row, int T, f
 // have been zeroed (rows of ids that never occur).  O(T^2 / 256) id comparisons per launch: 0.26 M at T = 8192.
 __global__ void __launch_bounds__(256) embed_bwd_kernel(const int* __restrict__ ids, const float* __restrict__ dx0, int T, int H,
                                                         float* __restrict__ dE) {
-  __shared__ int hit[256];
+  __shared__ unsigned int hits[8];                    // per warp: ballot of the candidates whose id matches
   __shared__ int any_before;
   const int t = blockIdx.x;
   const int id = ids[t];
@@ -93,11 +93,15 @@ __global__ void __launch_bounds__(256) embed_bwd_kernel(const int* __restrict__ 
   for (int k = 0; k < 32; ++k) acc[k] = 0.f;
   for (int base = t; base < T; base += 256) {
     const int u = base + threadIdx.x;
-    hit[threadIdx.x] = (u < T && ids[u] == id) ? 1 : 0;
+    const unsigned int b = __ballot_sync(0xffffffffu, u < T && ids[u] == id);
+    if ((threadIdx.x & 31) == 0) hits[threadIdx.x >> 5] = b;
     __syncthreads();
-    for (int j = 0; j < 256; ++j) {
-      if (hit[j]) {
-        const float* src = dx0 + static_cast<long long>(base + j) * H;
+    for (int w = 0; w < 8; ++w) {                     // increasing token order: warp 0's lanes first, bit 0 first
+      unsigned int mask = hits[w];
+      while (mask) {
+        const int j = __ffs(mask) - 1;
+        mask &= mask - 1;
+        const float* src = dx0 + static_cast<long long>(base + 32 * w + j) * H;
 #pragma unroll
         for (int k = 0; k < 32; ++k) {
           const int c = threadIdx.x + k * 256;
