@@ -140,11 +140,14 @@ lsp_status lsp_layer_step_host(lsp_ctx* ctx, const void* x_host, const void* dy_
  *   x [T,H] in_dtype (the stack output), targets int32 [T] in [0, vocab), vocab % 8 == 0.
  *   Outputs: loss DEVICE float[1]; lse fp32 [T] (natural log-sum-exp of the logits); dx fp32 [T,H]; dg_final fp32 [H];
  *   dw_head fp32 [vocab, H].  ws: lsp_head_workspace_bytes(ctx, vocab) bytes of scratch (256-byte aligned); it holds the
- *   fp32 logits [T, vocab] and their fp16 gradient -- 6 bytes per (token, class). */
+ *   fp32 logits [T, vocab] and their fp16 gradient -- 6 bytes per (token, class).
+ *   grad_scale > 0 multiplies the three gradients (not the loss): the layers' backward feeds 16-bit tensor-core
+ *   operands, and the gradient of a MEAN loss is ~1/T per element, below the fp16 normal range at training sizes; a
+ *   training step passes e.g. grad_scale = T and hands the same value to lsp_adamw_step, which divides it out. */
 size_t lsp_head_workspace_bytes(const lsp_ctx* ctx, int32_t vocab);
 lsp_status lsp_head_fwd_bwd(lsp_ctx* ctx, const void* x, const void* g_final, const void* w_head, const int32_t* targets,
-                            int32_t vocab, float* loss, float* lse, void* dx, float* dg_final, float* dw_head, void* ws,
-                            void* stream);
+                            int32_t vocab, float grad_scale, float* loss, float* lse, void* dx, float* dg_final,
+                            float* dw_head, void* ws, void* stream);
 /* Embedding backward (H-3): d_table [vocab, H] fp32 (fully written: zero for ids that do not occur) =
  * scatter-add of dx0 fp32 [T,H] by ids int32 [T]; duplicates are added in increasing token order (bit-reproducible). */
 lsp_status lsp_embed_bwd(lsp_ctx* ctx, const int32_t* ids, const void* dx0, int32_t vocab, float* d_table, void* stream);
@@ -154,7 +157,9 @@ lsp_status lsp_embed_bwd(lsp_ctx* ctx, const int32_t* ids, const void* dx0, int3
  * call (readings O-1 .. O-5 in DESIGN.md section 12).  Per tensor i of `n` elements (n % 4 == 0, pointers 16-byte
  * aligned): grad fp32 (read), master / m / v fp32 (updated in place), weight_bf16 (written: round-to-nearest-even of
  * the new master weight; may be NULL), decay = 1 if weight decay applies.  `tensors` is a HOST array of
- * 1 <= ntensors <= 16 entries.  gnorm_out: DEVICE float[2], receives {global norm, clip coefficient} (no host sync).
+ * 1 <= ntensors <= 1024 entries (a whole model: the kernels take them in groups of 16, the norm is over all of them).
+ * gnorm_out: DEVICE float[2], receives {global norm of the true gradients, factor applied to the stored gradients =
+ * clip coefficient / grad_scale} (no host sync).
  * Everything is enqueued on `stream`; results are bit-reproducible. */
 typedef struct {
   const void* grad; float* master; float* m; float* v; void* weight_bf16; int64_t n; int32_t decay;
@@ -162,6 +167,8 @@ typedef struct {
 typedef struct {
   float lr, beta1, beta2, eps, weight_decay, clip_norm;   /* paper: lr from lsp_lr_cosine, 0.90, 0.95, 1e-8, 0.01, 1.0 */
   int32_t step;                                            /* 1-based optimizer step t (bias correction 1 - beta^t) */
+  float grad_scale;                                        /* > 0: the stored gradients are grad_scale x the true ones
+                                                              (lsp_head_fwd_bwd); norm, clipping and update use g / grad_scale */
 } lsp_adamw_desc;
 lsp_status lsp_adamw_step(lsp_ctx* ctx, int ntensors, const lsp_adamw_tensor* tensors, const lsp_adamw_desc* desc,
                           float* gnorm_out, void* stream);

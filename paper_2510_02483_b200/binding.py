@@ -44,7 +44,7 @@ class lsp_adamw_tensor(C.Structure):
 
 class lsp_adamw_desc(C.Structure):
     _fields_ = [("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float),
-                ("weight_decay", C.c_float), ("clip_norm", C.c_float), ("step", C.c_int32)]
+                ("weight_decay", C.c_float), ("clip_norm", C.c_float), ("step", C.c_int32), ("grad_scale", C.c_float)]
 
 
 class lsp_layer_wgrads(C.Structure):
@@ -87,7 +87,7 @@ def lib():
         L.lsp_lr_cosine.restype = C.c_double
         L.lsp_head_workspace_bytes.argtypes = [vp, i32]
         L.lsp_head_workspace_bytes.restype = C.c_size_t
-        L.lsp_head_fwd_bwd.argtypes = [vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp]
+        L.lsp_head_fwd_bwd.argtypes = [vp, vp, vp, vp, vp, i32, C.c_float, vp, vp, vp, vp, vp, vp, vp]
         L.lsp_embed_bwd.argtypes = [vp, vp, vp, i32, vp, vp]
         for n in EXPORTS:
             if n not in ("lsp_saved_bytes", "lsp_workspace_bytes", "lsp_last_error", "lsp_launch_count", "lsp_lr_cosine",
@@ -213,14 +213,14 @@ def lsp_layer_step_host(ctx, x_host, dy_host, weights, y_host, dx_host, grads, x
 
 
 def lsp_adamw_step(ctx, tensors, *, lr, step, gnorm_out, beta1=0.90, beta2=0.95, eps=1e-8, weight_decay=0.01, clip_norm=1.0,
-                   stream=None):
+                   grad_scale=1.0, stream=None):
     """tensors: list of dicts {grad, master, m, v, weight (bf16 or None), decay (bool)} of torch CUDA tensors."""
     arr = (lsp_adamw_tensor * len(tensors))()
     for i, t in enumerate(tensors):
         w = t.get("weight")
         arr[i] = lsp_adamw_tensor(t["grad"].data_ptr(), t["master"].data_ptr(), t["m"].data_ptr(), t["v"].data_ptr(),
                                   None if w is None else w.data_ptr(), t["master"].numel(), 1 if t.get("decay", True) else 0)
-    d = lsp_adamw_desc(lr, beta1, beta2, eps, weight_decay, clip_norm, step)
+    d = lsp_adamw_desc(lr, beta1, beta2, eps, weight_decay, clip_norm, step, grad_scale)
     ctx.check(lib().lsp_adamw_step(ctx.handle, len(tensors), arr, C.byref(d), _ptr(gnorm_out), _stream(stream)))
 
 
@@ -232,8 +232,8 @@ def lsp_head_workspace_bytes(ctx, vocab: int) -> int:
     return int(lib().lsp_head_workspace_bytes(ctx.handle, vocab))
 
 
-def lsp_head_fwd_bwd(ctx, x, g_final, w_head, targets, vocab, loss, lse, dx, dg_final, dw_head, ws, stream=None):
-    ctx.check(lib().lsp_head_fwd_bwd(ctx.handle, _ptr(x), _ptr(g_final), _ptr(w_head), _ptr(targets), vocab, _ptr(loss), _ptr(lse),
+def lsp_head_fwd_bwd(ctx, x, g_final, w_head, targets, vocab, loss, lse, dx, dg_final, dw_head, ws, stream=None, grad_scale=1.0):
+    ctx.check(lib().lsp_head_fwd_bwd(ctx.handle, _ptr(x), _ptr(g_final), _ptr(w_head), _ptr(targets), vocab, grad_scale, _ptr(loss), _ptr(lse),
                                      _ptr(dx), _ptr(dg_final), _ptr(dw_head), _ptr(ws), _stream(stream)))
 
 

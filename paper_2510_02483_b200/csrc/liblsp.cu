@@ -557,7 +557,7 @@ lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device
     if (cudaMalloc(&ctx->sk_partial, pairs * GEMM2_PARTIAL_FLOATS * sizeof(float)) != cudaSuccess ||
         cudaMalloc(&ctx->sk_flags, pairs * 2 * sizeof(unsigned int)) != cudaSuccess ||
         cudaMemset(ctx->sk_flags, 0, pairs * 2 * sizeof(unsigned int)) != cudaSuccess ||
-        cudaMalloc(&ctx->opt_partial, 4096 * sizeof(float)) != cudaSuccess ||
+        cudaMalloc(&ctx->opt_partial, OPT_MAX_CHUNKS * opt_blocks_cap(ctx->num_sms) * sizeof(float)) != cudaSuccess ||
         cudaMalloc(&ctx->attn_sched, 16 * sizeof(unsigned int)) != cudaSuccess ||
         cudaMemset(ctx->attn_sched, 0, 16 * sizeof(unsigned int)) != cudaSuccess) {
       cudaFree(ctx->sk_partial); cudaFree(ctx->sk_flags); cudaFree(ctx->attn_sched); cudaFree(ctx->opt_partial); cudaFree(ctx->rope); delete ctx;
@@ -800,12 +800,13 @@ HeadLayout head_layout(const lsp_ctx* c, int vocab) {
 size_t lsp_head_workspace_bytes(const lsp_ctx* ctx, int32_t vocab) { return (ctx && vocab > 0) ? head_layout(ctx, vocab).total : 0; }
 
 lsp_status lsp_head_fwd_bwd(lsp_ctx* ctx, const void* x, const void* g_final, const void* w_head, const int32_t* targets,
-                            int32_t vocab, float* loss, float* lse, void* dx, float* dg_final, float* dw_head, void* ws,
-                            void* stream) {
+                            int32_t vocab, float grad_scale, float* loss, float* lse, void* dx, float* dg_final, float* dw_head,
+                            void* ws, void* stream) {
   if (!ctx) return LSP_EINVAL;
   const void* ptrs[] = {x, g_final, w_head, targets, loss, lse, dx, dg_final, dw_head, ws};
   LSP_TRY(check_common(ctx, nullptr, ws, 10, ptrs));
   if (vocab <= 0 || vocab % 8) return fail(ctx, LSP_EINVAL, "lsp_head_fwd_bwd: vocab must be a positive multiple of 8");
+  if (!(grad_scale > 0.f)) return fail(ctx, LSP_EINVAL, "lsp_head_fwd_bwd: grad_scale must be positive");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const int T = ctx->T, H = ctx->d.hidden, V = vocab;
   const HeadLayout L = head_layout(ctx, V);
@@ -837,7 +838,8 @@ lsp_status lsp_head_fwd_bwd(lsp_ctx* ctx, const void* x, const void* g_final, co
     };
     LSP_STAGE(ST_CE, 2, launch());
   }
-  const float alpha = 1.0f / (CE_DZ_SCALE * static_cast<float>(T));      // undo the fp16 scaling, apply the 1/T of the mean
+  // undo the fp16 scaling of dz, apply the 1/T of the mean and the caller's gradient (loss) scale
+  const float alpha = grad_scale / (CE_DZ_SCALE * static_cast<float>(T));
   // dW_head = dz^T xn ; dxn = dz W_head
   {
     EpiF32 e = epi_f32(dw_head, H);
@@ -874,39 +876,57 @@ lsp_status lsp_embed_bwd(lsp_ctx* ctx, const int32_t* ids, const void* dx0, int3
 lsp_status lsp_adamw_step(lsp_ctx* ctx, int ntensors, const lsp_adamw_tensor* tensors, const lsp_adamw_desc* desc,
                           float* gnorm_out, void* stream) {
   if (!ctx || !tensors || !desc || !gnorm_out) return LSP_EINVAL;
-  if (ntensors < 1 || ntensors > OPT_MAX_TENSORS) return fail(ctx, LSP_EINVAL, "lsp_adamw_step: 1 <= ntensors <= %d", OPT_MAX_TENSORS);
-  if (desc->step < 1 || !(desc->beta1 >= 0.f && desc->beta1 < 1.f) || !(desc->beta2 >= 0.f && desc->beta2 < 1.f) || !(desc->clip_norm > 0.f))
+  if (ntensors < 1 || ntensors > OPT_MAX_TENSORS * OPT_MAX_CHUNKS)
+    return fail(ctx, LSP_EINVAL, "lsp_adamw_step: 1 <= ntensors <= %d", OPT_MAX_TENSORS * OPT_MAX_CHUNKS);
+  if (desc->step < 1 || !(desc->beta1 >= 0.f && desc->beta1 < 1.f) || !(desc->beta2 >= 0.f && desc->beta2 < 1.f) || !(desc->clip_norm > 0.f) ||
+      !(desc->grad_scale > 0.f))
     return fail(ctx, LSP_EINVAL, "lsp_adamw_step: bad hyper-parameters");
-  OptTensors t;
-  memset(&t, 0, sizeof(t));
-  t.n = ntensors;
   for (int i = 0; i < ntensors; ++i) {
     const lsp_adamw_tensor& x = tensors[i];
     if (!x.grad || !x.master || !x.m || !x.v || x.n <= 0 || (x.n % 4)) return fail(ctx, LSP_EINVAL, "lsp_adamw_step: tensor %d: NULL pointer or n %% 4 != 0", i);
     if (!aligned(x.grad, 16) || !aligned(x.master, 16) || !aligned(x.m, 16) || !aligned(x.v, 16) || (x.weight_bf16 && !aligned(x.weight_bf16, 8)))
       return fail(ctx, LSP_EALIGN, "lsp_adamw_step: tensor %d is not 16-byte aligned", i);
-    t.g[i] = static_cast<const float*>(x.grad); t.p[i] = x.master; t.m[i] = x.m; t.v[i] = x.v;
-    t.w[i] = static_cast<__nv_bfloat16*>(x.weight_bf16);
-    t.start[i + 1] = t.start[i] + x.n / 4;
-    if (x.decay) t.decay_mask |= 1u << i;
   }
-  for (int i = ntensors; i < OPT_MAX_TENSORS; ++i) t.start[i + 1] = t.start[ntensors];
   OptHyper h;
   h.lr = desc->lr; h.beta1 = desc->beta1; h.beta2 = desc->beta2; h.eps = desc->eps; h.weight_decay = desc->weight_decay;
   h.inv_bc1 = static_cast<float>(1.0 / (1.0 - pow(static_cast<double>(desc->beta1), desc->step)));
   h.inv_bc2 = static_cast<float>(1.0 / (1.0 - pow(static_cast<double>(desc->beta2), desc->step)));
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  long long blocks = (t.start[ntensors] + OPT_THREADS - 1) / OPT_THREADS;
-  const long long cap = ctx->num_sms * 8LL < 4096 ? ctx->num_sms * 8LL : 4096;
-  if (blocks > cap) blocks = cap;
-  const int nb = static_cast<int>(blocks);
+  // The tensors go to the kernels in groups of OPT_MAX_TENSORS (the segment table is a kernel parameter); every group
+  // writes its own range of partial sums, one final kernel turns all of them into the global norm, then the groups update.
+  const int ngroups = (ntensors + OPT_MAX_TENSORS - 1) / OPT_MAX_TENSORS;
+  const long long cap = opt_blocks_cap(ctx->num_sms);
+  auto group = [&](int gi, OptTensors& t) {
+    memset(&t, 0, sizeof(t));
+    const int i0 = gi * OPT_MAX_TENSORS;
+    t.n = ntensors - i0 < OPT_MAX_TENSORS ? ntensors - i0 : OPT_MAX_TENSORS;
+    for (int i = 0; i < t.n; ++i) {
+      const lsp_adamw_tensor& x = tensors[i0 + i];
+      t.g[i] = static_cast<const float*>(x.grad); t.p[i] = x.master; t.m[i] = x.m; t.v[i] = x.v;
+      t.w[i] = static_cast<__nv_bfloat16*>(x.weight_bf16);
+      t.start[i + 1] = t.start[i] + x.n / 4;
+      if (x.decay) t.decay_mask |= 1u << i;
+    }
+    for (int i = t.n; i < OPT_MAX_TENSORS; ++i) t.start[i + 1] = t.start[t.n];
+    long long blocks = (t.start[t.n] + OPT_THREADS - 1) / OPT_THREADS;
+    return static_cast<int>(blocks > cap ? cap : blocks);
+  };
   auto launch = [&]() {
-    opt_gradsq_kernel<<<nb, OPT_THREADS, 0, st>>>(t, ctx->opt_partial);
-    opt_norm_final_kernel<<<1, 32, 0, st>>>(ctx->opt_partial, nb, desc->clip_norm, gnorm_out);
-    opt_adamw_kernel<<<nb, OPT_THREADS, 0, st>>>(t, h, gnorm_out);
+    OptTensors t;
+    int nparts = 0;
+    for (int gi = 0; gi < ngroups; ++gi) {
+      const int nb = group(gi, t);
+      opt_gradsq_kernel<<<nb, OPT_THREADS, 0, st>>>(t, ctx->opt_partial + nparts);
+      nparts += nb;
+    }
+    opt_norm_final_kernel<<<1, OPT_THREADS, 0, st>>>(ctx->opt_partial, nparts, desc->clip_norm, 1.0 / desc->grad_scale, gnorm_out);
+    for (int gi = 0; gi < ngroups; ++gi) {
+      const int nb = group(gi, t);
+      opt_adamw_kernel<<<nb, OPT_THREADS, 0, st>>>(t, h, gnorm_out);
+    }
     return cudaGetLastError();
   };
-  LSP_STAGE(ST_ADAMW, 3, launch());
+  LSP_STAGE(ST_ADAMW, 2 * ngroups + 1, launch());
   return LSP_OK;
 }
 

@@ -1,6 +1,6 @@
 // Optimizer step after the layer backward (Table 2): AdamW [40] with
 // global-norm gradient clipping, fp32 master weights and moments, bf16 model weights (BF16 mixed precision).
-// HBM-bound multi-tensor kernels: the squared-norm pass reads 4 B per parameter, the update reads 16 B and writes
+// HBM-bound multi-tensor kernels (16 tensors per launch, any number of tensors per step in groups of 16): the squared-norm pass reads 4 B per parameter, the update reads 16 B and writes
 // 14 B per parameter (g, p, m, v in; p, m, v, bf16 w out).  The clip coefficient stays on the device (no host sync);
 // all reductions run in a fixed order (bit-reproducible).
 #pragma once
@@ -10,6 +10,8 @@ namespace lsp {
 
 constexpr int OPT_MAX_TENSORS = 16;
 constexpr int OPT_THREADS = 256;
+constexpr int OPT_MAX_CHUNKS = 64;          // groups of OPT_MAX_TENSORS tensors per lsp_adamw_step call
+inline long long opt_blocks_cap(int num_sms) { return num_sms * 8LL; }      // blocks per group (grid-stride beyond)
 
 struct OptTensors {
   const float* g[OPT_MAX_TENSORS];
@@ -55,15 +57,23 @@ __global__ void __launch_bounds__(OPT_THREADS) opt_gradsq_kernel(const OptTensor
   }
 }
 
-// out[0] = global l2 norm, out[1] = min(1, clip / (norm + 1e-6)); one thread, fixed order, fp64 accumulation
-__global__ void opt_norm_final_kernel(const float* __restrict__ partial, int nparts, float clip, float* __restrict__ out) {
-  if (threadIdx.x == 0 && blockIdx.x == 0) {
-    double s = 0.0;
-    for (int i = 0; i < nparts; ++i) s += static_cast<double>(partial[i]);
-    const double norm = sqrt(s);
+// out[0] = global l2 norm of the true gradients g / grad_scale, out[1] = the factor the update applies to the stored
+// gradients = min(1, clip / (norm + 1e-6)) / grad_scale; one block, fp64, fixed order: thread i sums the
+// partials i, i + 256, ... in that order, then thread 0 adds the 256 thread sums in index order
+__global__ void __launch_bounds__(OPT_THREADS) opt_norm_final_kernel(const float* __restrict__ partial, int nparts, float clip,
+                                                                     double inv_scale, float* __restrict__ out) {
+  __shared__ double red[OPT_THREADS];
+  double s = 0.0;
+  for (int i = threadIdx.x; i < nparts; i += OPT_THREADS) s += static_cast<double>(partial[i]);
+  red[threadIdx.x] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double tot = 0.0;
+    for (int i = 0; i < OPT_THREADS; ++i) tot += red[i];
+    const double norm = sqrt(tot) * inv_scale;
     out[0] = static_cast<float>(norm);
     const double c = static_cast<double>(clip) / (norm + 1e-6);
-    out[1] = static_cast<float>(c < 1.0 ? c : 1.0);
+    out[1] = static_cast<float>((c < 1.0 ? c : 1.0) * inv_scale);
   }
 }
 

@@ -1,0 +1,166 @@
+"""One pre-training iteration of a Llama model on one B200, sequenced over the C ABI:
+
+    embedding gather -> n_layers x lsp_layer_fwd -> lsp_head_fwd_bwd (final RMSNorm, LM head, cross-entropy, gradients)
+    -> n_layers x lsp_layer_bwd -> lsp_embed_bwd -> lsp_adamw_step over every tensor of the model (one global norm).
+
+Host-side sequencing and buffer ownership only: every step runs in the library's kernels, on one stream, with no host
+synchronisation inside an iteration (the loss stays on the device until the caller reads it).  Weights are bf16 for the
+kernels with fp32 master copies and moments for the optimizer (Table 2).
+
+    python -m paper_2510_02483_b200.pretrain [--layers L] [--steps K]     # timing of the config-3 model, synthetic batch
+"""
+from __future__ import annotations
+
+import argparse
+import json
+
+import torch
+
+from . import binding as B
+from . import dp, harness, replicas, synth
+
+
+class PretrainStep:
+    def __init__(self, w: synth.Workload, n_layers: int, vocab: int, dev=None, weights=None, embedding=None, head=None, g_final=None,
+                 world: int = 1, group=None):
+        """weights: optional list of per-layer dicts of bf16 bit patterns (synth.layer_weights layout); embedding / head:
+        bf16 bit patterns [vocab, H]; g_final: bf16 bits [H].  Defaults: the seeded synthetic tensors of synth.py.
+        `w` is this rank's shard of the batch; world > 1: data-parallel replicas (dp.py), torch.distributed initialised."""
+        self.dev = dev or harness.require_cuda()
+        self.w, self.L, self.V = w, n_layers, vocab
+        self.ctx = harness.make_ctx(w, in_dtype=B.LSP_F32)
+        T, H = w.tokens, w.hidden
+        f32 = dict(dtype=torch.float32, device=self.dev)
+        self.saved = [torch.empty(self.ctx.saved_bytes, dtype=torch.uint8, device=self.dev) for _ in range(n_layers)]
+        self.ws = torch.empty(max(self.ctx.workspace_bytes, B.lsp_head_workspace_bytes(self.ctx, vocab)), dtype=torch.uint8, device=self.dev)
+        self.xs = [torch.empty((T, H), **f32) for _ in range(n_layers + 1)]
+        self.d = [torch.empty((T, H), **f32) for _ in range(2)]
+        self.loss = torch.zeros(1, **f32)
+        self.lse = torch.empty(T, **f32)
+        self.gnorm = torch.zeros(2, **f32)
+        # parameters: bf16 for the kernels, fp32 master / m / v / grad for the optimizer
+        self.params = []                      # dicts for lsp_adamw_step, in a fixed order
+        self.layer_w, self.layer_g = [], []
+        # gradient buckets (one flat buffer = one all-reduce each): the layers, then {head, final gain}, then the table
+        lshapes = harness.WEIGHT_SHAPES(w)
+        self.buckets = dp.GradBuckets([lshapes] * n_layers + [dict(head=(vocab, H), g_final=(H,)), dict(table=(vocab, H))],
+                                      self.dev, group)
+        self.world = world
+        for l in range(n_layers):
+            bits = weights[l] if weights is not None else synth.layer_weights(w, l)
+            wt = harness.upload_weights(bits, self.dev)
+            gr = self.buckets.views[l]
+            self.layer_w.append(wt)
+            self.layer_g.append(gr)
+            for k in synth.WEIGHT_NAMES:
+                self._register(wt[k], gr[k], decay=wt[k].dim() == 2)
+        st = None
+        if embedding is None or head is None:
+            st = synth.stack_inputs(w.with_(vocab=vocab))
+        self.table = harness.bf16_to_device(embedding if embedding is not None else st["embedding"], self.dev)
+        self.w_head = harness.bf16_to_device(head if head is not None else synth.normal_bf16(w.cfg_id, 0, "w_head", (vocab, H), 0.02), self.dev)
+        self.g_final = (harness.bf16_to_device(g_final, self.dev) if g_final is not None
+                        else torch.ones(H, dtype=torch.bfloat16, device=self.dev))
+        self.d_head, self.d_gfinal = self.buckets.views[n_layers]["head"], self.buckets.views[n_layers]["g_final"]
+        self.d_table = self.buckets.views[n_layers + 1]["table"]
+        self._register(self.table, self.d_table, decay=True)
+        self._register(self.w_head, self.d_head, decay=True)
+        self._register(self.g_final, self.d_gfinal, decay=False)
+        self.t = 0
+        # gradients are carried scaled by T (the gradient of the SUM loss): the mean's 1/T would push the layers' 16-bit
+        # backward operands under the fp16 normal range; lsp_adamw_step divides it out (exact for a power-of-two T),
+        # together with the number of replicas whose gradients were summed
+        self.head_scale = float(T)
+        self.grad_scale = dp.global_grad_scale(T, world)
+
+    def _register(self, weight, grad, decay):
+        self.params.append(dict(grad=grad, master=weight.float(), m=torch.zeros_like(grad), v=torch.zeros_like(grad), weight=weight,
+                                decay=decay))
+
+    @property
+    def n_params(self):
+        return sum(p["master"].numel() for p in self.params)
+
+    def forward_backward(self, ids: torch.Tensor, targets: torch.Tensor, stream=None):
+        """ids, targets: int32 [T] on the device.  Leaves the loss in self.loss (device) and every gradient in place."""
+        c, L = self.ctx, self.L
+        B.lsp_embed_fwd(c, ids, self.table, self.xs[0], stream)
+        for l in range(L):
+            B.lsp_layer_fwd(c, self.xs[l], self.layer_w[l], self.xs[l + 1], self.saved[l], self.ws, stream)
+        d_in = self.d[L & 1]
+        B.lsp_head_fwd_bwd(c, self.xs[L], self.g_final, self.w_head, targets, self.V, self.loss, self.lse, d_in, self.d_gfinal,
+                           self.d_head, self.ws, stream, grad_scale=self.head_scale)
+        self.buckets.reduce_async(L)
+        for l in range(L - 1, -1, -1):
+            d_out = self.d[l & 1]
+            B.lsp_layer_bwd(c, self.xs[l], d_in, self.layer_w[l], self.saved[l], d_out, self.layer_g[l], self.ws, stream)
+            self.buckets.reduce_async(l)            # overlaps the next layer's backward
+            d_in = d_out
+        B.lsp_embed_bwd(c, ids, d_in, self.V, self.d_table, stream)
+        self.buckets.reduce_async(L + 1)
+        return self.loss
+
+    def optimizer_step(self, lr=None, stream=None, **hyper):
+        self.t += 1
+        self.buckets.wait()
+        B.lsp_adamw_step(self.ctx, self.params, lr=B.lsp_lr_cosine(self.t) if lr is None else lr, step=self.t, gnorm_out=self.gnorm,
+                         grad_scale=self.grad_scale, stream=stream, **hyper)
+
+    def step(self, ids, targets, lr=None, stream=None, **hyper):
+        self.forward_backward(ids, targets, stream)
+        self.optimizer_step(lr, stream, **hyper)
+        return self.loss
+
+    def close(self):
+        self.ctx.close()
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--layers", type=int, default=synth.CFG3_3B_STACK.n_layers)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=2)
+    args = ap.parse_args(argv)
+    w = synth.CFG3_3B_STACK
+    # under torchrun: data-parallel replicas, every rank takes a batch of the config's size (weak scaling) with its own ids
+    renv = replicas.rank_env()
+    if renv.world_size > 1:
+        torch.cuda.set_device(renv.local_rank)
+    dev = harness.require_cuda()
+    replicas.init("nccl", renv)
+    run = PretrainStep(w, args.layers, w.vocab, dev, world=renv.world_size)
+    s = synth.stack_inputs(w)
+    ids = torch.from_numpy(s["ids"]).to(dev)
+    ids = torch.roll(ids, 997 * renv.rank)
+    targets = torch.roll(ids, -1)                     # next-token targets of the synthetic stream
+    losses = []
+    for _ in range(args.warmup):
+        losses.append(float(run.step(ids, targets).cpu()))
+    torch.cuda.synchronize()
+    replicas.barrier(dev)
+    e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    ms_fb = ms_opt = 0.0
+    for _ in range(args.steps):
+        e[0].record(); run.forward_backward(ids, targets)
+        e[1].record(); run.optimizer_step()
+        e[2].record(); torch.cuda.synchronize()
+        ms_fb += e[0].elapsed_time(e[1]); ms_opt += e[1].elapsed_time(e[2])
+        losses.append(float(run.loss.cpu()))
+    ms_fb /= args.steps; ms_opt /= args.steps
+    n = run.n_params
+    tok_s, ms_it, tokens = replicas.whole_job_throughput(w.tokens, ms_fb + ms_opt, dev)      # all ranks' tokens / max time
+    # the paper's accounting: 6 FLOPs per parameter per token without the embedding table, plus attention
+    flops = renv.world_size * (6.0 * (n - w.vocab * w.hidden) * w.tokens + args.layers * 3.5 * synth.attn_flops_fwd(w, causal=True))
+    if renv.is_main:
+        print(json.dumps({"config": f"pretrain_{w.name}_L{args.layers}", "n_gpus": renv.world_size, "params": n, "tokens": int(tokens),
+                          "ms_fwd_bwd": round(ms_fb, 3), "ms_adamw": round(ms_opt, 3), "ms_iteration": round(ms_it, 3),
+                          "tokens_per_s": round(tok_s, 1), "model_tflops": round(flops / (ms_it * 1e-3) / 1e12, 1),
+                          "adamw_GB_per_s": round(34.0 * n / (ms_opt * 1e-3) / 1e9, 1),
+                          "mem_GB": round(torch.cuda.max_memory_allocated() / 1e9, 1), "loss": [round(x, 4) for x in losses]}))
+    replicas.finalize()
+    run.close()
+    return 0
+
+
+if __name__ == "__main__":
+    raise SystemExit(main())

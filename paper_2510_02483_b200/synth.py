@@ -18,7 +18,7 @@ from dataclasses import dataclass, replace
 import numpy as np
 
 TENSOR_ID = dict(x=0, dy=1, wq=2, wk=3, wv=4, wo=5, w_gate=6, w_up=7, w_down=8, g_attn=9, g_mlp=10,
-                 ids=11, embedding=12, q=13, k=14, v=15, dO=16)
+                 ids=11, embedding=12, q=13, k=14, v=15, dO=16, w_head=17, g_final=18)
 WEIGHT_NAMES = ("wq", "wk", "wv", "wo", "g_attn", "w_gate", "w_up", "w_down", "g_mlp")
 
 

@@ -359,16 +359,17 @@ def test_adamw_step_vs_oracle(gpu):
     for step in range(1, 5):
         scale = 0.5 if step % 2 else 1e-3
         g = [(rng.standard_normal(s) * scale).astype(np.float32).astype(np.float64) for s in shapes]
-        tg = [torch.tensor(x, dtype=torch.float32, device=dev) for x in g]
+        gs = 1.0 if step < 3 else 64.0        # steps 3, 4: gradients stored scaled by 64 (grad_scale), same true gradients
+        tg = [torch.tensor(x * gs, dtype=torch.float32, device=dev) for x in g]
         lr = A.lr_cosine(step * 600, total=4000)
         tensors = [dict(grad=a, master=b, m=c, v=d, weight=e, decay=f) for a, b, c, d, e, f in zip(tg, tp, tm, tv, tw, decay)]
-        B.lsp_adamw_step(ctx, tensors, lr=lr, step=step, gnorm_out=gn)
+        B.lsp_adamw_step(ctx, tensors, lr=lr, step=step, gnorm_out=gn, grad_scale=gs)
         torch.cuda.synchronize()
         p_old = p
         p, m, v, norm = A.adamw_step(p, g, m, v, decay, step, lr)
         ref_p, ref_m, ref_v = p, m, v
         got_n, got_c = [float(x) for x in gn.cpu().numpy()]
-        assert abs(got_n - norm) <= 1e-6 * norm and abs(got_c - A.clip_coefficient(norm)) <= 2e-6
+        assert abs(got_n - norm) <= 1e-6 * norm and abs(got_c * gs - A.clip_coefficient(norm)) <= 2e-6
         for i in range(len(shapes)):
             gp = tp[i].cpu().numpy().astype(np.float64)
             assert norm_err(tm[i].cpu().numpy(), m[i]) < 2e-5 and norm_err(tv[i].cpu().numpy(), v[i]) < 2e-5, (step, i)
@@ -442,3 +443,79 @@ def test_embed_bwd_vs_oracle(gpu):
     assert not np.any(outs[0][5]) and np.array_equal(outs[0], outs[1])
     assert norm_err(outs[0], ref) < 1e-6
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------------- a whole pre-training iteration
+def _oracle_model_grads(ids, targets, layers, E, Wh, gf, shape, V):
+    """fp64 oracle of one model forward+backward composed from oracle/lspref.py and oracle/head_ref.py."""
+    from oracle import head_ref as Hd
+    xs = [R.embed_fwd(ids, E)]
+    caches = []
+    for wl in layers:
+        y, c = R.layer_fwd(xs[-1], wl, shape)
+        xs.append(y); caches.append(c)
+    out = Hd.head_loss_fwd_bwd(xs[-1], gf, Wh, targets, shape.rms_eps)
+    d = out["dx"]
+    lgrads = [None] * len(layers)
+    for l in range(len(layers) - 1, -1, -1):
+        d, lgrads[l], _ = R.layer_bwd(d, layers[l], shape, caches[l])
+    return out["loss"], lgrads, Hd.embed_bwd(ids, d, V), out["dw_head"], out["dg_final"]
+
+
+def test_pretrain_iterations_vs_oracle(gpu):
+    """Three whole iterations of pretrain.PretrainStep on a 2-layer model (21 parameter tensors: two groups of
+    lsp_adamw_step; gradients carried scaled by T): embedding -> layers -> head/loss -> backward -> embedding backward ->
+    AdamW with one global norm.  Every iteration the fp64 oracle (lspref + head_ref + adamw_ref) starts from the GPU's
+    own fp32 master state, so each comparison is one iteration: loss 1e-3 relative, every gradient of the model at the
+    layer's bar (2e-2 max|d|/rms), the global gradient norm 5e-3 relative, and the bf16 weights the kernels will use
+    next exactly the rounding of the master weights.  The loss must also fall from iteration to iteration (same batch)."""
+    import torch
+    from oracle import adamw_ref as A
+    from paper_2510_02483_b200 import pretrain
+    w = synth.Workload("pretrain_small", 9, 2, 192, 256, 4, 2, 128, 688, 1e-5, 500000.0, 2, 1000)
+    V, L = w.vocab, w.n_layers
+    run = pretrain.PretrainStep(w, L, V)
+    assert len(run.params) == 9 * L + 3
+    s = synth.stack_inputs(w)
+    ids = s["ids"]; targets = np.roll(ids, -1)
+    tid = torch.from_numpy(ids).cuda(); tt = torch.from_numpy(targets).cuda()
+    shape = oracle_shape(w)
+    names = list(synth.WEIGHT_NAMES)
+    losses = []
+    lr = 1.0e-3
+    for it in range(1, 4):
+        # the oracle's parameters = the bf16 weights the kernels read this iteration (= rounding of the master weights)
+        host = [p["weight"].float().cpu().numpy().astype(np.float64) for p in run.params]
+        master = [p["master"].cpu().numpy().astype(np.float64) for p in run.params]
+        for a, b in zip(host, master):
+            assert np.array_equal(a, A.bf16_rne(b))
+        m0 = [p["m"].cpu().numpy().astype(np.float64) for p in run.params]
+        v0 = [p["v"].cpu().numpy().astype(np.float64) for p in run.params]
+        layers = [dict(zip(names, host[9 * l:9 * l + 9])) for l in range(L)]
+        E, Wh, gf = host[9 * L], host[9 * L + 1], host[9 * L + 2]
+        run.step(tid, tt, lr=lr)
+        torch.cuda.synchronize()
+        loss_ref, lg, dE, dWh, dgf = _oracle_model_grads(ids, targets, layers, E, Wh, gf, shape, V)
+        loss = float(run.loss.cpu()); losses.append(loss)
+        assert abs(loss - loss_ref) <= 1e-3 * abs(loss_ref), (it, loss, loss_ref)
+        ref_g = [lg[l][k] for l in range(L) for k in names] + [dE, dWh, dgf]
+        got_g = [p["grad"].cpu().numpy().astype(np.float64) / run.grad_scale for p in run.params]
+        tags = [f"L{l}.d{k}" for l in range(L) for k in names] + ["d_table", "d_head", "d_gfinal"]
+        check(dict(zip(tags, got_g)), dict(zip(tags, ref_g)), tags)
+        norm_ref = A.global_grad_norm(ref_g)
+        got_n, got_c = [float(x) for x in run.gnorm.cpu().numpy()]
+        assert abs(got_n - norm_ref) <= 5e-3 * norm_ref, (it, got_n, norm_ref)
+        assert abs(got_c * run.grad_scale - A.clip_coefficient(got_n)) <= 1e-5
+        # the optimizer step itself, from the GPU's own gradients and state (one fp32 step against fp64)
+        decay = [bool(p["decay"]) for p in run.params]
+        p_ref, m_ref, v_ref, _ = A.adamw_step(master, got_g, m0, v0, decay, it, lr)
+        for i, p in enumerate(run.params):
+            gp = p["master"].cpu().numpy().astype(np.float64)
+            upd = p_ref[i] - master[i]
+            # one fp32 rounding of p (2^-24 |p|; the gains are ~1) against an update of rms ~ lr
+            bar = 5e-5 + 2.0 ** -23 * float(np.max(np.abs(master[i]))) / float(np.sqrt(np.mean(upd * upd)))
+            assert norm_err(gp - master[i], upd) < bar, (it, tags[i])
+            assert norm_err(p["m"].cpu().numpy(), m_ref[i]) < 5e-5 and norm_err(p["v"].cpu().numpy(), v_ref[i]) < 5e-5, (it, tags[i])
+    print("losses", losses)
+    assert losses[0] > losses[1] > losses[2]
+    run.close()
