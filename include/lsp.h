@@ -52,10 +52,11 @@ typedef struct {
   int32_t batch, seq, hidden, n_q_heads, n_kv_heads, head_dim, ffn;
   float rms_eps;            /* inside the sqrt, added to mean(x^2) (reading A-3) */
   double rope_base;         /* theta_i = pos * base^(-2i/d), no scaling (reading A-5) */
-  int32_t rope_layout;      /* 0 = adjacent pairs (2i,2i+1) as in ref [36]; others: LSP_EUNSUPPORTED */
+  int32_t rope_layout;      /* 0 = adjacent pairs (2i,2i+1) as in ref [36]; 1 = half-split pairs (i, i+d/2) */
   int32_t use_rope;         /* 1 in the layer path; 0 = no rotation */
   int32_t in_dtype;         /* lsp_dtype of x / a / dy / da inputs */
-  int32_t wgrad_accumulate; /* 0 = overwrite weight gradients; 1: LSP_EUNSUPPORTED in this revision */
+  int32_t wgrad_accumulate; /* 0 = overwrite the nine weight / gain gradients; 1 = add to what the buffers hold
+                             * (micro-batch gradient accumulation: one fp32 add per element, bit-reproducible) */
 } lsp_layer_desc;
 
 typedef struct {
@@ -143,13 +144,15 @@ lsp_status lsp_layer_step_host(lsp_ctx* ctx, const void* x_host, const void* dy_
  *   fp32 logits [T, vocab] and their fp16 gradient -- 6 bytes per (token, class).
  *   grad_scale > 0 multiplies the three gradients (not the loss): the layers' backward feeds 16-bit tensor-core
  *   operands, and the gradient of a MEAN loss is ~1/T per element, below the fp16 normal range at training sizes; a
- *   training step passes e.g. grad_scale = T and hands the same value to lsp_adamw_step, which divides it out. */
+ *   training step passes e.g. grad_scale = T and hands the same value to lsp_adamw_step, which divides it out.
+ *   On a context created with wgrad_accumulate = 1, dw_head and dg_final are added to (dx is always overwritten). */
 size_t lsp_head_workspace_bytes(const lsp_ctx* ctx, int32_t vocab);
 lsp_status lsp_head_fwd_bwd(lsp_ctx* ctx, const void* x, const void* g_final, const void* w_head, const int32_t* targets,
                             int32_t vocab, float grad_scale, float* loss, float* lse, void* dx, float* dg_final,
                             float* dw_head, void* ws, void* stream);
 /* Embedding backward (H-3): d_table [vocab, H] fp32 (fully written: zero for ids that do not occur) =
- * scatter-add of dx0 fp32 [T,H] by ids int32 [T]; duplicates are added in increasing token order (bit-reproducible). */
+ * scatter-add of dx0 fp32 [T,H] by ids int32 [T]; duplicates are added in increasing token order (bit-reproducible).
+ * On a context created with wgrad_accumulate = 1 the sums are added to what d_table holds (no zeroing). */
 lsp_status lsp_embed_bwd(lsp_ctx* ctx, const int32_t* ids, const void* dx0, int32_t vocab, float* d_table, void* stream);
 
 /* Optimizer step after the backward (Table 2): AdamW with decoupled weight decay

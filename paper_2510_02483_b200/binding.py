@@ -120,9 +120,9 @@ class Ctx:
     """Owns one lsp_ctx (a layer shape on a device)."""
 
     def __init__(self, *, batch, seq, hidden, n_q_heads, n_kv_heads, head_dim, ffn, rms_eps=1e-5, rope_base=10000.0,
-                 use_rope=True, in_dtype=LSP_BF16, device=0):
-        self.desc = lsp_layer_desc(batch, seq, hidden, n_q_heads, n_kv_heads, head_dim, ffn, rms_eps, rope_base, 0,
-                                   1 if use_rope else 0, in_dtype, 0)
+                 use_rope=True, in_dtype=LSP_BF16, device=0, rope_layout=0, wgrad_accumulate=False):
+        self.desc = lsp_layer_desc(batch, seq, hidden, n_q_heads, n_kv_heads, head_dim, ffn, rms_eps, rope_base, rope_layout,
+                                   1 if use_rope else 0, in_dtype, 1 if wgrad_accumulate else 0)
         self.handle = C.c_void_p()
         st = lib().lsp_create(C.byref(self.handle), C.byref(self.desc), device)
         if st != 0:

@@ -86,6 +86,20 @@ inline bool make_map_store2d(CUtensorMap* m, const void* base, long long rows, l
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// 4-D fp32 map that un-permutes rows on the way out (rope_layout = 1): the GEMM's row
+// head*d + 2i + half is row head*d + half*d/2 + i of the [rows, cols] output.  Dimensions (col, half, i, head); a box of
+// 32 cols x 2 halves x 16 i is 32 consecutive GEMM rows in shared memory (i-major, half-minor), 128 B each.
+inline bool make_map_store_perm(CUtensorMap* m, const void* base, long long rows, long long cols, long long ld, int d) {
+  PFN_encodeTiled fn = get_encode_fn();
+  if (!fn || rows <= 0 || cols <= 0 || d < 32 || rows % d) return false;
+  cuuint64_t dims[4] = {static_cast<cuuint64_t>(cols), 2, static_cast<cuuint64_t>(d / 2), static_cast<cuuint64_t>(rows / d)};
+  cuuint64_t strides[3] = {static_cast<cuuint64_t>(d / 2) * ld * 4, static_cast<cuuint64_t>(ld) * 4, static_cast<cuuint64_t>(d) * ld * 4};
+  cuuint32_t box[4] = {32u, 2u, 16u, 1u};
+  cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <int BN> struct GemmCfg {
   static constexpr int A_BYTES = GEMM_BM * GEMM_BK * 2;
   static constexpr int B_BYTES = BN * GEMM_BK * 2;
@@ -311,7 +325,8 @@ __device__ __forceinline__ void chunk_load(const WarpStage& st, RowPtr rowptr, f
 // clipped by the map.  Per-thread st.global of such a tile stalled the warps an order of magnitude longer (measured in
 // the attention forward: ~12 k vs ~1 k cycles for 4 chunks), the bulk store is asynchronous.
 template <int DT>
-__device__ __forceinline__ void chunk_store_tma(const WarpStage& st, const CUtensorMap* map, int c0, int r0, const float (&v)[32]) {
+__device__ __forceinline__ void chunk_store_tma(const WarpStage& st, const CUtensorMap* map, int c0, int r0, const float (&v)[32],
+                                                bool accumulate = false) {
   if (st.lane == 0) tma_store_wait_read<0>();    // the previous bulk store of this warp has read the tile
   __syncwarp();
   if constexpr (DT == DT_F32) {
@@ -324,7 +339,27 @@ __device__ __forceinline__ void chunk_store_tma(const WarpStage& st, const CUten
   }
   fence_proxy_async_smem();                      // generic-proxy writes -> visible to the async proxy
   __syncwarp();
-  if (st.lane == 0) { tma_store_2d(map, st.base, c0, r0); tma_store_commit(); }
+  if (st.lane == 0) {
+    if (accumulate) tma_reduce_add_2d(map, st.base, c0, r0);      // out += tile: one fp32 add per element, in the L2
+    else tma_store_2d(map, st.base, c0, r0);
+    tma_store_commit();
+  }
+}
+
+// fp32 chunk through a row-un-permuting 4-D map (make_map_store_perm): GEMM rows [r0, r0 + 32) of a head-aligned segment
+__device__ __forceinline__ void chunk_store_tma_perm(const WarpStage& st, const CUtensorMap* map, int c0, int r0, int d, const float (&v)[32],
+                                                     bool accumulate) {
+  if (st.lane == 0) tma_store_wait_read<0>();
+  __syncwarp();
+  st.put_row32(v);
+  fence_proxy_async_smem();
+  __syncwarp();
+  if (st.lane == 0) {
+    const int head = r0 / d, i0 = (r0 - head * d) >> 1;
+    if (accumulate) tma_reduce_add_4d(map, st.base, c0, 0, i0, head);
+    else tma_store_4d(map, st.base, c0, 0, i0, head);
+    tma_store_commit();
+  }
 }
 
 template <int DT>
@@ -358,12 +393,19 @@ struct EpiStore {
   float alpha;
   CUtensorMap omap[3];       // store maps of the up-to-three outputs (encoded by the host in encode())
   int use_tma;               // 0 when a 32-row chunk can straddle a split (splits not multiples of 32): per-thread stores
+  int accumulate = 0;        // 1: out += result (fp32 outputs; lsp_layer_desc.wgrad_accumulate) instead of out = result
+  int perm_d = 0;            // rope_layout = 1: head_dim; the rows of the segments in perm_segs leave through a 4-D map that
+  unsigned perm_segs = 0;    // un-permutes them (dWq, dWk of the row-permuted projection weights)
   bool encode(int M, int N) {
     use_tma = !((split1 < M && split1 % 32) || (split2 < M && split2 % 32));
-    if (!use_tma) return true;
+    if (!use_tma) return perm_segs == 0;
     const int s1 = split1 < M ? split1 : M, s2 = split2 < M ? split2 : M;
     const int rows[3] = {s1, s2 - s1, M - s2};
     for (int i = 0; i < 3; ++i) {
+      if (rows[i] > 0 && ((perm_segs >> i) & 1u)) {
+        if (ODT != DT_F32 || !make_map_store_perm(&omap[i], out[i], rows[i], N, ld, perm_d)) return false;
+        continue;
+      }
       if (rows[i] > 0 && !make_map_store2d(&omap[i], out[i], rows[i], N, ld, ODT)) return false;
       if (rows[i] <= 0) omap[i] = omap[0];
     }
@@ -396,16 +438,24 @@ struct EpiStore {
     if (use_tma) {
       const int seg = (m_base >= split1) + (m_base >= split2);      // a 32-row chunk never straddles a split
       const int mr = m_base - (seg == 0 ? 0 : (seg == 1 ? split1 : split2));
-      chunk_store_tma<ODT>(st, &omap[seg], n, mr, v);
+      if ((perm_segs >> seg) & 1u) chunk_store_tma_perm(st, &omap[seg], n, mr, perm_d, v, accumulate != 0);
+      else chunk_store_tma<ODT>(st, &omap[seg], n, mr, v, accumulate != 0);
     } else {
       using OT = typename OutElem<ODT>::type;
-      if (st.lane == 0) tma_store_wait_read<0>();
-      chunk_store<ODT>(st, [&](int rr) {
+      auto rowptr = [&](int rr) {
         const int m = m_base + rr;
         const int seg = (m >= split1) + (m >= split2);
         const int mr = m - (seg == 0 ? 0 : (seg == 1 ? split1 : split2));
         return reinterpret_cast<OT*>(out[seg]) + static_cast<long long>(mr) * ld + n;
-      }, v, nrows, nvalid);
+      };
+      if (accumulate) {
+        float r[32];
+        chunk_load<ODT>(st, rowptr, r, nrows, nvalid);
+#pragma unroll
+        for (int j = 0; j < 32; ++j) v[j] = r[j] + v[j];
+      }
+      if (st.lane == 0) tma_store_wait_read<0>();
+      chunk_store<ODT>(st, rowptr, v, nrows, nvalid);
     }
   }
 };

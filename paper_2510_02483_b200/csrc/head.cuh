@@ -73,9 +73,9 @@ __global__ void ce_loss_mean_kernel(const float* __restrict__ loss_row, int T, f
 
 // dE[v,:] = sum over {t : id_t = v} dx0[t,:], tokens added in increasing t (deterministic, no atomics).  One CTA per
 // token: the CTA of the FIRST occurrence of an id gathers all later occurrences in order; the others exit.  dE must
-// have been zeroed (rows of ids that never occur).  O(T^2 / 256) id comparisons per launch: 0.26 M at T = 8192.
+// have been zeroed (rows of ids that never occur), or hold the running sum when `accumulate` is set.  O(T^2 / 256) id comparisons per launch: 0.26 M at T = 8192.
 __global__ void __launch_bounds__(256) embed_bwd_kernel(const int* __restrict__ ids, const float* __restrict__ dx0, int T, int H,
-                                                        float* __restrict__ dE) {
+                                                        float* __restrict__ dE, int accumulate) {
   __shared__ unsigned int hits[8];                    // per warp: ballot of the candidates whose id matches
   __shared__ int any_before;
   const int t = blockIdx.x;
@@ -114,7 +114,7 @@ __global__ void __launch_bounds__(256) embed_bwd_kernel(const int* __restrict__ 
 #pragma unroll
   for (int k = 0; k < 32; ++k) {
     const int c = threadIdx.x + k * 256;
-    if (c < H) out[c] = acc[k];
+    if (c < H) out[c] = accumulate ? out[c] + acc[k] : acc[k];
   }
 }
 

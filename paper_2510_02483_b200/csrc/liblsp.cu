@@ -177,7 +177,7 @@ cudaError_t norm_fwd(const lsp_ctx* c, int dt, const void* x, const void* g, __h
 
 template <typename XT, typename RT>
 cudaError_t norm_bwd_t(const lsp_ctx* c, const void* x, const float* rstd, const void* g, const float* dxn, const void* dres,
-                       float* dx, __half* dx16, float* dg_part, float* dg, cudaStream_t st) {
+                       float* dx, __half* dx16, float* dg_part, float* dg, int dg_accumulate, cudaStream_t st) {
   const int H = c->d.hidden, nv = (H / 4 + NORMB_CONSUMERS - 1) / NORMB_CONSUMERS;
   const XT* xp = static_cast<const XT*>(x);
   const RT* rp = static_cast<const RT*>(dres);
@@ -197,17 +197,17 @@ cudaError_t norm_bwd_t(const lsp_ctx* c, const void* x, const float* rstd, const
 #undef LSP_NB
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  colsum_kernel<<<(H + 31) / 32, 256, 0, st>>>(dg_part, dg, nb, H);
+  colsum_kernel<<<(H + 31) / 32, 256, 0, st>>>(dg_part, dg, nb, H, dg_accumulate);
   return cudaGetLastError();
 }
 // x: forward input of the norm (XT = x_dt); dres: incoming residual gradient (RT = r_dt)
 cudaError_t norm_bwd(const lsp_ctx* c, int x_dt, int r_dt, const void* x, const float* rstd, const void* g, const float* dxn,
-                     const void* dres, float* dx, __half* dx16, float* dg_part, float* dg, cudaStream_t st) {
+                     const void* dres, float* dx, __half* dx16, float* dg_part, float* dg, int acc, cudaStream_t st) {
   if (x_dt == LSP_F32)
-    return r_dt == LSP_F32 ? norm_bwd_t<float, float>(c, x, rstd, g, dxn, dres, dx, dx16, dg_part, dg, st)
-                           : norm_bwd_t<float, __nv_bfloat16>(c, x, rstd, g, dxn, dres, dx, dx16, dg_part, dg, st);
-  return r_dt == LSP_F32 ? norm_bwd_t<__nv_bfloat16, float>(c, x, rstd, g, dxn, dres, dx, dx16, dg_part, dg, st)
-                         : norm_bwd_t<__nv_bfloat16, __nv_bfloat16>(c, x, rstd, g, dxn, dres, dx, dx16, dg_part, dg, st);
+    return r_dt == LSP_F32 ? norm_bwd_t<float, float>(c, x, rstd, g, dxn, dres, dx, dx16, dg_part, dg, acc, st)
+                           : norm_bwd_t<float, __nv_bfloat16>(c, x, rstd, g, dxn, dres, dx, dx16, dg_part, dg, acc, st);
+  return r_dt == LSP_F32 ? norm_bwd_t<__nv_bfloat16, float>(c, x, rstd, g, dxn, dres, dx, dx16, dg_part, dg, acc, st)
+                         : norm_bwd_t<__nv_bfloat16, __nv_bfloat16>(c, x, rstd, g, dxn, dres, dx, dx16, dg_part, dg, acc, st);
 }
 
 cudaError_t cast_f32_f16(const float* in, __half* out, long long n, int sms, cudaStream_t st) {
@@ -228,9 +228,11 @@ cudaError_t cast_bf16_f16(const __nv_bfloat16* in, __half* out, long long n, int
 }
 
 // up to CAST_MAX_SEGS bf16 -> fp16 weight casts in one launch (element counts are multiples of 8)
-cudaError_t cast_weights(const lsp_ctx* c, int nseg, const void* const* src, __half* const* dst, const long long* n, cudaStream_t st) {
+cudaError_t cast_weights(const lsp_ctx* c, int nseg, const void* const* src, __half* const* dst, const long long* n, cudaStream_t st,
+                         unsigned perm_mask = 0) {
   CastSegs segs;
   segs.nseg = nseg;
+  segs.perm_mask = perm_mask; segs.perm_d = c->d.head_dim; segs.row_units = c->d.hidden / 8;
   segs.start[0] = 0;
   for (int i = 0; i < CAST_MAX_SEGS; ++i) {
     segs.src[i] = i < nseg ? static_cast<const __nv_bfloat16*>(src[i]) : nullptr;
@@ -256,6 +258,13 @@ inline EpiF32 epi_f32(float* out, long long ld) {
   EpiF32 e;
   e.out[0] = out; e.out[1] = e.out[2] = nullptr;
   e.split1 = e.split2 = 0x7fffffff; e.ld = ld; e.res = nullptr; e.alpha = 1.0f;
+  return e;
+}
+
+// weight-gradient output: overwrite, or += when the context was created with wgrad_accumulate = 1
+inline EpiF32 epi_wgrad(const lsp_ctx* c, void* out, long long ld) {
+  EpiF32 e = epi_f32(static_cast<float*>(out), ld);
+  e.accumulate = c->d.wgrad_accumulate;
   return e;
 }
 
@@ -329,7 +338,9 @@ lsp_status attn_fwd_impl(lsp_ctx* ctx, int x_dt, const void* x, const lsp_layer_
     __half* dst[4] = {wqkv16, wqkv16 + static_cast<long long>(Nq) * H, wqkv16 + static_cast<long long>(Nq + Nkv) * H, wo16};
     const long long cnt[4] = {static_cast<long long>(Nq) * H, static_cast<long long>(Nkv) * H, static_cast<long long>(Nkv) * H,
                               static_cast<long long>(H) * Nq};
-    LSP_STAGE(ST_CAST, 1, cast_weights(ctx, 4, src, dst, cnt, st));
+    // rope_layout = 1: the rows of Wq, Wk are interleaved per head, so that the adjacent-pair rotation of the QKV epilogue
+    // acts on the half-split pairs (i, i + d/2); q.k is invariant under the common permutation
+    LSP_STAGE(ST_CAST, 1, cast_weights(ctx, 4, src, dst, cnt, st, (d.use_rope && d.rope_layout == 1) ? 0x3u : 0u));
   }
   // F1 RMSNorm-1
   LSP_STAGE(ST_NORM_FWD, 1, norm_fwd(ctx, x_dt, x, w->g_attn, xn, rstd1, st));
@@ -375,7 +386,7 @@ lsp_status attn_bwd_impl(lsp_ctx* ctx, int x_dt, const void* x, int da_dt, const
 
   // B6 dWo = da^T O ; dO = da Wo ; D = rowsum(dO * O32)
   LSP_STAGE(ST_WGRAD_O, 1, (gemm1<true, true>(ctx, H, Nq, T, Operand{da16, H, true}, Operand{o16, Nq, true},
-                              epi_f32(static_cast<float*>(g->wo), Nq), st)));
+                              epi_wgrad(ctx, g->wo, Nq), st)));
   {
     EpiStore<DT_F16, DT_F32, false> e;
     e.out[0] = dO16; e.out[1] = e.out[2] = nullptr; e.split1 = e.split2 = 0x7fffffff; e.ld = Nq; e.res = nullptr; e.alpha = 1.0f;
@@ -397,14 +408,15 @@ lsp_status attn_bwd_impl(lsp_ctx* ctx, int x_dt, const void* x, int da_dt, const
   LSP_TRY(attn_bwd_dispatch(ctx, p, st));
   // B9 dW{q,k,v} = d{q,k,v}^T xn (one GEMM, rows split over three outputs) ; dxn = [dq|dk|dv] [Wq;Wk;Wv] (one GEMM)
   {
-    EpiF32 e = epi_f32(static_cast<float*>(g->wq), H);
+    EpiF32 e = epi_wgrad(ctx, g->wq, H);
     e.out[1] = g->wk; e.out[2] = g->wv; e.split1 = Nq; e.split2 = Nq + Nkv;
+    if (d.use_rope && d.rope_layout == 1) { e.perm_d = d.head_dim; e.perm_segs = 0x3u; }     // dWq, dWk rows back to the caller's order
     LSP_STAGE(ST_WGRAD_QKV, 1, (gemm1<true, true>(ctx, Nqkv, H, T, Operand{dqkv, Nqkv, true}, Operand{xn, H, true}, e, st)));
   }
   LSP_STAGE(ST_DGRAD_QKV, 1, (gemm1<false, true>(ctx, T, H, Nqkv, Operand{dqkv, Nqkv, false}, Operand{wqkv16, H, true},
                                epi_f32(dxn, H), st)));
   // B10 RMSNorm-1 backward + residual gradient
-  LSP_STAGE(ST_NORM_BWD, 2, norm_bwd(ctx, x_dt, da_dt, x, rstd1, w->g_attn, dxn, da, dx, nullptr, dgpart, static_cast<float*>(g->g_attn), st));
+  LSP_STAGE(ST_NORM_BWD, 2, norm_bwd(ctx, x_dt, da_dt, x, rstd1, w->g_attn, dxn, da, dx, nullptr, dgpart, static_cast<float*>(g->g_attn), ctx->d.wgrad_accumulate, st));
   return LSP_OK;
 }
 
@@ -454,7 +466,7 @@ lsp_status mlp_bwd_impl(lsp_ctx* ctx, int a_dt, const void* a, int dy_dt, const 
   float* dgpart = at<float>(ws, ctx->ws.dgpart);
 
   // B2 dWd = dy^T h
-  LSP_STAGE(ST_WGRAD_DOWN, 1, (gemm1<true, true>(ctx, H, F, T, Operand{dy16, H, true}, Operand{h, F, true}, epi_f32(static_cast<float*>(g->w_down), F), st)));
+  LSP_STAGE(ST_WGRAD_DOWN, 1, (gemm1<true, true>(ctx, H, F, T, Operand{dy16, H, true}, Operand{h, F, true}, epi_wgrad(ctx, g->w_down, F), st)));
   // B1 dh = dy Wd with the SwiGLU-backward epilogue -> [dg | du]
   {
     EpiSwiGLUBwd e{g16, u16, F, dgu, F};
@@ -462,7 +474,7 @@ lsp_status mlp_bwd_impl(lsp_ctx* ctx, int a_dt, const void* a, int dy_dt, const 
   }
   // B4 dWg = dg^T an, dWu = du^T an (one GEMM over the 2F rows of [dg | du]^T)
   {
-    EpiF32 e = epi_f32(static_cast<float*>(g->w_gate), H);
+    EpiF32 e = epi_wgrad(ctx, g->w_gate, H);
     e.out[1] = g->w_up; e.split1 = F;
     LSP_STAGE(ST_WGRAD_GATEUP, 1, (gemm1<true, true>(ctx, 2 * F, H, T, Operand{dgu, 2LL * F, true}, Operand{an, H, true}, e, st)));
   }
@@ -470,7 +482,7 @@ lsp_status mlp_bwd_impl(lsp_ctx* ctx, int a_dt, const void* a, int dy_dt, const 
   LSP_STAGE(ST_DGRAD_GATEUP, 1, (gemm1<false, true>(ctx, T, H, 2 * F, Operand{dgu, 2LL * F, false}, Operand{wgu16, H, true},
                                   epi_f32(dan, H), st)));
   // B5 RMSNorm-2 backward + residual gradient
-  LSP_STAGE(ST_NORM_BWD, 2, norm_bwd(ctx, a_dt, dy_dt, a, rstd2, w->g_mlp, dan, dy, da, da16, dgpart, static_cast<float*>(g->g_mlp), st));
+  LSP_STAGE(ST_NORM_BWD, 2, norm_bwd(ctx, a_dt, dy_dt, a, rstd2, w->g_mlp, dan, dy, da, da16, dgpart, static_cast<float*>(g->g_mlp), ctx->d.wgrad_accumulate, st));
   return LSP_OK;
 }
 
@@ -508,7 +520,7 @@ lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device
   if (d.n_q_heads % d.n_kv_heads != 0) return LSP_EINVAL;
   if (d.head_dim != 64 && d.head_dim != 128) return LSP_EUNSUPPORTED;
   if (d.hidden % 8 || d.ffn % 8 || d.hidden > 8192) return LSP_EUNSUPPORTED;
-  if (d.rope_layout != 0 || d.wgrad_accumulate != 0) return LSP_EUNSUPPORTED;
+  if ((d.rope_layout != 0 && d.rope_layout != 1) || (d.wgrad_accumulate != 0 && d.wgrad_accumulate != 1)) return LSP_EUNSUPPORTED;
   if (d.in_dtype != LSP_BF16 && d.in_dtype != LSP_F32) return LSP_EINVAL;
   if (!(d.rms_eps >= 0.0f) || !(d.rope_base > 0.0)) return LSP_EINVAL;
   if (static_cast<long long>(d.batch) * d.seq > 0x7fffffffLL / 4) return LSP_EUNSUPPORTED;
@@ -842,7 +854,7 @@ lsp_status lsp_head_fwd_bwd(lsp_ctx* ctx, const void* x, const void* g_final, co
   const float alpha = grad_scale / (CE_DZ_SCALE * static_cast<float>(T));
   // dW_head = dz^T xn ; dxn = dz W_head
   {
-    EpiF32 e = epi_f32(dw_head, H);
+    EpiF32 e = epi_wgrad(ctx, dw_head, H);
     e.alpha = alpha;
     LSP_STAGE(ST_HEAD_GEMM, 1, (gemm1<true, true>(ctx, V, H, T, Operand{dz16, V, true}, Operand{xn16, H, true}, e, st)));
   }
@@ -853,7 +865,7 @@ lsp_status lsp_head_fwd_bwd(lsp_ctx* ctx, const void* x, const void* g_final, co
   }
   // final RMSNorm backward (no residual gradient)
   LSP_STAGE(ST_NORM_BWD, 2, norm_bwd(ctx, ctx->d.in_dtype, LSP_F32, x, rstd, g_final, dxn32, nullptr, static_cast<float*>(dx), nullptr,
-                                      dgpart, dg_final, st));
+                                      dgpart, dg_final, ctx->d.wgrad_accumulate, st));
   return LSP_OK;
 }
 
@@ -864,9 +876,10 @@ lsp_status lsp_embed_bwd(lsp_ctx* ctx, const int32_t* ids, const void* dx0, int3
   if (vocab <= 0) return fail(ctx, LSP_EINVAL, "lsp_embed_bwd: vocab must be positive");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const int T = ctx->T, H = ctx->d.hidden;
-  LSP_CUDA(cudaMemsetAsync(d_table, 0, static_cast<size_t>(vocab) * H * sizeof(float), st));
+  const int acc = ctx->d.wgrad_accumulate;
+  if (!acc) LSP_CUDA(cudaMemsetAsync(d_table, 0, static_cast<size_t>(vocab) * H * sizeof(float), st));
   auto launch = [&]() {
-    embed_bwd_kernel<<<T, 256, 0, st>>>(ids, static_cast<const float*>(dx0), T, H, d_table);
+    embed_bwd_kernel<<<T, 256, 0, st>>>(ids, static_cast<const float*>(dx0), T, H, d_table, acc);
     return cudaGetLastError();
   };
   LSP_STAGE(ST_EMBED_BWD, 1, launch());

@@ -207,8 +207,9 @@ rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, con
   }
 }
 
-// dg[col] = sum over CTAs of dg_part[cta][col], fixed order (deterministic).  Block = 32 columns x 8 partial groups.
-__global__ void __launch_bounds__(256) colsum_kernel(const float* __restrict__ part, float* __restrict__ out, int nparts, int H) {
+// dg[col] (+)= sum over CTAs of dg_part[cta][col], fixed order (deterministic).  Block = 32 columns x 8 partial groups.
+__global__ void __launch_bounds__(256) colsum_kernel(const float* __restrict__ part, float* __restrict__ out, int nparts, int H,
+                                                     int accumulate) {
   __shared__ float sm[8][33];
   const int cx = threadIdx.x & 31, gy = threadIdx.x >> 5;
   const int c = blockIdx.x * 32 + cx;
@@ -221,7 +222,7 @@ __global__ void __launch_bounds__(256) colsum_kernel(const float* __restrict__ p
     float t = 0.f;
 #pragma unroll
     for (int k = 0; k < 8; ++k) t += sm[k][cx];
-    out[c] = t;
+    out[c] = accumulate ? out[c] + t : t;
   }
 }
 
@@ -248,6 +249,8 @@ struct CastSegs {
   __half* dst[CAST_MAX_SEGS];
   long long start[CAST_MAX_SEGS + 1];
   int nseg;
+  unsigned perm_mask;        // segments whose ROWS are permuted on the way: dst row head*d + 2i + half = src row head*d + half*d/2 + i
+  int perm_d, row_units;     // head_dim; 16-byte units per row (in-features / 8)
 };
 __global__ void cast_multi_bf16_f16_kernel(const CastSegs segs) {
   const long long total = segs.start[segs.nseg];
@@ -256,7 +259,13 @@ __global__ void cast_multi_bf16_f16_kernel(const CastSegs segs) {
 #pragma unroll
     for (int k = 1; k < CAST_MAX_SEGS; ++k) s += (k < segs.nseg && i >= segs.start[k]) ? 1 : 0;
     const long long j = i - segs.start[s];
-    const uint4 u = __ldg(reinterpret_cast<const uint4*>(segs.src[s]) + j);
+    long long js = j;
+    if ((segs.perm_mask >> s) & 1u) {
+      const long long row = j / segs.row_units;
+      const int p = static_cast<int>(row % segs.perm_d);
+      js = (row - p + (p & 1) * (segs.perm_d >> 1) + (p >> 1)) * segs.row_units + (j - row * segs.row_units);
+    }
+    const uint4 u = __ldg(reinterpret_cast<const uint4*>(segs.src[s]) + js);
     reinterpret_cast<uint4*>(segs.dst[s])[j] = make_uint4(pack_f16(bf16_lo(u.x), bf16_hi(u.x)), pack_f16(bf16_lo(u.y), bf16_hi(u.y)),
                                                          pack_f16(bf16_lo(u.z), bf16_hi(u.z)), pack_f16(bf16_lo(u.w), bf16_hi(u.w)));
   }

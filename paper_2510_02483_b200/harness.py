@@ -34,10 +34,11 @@ def bf16_pinned(bits: np.ndarray) -> torch.Tensor:
     return t.pin_memory()
 
 
-def make_ctx(w: synth.Workload, use_rope=True, in_dtype=B.LSP_BF16) -> B.Ctx:
+def make_ctx(w: synth.Workload, use_rope=True, in_dtype=B.LSP_BF16, **desc_kw) -> B.Ctx:
+    """desc_kw: rope_layout (0 / 1), wgrad_accumulate (bool)."""
     return B.Ctx(batch=w.batch, seq=w.seq, hidden=w.hidden, n_q_heads=w.n_q_heads, n_kv_heads=w.n_kv_heads,
                  head_dim=w.head_dim, ffn=w.ffn, rms_eps=w.rms_eps, rope_base=w.rope_base, use_rope=use_rope,
-                 in_dtype=in_dtype, device=torch.cuda.current_device())
+                 in_dtype=in_dtype, device=torch.cuda.current_device(), **desc_kw)
 
 
 class LayerBuffers:
@@ -58,11 +59,15 @@ def upload_weights(wbits: dict, dev=None) -> dict:
     return {k: bf16_to_device(v, dev) for k, v in wbits.items()}
 
 
-def run_layer(w: synth.Workload, layer: int = 0):
-    """One lsp_layer_fwd + lsp_layer_bwd on the seeded inputs of workload `w`; returns numpy float32 results."""
+def run_layer(w: synth.Workload, layer: int = 0, grads_init: dict | None = None, **desc_kw):
+    """One lsp_layer_fwd + lsp_layer_bwd on the seeded inputs of workload `w`; returns numpy float32 results.
+    grads_init: numpy fp32 arrays the gradient buffers hold before the backward (wgrad_accumulate contexts)."""
     dev = require_cuda()
-    ctx = make_ctx(w)
+    ctx = make_ctx(w, **desc_kw)
     buf = LayerBuffers(ctx, w, dev)
+    if grads_init is not None:
+        for k, v in grads_init.items():
+            buf.grads[k].copy_(torch.from_numpy(v))
     weights = upload_weights(synth.layer_weights(w, layer), dev)
     inp = synth.layer_inputs(w)
     x, dy = bf16_to_device(inp["x"], dev), bf16_to_device(inp["dy"], dev)

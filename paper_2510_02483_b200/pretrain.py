@@ -22,20 +22,26 @@ from . import dp, harness, replicas, synth
 
 class PretrainStep:
     def __init__(self, w: synth.Workload, n_layers: int, vocab: int, dev=None, weights=None, embedding=None, head=None, g_final=None,
-                 world: int = 1, group=None):
+                 world: int = 1, group=None, micro_batches: int = 1):
         """weights: optional list of per-layer dicts of bf16 bit patterns (synth.layer_weights layout); embedding / head:
         bf16 bit patterns [vocab, H]; g_final: bf16 bits [H].  Defaults: the seeded synthetic tensors of synth.py.
-        `w` is this rank's shard of the batch; world > 1: data-parallel replicas (dp.py), torch.distributed initialised."""
+        `w` is one MICRO-batch of this rank's shard; micro_batches > 1: gradient accumulation (the paper's global batch of
+        256 sequences, Table 2, does not fit one step) -- the first micro-batch overwrites the gradient buffers,
+        the others run on a second context created with wgrad_accumulate = 1; world > 1: data-parallel replicas (dp.py)."""
         self.dev = dev or harness.require_cuda()
         self.w, self.L, self.V = w, n_layers, vocab
         self.ctx = harness.make_ctx(w, in_dtype=B.LSP_F32)
+        self.n_micro = micro_batches
+        self.ctx_acc = harness.make_ctx(w, in_dtype=B.LSP_F32, wgrad_accumulate=True) if micro_batches > 1 else None
         T, H = w.tokens, w.hidden
         f32 = dict(dtype=torch.float32, device=self.dev)
         self.saved = [torch.empty(self.ctx.saved_bytes, dtype=torch.uint8, device=self.dev) for _ in range(n_layers)]
         self.ws = torch.empty(max(self.ctx.workspace_bytes, B.lsp_head_workspace_bytes(self.ctx, vocab)), dtype=torch.uint8, device=self.dev)
         self.xs = [torch.empty((T, H), **f32) for _ in range(n_layers + 1)]
         self.d = [torch.empty((T, H), **f32) for _ in range(2)]
-        self.loss = torch.zeros(1, **f32)
+        self._loss_buf = torch.zeros((micro_batches, 4), **f32)      # one 16-byte aligned slot per micro-batch
+        self.micro_losses = self._loss_buf[:, 0]
+        self.loss = self._loss_buf[0, 0:1]
         self.lse = torch.empty(T, **f32)
         self.gnorm = torch.zeros(2, **f32)
         # parameters: bf16 for the kernels, fp32 master / m / v / grad for the optimizer
@@ -71,7 +77,7 @@ class PretrainStep:
         # backward operands under the fp16 normal range; lsp_adamw_step divides it out (exact for a power-of-two T),
         # together with the number of replicas whose gradients were summed
         self.head_scale = float(T)
-        self.grad_scale = dp.global_grad_scale(T, world)
+        self.grad_scale = dp.global_grad_scale(T * micro_batches, world)
 
     def _register(self, weight, grad, decay):
         self.params.append(dict(grad=grad, master=weight.float(), m=torch.zeros_like(grad), v=torch.zeros_like(grad), weight=weight,
@@ -81,23 +87,30 @@ class PretrainStep:
     def n_params(self):
         return sum(p["master"].numel() for p in self.params)
 
-    def forward_backward(self, ids: torch.Tensor, targets: torch.Tensor, stream=None):
-        """ids, targets: int32 [T] on the device.  Leaves the loss in self.loss (device) and every gradient in place."""
-        c, L = self.ctx, self.L
+    def forward_backward(self, ids: torch.Tensor, targets: torch.Tensor, stream=None, micro: int = 0):
+        """ids, targets: int32 [T] on the device (micro-batch `micro` of n_micro).  Leaves the loss of the micro-batch in
+        self.micro_losses[micro] (device) and every gradient in place; the all-reduces of the data-parallel replicas are
+        issued during the last micro-batch's backward."""
+        c, L = (self.ctx if micro == 0 else self.ctx_acc), self.L
+        last = micro == self.n_micro - 1
+        self.loss = self._loss_buf[micro, 0:1]
         B.lsp_embed_fwd(c, ids, self.table, self.xs[0], stream)
         for l in range(L):
             B.lsp_layer_fwd(c, self.xs[l], self.layer_w[l], self.xs[l + 1], self.saved[l], self.ws, stream)
         d_in = self.d[L & 1]
         B.lsp_head_fwd_bwd(c, self.xs[L], self.g_final, self.w_head, targets, self.V, self.loss, self.lse, d_in, self.d_gfinal,
                            self.d_head, self.ws, stream, grad_scale=self.head_scale)
-        self.buckets.reduce_async(L)
+        if last:
+            self.buckets.reduce_async(L)
         for l in range(L - 1, -1, -1):
             d_out = self.d[l & 1]
             B.lsp_layer_bwd(c, self.xs[l], d_in, self.layer_w[l], self.saved[l], d_out, self.layer_g[l], self.ws, stream)
-            self.buckets.reduce_async(l)            # overlaps the next layer's backward
+            if last:
+                self.buckets.reduce_async(l)        # overlaps the next layer's backward
             d_in = d_out
         B.lsp_embed_bwd(c, ids, d_in, self.V, self.d_table, stream)
-        self.buckets.reduce_async(L + 1)
+        if last:
+            self.buckets.reduce_async(L + 1)
         return self.loss
 
     def optimizer_step(self, lr=None, stream=None, **hyper):
@@ -107,12 +120,19 @@ class PretrainStep:
                          grad_scale=self.grad_scale, stream=stream, **hyper)
 
     def step(self, ids, targets, lr=None, stream=None, **hyper):
-        self.forward_backward(ids, targets, stream)
+        """One iteration.  ids / targets: one [T] tensor each, or a list of n_micro of them (gradient accumulation)."""
+        if isinstance(ids, torch.Tensor):
+            ids, targets = [ids], [targets]
+        assert len(ids) == self.n_micro == len(targets)
+        for i, (a, b) in enumerate(zip(ids, targets)):
+            self.forward_backward(a, b, stream, micro=i)
         self.optimizer_step(lr, stream, **hyper)
-        return self.loss
+        return self.micro_losses
 
     def close(self):
         self.ctx.close()
+        if self.ctx_acc is not None:
+            self.ctx_acc.close()
 
 
 def main(argv=None):

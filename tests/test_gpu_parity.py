@@ -22,9 +22,9 @@ def gpu():
     return harness
 
 
-def oracle_shape(w, use_rope=True):
+def oracle_shape(w, use_rope=True, rope_layout=0):
     return R.LayerShape(w.batch, w.seq, w.hidden, w.n_q_heads, w.n_kv_heads, w.head_dim, w.ffn, w.rms_eps, w.rope_base,
-                        0, use_rope)
+                        rope_layout, use_rope)
 
 
 def f64(d):
@@ -166,6 +166,35 @@ def test_layer_bit_reproducible(gpu):
     b = gpu.run_layer(MID)
     for n in ALL:
         assert np.array_equal(a[n], b[n]), n
+
+
+@pytest.mark.parametrize("w", [synth.CFG1_TINY, MID], ids=lambda w: w.name)
+def test_layer_rope_half_split_layout(gpu, w):
+    """rope_layout = 1 (pairs (i, i + d/2), the other common RoPE convention) against the oracle's layout-1 path: the
+    library permutes the rows of Wq / Wk per head on the way to the tensor core and un-permutes dWq / dWk through a 4-D
+    store map; head_dim 64 (cfg1) and 128."""
+    got = gpu.run_layer(w, rope_layout=1)
+    inp, wt = f64(synth.layer_inputs(w)), f64(synth.layer_weights(w))
+    ref = R.layer_fwd_bwd(inp["x"], inp["dy"], wt, oracle_shape(w, rope_layout=1))
+    check(got, ref, ALL)
+    other = R.layer_fwd_bwd(inp["x"], inp["dy"], wt, oracle_shape(w, rope_layout=0))
+    assert norm_err(other["dwq"], ref["dwq"]) > 0.1          # the two layouts are different functions of the same weights
+
+
+@pytest.mark.parametrize("w", [synth.CFG1_TINY, MID], ids=lambda w: w.name)
+def test_layer_wgrad_accumulate(gpu, w):
+    """wgrad_accumulate = 1: every weight / gain gradient buffer ends as fl32(G0 + g), g the gradient the overwrite mode
+    stores -- one fp32 add per element (TMA reduce-add stores, the per-thread path of ragged splits at cfg1, the gain
+    column sums), so the comparison is bit-exact; y and dx do not change.  Both RoPE layouts' store maps are covered."""
+    rng = np.random.default_rng([2510, 2483, 99])
+    for layout in (0, 1):
+        base = gpu.run_layer(w, rope_layout=layout)
+        g0 = {k: (rng.standard_normal(base["d" + k].shape) * float(np.sqrt(np.mean(base["d" + k] ** 2)))).astype(np.float32)
+              for k in synth.WEIGHT_NAMES}
+        got = gpu.run_layer(w, rope_layout=layout, wgrad_accumulate=True, grads_init=g0)
+        assert np.array_equal(got["y"], base["y"]) and np.array_equal(got["dx"], base["dx"])
+        for k in synth.WEIGHT_NAMES:
+            assert np.array_equal(got["d" + k], g0[k] + base["d" + k]), (layout, k)
 
 
 def test_layer_step_host_matches_device_path(gpu):
@@ -518,4 +547,37 @@ def test_pretrain_iterations_vs_oracle(gpu):
             assert norm_err(p["m"].cpu().numpy(), m_ref[i]) < 5e-5 and norm_err(p["v"].cpu().numpy(), v_ref[i]) < 5e-5, (it, tags[i])
     print("losses", losses)
     assert losses[0] > losses[1] > losses[2]
+    run.close()
+
+
+def test_pretrain_micro_batches_vs_oracle(gpu):
+    """Gradient accumulation: one iteration over 2 micro-batches of 2 sequences (second context with wgrad_accumulate = 1:
+    layers, head, final gain, embedding table all add) against the fp64 oracle on the 4-sequence batch: the mean of the
+    micro-batch losses, every gradient of the model (bar 2e-2) and the global norm (5e-3)."""
+    import torch
+    from oracle import adamw_ref as A
+    from paper_2510_02483_b200 import pretrain
+    w = synth.Workload("pretrain_micro", 10, 2, 192, 256, 4, 2, 128, 688, 1e-5, 500000.0, 2, 1000)
+    V, L, n_micro = w.vocab, w.n_layers, 2
+    run = pretrain.PretrainStep(w, L, V, micro_batches=n_micro)
+    w_all = w.with_(batch=w.batch * n_micro)
+    ids = synth.stack_inputs(w_all)["ids"]; targets = np.roll(ids, -1)
+    T = w.tokens
+    names = list(synth.WEIGHT_NAMES)
+    host = [p["weight"].float().cpu().numpy().astype(np.float64) for p in run.params]
+    run.step([torch.from_numpy(ids[i * T:(i + 1) * T].copy()).cuda() for i in range(n_micro)],
+             [torch.from_numpy(targets[i * T:(i + 1) * T].copy()).cuda() for i in range(n_micro)], lr=1e-3)
+    torch.cuda.synchronize()
+    layers = [dict(zip(names, host[9 * l:9 * l + 9])) for l in range(L)]
+    loss_ref, lg, dE, dWh, dgf = _oracle_model_grads(ids, targets, layers, host[9 * L], host[9 * L + 1], host[9 * L + 2],
+                                                     oracle_shape(w_all), V)
+    loss = float(run.micro_losses.mean().cpu())
+    assert abs(loss - loss_ref) <= 1e-3 * abs(loss_ref), (loss, loss_ref)
+    assert run.grad_scale == float(T * n_micro)
+    ref_g = [lg[l][k] for l in range(L) for k in names] + [dE, dWh, dgf]
+    got_g = [p["grad"].cpu().numpy().astype(np.float64) / run.grad_scale for p in run.params]
+    tags = [f"L{l}.d{k}" for l in range(L) for k in names] + ["d_table", "d_head", "d_gfinal"]
+    check(dict(zip(tags, got_g)), dict(zip(tags, ref_g)), tags)
+    norm_ref = A.global_grad_norm(ref_g)
+    assert abs(float(run.gnorm[0].cpu()) - norm_ref) <= 5e-3 * norm_ref
     run.close()
