@@ -57,6 +57,10 @@ typedef struct {
   int32_t in_dtype;         /* lsp_dtype of x / a / dy / da inputs */
   int32_t wgrad_accumulate; /* 0 = overwrite the nine weight / gain gradients; 1 = add to what the buffers hold
                              * (micro-batch gradient accumulation: one fp32 add per element, bit-reproducible) */
+  int32_t head_dim_logical; /* 0 = head_dim.  Otherwise an even width < head_dim of heads the caller ZERO-PADS to head_dim
+                             * (e.g. 104 -> 128, Table 1 30B: hidden 6656 / 64 heads): rows of wq/wk/wv and columns
+                             * of wo beyond it are zero in every head; softmax scale 1/sqrt(logical) and RoPE frequencies
+                             * base^(-2i/logical), identity on the padding (rope_layout 0 only) */
 } lsp_layer_desc;
 
 typedef struct {

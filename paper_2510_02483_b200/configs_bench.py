@@ -1,6 +1,6 @@
 """Device-side timing of every BASELINE.json configuration (bench.py covers the headline config 2 only).
 
-    python -m paper_2510_02483_b200.configs_bench [--steps K] [--only cfg2,cfg3,cfg4,cfg5,table1,adamw,head]
+    python -m paper_2510_02483_b200.configs_bench [--steps K] [--only cfg2,cfg3,cfg4,cfg5,table1,table1_30b,adamw,head]
 
 Prints one JSON line per configuration: ms per fwd+bwd step (CUDA events on the launching stream, after warm-up),
 tokens/s and executed TFLOP/s (causal attention FLOPs, SURVEY.md 8(d) convention).  Inputs are the seeded synthetic
@@ -31,11 +31,21 @@ def _time(fn, steps, warmup=3):
     return e0.elapsed_time(e1) / steps
 
 
-def bench_layer(w, steps):
+def bench_layer(w, steps, logical_head_dim=0):
+    """logical_head_dim: the workload's heads are that wide, zero-padded to w.head_dim (lsp_layer_desc.head_dim_logical);
+    the FLOPs returned are the LOGICAL ones (the padding is overhead, not work)."""
     dev = harness.require_cuda()
-    ctx = harness.make_ctx(w)
+    ctx = harness.make_ctx(w, head_dim_logical=logical_head_dim)
     buf = harness.LayerBuffers(ctx, w, dev)
-    weights = harness.upload_weights(synth.layer_weights(w), dev)
+    if logical_head_dim:
+        wl = w.with_(head_dim=logical_head_dim)
+        bits = synth.layer_weights(wl)
+        for k, n in dict(wq=w.n_q_heads, wk=w.n_kv_heads, wv=w.n_kv_heads, wo=w.n_q_heads).items():
+            bits[k] = harness.pad_heads(bits[k], k, n, logical_head_dim, w.head_dim)
+        weights = harness.upload_weights(bits, dev)
+    else:
+        wl = w
+        weights = harness.upload_weights(synth.layer_weights(w), dev)
     inp = synth.layer_inputs(w)
     x, dy = harness.bf16_to_device(inp["x"], dev), harness.bf16_to_device(inp["dy"], dev)
 
@@ -44,7 +54,7 @@ def bench_layer(w, steps):
         B.lsp_layer_bwd(ctx, x, dy, weights, buf.saved, buf.dx, buf.grads, buf.ws)
     ms = _time(step, steps)
     ctx.close()
-    return ms, synth.layer_flops(w, causal=True)
+    return ms, synth.layer_flops(wl, causal=True)
 
 
 def bench_stack(w, steps):
@@ -133,7 +143,7 @@ def bench_head(w, steps):
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--only", default="cfg2,cfg3,cfg4,cfg5,table1,adamw,head")
+    ap.add_argument("--only", default="cfg2,cfg3,cfg4,cfg5,table1,table1_30b,adamw,head")
     args = ap.parse_args(argv)
     B.lib()
     only = set(args.only.split(","))
@@ -144,6 +154,9 @@ def main(argv=None):
         jobs.append((synth.CFG4_30B_LAYER, bench_layer))
     if "table1" in only:      # the paper's own Table-1 3B layer shape: hidden 2048, 16q / 2kv, FFN 11008
         jobs.append((synth.Workload("table1_3b_layer", 6, 4, 4096, 2048, 16, 2, 128, 11008, 1e-5, 10000.0), bench_layer))
+    if "table1_30b" in only:  # Table-1 30B layer as printed: hidden 6656, 64 MHA heads of width 104 (zero-padded to 128), FFN 17920
+        w30 = synth.Workload("table1_30b_layer_64x104_padded", 7, 2, 4096, 6656, 64, 64, 128, 17920, 1e-5, 10000.0)
+        jobs.append((w30, lambda w, steps: bench_layer(w, steps, logical_head_dim=104)))
     if "cfg3" in only:
         jobs.append((synth.CFG3_3B_STACK, bench_stack))
     if "cfg5" in only:

@@ -37,6 +37,9 @@ struct WsLayout {
 
 }  // namespace
 
+// softmax scale and RoPE frequencies follow the logical head width (zero-padded heads: head_dim_logical < head_dim)
+static inline int logical_head_dim(const lsp_layer_desc& d) { return d.head_dim_logical > 0 ? d.head_dim_logical : d.head_dim; }
+
 // Pipeline stages (for launch counting and the optional per-stage device timing of lsp_timing_*).
 enum Stage : int {
   ST_CAST = 0, ST_NORM_FWD, ST_QKV, ST_ATTN_FWD, ST_OPROJ, ST_GATEUP, ST_DOWN,
@@ -355,7 +358,7 @@ lsp_status attn_fwd_impl(lsp_ctx* ctx, int x_dt, const void* x, const lsp_layer_
   p.q = qkv; p.k = qkv + Nq; p.v = qkv + Nq + Nkv;
   p.ldq = p.ldk = p.ldv = Nqkv;
   p.B = d.batch; p.S = d.seq; p.nq = d.n_q_heads; p.nkv = d.n_kv_heads;
-  p.scale = 1.0f / sqrtf(static_cast<float>(d.head_dim));
+  p.scale = 1.0f / sqrtf(static_cast<float>(logical_head_dim(d)));
   p.scale_log2 = p.scale * 1.4426950408889634f;
   p.o32 = o32; p.o16 = o16; p.ldo = Nq; p.lse = lse;
   LSP_STAGE(ST_ATTN_FWD, 1, attn_fwd_dispatch(ctx, p, st));
@@ -400,7 +403,7 @@ lsp_status attn_bwd_impl(lsp_ctx* ctx, int x_dt, const void* x, int da_dt, const
   p.q = qkv; p.k = qkv + Nq; p.v = qkv + Nq + Nkv; p.dO = dO16;
   p.ldq = p.ldk = p.ldv = Nqkv; p.lddo = Nq;
   p.B = d.batch; p.S = d.seq; p.nq = d.n_q_heads; p.nkv = d.n_kv_heads;
-  p.scale = 1.0f / sqrtf(static_cast<float>(d.head_dim));
+  p.scale = 1.0f / sqrtf(static_cast<float>(logical_head_dim(d)));
   p.scale_log2 = p.scale * 1.4426950408889634f;
   p.lse = const_cast<float*>(lse); p.dvec = dvec;
   p.rope = d.use_rope ? ctx->rope : nullptr;
@@ -519,6 +522,9 @@ lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device
   if (d.batch <= 0 || d.seq <= 0 || d.hidden <= 0 || d.n_q_heads <= 0 || d.n_kv_heads <= 0 || d.ffn <= 0) return LSP_EINVAL;
   if (d.n_q_heads % d.n_kv_heads != 0) return LSP_EINVAL;
   if (d.head_dim != 64 && d.head_dim != 128) return LSP_EUNSUPPORTED;
+  if (d.head_dim_logical != 0 && (d.head_dim_logical < 2 || d.head_dim_logical > d.head_dim || (d.head_dim_logical & 1) ||
+                                  (d.head_dim_logical != d.head_dim && d.rope_layout != 0)))
+    return LSP_EUNSUPPORTED;
   if (d.hidden % 8 || d.ffn % 8 || d.hidden > 8192) return LSP_EUNSUPPORTED;
   if ((d.rope_layout != 0 && d.rope_layout != 1) || (d.wgrad_accumulate != 0 && d.wgrad_accumulate != 1)) return LSP_EUNSUPPORTED;
   if (d.in_dtype != LSP_BF16 && d.in_dtype != LSP_F32) return LSP_EINVAL;
@@ -550,11 +556,12 @@ lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device
   plan_layout(ctx);
 
   // RoPE table: theta = pos * base^(-2i/d) in fp64 (reading A-5), stored as fp32 (cos, sin)
-  const int half = d.head_dim / 2;
+  // head_dim_logical < head_dim (zero-padded heads): frequencies of the logical width, identity on the padding pairs
+  const int half = d.head_dim / 2, dl = logical_head_dim(d);
   std::vector<float2> tab(static_cast<size_t>(d.seq) * half);
   for (int p = 0; p < d.seq; ++p)
     for (int i = 0; i < half; ++i) {
-      const double th = static_cast<double>(p) * pow(d.rope_base, -2.0 * i / d.head_dim);
+      const double th = 2 * i < dl ? static_cast<double>(p) * pow(d.rope_base, -2.0 * i / dl) : 0.0;
       tab[static_cast<size_t>(p) * half + i] = make_float2(static_cast<float>(cos(th)), static_cast<float>(sin(th)));
     }
   if (cudaMalloc(&ctx->rope, tab.size() * sizeof(float2)) != cudaSuccess) { delete ctx; return LSP_ENOMEM; }
@@ -687,7 +694,7 @@ lsp_status lsp_sdpa_fwd(lsp_ctx* ctx, const void* q, const void* k, const void* 
   p.q = q16; p.k = k16; p.v = v16;
   p.ldq = ctx->Nq; p.ldk = p.ldv = ctx->Nkv;
   p.B = d.batch; p.S = d.seq; p.nq = d.n_q_heads; p.nkv = d.n_kv_heads;
-  p.scale = 1.0f / sqrtf(static_cast<float>(d.head_dim));
+  p.scale = 1.0f / sqrtf(static_cast<float>(logical_head_dim(d)));
   p.scale_log2 = p.scale * 1.4426950408889634f;
   p.o32 = static_cast<float*>(o); p.ldo = ctx->Nq; p.lse = lse;
   LSP_STAGE(ST_ATTN_FWD, 1, attn_fwd_dispatch(ctx, p, st));
@@ -718,7 +725,7 @@ lsp_status lsp_sdpa_bwd(lsp_ctx* ctx, const void* q, const void* k, const void* 
   p.q = q16; p.k = k16; p.v = v16; p.dO = dO16;
   p.ldq = ctx->Nq; p.ldk = p.ldv = ctx->Nkv; p.lddo = ctx->Nq;
   p.B = d.batch; p.S = d.seq; p.nq = d.n_q_heads; p.nkv = d.n_kv_heads;
-  p.scale = 1.0f / sqrtf(static_cast<float>(d.head_dim));
+  p.scale = 1.0f / sqrtf(static_cast<float>(logical_head_dim(d)));
   p.scale_log2 = p.scale * 1.4426950408889634f;
   p.lse = const_cast<float*>(lse); p.dvec = dvec;
   p.dq32 = static_cast<float*>(dq); p.dk32 = static_cast<float*>(dk); p.dv32 = static_cast<float*>(dv);

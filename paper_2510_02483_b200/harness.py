@@ -59,7 +59,28 @@ def upload_weights(wbits: dict, dev=None) -> dict:
     return {k: bf16_to_device(v, dev) for k, v in wbits.items()}
 
 
-def run_layer(w: synth.Workload, layer: int = 0, grads_init: dict | None = None, **desc_kw):
+def pad_heads(t: np.ndarray, name: str, n_heads: int, d: int, d_pad: int) -> np.ndarray:
+    """Zero-pad every head of a projection tensor from width d to d_pad (lsp_layer_desc.head_dim_logical): rows of
+    wq / wk / wv ([heads*d, H]), columns of wo ([H, heads*d]).  Works on weights (uint16 bf16 bits) and gradients."""
+    if name == "wo":
+        out = np.zeros((t.shape[0], n_heads, d_pad), t.dtype)
+        out[:, :, :d] = t.reshape(t.shape[0], n_heads, d)
+        return out.reshape(t.shape[0], n_heads * d_pad)
+    out = np.zeros((n_heads, d_pad, t.shape[1]), t.dtype)
+    out[:, :d, :] = t.reshape(n_heads, d, t.shape[1])
+    return out.reshape(n_heads * d_pad, t.shape[1])
+
+
+def unpad_heads(t: np.ndarray, name: str, n_heads: int, d: int, d_pad: int):
+    """Inverse of pad_heads; returns (unpadded tensor, the padding part) so callers can check that the padding is zero."""
+    if name == "wo":
+        v = t.reshape(t.shape[0], n_heads, d_pad)
+        return v[:, :, :d].reshape(t.shape[0], n_heads * d), v[:, :, d:]
+    v = t.reshape(n_heads, d_pad, t.shape[1])
+    return v[:, :d, :].reshape(n_heads * d, t.shape[1]), v[:, d:, :]
+
+
+def run_layer(w: synth.Workload, layer: int = 0, grads_init: dict | None = None, weights_bits: dict | None = None, **desc_kw):
     """One lsp_layer_fwd + lsp_layer_bwd on the seeded inputs of workload `w`; returns numpy float32 results.
     grads_init: numpy fp32 arrays the gradient buffers hold before the backward (wgrad_accumulate contexts)."""
     dev = require_cuda()
@@ -68,7 +89,7 @@ def run_layer(w: synth.Workload, layer: int = 0, grads_init: dict | None = None,
     if grads_init is not None:
         for k, v in grads_init.items():
             buf.grads[k].copy_(torch.from_numpy(v))
-    weights = upload_weights(synth.layer_weights(w, layer), dev)
+    weights = upload_weights(weights_bits if weights_bits is not None else synth.layer_weights(w, layer), dev)
     inp = synth.layer_inputs(w)
     x, dy = bf16_to_device(inp["x"], dev), bf16_to_device(inp["dy"], dev)
     B.lsp_layer_fwd(ctx, x, weights, buf.y, buf.saved, buf.ws)

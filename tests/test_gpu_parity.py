@@ -197,6 +197,27 @@ def test_layer_wgrad_accumulate(gpu, w):
             assert np.array_equal(got["d" + k], g0[k] + base["d" + k]), (layout, k)
 
 
+def test_layer_padded_heads_104(gpu):
+    """PAPER.md Table 1, 30B row: hidden 6656 / 64 heads = head_dim 104 (reading A-15).  The caller zero-pads every head
+    to 128 and sets head_dim_logical = 104 (softmax scale 1/sqrt(104), RoPE frequencies base^(-2i/104)); results against
+    the oracle run at head_dim 104 itself, at a reduced width (hidden 512, 4q / 2kv heads), and the gradient of every
+    padding row / column must be exactly zero."""
+    wl = synth.Workload("pad104", 104, 2, 320, 512, 4, 2, 104, 1376, 1e-5, 10000.0)
+    wp = wl.with_(head_dim=128)
+    bits = synth.layer_weights(wl)
+    heads = dict(wq=wl.n_q_heads, wk=wl.n_kv_heads, wv=wl.n_kv_heads, wo=wl.n_q_heads)
+    padded = dict(bits)
+    for k, n in heads.items():
+        padded[k] = gpu.pad_heads(bits[k], k, n, 104, 128)
+    got = gpu.run_layer(wp, weights_bits=padded, head_dim_logical=104)
+    for k, n in heads.items():
+        got["d" + k], pad = gpu.unpad_heads(got["d" + k], k, n, 104, 128)
+        assert not np.any(pad), k
+    inp = f64(synth.layer_inputs(wl))
+    ref = R.layer_fwd_bwd(inp["x"], inp["dy"], f64(bits), oracle_shape(wl))
+    check(got, ref, ALL)
+
+
 def test_layer_step_host_matches_device_path(gpu):
     """lsp_layer_step_host (pinned HOST x, dy in; y, dx out; copies on context-owned streams overlapping the compute
     stream) returns exactly what lsp_layer_fwd + lsp_layer_bwd produce from device-resident inputs."""
