@@ -251,6 +251,23 @@ def run_ours(args):
     e2e_value, _, _ = replicas.whole_job_throughput(float(w.tokens) * Ke, e0.elapsed_time(e1), dev)
     h2d, d2h = 2 * n * 2, 2 * n * 4
 
+    # ------------------------------------------------------------------ per-step distribution, forward and backward apart
+    # (SURVEY.md 8(d) timing protocol: median / min / p90; a separate pass, the headline above is the bracketed K steps)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * K + 1)]
+    ev[0].record(stream)
+    for i in range(K):
+        B.lsp_layer_fwd(ctx, x, weights, buf.y, buf.saved, buf.ws, stream)
+        ev[2 * i + 1].record(stream)
+        B.lsp_layer_bwd(ctx, x, dy, weights, buf.saved, buf.dx, buf.grads, buf.ws, stream)
+        ev[2 * i + 2].record(stream)
+    torch.cuda.synchronize()
+    fwd_ms = sorted(ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(K))
+    bwd_ms = sorted(ev[2 * i + 1].elapsed_time(ev[2 * i + 2]) for i in range(K))
+    tot_ms = sorted(ev[2 * i].elapsed_time(ev[2 * i + 2]) for i in range(K))
+    pick = lambda v, q: v[min(len(v) - 1, int(q * len(v)))]
+    per_step = {"median": round(pick(tot_ms, 0.5), 4), "min": round(tot_ms[0], 4), "p90": round(pick(tot_ms, 0.9), 4),
+                "fwd_median": round(pick(fwd_ms, 0.5), 4), "bwd_median": round(pick(bwd_ms, 0.5), 4)}
+
     # ------------------------------------------------------------------ per-stage device times (roofline of the GEMM kernel)
     B.lsp_timing_enable(ctx, K * 64)
     for _ in range(K):
@@ -294,7 +311,7 @@ def run_ours(args):
             "frac_of_measured_burst": tflops / renv.world_size / peaks["bf16_tflops"],
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": "tokens/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": Ke},
-            "gpu_launches": int(launches), "roofline": roofline}
+            "gpu_launches": int(launches), "per_step_ms": per_step, "roofline": roofline}
 
     if renv.is_main and renv.world_size == 1 and not args.no_cpu_baseline:
         tps, dt, sample = time_oracle(w, 3, 1)

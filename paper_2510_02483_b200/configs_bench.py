@@ -1,6 +1,6 @@
 """Device-side timing of every BASELINE.json configuration (bench.py covers the headline config 2 only).
 
-    python -m paper_2510_02483_b200.configs_bench [--steps K] [--only cfg2,cfg3,cfg4,cfg5,table1,table1_30b,adamw,head]
+    python -m paper_2510_02483_b200.configs_bench [--steps K] [--only cfg2,fwd,cfg3,cfg4,cfg5,table1,table1_30b,adamw,head]
 
 Prints one JSON line per configuration: ms per fwd+bwd step (CUDA events on the launching stream, after warm-up),
 tokens/s and executed TFLOP/s (causal attention FLOPs, SURVEY.md 8(d) convention).  Inputs are the seeded synthetic
@@ -55,6 +55,18 @@ def bench_layer(w, steps, logical_head_dim=0):
     ms = _time(step, steps)
     ctx.close()
     return ms, synth.layer_flops(wl, causal=True)
+
+
+def bench_layer_fwd_only(w, steps):
+    """Forward pass alone (SURVEY.md 8(f) #3: the forward-only variant, prefill-style): lsp_layer_fwd, device-resident."""
+    dev = harness.require_cuda()
+    ctx = harness.make_ctx(w)
+    buf = harness.LayerBuffers(ctx, w, dev)
+    weights = harness.upload_weights(synth.layer_weights(w), dev)
+    x = harness.bf16_to_device(synth.layer_inputs(w)["x"], dev)
+    ms = _time(lambda: B.lsp_layer_fwd(ctx, x, weights, buf.y, buf.saved, buf.ws), steps)
+    ctx.close()
+    return ms, synth.layer_flops(w, causal=True) / 3.0 - synth.attn_flops_fwd(w, causal=True) * (3.5 / 3.0 - 1.0)
 
 
 def bench_stack(w, steps):
@@ -143,13 +155,15 @@ def bench_head(w, steps):
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--only", default="cfg2,cfg3,cfg4,cfg5,table1,table1_30b,adamw,head")
+    ap.add_argument("--only", default="cfg2,fwd,cfg3,cfg4,cfg5,table1,table1_30b,adamw,head")
     args = ap.parse_args(argv)
     B.lib()
     only = set(args.only.split(","))
     jobs = []
     if "cfg2" in only:
         jobs.append((synth.CFG2_3B_LAYER, bench_layer))
+    if "fwd" in only:
+        jobs.append((synth.CFG2_3B_LAYER.with_(name="cfg2_3b_layer_forward_only"), bench_layer_fwd_only))
     if "cfg4" in only:
         jobs.append((synth.CFG4_30B_LAYER, bench_layer))
     if "table1" in only:      # the paper's own Table-1 3B layer shape: hidden 2048, 16q / 2kv, FFN 11008

@@ -151,7 +151,7 @@ void plan_layout(lsp_ctx* c) {
   w.dO16 = take(T * Nq * 2);
   w.dvec = take(BnqS * 4);
   w.dqkv16 = take(T * Nqkv * 2);
-  w.dgpart = take(static_cast<size_t>(c->norm_blocks) * H * 4);
+  w.dgpart = take(static_cast<size_t>(c->norm_blocks) * 2 * H * 4);      // one row per (CTA, row group) of rmsnorm_bwd_kernel
   w.q16 = take(T * Nq * 2);
   w.k16 = take(T * c->Nkv * 2);
   w.v16 = take(T * c->Nkv * 2);
@@ -181,7 +181,10 @@ cudaError_t norm_fwd(const lsp_ctx* c, int dt, const void* x, const void* g, __h
 template <typename XT, typename RT>
 cudaError_t norm_bwd_t(const lsp_ctx* c, const void* x, const float* rstd, const void* g, const float* dxn, const void* dres,
                        float* dx, __half* dx16, float* dg_part, float* dg, int dg_accumulate, cudaStream_t st) {
-  const int H = c->d.hidden, nv = (H / 4 + NORMB_CONSUMERS - 1) / NORMB_CONSUMERS;
+  const int H = c->d.hidden;
+  // two row groups of 128 threads while a row is at most 8 float4 per thread (H <= 4096), else one group of 256
+  const int G = (H / 4 + 127) / 128 <= 8 ? 2 : 1;
+  const int gt = NORMB_CONSUMERS / G, nv = (H / 4 + gt - 1) / gt;
   const XT* xp = static_cast<const XT*>(x);
   const RT* rp = static_cast<const RT*>(dres);
   const __nv_bfloat16* gp = static_cast<const __nv_bfloat16*>(g);
@@ -191,16 +194,20 @@ cudaError_t norm_bwd_t(const lsp_ctx* c, const void* x, const float* rstd, const
   if (stages > NORMB_MAX_STAGES) stages = NORMB_MAX_STAGES;
   if (stages < 2) return cudaErrorInvalidValue;
   const size_t smem = stages * stage_bytes;
-#define LSP_NB(NV) case NV: { \
-    auto kern = rmsnorm_bwd_kernel<XT, RT, NV>; \
+#define LSP_NB(NV, GG) case NV: { \
+    auto kern = rmsnorm_bwd_kernel<XT, RT, NV, GG>; \
     static bool set = false; \
     if (!set) { cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, NORMB_SMEM_BUDGET); if (e != cudaSuccess) return e; set = true; } \
     kern<<<nb, NORMB_THREADS, smem, st>>>(xp, rstd, gp, dxn, rp, dx, dx16, dg_part, c->T, H, stages); } break;
-  switch (nv) { LSP_NB(1) LSP_NB(2) LSP_NB(3) LSP_NB(4) LSP_NB(5) LSP_NB(6) LSP_NB(7) LSP_NB(8) default: return cudaErrorInvalidValue; }
+  if (G == 2) {
+    switch (nv) { LSP_NB(1, 2) LSP_NB(2, 2) LSP_NB(3, 2) LSP_NB(4, 2) LSP_NB(5, 2) LSP_NB(6, 2) LSP_NB(7, 2) LSP_NB(8, 2) default: return cudaErrorInvalidValue; }
+  } else {
+    switch (nv) { LSP_NB(5, 1) LSP_NB(6, 1) LSP_NB(7, 1) LSP_NB(8, 1) default: return cudaErrorInvalidValue; }
+  }
 #undef LSP_NB
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  colsum_kernel<<<(H + 31) / 32, 256, 0, st>>>(dg_part, dg, nb, H, dg_accumulate);
+  colsum_kernel<<<(H + 31) / 32, 256, 0, st>>>(dg_part, dg, nb * G, H, dg_accumulate);
   return cudaGetLastError();
 }
 // x: forward input of the norm (XT = x_dt); dres: incoming residual gradient (RT = r_dt)
@@ -810,7 +817,7 @@ HeadLayout head_layout(const lsp_ctx* c, int vocab) {
   HeadLayout h;
   h.xn16 = take(T * H * 2); h.rstd = take(T * 4); h.w16 = take(V * H * 2); h.logits = take(T * V * 4);
   h.dz16 = take(T * V * 2); h.dxn32 = take(T * H * 4); h.loss_row = take(T * 4);
-  h.dgpart = take(static_cast<size_t>(c->norm_blocks) * H * 4);
+  h.dgpart = take(static_cast<size_t>(c->norm_blocks) * 2 * H * 4);
   h.total = o;
   return h;
 }

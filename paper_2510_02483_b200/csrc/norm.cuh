@@ -75,7 +75,8 @@ __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_fwd_kernel(const XT* __r
 // HBM-bound (x, dxn, dres read once, dx written once: 43-49 kB per token at H = 3072).  One persistent CTA per SM;
 // a producer warp streams whole rows of the three inputs into a shared-memory ring with 1-D bulk async copies
 // (cp.async.bulk, completion on an mbarrier), so ~150 KB per SM are in flight regardless of what the 8 consumer
-// warps are doing; the consumers read their columns from shared memory, reduce the row dot product, and store dx
+// warps are doing; the consumers (two row groups of 4 warps when the row fits 8 float4 per thread, else one group of 8)
+// read their columns from shared memory, reduce the row dot product, and store dx
 // (and its fp16 copy) straight from registers.  Each thread keeps its columns' dg partials in registers over all
 // rows of the CTA; colsum_kernel adds the per-CTA partials in a fixed order (deterministic, no atomics).
 constexpr int NORMB_CONSUMERS = 256;                       // 8 consumer warps
@@ -99,27 +100,29 @@ template <> __device__ __forceinline__ float4 lds_vec4<__nv_bfloat16>(const uint
   return make_float4(bf16_lo(u.x), bf16_hi(u.x), bf16_lo(u.y), bf16_hi(u.y));
 }
 
-// sum over the 256 consumer threads (named barrier 1; the producer warp never joins it)
-__device__ __forceinline__ float consumer_sum(float v, float* red) {
+// sum over the `nthreads` consumer threads of one row group (named barrier `bar_id`; the producer warp never joins it)
+__device__ __forceinline__ float consumer_sum(float v, float* red, int bar_id, int nthreads, int warp_in_group) {
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  named_bar_sync(1, NORMB_CONSUMERS);         // protect `red` from the previous row
-  if (lane == 0) red[warp] = v;
-  named_bar_sync(1, NORMB_CONSUMERS);
-  float t = (lane < NORMB_CONSUMERS / 32) ? red[lane] : 0.f;
-#pragma unroll
-  for (int off = 4; off > 0; off >>= 1) t += __shfl_xor_sync(0xffffffffu, t, off);
-  return __shfl_sync(0xffffffffu, t, 0);
+  const int lane = threadIdx.x & 31;
+  named_bar_sync(bar_id, nthreads);           // protect `red` from the previous row
+  if (lane == 0) red[warp_in_group] = v;
+  named_bar_sync(bar_id, nthreads);
+  float t = 0.f;
+  for (int k = 0; k < nthreads / 32; ++k) t += red[k];       // fixed order
+  return t;
 }
 
-template <typename XT, typename RT, int NV>
+template <typename XT, typename RT, int NV, int G>
 __global__ void __launch_bounds__(NORMB_THREADS, 1)
 rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, const __nv_bfloat16* __restrict__ g,
                    const float* __restrict__ dxn, const RT* __restrict__ dres, float* __restrict__ dx,
                    __half* __restrict__ dx16, float* __restrict__ dg_part, int T, int H, int stages) {
+  // G row groups of GT = 256 / G consumer threads: group q takes this CTA's rows q, q + G, ... so that the reduction
+  // latency of one row (shuffles, two named barriers) overlaps the loads and stores of the other group's row.
+  constexpr int GT = NORMB_CONSUMERS / G;
   extern __shared__ __align__(128) uint8_t nsm[];
-  __shared__ float red[NORMB_CONSUMERS / 32];
+  __shared__ float red[G][GT / 32];
   __shared__ __align__(8) unsigned long long bars[2 * NORMB_MAX_STAGES];
   // dres may be null (no residual gradient: the final norm before the LM head)
   const uint32_t xb = static_cast<uint32_t>(H) * sizeof(XT), db = static_cast<uint32_t>(H) * 4u,
@@ -129,7 +132,7 @@ rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, con
   auto full = [&](int s) { return smem_u32(&bars[s]); };
   auto empty = [&](int s) { return smem_u32(&bars[NORMB_MAX_STAGES + s]); };
   if (threadIdx.x == 0) {
-    for (int s = 0; s < stages; ++s) { mbar_init(full(s), 1); mbar_init(empty(s), NORMB_CONSUMERS / 32); }
+    for (int s = 0; s < stages; ++s) { mbar_init(full(s), 1); mbar_init(empty(s), GT / 32); }
     fence_barrier_init();
   }
   __syncthreads();
@@ -152,16 +155,19 @@ rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, con
     return;
   }
   // -------------------------------------------------------------------- consumers
+  const int grp = threadIdx.x / GT, tg = threadIdx.x - grp * GT;
   float4 gg[NV], acc[NV];
 #pragma unroll
   for (int i = 0; i < NV; ++i) {
-    const int c = (threadIdx.x + i * NORMB_CONSUMERS) * 4;
+    const int c = (tg + i * GT) * 4;
     acc[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     gg[i] = (c < H) ? Vec4<__nv_bfloat16>::load(g + c) : make_float4(0.f, 0.f, 0.f, 0.f);
   }
   const float invH = 1.0f / static_cast<float>(H);
-  int s = 0; uint32_t ph = 0;
-  for (long long row = blockIdx.x; row < T; row += gridDim.x) {
+  long long k = grp;                                          // index of the row among this CTA's rows
+  for (long long row = blockIdx.x + static_cast<long long>(grp) * gridDim.x; row < T; row += static_cast<long long>(G) * gridDim.x, k += G) {
+    const int s = static_cast<int>(k % stages);
+    const uint32_t ph = static_cast<uint32_t>(k / stages) & 1u;
     const float r = rstd[row];
     mbar_wait(full(s), ph);
     const uint8_t* sx = nsm + static_cast<size_t>(s) * stage_bytes;
@@ -171,7 +177,7 @@ rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, con
     float dot = 0.f;
 #pragma unroll
     for (int i = 0; i < NV; ++i) {
-      const int c = (threadIdx.x + i * NORMB_CONSUMERS) * 4;
+      const int c = (tg + i * GT) * 4;
       if (c < H) {
         const float4 xv = lds_vec4<XT>(sx, c);
         const float4 d = lds_vec4<float>(sd, c);
@@ -184,11 +190,10 @@ rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, con
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(empty(s));                    // this warp has read its part of the stage
-    if (++s == stages) { s = 0; ph ^= 1u; }
-    dot = consumer_sum(dot, red) * invH;
+    dot = consumer_sum(dot, red[grp], 1 + grp, GT, tg >> 5) * invH;
 #pragma unroll
     for (int i = 0; i < NV; ++i) {
-      const int c = (threadIdx.x + i * NORMB_CONSUMERS) * 4;
+      const int c = (tg + i * GT) * 4;
       if (c < H) {
         float4 o;
         o.x = rs[i].x + r * (dn[i].x - n[i].x * dot);
@@ -200,10 +205,11 @@ rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, con
       }
     }
   }
+  // one row of dg partials per (CTA, group)
 #pragma unroll
   for (int i = 0; i < NV; ++i) {
-    const int c = (threadIdx.x + i * NORMB_CONSUMERS) * 4;
-    if (c < H) *reinterpret_cast<float4*>(dg_part + static_cast<long long>(blockIdx.x) * H + c) = acc[i];
+    const int c = (tg + i * GT) * 4;
+    if (c < H) *reinterpret_cast<float4*>(dg_part + (static_cast<long long>(blockIdx.x) * G + grp) * H + c) = acc[i];
   }
 }
 
@@ -252,22 +258,42 @@ struct CastSegs {
   unsigned perm_mask;        // segments whose ROWS are permuted on the way: dst row head*d + 2i + half = src row head*d + half*d/2 + i
   int perm_d, row_units;     // head_dim; 16-byte units per row (in-features / 8)
 };
-__global__ void cast_multi_bf16_f16_kernel(const CastSegs segs) {
-  const long long total = segs.start[segs.nseg];
-  for (long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i < total; i += static_cast<long long>(gridDim.x) * blockDim.x) {
-    int s = 0;
+__device__ __forceinline__ long long cast_src_unit(const CastSegs& segs, long long i, int& s) {
+  s = 0;
 #pragma unroll
-    for (int k = 1; k < CAST_MAX_SEGS; ++k) s += (k < segs.nseg && i >= segs.start[k]) ? 1 : 0;
-    const long long j = i - segs.start[s];
-    long long js = j;
-    if ((segs.perm_mask >> s) & 1u) {
-      const long long row = j / segs.row_units;
-      const int p = static_cast<int>(row % segs.perm_d);
-      js = (row - p + (p & 1) * (segs.perm_d >> 1) + (p >> 1)) * segs.row_units + (j - row * segs.row_units);
+  for (int k = 1; k < CAST_MAX_SEGS; ++k) s += (k < segs.nseg && i >= segs.start[k]) ? 1 : 0;
+  const long long j = i - segs.start[s];
+  if ((segs.perm_mask >> s) & 1u) {
+    const long long row = j / segs.row_units;
+    const int p = static_cast<int>(row % segs.perm_d);
+    return (row - p + (p & 1) * (segs.perm_d >> 1) + (p >> 1)) * segs.row_units + (j - row * segs.row_units);
+  }
+  return j;
+}
+// four independent 16-byte loads in flight per thread (the kernel is latency-bound otherwise: 2.7 TB/s with one)
+__global__ void __launch_bounds__(256) cast_multi_bf16_f16_kernel(const CastSegs segs) {
+  const long long total = segs.start[segs.nseg];
+  const long long stride = static_cast<long long>(gridDim.x) * blockDim.x;
+  for (long long i0 = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i0 < total; i0 += 4 * stride) {
+    uint4 u[4];
+    int sg[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const long long i = i0 + k * stride;
+      sg[k] = 0;
+      if (i < total) {
+        const long long js = cast_src_unit(segs, i, sg[k]);
+        u[k] = __ldg(reinterpret_cast<const uint4*>(segs.src[sg[k]]) + js);
+      }
     }
-    const uint4 u = __ldg(reinterpret_cast<const uint4*>(segs.src[s]) + js);
-    reinterpret_cast<uint4*>(segs.dst[s])[j] = make_uint4(pack_f16(bf16_lo(u.x), bf16_hi(u.x)), pack_f16(bf16_lo(u.y), bf16_hi(u.y)),
-                                                         pack_f16(bf16_lo(u.z), bf16_hi(u.z)), pack_f16(bf16_lo(u.w), bf16_hi(u.w)));
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const long long i = i0 + k * stride;
+      if (i < total)
+        reinterpret_cast<uint4*>(segs.dst[sg[k]])[i - segs.start[sg[k]]] =
+            make_uint4(pack_f16(bf16_lo(u[k].x), bf16_hi(u[k].x)), pack_f16(bf16_lo(u[k].y), bf16_hi(u[k].y)),
+                       pack_f16(bf16_lo(u[k].z), bf16_hi(u[k].z)), pack_f16(bf16_lo(u[k].w), bf16_hi(u[k].w)));
+    }
   }
 }
 
