@@ -139,6 +139,17 @@ lsp_status lsp_layer_step_host(lsp_ctx* ctx, const void* x_host, const void* dy_
                                void* y_host, void* dx_host, lsp_layer_wgrads* grads, void* x_dev, void* dy_dev,
                                void* y_dev, void* dx_dev, void* saved, void* ws, void* stream);
 
+/* Pipelined form of lsp_layer_step_host for a stream of steps: same arguments and results, but the call does NOT make
+ * `stream` wait for its downloads, so the uploads of the next step overlap this step's compute and this step's
+ * downloads overlap the next step's compute (PCIe is full duplex).  Rules: consecutive calls must ALTERNATE between two
+ * (x_dev, dy_dev) staging sets (a set is overwritten by the call two steps later, after the backward that read it);
+ * y_dev / dx_dev may be reused every call (the library orders the rewrite after the previous download) or alternated;
+ * y_host / dx_host are complete only after lsp_host_copies_wait(ctx, stream) and completion of `stream`. */
+lsp_status lsp_layer_step_host_async(lsp_ctx* ctx, const void* x_host, const void* dy_host, const lsp_layer_weights* w,
+                                     void* y_host, void* dx_host, lsp_layer_wgrads* grads, void* x_dev, void* dy_dev,
+                                     void* y_dev, void* dx_dev, void* saved, void* ws, void* stream);
+lsp_status lsp_host_copies_wait(lsp_ctx* ctx, void* stream);
+
 /* Model head (readings H-1 .. H-3 in DESIGN.md section 13): final RMSNorm (gain g_final, the
  * context's rms_eps), bias-free LM head w_head bf16 [vocab, H] ([out,in]), mean next-token cross-entropy, and all their
  * gradients, in one call:  xn = RMSNorm(x; g_final); z = xn w_head^T; loss = mean_t (lse_t - z[t, targets[t]]).

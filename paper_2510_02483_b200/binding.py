@@ -19,7 +19,7 @@ EXPORTS = ("lsp_create", "lsp_destroy", "lsp_saved_bytes", "lsp_workspace_bytes"
            "lsp_attn_fwd", "lsp_attn_bwd", "lsp_mlp_fwd", "lsp_mlp_bwd", "lsp_layer_fwd", "lsp_layer_bwd",
            "lsp_sdpa_fwd", "lsp_sdpa_bwd", "lsp_embed_fwd", "lsp_gemm", "lsp_layer_step_host", "lsp_launch_count",
            "lsp_timing_enable", "lsp_timing_read", "lsp_adamw_step", "lsp_lr_cosine", "lsp_head_workspace_bytes",
-           "lsp_head_fwd_bwd", "lsp_embed_bwd")
+           "lsp_head_fwd_bwd", "lsp_embed_bwd", "lsp_layer_step_host_async", "lsp_host_copies_wait")
 
 
 class LspError(RuntimeError):
@@ -79,6 +79,8 @@ def lib():
         L.lsp_embed_fwd.argtypes = [vp, vp, vp, vp, vp]
         L.lsp_gemm.argtypes = [vp, i32, i32, i32, i32, vp, i64, i32, vp, i64, i32, vp, i64, vp]
         L.lsp_layer_step_host.argtypes = [vp, vp, vp, pw, vp, vp, pg, vp, vp, vp, vp, vp, vp, vp]
+        L.lsp_layer_step_host_async.argtypes = [vp, vp, vp, pw, vp, vp, pg, vp, vp, vp, vp, vp, vp, vp]
+        L.lsp_host_copies_wait.argtypes = [vp, vp]
         L.lsp_launch_count.argtypes = [vp]; L.lsp_launch_count.restype = C.c_longlong
         L.lsp_timing_enable.argtypes = [vp, i32]
         L.lsp_timing_read.argtypes = [vp, i32, C.POINTER(C.c_char_p), C.POINTER(C.c_float), C.POINTER(i32)]
@@ -210,6 +212,18 @@ def lsp_layer_step_host(ctx, x_host, dy_host, weights, y_host, dx_host, grads, x
     ctx.check(lib().lsp_layer_step_host(ctx.handle, _ptr(x_host), _ptr(dy_host), C.byref(w), _ptr(y_host), _ptr(dx_host),
                                         C.byref(g), _ptr(x_dev), _ptr(dy_dev), _ptr(y_dev), _ptr(dx_dev), _ptr(saved),
                                         _ptr(ws), _stream(stream)))
+
+
+def lsp_layer_step_host_async(ctx, x_host, dy_host, weights, y_host, dx_host, grads, x_dev, dy_dev, y_dev, dx_dev, saved, ws,
+                              stream=None):
+    w, g = _pack(lsp_layer_weights, weights), _pack(lsp_layer_wgrads, grads)
+    ctx.check(lib().lsp_layer_step_host_async(ctx.handle, _ptr(x_host), _ptr(dy_host), C.byref(w), _ptr(y_host), _ptr(dx_host),
+                                              C.byref(g), _ptr(x_dev), _ptr(dy_dev), _ptr(y_dev), _ptr(dx_dev), _ptr(saved),
+                                              _ptr(ws), _stream(stream)))
+
+
+def lsp_host_copies_wait(ctx, stream=None):
+    ctx.check(lib().lsp_host_copies_wait(ctx.handle, _stream(stream)))
 
 
 def lsp_adamw_step(ctx, tensors, *, lr, step, gnorm_out, beta1=0.90, beta2=0.95, eps=1e-8, weight_decay=0.01, clip_norm=1.0,

@@ -69,6 +69,9 @@ struct lsp_ctx {
   float* opt_partial;            // per-block partial sums of the gradient-norm pass (device)
   cudaStream_t s_in, s_out;      // copy streams of lsp_layer_step_host (H2D / D2H overlap the compute stream)
   cudaEvent_t ev[6];             // start, x in, dy in, fwd done, bwd done, copies out
+  cudaEvent_t pev[2][6];         // lsp_layer_step_host_async, per call parity: x in, dy in, fwd done, bwd done, y out, dx out
+  long long host_seq;            // number of async host steps issued
+  const void* prev_y_dev; const void* prev_dx_dev;   // device result buffers of the previous async step
   int norm_blocks;      // persistent grid of the RMSNorm backward
   SavedLayout sv;
   WsLayout ws;
@@ -597,6 +600,8 @@ lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device
   }
   for (int i = 0; i < 6; ++i)
     if (cudaEventCreateWithFlags(&ctx->ev[i], cudaEventDisableTiming) != cudaSuccess) { lsp_destroy(ctx); return LSP_ECUDA; }
+  for (int i = 0; i < 12; ++i)
+    if (cudaEventCreateWithFlags(&ctx->pev[i / 6][i % 6], cudaEventDisableTiming) != cudaSuccess) { lsp_destroy(ctx); return LSP_ECUDA; }
   *out = ctx;
   return LSP_OK;
 }
@@ -613,6 +618,8 @@ lsp_status lsp_destroy(lsp_ctx* ctx) {
   if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
   for (int i = 0; i < 6; ++i)
     if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+  for (int i = 0; i < 12; ++i)
+    if (ctx->pev[i / 6][i % 6]) cudaEventDestroy(ctx->pev[i / 6][i % 6]);
   delete ctx;
   return LSP_OK;
 }
@@ -805,6 +812,69 @@ lsp_status lsp_layer_step_host(lsp_ctx* ctx, const void* x_host, const void* dy_
   LSP_CUDA(cudaMemcpyAsync(dx_host, dx_dev, n * 4, cudaMemcpyDeviceToHost, ctx->s_out));
   LSP_CUDA(cudaEventRecord(ev[5], ctx->s_out));
   LSP_CUDA(cudaStreamWaitEvent(st, ev[5], 0));
+  return LSP_OK;
+}
+
+// Pipelined variant: consecutive calls overlap -- the uploads of step i+1 run during the compute of step i, the
+// downloads of step i during the compute of step i+1 (PCIe is full duplex).  Hazards are ordered with per-parity events:
+//   x_dev / dy_dev of this call were last read by the backward of the call two steps ago (the caller alternates two
+//   staging sets); y_dev / dx_dev, if they are the previous call's, are rewritten only after their downloads.
+lsp_status lsp_layer_step_host_async(lsp_ctx* ctx, const void* x_host, const void* dy_host, const lsp_layer_weights* w,
+                                     void* y_host, void* dx_host, lsp_layer_wgrads* g, void* x_dev, void* dy_dev, void* y_dev,
+                                     void* dx_dev, void* saved, void* ws, void* stream) {
+  if (!ctx || !x_host || !dy_host || !y_host || !dx_host || !x_dev || !dy_dev || !y_dev || !dx_dev) return LSP_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const size_t n = static_cast<size_t>(ctx->T) * ctx->d.hidden;
+  const size_t in_bytes = n * (ctx->d.in_dtype == LSP_F32 ? 4 : 2);
+  const int p = static_cast<int>(ctx->host_seq & 1), q = p ^ 1;
+  enum { E_X = 0, E_DY, E_FWD, E_BWD, E_Y, E_DX };
+  cudaEvent_t* e = ctx->pev[p];
+  cudaEvent_t* eq = ctx->pev[q];
+  const bool first = ctx->host_seq == 0;
+  // uploads: after whatever `stream` held when the pipeline started, and after the backward that last read this staging set
+  if (first) {
+    LSP_CUDA(cudaEventRecord(ctx->ev[0], st));
+    LSP_CUDA(cudaStreamWaitEvent(ctx->s_in, ctx->ev[0], 0));
+    LSP_CUDA(cudaStreamWaitEvent(ctx->s_out, ctx->ev[0], 0));
+  }
+  if (ctx->host_seq >= 2) LSP_CUDA(cudaStreamWaitEvent(ctx->s_in, e[E_BWD], 0));
+  LSP_CUDA(cudaMemcpyAsync(x_dev, x_host, in_bytes, cudaMemcpyHostToDevice, ctx->s_in));
+  LSP_CUDA(cudaEventRecord(e[E_X], ctx->s_in));
+  LSP_CUDA(cudaMemcpyAsync(dy_dev, dy_host, in_bytes, cudaMemcpyHostToDevice, ctx->s_in));
+  LSP_CUDA(cudaEventRecord(e[E_DY], ctx->s_in));
+  // forward
+  LSP_CUDA(cudaStreamWaitEvent(st, e[E_X], 0));
+  if (!first && y_dev == ctx->prev_y_dev) LSP_CUDA(cudaStreamWaitEvent(st, eq[E_Y], 0));
+  LSP_TRY(lsp_layer_fwd(ctx, x_dev, w, y_dev, saved, ws, stream));
+  LSP_CUDA(cudaEventRecord(e[E_FWD], st));
+  LSP_CUDA(cudaStreamWaitEvent(ctx->s_out, e[E_FWD], 0));
+  LSP_CUDA(cudaMemcpyAsync(y_host, y_dev, n * 4, cudaMemcpyDeviceToHost, ctx->s_out));
+  LSP_CUDA(cudaEventRecord(e[E_Y], ctx->s_out));
+  // backward
+  LSP_CUDA(cudaStreamWaitEvent(st, e[E_DY], 0));
+  if (!first && dx_dev == ctx->prev_dx_dev) LSP_CUDA(cudaStreamWaitEvent(st, eq[E_DX], 0));
+  LSP_TRY(lsp_layer_bwd(ctx, x_dev, dy_dev, w, saved, dx_dev, g, ws, stream));
+  LSP_CUDA(cudaEventRecord(e[E_BWD], st));
+  LSP_CUDA(cudaStreamWaitEvent(ctx->s_out, e[E_BWD], 0));
+  LSP_CUDA(cudaMemcpyAsync(dx_host, dx_dev, n * 4, cudaMemcpyDeviceToHost, ctx->s_out));
+  LSP_CUDA(cudaEventRecord(e[E_DX], ctx->s_out));
+  ctx->prev_y_dev = y_dev; ctx->prev_dx_dev = dx_dev;
+  ++ctx->host_seq;
+  return LSP_OK;
+}
+
+// `stream` waits for every copy the async host steps have issued, and the pipeline restarts (next call is a "first").
+lsp_status lsp_host_copies_wait(lsp_ctx* ctx, void* stream) {
+  if (!ctx) return LSP_EINVAL;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (ctx->host_seq > 0) {
+    LSP_CUDA(cudaEventRecord(ctx->ev[5], ctx->s_out));
+    LSP_CUDA(cudaStreamWaitEvent(st, ctx->ev[5], 0));
+    LSP_CUDA(cudaEventRecord(ctx->ev[1], ctx->s_in));
+    LSP_CUDA(cudaStreamWaitEvent(st, ctx->ev[1], 0));
+  }
+  ctx->host_seq = 0;
+  ctx->prev_y_dev = ctx->prev_dx_dev = nullptr;
   return LSP_OK;
 }
 

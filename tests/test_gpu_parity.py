@@ -351,6 +351,45 @@ def test_stack_fwd_bwd(gpu):
     run.close()
 
 
+def test_layer_step_host_async_pipeline(gpu):
+    """Four pipelined host steps (lsp_layer_step_host_async, alternating staging sets, shared y_dev / dx_dev) with a
+    different x per step: every step's y / dx in its own pinned buffers equals the device-resident path bit for bit
+    (the uploads of step i+1 and the downloads of step i-1 run during step i: a missed hazard shows up as a mix-up)."""
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    w = MID
+    dev = gpu.require_cuda()
+    ctx = gpu.make_ctx(w)
+    buf = gpu.LayerBuffers(ctx, w, dev)
+    weights = gpu.upload_weights(synth.layer_weights(w, 0), dev)
+    inp = synth.layer_inputs(w)
+    T, H = w.tokens, w.hidden
+    xs = [np.roll(inp["x"], 17 * k, axis=0).copy() for k in range(4)]
+    hx = [gpu.bf16_pinned(v) for v in xs]
+    hdy = gpu.bf16_pinned(inp["dy"])
+    hy = [torch.empty((T, H), dtype=torch.float32).pin_memory() for _ in range(4)]
+    hdx = [torch.empty((T, H), dtype=torch.float32).pin_memory() for _ in range(4)]
+    x_st = [torch.empty((T, H), dtype=torch.bfloat16, device=dev) for _ in range(2)]
+    dy_st = [torch.empty((T, H), dtype=torch.bfloat16, device=dev) for _ in range(2)]
+    for k in range(4):
+        B.lsp_layer_step_host_async(ctx, hx[k], hdy, weights, hy[k], hdx[k], buf.grads, x_st[k & 1], dy_st[k & 1], buf.y, buf.dx,
+                                    buf.saved, buf.ws)
+    B.lsp_host_copies_wait(ctx)
+    torch.cuda.synchronize()
+    last_grads = {k: v.cpu().numpy() for k, v in buf.grads.items()}
+    dy = gpu.bf16_to_device(inp["dy"], dev)
+    for k in range(4):
+        x = gpu.bf16_to_device(xs[k], dev)
+        B.lsp_layer_fwd(ctx, x, weights, buf.y, buf.saved, buf.ws)
+        B.lsp_layer_bwd(ctx, x, dy, weights, buf.saved, buf.dx, buf.grads, buf.ws)
+        torch.cuda.synchronize()
+        assert np.array_equal(hy[k].numpy(), buf.y.cpu().numpy()), k
+        assert np.array_equal(hdx[k].numpy(), buf.dx.cpu().numpy()), k
+    for k, v in buf.grads.items():
+        assert np.array_equal(last_grads[k], v.cpu().numpy()), k
+    ctx.close()
+
+
 # ------------------------------------------------------------------------------------------- full-size configurations
 def _layer_full(gpu, w):
     got = gpu.run_layer(w)
