@@ -129,6 +129,15 @@ lsp_status lsp_embed_fwd(lsp_ctx* ctx, const int32_t* ids, const void* table, vo
 lsp_status lsp_gemm(lsp_ctx* ctx, int op, int M, int N, int K, const void* A, int64_t lda, int a_dtype, const void* B,
                     int64_t ldb, int b_dtype, float* C, int64_t ldc, void* stream);
 
+/* Packed variable-length sequences (the SFT / DPO data layout of PAPER.md:176-186): the context's
+ * batch * seq tokens (batch must be 1, head_dim 128) are n_seqs sequences laid end to end, sequence i = tokens
+ * [cu_seqlens[i], cu_seqlens[i+1]) with cu_seqlens[0] = 0, cu_seqlens[n_seqs] = batch*seq, strictly increasing (HOST
+ * array of n_seqs + 1 entries, read before the call returns).  From then on every attention call of the context is
+ * causal WITHIN each sequence (a query sees the keys of its own sequence up to itself; key blocks of other sequences are
+ * skipped, not just masked) and RoPE positions restart at 0 at every sequence start.  n_seqs = 0 switches back to
+ * `batch` sequences of `seq` tokens.  Enqueues one small copy on `stream`. */
+lsp_status lsp_set_packed_sequences(lsp_ctx* ctx, const int32_t* cu_seqlens_host, int32_t n_seqs, void* stream);
+
 /* End-to-end step with HOST buffers (bench.py `e2e`): copies x, dy (in_dtype, [T,H]; pinned host memory for
  * asynchronous copies) to the caller's device staging buffers x_dev / dy_dev, runs lsp_layer_fwd + lsp_layer_bwd,
  * and copies y and dx (fp32 [T,H]) back to y_host / dx_host (no sync).  The copies run on two context-owned streams

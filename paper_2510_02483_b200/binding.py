@@ -19,7 +19,7 @@ EXPORTS = ("lsp_create", "lsp_destroy", "lsp_saved_bytes", "lsp_workspace_bytes"
            "lsp_attn_fwd", "lsp_attn_bwd", "lsp_mlp_fwd", "lsp_mlp_bwd", "lsp_layer_fwd", "lsp_layer_bwd",
            "lsp_sdpa_fwd", "lsp_sdpa_bwd", "lsp_embed_fwd", "lsp_gemm", "lsp_layer_step_host", "lsp_launch_count",
            "lsp_timing_enable", "lsp_timing_read", "lsp_adamw_step", "lsp_lr_cosine", "lsp_head_workspace_bytes",
-           "lsp_head_fwd_bwd", "lsp_embed_bwd", "lsp_layer_step_host_async", "lsp_host_copies_wait")
+           "lsp_head_fwd_bwd", "lsp_embed_bwd", "lsp_layer_step_host_async", "lsp_host_copies_wait", "lsp_set_packed_sequences")
 
 
 class LspError(RuntimeError):
@@ -81,6 +81,7 @@ def lib():
         L.lsp_layer_step_host.argtypes = [vp, vp, vp, pw, vp, vp, pg, vp, vp, vp, vp, vp, vp, vp]
         L.lsp_layer_step_host_async.argtypes = [vp, vp, vp, pw, vp, vp, pg, vp, vp, vp, vp, vp, vp, vp]
         L.lsp_host_copies_wait.argtypes = [vp, vp]
+        L.lsp_set_packed_sequences.argtypes = [vp, C.POINTER(C.c_int32), i32, vp]
         L.lsp_launch_count.argtypes = [vp]; L.lsp_launch_count.restype = C.c_longlong
         L.lsp_timing_enable.argtypes = [vp, i32]
         L.lsp_timing_read.argtypes = [vp, i32, C.POINTER(C.c_char_p), C.POINTER(C.c_float), C.POINTER(i32)]
@@ -220,6 +221,13 @@ def lsp_layer_step_host_async(ctx, x_host, dy_host, weights, y_host, dx_host, gr
     ctx.check(lib().lsp_layer_step_host_async(ctx.handle, _ptr(x_host), _ptr(dy_host), C.byref(w), _ptr(y_host), _ptr(dx_host),
                                               C.byref(g), _ptr(x_dev), _ptr(dy_dev), _ptr(y_dev), _ptr(dx_dev), _ptr(saved),
                                               _ptr(ws), _stream(stream)))
+
+
+def lsp_set_packed_sequences(ctx, cu_seqlens, stream=None):
+    """cu_seqlens: host sequence of n_seqs + 1 ints (0 ... total tokens); empty / None switches packing off."""
+    n = 0 if not cu_seqlens else len(cu_seqlens) - 1
+    arr = (C.c_int32 * (n + 1))(*([0] if n == 0 else [int(v) for v in cu_seqlens]))
+    ctx.check(lib().lsp_set_packed_sequences(ctx.handle, arr, n, _stream(stream)))
 
 
 def lsp_host_copies_wait(ctx, stream=None):

@@ -1,6 +1,6 @@
 """Device-side timing of every BASELINE.json configuration (bench.py covers the headline config 2 only).
 
-    python -m paper_2510_02483_b200.configs_bench [--steps K] [--only cfg2,fwd,cfg3,cfg4,cfg5,table1,table1_30b,adamw,head]
+    python -m paper_2510_02483_b200.configs_bench [--steps K] [--only cfg2,fwd,packed,cfg3,cfg4,cfg5,table1,table1_30b,adamw,head]
 
 Prints one JSON line per configuration: ms per fwd+bwd step (CUDA events on the launching stream, after warm-up),
 tokens/s and executed TFLOP/s (causal attention FLOPs, SURVEY.md 8(d) convention).  Inputs are the seeded synthetic
@@ -55,6 +55,28 @@ def bench_layer(w, steps, logical_head_dim=0):
     ms = _time(step, steps)
     ctx.close()
     return ms, synth.layer_flops(wl, causal=True)
+
+
+def bench_layer_packed(w, steps, cu):
+    """cfg-2 layer on packed variable-length sequences (lsp_set_packed_sequences): batch 1, seq = all tokens, sequence
+    boundaries `cu`.  FLOPs: GEMMs as usual, causal attention summed over the sequences."""
+    dev = harness.require_cuda()
+    ctx = harness.make_ctx(w)
+    buf = harness.LayerBuffers(ctx, w, dev)
+    weights = harness.upload_weights(synth.layer_weights(w), dev)
+    inp = synth.layer_inputs(w)
+    x, dy = harness.bf16_to_device(inp["x"], dev), harness.bf16_to_device(inp["dy"], dev)
+    B.lsp_set_packed_sequences(ctx, cu)
+
+    def step():
+        B.lsp_layer_fwd(ctx, x, weights, buf.y, buf.saved, buf.ws)
+        B.lsp_layer_bwd(ctx, x, dy, weights, buf.saved, buf.dx, buf.grads, buf.ws)
+    ms = _time(step, steps)
+    ctx.close()
+    one = w.with_(seq=1)
+    gemm = synth.layer_flops(one, causal=True) - 3.5 * synth.attn_flops_fwd(one, causal=True)
+    attn = sum(3.5 * synth.attn_flops_fwd(w.with_(batch=1, seq=b - a), causal=True) for a, b in zip(cu, cu[1:]))
+    return ms, gemm * w.tokens + attn
 
 
 def bench_layer_fwd_only(w, steps):
@@ -155,13 +177,18 @@ def bench_head(w, steps):
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--only", default="cfg2,fwd,cfg3,cfg4,cfg5,table1,table1_30b,adamw,head")
+    ap.add_argument("--only", default="cfg2,fwd,packed,cfg3,cfg4,cfg5,table1,table1_30b,adamw,head")
     args = ap.parse_args(argv)
     B.lib()
     only = set(args.only.split(","))
     jobs = []
     if "cfg2" in only:
         jobs.append((synth.CFG2_3B_LAYER, bench_layer))
+    if "packed" in only:      # 16384 tokens of the 3B-shape layer as ONE row holding 7 sequences of 333 ... 6000 tokens
+        cu = [0, 333, 1500, 5596, 6000, 12000, 14048, 16384]
+        wp = synth.CFG2_3B_LAYER.with_(name="cfg2_3b_layer_packed_7_sequences", batch=1, seq=16384)
+        jobs.append((wp, lambda w, steps: bench_layer_packed(w, steps, cu)))
+        jobs.append((wp.with_(name="cfg2_3b_layer_one_sequence_of_16384"), lambda w, steps: bench_layer_packed(w, steps, [0, 16384])))
     if "fwd" in only:
         jobs.append((synth.CFG2_3B_LAYER.with_(name="cfg2_3b_layer_forward_only"), bench_layer_fwd_only))
     if "cfg4" in only:

@@ -34,6 +34,9 @@ struct AttnTcParams {
   float* o32; __half* o16; long long ldo;        // [T, ldo] outputs (either may be null)
   float* lse;                                    // [B, nq, S]
   unsigned int* sched;                           // [2] work-item counter and finished-CTA counter (zero between launches)
+  // packed variable-length sequences (B = 1): token t attends keys [doc_start[t], t]; doc_end[t] = end (exclusive) of
+  // t's sequence; both non-decreasing in t.  Null: every sequence starts at position 0 of its batch row.
+  const int* doc_start; const int* doc_end;
 };
 
 constexpr int ATC_D = 128;
@@ -96,8 +99,8 @@ __device__ __forceinline__ uint64_t atc_desc_mnmajor(uint32_t tile, int kk) {
 // last P V, and the O epilogue of a tile (TMEM -> registers -> staging tile -> coalesced global stores) overlaps the
 // other tile's and the next item's MMAs (o_free tells the MMA warp when O_t may be overwritten).  The ~19 k cycles of
 // fill / drain / launch that every one of the 1536 one-shot CTAs paid before are gone (profiles/r1c_attn_notes.md).
-struct AttnItem { int q0, h, b, kvh, n0, n1, nmax; };
-__device__ __forceinline__ AttnItem attn_fwd_item(uint32_t i, const AttnTcParams& p, int nqb) {
+struct AttnItem { int q0, h, b, kvh, n0, n1, nmax, j0; };         // j0: first 128-key block (packed sequences), else 0
+__device__ __forceinline__ AttnItem attn_fwd_item(uint32_t i, const AttnTcParams& p, int nqb, const int* doc_start) {
   const int per_lvl = p.nq * p.B;
   const int lvl = static_cast<int>(i) / per_lvl, r = static_cast<int>(i) - lvl * per_lvl;
   AttnItem it;
@@ -105,15 +108,23 @@ __device__ __forceinline__ AttnItem attn_fwd_item(uint32_t i, const AttnTcParams
   it.b = r / p.nq; it.h = r - it.b * p.nq;
   it.kvh = it.h / (p.nq / p.nkv);
   // key blocks per tile: tile t covers queries [q0 + 128 t, +128); causal => keys [0, q0 + 128 t + 128)
-  it.n0 = it.q0 / 128 + 1;
+  // packed sequences: nothing before the start of the sequence of the item's first query is visited (starts are
+  // non-decreasing, so that is the smallest start of the item); both tiles share the K/V stream
+  it.j0 = doc_start ? doc_start[it.q0] / 128 : 0;
+  it.n0 = it.q0 / 128 + 1 - it.j0;
   it.n1 = (it.q0 + 128 < p.S) ? it.n0 + 1 : 0;
   it.nmax = it.n1 > it.n0 ? it.n1 : it.n0;
   return it;
 }
 constexpr int ATC_ITEM_RING = 4;
 
+template <bool DOC>
 __global__ void __launch_bounds__(ATC_FWD_THREADS, 1)
 attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p) {
+  // packed sequences compiled in only for DOC: the plain kernels carry none of the bound / mask code
+  const int* const doc_start = DOC ? p.doc_start : nullptr;
+  const int* const doc_end = DOC ? p.doc_end : nullptr;
+  (void)doc_start; (void)doc_end;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = smem_base;                              // 2 tiles
@@ -180,7 +191,7 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
       uint32_t item = atomicAdd(p.sched, 1u);
       publish(0, item);
       for (uint32_t it = 0; item < nitems; ++it) {
-        const AttnItem w = attn_fwd_item(item, p, nqb);
+        const AttnItem w = attn_fwd_item(item, p, nqb, doc_start);
         mbar_wait(q_empty(0), (qc0 & 1u) ^ 1u);
         atc_load_tile(sQ, &maps.q, q_full(0), w.h * ATC_D, w.q0, w.b);
         ++qc0;
@@ -194,9 +205,9 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
           const int st = kvc & 1;
           const uint32_t ph = ((kvc >> 1) & 1u) ^ 1u;
           mbar_wait(k_empty(st), ph);
-          atc_load_tile(sK + st * ATC_TILE_BYTES, &maps.k, k_full(st), w.kvh * ATC_D, j * 128, w.b);
+          atc_load_tile(sK + st * ATC_TILE_BYTES, &maps.k, k_full(st), w.kvh * ATC_D, (w.j0 + j) * 128, w.b);
           mbar_wait(v_empty(st), ph);
-          atc_load_tile(sV + st * ATC_TILE_BYTES, &maps.v, v_full(st), w.kvh * ATC_D, j * 128, w.b);
+          atc_load_tile(sV + st * ATC_TILE_BYTES, &maps.v, v_full(st), w.kvh * ATC_D, (w.j0 + j) * 128, w.b);
         }
         publish(it + 1, next);
         item = next;
@@ -239,7 +250,7 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
     for (uint32_t it = 0;; ++it) {
       const uint32_t item = get_item(it);
       if (item >= nitems) break;
-      const AttnItem w = attn_fwd_item(item, p, nqb);
+      const AttnItem w = attn_fwd_item(item, p, nqb, doc_start);
       const int nt[2] = {w.n0, w.n1};
       // first S of both tiles (for the second and later items this overlaps the previous item's epilogues)
       {
@@ -300,11 +311,12 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
     for (uint32_t it = 0;; ++it) {
       const uint32_t item = get_item(it);
       if (item >= nitems) break;
-      const AttnItem w = attn_fwd_item(item, p, nqb);
+      const AttnItem w = attn_fwd_item(item, p, nqb, doc_start);
       const int nblk = t == 0 ? w.n0 : w.n1;
       if (nblk == 0) continue;
       const int qi = w.q0 + t * 128 + row;                       // position in the sequence
       float m_run = -INFINITY, l_run = 0.f;
+      const int dstart = doc_start ? doc_start[min(qi, p.S - 1)] : 0;     // first key this query may see
 
       for (int j = 0; j < nblk; ++j, ++cnt) {
         mbar_wait(s_full(t), cnt & 1u);
@@ -321,12 +333,22 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
             for (int i = 0; i < 32; ++i)
               if (q * 32 + i > row) s[q][i] = -INFINITY;
         }
+        if (DOC && __any_sync(0xffffffffu, (w.j0 + j) * 128 < dstart)) {   // packed sequences: keys of earlier sequences
+          const int kb0 = (w.j0 + j) * 128;
+#pragma unroll
+          for (int q = 0; q < 4; ++q)
+#pragma unroll
+            for (int i = 0; i < 32; ++i)
+              if (kb0 + q * 32 + i < dstart) s[q][i] = -INFINITY;
+        }
         float mx0 = s[0][0], mx1 = s[1][0], mx2 = s[2][0], mx3 = s[3][0];
 #pragma unroll
         for (int i = 1; i < 32; ++i) {
           mx0 = fmaxf(mx0, s[0][i]); mx1 = fmaxf(mx1, s[1][i]); mx2 = fmaxf(mx2, s[2][i]); mx3 = fmaxf(mx3, s[3][i]);
         }
-        const float m_new = fmaxf(m_run, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)));
+        // a row whose keys so far are all masked (packed sequences only) keeps a finite reference maximum: P = 0, no NaN
+        const float m_blk = fmaxf(m_run, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)));
+        const float m_new = DOC ? fmaxf(m_blk, -1.0e30f) : m_blk;
         float m_use = m_run;
         if (j == 0) {
           m_use = m_new;
@@ -436,7 +458,9 @@ inline cudaError_t attn_fwd_tc_launch(const __half* q, long long ldq, const __ha
                                       long long ldv, const AttnTcParams& p, int num_sms, cudaStream_t st) {
   static bool set = false;
   if (!set) {
-    cudaError_t e = cudaFuncSetAttribute(attn_fwd_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_FWD_SMEM);
+    cudaError_t e = cudaFuncSetAttribute(attn_fwd_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_FWD_SMEM);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(attn_fwd_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_FWD_SMEM);
     if (e != cudaSuccess) return e;
     set = true;
   }
@@ -450,7 +474,8 @@ inline cudaError_t attn_fwd_tc_launch(const __half* q, long long ldq, const __ha
   if (p.o16 && !make_map_store(&maps.o16, p.o16, p.nq * ATC_D, p.S, p.B, p.ldo, false)) return cudaErrorInvalidValue;
   const int nitems = ((p.S + 255) / 256) * p.nq * p.B;
   const int grid = nitems < num_sms ? nitems : num_sms;        // persistent: one CTA per SM
-  attn_fwd_tc_kernel<<<grid, ATC_FWD_THREADS, ATC_FWD_SMEM, st>>>(maps, p);
+  if (p.doc_start) attn_fwd_tc_kernel<true><<<grid, ATC_FWD_THREADS, ATC_FWD_SMEM, st>>>(maps, p);
+  else attn_fwd_tc_kernel<false><<<grid, ATC_FWD_THREADS, ATC_FWD_SMEM, st>>>(maps, p);
   return cudaGetLastError();
 }
 
@@ -489,6 +514,7 @@ struct AttnTcBwdParams {
   float* dq32; float* dk32; float* dv32; long long lddq32, lddk32;
   __half* dq16; __half* dk16; __half* dv16; long long ldd16;
   unsigned int* sched;         // work-item counters of the persistent kernels ([4], [5]: dQ kernel), zero between launches
+  const int* doc_start; const int* doc_end;      // packed sequences (see AttnTcParams); rope rows are then t - doc_start[t]
 };
 
 __device__ __forceinline__ void atc_load_half_tile(uint32_t dst, const CUtensorMap* m, uint32_t bar, int col0, int s0, int b) {
@@ -535,8 +561,13 @@ __device__ __forceinline__ void atc_store_grad32(const WarpStage& st, float (&v)
 }
 
 // --------------------------------------------------------------------------------------------- dK, dV
+template <bool DOC>
 __global__ void __launch_bounds__(ATC_BWD_THREADS, 1)
 attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdParams p) {
+  // packed sequences compiled in only for DOC: the plain kernels carry none of the bound / mask code
+  const int* const doc_start = DOC ? p.doc_start : nullptr;
+  const int* const doc_end = DOC ? p.doc_end : nullptr;
+  (void)doc_start; (void)doc_end;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sK = smem_base, sV = sK + ATC_TILE_BYTES;
@@ -561,8 +592,16 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
   const int kb = blockIdx.x, kvh = blockIdx.y, b = blockIdx.z;
   const int G = p.nq / p.nkv;
   const int k0 = kb * 128;
-  const int nq64 = (p.S + 63) / 64;
+  // packed sequences: no query past the end of the sequence of this block's last key attends any of its keys
+  const int q_end = doc_end ? doc_end[min(k0 + 127, p.S - 1)] : p.S;
+  const int nq64 = (q_end + 63) / 64;
   const int per_head = nq64 - 2 * kb;                            // 64-query blocks at / below the diagonal
+  // early positions of a sequence take hi + lo fp16 operands: a 64-query block splits when its last query is closer
+  // than ATC_SPLIT_ROWS to the start of that query's sequence (position 0 without packing)
+  auto split_block = [&](int qblk) {
+    const int qs = qblk * 64;
+    return qs - (doc_start ? doc_start[min(qs + 63, p.S - 1)] : 0) < ATC_SPLIT_ROWS;
+  };
   const int iters = per_head * G;
 
   if (threadIdx.x == 0) {
@@ -640,7 +679,7 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
       const uint32_t ph = (it >> 1) & 1;
       if (it + 1 < iters) issue_sdp(it + 1);
       const uint64_t qa = desc_adv(dQm, st * ATC_HALF_TILE), da = desc_adv(dDOm, st * ATC_HALF_TILE);
-      const bool split = (2 * kb + it % per_head) * 64 < ATC_SPLIT_ROWS;
+      const bool split = split_block(2 * kb + it % per_head);
       mbar_wait(p_full(buf), ph);
       tc_fence_after();
       if (leader) {
@@ -679,6 +718,7 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
     const uint32_t lane_off = static_cast<uint32_t>(quarter * 32) << 16;
     const int col0 = half * 32;
     const float c = p.scale_log2;
+    const int dend = doc_end ? doc_end[min(k0 + row, p.S - 1)] : p.S;   // end of this key's sequence
     for (int it = 0; it < iters; ++it) {
       const int st = it % ATC_NST, buf = it & 1;
       const int rel = it % per_head;                                   // 64-query block index relative to the diagonal
@@ -706,7 +746,15 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
         for (int i = 0; i < 32; ++i)
           if (qrel + i < row) pv[i] = 0.f;
       }
-      const bool split = (2 * kb + rel) * 64 < ATC_SPLIT_ROWS;      // early query positions: hi + lo operands
+      if (doc_end) {                                                 // packed sequences: queries of later sequences
+        const int qabs = (2 * kb + rel) * 64 + col0;
+        if (__any_sync(0xffffffffu, qabs + 31 >= dend)) {
+#pragma unroll
+          for (int i = 0; i < 32; ++i)
+            if (qabs + i >= dend) pv[i] = 0.f;
+        }
+      }
+      const bool split = split_block(2 * kb + rel);                  // early query positions: hi + lo operands
       uint32_t pk[16], pl[16];
       if (split) {
 #pragma unroll
@@ -762,7 +810,7 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
         tmem_ld32(tmem_base + lane_off + 384 + cc, a);
         tmem_ld_wait();
         atc_store_grad32(wst, reinterpret_cast<float(&)[32]>(a), p.scale,
-                         (p.rope && valid) ? p.rope + static_cast<long long>(key) * 64 + (cc >> 1) : nullptr,
+                         (p.rope && valid) ? p.rope + static_cast<long long>(key - (doc_start ? doc_start[key] : 0)) * 64 + (cc >> 1) : nullptr,
                          p.dk32 ? &maps.g32[1] : nullptr, p.dk16 ? &maps.g16[1] : nullptr, kvh * ATC_D + cc, s0, b);
       }
     }
@@ -787,20 +835,29 @@ constexpr int ATC_DQ_ACC = 2 * 64 * ATC_DQ_NB;   // dQ accumulator column
 // (p.sched + 4); Q / dO of the next item are fetched as soon as the item's last S / dP MMA has been issued (qdo_empty),
 // the dQ epilogue (TMEM -> staging tile -> bulk stores) overlaps the first S / dP MMAs of the next item, and acc_free
 // tells the MMA warp when the dQ accumulator may be overwritten.
-struct AttnDqItem { int q0, h, b, kvh, iters; };
-__device__ __forceinline__ AttnDqItem attn_dq_item(uint32_t i, const AttnTcBwdParams& p, int nqb) {
+struct AttnDqItem { int q0, h, b, kvh, iters, j0, split; };        // j0: first 64-key block (packed sequences), else 0
+__device__ __forceinline__ AttnDqItem attn_dq_item(uint32_t i, const AttnTcBwdParams& p, int nqb, const int* doc_start) {
   const int per_lvl = p.nq * p.B;
   const int lvl = static_cast<int>(i) / per_lvl, r = static_cast<int>(i) - lvl * per_lvl;
   AttnDqItem it;
   it.q0 = (nqb - 1 - lvl) * 128;                                 // heavy (late) query blocks first
   it.b = r / p.nq; it.h = r - it.b * p.nq;
   it.kvh = it.h / (p.nq / p.nkv);
-  it.iters = (min(p.S, it.q0 + 128) + 63) / 64;                  // 64-key blocks [0, kv_end)
+  // packed sequences: keys before the start of the sequence of the item's first query are never visited
+  it.j0 = doc_start ? doc_start[it.q0] / 64 : 0;
+  it.iters = (min(p.S, it.q0 + 128) + 63) / 64 - it.j0;          // 64-key blocks [64 j0, kv_end)
+  // hi + lo fp16 dS operands while the tile's last query is closer than ATC_SPLIT_ROWS to the start of its sequence
+  it.split = it.q0 - (doc_start ? doc_start[min(it.q0 + 127, p.S - 1)] : 0) < ATC_SPLIT_ROWS;
   return it;
 }
 
+template <bool DOC>
 __global__ void __launch_bounds__(ATC_BWD_THREADS, 1)
 attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdParams p) {
+  // packed sequences compiled in only for DOC: the plain kernels carry none of the bound / mask code
+  const int* const doc_start = DOC ? p.doc_start : nullptr;
+  const int* const doc_end = DOC ? p.doc_end : nullptr;
+  (void)doc_start; (void)doc_end;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t sQ = smem_base, sDO = sQ + ATC_TILE_BYTES;
@@ -858,7 +915,7 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
       uint32_t item = atomicAdd(sched, 1u);
       publish(0, item);
       for (uint32_t it = 0; item < nitems; ++it) {
-        const AttnDqItem w = attn_dq_item(item, p, nqb);
+        const AttnDqItem w = attn_dq_item(item, p, nqb, doc_start);
         mbar_wait(qdo_empty(), (it & 1u) ^ 1u);                  // the previous item's S / dP MMAs have read Q, dO
         mbar_expect_tx(qdo_full(), 2 * ATC_TILE_BYTES);
         tma_load_3d(sQ, &maps.q, qdo_full(), w.h * ATC_D, w.q0, w.b);
@@ -870,10 +927,10 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
           const int st = g % ATC_DQ_NST;
           mbar_wait(kv_empty(st), ((g / ATC_DQ_NST) & 1u) ^ 1u);
           mbar_expect_tx(kv_full(st), 2 * ATC_HALF_TILE);
-          tma_load_3d(sK + st * ATC_HALF_TILE, &maps.k, kv_full(st), w.kvh * ATC_D, j * 64, w.b);
-          tma_load_3d(sK + st * ATC_HALF_TILE + 64 * 128, &maps.k, kv_full(st), w.kvh * ATC_D + 64, j * 64, w.b);
-          tma_load_3d(sV + st * ATC_HALF_TILE, &maps.v, kv_full(st), w.kvh * ATC_D, j * 64, w.b);
-          tma_load_3d(sV + st * ATC_HALF_TILE + 64 * 128, &maps.v, kv_full(st), w.kvh * ATC_D + 64, j * 64, w.b);
+          tma_load_3d(sK + st * ATC_HALF_TILE, &maps.k, kv_full(st), w.kvh * ATC_D, (w.j0 + j) * 64, w.b);
+          tma_load_3d(sK + st * ATC_HALF_TILE + 64 * 128, &maps.k, kv_full(st), w.kvh * ATC_D + 64, (w.j0 + j) * 64, w.b);
+          tma_load_3d(sV + st * ATC_HALF_TILE, &maps.v, kv_full(st), w.kvh * ATC_D, (w.j0 + j) * 64, w.b);
+          tma_load_3d(sV + st * ATC_HALF_TILE + 64 * 128, &maps.v, kv_full(st), w.kvh * ATC_D + 64, (w.j0 + j) * 64, w.b);
         }
         publish(it + 1, next);
         item = next;
@@ -909,7 +966,7 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
     for (uint32_t it = 0;; ++it) {
       const uint32_t item = get_item(it);
       if (item >= nitems) break;
-      const AttnDqItem w = attn_dq_item(item, p, nqb);
+      const AttnDqItem w = attn_dq_item(item, p, nqb, doc_start);
       const int iters = w.iters;
       mbar_wait(qdo_full(), it & 1u);
       issue_sdp(g0);
@@ -931,7 +988,7 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
           for (int kk = 0; kk < 4; ++kk)
             umma_f16_ts(tmem_base + ATC_DQ_ACC, tmem_base + buf * 64 + atc_half_operand_col(kk), desc_adv(ka, kk * 2048), idesc_acc,
                         (j | kk) != 0 ? 1u : 0u);
-          if (w.q0 < ATC_SPLIT_ROWS) {                                // early query rows: + dS_lo K
+          if (w.split) {                                // early query rows: + dS_lo K
 #pragma unroll
             for (int kk = 0; kk < 4; ++kk)
               umma_f16_ts(tmem_base + ATC_DQ_ACC, tmem_base + buf * 64 + 16 + atc_half_operand_col(kk), desc_adv(ka, kk * 2048),
@@ -955,12 +1012,13 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
     for (uint32_t it = 0;; ++it) {
       const uint32_t item = get_item(it);
       if (item >= nitems) break;
-      const AttnDqItem w = attn_dq_item(item, p, nqb);
+      const AttnDqItem w = attn_dq_item(item, p, nqb, doc_start);
       const int q0 = w.q0, qi = q0 + row;
       const bool valid = qi < p.S;
       const long long vidx = (static_cast<long long>(w.b) * p.nq + w.h) * p.S + qi;
       const float L2 = valid ? p.lse[vidx] * 1.4426950408889634f : INFINITY;
       const float Dr = valid ? p.dvec[vidx] : 0.f;
+      const int dstart = doc_start ? doc_start[min(qi, p.S - 1)] : 0;      // first key this query may see
       for (int j = 0; j < w.iters; ++j, ++g) {
         const int buf = g % ATC_DQ_NB;
         mbar_wait(sdp_full(buf), (g / ATC_DQ_NB) & 1u);
@@ -973,14 +1031,20 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
 #pragma unroll
         for (int i = 0; i < 32; ++i)
           ds[i] = ex2_approx(fmaf(__uint_as_float(sr[i]), c, -L2)) * (__uint_as_float(dr[i]) - Dr);
-        if (j * 64 + 63 > q0) {                                      // diagonal blocks: key > query is masked
-          const int krel = j * 64 + col0 - q0;
+        if ((w.j0 + j) * 64 + 63 > q0) {                             // diagonal blocks: key > query is masked
+          const int krel = (w.j0 + j) * 64 + col0 - q0;
 #pragma unroll
           for (int i = 0; i < 32; ++i)
             if (krel + i > row) ds[i] = 0.f;
         }
+        if (DOC && __any_sync(0xffffffffu, (w.j0 + j) * 64 + col0 < dstart)) {   // packed sequences: keys of earlier sequences
+          const int kabs = (w.j0 + j) * 64 + col0;
+#pragma unroll
+          for (int i = 0; i < 32; ++i)
+            if (kabs + i < dstart) ds[i] = 0.f;
+        }
         uint32_t pk[16];
-        if (q0 < ATC_SPLIT_ROWS) {
+        if (w.split) {
           uint32_t pl[16];
 #pragma unroll
           for (int i = 0; i < 16; ++i) atc_split_pack(ds[2 * i], ds[2 * i + 1], pk[i], pl[i]);
@@ -1007,7 +1071,7 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
       __syncwarp();
       if (lane == 0) mbar_arrive(acc_free());
       if (s0 < p.S) {
-        const float2* rr = (p.rope && valid) ? p.rope + static_cast<long long>(qi) * 64 + half * 32 : nullptr;
+        const float2* rr = (p.rope && valid) ? p.rope + static_cast<long long>(qi - dstart) * 64 + half * 32 : nullptr;
         atc_store_grad32(wst, reinterpret_cast<float(&)[32]>(a0), p.scale, rr, p.dq32 ? &maps.g32[0] : nullptr,
                          p.dq16 ? &maps.g16[0] : nullptr, w.h * ATC_D + half * 64, s0, w.b);
         atc_store_grad32(wst, reinterpret_cast<float(&)[32]>(a1), p.scale, rr ? rr + 16 : nullptr, p.dq32 ? &maps.g32[0] : nullptr,
@@ -1025,9 +1089,13 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
 inline cudaError_t attn_bwd_tc_set_attrs() {
   static bool set = false;
   if (!set) {
-    cudaError_t e = cudaFuncSetAttribute(attn_bwd_dkdv_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_BWD_SMEM);
+    cudaError_t e = cudaFuncSetAttribute(attn_bwd_dkdv_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_BWD_SMEM);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(attn_bwd_dq_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_DQ_SMEM);
+    e = cudaFuncSetAttribute(attn_bwd_dkdv_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_BWD_SMEM);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(attn_bwd_dq_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_DQ_SMEM);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(attn_bwd_dq_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_DQ_SMEM);
     if (e != cudaSuccess) return e;
     set = true;
   }
@@ -1051,7 +1119,8 @@ inline cudaError_t attn_bwd_dkdv_tc_launch(const __half* q, long long ldq, const
       (p.dk16 && !make_map_store(&m1.g16[1], p.dk16, p.nkv * ATC_D, p.S, p.B, p.ldd16, false)))
     return cudaErrorInvalidValue;
   dim3 g1((p.S + 127) / 128, p.nkv, p.B);
-  attn_bwd_dkdv_tc_kernel<<<g1, ATC_BWD_THREADS, ATC_BWD_SMEM, st>>>(m1, p);
+  if (p.doc_start) attn_bwd_dkdv_tc_kernel<true><<<g1, ATC_BWD_THREADS, ATC_BWD_SMEM, st>>>(m1, p);
+  else attn_bwd_dkdv_tc_kernel<false><<<g1, ATC_BWD_THREADS, ATC_BWD_SMEM, st>>>(m1, p);
   return cudaGetLastError();
 }
 
@@ -1071,7 +1140,8 @@ inline cudaError_t attn_bwd_dq_tc_launch(const __half* q, long long ldq, const _
     return cudaErrorInvalidValue;
   const int nitems = ((p.S + 127) / 128) * p.nq * p.B;
   const int grid = nitems < num_sms ? nitems : num_sms;        // persistent: one CTA per SM
-  attn_bwd_dq_tc_kernel<<<grid, ATC_BWD_THREADS, ATC_DQ_SMEM, st>>>(m2, p);
+  if (p.doc_start) attn_bwd_dq_tc_kernel<true><<<grid, ATC_BWD_THREADS, ATC_DQ_SMEM, st>>>(m2, p);
+  else attn_bwd_dq_tc_kernel<false><<<grid, ATC_BWD_THREADS, ATC_DQ_SMEM, st>>>(m2, p);
   return cudaGetLastError();
 }
 

@@ -470,6 +470,7 @@ struct EpiQKVRope {
   const float2* rope; int S, d;
   int rot_cols;              // columns [0, rot_cols) are rotated (Nq + Nkv, or 0 when use_rope = 0)
   CUtensorMap omap;
+  const int* doc_start = nullptr;      // packed sequences: the position of token m is m - doc_start[m] instead of m % S
   bool encode(int M, int N) { return make_map_store2d(&omap, out, M, N, ld, DT_F16); }
   __device__ __forceinline__ void prefetch(int, int, int, int, int) const {}      // the rope table stays L2-resident
   __device__ __forceinline__ void operator()(const WarpStage& st, int m_base, int n, float (&v)[32], int nrows, int nvalid) const {
@@ -478,7 +479,9 @@ struct EpiQKVRope {
       float cs[32];
       const int half_d = d >> 1, c0 = (n % d) >> 1;
       chunk_load<DT_F32>(st, [&](int rr) {
-        return reinterpret_cast<const float*>(rope + static_cast<long long>((m_base + rr) % S) * half_d + c0);
+        const int m = m_base + rr;
+        const int pos = doc_start ? m - __ldg(doc_start + m) : m % S;
+        return reinterpret_cast<const float*>(rope + static_cast<long long>(pos) * half_d + c0);
       }, cs, nrows, 32);
 #pragma unroll
       for (int j = 0; j < 16; ++j) {

@@ -71,6 +71,8 @@ struct lsp_ctx {
   cudaEvent_t ev[6];             // start, x in, dy in, fwd done, bwd done, copies out
   cudaEvent_t pev[2][6];         // lsp_layer_step_host_async, per call parity: x in, dy in, fwd done, bwd done, y out, dx out
   long long host_seq;            // number of async host steps issued
+  int* doc_start; int* doc_end;  // [T] each (device): packed-sequence bounds per token (lsp_set_packed_sequences)
+  int doc_on;
   const void* prev_y_dev; const void* prev_dx_dev;   // device result buffers of the previous async step
   int norm_blocks;      // persistent grid of the RMSNorm backward
   SavedLayout sv;
@@ -310,8 +312,10 @@ cudaError_t attn_fwd_dispatch(const lsp_ctx* c, const AttnParams& p, cudaStream_
     AttnTcParams t;
     t.B = p.B; t.S = p.S; t.nq = p.nq; t.nkv = p.nkv; t.scale_log2 = p.scale_log2; t.scale = p.scale;
     t.o32 = p.o32; t.o16 = p.o16; t.ldo = p.ldo; t.lse = p.lse; t.sched = c->attn_sched;
+    t.doc_start = c->doc_on ? c->doc_start : nullptr; t.doc_end = c->doc_on ? c->doc_end : nullptr;
     return attn_fwd_tc_launch(p.q, p.ldq, p.k, p.ldk, p.v, p.ldv, t, c->num_sms, st);
   }
+  if (c->doc_on) return cudaErrorNotSupported;            // packed sequences: head_dim 128 kernels only
   return attn_fwd_launch<64>(p, st);
 }
 
@@ -323,10 +327,12 @@ lsp_status attn_bwd_dispatch(lsp_ctx* ctx, const AttnParams& p, cudaStream_t st)
     t.lse = p.lse; t.dvec = p.dvec; t.rope = p.rope;
     t.dq32 = p.dq32; t.dk32 = p.dk32; t.dv32 = p.dv32; t.lddq32 = p.lddq32; t.lddk32 = p.lddk32;
     t.dq16 = p.dq16; t.dk16 = p.dk16; t.dv16 = p.dv16; t.ldd16 = p.ldd16; t.sched = ctx->attn_sched;
+    t.doc_start = ctx->doc_on ? ctx->doc_start : nullptr; t.doc_end = ctx->doc_on ? ctx->doc_end : nullptr;
     LSP_STAGE(ST_ATTN_BWD, 1, attn_bwd_dkdv_tc_launch(p.q, p.ldq, p.k, p.ldk, p.v, p.ldv, p.dO, p.lddo, t, st));
     LSP_STAGE(ST_ATTN_BWD_DQ, 1, attn_bwd_dq_tc_launch(p.q, p.ldq, p.k, p.ldk, p.v, p.ldv, p.dO, p.lddo, t, ctx->num_sms, st));
     return LSP_OK;
   }
+  if (ctx->doc_on) return fail(ctx, LSP_EUNSUPPORTED, "packed sequences need head_dim 128");
   LSP_STAGE(ST_ATTN_BWD, 2, attn_bwd_launch<64>(p, st));
   return LSP_OK;
 }
@@ -360,6 +366,7 @@ lsp_status attn_fwd_impl(lsp_ctx* ctx, int x_dt, const void* x, const lsp_layer_
   // F2 fused QKV projection with the RoPE epilogue (q, k rotated; v plain) into one [T, Nq+2Nkv] fp16 buffer
   {
     EpiQKVRope e{qkv, Nqkv, ctx->rope, d.seq, d.head_dim, d.use_rope ? Nq + Nkv : 0};
+    e.doc_start = ctx->doc_on ? ctx->doc_start : nullptr;
     LSP_STAGE(ST_QKV, 1, (gemm1<false, false>(ctx, T, Nqkv, H, Operand{xn, H, false}, Operand{wqkv16, H, false}, e, st)));
   }
   // F3 causal GQA flash forward
@@ -588,8 +595,9 @@ lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device
         cudaMemset(ctx->sk_flags, 0, pairs * 2 * sizeof(unsigned int)) != cudaSuccess ||
         cudaMalloc(&ctx->opt_partial, OPT_MAX_CHUNKS * opt_blocks_cap(ctx->num_sms) * sizeof(float)) != cudaSuccess ||
         cudaMalloc(&ctx->attn_sched, 16 * sizeof(unsigned int)) != cudaSuccess ||
+        cudaMalloc(&ctx->doc_start, 2 * static_cast<size_t>(ctx->T) * sizeof(int)) != cudaSuccess ||
         cudaMemset(ctx->attn_sched, 0, 16 * sizeof(unsigned int)) != cudaSuccess) {
-      cudaFree(ctx->sk_partial); cudaFree(ctx->sk_flags); cudaFree(ctx->attn_sched); cudaFree(ctx->opt_partial); cudaFree(ctx->rope); delete ctx;
+      cudaFree(ctx->sk_partial); cudaFree(ctx->sk_flags); cudaFree(ctx->attn_sched); cudaFree(ctx->opt_partial); cudaFree(ctx->doc_start); cudaFree(ctx->rope); delete ctx;
       return LSP_ENOMEM;
     }
   }
@@ -614,6 +622,7 @@ lsp_status lsp_destroy(lsp_ctx* ctx) {
   cudaFree(ctx->sk_flags);
   cudaFree(ctx->attn_sched);
   cudaFree(ctx->opt_partial);
+  cudaFree(ctx->doc_start);
   if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
   if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
   for (int i = 0; i < 6; ++i)
@@ -1031,6 +1040,27 @@ double lsp_lr_cosine(int step, double lr_max, double lr_min, int warmup, int tot
   if (warmup > 0 && step <= warmup) return lr_max * step / warmup;
   if (step >= total) return lr_min;
   return lr_min + 0.5 * (lr_max - lr_min) * (1.0 + cos(3.14159265358979323846 * (step - warmup) / (total - warmup)));
+}
+
+lsp_status lsp_set_packed_sequences(lsp_ctx* ctx, const int32_t* cu_seqlens_host, int32_t n_seqs, void* stream) {
+  if (!ctx) return LSP_EINVAL;
+  if (n_seqs == 0) { ctx->doc_on = 0; return LSP_OK; }
+  if (!cu_seqlens_host || n_seqs < 0) return LSP_EINVAL;
+  if (ctx->d.batch != 1 || ctx->d.head_dim != 128)
+    return fail(ctx, LSP_EUNSUPPORTED, "packed sequences need batch = 1 (seq = total tokens) and head_dim = 128");
+  const int T = ctx->T;
+  if (cu_seqlens_host[0] != 0 || cu_seqlens_host[n_seqs] != T) return fail(ctx, LSP_EINVAL, "cu_seqlens must run from 0 to batch*seq");
+  std::vector<int> host(2 * static_cast<size_t>(T));
+  for (int i = 0; i < n_seqs; ++i) {
+    const int a = cu_seqlens_host[i], b = cu_seqlens_host[i + 1];
+    if (b <= a) return fail(ctx, LSP_EINVAL, "cu_seqlens must be strictly increasing (sequence %d is empty)", i);
+    for (int t = a; t < b; ++t) { host[t] = a; host[T + t] = b; }
+  }
+  ctx->doc_end = ctx->doc_start + T;
+  // pageable source: the copy has left the host buffer when the call returns
+  LSP_CUDA(cudaMemcpyAsync(ctx->doc_start, host.data(), host.size() * sizeof(int), cudaMemcpyHostToDevice, static_cast<cudaStream_t>(stream)));
+  ctx->doc_on = 1;
+  return LSP_OK;
 }
 
 long long lsp_launch_count(const lsp_ctx* ctx) { return ctx ? ctx->launches : -1; }

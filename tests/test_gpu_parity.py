@@ -308,6 +308,84 @@ def test_sdpa_fwd_bwd(gpu, B_, S, nq, nkv, d):
     ctx.close()
 
 
+# ------------------------------------------------------------------------------------------- packed variable-length sequences
+PACKED = [[0, 130, 131, 400, 777, 1000], [0, 1000], [0, 64, 128, 192, 448, 449, 450, 1000], [0, 997, 1000]]
+
+
+@pytest.mark.parametrize("cu", PACKED, ids=lambda c: "x".join(str(b - a) for a, b in zip(c, c[1:])))
+def test_sdpa_packed_sequences(gpu, cu):
+    """lsp_set_packed_sequences + lsp_sdpa_fwd/bwd: 1000 tokens holding several sequences laid end to end (lengths 1 to
+    997; starts inside 64- and 128-row tiles, on tile boundaries, a sequence of one token) against the oracle run on
+    every sequence by itself; then packing is switched off again and the plain causal result must come back."""
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    S, nq, nkv, d = cu[-1], 6, 2, 128
+    w = synth.Workload("sdpa_packed", 55, 1, S, nq * d, nq, nkv, d, 64)
+    bits = synth.attn_inputs(w)
+    ctx = gpu.make_ctx(w, use_rope=False)
+    dev = torch.device("cuda")
+    t = {k: gpu.bf16_to_device(v) for k, v in bits.items()}
+    o = torch.empty((1, S, nq, d), dtype=torch.float32, device=dev)
+    lse = torch.empty((1, nq, S), dtype=torch.float32, device=dev)
+    dq = torch.empty_like(o)
+    dk = torch.empty((1, S, nkv, d), dtype=torch.float32, device=dev)
+    dv = torch.empty_like(dk)
+    ws = torch.empty(ctx.workspace_bytes, dtype=torch.uint8, device=dev)
+    i64 = f64(bits)
+
+    def run():
+        B.lsp_sdpa_fwd(ctx, t["q"], t["k"], t["v"], o, lse, ws)
+        B.lsp_sdpa_bwd(ctx, t["q"], t["k"], t["v"], o, lse, t["dO"], dq, dk, dv, ws)
+        torch.cuda.synchronize()
+        return dict(O=o.cpu().numpy(), L=lse.cpu().numpy(), dq=dq.cpu().numpy(), dk=dk.cpu().numpy(), dv=dv.cpu().numpy())
+
+    def oracle(bounds):
+        ref = dict(O=np.zeros((1, S, nq, d)), L=np.zeros((1, nq, S)), dq=np.zeros((1, S, nq, d)), dk=np.zeros((1, S, nkv, d)),
+                   dv=np.zeros((1, S, nkv, d)))
+        for a, b in zip(bounds, bounds[1:]):
+            sl = {k: v[:, a:b] for k, v in i64.items()}
+            ref["O"][:, a:b], ref["L"][:, :, a:b] = R.sdpa_fwd(sl["q"], sl["k"], sl["v"])
+            ref["dq"][:, a:b], ref["dk"][:, a:b], ref["dv"][:, a:b] = R.sdpa_bwd(sl["q"], sl["k"], sl["v"], sl["dO"])
+        return ref
+
+    names = ["O", "L", "dq", "dk", "dv"]
+    B.lsp_set_packed_sequences(ctx, cu)
+    check(run(), oracle(cu), names)
+    B.lsp_set_packed_sequences(ctx, None)
+    check(run(), oracle([0, S]), names)
+    ctx.close()
+
+
+def test_layer_packed_sequences(gpu):
+    """The whole layer on packed sequences (RoPE positions restart at every sequence start; attention stays inside a
+    sequence): y, dx and the nine gradients against the oracle run per sequence (weight gradients summed)."""
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    cu = [0, 200, 333, 334, 640]
+    w = synth.Workload("layer_packed", 56, 1, cu[-1], 512, 8, 2, 128, 1376, 1e-5, 500000.0)
+    dev = gpu.require_cuda()
+    ctx = gpu.make_ctx(w)
+    buf = gpu.LayerBuffers(ctx, w, dev)
+    bits_w, inp = synth.layer_weights(w), synth.layer_inputs(w)
+    weights = gpu.upload_weights(bits_w, dev)
+    x, dy = gpu.bf16_to_device(inp["x"], dev), gpu.bf16_to_device(inp["dy"], dev)
+    B.lsp_set_packed_sequences(ctx, cu)
+    B.lsp_layer_fwd(ctx, x, weights, buf.y, buf.saved, buf.ws)
+    B.lsp_layer_bwd(ctx, x, dy, weights, buf.saved, buf.dx, buf.grads, buf.ws)
+    torch.cuda.synchronize()
+    got = dict(y=buf.y.cpu().numpy(), dx=buf.dx.cpu().numpy())
+    got.update({"d" + k: v.cpu().numpy() for k, v in buf.grads.items()})
+    i64, w64 = f64(inp), f64(bits_w)
+    ref = {n: np.zeros(got[n].shape) for n in ALL}
+    for a, b in zip(cu, cu[1:]):
+        r = R.layer_fwd_bwd(i64["x"][a:b], i64["dy"][a:b], w64, oracle_shape(w.with_(seq=b - a)))
+        ref["y"][a:b], ref["dx"][a:b] = r["y"], r["dx"]
+        for n in ALL[2:]:
+            ref[n] += r[n]
+    check(got, ref, ALL)
+    ctx.close()
+
+
 # ------------------------------------------------------------------------------------------- embedding gather
 def test_embed_bit_exact(gpu):
     """lsp_embed_fwd: x0[t,:] = E[id_t,:], integer indexing -> bit-exact against the oracle."""
