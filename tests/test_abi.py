@@ -50,6 +50,23 @@ def test_null_arguments_are_rejected_without_a_gpu(libpath):
     assert lib.lsp_layer_fwd(None, None, None, None, None, None, None) == -1
 
 
+def test_create_rejects_bad_shapes_without_a_gpu(libpath):
+    """lsp_create checks the descriptor before it touches the device: empty and unsupported shapes come back as a
+    status, never as a crash or a silent fallback (include/lsp.h, error behaviour)."""
+    from paper_2510_02483_b200 import binding as B
+    B.lib()
+    ok = dict(batch=1, seq=128, hidden=256, n_q_heads=4, n_kv_heads=2, head_dim=64, ffn=688)
+    cases = [(dict(batch=0), "LSP_EINVAL"), (dict(seq=0), "LSP_EINVAL"), (dict(n_kv_heads=3), "LSP_EINVAL"),
+             (dict(head_dim=96), "LSP_EUNSUPPORTED"), (dict(hidden=260), "LSP_EUNSUPPORTED"), (dict(ffn=690), "LSP_EUNSUPPORTED"),
+             (dict(hidden=16384), "LSP_EUNSUPPORTED"), (dict(rope_layout=2), "LSP_EUNSUPPORTED"),
+             (dict(head_dim_logical=51), "LSP_EUNSUPPORTED"), (dict(head_dim_logical=80), "LSP_EUNSUPPORTED"),
+             (dict(head_dim_logical=52, rope_layout=1), "LSP_EUNSUPPORTED"), (dict(rope_base=0.0), "LSP_EINVAL"),
+             (dict(in_dtype=7), "LSP_EINVAL"), (dict(batch=1 << 20, seq=1 << 12), "LSP_EUNSUPPORTED")]
+    for kw, status in cases:
+        with pytest.raises(B.LspError, match=status):
+            B.Ctx(**dict(ok, **kw))
+
+
 def test_sass_is_blackwell_native(libpath):
     """The GEMM kernels must contain tcgen05 MMA (UTC*MMA), TMEM loads (LDTM) and TMA loads (UTMALDG)."""
     import subprocess
@@ -58,6 +75,7 @@ def test_sass_is_blackwell_native(libpath):
         pytest.skip("cuobjdump not available")
     sass = subprocess.run([cuobjdump, "-sass", libpath], capture_output=True, text=True).stdout
     assert re.search(r"UTC[A-Z]*MMA", sass) and "LDTM" in sass and "UTMALDG" in sass
+    assert "UTMASTG" in sass and "UTMAREDG" in sass          # TMA tensor stores and reduce-add stores (epilogues, wgrad accumulation)
 
 
 def test_lr_cosine_host_helper_matches_oracle(libpath):

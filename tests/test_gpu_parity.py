@@ -386,6 +386,44 @@ def test_layer_packed_sequences(gpu):
     ctx.close()
 
 
+def test_call_errors_are_statuses(gpu):
+    """Per-call argument errors come back as statuses with a message (no launch, no crash): misaligned and NULL pointers,
+    malformed cu_seqlens, packing on a batched context, optimizer tensors that are not multiples of 4, ragged vocab."""
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    w = MID
+    dev = gpu.require_cuda()
+    ctx = gpu.make_ctx(w)
+    buf = gpu.LayerBuffers(ctx, w, dev)
+    weights = gpu.upload_weights(synth.layer_weights(w, 0), dev)
+    x = gpu.bf16_to_device(synth.layer_inputs(w)["x"], dev)
+    with pytest.raises(B.LspError, match="LSP_EALIGN"):
+        B.lsp_layer_fwd(ctx, x.view(-1)[1:-1], weights, buf.y, buf.saved, buf.ws)
+    with pytest.raises(B.LspError, match="LSP_EALIGN"):
+        B.lsp_layer_fwd(ctx, x, weights, buf.y, buf.saved[16:], buf.ws)
+    with pytest.raises(B.LspError, match="LSP_EINVAL"):
+        B.lsp_layer_fwd(ctx, x, weights, None, buf.saved, buf.ws)
+    with pytest.raises(B.LspError, match="LSP_EUNSUPPORTED"):       # batch 2: packing needs one row
+        B.lsp_set_packed_sequences(ctx, [0, 100, w.tokens])
+    one = gpu.make_ctx(w.with_(batch=1, seq=w.tokens))
+    for bad in ([0, 100, 100, w.tokens], [0, 100, w.tokens - 1], [1, 100, w.tokens]):
+        with pytest.raises(B.LspError, match="LSP_EINVAL"):
+            B.lsp_set_packed_sequences(one, bad)
+    f = lambda n: torch.zeros(n, dtype=torch.float32, device=dev)
+    gn = torch.zeros(2, dtype=torch.float32, device=dev)
+    with pytest.raises(B.LspError, match="LSP_EINVAL"):
+        B.lsp_adamw_step(ctx, [dict(grad=f(6), master=f(6), m=f(6), v=f(6), weight=None)], lr=1e-3, step=1, gnorm_out=gn)
+    with pytest.raises(B.LspError, match="LSP_EINVAL"):
+        B.lsp_adamw_step(ctx, [dict(grad=f(8), master=f(8), m=f(8), v=f(8), weight=None)], lr=1e-3, step=0, gnorm_out=gn)
+    with pytest.raises(B.LspError, match="LSP_EINVAL"):
+        B.lsp_head_workspace_bytes(ctx, 1000) and B.lsp_head_fwd_bwd(ctx, x, x, x, x, 1001, gn, gn, x, gn, gn, buf.ws)
+    # the context still works after the refused calls
+    B.lsp_layer_fwd(ctx, x, weights, buf.y, buf.saved, buf.ws)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(buf.y).all())
+    one.close(); ctx.close()
+
+
 # ------------------------------------------------------------------------------------------- embedding gather
 def test_embed_bit_exact(gpu):
     """lsp_embed_fwd: x0[t,:] = E[id_t,:], integer indexing -> bit-exact against the oracle."""
