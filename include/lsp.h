@@ -61,6 +61,11 @@ typedef struct {
                              * (e.g. 104 -> 128, Table 1 30B: hidden 6656 / 64 heads): rows of wq/wk/wv and columns
                              * of wo beyond it are zero in every head; softmax scale 1/sqrt(logical) and RoPE frequencies
                              * base^(-2i/logical), identity on the padding (rope_layout 0 only) */
+  int32_t residual_scale_set; /* 0: the residual branches have weight 1 (a = x + attn(x), y = a + mlp(a)) */
+  float residual_scale;     /* used when residual_scale_set = 1: a = s*x + attn(x), y = s*a + mlp(a), and s * the incoming
+                             * residual gradients in the backward.  Tensor parallelism: every rank holds a
+                             * slice of the heads and FFN columns and produces a PARTIAL a / y / da / dx; rank 0 runs with
+                             * s = 1, the others with s = 0, and the sum over ranks is the full result (tp.py) */
 } lsp_layer_desc;
 
 typedef struct {

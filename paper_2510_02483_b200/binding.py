@@ -30,7 +30,8 @@ class lsp_layer_desc(C.Structure):
     _fields_ = [("batch", C.c_int32), ("seq", C.c_int32), ("hidden", C.c_int32), ("n_q_heads", C.c_int32),
                 ("n_kv_heads", C.c_int32), ("head_dim", C.c_int32), ("ffn", C.c_int32), ("rms_eps", C.c_float),
                 ("rope_base", C.c_double), ("rope_layout", C.c_int32), ("use_rope", C.c_int32),
-                ("in_dtype", C.c_int32), ("wgrad_accumulate", C.c_int32), ("head_dim_logical", C.c_int32)]
+                ("in_dtype", C.c_int32), ("wgrad_accumulate", C.c_int32), ("head_dim_logical", C.c_int32),
+                ("residual_scale_set", C.c_int32), ("residual_scale", C.c_float)]
 
 
 class lsp_layer_weights(C.Structure):
@@ -123,9 +124,10 @@ class Ctx:
     """Owns one lsp_ctx (a layer shape on a device)."""
 
     def __init__(self, *, batch, seq, hidden, n_q_heads, n_kv_heads, head_dim, ffn, rms_eps=1e-5, rope_base=10000.0,
-                 use_rope=True, in_dtype=LSP_BF16, device=0, rope_layout=0, wgrad_accumulate=False, head_dim_logical=0):
+                 use_rope=True, in_dtype=LSP_BF16, device=0, rope_layout=0, wgrad_accumulate=False, head_dim_logical=0, residual_scale=None):
         self.desc = lsp_layer_desc(batch, seq, hidden, n_q_heads, n_kv_heads, head_dim, ffn, rms_eps, rope_base, rope_layout,
-                                   1 if use_rope else 0, in_dtype, 1 if wgrad_accumulate else 0, head_dim_logical)
+                                   1 if use_rope else 0, in_dtype, 1 if wgrad_accumulate else 0, head_dim_logical,
+                                   0 if residual_scale is None else 1, 1.0 if residual_scale is None else float(residual_scale))
         self.handle = C.c_void_p()
         st = lib().lsp_create(C.byref(self.handle), C.byref(self.desc), device)
         if st != 0:

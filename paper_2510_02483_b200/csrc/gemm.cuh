@@ -394,6 +394,7 @@ struct EpiStore {
   CUtensorMap omap[3];       // store maps of the up-to-three outputs (encoded by the host in encode())
   int use_tma;               // 0 when a 32-row chunk can straddle a split (splits not multiples of 32): per-thread stores
   int accumulate = 0;        // 1: out += result (fp32 outputs; lsp_layer_desc.wgrad_accumulate) instead of out = result
+  float res_scale = 1.0f;    // weight of the residual (lsp_layer_desc.residual_scale: 0 on all but one tensor-parallel rank)
   int perm_d = 0;            // rope_layout = 1: head_dim; the rows of the segments in perm_segs leave through a 4-D map that
   unsigned perm_segs = 0;    // un-permutes them (dWq, dWk of the row-permuted projection weights)
   bool encode(int M, int N) {
@@ -433,7 +434,7 @@ struct EpiStore {
       const RT* rbase = reinterpret_cast<const RT*>(res) + static_cast<long long>(m_base) * ld + n;
       chunk_load<RDT>(st, [&](int rr) { return rbase + rr * ld; }, r, nrows, nvalid);
 #pragma unroll
-      for (int j = 0; j < 32; ++j) v[j] += r[j];
+      for (int j = 0; j < 32; ++j) v[j] = fmaf(res_scale, r[j], v[j]);
     }
     if (use_tma) {
       const int seg = (m_base >= split1) + (m_base >= split2);      // a 32-row chunk never straddles a split

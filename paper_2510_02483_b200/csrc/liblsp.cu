@@ -38,6 +38,8 @@ struct WsLayout {
 }  // namespace
 
 // softmax scale and RoPE frequencies follow the logical head width (zero-padded heads: head_dim_logical < head_dim)
+// weight of the residual branch: 1 unless the descriptor says otherwise (tensor-parallel ranks other than the first: 0)
+static inline float residual_scale(const lsp_layer_desc& d) { return d.residual_scale_set ? d.residual_scale : 1.0f; }
 static inline int logical_head_dim(const lsp_layer_desc& d) { return d.head_dim_logical > 0 ? d.head_dim_logical : d.head_dim; }
 
 // Pipeline stages (for launch counting and the optional per-stage device timing of lsp_timing_*).
@@ -203,7 +205,7 @@ cudaError_t norm_bwd_t(const lsp_ctx* c, const void* x, const float* rstd, const
     auto kern = rmsnorm_bwd_kernel<XT, RT, NV, GG>; \
     static bool set = false; \
     if (!set) { cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, NORMB_SMEM_BUDGET); if (e != cudaSuccess) return e; set = true; } \
-    kern<<<nb, NORMB_THREADS, smem, st>>>(xp, rstd, gp, dxn, rp, dx, dx16, dg_part, c->T, H, stages); } break;
+    kern<<<nb, NORMB_THREADS, smem, st>>>(xp, rstd, gp, dxn, rp, dx, dx16, dg_part, c->T, H, stages, residual_scale(c->d)); } break;
   if (G == 2) {
     switch (nv) { LSP_NB(1, 2) LSP_NB(2, 2) LSP_NB(3, 2) LSP_NB(4, 2) LSP_NB(5, 2) LSP_NB(6, 2) LSP_NB(7, 2) LSP_NB(8, 2) default: return cudaErrorInvalidValue; }
   } else {
@@ -299,10 +301,12 @@ cudaError_t gemm_fwd_residual(const lsp_ctx* c, const __half* A, int K, const __
   if (res_dt == LSP_F32) {
     EpiStore<DT_F32, DT_F32, true> e;
     e.out[0] = out; e.out[1] = e.out[2] = nullptr; e.split1 = e.split2 = 0x7fffffff; e.ld = H; e.res = res; e.alpha = 1.0f;
+    e.res_scale = residual_scale(c->d);
     return gemm1<false, false>(c, T, H, K, a, b, e, st);
   }
   EpiStore<DT_F32, DT_BF16, true> e;
   e.out[0] = out; e.out[1] = e.out[2] = nullptr; e.split1 = e.split2 = 0x7fffffff; e.ld = H; e.res = res; e.alpha = 1.0f;
+  e.res_scale = residual_scale(c->d);
   return gemm1<false, false>(c, T, H, K, a, b, e, st);
 }
 

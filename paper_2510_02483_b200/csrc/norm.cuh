@@ -117,7 +117,7 @@ template <typename XT, typename RT, int NV, int G>
 __global__ void __launch_bounds__(NORMB_THREADS, 1)
 rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, const __nv_bfloat16* __restrict__ g,
                    const float* __restrict__ dxn, const RT* __restrict__ dres, float* __restrict__ dx,
-                   __half* __restrict__ dx16, float* __restrict__ dg_part, int T, int H, int stages) {
+                   __half* __restrict__ dx16, float* __restrict__ dg_part, int T, int H, int stages, float res_scale) {
   // G row groups of GT = 256 / G consumer threads: group q takes this CTA's rows q, q + G, ... so that the reduction
   // latency of one row (shuffles, two named barriers) overlaps the loads and stores of the other group's row.
   constexpr int GT = NORMB_CONSUMERS / G;
@@ -196,10 +196,10 @@ rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, con
       const int c = (tg + i * GT) * 4;
       if (c < H) {
         float4 o;
-        o.x = rs[i].x + r * (dn[i].x - n[i].x * dot);
-        o.y = rs[i].y + r * (dn[i].y - n[i].y * dot);
-        o.z = rs[i].z + r * (dn[i].z - n[i].z * dot);
-        o.w = rs[i].w + r * (dn[i].w - n[i].w * dot);
+        o.x = fmaf(res_scale, rs[i].x, r * (dn[i].x - n[i].x * dot));
+        o.y = fmaf(res_scale, rs[i].y, r * (dn[i].y - n[i].y * dot));
+        o.z = fmaf(res_scale, rs[i].z, r * (dn[i].z - n[i].z * dot));
+        o.w = fmaf(res_scale, rs[i].w, r * (dn[i].w - n[i].w * dot));
         *reinterpret_cast<float4*>(dx + row * H + c) = o;
         if (dx16) store_f16x4(dx16 + row * H + c, o);
       }

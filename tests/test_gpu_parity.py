@@ -386,6 +386,30 @@ def test_layer_packed_sequences(gpu):
     ctx.close()
 
 
+@pytest.mark.parametrize("tp", [2, 4])
+def test_tensor_parallel_shards_sum_to_the_layer(gpu, tp):
+    """tp.TPLayer: the layer split over `tp` ranks by heads and FFN columns (residual_scale 1 on rank 0, 0 elsewhere),
+    the shards driven one after the other on this GPU and their partial a / y / da / dx added where the ranks would
+    all-reduce: y, dx and the re-assembled nine gradients against the oracle on the WHOLE layer."""
+    import torch
+    from paper_2510_02483_b200 import tp as TP
+    w = synth.Workload("tp_layer", 57, 2, 320, 512, 8, 4, 128, 1408, 1e-5, 500000.0)
+    bits, inp = synth.layer_weights(w), synth.layer_inputs(w)
+    dev = gpu.require_cuda()
+    x = gpu.bf16_to_device(inp["x"], dev).float()
+    dy = gpu.bf16_to_device(inp["dy"], dev).float()
+    shards = [TP.TPLayer(w, tp, r, bits, dev) for r in range(tp)]
+    y, dx = TP.phases(shards, x, dy)
+    torch.cuda.synchronize()
+    grads = TP.unshard_grads([{k: v.cpu().numpy() for k, v in s.buf.grads.items()} for s in shards], w)
+    got = dict(y=y.cpu().numpy(), dx=dx.cpu().numpy(), **{"d" + k: v for k, v in grads.items()})
+    i64 = f64(inp)
+    ref = R.layer_fwd_bwd(i64["x"], i64["dy"], f64(bits), oracle_shape(w))
+    check(got, ref, ALL)
+    for s in shards:
+        s.close()
+
+
 def test_call_errors_are_statuses(gpu):
     """Per-call argument errors come back as statuses with a message (no launch, no crash): misaligned and NULL pointers,
     malformed cu_seqlens, packing on a batched context, optimizer tensors that are not multiples of 4, ragged vocab."""
