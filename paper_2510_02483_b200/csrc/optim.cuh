@@ -78,30 +78,49 @@ __global__ void __launch_bounds__(OPT_THREADS) opt_norm_final_kernel(const float
 }
 
 // m <- b1 m + (1 - b1) g ; v <- b2 v + (1 - b2) g^2 ; p <- p - lr (m_hat / (sqrt(v_hat) + eps) + wd p) ; w = bf16(p)
+// Two float4 units per thread and iteration: eight independent 16-byte loads in flight before the first store.
 __global__ void __launch_bounds__(OPT_THREADS) opt_adamw_kernel(const OptTensors t, const OptHyper h, const float* __restrict__ norm_coef) {
   const long long total = t.start[t.n];
   const float c = norm_coef[1];
-  for (long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i < total; i += static_cast<long long>(gridDim.x) * blockDim.x) {
-    const int s = opt_segment(t, i);
-    const long long j = i - t.start[s];
-    const float4 g4 = __ldg(reinterpret_cast<const float4*>(t.g[s]) + j);
-    float4 p4 = reinterpret_cast<float4*>(t.p[s])[j];
-    float4 m4 = reinterpret_cast<float4*>(t.m[s])[j];
-    float4 v4 = reinterpret_cast<float4*>(t.v[s])[j];
-    const float wd = ((t.decay_mask >> s) & 1u) ? h.weight_decay : 0.f;
-    const float g[4] = {g4.x * c, g4.y * c, g4.z * c, g4.w * c};
-    float p[4] = {p4.x, p4.y, p4.z, p4.w}, m[4] = {m4.x, m4.y, m4.z, m4.w}, v[4] = {v4.x, v4.y, v4.z, v4.w};
+  const long long stride = static_cast<long long>(gridDim.x) * blockDim.x;
+  for (long long i0 = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i0 < total; i0 += 2 * stride) {
+    float4 g4[2], p4[2], m4[2], v4[2];
+    int sg[2];
+    long long jj[2];
 #pragma unroll
-    for (int e = 0; e < 4; ++e) {
-      m[e] = h.beta1 * m[e] + (1.0f - h.beta1) * g[e];
-      v[e] = h.beta2 * v[e] + (1.0f - h.beta2) * g[e] * g[e];
-      const float m_hat = m[e] * h.inv_bc1, v_hat = v[e] * h.inv_bc2;
-      p[e] = p[e] - h.lr * (m_hat / (sqrtf(v_hat) + h.eps) + wd * p[e]);
+    for (int u = 0; u < 2; ++u) {
+      const long long i = i0 + u * stride;
+      sg[u] = 0; jj[u] = 0;
+      if (i < total) {
+        sg[u] = opt_segment(t, i);
+        jj[u] = i - t.start[sg[u]];
+        g4[u] = __ldg(reinterpret_cast<const float4*>(t.g[sg[u]]) + jj[u]);
+        p4[u] = reinterpret_cast<float4*>(t.p[sg[u]])[jj[u]];
+        m4[u] = reinterpret_cast<float4*>(t.m[sg[u]])[jj[u]];
+        v4[u] = reinterpret_cast<float4*>(t.v[sg[u]])[jj[u]];
+      }
     }
-    reinterpret_cast<float4*>(t.p[s])[j] = make_float4(p[0], p[1], p[2], p[3]);
-    reinterpret_cast<float4*>(t.m[s])[j] = make_float4(m[0], m[1], m[2], m[3]);
-    reinterpret_cast<float4*>(t.v[s])[j] = make_float4(v[0], v[1], v[2], v[3]);
-    if (t.w[s]) reinterpret_cast<uint2*>(t.w[s])[j] = make_uint2(pack_bf16(p[0], p[1]), pack_bf16(p[2], p[3]));
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      if (i0 + u * stride >= total) continue;
+      const int s = sg[u];
+      const long long j = jj[u];
+      const float wd = ((t.decay_mask >> s) & 1u) ? h.weight_decay : 0.f;
+      const float g[4] = {g4[u].x * c, g4[u].y * c, g4[u].z * c, g4[u].w * c};
+      float p[4] = {p4[u].x, p4[u].y, p4[u].z, p4[u].w}, m[4] = {m4[u].x, m4[u].y, m4[u].z, m4[u].w},
+            v[4] = {v4[u].x, v4[u].y, v4[u].z, v4[u].w};
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        m[e] = h.beta1 * m[e] + (1.0f - h.beta1) * g[e];
+        v[e] = h.beta2 * v[e] + (1.0f - h.beta2) * g[e] * g[e];
+        const float m_hat = m[e] * h.inv_bc1, v_hat = v[e] * h.inv_bc2;
+        p[e] = p[e] - h.lr * (m_hat / (sqrtf(v_hat) + h.eps) + wd * p[e]);
+      }
+      reinterpret_cast<float4*>(t.p[s])[j] = make_float4(p[0], p[1], p[2], p[3]);
+      reinterpret_cast<float4*>(t.m[s])[j] = make_float4(m[0], m[1], m[2], m[3]);
+      reinterpret_cast<float4*>(t.v[s])[j] = make_float4(v[0], v[1], v[2], v[3]);
+      if (t.w[s]) reinterpret_cast<uint2*>(t.w[s])[j] = make_uint2(pack_bf16(p[0], p[1]), pack_bf16(p[2], p[3]));
+    }
   }
 }
 
