@@ -939,7 +939,7 @@ lsp_status lsp_head_fwd_bwd(lsp_ctx* ctx, const void* x, const void* g_final, co
   LSP_STAGE(ST_HEAD_GEMM, 1, (gemm1<false, false>(ctx, T, V, H, Operand{xn16, H, false}, Operand{w16, H, false}, epi_f32(logits, V), st)));
   // cross-entropy: lse, per-token loss, dz = (softmax - onehot) * 2^12 in fp16
   {
-    int blocks = ctx->num_sms < T ? ctx->num_sms : T;
+    int blocks = 2 * ctx->num_sms < T ? 2 * ctx->num_sms : T;      // two CTAs of 512 threads per SM: one row reduces while the other streams
     auto launch = [&]() {
       ce_fwd_bwd_kernel<<<blocks, CE_THREADS, 0, st>>>(logits, targets, T, V, lse, loss_row, dz16);
       ce_loss_mean_kernel<<<1, 32, 0, st>>>(loss_row, T, loss);
