@@ -110,6 +110,11 @@ lsp_status lsp_mlp_bwd(lsp_ctx* ctx, const void* a, const void* dy, const lsp_la
 lsp_status lsp_layer_fwd(lsp_ctx* ctx, const void* x, const lsp_layer_weights* w, void* y_out, void* saved, void* ws,
                          void* stream);
 /* x: the forward input; dy in_dtype -> dx fp32; writes all nine gradients. */
+/* Forward pass only (inference-style): the same y as lsp_layer_fwd, bit for bit, without the tensors
+ * only a backward pass would read (the fp16 gate / up pre-activations, the fp32 copy of O).  `scratch` is
+ * lsp_saved_bytes(ctx) of device memory used for the intermediates; it is NOT a valid `saved` for lsp_layer_bwd. */
+lsp_status lsp_layer_fwd_infer(lsp_ctx* ctx, const void* x, const lsp_layer_weights* w, void* y_out, void* scratch, void* ws,
+                               void* stream);
 lsp_status lsp_layer_bwd(lsp_ctx* ctx, const void* x, const void* dy, const lsp_layer_weights* w, const void* saved,
                          void* dx, lsp_layer_wgrads* grads, void* ws, void* stream);
 

@@ -19,7 +19,7 @@ EXPORTS = ("lsp_create", "lsp_destroy", "lsp_saved_bytes", "lsp_workspace_bytes"
            "lsp_attn_fwd", "lsp_attn_bwd", "lsp_mlp_fwd", "lsp_mlp_bwd", "lsp_layer_fwd", "lsp_layer_bwd",
            "lsp_sdpa_fwd", "lsp_sdpa_bwd", "lsp_embed_fwd", "lsp_gemm", "lsp_layer_step_host", "lsp_launch_count",
            "lsp_timing_enable", "lsp_timing_read", "lsp_adamw_step", "lsp_lr_cosine", "lsp_head_workspace_bytes",
-           "lsp_head_fwd_bwd", "lsp_embed_bwd", "lsp_layer_step_host_async", "lsp_host_copies_wait", "lsp_set_packed_sequences")
+           "lsp_head_fwd_bwd", "lsp_embed_bwd", "lsp_layer_step_host_async", "lsp_host_copies_wait", "lsp_set_packed_sequences", "lsp_layer_fwd_infer")
 
 
 class LspError(RuntimeError):
@@ -74,6 +74,7 @@ def lib():
         L.lsp_mlp_fwd.argtypes = [vp, vp, pw, vp, vp, vp, vp]
         L.lsp_mlp_bwd.argtypes = [vp, vp, vp, pw, vp, vp, pg, vp, vp]
         L.lsp_layer_fwd.argtypes = [vp, vp, pw, vp, vp, vp, vp]
+        L.lsp_layer_fwd_infer.argtypes = [vp, vp, pw, vp, vp, vp, vp]
         L.lsp_layer_bwd.argtypes = [vp, vp, vp, pw, vp, vp, pg, vp, vp]
         L.lsp_sdpa_fwd.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
         L.lsp_sdpa_bwd.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -178,6 +179,11 @@ def lsp_mlp_bwd(ctx, a, dy, weights, saved, da, grads, ws, stream=None):
     w, g = _pack(lsp_layer_weights, weights), _pack(lsp_layer_wgrads, grads)
     ctx.check(lib().lsp_mlp_bwd(ctx.handle, _ptr(a), _ptr(dy), C.byref(w), _ptr(saved), _ptr(da), C.byref(g), _ptr(ws),
                                 _stream(stream)))
+
+
+def lsp_layer_fwd_infer(ctx, x, weights, y_out, scratch, ws, stream=None):
+    w = _pack(lsp_layer_weights, weights)
+    ctx.check(lib().lsp_layer_fwd_infer(ctx.handle, _ptr(x), C.byref(w), _ptr(y_out), _ptr(scratch), _ptr(ws), _stream(stream)))
 
 
 def lsp_layer_fwd(ctx, x, weights, y_out, saved, ws, stream=None):

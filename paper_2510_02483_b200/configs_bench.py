@@ -79,14 +79,16 @@ def bench_layer_packed(w, steps, cu):
     return ms, gemm * w.tokens + attn
 
 
-def bench_layer_fwd_only(w, steps):
-    """Forward pass alone (SURVEY.md 8(f) #3: the forward-only variant, prefill-style): lsp_layer_fwd, device-resident."""
+def bench_layer_fwd_only(w, steps, infer=False):
+    """Forward pass alone (the forward-only variant, prefill-style), device-resident: lsp_layer_fwd, or
+    lsp_layer_fwd_infer (nothing kept for a backward pass)."""
     dev = harness.require_cuda()
     ctx = harness.make_ctx(w)
     buf = harness.LayerBuffers(ctx, w, dev)
     weights = harness.upload_weights(synth.layer_weights(w), dev)
     x = harness.bf16_to_device(synth.layer_inputs(w)["x"], dev)
-    ms = _time(lambda: B.lsp_layer_fwd(ctx, x, weights, buf.y, buf.saved, buf.ws), steps)
+    fn = B.lsp_layer_fwd_infer if infer else B.lsp_layer_fwd
+    ms = _time(lambda: fn(ctx, x, weights, buf.y, buf.saved, buf.ws), steps)
     ctx.close()
     return ms, synth.layer_flops(w, causal=True) / 3.0 - synth.attn_flops_fwd(w, causal=True) * (3.5 / 3.0 - 1.0)
 
@@ -191,6 +193,7 @@ def main(argv=None):
         jobs.append((wp.with_(name="cfg2_3b_layer_one_sequence_of_16384"), lambda w, steps: bench_layer_packed(w, steps, [0, 16384])))
     if "fwd" in only:
         jobs.append((synth.CFG2_3B_LAYER.with_(name="cfg2_3b_layer_forward_only"), bench_layer_fwd_only))
+        jobs.append((synth.CFG2_3B_LAYER.with_(name="cfg2_3b_layer_forward_infer"), lambda w, steps: bench_layer_fwd_only(w, steps, True)))
     if "cfg4" in only:
         jobs.append((synth.CFG4_30B_LAYER, bench_layer))
     if "table1" in only:      # the paper's own Table-1 3B layer shape: hidden 2048, 16q / 2kv, FFN 11008

@@ -500,15 +500,19 @@ struct EpiSwiGLU {
   static constexpr bool kStoreOnly = true;
   __half* h; __half* g16; __half* u16; long long ld;
   CUtensorMap hmap, gmap, umap;
+  int save_gu = 1;           // 0: forward-only call, g and u are not kept for a backward pass
   bool encode(int M, int N) {
-    return make_map_store2d(&hmap, h, M, N, ld, DT_F16) && make_map_store2d(&gmap, g16, M, N, ld, DT_F16) &&
-           make_map_store2d(&umap, u16, M, N, ld, DT_F16);
+    if (!make_map_store2d(&hmap, h, M, N, ld, DT_F16)) return false;
+    if (!save_gu) { gmap = hmap; umap = hmap; return true; }
+    return make_map_store2d(&gmap, g16, M, N, ld, DT_F16) && make_map_store2d(&umap, u16, M, N, ld, DT_F16);
   }
   __device__ __forceinline__ void prefetch(int, int, int, int, int) const {}
   __device__ __forceinline__ void operator()(const WarpStage& st, int m_base, int n, float (&g)[32], float (&u)[32], int nrows,
                                              int nvalid) const {
-    chunk_store_tma<DT_F16>(st, &gmap, n, m_base, g);
-    chunk_store_tma<DT_F16>(st, &umap, n, m_base, u);
+    if (save_gu) {
+      chunk_store_tma<DT_F16>(st, &gmap, n, m_base, g);
+      chunk_store_tma<DT_F16>(st, &umap, n, m_base, u);
+    }
 #pragma unroll
     for (int j = 0; j < 32; ++j) {
       const float sg = __fdividef(1.0f, 1.0f + __expf(-g[j]));   // MUFU.EX2 + MUFU.RCP: 2 ulp, far below the 16-bit outputs

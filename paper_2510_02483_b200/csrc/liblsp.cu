@@ -344,7 +344,7 @@ lsp_status attn_bwd_dispatch(lsp_ctx* ctx, const AttnParams& p, cudaStream_t st)
 // ------------------------------------------------------------------------------------------- attention block
 // x [T,H] x_dt -> a32 [T,H] fp32.  SURVEY 8(a) F1-F4.
 lsp_status attn_fwd_impl(lsp_ctx* ctx, int x_dt, const void* x, const lsp_layer_weights* w, float* a_out, void* saved,
-                         cudaStream_t st) {
+                         cudaStream_t st, bool keep = true) {
   const lsp_layer_desc& d = ctx->d;
   const int T = ctx->T, H = d.hidden, Nq = ctx->Nq, Nkv = ctx->Nkv, Nqkv = ctx->Nqkv;
   __half* xn = at<__half>(saved, ctx->sv.xn);
@@ -381,7 +381,7 @@ lsp_status attn_fwd_impl(lsp_ctx* ctx, int x_dt, const void* x, const lsp_layer_
   p.B = d.batch; p.S = d.seq; p.nq = d.n_q_heads; p.nkv = d.n_kv_heads;
   p.scale = 1.0f / sqrtf(static_cast<float>(logical_head_dim(d)));
   p.scale_log2 = p.scale * 1.4426950408889634f;
-  p.o32 = o32; p.o16 = o16; p.ldo = Nq; p.lse = lse;
+  p.o32 = keep ? o32 : nullptr; p.o16 = o16; p.ldo = Nq; p.lse = lse;     // the fp32 copy of O only feeds the backward (P-3)
   LSP_STAGE(ST_ATTN_FWD, 1, attn_fwd_dispatch(ctx, p, st));
   // F4 O-projection + residual
   LSP_STAGE(ST_OPROJ, 1, gemm_fwd_residual(ctx, o16, Nq, wo16, x_dt, x, a_out, st));
@@ -446,7 +446,8 @@ lsp_status attn_bwd_impl(lsp_ctx* ctx, int x_dt, const void* x, int da_dt, const
 
 // ------------------------------------------------------------------------------------------- MLP block
 // a (a_dt) -> y fp32.  SURVEY 8(a) F5-F7.
-lsp_status mlp_fwd_impl(lsp_ctx* ctx, int a_dt, const void* a, const lsp_layer_weights* w, float* y, void* saved, cudaStream_t st) {
+lsp_status mlp_fwd_impl(lsp_ctx* ctx, int a_dt, const void* a, const lsp_layer_weights* w, float* y, void* saved, cudaStream_t st,
+                        bool keep = true) {
   const lsp_layer_desc& d = ctx->d;
   const int T = ctx->T, H = d.hidden, F = d.ffn;
   __half* an = at<__half>(saved, ctx->sv.an);
@@ -465,6 +466,7 @@ lsp_status mlp_fwd_impl(lsp_ctx* ctx, int a_dt, const void* a, const lsp_layer_w
   }
   LSP_STAGE(ST_NORM_FWD, 1, norm_fwd(ctx, a_dt, a, w->g_mlp, an, rstd2, st));
   EpiSwiGLU e{h, g16, u16, F};
+  e.save_gu = keep ? 1 : 0;
   const GemmSKRes sk{ctx->sk_partial, ctx->sk_flags, ++ctx->gemm_seq};
   LSP_STAGE(ST_GATEUP, 1, gemm_run_dual(T, F, H, Operand{an, H, false}, Operand{wgu16, H, false}, Operand{wgu16 + FH, H, false}, e,
                          ctx->num_sms, st, &sk));
@@ -685,6 +687,17 @@ lsp_status lsp_layer_fwd(lsp_ctx* ctx, const void* x, const lsp_layer_weights* w
   float* a32 = at<float>(saved, ctx->sv.a32);
   LSP_TRY(attn_fwd_impl(ctx, ctx->d.in_dtype, x, w, a32, saved, st));
   return mlp_fwd_impl(ctx, LSP_F32, a32, w, static_cast<float*>(y_out), saved, st);
+}
+
+lsp_status lsp_layer_fwd_infer(lsp_ctx* ctx, const void* x, const lsp_layer_weights* w, void* y_out, void* scratch, void* ws,
+                               void* stream) {
+  if (!ctx || !w) return LSP_EINVAL;
+  const void* ptrs[] = {x, y_out, scratch, ws, w->wq, w->wk, w->wv, w->wo, w->g_attn, w->w_gate, w->w_up, w->w_down, w->g_mlp};
+  LSP_TRY(check_common(ctx, scratch, ws, 13, ptrs));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  float* a32 = at<float>(scratch, ctx->sv.a32);
+  LSP_TRY(attn_fwd_impl(ctx, ctx->d.in_dtype, x, w, a32, scratch, st, false));
+  return mlp_fwd_impl(ctx, LSP_F32, a32, w, static_cast<float*>(y_out), scratch, st, false);
 }
 
 lsp_status lsp_layer_bwd(lsp_ctx* ctx, const void* x, const void* dy, const lsp_layer_weights* w, const void* saved, void* dx,

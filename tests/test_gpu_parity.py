@@ -218,6 +218,24 @@ def test_layer_padded_heads_104(gpu):
     check(got, ref, ALL)
 
 
+def test_layer_fwd_infer_matches_training_forward(gpu):
+    """lsp_layer_fwd_infer (no tensors kept for a backward pass) returns the same y as lsp_layer_fwd, bit for bit."""
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    for w in (synth.CFG1_TINY, MID):
+        ref = gpu.run_layer(w)
+        dev = gpu.require_cuda()
+        ctx = gpu.make_ctx(w)
+        buf = gpu.LayerBuffers(ctx, w, dev)
+        weights = gpu.upload_weights(synth.layer_weights(w, 0), dev)
+        x = gpu.bf16_to_device(synth.layer_inputs(w)["x"], dev)
+        buf.saved.fill_(0xFF)
+        B.lsp_layer_fwd_infer(ctx, x, weights, buf.y, buf.saved, buf.ws)
+        torch.cuda.synchronize()
+        assert np.array_equal(buf.y.cpu().numpy(), ref["y"]), w.name
+        ctx.close()
+
+
 def test_layer_step_host_matches_device_path(gpu):
     """lsp_layer_step_host (pinned HOST x, dy in; y, dx out; copies on context-owned streams overlapping the compute
     stream) returns exactly what lsp_layer_fwd + lsp_layer_bwd produce from device-resident inputs."""
