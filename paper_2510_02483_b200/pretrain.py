@@ -22,12 +22,14 @@ from . import dp, harness, replicas, synth
 
 class PretrainStep:
     def __init__(self, w: synth.Workload, n_layers: int, vocab: int, dev=None, weights=None, embedding=None, head=None, g_final=None,
-                 world: int = 1, group=None, micro_batches: int = 1):
+                 world: int = 1, group=None, micro_batches: int = 1, recompute: bool = False):
         """weights: optional list of per-layer dicts of bf16 bit patterns (synth.layer_weights layout); embedding / head:
         bf16 bit patterns [vocab, H]; g_final: bf16 bits [H].  Defaults: the seeded synthetic tensors of synth.py.
         `w` is one MICRO-batch of this rank's shard; micro_batches > 1: gradient accumulation (the paper's global batch of
         256 sequences, Table 2, does not fit one step) -- the first micro-batch overwrites the gradient buffers,
-        the others run on a second context created with wgrad_accumulate = 1; world > 1: data-parallel replicas (dp.py)."""
+        the others run on a second context created with wgrad_accumulate = 1; world > 1: data-parallel replicas (dp.py);
+        recompute: keep only every layer's INPUT from the forward pass and re-run the layer's forward in front of its
+        backward (one shared `saved` buffer instead of n_layers: activation memory / n_layers for one more forward)."""
         self.dev = dev or harness.require_cuda()
         self.w, self.L, self.V = w, n_layers, vocab
         self.ctx = harness.make_ctx(w, in_dtype=B.LSP_F32)
@@ -35,7 +37,10 @@ class PretrainStep:
         self.ctx_acc = harness.make_ctx(w, in_dtype=B.LSP_F32, wgrad_accumulate=True) if micro_batches > 1 else None
         T, H = w.tokens, w.hidden
         f32 = dict(dtype=torch.float32, device=self.dev)
-        self.saved = [torch.empty(self.ctx.saved_bytes, dtype=torch.uint8, device=self.dev) for _ in range(n_layers)]
+        self.recompute = recompute
+        shared = torch.empty(self.ctx.saved_bytes, dtype=torch.uint8, device=self.dev) if recompute else None
+        self.saved = [shared if recompute else torch.empty(self.ctx.saved_bytes, dtype=torch.uint8, device=self.dev)
+                      for _ in range(n_layers)]
         self.ws = torch.empty(max(self.ctx.workspace_bytes, B.lsp_head_workspace_bytes(self.ctx, vocab)), dtype=torch.uint8, device=self.dev)
         self.xs = [torch.empty((T, H), **f32) for _ in range(n_layers + 1)]
         self.d = [torch.empty((T, H), **f32) for _ in range(2)]
@@ -104,6 +109,8 @@ class PretrainStep:
             self.buckets.reduce_async(L)
         for l in range(L - 1, -1, -1):
             d_out = self.d[l & 1]
+            if self.recompute and l != L - 1:           # the shared buffer still holds the last layer's activations
+                B.lsp_layer_fwd(c, self.xs[l], self.layer_w[l], self.xs[l + 1], self.saved[l], self.ws, stream)
             B.lsp_layer_bwd(c, self.xs[l], d_in, self.layer_w[l], self.saved[l], d_out, self.layer_g[l], self.ws, stream)
             if last:
                 self.buckets.reduce_async(l)        # overlaps the next layer's backward
@@ -140,6 +147,7 @@ def main(argv=None):
     ap.add_argument("--layers", type=int, default=synth.CFG3_3B_STACK.n_layers)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=2)
+    ap.add_argument("--recompute", action="store_true", help="keep layer inputs only; re-run each layer's forward before its backward")
     args = ap.parse_args(argv)
     w = synth.CFG3_3B_STACK
     # under torchrun: data-parallel replicas, every rank takes a batch of the config's size (weak scaling) with its own ids
@@ -148,7 +156,7 @@ def main(argv=None):
         torch.cuda.set_device(renv.local_rank)
     dev = harness.require_cuda()
     replicas.init("nccl", renv)
-    run = PretrainStep(w, args.layers, w.vocab, dev, world=renv.world_size)
+    run = PretrainStep(w, args.layers, w.vocab, dev, world=renv.world_size, recompute=args.recompute)
     s = synth.stack_inputs(w)
     ids = torch.from_numpy(s["ids"]).to(dev)
     ids = torch.roll(ids, 997 * renv.rank)
@@ -172,7 +180,7 @@ def main(argv=None):
     # the paper's accounting: 6 FLOPs per parameter per token without the embedding table, plus attention
     flops = renv.world_size * (6.0 * (n - w.vocab * w.hidden) * w.tokens + args.layers * 3.5 * synth.attn_flops_fwd(w, causal=True))
     if renv.is_main:
-        print(json.dumps({"config": f"pretrain_{w.name}_L{args.layers}", "n_gpus": renv.world_size, "params": n, "tokens": int(tokens),
+        print(json.dumps({"config": f"pretrain_{w.name}_L{args.layers}" + ("_recompute" if args.recompute else ""), "n_gpus": renv.world_size, "params": n, "tokens": int(tokens),
                           "ms_fwd_bwd": round(ms_fb, 3), "ms_adamw": round(ms_opt, 3), "ms_iteration": round(ms_it, 3),
                           "tokens_per_s": round(tok_s, 1), "model_tflops": round(flops / (ms_it * 1e-3) / 1e12, 1),
                           "adamw_GB_per_s": round(34.0 * n / (ms_opt * 1e-3) / 1e9, 1),

@@ -799,3 +799,23 @@ def test_pretrain_micro_batches_vs_oracle(gpu):
     norm_ref = A.global_grad_norm(ref_g)
     assert abs(float(run.gnorm[0].cpu()) - norm_ref) <= 5e-3 * norm_ref
     run.close()
+
+
+def test_pretrain_recompute_is_bit_identical(gpu):
+    """PretrainStep(recompute=True) -- layer inputs kept, each layer's forward re-run in front of its backward, one shared
+    `saved` buffer -- gives the same loss and the same gradients, bit for bit, as keeping every layer's activations."""
+    import torch
+    from paper_2510_02483_b200 import pretrain
+    w = synth.Workload("pretrain_rc", 11, 2, 192, 256, 4, 2, 128, 688, 1e-5, 500000.0, 3, 1000)
+    ids = synth.stack_inputs(w)["ids"]
+    tid = torch.from_numpy(ids).cuda(); tt = torch.from_numpy(np.roll(ids, -1)).cuda()
+    outs = []
+    for rc in (False, True):
+        run = pretrain.PretrainStep(w, w.n_layers, w.vocab, recompute=rc)
+        run.forward_backward(tid, tt)
+        torch.cuda.synchronize()
+        outs.append((float(run.loss.cpu()), [p["grad"].cpu().numpy().copy() for p in run.params]))
+        run.close()
+    assert outs[0][0] == outs[1][0]
+    for a, b in zip(outs[0][1], outs[1][1]):
+        assert np.array_equal(a, b)
