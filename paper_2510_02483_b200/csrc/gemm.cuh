@@ -49,7 +49,7 @@ struct GemmShape {
   // stream-K tail of the CTA-pair kernel (all zero / null: data-parallel only)
   int sk_split;                      // s >= 2: the T mod C tiles of the last wave are each cut into s K-slices (0: off)
   float* sk_partial;                 // [clusters][2 CTAs][8 chunks][128 rows][32] fp32 partial accumulators
-  unsigned int* sk_flags;            // [clusters][2]: epoch of the partial last published by that CTA
+  unsigned int* sk_flags;            // [clusters][2]: epoch of the partial published by that CTA; 0 again once consumed
   unsigned int sk_epoch;             // unique per launch on this context, > 0
 };
 
@@ -1037,6 +1037,11 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive_cluster(acc == 0 ? tempty_leader0 : tempty_leader1);
+      if (it.mode == 2) {                       // every epilogue thread has read the partials: re-arm their flags, so that a
+        named_bar_sync_gemm(1, GEMM_EPI_WARPS * 32);          // replay of this launch with the same epoch (CUDA graph) waits again
+        if (warp == 2 && lane == 0)
+          for (int jj = 0; jj < work.split - 1; ++jj) sh.sk_flags[(jj * work.rem + t_sk) * 2 + rank] = 0u;
+      }
       if (it.mode == 1) {                       // all 8 epilogue warps of this CTA have stored: publish
         named_bar_sync_gemm(1, GEMM_EPI_WARPS * 32);
         if (warp == 2 && lane == 0) {

@@ -819,3 +819,48 @@ def test_pretrain_recompute_is_bit_identical(gpu):
     assert outs[0][0] == outs[1][0]
     for a, b in zip(outs[0][1], outs[1][1]):
         assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("w", [synth.CFG1_TINY, MID], ids=lambda w: w.name)
+def test_layer_step_replays_from_a_cuda_graph(gpu, w):
+    """lsp_layer_fwd + lsp_layer_bwd captured into a CUDA graph (torch.cuda.graph: the library enqueues on the capturing
+    stream, allocates and synchronises nothing) and replayed three times over cleared outputs: every replay equals the
+    eager step bit for bit -- the split-K flags of the GEMM tail and the work-queue counters of the persistent attention
+    kernels re-arm themselves inside the launch, so a replay with frozen kernel parameters is safe."""
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    ref = gpu.run_layer(w)
+    dev = gpu.require_cuda()
+    ctx = gpu.make_ctx(w)
+    buf = gpu.LayerBuffers(ctx, w, dev)
+    weights = gpu.upload_weights(synth.layer_weights(w, 0), dev)
+    inp = synth.layer_inputs(w)
+    x, dy = gpu.bf16_to_device(inp["x"], dev), gpu.bf16_to_device(inp["dy"], dev)
+
+    def step():
+        B.lsp_layer_fwd(ctx, x, weights, buf.y, buf.saved, buf.ws)
+        B.lsp_layer_bwd(ctx, x, dy, weights, buf.saved, buf.dx, buf.grads, buf.ws)
+    step()                                            # eager once: function attributes are set outside the capture
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        step()
+    for _ in range(3):
+        for t in [buf.y, buf.dx] + list(buf.grads.values()):
+            t.fill_(float("nan"))
+        graph.replay()
+        torch.cuda.synchronize()
+        got = dict(y=buf.y.cpu().numpy(), dx=buf.dx.cpu().numpy(), **{"d" + k: v.cpu().numpy() for k, v in buf.grads.items()})
+        for n in ALL:
+            assert np.array_equal(got[n], ref[n]), n
+    # launch-bound shapes gain from the replay: report both
+    def timed(fn, n=20):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        fn(); torch.cuda.synchronize(); e0.record()
+        for _ in range(n):
+            fn()
+        e1.record(); torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+    print(f"{w.name}: eager {timed(step):.4f} ms/step, graph replay {timed(graph.replay):.4f} ms/step")
+    del graph
+    ctx.close()
