@@ -206,6 +206,12 @@ typedef struct {
   int32_t step;                                            /* 1-based optimizer step t (bias correction 1 - beta^t) */
   float grad_scale;                                        /* > 0: the stored gradients are grad_scale x the true ones
                                                               (lsp_head_fwd_bwd); norm, clipping and update use g / grad_scale */
+  int32_t phase;                                           /* 0: the whole step.  Sharded optimizer state (ZeRO stage 1,
+                                                              PAPER.md:73), every rank holding a slice of the tensors:
+                                                              1 = only gnorm_out[0] <- sum of g^2 over this call's
+                                                              (stored) gradients; the caller all-reduces that scalar;
+                                                              2 = gnorm_out[0] holds the global sum: norm, clipping
+                                                              coefficient and the update of this call's tensors */
 } lsp_adamw_desc;
 lsp_status lsp_adamw_step(lsp_ctx* ctx, int ntensors, const lsp_adamw_tensor* tensors, const lsp_adamw_desc* desc,
                           float* gnorm_out, void* stream);

@@ -45,7 +45,7 @@ class lsp_adamw_tensor(C.Structure):
 
 class lsp_adamw_desc(C.Structure):
     _fields_ = [("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float),
-                ("weight_decay", C.c_float), ("clip_norm", C.c_float), ("step", C.c_int32), ("grad_scale", C.c_float)]
+                ("weight_decay", C.c_float), ("clip_norm", C.c_float), ("step", C.c_int32), ("grad_scale", C.c_float), ("phase", C.c_int32)]
 
 
 class lsp_layer_wgrads(C.Structure):
@@ -243,14 +243,14 @@ def lsp_host_copies_wait(ctx, stream=None):
 
 
 def lsp_adamw_step(ctx, tensors, *, lr, step, gnorm_out, beta1=0.90, beta2=0.95, eps=1e-8, weight_decay=0.01, clip_norm=1.0,
-                   grad_scale=1.0, stream=None):
+                   grad_scale=1.0, phase=0, stream=None):
     """tensors: list of dicts {grad, master, m, v, weight (bf16 or None), decay (bool)} of torch CUDA tensors."""
     arr = (lsp_adamw_tensor * len(tensors))()
     for i, t in enumerate(tensors):
         w = t.get("weight")
         arr[i] = lsp_adamw_tensor(t["grad"].data_ptr(), t["master"].data_ptr(), t["m"].data_ptr(), t["v"].data_ptr(),
                                   None if w is None else w.data_ptr(), t["master"].numel(), 1 if t.get("decay", True) else 0)
-    d = lsp_adamw_desc(lr, beta1, beta2, eps, weight_decay, clip_norm, step, grad_scale)
+    d = lsp_adamw_desc(lr, beta1, beta2, eps, weight_decay, clip_norm, step, grad_scale, phase)
     ctx.check(lib().lsp_adamw_step(ctx.handle, len(tensors), arr, C.byref(d), _ptr(gnorm_out), _stream(stream)))
 
 

@@ -1034,22 +1034,30 @@ lsp_status lsp_adamw_step(lsp_ctx* ctx, int ntensors, const lsp_adamw_tensor* te
     long long blocks = (t.start[t.n] + OPT_THREADS - 1) / OPT_THREADS;
     return static_cast<int>(blocks > cap ? cap : blocks);
   };
+  const int phase = desc->phase;
+  if (phase < 0 || phase > 2) return fail(ctx, LSP_EINVAL, "lsp_adamw_step: phase must be 0, 1 or 2");
   auto launch = [&]() {
     OptTensors t;
-    int nparts = 0;
-    for (int gi = 0; gi < ngroups; ++gi) {
-      const int nb = group(gi, t);
-      opt_gradsq_kernel<<<nb, OPT_THREADS, 0, st>>>(t, ctx->opt_partial + nparts);
-      nparts += nb;
+    if (phase != 2) {                       // squared norm of the call's gradients
+      int nparts = 0;
+      for (int gi = 0; gi < ngroups; ++gi) {
+        const int nb = group(gi, t);
+        opt_gradsq_kernel<<<nb, OPT_THREADS, 0, st>>>(t, ctx->opt_partial + nparts);
+        nparts += nb;
+      }
+      opt_norm_final_kernel<<<1, OPT_THREADS, 0, st>>>(ctx->opt_partial, nparts, desc->clip_norm, 1.0 / desc->grad_scale, phase == 1, gnorm_out);
+    } else {                                // gnorm_out[0] holds the GLOBAL sum of g^2 (all ranks): norm and coefficient from it
+      opt_norm_final_kernel<<<1, OPT_THREADS, 0, st>>>(gnorm_out, 1, desc->clip_norm, 1.0 / desc->grad_scale, 0, gnorm_out);
     }
-    opt_norm_final_kernel<<<1, OPT_THREADS, 0, st>>>(ctx->opt_partial, nparts, desc->clip_norm, 1.0 / desc->grad_scale, gnorm_out);
-    for (int gi = 0; gi < ngroups; ++gi) {
-      const int nb = group(gi, t);
-      opt_adamw_kernel<<<nb, OPT_THREADS, 0, st>>>(t, h, gnorm_out);
+    if (phase != 1) {
+      for (int gi = 0; gi < ngroups; ++gi) {
+        const int nb = group(gi, t);
+        opt_adamw_kernel<<<nb, OPT_THREADS, 0, st>>>(t, h, gnorm_out);
+      }
     }
     return cudaGetLastError();
   };
-  LSP_STAGE(ST_ADAMW, 2 * ngroups + 1, launch());
+  LSP_STAGE(ST_ADAMW, (phase == 0 ? 2 : 1) * ngroups + 1, launch());
   return LSP_OK;
 }
 

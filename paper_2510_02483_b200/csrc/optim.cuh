@@ -57,11 +57,12 @@ __global__ void __launch_bounds__(OPT_THREADS) opt_gradsq_kernel(const OptTensor
   }
 }
 
+// raw_sum: out[0] = sum of the partials (nothing else).  Otherwise:
 // out[0] = global l2 norm of the true gradients g / grad_scale, out[1] = the factor the update applies to the stored
 // gradients = min(1, clip / (norm + 1e-6)) / grad_scale; one block, fp64, fixed order: thread i sums the
 // partials i, i + 256, ... in that order, then thread 0 adds the 256 thread sums in index order
 __global__ void __launch_bounds__(OPT_THREADS) opt_norm_final_kernel(const float* __restrict__ partial, int nparts, float clip,
-                                                                     double inv_scale, float* __restrict__ out) {
+                                                                     double inv_scale, int raw_sum, float* __restrict__ out) {
   __shared__ double red[OPT_THREADS];
   double s = 0.0;
   for (int i = threadIdx.x; i < nparts; i += OPT_THREADS) s += static_cast<double>(partial[i]);
@@ -70,6 +71,7 @@ __global__ void __launch_bounds__(OPT_THREADS) opt_norm_final_kernel(const float
   if (threadIdx.x == 0) {
     double tot = 0.0;
     for (int i = 0; i < OPT_THREADS; ++i) tot += red[i];
+    if (raw_sum) { out[0] = static_cast<float>(tot); return; }      // phase 1 of a sharded step: this rank's sum of g^2
     const double norm = sqrt(tot) * inv_scale;
     out[0] = static_cast<float>(norm);
     const double c = static_cast<double>(clip) / (norm + 1e-6);

@@ -29,21 +29,27 @@ def global_grad_scale(tokens_local: int, world: int) -> float:
     return float(tokens_local) * float(world)
 
 
+def bucket_layout(shapes: dict):
+    """Offsets (in elements) of the tensors of a bucket inside its flat buffer, each on a 64-element boundary, and the
+    flat length (a multiple of 64, so it divides by 4 * world for world <= 16)."""
+    offs, n = {}, 0
+    for k, s in shapes.items():
+        offs[k] = n
+        n += (torch.Size(s).numel() + 63) // 64 * 64
+    return offs, n
+
+
 class GradBuckets:
-    def __init__(self, buckets, device, group=None):
-        """buckets: list of dicts name -> shape.  Allocates one flat fp32 buffer per bucket; `views[i][name]` are the
-        gradient tensors the backward writes into (each starts on a 256-byte boundary: TMA stores, float4 loads)."""
+    def __init__(self, buckets, device, group=None, dtype=torch.float32):
+        """buckets: list of dicts name -> shape.  Allocates one flat buffer per bucket (fp32 for gradients; the same
+        class lays out the bf16 weights for the sharded optimizer); `views[i][name]` are the tensors the kernels read or
+        write (each starts on a 256-byte boundary for fp32: TMA stores, float4 loads)."""
         self.group = group
+        self.shapes = list(buckets)
         self.flat, self.views, self._pending = [], [], []
         for shapes in buckets:
-            offs, n = {}, 0
-            for k, s in shapes.items():
-                offs[k] = n
-                cnt = 1
-                for d in s:
-                    cnt *= d
-                n += (cnt + 63) // 64 * 64
-            flat = torch.zeros(n, dtype=torch.float32, device=device)
+            offs, n = bucket_layout(shapes)
+            flat = torch.zeros(n, dtype=dtype, device=device)
             self.flat.append(flat)
             self.views.append({k: flat[offs[k]:offs[k] + torch.Size(s).numel()].view(s) for k, s in shapes.items()})
 
@@ -66,3 +72,83 @@ def mean_loss(loss: torch.Tensor, group=None) -> torch.Tensor:
         dist.all_reduce(loss, op=dist.ReduceOp.SUM, group=group)
         loss /= dist.get_world_size(group)
     return loss
+
+
+class Zero1State:
+    """ZeRO stage 1: the model is replicated, the optimizer state is not.  Rank r owns the r-th 1/world of
+    every gradient bucket: the bucket's gradient is reduce-scattered instead of all-reduced, the rank keeps fp32 master
+    weights and moments for its slice only (12 bytes per parameter / world instead of 12), updates the slice, and the
+    bf16 weights are all-gathered back into every replica's flat weight bucket.  The global gradient norm needs one
+    scalar all-reduce between the two phases of the optimizer call (lsp_adamw_step phase 1 / 2).
+
+    Device-agnostic: `step(phase_fn, ...)` takes the function that runs a phase on a list of tensor dicts -- the library
+    call on the GPU, the fp64 oracle in the CPU tests."""
+
+    def __init__(self, grads: GradBuckets, weights: GradBuckets, decay: list, world: int, rank: int, group=None):
+        """grads / weights: buckets of identical layout (fp32 / bf16); decay: per bucket, dict name -> bool."""
+        self.grads, self.weights, self.world, self.rank, self.group = grads, weights, world, rank, group
+        self.lo, self.g_shard, self.master, self.m, self.v, self.segments = [], [], [], [], [], []
+        self._pending = []
+        for b, shapes in enumerate(grads.shapes):
+            offs, n = bucket_layout(shapes)
+            per = n // world
+            lo, hi = rank * per, (rank + 1) * per
+            self.lo.append(lo)
+            flat_g = grads.flat[b]
+            self.g_shard.append(flat_g[lo:hi] if world == 1 else torch.zeros(per, dtype=flat_g.dtype, device=flat_g.device))
+            self.master.append(weights.flat[b][lo:hi].float())
+            self.m.append(torch.zeros(per, dtype=torch.float32, device=flat_g.device))
+            self.v.append(torch.zeros(per, dtype=torch.float32, device=flat_g.device))
+            segs = []
+            for k, s in shapes.items():
+                a, e = max(offs[k], lo), min(offs[k] + torch.Size(s).numel(), hi)
+                if a < e:
+                    segs.append((k, a, e, bool(decay[b][k])))
+            self.segments.append(segs)
+
+    def _native(self) -> bool:
+        return dist.get_backend(self.group) != "gloo"       # gloo (CPU tests) has no reduce-scatter: emulate with all-reduce
+
+    def reduce_scatter_async(self, b: int):
+        if self.world > 1:
+            if self._native():
+                self._pending.append(dist.reduce_scatter_tensor(self.g_shard[b], self.grads.flat[b], op=dist.ReduceOp.SUM,
+                                                                group=self.group, async_op=True))
+            else:
+                dist.all_reduce(self.grads.flat[b], op=dist.ReduceOp.SUM, group=self.group)
+                per = self.g_shard[b].numel()
+                self.g_shard[b].copy_(self.grads.flat[b][self.lo[b]:self.lo[b] + per])
+
+    def tensors(self):
+        """The tensor dicts of lsp_adamw_step for this rank's slices (a parameter cut by a slice boundary appears as the
+        part this rank owns)."""
+        out = []
+        for b, segs in enumerate(self.segments):
+            lo = self.lo[b]
+            for _, a, e, dec in segs:
+                out.append(dict(grad=self.g_shard[b][a - lo:e - lo], master=self.master[b][a - lo:e - lo], m=self.m[b][a - lo:e - lo],
+                                v=self.v[b][a - lo:e - lo], weight=self.weights.flat[b][a:e], decay=dec))
+        return out
+
+    def step(self, phase_fn, sumsq: torch.Tensor):
+        """phase_fn(tensors, phase, sumsq): phase 1 leaves this rank's sum of g^2 in sumsq[0]; phase 2 finds the global sum
+        there and updates master / m / v / weight of the slices.  Then every replica gets all updated bf16 weights."""
+        for h in self._pending:
+            h.wait()
+        self._pending = []
+        t = self.tensors()
+        phase_fn(t, 1, sumsq)
+        if self.world > 1:
+            dist.all_reduce(sumsq[0:1], op=dist.ReduceOp.SUM, group=self.group)
+        phase_fn(t, 2, sumsq)
+        if self.world > 1:
+            for b in range(len(self.segments)):
+                per = self.g_shard[b].numel()
+                lo = self.lo[b]
+                mine = self.weights.flat[b][lo:lo + per].clone()
+                if self._native():
+                    dist.all_gather_into_tensor(self.weights.flat[b], mine, group=self.group)
+                else:
+                    parts = [torch.empty_like(mine) for _ in range(self.world)]
+                    dist.all_gather(parts, mine, group=self.group)
+                    self.weights.flat[b].copy_(torch.cat(parts))

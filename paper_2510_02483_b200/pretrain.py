@@ -22,14 +22,16 @@ from . import dp, harness, replicas, synth
 
 class PretrainStep:
     def __init__(self, w: synth.Workload, n_layers: int, vocab: int, dev=None, weights=None, embedding=None, head=None, g_final=None,
-                 world: int = 1, group=None, micro_batches: int = 1, recompute: bool = False):
+                 world: int = 1, group=None, micro_batches: int = 1, recompute: bool = False,
+                 zero1: bool = False, rank: int = 0):
         """weights: optional list of per-layer dicts of bf16 bit patterns (synth.layer_weights layout); embedding / head:
         bf16 bit patterns [vocab, H]; g_final: bf16 bits [H].  Defaults: the seeded synthetic tensors of synth.py.
         `w` is one MICRO-batch of this rank's shard; micro_batches > 1: gradient accumulation (the paper's global batch of
         256 sequences, Table 2, does not fit one step) -- the first micro-batch overwrites the gradient buffers,
         the others run on a second context created with wgrad_accumulate = 1; world > 1: data-parallel replicas (dp.py);
         recompute: keep only every layer's INPUT from the forward pass and re-run the layer's forward in front of its
-        backward (one shared `saved` buffer instead of n_layers: activation memory / n_layers for one more forward)."""
+        backward (one shared `saved` buffer instead of n_layers: activation memory / n_layers for one more forward);
+        zero1: optimizer state sharded over the `world` replicas (dp.Zero1State), `rank` = this replica."""
         self.dev = dev or harness.require_cuda()
         self.w, self.L, self.V = w, n_layers, vocab
         self.ctx = harness.make_ctx(w, in_dtype=B.LSP_F32)
@@ -54,29 +56,33 @@ class PretrainStep:
         self.layer_w, self.layer_g = [], []
         # gradient buckets (one flat buffer = one all-reduce each): the layers, then {head, final gain}, then the table
         lshapes = harness.WEIGHT_SHAPES(w)
-        self.buckets = dp.GradBuckets([lshapes] * n_layers + [dict(head=(vocab, H), g_final=(H,)), dict(table=(vocab, H))],
-                                      self.dev, group)
+        bshapes = [lshapes] * n_layers + [dict(head=(vocab, H), g_final=(H,)), dict(table=(vocab, H))]
+        self.buckets = dp.GradBuckets(bshapes, self.dev, group)
+        self.wbuckets = dp.GradBuckets(bshapes, self.dev, group, dtype=torch.bfloat16)     # the bf16 weights, same layout
         self.world = world
         for l in range(n_layers):
             bits = weights[l] if weights is not None else synth.layer_weights(w, l)
-            wt = harness.upload_weights(bits, self.dev)
-            gr = self.buckets.views[l]
-            self.layer_w.append(wt)
-            self.layer_g.append(gr)
-            for k in synth.WEIGHT_NAMES:
-                self._register(wt[k], gr[k], decay=wt[k].dim() == 2)
+            for k, t in harness.upload_weights(bits, self.dev).items():
+                self.wbuckets.views[l][k].copy_(t)
+            self.layer_w.append(self.wbuckets.views[l])
+            self.layer_g.append(self.buckets.views[l])
         st = None
         if embedding is None or head is None:
             st = synth.stack_inputs(w.with_(vocab=vocab))
-        self.table = harness.bf16_to_device(embedding if embedding is not None else st["embedding"], self.dev)
-        self.w_head = harness.bf16_to_device(head if head is not None else synth.normal_bf16(w.cfg_id, 0, "w_head", (vocab, H), 0.02), self.dev)
-        self.g_final = (harness.bf16_to_device(g_final, self.dev) if g_final is not None
-                        else torch.ones(H, dtype=torch.bfloat16, device=self.dev))
+        self.table, self.w_head = self.wbuckets.views[n_layers + 1]["table"], self.wbuckets.views[n_layers]["head"]
+        self.g_final = self.wbuckets.views[n_layers]["g_final"]
+        self.table.copy_(harness.bf16_to_device(embedding if embedding is not None else st["embedding"], self.dev))
+        self.w_head.copy_(harness.bf16_to_device(head if head is not None else synth.normal_bf16(w.cfg_id, 0, "w_head", (vocab, H), 0.02), self.dev))
+        self.g_final.copy_(harness.bf16_to_device(g_final, self.dev) if g_final is not None
+                           else torch.ones(H, dtype=torch.bfloat16, device=self.dev))
         self.d_head, self.d_gfinal = self.buckets.views[n_layers]["head"], self.buckets.views[n_layers]["g_final"]
         self.d_table = self.buckets.views[n_layers + 1]["table"]
-        self._register(self.table, self.d_table, decay=True)
-        self._register(self.w_head, self.d_head, decay=True)
-        self._register(self.g_final, self.d_gfinal, decay=False)
+        decay = [{k: len(s) == 2 for k, s in b.items()} for b in bshapes]
+        self.zero = dp.Zero1State(self.buckets, self.wbuckets, decay, world, rank, group) if zero1 else None
+        if not zero1:
+            for b, shapes in enumerate(bshapes):
+                for k in (synth.WEIGHT_NAMES if b < n_layers else shapes):
+                    self._register(self.wbuckets.views[b][k], self.buckets.views[b][k], decay=decay[b][k])
         self.t = 0
         # gradients are carried scaled by T (the gradient of the SUM loss): the mean's 1/T would push the layers' 16-bit
         # backward operands under the fp16 normal range; lsp_adamw_step divides it out (exact for a power-of-two T),
@@ -90,7 +96,7 @@ class PretrainStep:
 
     @property
     def n_params(self):
-        return sum(p["master"].numel() for p in self.params)
+        return sum(torch.Size(s).numel() for b in self.buckets.shapes for s in b.values())
 
     def forward_backward(self, ids: torch.Tensor, targets: torch.Tensor, stream=None, micro: int = 0):
         """ids, targets: int32 [T] on the device (micro-batch `micro` of n_micro).  Leaves the loss of the micro-batch in
@@ -106,24 +112,36 @@ class PretrainStep:
         B.lsp_head_fwd_bwd(c, self.xs[L], self.g_final, self.w_head, targets, self.V, self.loss, self.lse, d_in, self.d_gfinal,
                            self.d_head, self.ws, stream, grad_scale=self.head_scale)
         if last:
-            self.buckets.reduce_async(L)
+            self._reduce(L)
         for l in range(L - 1, -1, -1):
             d_out = self.d[l & 1]
             if self.recompute and l != L - 1:           # the shared buffer still holds the last layer's activations
                 B.lsp_layer_fwd(c, self.xs[l], self.layer_w[l], self.xs[l + 1], self.saved[l], self.ws, stream)
             B.lsp_layer_bwd(c, self.xs[l], d_in, self.layer_w[l], self.saved[l], d_out, self.layer_g[l], self.ws, stream)
             if last:
-                self.buckets.reduce_async(l)        # overlaps the next layer's backward
+                self._reduce(l)                     # overlaps the next layer's backward
             d_in = d_out
         B.lsp_embed_bwd(c, ids, d_in, self.V, self.d_table, stream)
         if last:
-            self.buckets.reduce_async(L + 1)
+            self._reduce(L + 1)
         return self.loss
+
+    def _reduce(self, b: int):
+        """Exchange step of bucket b: all-reduce of the gradients, or reduce-scatter to their owners under ZeRO-1."""
+        if self.zero is not None:
+            self.zero.reduce_scatter_async(b)
+        else:
+            self.buckets.reduce_async(b)
 
     def optimizer_step(self, lr=None, stream=None, **hyper):
         self.t += 1
+        lr = B.lsp_lr_cosine(self.t) if lr is None else lr
+        if self.zero is not None:
+            self.zero.step(lambda t, phase, gn: B.lsp_adamw_step(self.ctx, t, lr=lr, step=self.t, gnorm_out=gn, phase=phase,
+                                                                 grad_scale=self.grad_scale, stream=stream, **hyper), self.gnorm)
+            return
         self.buckets.wait()
-        B.lsp_adamw_step(self.ctx, self.params, lr=B.lsp_lr_cosine(self.t) if lr is None else lr, step=self.t, gnorm_out=self.gnorm,
+        B.lsp_adamw_step(self.ctx, self.params, lr=lr, step=self.t, gnorm_out=self.gnorm,
                          grad_scale=self.grad_scale, stream=stream, **hyper)
 
     def step(self, ids, targets, lr=None, stream=None, **hyper):
@@ -147,6 +165,7 @@ def main(argv=None):
     ap.add_argument("--layers", type=int, default=synth.CFG3_3B_STACK.n_layers)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=2)
+    ap.add_argument("--zero1", action="store_true", help="optimizer state sharded over the data-parallel replicas (ZeRO stage 1)")
     ap.add_argument("--recompute", action="store_true", help="keep layer inputs only; re-run each layer's forward before its backward")
     args = ap.parse_args(argv)
     w = synth.CFG3_3B_STACK
@@ -156,7 +175,7 @@ def main(argv=None):
         torch.cuda.set_device(renv.local_rank)
     dev = harness.require_cuda()
     replicas.init("nccl", renv)
-    run = PretrainStep(w, args.layers, w.vocab, dev, world=renv.world_size, recompute=args.recompute)
+    run = PretrainStep(w, args.layers, w.vocab, dev, world=renv.world_size, recompute=args.recompute, zero1=args.zero1, rank=renv.rank)
     s = synth.stack_inputs(w)
     ids = torch.from_numpy(s["ids"]).to(dev)
     ids = torch.roll(ids, 997 * renv.rank)
@@ -180,7 +199,7 @@ def main(argv=None):
     # the paper's accounting: 6 FLOPs per parameter per token without the embedding table, plus attention
     flops = renv.world_size * (6.0 * (n - w.vocab * w.hidden) * w.tokens + args.layers * 3.5 * synth.attn_flops_fwd(w, causal=True))
     if renv.is_main:
-        print(json.dumps({"config": f"pretrain_{w.name}_L{args.layers}" + ("_recompute" if args.recompute else ""), "n_gpus": renv.world_size, "params": n, "tokens": int(tokens),
+        print(json.dumps({"config": f"pretrain_{w.name}_L{args.layers}" + ("_recompute" if args.recompute else "") + ("_zero1" if args.zero1 else ""), "n_gpus": renv.world_size, "params": n, "tokens": int(tokens),
                           "ms_fwd_bwd": round(ms_fb, 3), "ms_adamw": round(ms_opt, 3), "ms_iteration": round(ms_it, 3),
                           "tokens_per_s": round(tok_s, 1), "model_tflops": round(flops / (ms_it * 1e-3) / 1e12, 1),
                           "adamw_GB_per_s": round(34.0 * n / (ms_opt * 1e-3) / 1e9, 1),

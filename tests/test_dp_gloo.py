@@ -107,3 +107,90 @@ def test_two_gloo_ranks_sum_to_full_batch_gradient():
         assert o["aligned"]
         assert o["worst"] < 1e-6                                   # fp32 buffers: one rounding per addend
         assert o["loss"] == pytest.approx(o["full_loss"], rel=1e-12)
+
+
+ZERO_WORKER = r"""
+import json, os, sys
+sys.path.insert(0, os.environ["LSP_ROOT"])
+import numpy as np, torch, torch.distributed as dist
+from oracle import adamw_ref as A
+from paper_2510_02483_b200 import dp
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+dist.init_process_group("gloo", rank=rank, world_size=world)
+shapes = [dict(wa=(24, 40), ga=(40,), wb=(40, 24)), dict(head=(50, 40), g_final=(40,)), dict(table=(50, 40))]
+decay = [{k: len(s) == 2 for k, s in b.items()} for b in shapes]
+rng = np.random.default_rng(11)                       # same initial weights everywhere
+grads, weights = dp.GradBuckets(shapes, "cpu"), dp.GradBuckets(shapes, "cpu", dtype=torch.bfloat16)
+for b in weights.views:
+    for k, v in b.items():
+        v.copy_(torch.from_numpy(0.05 * rng.standard_normal(tuple(v.shape))).to(torch.bfloat16))
+w0 = [{k: v.float().numpy().astype(np.float64).copy() for k, v in b.items()} for b in weights.views]
+T_local, scale = 16, dp.global_grad_scale(16, world)
+def local_grads(r):                                   # what rank r's backward leaves in its buckets (scaled by T_local)
+    g = np.random.default_rng(100 + r)
+    return [{k: (3.0 * g.standard_normal(s) * T_local).astype(np.float32) for k, s in b.items()} for b in shapes]
+mine = local_grads(rank)
+for b, gb in enumerate(mine):
+    for k, v in gb.items():
+        grads.views[b][k].copy_(torch.from_numpy(v))
+zero = dp.Zero1State(grads, weights, decay, world, rank)
+lr, step = 1.0e-3, 1
+
+def phase_fn(tensors, phase, sumsq):                  # the fp64 oracle in place of lsp_adamw_step
+    if phase == 1:
+        sumsq[0] = float(sum(float(np.sum(t["grad"].numpy().astype(np.float64) ** 2)) for t in tensors))
+        return
+    norm = float(np.sqrt(float(sumsq[0]))) / scale
+    c = A.clip_coefficient(norm)
+    for t in tensors:
+        p, m, v, _ = A.adamw_step([t["master"].numpy()], [t["grad"].numpy().astype(np.float64) * (c / scale)], [t["m"].numpy()],
+                                  [t["v"].numpy()], [t["decay"]], step, lr, clip=1e30)
+        t["master"].copy_(torch.from_numpy(p[0])); t["m"].copy_(torch.from_numpy(m[0])); t["v"].copy_(torch.from_numpy(v[0]))
+        t["weight"].copy_(torch.from_numpy(A.bf16_rne(t["master"].numpy())).to(torch.bfloat16))
+    sumsq[0] = norm
+
+for b in range(len(shapes)):
+    zero.reduce_scatter_async(b)
+sumsq = torch.zeros(2, dtype=torch.float32)
+zero.step(phase_fn, sumsq)
+# reference: one process, the summed gradients of both ranks, the whole model
+tot = [{k: sum(local_grads(r)[b][k].astype(np.float64) for r in range(world)) / scale for k in shapes[b]} for b in range(len(shapes))]
+names = [(b, k) for b in range(len(shapes)) for k in shapes[b]]
+p_ref, _, _, norm_ref = A.adamw_step([w0[b][k] for b, k in names], [tot[b][k] for b, k in names], [np.zeros(shapes[b][k]) for b, k in names],
+                                     [np.zeros(shapes[b][k]) for b, k in names], [decay[b][k] for b, k in names], step, lr)
+worst, flips, n = 0.0, 0, 0
+for (b, k), pr in zip(names, p_ref):
+    got = weights.views[b][k].float().numpy().astype(np.float64)
+    ref = A.bf16_rne(pr)
+    flips += int(np.sum(got != ref)); n += got.size
+    worst = max(worst, float(np.max(np.abs(got - pr) / (np.abs(pr) * 2.0 ** -8 + 1e-12))))
+owned = sum(e - a for segs in zero.segments for _, a, e, _ in segs)
+print(json.dumps(dict(rank=rank, norm=float(sumsq[0]), norm_ref=norm_ref, flips=flips, n=n, worst=worst, owned=owned)), flush=True)
+dist.destroy_process_group()
+"""
+
+
+@pytest.mark.timeout(300)
+def test_zero1_two_gloo_ranks_match_full_adamw():
+    """dp.Zero1State over two gloo ranks with the fp64 oracle as the update function: reduce-scatter of the gradient
+    buckets, sum of g^2 all-reduced between the two optimizer phases, slices updated by their owners, bf16 weights
+    all-gathered -- every replica ends with the weights one process gets from AdamW on the summed gradients."""
+    port = free_port()
+    procs = []
+    for r in range(2):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port), LSP_ROOT=ROOT)
+        procs.append(subprocess.Popen([sys.executable, "-c", ZERO_WORKER], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.PIPE, text=True))
+    outs = []
+    for p in procs:
+        o, e = p.communicate(timeout=280)
+        assert p.returncode == 0, e
+        outs.append(json.loads(o.strip().splitlines()[-1]))
+    total = sum(int(np.prod(s)) for b in [dict(wa=(24, 40), ga=(40,), wb=(40, 24)), dict(head=(50, 40), g_final=(40,)), dict(table=(50, 40))]
+                for s in b.values())
+    assert sum(o["owned"] for o in outs) == total                  # every parameter has exactly one owner
+    for o in outs:
+        assert o["norm"] == pytest.approx(o["norm_ref"], rel=1e-6)
+        assert o["worst"] <= 1.01                                   # within half a bf16 ulp (+ fp32 master rounding) of the fp64 result
+        assert o["flips"] <= 2e-3 * o["n"]                          # bf16 rounding of an fp32 vs an fp64 master weight

@@ -739,15 +739,15 @@ def test_pretrain_iterations_vs_oracle(gpu):
         m0 = [p["m"].cpu().numpy().astype(np.float64) for p in run.params]
         v0 = [p["v"].cpu().numpy().astype(np.float64) for p in run.params]
         layers = [dict(zip(names, host[9 * l:9 * l + 9])) for l in range(L)]
-        E, Wh, gf = host[9 * L], host[9 * L + 1], host[9 * L + 2]
+        Wh, gf, E = host[9 * L], host[9 * L + 1], host[9 * L + 2]          # parameter order: layers, head, final gain, table
         run.step(tid, tt, lr=lr)
         torch.cuda.synchronize()
         loss_ref, lg, dE, dWh, dgf = _oracle_model_grads(ids, targets, layers, E, Wh, gf, shape, V)
         loss = float(run.loss.cpu()); losses.append(loss)
         assert abs(loss - loss_ref) <= 1e-3 * abs(loss_ref), (it, loss, loss_ref)
-        ref_g = [lg[l][k] for l in range(L) for k in names] + [dE, dWh, dgf]
+        ref_g = [lg[l][k] for l in range(L) for k in names] + [dWh, dgf, dE]
         got_g = [p["grad"].cpu().numpy().astype(np.float64) / run.grad_scale for p in run.params]
-        tags = [f"L{l}.d{k}" for l in range(L) for k in names] + ["d_table", "d_head", "d_gfinal"]
+        tags = [f"L{l}.d{k}" for l in range(L) for k in names] + ["d_head", "d_gfinal", "d_table"]
         check(dict(zip(tags, got_g)), dict(zip(tags, ref_g)), tags)
         norm_ref = A.global_grad_norm(ref_g)
         got_n, got_c = [float(x) for x in run.gnorm.cpu().numpy()]
@@ -787,14 +787,14 @@ def test_pretrain_micro_batches_vs_oracle(gpu):
              [torch.from_numpy(targets[i * T:(i + 1) * T].copy()).cuda() for i in range(n_micro)], lr=1e-3)
     torch.cuda.synchronize()
     layers = [dict(zip(names, host[9 * l:9 * l + 9])) for l in range(L)]
-    loss_ref, lg, dE, dWh, dgf = _oracle_model_grads(ids, targets, layers, host[9 * L], host[9 * L + 1], host[9 * L + 2],
+    loss_ref, lg, dE, dWh, dgf = _oracle_model_grads(ids, targets, layers, host[9 * L + 2], host[9 * L], host[9 * L + 1],
                                                      oracle_shape(w_all), V)
     loss = float(run.micro_losses.mean().cpu())
     assert abs(loss - loss_ref) <= 1e-3 * abs(loss_ref), (loss, loss_ref)
     assert run.grad_scale == float(T * n_micro)
-    ref_g = [lg[l][k] for l in range(L) for k in names] + [dE, dWh, dgf]
+    ref_g = [lg[l][k] for l in range(L) for k in names] + [dWh, dgf, dE]
     got_g = [p["grad"].cpu().numpy().astype(np.float64) / run.grad_scale for p in run.params]
-    tags = [f"L{l}.d{k}" for l in range(L) for k in names] + ["d_table", "d_head", "d_gfinal"]
+    tags = [f"L{l}.d{k}" for l in range(L) for k in names] + ["d_head", "d_gfinal", "d_table"]
     check(dict(zip(tags, got_g)), dict(zip(tags, ref_g)), tags)
     norm_ref = A.global_grad_norm(ref_g)
     assert abs(float(run.gnorm[0].cpu()) - norm_ref) <= 5e-3 * norm_ref
@@ -864,3 +864,37 @@ def test_layer_step_replays_from_a_cuda_graph(gpu, w):
     print(f"{w.name}: eager {timed(step):.4f} ms/step, graph replay {timed(graph.replay):.4f} ms/step")
     del graph
     ctx.close()
+
+
+def test_pretrain_zero1_matches_replicated_optimizer(gpu):
+    """PretrainStep(zero1=True) on one rank (its slice is everything; the two-phase lsp_adamw_step with the sum of g^2
+    handed over in between) against the plain path over three iterations: same losses (1e-6), the same bf16 weights in
+    every tensor up to isolated last-bit flips (the norm passes through one extra fp32 rounding), and a slice plan for
+    world = 2 that covers every parameter exactly once with 4-aligned cuts."""
+    import torch
+    from paper_2510_02483_b200 import dp, pretrain
+    w = synth.Workload("pretrain_z1", 12, 2, 192, 256, 4, 2, 128, 688, 1e-5, 500000.0, 2, 1000)
+    ids = synth.stack_inputs(w)["ids"]
+    tid = torch.from_numpy(ids).cuda(); tt = torch.from_numpy(np.roll(ids, -1)).cuda()
+    runs = [pretrain.PretrainStep(w, w.n_layers, w.vocab, zero1=z) for z in (False, True)]
+    for it in range(3):
+        losses = [float(r.step(tid, tt, lr=1e-3).cpu()) for r in runs]
+        torch.cuda.synchronize()
+        assert abs(losses[0] - losses[1]) <= 1e-6 * abs(losses[0]), (it, losses)
+        n0, n1 = float(runs[0].gnorm[0].cpu()), float(runs[1].gnorm[0].cpu())
+        assert abs(n0 - n1) <= 1e-6 * n0
+        for fa, fb in zip(runs[0].wbuckets.flat, runs[1].wbuckets.flat):
+            a, b = fa.float().cpu().numpy(), fb.float().cpu().numpy()
+            assert np.mean(a != b) < 1e-4 and np.max(np.abs(a - b)) <= 2.0 ** -7 * np.max(np.abs(a))
+    # slice plan of two ranks over the same buckets
+    decay = [{k: len(s) == 2 for k, s in b.items()} for b in runs[0].buckets.shapes]
+    plans = [dp.Zero1State(runs[0].buckets, runs[0].wbuckets, decay, 2, r) for r in range(2)]
+    for b, shapes in enumerate(runs[0].buckets.shapes):
+        covered = {k: 0 for k in shapes}
+        for p in plans:
+            for k, a, e, dec in p.segments[b]:
+                assert a % 4 == 0 and e % 4 == 0 and dec == decay[b][k]
+                covered[k] += e - a
+        assert covered == {k: int(np.prod(s)) for k, s in shapes.items()}
+    for r in runs:
+        r.close()
