@@ -123,6 +123,31 @@ def test_sdpa_vs_torch_library():
         np.testing.assert_allclose(got, t.grad.permute(0, 2, 1, 3).numpy(), atol=1e-12)
 
 
+def test_packed_sequences_equal_block_diagonal_mask():
+    """The reference the packed-sequence GPU tests build (the oracle run on every sequence by itself, results laid end to
+    end) is attention over the packed row under a block-diagonal causal mask: checked against torch's float64
+    scaled_dot_product_attention with that mask, forward and backward."""
+    cu = [0, 5, 6, 19, 33]
+    S, nq, nkv, d = cu[-1], 4, 2, 8
+    q = rng.normal(size=(1, S, nq, d)); k = rng.normal(size=(1, S, nkv, d)); v = rng.normal(size=(1, S, nkv, d))
+    dO = rng.normal(size=(1, S, nq, d))
+    start = np.zeros(S, dtype=np.int64)
+    for a, b in zip(cu, cu[1:]):
+        start[a:b] = a
+    idx = np.arange(S)
+    mask = torch.tensor((idx[None, :] <= idx[:, None]) & (idx[None, :] >= start[:, None]))      # [query, key]
+    tq, tk, tv = (torch.tensor(t).permute(0, 2, 1, 3).requires_grad_(True) for t in (q, k, v))
+    to = F.scaled_dot_product_attention(tq, tk, tv, attn_mask=mask, enable_gqa=True)
+    to.backward(torch.tensor(dO).permute(0, 2, 1, 3))
+    O = np.zeros_like(q); dq = np.zeros_like(q); dk = np.zeros_like(k); dv = np.zeros_like(v)
+    for a, b in zip(cu, cu[1:]):
+        O[:, a:b], _ = R.sdpa_fwd(q[:, a:b], k[:, a:b], v[:, a:b])
+        dq[:, a:b], dk[:, a:b], dv[:, a:b] = R.sdpa_bwd(q[:, a:b], k[:, a:b], v[:, a:b], dO[:, a:b])
+    np.testing.assert_allclose(O, to.detach().permute(0, 2, 1, 3).numpy(), atol=1e-12)
+    for got, t in ((dq, tq), (dk, tk), (dv, tv)):
+        np.testing.assert_allclose(got, t.grad.permute(0, 2, 1, 3).numpy(), atol=1e-12)
+
+
 def test_gqa_reduces_to_mha_and_group_sum():
     B, S, nq, nkv, d = 1, 10, 6, 2, 4
     G = nq // nkv
@@ -194,6 +219,21 @@ def test_rope_closed_form_and_frequencies():
     r = R.rope_apply(z, th, 0)
     np.testing.assert_allclose(r[0, :, 0, 0], np.cos(np.arange(5)), atol=1e-15)
     np.testing.assert_allclose(r[0, :, 0, 1], np.sin(np.arange(5)), atol=1e-15)   # counter-clockwise by +theta
+
+
+def test_half_split_rope_is_adjacent_rope_on_interleaved_rows():
+    """The identity the library's rope_layout = 1 rests on: with the features of a head
+    interleaved, z'[2i] = z[i], z'[2i + 1] = z[i + d/2], adjacent-pair rotation of z' is the interleaved half-split
+    rotation of z, and q'.k' = q.k because the same permutation acts on both."""
+    S_, h, d = 7, 3, 16
+    z = rng.normal(size=(1, S_, h, d)); k = rng.normal(size=(1, S_, h, d))
+    th = R.rope_angles(S_, d, 10000.0)
+    perm = np.empty(d, dtype=np.int64)
+    perm[0::2] = np.arange(d // 2); perm[1::2] = np.arange(d // 2) + d // 2
+    np.testing.assert_allclose(R.rope_apply(z[..., perm], th, 0), R.rope_apply(z, th, 1)[..., perm], atol=1e-14)
+    a, b = R.rope_apply(z[..., perm], th, 0), R.rope_apply(k[..., perm], th, 0)
+    a1, b1 = R.rope_apply(z, th, 1), R.rope_apply(k, th, 1)
+    np.testing.assert_allclose(np.einsum("bshd,bthd->bhst", a, b), np.einsum("bshd,bthd->bhst", a1, b1), atol=1e-12)
 
 
 def test_rope_relative_position_property():
