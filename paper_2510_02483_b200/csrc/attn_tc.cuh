@@ -46,6 +46,31 @@ constexpr int ATC_FWD_THREADS = 320;
 constexpr int ATC_FWD_SMEM = 6 * ATC_TILE_BYTES + 8 * GEMM_STAGE_TILE_BYTES + 1024 + 256;
 constexpr float ATC_RESCALE_LOG2 = 8.0f;
 
+// Share of the forward's exponentials computed on the FMA pipe instead of the SFU (0 = none, 1 = a quarter, 2 = half):
+// the 128 MUFU.EX2 of a row occupy the SFU for 1024 cycles of its warp, the FMA-pipe version fills issue slots that the
+// warp leaves empty between them (DESIGN.md section 19 item 1).
+#ifndef LSP_ATTN_POLY_EXP
+#define LSP_ATTN_POLY_EXP 0
+#endif
+
+// 2^x for a pair of values <= ~2^8 without the SFU: x clamped at -126 (masked keys are -inf), n = round(x) through the
+// 1.5 * 2^23 addition, 2^f on [-0.5, 0.5] by the degree-4 Taylor polynomial (relative error <= 4.2e-5, below the fp16
+// rounding of P), 2^n by an add into the exponent field.
+__device__ __forceinline__ float2 ex2_poly2(float2 x) {
+  x.x = fmaxf(x.x, -126.0f);
+  x.y = fmaxf(x.y, -126.0f);
+  const float2 t = fadd2(x, make_float2(12582912.0f, 12582912.0f));
+  const float2 n = fadd2(t, make_float2(-12582912.0f, -12582912.0f));
+  const float2 f = ffma2(n, make_float2(-1.0f, -1.0f), x);
+  float2 r = ffma2(f, make_float2(0.00961813f, 0.00961813f), make_float2(0.05550411f, 0.05550411f));
+  r = ffma2(r, f, make_float2(0.24022651f, 0.24022651f));
+  r = ffma2(r, f, make_float2(0.69314718f, 0.69314718f));
+  r = ffma2(r, f, make_float2(1.0f, 1.0f));
+  r.x = __uint_as_float(__float_as_uint(r.x) + (__float_as_uint(t.x) << 23));
+  r.y = __uint_as_float(__float_as_uint(r.y) + (__float_as_uint(t.y) << 23));
+  return r;
+}
+
 // 3-D map over a [B*S, ld] fp16 matrix seen as (column, position, batch); box = 64 columns x box_rows positions.
 inline bool make_map_attn(CUtensorMap* m, const void* base, int ncols, int S, int B, long long ld, int box_rows = 128) {
   PFN_encodeTiled fn = get_encode_fn();
@@ -384,7 +409,12 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
           for (int i = 0; i < 16; ++i) {
             float2 a = ffma2(make_float2(s[2 * q][2 * i], s[2 * q][2 * i + 1]), c2, neg2);
             float2 b2 = ffma2(make_float2(s[2 * q + 1][2 * i], s[2 * q + 1][2 * i + 1]), c2, neg2);
-            a.x = ex2_approx(a.x); a.y = ex2_approx(a.y); b2.x = ex2_approx(b2.x); b2.y = ex2_approx(b2.y);
+            a.x = ex2_approx(a.x); a.y = ex2_approx(a.y);
+            if (LSP_ATTN_POLY_EXP == 2 || (LSP_ATTN_POLY_EXP == 1 && (i & 1))) {
+              b2 = ex2_poly2(b2);
+            } else {
+              b2.x = ex2_approx(b2.x); b2.y = ex2_approx(b2.y);
+            }
             acc0 = fadd2(acc0, a); acc1 = fadd2(acc1, b2);
             pk[i] = pack_f16(a.x, a.y);
             pk[16 + i] = pack_f16(b2.x, b2.y);
