@@ -1,6 +1,6 @@
 """Device-side timing of every BASELINE.json configuration (bench.py covers the headline config 2 only).
 
-    python -m paper_2510_02483_b200.configs_bench [--steps K] [--only cfg2,fwd,packed,cfg3,cfg4,cfg5,table1,table1_30b,adamw,head]
+    python bench_configs.py [--steps K] [--only cfg2,fwd,packed,cfg3,cfg4,cfg5,table1,table1_30b,adamw,head]
 
 Prints one JSON line per configuration: ms per fwd+bwd step (CUDA events on the launching stream, after warm-up),
 tokens/s and executed TFLOP/s (causal attention FLOPs, SURVEY.md 8(d) convention).  Inputs are the seeded synthetic
@@ -14,8 +14,13 @@ import math
 
 import torch
 
-from . import binding as B
-from . import harness, synth
+import os
+import sys
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+
+from paper_2510_02483_b200 import binding as B  # noqa: E402
+from paper_2510_02483_b200 import harness, synth  # noqa: E402
 
 
 def _time(fn, steps, warmup=3):
