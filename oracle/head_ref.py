@@ -10,7 +10,10 @@ standard Llama components; its FLOP accounting includes the LM hea
   H-1  the model ends with an RMSNorm (gain g_final, same eps as the layers, reading A-3) and a bias-free LM head
        W_head [V, H] ([out, in] like every projection, reading A-9; not tied to the embedding);
   H-2  loss = mean over the T tokens of the natural-log cross-entropy of softmax(logits_t) against target id y_t;
-  H-3  the embedding gradient is the scatter-add of the gradient rows: dE[v,:] = sum over {t : id_t = v} of dx0[t,:].
+  H-3  the embedding gradient is the scatter-add of the gradient rows: dE[v,:] = sum over {t : id_t = v} of dx0[t,:];
+  H-4  a target outside [0, V) (e.g. -100: padding, or the last token of each sequence of a packed SFT / DPO batch,
+       PAPER.md:176-186) carries no loss: the mean of H-2 runs over the n COUNTED tokens only (the convention of
+       torch.nn.functional.cross_entropy(ignore_index=...)); with every target counted this is H-2 unchanged.
 Plain numpy float64, one statement per formula; numpy.matmul is the only library primitive.
 """
 from __future__ import annotations
@@ -26,6 +29,8 @@ def head_loss_fwd_bwd(x, g_final, w_head, targets, eps):
     r_t = 1/sqrt(mean_j x_tj^2 + eps);  xn = x r g_final                                   (H-1, A-3)
     z = xn W_head^T;  lse_t = m_t + log sum_v exp(z_tv - m_t), m_t = max_v z_tv;  loss = mean_t (lse_t - z_t,y_t)   (H-2)
     dz_tv = (exp(z_tv - lse_t) - [v = y_t]) / T;  dW_head = dz^T xn;  dxn = dz W_head;  then the RMSNorm backward.
+    H-4: the mean and the 1/T run over the n tokens whose target lies in [0, V); the other rows of dz are zero
+    (n = 0: loss 0, all gradients 0).
     """
     x = np.asarray(x, F64); g_final = np.asarray(g_final, F64); w_head = np.asarray(w_head, F64)
     y = np.asarray(targets, np.int64)
@@ -36,10 +41,14 @@ def head_loss_fwd_bwd(x, g_final, w_head, targets, eps):
     z = np.matmul(xn, w_head.T)
     m = np.max(z, axis=1)
     lse = m + np.log(np.sum(np.exp(z - m[:, None]), axis=1))
-    loss = float(np.mean(lse - z[np.arange(T), y]))
+    counted = (y >= 0) & (y < w_head.shape[0])
+    tc = np.arange(T)[counted]
+    n_counted = int(tc.size)
+    loss = float(np.sum(lse[tc] - z[tc, y[tc]]) / n_counted) if n_counted else 0.0
     dz = np.exp(z - lse[:, None])
-    dz[np.arange(T), y] -= 1.0
-    dz /= T
+    dz[tc, y[tc]] -= 1.0
+    dz[~counted, :] = 0.0
+    dz /= max(n_counted, 1)
     dw_head = np.matmul(dz.T, xn)
     dxn = np.matmul(dz, w_head)
     dn = dxn * g_final[None, :]

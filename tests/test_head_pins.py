@@ -78,6 +78,39 @@ def test_against_torch_float64():
     np.testing.assert_allclose(out["dw_head"], tw.grad.numpy(), rtol=1e-10, atol=1e-15)
 
 
+def test_ignored_targets():
+    """Reading H-4: targets outside [0, V) carry no loss and the mean runs over the counted tokens.  Pins: (i) the result
+    equals the oracle run on the counted rows alone (loss, dg, dW) with zero dx rows where ignored -- a token's loss term
+    touches only its own row of x; (ii) torch float64 cross_entropy(ignore_index=-100) under autograd; (iii) all ignored:
+    zero loss and gradients; (iv) no ignored target: identical to the plain mean of H-2."""
+    import torch
+    import torch.nn.functional as F
+    x, g, w, y = _case(8, T=20, H=24, V=50)
+    yi = y.copy()
+    yi[[0, 3, 4, 11, 19]] = -100
+    yi[7] = 50                                       # >= V: not counted either
+    keep = (yi >= 0) & (yi < 50)
+    out = Hd.head_loss_fwd_bwd(x, g, w, yi, EPS)
+    sub = Hd.head_loss_fwd_bwd(x[keep], g, w, yi[keep], EPS)
+    assert out["loss"] == pytest.approx(sub["loss"], rel=1e-14)
+    np.testing.assert_allclose(out["dx"][keep], sub["dx"], rtol=1e-12, atol=1e-16)
+    assert not np.any(out["dx"][~keep])
+    np.testing.assert_allclose(out["dg_final"], sub["dg_final"], rtol=1e-12, atol=1e-16)
+    np.testing.assert_allclose(out["dw_head"], sub["dw_head"], rtol=1e-12, atol=1e-16)
+    yt = yi.copy(); yt[7] = -100
+    tx = torch.tensor(x, requires_grad=True); tg = torch.tensor(g, requires_grad=True); tw = torch.tensor(w, requires_grad=True)
+    loss = F.cross_entropy(F.linear(F.rms_norm(tx, (x.shape[1],), tg, EPS), tw), torch.tensor(yt), ignore_index=-100)
+    loss.backward()
+    assert out["loss"] == pytest.approx(float(loss.detach()), rel=1e-13)
+    np.testing.assert_allclose(out["dx"], tx.grad.numpy(), rtol=1e-10, atol=1e-15)
+    np.testing.assert_allclose(out["dw_head"], tw.grad.numpy(), rtol=1e-10, atol=1e-15)
+    none = Hd.head_loss_fwd_bwd(x, g, w, np.full_like(y, -1), EPS)
+    assert none["loss"] == 0.0 and not np.any(none["dx"]) and not np.any(none["dw_head"]) and not np.any(none["dg_final"])
+    full = Hd.head_loss_fwd_bwd(x, g, w, y, EPS)
+    z = (x / np.sqrt(np.mean(x * x, axis=1) + EPS)[:, None] * g) @ w.T
+    assert full["loss"] == pytest.approx(float(np.mean(full["lse"] - z[np.arange(20), y])), rel=1e-14)
+
+
 def test_embed_bwd():
     rng = np.random.default_rng(7)
     ids = np.array([3, 1, 3, 0, 1, 3, 6])
