@@ -70,6 +70,12 @@ typedef struct {
 
 typedef struct {
   const void *wq, *wk, *wv, *wo, *g_attn, *w_gate, *w_up, *w_down, *g_mlp;   /* bf16 */
+  const void* f16_cache;    /* NULL, or lsp_weight_cache_bytes(ctx) bytes (256-byte aligned) holding the fp16 tensor-core
+                             * operand copies of THESE seven projection weights, as left by lsp_layer_prepare_weights (or by
+                             * lsp_adamw_step through lsp_adamw_tensor.weight_f16).  NULL: every forward call converts the
+                             * bf16 weights itself (two cast launches, ~0.6 GB of traffic at the 3B shape) into `saved`.
+                             * Non-NULL: forward and backward read the cache and launch no weight cast; the caller must
+                             * refresh it whenever the bf16 weights change -- a stale cache is used as is. */
 } lsp_layer_weights;
 
 typedef struct {
@@ -88,6 +94,26 @@ lsp_status lsp_destroy(lsp_ctx* ctx);
 size_t lsp_saved_bytes(const lsp_ctx* ctx);
 size_t lsp_workspace_bytes(const lsp_ctx* ctx);
 const char* lsp_last_error(const lsp_ctx* ctx);
+
+/* Operand range (reading P-2'; the paper trains in BF16 mixed precision).  The tensor-core
+ * operands of this library are fp16: bf16's rate with three more mantissa bits, which is what holds the 2e-2 parity bar
+ * for the weight gradients, at the price of bf16's exponent range.  Supported magnitudes of every caller tensor that
+ * becomes an operand (weights, dy / da, the attention-core inputs): |v| <= 65504; values below 2^-24 flush to zero.
+ * A value beyond the range is NOT turned into inf: the conversion saturates it to +-65504 (NaN stays NaN) and counts it.
+ * lsp_overflow_count copies the number of values clamped (or found non-finite) since the last reset to *count (HOST),
+ * after synchronising `stream`; reset != 0 zeroes the counter.  A non-zero count means results are outside the parity
+ * contract (rescale the loss / gradient: lsp_head_fwd_bwd's grad_scale).  Internal operands (normalised activations,
+ * q, k, v, h, ...) are O(1)-O(100) for in-range inputs. */
+lsp_status lsp_overflow_count(lsp_ctx* ctx, unsigned long long* count, int reset, void* stream);
+
+/* fp16 operand cache of one layer's projection weights (see lsp_layer_weights.f16_cache): its size, the conversion
+ * call (two launches on `stream`; applies the row permutation of rope_layout = 1), and the byte offset inside the cache
+ * of tensor `which` (0 wq, 1 wk, 2 wv, 3 wo, 4 w_gate, 5 w_up, 6 w_down; same [out,in] row-major layout as the bf16
+ * tensor) for writers that produce the fp16 copy themselves (lsp_adamw_tensor.weight_f16).  The offset is -1 for wq / wk
+ * under rope_layout = 1 (their rows are permuted inside the cache: use lsp_layer_prepare_weights) and for a bad index. */
+size_t lsp_weight_cache_bytes(const lsp_ctx* ctx);
+lsp_status lsp_layer_prepare_weights(lsp_ctx* ctx, const lsp_layer_weights* w, void* cache, void* stream);
+long long lsp_weight_cache_offset(const lsp_ctx* ctx, int which);
 
 /* Attention block:  a = x + Wo . GQA(RoPE(Wq xn), RoPE(Wk xn), Wv xn), xn = RMSNorm(x; g_attn).
  *   x [T,H] in_dtype -> a_out [T,H] fp32. */
@@ -126,7 +152,8 @@ lsp_status lsp_sdpa_fwd(lsp_ctx* ctx, const void* q, const void* k, const void* 
 lsp_status lsp_sdpa_bwd(lsp_ctx* ctx, const void* q, const void* k, const void* v, const void* o, const float* lse,
                         const void* d_o, void* dq, void* dk, void* dv, void* ws, void* stream);
 
-/* Embedding gather (config 3):  x0[t,:] = table[ids[t],:]; ids int32 [T], table bf16 [vocab,H] -> x0 fp32 [T,H]. */
+/* Embedding gather (config 3):  x0[t,:] = table[ids[t],:]; ids int32 [T], table bf16 [vocab,H] -> x0 fp32 [T,H].
+ * Contract: every id is in [0, vocab); ids are used as row indices without a range check (here and in lsp_embed_bwd). */
 lsp_status lsp_embed_fwd(lsp_ctx* ctx, const int32_t* ids, const void* table, void* x0, void* stream);
 
 /* Building block / test hook: one bias-free linear-layer GEMM on the tcgen05 kernel, 16-bit in, fp32 out.
@@ -172,7 +199,9 @@ lsp_status lsp_host_copies_wait(lsp_ctx* ctx, void* stream);
 /* Model head (readings H-1 .. H-3 in DESIGN.md section 13): final RMSNorm (gain g_final, the
  * context's rms_eps), bias-free LM head w_head bf16 [vocab, H] ([out,in]), mean next-token cross-entropy, and all their
  * gradients, in one call:  xn = RMSNorm(x; g_final); z = xn w_head^T; loss = mean_t (lse_t - z[t, targets[t]]).
- *   x [T,H] in_dtype (the stack output), targets int32 [T] in [0, vocab), vocab % 8 == 0.
+ *   x [T,H] in_dtype (the stack output), targets int32 [T], vocab % 8 == 0.  A target outside [0, vocab) (use a negative
+ *   value, e.g. -100: padding, or the last token of each packed sequence) carries no loss (reading H-4): its row adds
+ *   nothing to the loss or to any gradient, and the mean is over the COUNTED targets (loss = 0 when none counts).
  *   Outputs: loss DEVICE float[1]; lse fp32 [T] (natural log-sum-exp of the logits); dx fp32 [T,H]; dg_final fp32 [H];
  *   dw_head fp32 [vocab, H].  ws: lsp_head_workspace_bytes(ctx, vocab) bytes of scratch (256-byte aligned); it holds the
  *   fp32 logits [T, vocab] and their fp16 gradient -- 6 bytes per (token, class).
@@ -196,10 +225,14 @@ lsp_status lsp_embed_bwd(lsp_ctx* ctx, const int32_t* ids, const void* dx0, int3
  * the new master weight; may be NULL), decay = 1 if weight decay applies.  `tensors` is a HOST array of
  * 1 <= ntensors <= 1024 entries (a whole model: the kernels take them in groups of 16, the norm is over all of them).
  * gnorm_out: DEVICE float[2], receives {global norm of the true gradients, factor applied to the stored gradients =
- * clip coefficient / grad_scale} (no host sync).
+ * clip coefficient / grad_scale} (no host sync).  If the norm is not finite (an inf / NaN gradient) the step is SKIPPED:
+ * master, m, v and the weights stay as they are, gnorm_out = {the non-finite norm, 0} is the flag.
+ * weight_f16 (may be NULL): also written, as the fp16 value of the new bf16 weight -- point it into the layer's operand
+ * cache (lsp_weight_cache_offset) and the next forward needs no weight cast.
  * Everything is enqueued on `stream`; results are bit-reproducible. */
 typedef struct {
   const void* grad; float* master; float* m; float* v; void* weight_bf16; int64_t n; int32_t decay;
+  void* weight_f16;
 } lsp_adamw_tensor;
 typedef struct {
   float lr, beta1, beta2, eps, weight_decay, clip_norm;   /* paper: lr from lsp_lr_cosine, 0.90, 0.95, 1e-8, 0.01, 1.0 */

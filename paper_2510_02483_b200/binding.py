@@ -19,7 +19,8 @@ EXPORTS = ("lsp_create", "lsp_destroy", "lsp_saved_bytes", "lsp_workspace_bytes"
            "lsp_attn_fwd", "lsp_attn_bwd", "lsp_mlp_fwd", "lsp_mlp_bwd", "lsp_layer_fwd", "lsp_layer_bwd",
            "lsp_sdpa_fwd", "lsp_sdpa_bwd", "lsp_embed_fwd", "lsp_gemm", "lsp_layer_step_host", "lsp_launch_count",
            "lsp_timing_enable", "lsp_timing_read", "lsp_adamw_step", "lsp_lr_cosine", "lsp_head_workspace_bytes",
-           "lsp_head_fwd_bwd", "lsp_embed_bwd", "lsp_layer_step_host_async", "lsp_host_copies_wait", "lsp_set_packed_sequences", "lsp_layer_fwd_infer")
+           "lsp_head_fwd_bwd", "lsp_embed_bwd", "lsp_layer_step_host_async", "lsp_host_copies_wait", "lsp_set_packed_sequences", "lsp_layer_fwd_infer",
+           "lsp_overflow_count", "lsp_weight_cache_bytes", "lsp_layer_prepare_weights", "lsp_weight_cache_offset")
 
 
 class LspError(RuntimeError):
@@ -35,12 +36,12 @@ class lsp_layer_desc(C.Structure):
 
 
 class lsp_layer_weights(C.Structure):
-    _fields_ = [(n, C.c_void_p) for n in WEIGHT_FIELDS]
+    _fields_ = [(n, C.c_void_p) for n in WEIGHT_FIELDS] + [("f16_cache", C.c_void_p)]
 
 
 class lsp_adamw_tensor(C.Structure):
     _fields_ = [("grad", C.c_void_p), ("master", C.c_void_p), ("m", C.c_void_p), ("v", C.c_void_p),
-                ("weight_bf16", C.c_void_p), ("n", C.c_int64), ("decay", C.c_int32)]
+                ("weight_bf16", C.c_void_p), ("n", C.c_int64), ("decay", C.c_int32), ("weight_f16", C.c_void_p)]
 
 
 class lsp_adamw_desc(C.Structure):
@@ -94,9 +95,15 @@ def lib():
         L.lsp_head_workspace_bytes.restype = C.c_size_t
         L.lsp_head_fwd_bwd.argtypes = [vp, vp, vp, vp, vp, i32, C.c_float, vp, vp, vp, vp, vp, vp, vp]
         L.lsp_embed_bwd.argtypes = [vp, vp, vp, i32, vp, vp]
+        L.lsp_overflow_count.argtypes = [vp, C.POINTER(C.c_ulonglong), i32, vp]
+        L.lsp_weight_cache_bytes.argtypes = [vp]
+        L.lsp_weight_cache_bytes.restype = C.c_size_t
+        L.lsp_layer_prepare_weights.argtypes = [vp, pw, vp, vp]
+        L.lsp_weight_cache_offset.argtypes = [vp, i32]
+        L.lsp_weight_cache_offset.restype = C.c_longlong
         for n in EXPORTS:
             if n not in ("lsp_saved_bytes", "lsp_workspace_bytes", "lsp_last_error", "lsp_launch_count", "lsp_lr_cosine",
-                         "lsp_head_workspace_bytes"):
+                         "lsp_head_workspace_bytes", "lsp_weight_cache_bytes", "lsp_weight_cache_offset"):
                 getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -114,10 +121,14 @@ def _stream(stream):
 
 
 def _pack(struct_t, tensors: dict):
+    """tensors: {field: torch tensor}; weights may carry "f16_cache" (a buffer filled by lsp_layer_prepare_weights)."""
     s = struct_t()
     for n in WEIGHT_FIELDS:
         t = tensors.get(n)
         setattr(s, n, None if t is None else t.data_ptr())
+    if struct_t is lsp_layer_weights:
+        t = tensors.get("f16_cache")
+        s.f16_cache = None if t is None else t.data_ptr()
     return s
 
 
@@ -157,6 +168,10 @@ class Ctx:
     @property
     def workspace_bytes(self):
         return lib().lsp_workspace_bytes(self.handle)
+
+    @property
+    def weight_cache_bytes(self):
+        return lib().lsp_weight_cache_bytes(self.handle)
 
 
 def lsp_attn_fwd(ctx, x, weights, a_out, saved, ws, stream=None):
@@ -238,18 +253,39 @@ def lsp_set_packed_sequences(ctx, cu_seqlens, stream=None):
     ctx.check(lib().lsp_set_packed_sequences(ctx.handle, arr, n, _stream(stream)))
 
 
+def lsp_layer_prepare_weights(ctx, weights, cache, stream=None):
+    w = _pack(lsp_layer_weights, weights)
+    ctx.check(lib().lsp_layer_prepare_weights(ctx.handle, C.byref(w), _ptr(cache), _stream(stream)))
+
+
+def lsp_weight_cache_bytes(ctx) -> int:
+    return int(lib().lsp_weight_cache_bytes(ctx.handle))
+
+
+def lsp_weight_cache_offset(ctx, which: int) -> int:
+    return int(lib().lsp_weight_cache_offset(ctx.handle, which))
+
+
+def lsp_overflow_count(ctx, reset=False, stream=None) -> int:
+    n = C.c_ulonglong(0)
+    ctx.check(lib().lsp_overflow_count(ctx.handle, C.byref(n), 1 if reset else 0, _stream(stream)))
+    return int(n.value)
+
+
 def lsp_host_copies_wait(ctx, stream=None):
     ctx.check(lib().lsp_host_copies_wait(ctx.handle, _stream(stream)))
 
 
 def lsp_adamw_step(ctx, tensors, *, lr, step, gnorm_out, beta1=0.90, beta2=0.95, eps=1e-8, weight_decay=0.01, clip_norm=1.0,
                    grad_scale=1.0, phase=0, stream=None):
-    """tensors: list of dicts {grad, master, m, v, weight (bf16 or None), decay (bool)} of torch CUDA tensors."""
+    """tensors: list of dicts {grad, master, m, v, weight (bf16 or None), decay (bool), weight_f16 (fp16 view or None)} of
+    torch CUDA tensors."""
     arr = (lsp_adamw_tensor * len(tensors))()
     for i, t in enumerate(tensors):
-        w = t.get("weight")
+        w, w16 = t.get("weight"), t.get("weight_f16")
         arr[i] = lsp_adamw_tensor(t["grad"].data_ptr(), t["master"].data_ptr(), t["m"].data_ptr(), t["v"].data_ptr(),
-                                  None if w is None else w.data_ptr(), t["master"].numel(), 1 if t.get("decay", True) else 0)
+                                  None if w is None else w.data_ptr(), t["master"].numel(), 1 if t.get("decay", True) else 0,
+                                  None if w16 is None else w16.data_ptr())
     d = lsp_adamw_desc(lr, beta1, beta2, eps, weight_decay, clip_norm, step, grad_scale, phase)
     ctx.check(lib().lsp_adamw_step(ctx.handle, len(tensors), arr, C.byref(d), _ptr(gnorm_out), _stream(stream)))
 

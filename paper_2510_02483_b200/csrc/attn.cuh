@@ -227,8 +227,10 @@ __global__ void __launch_bounds__(256, 1) attn_fwd_kernel(const AttnParams p) {
 }
 
 // ------------------------------------------------------------------------------------------- D = rowsum(dO * O32)
-// one warp per (token, head); dO fp16 (the tensor-core operand), O fp32.
-template <int D>
+// one warp per (token, head); dO fp16 (the tensor-core operand), O fp32.  Used where no O-projection dgrad precedes the
+// attention backward (lsp_sdpa_bwd) and on the head_dim 64 path; inside the layer the sums are formed by that GEMM's
+// epilogue (EpiDOutDvec).  PARTS4: write the [B, nq, S, 4] partial-sum layout the tcgen05 kernels read, as (D, 0, 0, 0).
+template <int D, bool PARTS4>
 __global__ void attn_dvec_kernel(const __half* dO, long long lddo, const float* o32, long long ldo, float* dvec,
                                  int B, int S, int nq) {
   const long long gw = (static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x) >> 5;
@@ -247,7 +249,9 @@ __global__ void attn_dvec_kernel(const __half* dO, long long lddo, const float* 
   for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
   if (lane == 0) {
     const int b = static_cast<int>(t / S), s = static_cast<int>(t % S);
-    dvec[(static_cast<long long>(b) * nq + h) * S + s] = acc;
+    const long long idx = (static_cast<long long>(b) * nq + h) * S + s;
+    if (PARTS4) reinterpret_cast<float4*>(dvec)[idx] = make_float4(acc, 0.f, 0.f, 0.f);
+    else dvec[idx] = acc;
   }
 }
 
@@ -562,28 +566,34 @@ template <int D> constexpr int attn_dq_smem() { return (2 * 64 + 4 * 64) * D * 2
 
 template <int D>
 cudaError_t attn_fwd_launch(const AttnParams& p, cudaStream_t st) {
-  static bool set = false;
-  if (!set) { cudaFuncSetAttribute(attn_fwd_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_fwd_smem<D>()); set = true; }
+  static DeviceOnce once;
+  if (once.need()) {
+    cudaError_t e = cudaFuncSetAttribute(attn_fwd_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_fwd_smem<D>());
+    if (e != cudaSuccess) return e;
+    once.done();
+  }
   dim3 grid((p.S + 127) / 128, p.nq, p.B);
   attn_fwd_kernel<D><<<grid, 256, attn_fwd_smem<D>(), st>>>(p);
   return cudaGetLastError();
 }
-template <int D>
+template <int D, bool PARTS4>
 cudaError_t attn_dvec_launch(const __half* dO, long long lddo, const float* o32, long long ldo, float* dvec, int B, int S,
                              int nq, cudaStream_t st) {
   const long long warps = static_cast<long long>(B) * S * nq;
   const int threads = 256;
   const long long blocks = (warps * 32 + threads - 1) / threads;
-  attn_dvec_kernel<D><<<static_cast<unsigned>(blocks), threads, 0, st>>>(dO, lddo, o32, ldo, dvec, B, S, nq);
+  attn_dvec_kernel<D, PARTS4><<<static_cast<unsigned>(blocks), threads, 0, st>>>(dO, lddo, o32, ldo, dvec, B, S, nq);
   return cudaGetLastError();
 }
 template <int D>
 cudaError_t attn_bwd_launch(const AttnParams& p, cudaStream_t st) {
-  static bool set = false;
-  if (!set) {
-    cudaFuncSetAttribute(attn_bwd_dkdv_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_dkdv_smem<D>());
-    cudaFuncSetAttribute(attn_bwd_dq_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_dq_smem<D>());
-    set = true;
+  static DeviceOnce once;
+  if (once.need()) {
+    cudaError_t e = cudaFuncSetAttribute(attn_bwd_dkdv_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_dkdv_smem<D>());
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(attn_bwd_dq_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, attn_dq_smem<D>());
+    if (e != cudaSuccess) return e;
+    once.done();
   }
   dim3 g1((p.S + 63) / 64, p.nkv, p.B);
   attn_bwd_dkdv_kernel<D><<<g1, 128, attn_dkdv_smem<D>(), st>>>(p);

@@ -486,13 +486,13 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
 // q [B*S, ldq] (head h at columns h*128), k, v [B*S, ldk/ldv] (kv head at columns kvh*128), all fp16.
 inline cudaError_t attn_fwd_tc_launch(const __half* q, long long ldq, const __half* k, long long ldk, const __half* v,
                                       long long ldv, const AttnTcParams& p, int num_sms, cudaStream_t st) {
-  static bool set = false;
-  if (!set) {
+  static DeviceOnce once;
+  if (once.need()) {
     cudaError_t e = cudaFuncSetAttribute(attn_fwd_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_FWD_SMEM);
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(attn_fwd_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_FWD_SMEM);
     if (e != cudaSuccess) return e;
-    set = true;
+    once.done();
   }
   AttnTcMaps maps;
   if (!make_map_attn(&maps.q, q, p.nq * ATC_D, p.S, p.B, ldq) || !make_map_attn(&maps.k, k, p.nkv * ATC_D, p.S, p.B, ldk) ||
@@ -539,7 +539,8 @@ struct AttnTcBwdParams {
   int B, S, nq, nkv;
   float scale_log2, scale;
   const float* lse;            // [B, nq, S]
-  const float* dvec;           // [B, nq, S]
+  const float* dvec;           // [B, nq, S, 4]: D = rowsum(dO * O) as four partial sums (one per 32-column chunk of the
+                               // head, written by the O-projection dgrad epilogue); readers add them as (x + y) + (z + w)
   const float2* rope;          // (cos, sin) [S, 64] or null: inverse rotation of dq, dk on store
   float* dq32; float* dk32; float* dv32; long long lddq32, lddk32;
   __half* dq16; __half* dk16; __half* dv16; long long ldd16;
@@ -565,11 +566,9 @@ __device__ __forceinline__ uint32_t atc_half_operand_col(int kk) { return static
 
 // x = hi + lo with both halves fp16: packs two values' hi parts and lo parts.
 __device__ __forceinline__ void atc_split_pack(float x0, float x1, uint32_t& hi, uint32_t& lo) {
-  const __half2 h = __floats2half2_rn(x0, x1);
-  const float2 hf = __half22float2(h);
-  const __half2 l = __floats2half2_rn(x0 - hf.x, x1 - hf.y);
-  hi = *reinterpret_cast<const uint32_t*>(&h);
-  lo = *reinterpret_cast<const uint32_t*>(&l);
+  hi = pack_f16(x0, x1);
+  const float2 hf = __half22float2(*reinterpret_cast<const __half2*>(&hi));
+  lo = pack_f16(x0 - hf.x, x1 - hf.y);
 }
 
 // Scale, optionally rotate by -theta (transpose of the forward rotation) 32 columns of this thread's row, then write the
@@ -619,7 +618,12 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
   const int warp = warp_idx_uniform(), lane = threadIdx.x & 31;
-  const int kb = blockIdx.x, kvh = blockIdx.y, b = blockIdx.z;
+  // 1-D grid, key block SLOWEST: CTAs are dispatched in linear order and a CTA's work falls linearly with its key block
+  // (causal), so the heaviest CTAs of ALL (kv head, batch) groups start first and the light ones fill the tail
+  // (longest-processing-time order: makespan 696 instead of 792 block units on 148 SMs at S = 4096, 8 kv heads x 4).
+  const int ngroups = p.nkv * p.B;
+  const int kb = static_cast<int>(blockIdx.x) / ngroups, grp = static_cast<int>(blockIdx.x) - kb * ngroups;
+  const int kvh = grp % p.nkv, b = grp / p.nkv;
   const int G = p.nq / p.nkv;
   const int k0 = kb * 128;
   // packed sequences: no query past the end of the sequence of this block's last key attends any of its keys
@@ -674,7 +678,8 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
         const int s = s0 + lane + 32 * r;
         const bool ok = s < p.S;
         sLD_ptr[st * 128 + lane + 32 * r] = ok ? p.lse[vbase + s] * 1.4426950408889634f : INFINITY;
-        sLD_ptr[st * 128 + 64 + lane + 32 * r] = ok ? p.dvec[vbase + s] : 0.f;
+        const float4 d4 = ok ? __ldg(reinterpret_cast<const float4*>(p.dvec) + vbase + s) : make_float4(0.f, 0.f, 0.f, 0.f);
+        sLD_ptr[st * 128 + 64 + lane + 32 * r] = (d4.x + d4.y) + (d4.z + d4.w);
       }
       mbar_arrive(ld_full(st));
     }
@@ -853,18 +858,25 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
 }
 
 // --------------------------------------------------------------------------------------------- dQ
-// Three S / dP accumulator buffers (TMEM: S [0,192), dP [192,384), dQ [384,512)) and four K/V stages: the tensor core
-// works two key blocks ahead of the softmax threads, so the commit -> mbarrier -> tcgen05.ld round trip (~800 cycles
-// measured) is off the critical path.
-constexpr int ATC_DQ_NB = 3;
+// Q and dO of the item are the A operands of EVERY S = Q K^T and dP = dO V^T block of its key loop.  As shared-memory
+// operands (SS) an M = 128 MMA re-reads them at 32 cycles per K = 16 step whatever N is, which made the N = 64 steps cost
+// 48 cycles instead of 32 (shared-memory bound, measured; 1024 instead of 768 tensor cycles per 128 x 64 block).  They
+// now live in TMEM: the 8 softmax warps copy the TMA-landed tiles (lane = query row, two 16-bit values per column)
+// once per item, and S / dP run as TS MMAs whose only shared-memory traffic is the 64-key K / V tile.
+// TMEM: Q [0,64) dO [64,128) | S buffers [128,256) | dP buffers [256,384) | dQ [384,512).  Two S / dP buffers: the tensor
+// core works one key block ahead of the softmax threads (768 tensor cycles per block against ~500 of softmax).
+constexpr int ATC_DQ_NB = 2;
 constexpr int ATC_DQ_NST = 4;
 constexpr int ATC_DQ_SMEM = 2 * ATC_TILE_BYTES + 2 * ATC_DQ_NST * ATC_HALF_TILE + 8 * GEMM_STAGE_TILE_BYTES + 1024 + 256;
-constexpr int ATC_DQ_DP = 64 * ATC_DQ_NB;        // first dP column
-constexpr int ATC_DQ_ACC = 2 * 64 * ATC_DQ_NB;   // dQ accumulator column
+constexpr int ATC_DQ_QA = 0;                     // Q operand columns
+constexpr int ATC_DQ_DOA = 64;                   // dO operand columns
+constexpr int ATC_DQ_S = 128;                    // first S column
+constexpr int ATC_DQ_DP = 256;                   // first dP column
+constexpr int ATC_DQ_ACC = 384;                  // dQ accumulator column
 // Persistent like the forward: work items (128-query block, head, batch) come heaviest-first from an atomic counter
-// (p.sched + 4); Q / dO of the next item are fetched as soon as the item's last S / dP MMA has been issued (qdo_empty),
-// the dQ epilogue (TMEM -> staging tile -> bulk stores) overlaps the first S / dP MMAs of the next item, and acc_free
-// tells the MMA warp when the dQ accumulator may be overwritten.
+// (p.sched + 4); Q / dO of the next item are fetched as soon as the softmax warps have copied the current ones to TMEM
+// (qdo_empty), the dQ epilogue (TMEM -> staging tile -> bulk stores) overlaps the first S / dP MMAs of the next item, and
+// acc_free tells the MMA warp when the dQ accumulator may be overwritten.
 struct AttnDqItem { int q0, h, b, kvh, iters, j0, split; };        // j0: first 64-key block (packed sequences), else 0
 __device__ __forceinline__ AttnDqItem attn_dq_item(uint32_t i, const AttnTcBwdParams& p, int nqb, const int* doc_start) {
   const int per_lvl = p.nq * p.B;
@@ -881,6 +893,16 @@ __device__ __forceinline__ AttnDqItem attn_dq_item(uint32_t i, const AttnTcBwdPa
   return it;
 }
 
+// This thread's row of one 64-column chunk of a TMA-landed 128 x 128 fp16 tile (128B swizzle) -> 32 TMEM columns.
+__device__ __forceinline__ void atc_row_chunk_to_tmem(uint32_t chunk_smem, int row, uint32_t taddr) {
+  uint32_t w[32];
+#pragma unroll
+  for (int u = 0; u < 8; ++u)
+    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(w[4 * u]), "=r"(w[4 * u + 1]), "=r"(w[4 * u + 2]), "=r"(w[4 * u + 3])
+                 : "r"(chunk_smem + row * 128 + ((u ^ (row & 7)) << 4)) : "memory");
+  tmem_st32(taddr, w);
+}
+
 template <bool DOC>
 __global__ void __launch_bounds__(ATC_BWD_THREADS, 1)
 attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdParams p) {
@@ -895,16 +917,18 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
   const uint32_t sV = sK + ATC_DQ_NST * ATC_HALF_TILE;
   const uint32_t stage_tiles = sV + ATC_DQ_NST * ATC_HALF_TILE;      // 8 x 4 KB staging tiles (epilogue)
   const uint32_t bar_base = stage_tiles + 8 * GEMM_STAGE_TILE_BYTES;
-  auto qdo_full = [&]() { return bar_base; };
+  auto qdo_full = [&]() { return bar_base; };                    // TMA: Q, dO of the item have landed in shared memory
   auto acc_full = [&]() { return bar_base + 8u; };
-  auto qdo_empty = [&]() { return bar_base + 16u; };
+  auto qdo_empty = [&]() { return bar_base + 16u; };             // 8 softmax warps: the tiles have been copied out
   auto acc_free = [&]() { return bar_base + 24u; };
-  auto kv_full = [&](int s) { return bar_base + 8u * (4 + s); };
-  auto kv_empty = [&](int s) { return bar_base + 8u * (4 + ATC_DQ_NST + s); };
-  auto sdp_full = [&](int s) { return bar_base + 8u * (4 + 2 * ATC_DQ_NST + s); };
-  auto ds_full = [&](int s) { return bar_base + 8u * (4 + ATC_DQ_NB + 2 * ATC_DQ_NST + s); };
-  auto item_bar = [&](int s) { return bar_base + 8u * (4 + 2 * ATC_DQ_NB + 2 * ATC_DQ_NST + s); };
-  const uint32_t item_slots = bar_base + 8u * (4 + 2 * ATC_DQ_NB + 2 * ATC_DQ_NST + ATC_ITEM_RING);
+  auto qa_full = [&]() { return bar_base + 32u; };               // 8 softmax warps: the TMEM operands of the item are written
+  auto qa_free = [&]() { return bar_base + 40u; };               // MMA: the item's last S / dP has read them
+  auto kv_full = [&](int s) { return bar_base + 8u * (6 + s); };
+  auto kv_empty = [&](int s) { return bar_base + 8u * (6 + ATC_DQ_NST + s); };
+  auto sdp_full = [&](int s) { return bar_base + 8u * (6 + 2 * ATC_DQ_NST + s); };
+  auto ds_full = [&](int s) { return bar_base + 8u * (6 + ATC_DQ_NB + 2 * ATC_DQ_NST + s); };
+  auto item_bar = [&](int s) { return bar_base + 8u * (6 + 2 * ATC_DQ_NB + 2 * ATC_DQ_NST + s); };
+  const uint32_t item_slots = bar_base + 8u * (6 + 2 * ATC_DQ_NB + 2 * ATC_DQ_NST + ATC_ITEM_RING);
   const uint32_t tmem_slot = item_slots + 4u * ATC_ITEM_RING;
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
   volatile uint32_t* item_slot_ptr = reinterpret_cast<volatile uint32_t*>(smem_raw + (item_slots - smem_u32(smem_raw)));
@@ -917,7 +941,8 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
   if (threadIdx.x == 0) {
     tma_prefetch_desc(&maps.q); tma_prefetch_desc(&maps.k); tma_prefetch_desc(&maps.v); tma_prefetch_desc(&maps.dO);
     tma_prefetch_desc(&maps.g32[0]); tma_prefetch_desc(&maps.g16[0]);
-    mbar_init(qdo_full(), 1); mbar_init(acc_full(), 1); mbar_init(qdo_empty(), 1); mbar_init(acc_free(), 8);
+    mbar_init(qdo_full(), 1); mbar_init(acc_full(), 1); mbar_init(qdo_empty(), 8); mbar_init(acc_free(), 8);
+    mbar_init(qa_full(), 8); mbar_init(qa_free(), 1);
     for (int i = 0; i < ATC_DQ_NST; ++i) { mbar_init(kv_full(i), 1); mbar_init(kv_empty(i), 1); }
     for (int i = 0; i < ATC_DQ_NB; ++i) { mbar_init(sdp_full(i), 1); mbar_init(ds_full(i), 8); }
     for (int i = 0; i < ATC_ITEM_RING; ++i) mbar_init(item_bar(i), 1);
@@ -946,7 +971,7 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
       publish(0, item);
       for (uint32_t it = 0; item < nitems; ++it) {
         const AttnDqItem w = attn_dq_item(item, p, nqb, doc_start);
-        mbar_wait(qdo_empty(), (it & 1u) ^ 1u);                  // the previous item's S / dP MMAs have read Q, dO
+        mbar_wait(qdo_empty(), (it & 1u) ^ 1u);                  // the previous item's Q, dO have been copied to TMEM
         mbar_expect_tx(qdo_full(), 2 * ATC_TILE_BYTES);
         tma_load_3d(sQ, &maps.q, qdo_full(), w.h * ATC_D, w.q0, w.b);
         tma_load_3d(sQ + ATC_CHUNK_BYTES, &maps.q, qdo_full(), w.h * ATC_D + 64, w.q0, w.b);
@@ -971,9 +996,8 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
   } else if (warp == 1) {
     // ===================================================================== MMA issuer (whole warp, elected lane issues)
     const uint32_t leader = elect_one();
-    const uint32_t idesc_sdp = umma_idesc(128, 64, 0, 0, 0, 0);     // [128 queries x 64 keys]
+    const uint32_t idesc_sdp = umma_idesc(128, 64, 0, 0, 0, 0);     // [128 queries x 64 keys], A from TMEM
     const uint32_t idesc_acc = umma_idesc(128, 128, 0, 0, 0, 1);    // dQ [128 x 128] += dS(TMEM) K(MN-major)
-    const uint64_t dQd = umma_smem_desc(sQ, 16, 1024), dDO = umma_smem_desc(sDO, 16, 1024);
     const uint64_t dKk = umma_smem_desc(sK, 16, 1024), dVk = umma_smem_desc(sV, 16, 1024);
     const uint64_t dKm = umma_smem_desc(sK, 64 * 128, 1024);
     auto issue_sdp = [&](uint32_t g) {                               // g: global block index (ring positions)
@@ -984,10 +1008,10 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
         const uint64_t ka = desc_adv(dKk, st * ATC_HALF_TILE), va = desc_adv(dVk, st * ATC_HALF_TILE);
 #pragma unroll
         for (int kk = 0; kk < 8; ++kk) {                              // two independent accumulation chains, interleaved
-          umma_f16(tmem_base + buf * 64, desc_adv(dQd, (kk >> 2) * ATC_CHUNK_BYTES + (kk & 3) * 32),
-                   desc_adv(ka, (kk >> 2) * (64 * 128) + (kk & 3) * 32), idesc_sdp, kk != 0 ? 1u : 0u);
-          umma_f16(tmem_base + ATC_DQ_DP + buf * 64, desc_adv(dDO, (kk >> 2) * ATC_CHUNK_BYTES + (kk & 3) * 32),
-                   desc_adv(va, (kk >> 2) * (64 * 128) + (kk & 3) * 32), idesc_sdp, kk != 0 ? 1u : 0u);
+          umma_f16_ts(tmem_base + ATC_DQ_S + buf * 64, tmem_base + ATC_DQ_QA + kk * 8,
+                      desc_adv(ka, (kk >> 2) * (64 * 128) + (kk & 3) * 32), idesc_sdp, kk != 0 ? 1u : 0u);
+          umma_f16_ts(tmem_base + ATC_DQ_DP + buf * 64, tmem_base + ATC_DQ_DOA + kk * 8,
+                      desc_adv(va, (kk >> 2) * (64 * 128) + (kk & 3) * 32), idesc_sdp, kk != 0 ? 1u : 0u);
         }
         umma_commit(sdp_full(buf));
       }
@@ -998,17 +1022,14 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
       if (item >= nitems) break;
       const AttnDqItem w = attn_dq_item(item, p, nqb, doc_start);
       const int iters = w.iters;
-      mbar_wait(qdo_full(), it & 1u);
+      mbar_wait(qa_full(), it & 1u);                                 // Q, dO operands of this item are in TMEM
+      tc_fence_after();
       issue_sdp(g0);
       if (iters > 1) issue_sdp(g0 + 1);
-      if (iters <= 2 && leader) umma_commit(qdo_empty());            // those were the item's last S / dP MMAs
+      if (iters <= 2 && leader) umma_commit(qa_free());              // those were the item's last S / dP MMAs
       for (int j = 0; j < iters; ++j) {
         const uint32_t g = g0 + j;
         const int st = g % ATC_DQ_NST, buf = g % ATC_DQ_NB;
-        if (j + 2 < iters) {
-          issue_sdp(g + 2);                                          // its buffers were released by dQ(j - 1), already issued
-          if (j + 3 == iters && leader) umma_commit(qdo_empty());
-        }
         mbar_wait(ds_full(buf), (g / ATC_DQ_NB) & 1u);
         if (j == 0 && it > 0) mbar_wait(acc_free(), (it - 1u) & 1u); // the previous item's dQ has been read out
         tc_fence_after();
@@ -1016,15 +1037,19 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
           const uint64_t ka = desc_adv(dKm, st * ATC_HALF_TILE);
 #pragma unroll
           for (int kk = 0; kk < 4; ++kk)
-            umma_f16_ts(tmem_base + ATC_DQ_ACC, tmem_base + buf * 64 + atc_half_operand_col(kk), desc_adv(ka, kk * 2048), idesc_acc,
-                        (j | kk) != 0 ? 1u : 0u);
+            umma_f16_ts(tmem_base + ATC_DQ_ACC, tmem_base + ATC_DQ_S + buf * 64 + atc_half_operand_col(kk), desc_adv(ka, kk * 2048),
+                        idesc_acc, (j | kk) != 0 ? 1u : 0u);
           if (w.split) {                                // early query rows: + dS_lo K
 #pragma unroll
             for (int kk = 0; kk < 4; ++kk)
-              umma_f16_ts(tmem_base + ATC_DQ_ACC, tmem_base + buf * 64 + 16 + atc_half_operand_col(kk), desc_adv(ka, kk * 2048),
-                          idesc_acc, 1u);
+              umma_f16_ts(tmem_base + ATC_DQ_ACC, tmem_base + ATC_DQ_S + buf * 64 + 16 + atc_half_operand_col(kk),
+                          desc_adv(ka, kk * 2048), idesc_acc, 1u);
           }
           umma_commit(kv_empty(st));
+        }
+        if (j + 2 < iters) {                                         // this block's S / dP buffers are free again (in-order issue)
+          issue_sdp(g + 2);
+          if (j + 3 == iters && leader) umma_commit(qa_free());
         }
       }
       if (leader) umma_commit(acc_full());
@@ -1039,22 +1064,38 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
     const float c = p.scale_log2;
     const WarpStage wst{stage_tiles + static_cast<uint32_t>(warp - 2) * GEMM_STAGE_TILE_BYTES, lane};
     uint32_t g = 0;                                                  // global block index
-    for (uint32_t it = 0;; ++it) {
-      const uint32_t item = get_item(it);
-      if (item >= nitems) break;
+    // Q, dO of item `k`: this warp copies its 32 rows x its 64-column chunk of both TMA-landed tiles to the TMEM operand
+    // columns, then releases the shared-memory tiles to the producer.  Done for item k + 1 right after the LAST dS of
+    // item k has been handed over and BEFORE item k's epilogue, so that the MMA warp finds the next operands ready when
+    // it has issued item k's last dQ: no tensor bubble between items.
+    auto copy_in = [&](uint32_t k) {
+      mbar_wait(qdo_full(), k & 1u);
+      if (k > 0) mbar_wait(qa_free(), (k - 1u) & 1u);                // the previous item's S / dP MMAs have read the operands
+      tc_fence_after();
+      atc_row_chunk_to_tmem(sQ + half * ATC_CHUNK_BYTES, row, tmem_base + lane_off + ATC_DQ_QA + half * 32);
+      atc_row_chunk_to_tmem(sDO + half * ATC_CHUNK_BYTES, row, tmem_base + lane_off + ATC_DQ_DOA + half * 32);
+      tmem_st_wait();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) { mbar_arrive(qa_full()); mbar_arrive(qdo_empty()); }
+    };
+    uint32_t item = get_item(0);
+    if (item < nitems) copy_in(0);
+    for (uint32_t it = 0; item < nitems; ++it) {
       const AttnDqItem w = attn_dq_item(item, p, nqb, doc_start);
       const int q0 = w.q0, qi = q0 + row;
       const bool valid = qi < p.S;
       const long long vidx = (static_cast<long long>(w.b) * p.nq + w.h) * p.S + qi;
       const float L2 = valid ? p.lse[vidx] * 1.4426950408889634f : INFINITY;
-      const float Dr = valid ? p.dvec[vidx] : 0.f;
+      const float4 d4 = valid ? __ldg(reinterpret_cast<const float4*>(p.dvec) + vidx) : make_float4(0.f, 0.f, 0.f, 0.f);
+      const float Dr = (d4.x + d4.y) + (d4.z + d4.w);
       const int dstart = doc_start ? doc_start[min(qi, p.S - 1)] : 0;      // first key this query may see
       for (int j = 0; j < w.iters; ++j, ++g) {
         const int buf = g % ATC_DQ_NB;
         mbar_wait(sdp_full(buf), (g / ATC_DQ_NB) & 1u);
         tc_fence_after();
         uint32_t sr[32], dr[32];
-        tmem_ld32(tmem_base + lane_off + buf * 64 + col0, sr);
+        tmem_ld32(tmem_base + lane_off + ATC_DQ_S + buf * 64 + col0, sr);
         tmem_ld32(tmem_base + lane_off + ATC_DQ_DP + buf * 64 + col0, dr);
         tmem_ld_wait();
         float ds[32];
@@ -1078,17 +1119,19 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
           uint32_t pl[16];
 #pragma unroll
           for (int i = 0; i < 16; ++i) atc_split_pack(ds[2 * i], ds[2 * i + 1], pk[i], pl[i]);
-          tmem_st16(tmem_base + lane_off + buf * 64 + col0 + 16, pl);
+          tmem_st16(tmem_base + lane_off + ATC_DQ_S + buf * 64 + col0 + 16, pl);
         } else {
 #pragma unroll
           for (int i = 0; i < 16; ++i) pk[i] = pack_f16(ds[2 * i], ds[2 * i + 1]);
         }
-        tmem_st16(tmem_base + lane_off + buf * 64 + col0, pk);
+        tmem_st16(tmem_base + lane_off + ATC_DQ_S + buf * 64 + col0, pk);
         tmem_st_wait();
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(ds_full(buf));
       }
+      const uint32_t next = get_item(it + 1);
+      if (next < nitems) copy_in(it + 1);
       // epilogue: this warp stores rows [32 quarter, +32), columns [64 half, +64) of dQ, then releases the accumulator
       mbar_wait(acc_full(), it & 1u);
       tc_fence_after();
@@ -1107,6 +1150,7 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
         atc_store_grad32(wst, reinterpret_cast<float(&)[32]>(a1), p.scale, rr ? rr + 16 : nullptr, p.dq32 ? &maps.g32[0] : nullptr,
                          p.dq16 ? &maps.g16[0] : nullptr, w.h * ATC_D + half * 64 + 32, s0, w.b);
       }
+      item = next;
     }
     if (lane == 0) tma_store_wait_all<0>();
   }
@@ -1117,8 +1161,8 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
 }
 
 inline cudaError_t attn_bwd_tc_set_attrs() {
-  static bool set = false;
-  if (!set) {
+  static DeviceOnce once;
+  if (once.need()) {
     cudaError_t e = cudaFuncSetAttribute(attn_bwd_dkdv_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_BWD_SMEM);
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(attn_bwd_dkdv_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_BWD_SMEM);
@@ -1127,7 +1171,7 @@ inline cudaError_t attn_bwd_tc_set_attrs() {
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(attn_bwd_dq_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ATC_DQ_SMEM);
     if (e != cudaSuccess) return e;
-    set = true;
+    once.done();
   }
   return cudaSuccess;
 }
@@ -1148,7 +1192,7 @@ inline cudaError_t attn_bwd_dkdv_tc_launch(const __half* q, long long ldq, const
       (p.dv16 && !make_map_store(&m1.g16[0], p.dv16, p.nkv * ATC_D, p.S, p.B, p.ldd16, false)) ||
       (p.dk16 && !make_map_store(&m1.g16[1], p.dk16, p.nkv * ATC_D, p.S, p.B, p.ldd16, false)))
     return cudaErrorInvalidValue;
-  dim3 g1((p.S + 127) / 128, p.nkv, p.B);
+  dim3 g1(((p.S + 127) / 128) * p.nkv * p.B, 1, 1);
   if (p.doc_start) attn_bwd_dkdv_tc_kernel<true><<<g1, ATC_BWD_THREADS, ATC_BWD_SMEM, st>>>(m1, p);
   else attn_bwd_dkdv_tc_kernel<false><<<g1, ATC_BWD_THREADS, ATC_BWD_SMEM, st>>>(m1, p);
   return cudaGetLastError();

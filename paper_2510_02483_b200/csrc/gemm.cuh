@@ -391,6 +391,8 @@ struct EpiStore {
   long long ld;              // row pitch (elements) of every output and of the residual
   const void* res;
   float alpha;
+  const float* alpha_dev = nullptr;   // optional DEVICE scalar multiplied into alpha (a factor only the device knows: the
+                                      // valid-token count of the cross-entropy, lsp_head_fwd_bwd)
   CUtensorMap omap[3];       // store maps of the up-to-three outputs (encoded by the host in encode())
   int use_tma;               // 0 when a 32-row chunk can straddle a split (splits not multiples of 32): per-thread stores
   int accumulate = 0;        // 1: out += result (fp32 outputs; lsp_layer_desc.wgrad_accumulate) instead of out = result
@@ -424,9 +426,10 @@ struct EpiStore {
     }
   }
   __device__ __forceinline__ void operator()(const WarpStage& st, int m_base, int n, float (&v)[32], int nrows, int nvalid) const {
-    if (alpha != 1.0f) {
+    const float al = alpha_dev ? alpha * __ldg(alpha_dev) : alpha;
+    if (al != 1.0f) {
 #pragma unroll
-      for (int j = 0; j < 32; ++j) v[j] *= alpha;
+      for (int j = 0; j < 32; ++j) v[j] *= al;
     }
     if constexpr (HAS_RES) {
       using RT = typename OutElem<RDT>::type;
@@ -551,6 +554,47 @@ struct EpiSwiGLUBwd {
     }
     chunk_store_tma<DT_F16>(st, &dgmap, n, m_base, g);
     chunk_store_tma<DT_F16>(st, &dumap, n, m_base, u);
+  }
+};
+
+// O-projection dgrad with the row sums of the attention backward fused in: acc = dO = da Wo; writes dO
+// (fp16, the operand of the attention backward) and, per 32-column chunk, the partial sum over the chunk of dO * O with
+// the fp32 copy of O (precision plan P-3) -- D_i = rowsum(dO_i * O_i) = sum_j P_ij dP_ij is the row term of the softmax
+// backward.  The products use the fp16-ROUNDED dO, the value the dP MMAs will see, so that sum_j dS_ij = 0 holds to
+// rounding.  head_dim 128 = 4 chunks: dvec4 is [B, nq, S, 4] and its readers add the four partials in the fixed order
+// (x + y) + (z + w).  Row m is token (b, s) = (m / S, m % S).  Replaces a separate pass over dO and O (0.10 ms at cfg 2).
+struct EpiDOutDvec {
+  static constexpr bool kStoreOnly = false;
+  __half* dO; long long ld;          // [T, Nq] fp16 out
+  const float* o32;                  // [T, Nq] fp32 (saved by the forward)
+  float* dvec4;                      // [B, nq, S, 4]
+  int S, nq;
+  CUtensorMap omap;
+  bool encode(int M, int N) { return make_map_store2d(&omap, dO, M, N, ld, DT_F16); }
+  __device__ __forceinline__ void prefetch(int lane, int m_base, int n0, int nrows, int ncols) const {
+    if (lane < nrows) {
+      const float* rp = o32 + static_cast<long long>(m_base + lane) * ld + n0;
+      for (int c = 0; c < ncols; c += 32) prefetch_l2(rp + c);
+    }
+  }
+  __device__ __forceinline__ void operator()(const WarpStage& st, int m_base, int n, float (&v)[32], int nrows, int nvalid) const {
+    float o[32];
+    const float* obase = o32 + static_cast<long long>(m_base) * ld + n;
+    chunk_load<DT_F32>(st, [&](int rr) { return obase + rr * ld; }, o, nrows, nvalid);
+    float acc0 = 0.f, acc1 = 0.f;
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+      const __half2 h = __floats2half2_rn(v[2 * j], v[2 * j + 1]);
+      const float2 f = __half22float2(h);
+      acc0 = fmaf(f.x, o[2 * j], acc0);
+      acc1 = fmaf(f.y, o[2 * j + 1], acc1);
+    }
+    if (st.lane < nrows) {
+      const int m = m_base + st.lane;
+      const int b = m / S, sq = m - b * S;
+      dvec4[((static_cast<long long>(b) * nq + (n >> 7)) * S + sq) * 4 + ((n >> 5) & 3)] = acc0 + acc1;
+    }
+    chunk_store_tma<DT_F16>(st, &omap, n, m_base, v);
   }
 };
 
@@ -1165,11 +1209,11 @@ cudaError_t launch_gemm_pair(const GemmMaps& maps, GemmShape sh, const Epi& epi,
                              const GemmSKRes* sk) {
   using G = Gemm2Cfg<MT>;
   auto kern = gemm_pair_tcgen05_kernel<A_MN, B_MN, DUAL, MT, Epi>;
-  static bool attr_set = false;
-  if (!attr_set) {
+  static DeviceOnce once;
+  if (once.need()) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEM_BYTES);
     if (e != cudaSuccess) return e;
-    attr_set = true;
+    once.done();
   }
   constexpr int NOUT = DUAL ? 128 : 256;
   const int mblocks = (sh.M + 2 * MT * GEMM_BM - 1) / (2 * MT * GEMM_BM), nblocks = (sh.N + NOUT - 1) / NOUT;
@@ -1193,11 +1237,11 @@ template <int BN, bool A_MN, bool B_MN, bool DUAL, class Epi>
 cudaError_t launch_gemm(const GemmMaps& maps, GemmShape sh, const Epi& epi, int num_sms, cudaStream_t st) {
   using Cfg = GemmCfg<BN>;
   auto kern = gemm_tcgen05_kernel<BN, A_MN, B_MN, DUAL, Epi>;
-  static bool attr_set = false;
-  if (!attr_set) {
+  static DeviceOnce once;
+  if (once.need()) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES);
     if (e != cudaSuccess) return e;
-    attr_set = true;
+    once.done();
   }
   constexpr int NOUT = DUAL ? BN / 2 : BN;
   const int mblocks = (sh.M + GEMM_BM - 1) / GEMM_BM, nblocks = (sh.N + NOUT - 1) / NOUT;

@@ -35,6 +35,8 @@ __device__ __forceinline__ void ce_block_reduce(float& m, float& s, float2* red)
 // loads per thread in flight; pass 2: dz from the row, mostly still in L2 (296 rows x 513 KB at V = 128256 is a little
 // over the 126 MB L2).  loss_row[t] = lse_t - z[t, y_t].  V % 4 == 0.  Measured at T = 8192, V = 128256: 3.95 ms with
 // three passes and one load in flight -> 2.06 ms (6.3 GB of algorithmic traffic: 3.1 TB/s).
+// A target outside [0, V) (reading H-4: negative = "no loss at this position", e.g. padding or the last token of a
+// packed sequence) is never used as an index: the row's loss is 0 and its dz row is zero; lse is still written.
 __global__ void __launch_bounds__(CE_THREADS, 2) ce_fwd_bwd_kernel(const float* __restrict__ z, const int* __restrict__ y, int T, int V,
                                                                    float* __restrict__ lse, float* __restrict__ loss_row,
                                                                    __half* __restrict__ dz) {
@@ -63,9 +65,10 @@ __global__ void __launch_bounds__(CE_THREADS, 2) ce_fwd_bwd_kernel(const float* 
     ce_block_reduce(m, s, red);
     const float L = m + logf(s);
     const int yt = y[t];
+    const bool counted = yt >= 0 && yt < V;
     if (threadIdx.x == 0) {
       lse[t] = L;
-      loss_row[t] = L - z[static_cast<long long>(t) * V + yt];
+      loss_row[t] = counted ? L - z[static_cast<long long>(t) * V + yt] : 0.f;
     }
     uint2* dr = reinterpret_cast<uint2*>(dz + static_cast<long long>(t) * V);
     for (int i0 = threadIdx.x; i0 < V4; i0 += CE_UNROLL * CE_THREADS) {
@@ -81,6 +84,7 @@ __global__ void __launch_bounds__(CE_THREADS, 2) ce_fwd_bwd_kernel(const float* 
         if (i < V4) {
           float p[4] = {__expf(a[u].x - L), __expf(a[u].y - L), __expf(a[u].z - L), __expf(a[u].w - L)};
           const int c = 4 * i;
+          if (!counted) { p[0] = p[1] = p[2] = p[3] = 0.f; }
           if (yt >= c && yt < c + 4) p[yt - c] -= 1.0f;
           dr[i] = make_uint2(pack_f16(p[0] * CE_DZ_SCALE, p[1] * CE_DZ_SCALE), pack_f16(p[2] * CE_DZ_SCALE, p[3] * CE_DZ_SCALE));
         }
@@ -89,12 +93,19 @@ __global__ void __launch_bounds__(CE_THREADS, 2) ce_fwd_bwd_kernel(const float* 
   }
 }
 
-// loss = mean of loss_row (one thread, fp64, fixed order)
-__global__ void ce_loss_mean_kernel(const float* __restrict__ loss_row, int T, float* __restrict__ loss) {
+// loss = mean of loss_row over the COUNTED tokens (targets in [0, V)); one thread, fp64, fixed order.
+// inv_count[0] = T / n_counted (0 if none): the factor that turns the 1 / T the gradient GEMMs apply into 1 / n_counted.
+__global__ void ce_loss_mean_kernel(const float* __restrict__ loss_row, const int* __restrict__ y, int T, int V,
+                                    float* __restrict__ loss, float* __restrict__ inv_count) {
   if (threadIdx.x == 0 && blockIdx.x == 0) {
     double s = 0.0;
-    for (int t = 0; t < T; ++t) s += static_cast<double>(loss_row[t]);
-    loss[0] = static_cast<float>(s / T);
+    int n = 0;
+    for (int t = 0; t < T; ++t) {
+      s += static_cast<double>(loss_row[t]);
+      n += (y[t] >= 0 && y[t] < V) ? 1 : 0;
+    }
+    loss[0] = n > 0 ? static_cast<float>(s / n) : 0.f;
+    inv_count[0] = n > 0 ? static_cast<float>(static_cast<double>(T) / n) : 0.f;
   }
 }
 

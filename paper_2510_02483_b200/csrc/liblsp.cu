@@ -34,6 +34,9 @@ struct SavedLayout {
 struct WsLayout {
   size_t in16, dgu, dn32, da32, da16, dO16, dvec, dqkv16, dgpart, q16, k16, v16, total;
 };
+// fp16 operand copies of one layer's projection weights (lsp_weight_cache_bytes): [Wq; Wk; Wv] | Wo | [Wg; Wu] | Wd.
+// The same four blocks exist inside `saved` for calls that pass no cache.
+struct WCacheLayout { size_t wqkv16, wo16, wgu16, wd16, total; };
 
 }  // namespace
 
@@ -79,6 +82,8 @@ struct lsp_ctx {
   int norm_blocks;      // persistent grid of the RMSNorm backward
   SavedLayout sv;
   WsLayout ws;
+  WCacheLayout wc;
+  unsigned long long* overflow;  // device counter: values the fp16 operand casts clamped or found non-finite (lsp_overflow_count)
   char err[512];
 };
 
@@ -156,14 +161,42 @@ void plan_layout(lsp_ctx* c) {
   w.da32 = take(T * H * 4);
   w.da16 = take(T * H * 2);
   w.dO16 = take(T * Nq * 2);
-  w.dvec = take(BnqS * 4);
+  w.dvec = take(BnqS * 16);              // four partial sums per (batch, head, position) at head_dim 128
   w.dqkv16 = take(T * Nqkv * 2);
   w.dgpart = take(static_cast<size_t>(c->norm_blocks) * 2 * H * 4);      // one row per (CTA, row group) of rmsnorm_bwd_kernel
   w.q16 = take(T * Nq * 2);
   w.k16 = take(T * c->Nkv * 2);
   w.v16 = take(T * c->Nkv * 2);
   w.total = o;
+
+  o = 0;
+  WCacheLayout& k = c->wc;
+  k.wqkv16 = take(Nqkv * H * 2);
+  k.wo16 = take(H * Nq * 2);
+  k.wgu16 = take(2 * F * H * 2);
+  k.wd16 = take(H * F * 2);
+  k.total = o;
 }
+
+// Makes the context's device current for the duration of an entry point and restores the caller's on exit (several
+// contexts on several devices may live in one process); publishes the device to the per-device launch setup (DeviceOnce).
+struct DeviceGuard {
+  int prev = -1, prev_tls;
+  bool ok = true;
+  explicit DeviceGuard(int dev) : prev_tls(tls_device()) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; ok = false; return; }
+    if (prev != dev && cudaSetDevice(dev) != cudaSuccess) { ok = false; return; }
+    tls_device() = dev;
+  }
+  ~DeviceGuard() {
+    tls_device() = prev_tls;
+    int cur = -1;
+    if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev);
+  }
+};
+#define LSP_ENTER(ctx)                                                                     \
+  DeviceGuard guard__((ctx)->device);                                                      \
+  if (!guard__.ok) return fail((ctx), LSP_ECUDA, "cannot make device %d current", (ctx)->device)
 
 template <typename T> T* at(void* base, size_t off) { return reinterpret_cast<T*>(static_cast<uint8_t*>(base) + off); }
 template <typename T> const T* at(const void* base, size_t off) {
@@ -203,9 +236,9 @@ cudaError_t norm_bwd_t(const lsp_ctx* c, const void* x, const float* rstd, const
   const size_t smem = stages * stage_bytes;
 #define LSP_NB(NV, GG) case NV: { \
     auto kern = rmsnorm_bwd_kernel<XT, RT, NV, GG>; \
-    static bool set = false; \
-    if (!set) { cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, NORMB_SMEM_BUDGET); if (e != cudaSuccess) return e; set = true; } \
-    kern<<<nb, NORMB_THREADS, smem, st>>>(xp, rstd, gp, dxn, rp, dx, dx16, dg_part, c->T, H, stages, residual_scale(c->d)); } break;
+    static DeviceOnce once; \
+    if (once.need()) { cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, NORMB_SMEM_BUDGET); if (e != cudaSuccess) return e; once.done(); } \
+    kern<<<nb, NORMB_THREADS, smem, st>>>(xp, rstd, gp, dxn, rp, dx, dx16, dg_part, c->T, H, stages, residual_scale(c->d), c->overflow); } break;
   if (G == 2) {
     switch (nv) { LSP_NB(1, 2) LSP_NB(2, 2) LSP_NB(3, 2) LSP_NB(4, 2) LSP_NB(5, 2) LSP_NB(6, 2) LSP_NB(7, 2) LSP_NB(8, 2) default: return cudaErrorInvalidValue; }
   } else {
@@ -227,20 +260,20 @@ cudaError_t norm_bwd(const lsp_ctx* c, int x_dt, int r_dt, const void* x, const 
                          : norm_bwd_t<__nv_bfloat16, __nv_bfloat16>(c, x, rstd, g, dxn, dres, dx, dx16, dg_part, dg, acc, st);
 }
 
-cudaError_t cast_f32_f16(const float* in, __half* out, long long n, int sms, cudaStream_t st) {
+cudaError_t cast_f32_f16(const float* in, __half* out, long long n, int sms, unsigned long long* counter, cudaStream_t st) {
   const long long n8 = n / 8;
   long long blocks = (n8 + 255) / 256;
   if (blocks > sms * 16LL) blocks = sms * 16LL;
   if (blocks < 1) blocks = 1;
-  cast_f32_f16_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(in, out, n8);
+  cast_f32_f16_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(in, out, n8, counter);
   return cudaGetLastError();
 }
-cudaError_t cast_bf16_f16(const __nv_bfloat16* in, __half* out, long long n, int sms, cudaStream_t st) {
+cudaError_t cast_bf16_f16(const __nv_bfloat16* in, __half* out, long long n, int sms, unsigned long long* counter, cudaStream_t st) {
   const long long n8 = n / 8;
   long long blocks = (n8 + 255) / 256;
   if (blocks > sms * 16LL) blocks = sms * 16LL;
   if (blocks < 1) blocks = 1;
-  cast_bf16_f16_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(in, out, n8);
+  cast_bf16_f16_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(in, out, n8, counter);
   return cudaGetLastError();
 }
 
@@ -250,6 +283,7 @@ cudaError_t cast_weights(const lsp_ctx* c, int nseg, const void* const* src, __h
   CastSegs segs;
   segs.nseg = nseg;
   segs.perm_mask = perm_mask; segs.perm_d = c->d.head_dim; segs.row_units = c->d.hidden / 8;
+  segs.counter = c->overflow;
   segs.start[0] = 0;
   for (int i = 0; i < CAST_MAX_SEGS; ++i) {
     segs.src[i] = i < nseg ? static_cast<const __nv_bfloat16*>(src[i]) : nullptr;
@@ -310,6 +344,38 @@ cudaError_t gemm_fwd_residual(const lsp_ctx* c, const __half* A, int K, const __
   return gemm1<false, false>(c, T, H, K, a, b, e, st);
 }
 
+// fp16 operand copies of the projection weights: the caller's cache (lsp_layer_weights.f16_cache, filled by
+// lsp_layer_prepare_weights or by lsp_adamw_step's weight_f16 outputs) or the blocks inside `saved` that every forward
+// call refreshes itself.
+struct W16 { __half *wqkv, *wo, *wgu, *wd; bool cached; };
+inline W16 w16_of(const lsp_ctx* c, const lsp_layer_weights* w, const void* saved) {
+  if (w->f16_cache) {
+    void* k = const_cast<void*>(w->f16_cache);
+    return W16{at<__half>(k, c->wc.wqkv16), at<__half>(k, c->wc.wo16), at<__half>(k, c->wc.wgu16), at<__half>(k, c->wc.wd16), true};
+  }
+  void* k = const_cast<void*>(saved);
+  return W16{at<__half>(k, c->sv.wqkv16), at<__half>(k, c->sv.wo16), at<__half>(k, c->sv.wgu16), at<__half>(k, c->sv.wd16), false};
+}
+lsp_status cast_attn_weights(lsp_ctx* ctx, const lsp_layer_weights* w, const W16& k, cudaStream_t st) {
+  const lsp_layer_desc& d = ctx->d;
+  const long long H = d.hidden, Nq = ctx->Nq, Nkv = ctx->Nkv;
+  const void* src[4] = {w->wq, w->wk, w->wv, w->wo};
+  __half* dst[4] = {k.wqkv, k.wqkv + Nq * H, k.wqkv + (Nq + Nkv) * H, k.wo};
+  const long long cnt[4] = {Nq * H, Nkv * H, Nkv * H, H * Nq};
+  // rope_layout = 1: the rows of Wq, Wk are interleaved per head, so that the adjacent-pair rotation of the QKV epilogue
+  // acts on the half-split pairs (i, i + d/2); q.k is invariant under the common permutation
+  LSP_STAGE(ST_CAST, 1, cast_weights(ctx, 4, src, dst, cnt, st, (d.use_rope && d.rope_layout == 1) ? 0x3u : 0u));
+  return LSP_OK;
+}
+lsp_status cast_mlp_weights(lsp_ctx* ctx, const lsp_layer_weights* w, const W16& k, cudaStream_t st) {
+  const long long FH = static_cast<long long>(ctx->d.ffn) * ctx->d.hidden;
+  const void* src[3] = {w->w_gate, w->w_up, w->w_down};
+  __half* dst[3] = {k.wgu, k.wgu + FH, k.wd};
+  const long long cnt[3] = {FH, FH, FH};
+  LSP_STAGE(ST_CAST, 1, cast_weights(ctx, 3, src, dst, cnt, st));
+  return LSP_OK;
+}
+
 // F3 dispatch: head_dim 128 runs on tcgen05 (attn_tc.cuh); head_dim 64 on the mma.sync kernel (attn.cuh).
 cudaError_t attn_fwd_dispatch(const lsp_ctx* c, const AttnParams& p, cudaStream_t st) {
   if (c->d.head_dim == 128) {
@@ -353,18 +419,10 @@ lsp_status attn_fwd_impl(lsp_ctx* ctx, int x_dt, const void* x, const lsp_layer_
   float* o32 = at<float>(saved, ctx->sv.o32);
   __half* o16 = at<__half>(saved, ctx->sv.o16);
   float* lse = at<float>(saved, ctx->sv.lse);
-  __half* wqkv16 = at<__half>(saved, ctx->sv.wqkv16);
-  __half* wo16 = at<__half>(saved, ctx->sv.wo16);
-
-  {
-    const void* src[4] = {w->wq, w->wk, w->wv, w->wo};
-    __half* dst[4] = {wqkv16, wqkv16 + static_cast<long long>(Nq) * H, wqkv16 + static_cast<long long>(Nq + Nkv) * H, wo16};
-    const long long cnt[4] = {static_cast<long long>(Nq) * H, static_cast<long long>(Nkv) * H, static_cast<long long>(Nkv) * H,
-                              static_cast<long long>(H) * Nq};
-    // rope_layout = 1: the rows of Wq, Wk are interleaved per head, so that the adjacent-pair rotation of the QKV epilogue
-    // acts on the half-split pairs (i, i + d/2); q.k is invariant under the common permutation
-    LSP_STAGE(ST_CAST, 1, cast_weights(ctx, 4, src, dst, cnt, st, (d.use_rope && d.rope_layout == 1) ? 0x3u : 0u));
-  }
+  const W16 k16 = w16_of(ctx, w, saved);
+  __half* wqkv16 = k16.wqkv;
+  __half* wo16 = k16.wo;
+  if (!k16.cached) LSP_TRY(cast_attn_weights(ctx, w, k16, st));
   // F1 RMSNorm-1
   LSP_STAGE(ST_NORM_FWD, 1, norm_fwd(ctx, x_dt, x, w->g_attn, xn, rstd1, st));
   // F2 fused QKV projection with the RoPE epilogue (q, k rotated; v plain) into one [T, Nq+2Nkv] fp16 buffer
@@ -400,8 +458,9 @@ lsp_status attn_bwd_impl(lsp_ctx* ctx, int x_dt, const void* x, int da_dt, const
   const float* o32 = at<float>(saved, ctx->sv.o32);
   const __half* o16 = at<__half>(saved, ctx->sv.o16);
   const float* lse = at<float>(saved, ctx->sv.lse);
-  const __half* wqkv16 = at<__half>(saved, ctx->sv.wqkv16);
-  const __half* wo16 = at<__half>(saved, ctx->sv.wo16);
+  const W16 k16 = w16_of(ctx, w, saved);
+  const __half* wqkv16 = k16.wqkv;
+  const __half* wo16 = k16.wo;
   __half* dO16 = at<__half>(ws, ctx->ws.dO16);
   float* dvec = at<float>(ws, ctx->ws.dvec);
   __half* dqkv = at<__half>(ws, ctx->ws.dqkv16);
@@ -411,13 +470,16 @@ lsp_status attn_bwd_impl(lsp_ctx* ctx, int x_dt, const void* x, int da_dt, const
   // B6 dWo = da^T O ; dO = da Wo ; D = rowsum(dO * O32)
   LSP_STAGE(ST_WGRAD_O, 1, (gemm1<true, true>(ctx, H, Nq, T, Operand{da16, H, true}, Operand{o16, Nq, true},
                               epi_wgrad(ctx, g->wo, Nq), st)));
-  {
+  if (d.head_dim == 128) {
+    // the row sums D = rowsum(dO * O) leave the dgrad's epilogue as four partial sums per (head, position)
+    EpiDOutDvec e{dO16, Nq, o32, dvec, d.seq, d.n_q_heads};
+    LSP_STAGE(ST_DGRAD_O, 1, (gemm1<false, true>(ctx, T, Nq, H, Operand{da16, H, false}, Operand{wo16, Nq, true}, e, st)));
+  } else {
     EpiStore<DT_F16, DT_F32, false> e;
     e.out[0] = dO16; e.out[1] = e.out[2] = nullptr; e.split1 = e.split2 = 0x7fffffff; e.ld = Nq; e.res = nullptr; e.alpha = 1.0f;
     LSP_STAGE(ST_DGRAD_O, 1, (gemm1<false, true>(ctx, T, Nq, H, Operand{da16, H, false}, Operand{wo16, Nq, true}, e, st)));
+    LSP_STAGE(ST_DVEC, 1, (attn_dvec_launch<64, false>(dO16, Nq, o32, Nq, dvec, d.batch, d.seq, d.n_q_heads, st)));
   }
-  if (d.head_dim == 128) LSP_STAGE(ST_DVEC, 1, attn_dvec_launch<128>(dO16, Nq, o32, Nq, dvec, d.batch, d.seq, d.n_q_heads, st));
-  else LSP_STAGE(ST_DVEC, 1, attn_dvec_launch<64>(dO16, Nq, o32, Nq, dvec, d.batch, d.seq, d.n_q_heads, st));
   // B7 + B8 flash backward with the inverse rotation on store
   AttnParams p;
   memset(&p, 0, sizeof(p));
@@ -455,15 +517,11 @@ lsp_status mlp_fwd_impl(lsp_ctx* ctx, int a_dt, const void* a, const lsp_layer_w
   __half* g16 = at<__half>(saved, ctx->sv.g16);
   __half* u16 = at<__half>(saved, ctx->sv.u16);
   __half* h = at<__half>(saved, ctx->sv.h);
-  __half* wgu16 = at<__half>(saved, ctx->sv.wgu16);
-  __half* wd16 = at<__half>(saved, ctx->sv.wd16);
+  const W16 k16 = w16_of(ctx, w, saved);
+  __half* wgu16 = k16.wgu;
+  __half* wd16 = k16.wd;
   const long long FH = static_cast<long long>(F) * H;
-  {
-    const void* src[3] = {w->w_gate, w->w_up, w->w_down};
-    __half* dst[3] = {wgu16, wgu16 + FH, wd16};
-    const long long cnt[3] = {FH, FH, FH};
-    LSP_STAGE(ST_CAST, 1, cast_weights(ctx, 3, src, dst, cnt, st));
-  }
+  if (!k16.cached) LSP_TRY(cast_mlp_weights(ctx, w, k16, st));
   LSP_STAGE(ST_NORM_FWD, 1, norm_fwd(ctx, a_dt, a, w->g_mlp, an, rstd2, st));
   EpiSwiGLU e{h, g16, u16, F};
   e.save_gu = keep ? 1 : 0;
@@ -485,8 +543,9 @@ lsp_status mlp_bwd_impl(lsp_ctx* ctx, int a_dt, const void* a, int dy_dt, const 
   const __half* g16 = at<__half>(saved, ctx->sv.g16);
   const __half* u16 = at<__half>(saved, ctx->sv.u16);
   const __half* h = at<__half>(saved, ctx->sv.h);
-  const __half* wgu16 = at<__half>(saved, ctx->sv.wgu16);
-  const __half* wd16 = at<__half>(saved, ctx->sv.wd16);
+  const W16 k16 = w16_of(ctx, w, saved);
+  const __half* wgu16 = k16.wgu;
+  const __half* wd16 = k16.wd;
   __half* dgu = at<__half>(ws, ctx->ws.dgu);
   float* dan = at<float>(ws, ctx->ws.dn32);
   float* dgpart = at<float>(ws, ctx->ws.dgpart);
@@ -523,12 +582,17 @@ lsp_status check_common(lsp_ctx* ctx, const void* saved, const void* ws, int n, 
   return LSP_OK;
 }
 
+lsp_status check_cache(lsp_ctx* ctx, const lsp_layer_weights* w) {
+  if (w->f16_cache && !aligned(w->f16_cache, ALIGN)) return fail(ctx, LSP_EALIGN, "`f16_cache` must be 256-byte aligned");
+  return LSP_OK;
+}
+
 // fp16 operand copy of an activation-gradient input (bf16: exact for normal-range values; fp32: rounded), in ws.in16
 lsp_status as_f16(lsp_ctx* ctx, const void* in, void* ws, cudaStream_t st, const __half** out) {
   __half* t = at<__half>(ws, ctx->ws.in16);
   const long long n = static_cast<long long>(ctx->T) * ctx->d.hidden;
-  if (ctx->d.in_dtype == LSP_BF16) LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(in), t, n, ctx->num_sms, st));
-  else LSP_STAGE(ST_CAST, 1, cast_f32_f16(static_cast<const float*>(in), t, n, ctx->num_sms, st));
+  if (ctx->d.in_dtype == LSP_BF16) LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(in), t, n, ctx->num_sms, ctx->overflow, st));
+  else LSP_STAGE(ST_CAST, 1, cast_f32_f16(static_cast<const float*>(in), t, n, ctx->num_sms, ctx->overflow, st));
   *out = t;
   return LSP_OK;
 }
@@ -566,7 +630,8 @@ lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device
   ctx->G = d.n_q_heads / d.n_kv_heads;
 
   cudaDeviceProp prop;
-  if (cudaSetDevice(cuda_device) != cudaSuccess || cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) {
+  DeviceGuard guard(cuda_device);                 // the caller's current device is restored on every return path
+  if (!guard.ok || cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) {
     delete ctx;
     return LSP_ECUDA;
   }
@@ -601,9 +666,11 @@ lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device
         cudaMemset(ctx->sk_flags, 0, pairs * 2 * sizeof(unsigned int)) != cudaSuccess ||
         cudaMalloc(&ctx->opt_partial, OPT_MAX_CHUNKS * opt_blocks_cap(ctx->num_sms) * sizeof(float)) != cudaSuccess ||
         cudaMalloc(&ctx->attn_sched, 16 * sizeof(unsigned int)) != cudaSuccess ||
+        cudaMalloc(&ctx->overflow, sizeof(unsigned long long)) != cudaSuccess ||
+        cudaMemset(ctx->overflow, 0, sizeof(unsigned long long)) != cudaSuccess ||
         cudaMalloc(&ctx->doc_start, 2 * static_cast<size_t>(ctx->T) * sizeof(int)) != cudaSuccess ||
         cudaMemset(ctx->attn_sched, 0, 16 * sizeof(unsigned int)) != cudaSuccess) {
-      cudaFree(ctx->sk_partial); cudaFree(ctx->sk_flags); cudaFree(ctx->attn_sched); cudaFree(ctx->opt_partial); cudaFree(ctx->doc_start); cudaFree(ctx->rope); delete ctx;
+      cudaFree(ctx->sk_partial); cudaFree(ctx->sk_flags); cudaFree(ctx->attn_sched); cudaFree(ctx->overflow); cudaFree(ctx->opt_partial); cudaFree(ctx->doc_start); cudaFree(ctx->rope); delete ctx;
       return LSP_ENOMEM;
     }
   }
@@ -622,7 +689,9 @@ lsp_status lsp_create(lsp_ctx** out, const lsp_layer_desc* desc, int cuda_device
 
 lsp_status lsp_destroy(lsp_ctx* ctx) {
   if (!ctx) return LSP_EINVAL;
+  DeviceGuard guard(ctx->device);
   lsp_timing_enable(ctx, 0);
+  cudaFree(ctx->overflow);
   cudaFree(ctx->rope);
   cudaFree(ctx->sk_partial);
   cudaFree(ctx->sk_flags);
@@ -643,18 +712,63 @@ size_t lsp_saved_bytes(const lsp_ctx* ctx) { return ctx ? ctx->sv.total : 0; }
 size_t lsp_workspace_bytes(const lsp_ctx* ctx) { return ctx ? ctx->ws.total : 0; }
 const char* lsp_last_error(const lsp_ctx* ctx) { return ctx ? ctx->err : "lsp: NULL context"; }
 
+size_t lsp_weight_cache_bytes(const lsp_ctx* ctx) { return ctx ? ctx->wc.total : 0; }
+
+long long lsp_weight_cache_offset(const lsp_ctx* ctx, int which) {
+  if (!ctx || which < 0 || which > 6) return -1;
+  // the rows of Wq, Wk are permuted inside the cache when rope_layout = 1: only lsp_layer_prepare_weights can fill them
+  if (ctx->d.use_rope && ctx->d.rope_layout == 1 && which <= 1) return -1;
+  const long long H = ctx->d.hidden, Nq = ctx->Nq, Nkv = ctx->Nkv, F = ctx->d.ffn;
+  switch (which) {
+    case 0: return static_cast<long long>(ctx->wc.wqkv16);
+    case 1: return static_cast<long long>(ctx->wc.wqkv16) + Nq * H * 2;
+    case 2: return static_cast<long long>(ctx->wc.wqkv16) + (Nq + Nkv) * H * 2;
+    case 3: return static_cast<long long>(ctx->wc.wo16);
+    case 4: return static_cast<long long>(ctx->wc.wgu16);
+    case 5: return static_cast<long long>(ctx->wc.wgu16) + F * H * 2;
+    default: return static_cast<long long>(ctx->wc.wd16);
+  }
+}
+
+lsp_status lsp_layer_prepare_weights(lsp_ctx* ctx, const lsp_layer_weights* w, void* cache, void* stream) {
+  if (!ctx || !w) return LSP_EINVAL;
+  LSP_ENTER(ctx);
+  const void* ptrs[] = {cache, w->wq, w->wk, w->wv, w->wo, w->w_gate, w->w_up, w->w_down};
+  LSP_TRY(check_common(ctx, cache, nullptr, 8, ptrs));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  lsp_layer_weights wc = *w;
+  wc.f16_cache = cache;
+  const W16 k = w16_of(ctx, &wc, nullptr);
+  LSP_TRY(cast_attn_weights(ctx, w, k, st));
+  return cast_mlp_weights(ctx, w, k, st);
+}
+
+lsp_status lsp_overflow_count(lsp_ctx* ctx, unsigned long long* count, int reset, void* stream) {
+  if (!ctx || !count) return LSP_EINVAL;
+  LSP_ENTER(ctx);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  LSP_CUDA(cudaMemcpyAsync(count, ctx->overflow, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+  LSP_CUDA(cudaStreamSynchronize(st));
+  if (reset) LSP_CUDA(cudaMemsetAsync(ctx->overflow, 0, sizeof(unsigned long long), st));
+  return LSP_OK;
+}
+
 lsp_status lsp_attn_fwd(lsp_ctx* ctx, const void* x, const lsp_layer_weights* w, void* a_out, void* saved, void* ws, void* stream) {
   if (!ctx || !w) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   const void* ptrs[] = {x, a_out, saved, ws, w->wq, w->wk, w->wv, w->wo, w->g_attn};
   LSP_TRY(check_common(ctx, saved, ws, 9, ptrs));
+  LSP_TRY(check_cache(ctx, w));
   return attn_fwd_impl(ctx, ctx->d.in_dtype, x, w, static_cast<float*>(a_out), saved, static_cast<cudaStream_t>(stream));
 }
 
 lsp_status lsp_attn_bwd(lsp_ctx* ctx, const void* x, const void* da, const lsp_layer_weights* w, const void* saved, void* dx,
                         lsp_layer_wgrads* g, void* ws, void* stream) {
   if (!ctx || !w || !g) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   const void* ptrs[] = {x, da, saved, dx, ws, w->wq, w->wk, w->wv, w->wo, w->g_attn, g->wq, g->wk, g->wv, g->wo, g->g_attn};
   LSP_TRY(check_common(ctx, saved, ws, 15, ptrs));
+  LSP_TRY(check_cache(ctx, w));
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const __half* da16;
   LSP_TRY(as_f16(ctx, da, ws, st, &da16));
@@ -663,16 +777,20 @@ lsp_status lsp_attn_bwd(lsp_ctx* ctx, const void* x, const void* da, const lsp_l
 
 lsp_status lsp_mlp_fwd(lsp_ctx* ctx, const void* a, const lsp_layer_weights* w, void* y_out, void* saved, void* ws, void* stream) {
   if (!ctx || !w) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   const void* ptrs[] = {a, y_out, saved, ws, w->w_gate, w->w_up, w->w_down, w->g_mlp};
   LSP_TRY(check_common(ctx, saved, ws, 8, ptrs));
+  LSP_TRY(check_cache(ctx, w));
   return mlp_fwd_impl(ctx, ctx->d.in_dtype, a, w, static_cast<float*>(y_out), saved, static_cast<cudaStream_t>(stream));
 }
 
 lsp_status lsp_mlp_bwd(lsp_ctx* ctx, const void* a, const void* dy, const lsp_layer_weights* w, const void* saved, void* da,
                        lsp_layer_wgrads* g, void* ws, void* stream) {
   if (!ctx || !w || !g) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   const void* ptrs[] = {a, dy, saved, da, ws, w->w_gate, w->w_up, w->w_down, w->g_mlp, g->w_gate, g->w_up, g->w_down, g->g_mlp};
   LSP_TRY(check_common(ctx, saved, ws, 13, ptrs));
+  LSP_TRY(check_cache(ctx, w));
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const __half* dy16;
   LSP_TRY(as_f16(ctx, dy, ws, st, &dy16));
@@ -681,8 +799,10 @@ lsp_status lsp_mlp_bwd(lsp_ctx* ctx, const void* a, const void* dy, const lsp_la
 
 lsp_status lsp_layer_fwd(lsp_ctx* ctx, const void* x, const lsp_layer_weights* w, void* y_out, void* saved, void* ws, void* stream) {
   if (!ctx || !w) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   const void* ptrs[] = {x, y_out, saved, ws, w->wq, w->wk, w->wv, w->wo, w->g_attn, w->w_gate, w->w_up, w->w_down, w->g_mlp};
   LSP_TRY(check_common(ctx, saved, ws, 13, ptrs));
+  LSP_TRY(check_cache(ctx, w));
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   float* a32 = at<float>(saved, ctx->sv.a32);
   LSP_TRY(attn_fwd_impl(ctx, ctx->d.in_dtype, x, w, a32, saved, st));
@@ -692,8 +812,10 @@ lsp_status lsp_layer_fwd(lsp_ctx* ctx, const void* x, const lsp_layer_weights* w
 lsp_status lsp_layer_fwd_infer(lsp_ctx* ctx, const void* x, const lsp_layer_weights* w, void* y_out, void* scratch, void* ws,
                                void* stream) {
   if (!ctx || !w) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   const void* ptrs[] = {x, y_out, scratch, ws, w->wq, w->wk, w->wv, w->wo, w->g_attn, w->w_gate, w->w_up, w->w_down, w->g_mlp};
   LSP_TRY(check_common(ctx, scratch, ws, 13, ptrs));
+  LSP_TRY(check_cache(ctx, w));
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   float* a32 = at<float>(scratch, ctx->sv.a32);
   LSP_TRY(attn_fwd_impl(ctx, ctx->d.in_dtype, x, w, a32, scratch, st, false));
@@ -703,9 +825,11 @@ lsp_status lsp_layer_fwd_infer(lsp_ctx* ctx, const void* x, const lsp_layer_weig
 lsp_status lsp_layer_bwd(lsp_ctx* ctx, const void* x, const void* dy, const lsp_layer_weights* w, const void* saved, void* dx,
                          lsp_layer_wgrads* g, void* ws, void* stream) {
   if (!ctx || !w || !g) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   const void* ptrs[] = {x, dy, saved, dx, ws, w->wq, w->wk, w->wv, w->wo, w->g_attn, w->w_gate, w->w_up, w->w_down, w->g_mlp,
                         g->wq, g->wk, g->wv, g->wo, g->g_attn, g->w_gate, g->w_up, g->w_down, g->g_mlp};
   LSP_TRY(check_common(ctx, saved, ws, 23, ptrs));
+  LSP_TRY(check_cache(ctx, w));
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const __half* dy16;
   LSP_TRY(as_f16(ctx, dy, ws, st, &dy16));
@@ -718,6 +842,7 @@ lsp_status lsp_layer_bwd(lsp_ctx* ctx, const void* x, const void* dy, const lsp_
 
 lsp_status lsp_sdpa_fwd(lsp_ctx* ctx, const void* q, const void* k, const void* v, void* o, float* lse, void* ws, void* stream) {
   if (!ctx) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   const void* ptrs[] = {q, k, v, o, lse, ws};
   LSP_TRY(check_common(ctx, nullptr, ws, 6, ptrs));
   cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -726,9 +851,9 @@ lsp_status lsp_sdpa_fwd(lsp_ctx* ctx, const void* q, const void* k, const void* 
   __half* q16 = at<__half>(ws, ctx->ws.q16);
   __half* k16 = at<__half>(ws, ctx->ws.k16);
   __half* v16 = at<__half>(ws, ctx->ws.v16);
-  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(q), q16, T * ctx->Nq, ctx->num_sms, st));
-  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(k), k16, T * ctx->Nkv, ctx->num_sms, st));
-  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(v), v16, T * ctx->Nkv, ctx->num_sms, st));
+  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(q), q16, T * ctx->Nq, ctx->num_sms, ctx->overflow, st));
+  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(k), k16, T * ctx->Nkv, ctx->num_sms, ctx->overflow, st));
+  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(v), v16, T * ctx->Nkv, ctx->num_sms, ctx->overflow, st));
   AttnParams p;
   memset(&p, 0, sizeof(p));
   p.q = q16; p.k = k16; p.v = v16;
@@ -744,6 +869,7 @@ lsp_status lsp_sdpa_fwd(lsp_ctx* ctx, const void* q, const void* k, const void* 
 lsp_status lsp_sdpa_bwd(lsp_ctx* ctx, const void* q, const void* k, const void* v, const void* o, const float* lse,
                         const void* d_o, void* dq, void* dk, void* dv, void* ws, void* stream) {
   if (!ctx) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   const void* ptrs[] = {q, k, v, o, lse, d_o, dq, dk, dv, ws};
   LSP_TRY(check_common(ctx, nullptr, ws, 10, ptrs));
   cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -754,12 +880,12 @@ lsp_status lsp_sdpa_bwd(lsp_ctx* ctx, const void* q, const void* k, const void* 
   __half* v16 = at<__half>(ws, ctx->ws.v16);
   __half* dO16 = at<__half>(ws, ctx->ws.dO16);
   float* dvec = at<float>(ws, ctx->ws.dvec);
-  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(q), q16, T * ctx->Nq, ctx->num_sms, st));
-  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(k), k16, T * ctx->Nkv, ctx->num_sms, st));
-  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(v), v16, T * ctx->Nkv, ctx->num_sms, st));
-  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(d_o), dO16, T * ctx->Nq, ctx->num_sms, st));
-  if (d.head_dim == 128) LSP_STAGE(ST_DVEC, 1, attn_dvec_launch<128>(dO16, ctx->Nq, static_cast<const float*>(o), ctx->Nq, dvec, d.batch, d.seq, d.n_q_heads, st));
-  else LSP_STAGE(ST_DVEC, 1, attn_dvec_launch<64>(dO16, ctx->Nq, static_cast<const float*>(o), ctx->Nq, dvec, d.batch, d.seq, d.n_q_heads, st));
+  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(q), q16, T * ctx->Nq, ctx->num_sms, ctx->overflow, st));
+  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(k), k16, T * ctx->Nkv, ctx->num_sms, ctx->overflow, st));
+  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(v), v16, T * ctx->Nkv, ctx->num_sms, ctx->overflow, st));
+  LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(d_o), dO16, T * ctx->Nq, ctx->num_sms, ctx->overflow, st));
+  if (d.head_dim == 128) LSP_STAGE(ST_DVEC, 1, (attn_dvec_launch<128, true>(dO16, ctx->Nq, static_cast<const float*>(o), ctx->Nq, dvec, d.batch, d.seq, d.n_q_heads, st)));
+  else LSP_STAGE(ST_DVEC, 1, (attn_dvec_launch<64, false>(dO16, ctx->Nq, static_cast<const float*>(o), ctx->Nq, dvec, d.batch, d.seq, d.n_q_heads, st)));
   AttnParams p;
   memset(&p, 0, sizeof(p));
   p.q = q16; p.k = k16; p.v = v16; p.dO = dO16;
@@ -776,6 +902,7 @@ lsp_status lsp_sdpa_bwd(lsp_ctx* ctx, const void* q, const void* k, const void* 
 
 lsp_status lsp_embed_fwd(lsp_ctx* ctx, const int32_t* ids, const void* table, void* x0, void* stream) {
   if (!ctx) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   const void* ptrs[] = {ids, table, x0};
   LSP_TRY(check_common(ctx, nullptr, nullptr, 3, ptrs));
   cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -790,6 +917,7 @@ lsp_status lsp_embed_fwd(lsp_ctx* ctx, const int32_t* ids, const void* table, vo
 lsp_status lsp_gemm(lsp_ctx* ctx, int op, int M, int N, int K, const void* A, int64_t lda, int a_dtype, const void* B,
                     int64_t ldb, int b_dtype, float* C, int64_t ldc, void* stream) {
   if (!ctx) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   const void* ptrs[] = {A, B, C};
   LSP_TRY(check_common(ctx, nullptr, nullptr, 3, ptrs));
   if (M <= 0 || N <= 0 || K <= 0 || (lda % 8) || (ldb % 8) || (ldc % 8) || (N % 8)) return fail(ctx, LSP_EINVAL, "lsp_gemm: bad extents/pitches");
@@ -813,6 +941,7 @@ lsp_status lsp_layer_step_host(lsp_ctx* ctx, const void* x_host, const void* dy_
                                void* y_host, void* dx_host, lsp_layer_wgrads* g, void* x_dev, void* dy_dev, void* y_dev,
                                void* dx_dev, void* saved, void* ws, void* stream) {
   if (!ctx || !x_host || !dy_host || !y_host || !dx_host || !x_dev || !dy_dev || !y_dev || !dx_dev) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const size_t n = static_cast<size_t>(ctx->T) * ctx->d.hidden;
   const size_t in_bytes = n * (ctx->d.in_dtype == LSP_F32 ? 4 : 2);
@@ -849,6 +978,7 @@ lsp_status lsp_layer_step_host_async(lsp_ctx* ctx, const void* x_host, const voi
                                      void* y_host, void* dx_host, lsp_layer_wgrads* g, void* x_dev, void* dy_dev, void* y_dev,
                                      void* dx_dev, void* saved, void* ws, void* stream) {
   if (!ctx || !x_host || !dy_host || !y_host || !dx_host || !x_dev || !dy_dev || !y_dev || !dx_dev) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const size_t n = static_cast<size_t>(ctx->T) * ctx->d.hidden;
   const size_t in_bytes = n * (ctx->d.in_dtype == LSP_F32 ? 4 : 2);
@@ -871,6 +1001,9 @@ lsp_status lsp_layer_step_host_async(lsp_ctx* ctx, const void* x_host, const voi
   // forward
   LSP_CUDA(cudaStreamWaitEvent(st, e[E_X], 0));
   if (!first && y_dev == ctx->prev_y_dev) LSP_CUDA(cudaStreamWaitEvent(st, eq[E_Y], 0));
+  // alternating result buffers: this y_dev was downloaded by the call two steps ago (same parity: e[E_Y] still holds that
+  // record; it is re-recorded below, after this wait has been enqueued)
+  if (ctx->host_seq >= 2) LSP_CUDA(cudaStreamWaitEvent(st, e[E_Y], 0));
   LSP_TRY(lsp_layer_fwd(ctx, x_dev, w, y_dev, saved, ws, stream));
   LSP_CUDA(cudaEventRecord(e[E_FWD], st));
   LSP_CUDA(cudaStreamWaitEvent(ctx->s_out, e[E_FWD], 0));
@@ -879,6 +1012,7 @@ lsp_status lsp_layer_step_host_async(lsp_ctx* ctx, const void* x_host, const voi
   // backward
   LSP_CUDA(cudaStreamWaitEvent(st, e[E_DY], 0));
   if (!first && dx_dev == ctx->prev_dx_dev) LSP_CUDA(cudaStreamWaitEvent(st, eq[E_DX], 0));
+  if (ctx->host_seq >= 2) LSP_CUDA(cudaStreamWaitEvent(st, e[E_DX], 0));
   LSP_TRY(lsp_layer_bwd(ctx, x_dev, dy_dev, w, saved, dx_dev, g, ws, stream));
   LSP_CUDA(cudaEventRecord(e[E_BWD], st));
   LSP_CUDA(cudaStreamWaitEvent(ctx->s_out, e[E_BWD], 0));
@@ -892,6 +1026,7 @@ lsp_status lsp_layer_step_host_async(lsp_ctx* ctx, const void* x_host, const voi
 // `stream` waits for every copy the async host steps have issued, and the pipeline restarts (next call is a "first").
 lsp_status lsp_host_copies_wait(lsp_ctx* ctx, void* stream) {
   if (!ctx) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   if (ctx->host_seq > 0) {
     LSP_CUDA(cudaEventRecord(ctx->ev[5], ctx->s_out));
@@ -905,7 +1040,7 @@ lsp_status lsp_host_copies_wait(lsp_ctx* ctx, void* stream) {
 }
 
 namespace {
-struct HeadLayout { size_t xn16, rstd, w16, logits, dz16, dxn32, loss_row, dgpart, total; };
+struct HeadLayout { size_t xn16, rstd, w16, logits, dz16, dxn32, loss_row, dgpart, inv_count, total; };
 HeadLayout head_layout(const lsp_ctx* c, int vocab) {
   const size_t T = c->T, H = c->d.hidden, V = vocab;
   size_t o = 0;
@@ -914,6 +1049,7 @@ HeadLayout head_layout(const lsp_ctx* c, int vocab) {
   h.xn16 = take(T * H * 2); h.rstd = take(T * 4); h.w16 = take(V * H * 2); h.logits = take(T * V * 4);
   h.dz16 = take(T * V * 2); h.dxn32 = take(T * H * 4); h.loss_row = take(T * 4);
   h.dgpart = take(static_cast<size_t>(c->norm_blocks) * 2 * H * 4);
+  h.inv_count = take(4);
   h.total = o;
   return h;
 }
@@ -925,6 +1061,7 @@ lsp_status lsp_head_fwd_bwd(lsp_ctx* ctx, const void* x, const void* g_final, co
                             int32_t vocab, float grad_scale, float* loss, float* lse, void* dx, float* dg_final, float* dw_head,
                             void* ws, void* stream) {
   if (!ctx) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   const void* ptrs[] = {x, g_final, w_head, targets, loss, lse, dx, dg_final, dw_head, ws};
   LSP_TRY(check_common(ctx, nullptr, ws, 10, ptrs));
   if (vocab <= 0 || vocab % 8) return fail(ctx, LSP_EINVAL, "lsp_head_fwd_bwd: vocab must be a positive multiple of 8");
@@ -940,6 +1077,7 @@ lsp_status lsp_head_fwd_bwd(lsp_ctx* ctx, const void* x, const void* g_final, co
   float* dxn32 = at<float>(ws, L.dxn32);
   float* loss_row = at<float>(ws, L.loss_row);
   float* dgpart = at<float>(ws, L.dgpart);
+  float* inv_count = at<float>(ws, L.inv_count);
   // final RMSNorm, fp16 copy of the head weights
   LSP_STAGE(ST_NORM_FWD, 1, norm_fwd(ctx, ctx->d.in_dtype, x, g_final, xn16, rstd, st));
   {
@@ -955,22 +1093,23 @@ lsp_status lsp_head_fwd_bwd(lsp_ctx* ctx, const void* x, const void* g_final, co
     int blocks = 2 * ctx->num_sms < T ? 2 * ctx->num_sms : T;      // two CTAs of 512 threads per SM: one row reduces while the other streams
     auto launch = [&]() {
       ce_fwd_bwd_kernel<<<blocks, CE_THREADS, 0, st>>>(logits, targets, T, V, lse, loss_row, dz16);
-      ce_loss_mean_kernel<<<1, 32, 0, st>>>(loss_row, T, loss);
+      ce_loss_mean_kernel<<<1, 32, 0, st>>>(loss_row, targets, T, V, loss, inv_count);
       return cudaGetLastError();
     };
     LSP_STAGE(ST_CE, 2, launch());
   }
-  // undo the fp16 scaling of dz, apply the 1/T of the mean and the caller's gradient (loss) scale
+  // undo the fp16 scaling of dz, apply the 1/T of the mean and the caller's gradient (loss) scale; the device scalar
+  // inv_count = T / (number of counted targets) turns 1/T into the mean over the counted tokens (exactly 1 if all count)
   const float alpha = grad_scale / (CE_DZ_SCALE * static_cast<float>(T));
   // dW_head = dz^T xn ; dxn = dz W_head
   {
     EpiF32 e = epi_wgrad(ctx, dw_head, H);
-    e.alpha = alpha;
+    e.alpha = alpha; e.alpha_dev = inv_count;
     LSP_STAGE(ST_HEAD_GEMM, 1, (gemm1<true, true>(ctx, V, H, T, Operand{dz16, V, true}, Operand{xn16, H, true}, e, st)));
   }
   {
     EpiF32 e = epi_f32(dxn32, H);
-    e.alpha = alpha;
+    e.alpha = alpha; e.alpha_dev = inv_count;
     LSP_STAGE(ST_HEAD_GEMM, 1, (gemm1<false, true>(ctx, T, H, V, Operand{dz16, V, false}, Operand{w16, H, true}, e, st)));
   }
   // final RMSNorm backward (no residual gradient)
@@ -981,6 +1120,7 @@ lsp_status lsp_head_fwd_bwd(lsp_ctx* ctx, const void* x, const void* g_final, co
 
 lsp_status lsp_embed_bwd(lsp_ctx* ctx, const int32_t* ids, const void* dx0, int32_t vocab, float* d_table, void* stream) {
   if (!ctx) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   const void* ptrs[] = {ids, dx0, d_table};
   LSP_TRY(check_common(ctx, nullptr, nullptr, 3, ptrs));
   if (vocab <= 0) return fail(ctx, LSP_EINVAL, "lsp_embed_bwd: vocab must be positive");
@@ -999,6 +1139,7 @@ lsp_status lsp_embed_bwd(lsp_ctx* ctx, const int32_t* ids, const void* dx0, int3
 lsp_status lsp_adamw_step(lsp_ctx* ctx, int ntensors, const lsp_adamw_tensor* tensors, const lsp_adamw_desc* desc,
                           float* gnorm_out, void* stream) {
   if (!ctx || !tensors || !desc || !gnorm_out) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   if (ntensors < 1 || ntensors > OPT_MAX_TENSORS * OPT_MAX_CHUNKS)
     return fail(ctx, LSP_EINVAL, "lsp_adamw_step: 1 <= ntensors <= %d", OPT_MAX_TENSORS * OPT_MAX_CHUNKS);
   if (desc->step < 1 || !(desc->beta1 >= 0.f && desc->beta1 < 1.f) || !(desc->beta2 >= 0.f && desc->beta2 < 1.f) || !(desc->clip_norm > 0.f) ||
@@ -1007,7 +1148,8 @@ lsp_status lsp_adamw_step(lsp_ctx* ctx, int ntensors, const lsp_adamw_tensor* te
   for (int i = 0; i < ntensors; ++i) {
     const lsp_adamw_tensor& x = tensors[i];
     if (!x.grad || !x.master || !x.m || !x.v || x.n <= 0 || (x.n % 4)) return fail(ctx, LSP_EINVAL, "lsp_adamw_step: tensor %d: NULL pointer or n %% 4 != 0", i);
-    if (!aligned(x.grad, 16) || !aligned(x.master, 16) || !aligned(x.m, 16) || !aligned(x.v, 16) || (x.weight_bf16 && !aligned(x.weight_bf16, 8)))
+    if (!aligned(x.grad, 16) || !aligned(x.master, 16) || !aligned(x.m, 16) || !aligned(x.v, 16) || (x.weight_bf16 && !aligned(x.weight_bf16, 8)) ||
+        (x.weight_f16 && !aligned(x.weight_f16, 8)))
       return fail(ctx, LSP_EALIGN, "lsp_adamw_step: tensor %d is not 16-byte aligned", i);
   }
   OptHyper h;
@@ -1027,6 +1169,7 @@ lsp_status lsp_adamw_step(lsp_ctx* ctx, int ntensors, const lsp_adamw_tensor* te
       const lsp_adamw_tensor& x = tensors[i0 + i];
       t.g[i] = static_cast<const float*>(x.grad); t.p[i] = x.master; t.m[i] = x.m; t.v[i] = x.v;
       t.w[i] = static_cast<__nv_bfloat16*>(x.weight_bf16);
+      t.w16[i] = static_cast<__half*>(x.weight_f16);
       t.start[i + 1] = t.start[i] + x.n / 4;
       if (x.decay) t.decay_mask |= 1u << i;
     }
@@ -1069,6 +1212,7 @@ double lsp_lr_cosine(int step, double lr_max, double lr_min, int warmup, int tot
 
 lsp_status lsp_set_packed_sequences(lsp_ctx* ctx, const int32_t* cu_seqlens_host, int32_t n_seqs, void* stream) {
   if (!ctx) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   if (n_seqs == 0) { ctx->doc_on = 0; return LSP_OK; }
   if (!cu_seqlens_host || n_seqs < 0) return LSP_EINVAL;
   if (ctx->d.batch != 1 || ctx->d.head_dim != 128)
@@ -1092,6 +1236,7 @@ long long lsp_launch_count(const lsp_ctx* ctx) { return ctx ? ctx->launches : -1
 
 lsp_status lsp_timing_enable(lsp_ctx* ctx, int max_records) {
   if (!ctx || max_records < 0) return LSP_EINVAL;
+  LSP_ENTER(ctx);
   if (ctx->recs) {
     for (TimingRec& r : *ctx->recs) { cudaEventDestroy(r.beg); cudaEventDestroy(r.end); }
     delete ctx->recs;

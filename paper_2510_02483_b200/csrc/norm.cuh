@@ -117,7 +117,8 @@ template <typename XT, typename RT, int NV, int G>
 __global__ void __launch_bounds__(NORMB_THREADS, 1)
 rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, const __nv_bfloat16* __restrict__ g,
                    const float* __restrict__ dxn, const RT* __restrict__ dres, float* __restrict__ dx,
-                   __half* __restrict__ dx16, float* __restrict__ dg_part, int T, int H, int stages, float res_scale) {
+                   __half* __restrict__ dx16, float* __restrict__ dg_part, int T, int H, int stages, float res_scale,
+                   unsigned long long* __restrict__ counter) {
   // G row groups of GT = 256 / G consumer threads: group q takes this CTA's rows q, q + G, ... so that the reduction
   // latency of one row (shuffles, two named barriers) overlaps the loads and stores of the other group's row.
   constexpr int GT = NORMB_CONSUMERS / G;
@@ -164,6 +165,7 @@ rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, con
     gg[i] = (c < H) ? Vec4<__nv_bfloat16>::load(g + c) : make_float4(0.f, 0.f, 0.f, 0.f);
   }
   const float invH = 1.0f / static_cast<float>(H);
+  unsigned int bad = 0;
   long long k = grp;                                          // index of the row among this CTA's rows
   for (long long row = blockIdx.x + static_cast<long long>(grp) * gridDim.x; row < T; row += static_cast<long long>(G) * gridDim.x, k += G) {
     const int s = static_cast<int>(k % stages);
@@ -201,10 +203,12 @@ rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, con
         o.z = fmaf(res_scale, rs[i].z, r * (dn[i].z - n[i].z * dot));
         o.w = fmaf(res_scale, rs[i].w, r * (dn[i].w - n[i].w * dot));
         *reinterpret_cast<float4*>(dx + row * H + c) = o;
-        if (dx16) store_f16x4(dx16 + row * H + c, o);
+        if (dx16)      // the fp16 operand copy of this gradient: saturating and counted like the input casts (pack_f16_sat)
+          *reinterpret_cast<uint2*>(dx16 + row * H + c) = make_uint2(pack_f16_sat(o.x, o.y, bad), pack_f16_sat(o.z, o.w, bad));
       }
     }
   }
+  cast_report(bad, counter);
   // one row of dg partials per (CTA, group)
 #pragma unroll
   for (int i = 0; i < NV; ++i) {
@@ -233,18 +237,28 @@ __global__ void __launch_bounds__(256) colsum_kernel(const float* __restrict__ p
 }
 
 // 8 elements per thread casts (n is a multiple of 8)
-__global__ void cast_f32_f16_kernel(const float* __restrict__ in, __half* __restrict__ out, long long n8) {
+// fp16 operand copies of caller tensors (P-2'): fp16 has bf16's tensor-core rate and three more
+// mantissa bits, but a narrower exponent -- |v| > 65504 would become inf and poison every sum it enters.  The casts
+// therefore SATURATE to +-65504 (NaN stays NaN) and COUNT the values they had to clamp or found non-finite in a
+// context-owned device counter (lsp_overflow_count): out-of-range input is reported, never silent.  Values below 2^-24
+// flush to zero (an absolute error far under the parity bar).
+__global__ void cast_f32_f16_kernel(const float* __restrict__ in, __half* __restrict__ out, long long n8, unsigned long long* counter) {
+  unsigned int bad = 0;
   for (long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i < n8; i += static_cast<long long>(gridDim.x) * blockDim.x) {
     const float4 a = __ldg(reinterpret_cast<const float4*>(in) + 2 * i), b = __ldg(reinterpret_cast<const float4*>(in) + 2 * i + 1);
-    reinterpret_cast<uint4*>(out)[i] = make_uint4(pack_f16(a.x, a.y), pack_f16(a.z, a.w), pack_f16(b.x, b.y), pack_f16(b.z, b.w));
+    reinterpret_cast<uint4*>(out)[i] = make_uint4(pack_f16_sat(a.x, a.y, bad), pack_f16_sat(a.z, a.w, bad), pack_f16_sat(b.x, b.y, bad),
+                                                  pack_f16_sat(b.z, b.w, bad));
   }
+  cast_report(bad, counter);
 }
-__global__ void cast_bf16_f16_kernel(const __nv_bfloat16* __restrict__ in, __half* __restrict__ out, long long n8) {
+__global__ void cast_bf16_f16_kernel(const __nv_bfloat16* __restrict__ in, __half* __restrict__ out, long long n8, unsigned long long* counter) {
+  unsigned int bad = 0;
   for (long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i < n8; i += static_cast<long long>(gridDim.x) * blockDim.x) {
     const uint4 u = __ldg(reinterpret_cast<const uint4*>(in) + i);
-    reinterpret_cast<uint4*>(out)[i] = make_uint4(pack_f16(bf16_lo(u.x), bf16_hi(u.x)), pack_f16(bf16_lo(u.y), bf16_hi(u.y)),
-                                                  pack_f16(bf16_lo(u.z), bf16_hi(u.z)), pack_f16(bf16_lo(u.w), bf16_hi(u.w)));
+    reinterpret_cast<uint4*>(out)[i] = make_uint4(pack_f16_sat(bf16_lo(u.x), bf16_hi(u.x), bad), pack_f16_sat(bf16_lo(u.y), bf16_hi(u.y), bad),
+                                                  pack_f16_sat(bf16_lo(u.z), bf16_hi(u.z), bad), pack_f16_sat(bf16_lo(u.w), bf16_hi(u.w), bad));
   }
+  cast_report(bad, counter);
 }
 
 // Several bf16 -> fp16 casts in one launch (the weight tensors of a block): segment s covers 8-element groups
@@ -257,6 +271,7 @@ struct CastSegs {
   int nseg;
   unsigned perm_mask;        // segments whose ROWS are permuted on the way: dst row head*d + 2i + half = src row head*d + half*d/2 + i
   int perm_d, row_units;     // head_dim; 16-byte units per row (in-features / 8)
+  unsigned long long* counter;   // clamped / non-finite values (see pack_f16_sat); may be null
 };
 __device__ __forceinline__ long long cast_src_unit(const CastSegs& segs, long long i, int& s) {
   s = 0;
@@ -274,6 +289,7 @@ __device__ __forceinline__ long long cast_src_unit(const CastSegs& segs, long lo
 __global__ void __launch_bounds__(256) cast_multi_bf16_f16_kernel(const CastSegs segs) {
   const long long total = segs.start[segs.nseg];
   const long long stride = static_cast<long long>(gridDim.x) * blockDim.x;
+  unsigned int bad = 0;
   for (long long i0 = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i0 < total; i0 += 4 * stride) {
     uint4 u[4];
     int sg[4];
@@ -291,10 +307,11 @@ __global__ void __launch_bounds__(256) cast_multi_bf16_f16_kernel(const CastSegs
       const long long i = i0 + k * stride;
       if (i < total)
         reinterpret_cast<uint4*>(segs.dst[sg[k]])[i - segs.start[sg[k]]] =
-            make_uint4(pack_f16(bf16_lo(u[k].x), bf16_hi(u[k].x)), pack_f16(bf16_lo(u[k].y), bf16_hi(u[k].y)),
-                       pack_f16(bf16_lo(u[k].z), bf16_hi(u[k].z)), pack_f16(bf16_lo(u[k].w), bf16_hi(u[k].w)));
+            make_uint4(pack_f16_sat(bf16_lo(u[k].x), bf16_hi(u[k].x), bad), pack_f16_sat(bf16_lo(u[k].y), bf16_hi(u[k].y), bad),
+                       pack_f16_sat(bf16_lo(u[k].z), bf16_hi(u[k].z), bad), pack_f16_sat(bf16_lo(u[k].w), bf16_hi(u[k].w), bad));
     }
   }
+  cast_report(bad, segs.counter);
 }
 
 // x0[t,:] = E[id_t,:]  (bf16 table row -> fp32 or bf16 stream).  One block per token.

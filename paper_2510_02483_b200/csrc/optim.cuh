@@ -19,6 +19,7 @@ struct OptTensors {
   float* m[OPT_MAX_TENSORS];
   float* v[OPT_MAX_TENSORS];
   __nv_bfloat16* w[OPT_MAX_TENSORS];
+  __half* w16[OPT_MAX_TENSORS];              // optional fp16 operand copy of the new bf16 weight (lsp_adamw_tensor.weight_f16)
   long long start[OPT_MAX_TENSORS + 1];      // prefix sums of the tensor sizes in float4 units
   unsigned int decay_mask;                   // bit i: weight decay applies to tensor i
   int n;
@@ -60,7 +61,10 @@ __global__ void __launch_bounds__(OPT_THREADS) opt_gradsq_kernel(const OptTensor
 // raw_sum: out[0] = sum of the partials (nothing else).  Otherwise:
 // out[0] = global l2 norm of the true gradients g / grad_scale, out[1] = the factor the update applies to the stored
 // gradients = min(1, clip / (norm + 1e-6)) / grad_scale; one block, fp64, fixed order: thread i sums the
-// partials i, i + 256, ... in that order, then thread 0 adds the 256 thread sums in index order
+// partials i, i + 256, ... in that order, then thread 0 adds the 256 thread sums in index order.
+// A non-finite norm (an inf / NaN gradient: e.g. an fp16 operand overflow upstream) makes the step a NO-OP: out[0]
+// carries the non-finite norm as the flag, out[1] = 0, and opt_adamw_kernel leaves p, m, v and the weights untouched
+// (without this, c = clip / inf = 0 and g * c = inf * 0 = NaN would be written into the state for good).
 __global__ void __launch_bounds__(OPT_THREADS) opt_norm_final_kernel(const float* __restrict__ partial, int nparts, float clip,
                                                                      double inv_scale, int raw_sum, float* __restrict__ out) {
   __shared__ double red[OPT_THREADS];
@@ -74,6 +78,7 @@ __global__ void __launch_bounds__(OPT_THREADS) opt_norm_final_kernel(const float
     if (raw_sum) { out[0] = static_cast<float>(tot); return; }      // phase 1 of a sharded step: this rank's sum of g^2
     const double norm = sqrt(tot) * inv_scale;
     out[0] = static_cast<float>(norm);
+    if (!isfinite(norm) || !isfinite(static_cast<float>(norm))) { out[1] = 0.f; return; }      // skip-step flag
     const double c = static_cast<double>(clip) / (norm + 1e-6);
     out[1] = static_cast<float>((c < 1.0 ? c : 1.0) * inv_scale);
   }
@@ -84,6 +89,7 @@ __global__ void __launch_bounds__(OPT_THREADS) opt_norm_final_kernel(const float
 __global__ void __launch_bounds__(OPT_THREADS) opt_adamw_kernel(const OptTensors t, const OptHyper h, const float* __restrict__ norm_coef) {
   const long long total = t.start[t.n];
   const float c = norm_coef[1];
+  if (!(c > 0.f)) return;                    // non-finite gradient norm: skipped step (see opt_norm_final_kernel)
   const long long stride = static_cast<long long>(gridDim.x) * blockDim.x;
   for (long long i0 = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i0 < total; i0 += 2 * stride) {
     float4 g4[2], p4[2], m4[2], v4[2];
@@ -121,7 +127,10 @@ __global__ void __launch_bounds__(OPT_THREADS) opt_adamw_kernel(const OptTensors
       reinterpret_cast<float4*>(t.p[s])[j] = make_float4(p[0], p[1], p[2], p[3]);
       reinterpret_cast<float4*>(t.m[s])[j] = make_float4(m[0], m[1], m[2], m[3]);
       reinterpret_cast<float4*>(t.v[s])[j] = make_float4(v[0], v[1], v[2], v[3]);
-      if (t.w[s]) reinterpret_cast<uint2*>(t.w[s])[j] = make_uint2(pack_bf16(p[0], p[1]), pack_bf16(p[2], p[3]));
+      const uint2 wb = make_uint2(pack_bf16(p[0], p[1]), pack_bf16(p[2], p[3]));
+      if (t.w[s]) reinterpret_cast<uint2*>(t.w[s])[j] = wb;
+      if (t.w16[s])                          // fp16 of the bf16-ROUNDED weight: what the forward's own cast would produce
+        reinterpret_cast<uint2*>(t.w16[s])[j] = make_uint2(pack_f16(bf16_lo(wb.x), bf16_hi(wb.x)), pack_f16(bf16_lo(wb.y), bf16_hi(wb.y)));
     }
   }
 }

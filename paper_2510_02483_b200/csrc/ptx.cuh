@@ -9,7 +9,29 @@
 #include <stdint.h>
 #include <stdio.h>
 
+#include <atomic>
+
 namespace lsp {
+
+// ------------------------------------------------------------------------------------------- per-device one-time setup
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is a PER-DEVICE property of a kernel, and contexts of several devices
+// (and several host threads) can live in one process: every launcher keeps one DeviceOnce and repeats the opt-in on each
+// device it meets.  The device is the one the entry point made current (DeviceGuard in liblsp.cu sets tls_device()).
+inline int& tls_device() {
+  static thread_local int d = 0;
+  return d;
+}
+struct DeviceOnce {
+  std::atomic<unsigned long long> mask{0};        // bit d: done on device d (devices 0..63; beyond: always repeat)
+  bool need() const {
+    const int d = tls_device();
+    return d > 63 || !((mask.load(std::memory_order_acquire) >> d) & 1ull);
+  }
+  void done() {
+    const int d = tls_device();
+    if (d <= 63) mask.fetch_or(1ull << d, std::memory_order_release);     // setting an attribute twice is harmless
+  }
+};
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
@@ -334,9 +356,24 @@ __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
   __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
   return *reinterpret_cast<uint32_t*>(&v);
 }
+// Two fp32 -> packed fp16 (a in the low half), round to nearest even, SATURATING: |v| > 65504 becomes +-65504, never
+// inf (one F2FP.SATFINITE, the cost of the plain conversion).  Every fp16 tensor-core operand the kernels produce goes
+// through this, so an out-of-range value (counted where caller data enters, pack_f16_sat) cannot turn the sums it
+// enters into inf / NaN further down.
 __device__ __forceinline__ uint32_t pack_f16(float a, float b) {
-  __half2 v = __floats2half2_rn(a, b);
-  return *reinterpret_cast<uint32_t*>(&v);
+  uint32_t r;
+  asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(b), "f"(a));
+  return r;
+}
+// fp16 operand conversions of caller-supplied values: saturating and counted (see the comment at the cast kernels of
+// norm.cuh and "Operand range" in include/lsp.h)
+constexpr float F16_MAX = 65504.0f;
+__device__ __forceinline__ uint32_t pack_f16_sat(float a, float b, unsigned int& bad) {
+  bad += (!(fabsf(a) <= F16_MAX)) + (!(fabsf(b) <= F16_MAX));
+  return pack_f16(fabsf(a) > F16_MAX ? copysignf(F16_MAX, a) : a, fabsf(b) > F16_MAX ? copysignf(F16_MAX, b) : b);
+}
+__device__ __forceinline__ void cast_report(unsigned int bad, unsigned long long* counter) {
+  if (bad && counter) atomicAdd(counter, static_cast<unsigned long long>(bad));      // rare path: integer atomic, no data involved
 }
 __device__ __forceinline__ void prefetch_l2(const void* p) {
   asm volatile("prefetch.global.L2 [%0];" ::"l"(p));

@@ -29,26 +29,30 @@ def global_grad_scale(tokens_local: int, world: int) -> float:
     return float(tokens_local) * float(world)
 
 
-def bucket_layout(shapes: dict):
+def bucket_layout(shapes: dict, multiple: int = 64):
     """Offsets (in elements) of the tensors of a bucket inside its flat buffer, each on a 64-element boundary, and the
-    flat length (a multiple of 64, so it divides by 4 * world for world <= 16)."""
+    flat length, padded to a multiple of `multiple` (itself a multiple of 64).  ZeRO-1 slices the flat buffer in `world`
+    equal parts whose boundaries must stay on 4-element / 16-byte boundaries (lsp_adamw_step): use multiple = 64 * world
+    (64 alone covers world = 1, 2, 4, 8, 16 only)."""
+    assert multiple % 64 == 0
     offs, n = {}, 0
     for k, s in shapes.items():
         offs[k] = n
         n += (torch.Size(s).numel() + 63) // 64 * 64
-    return offs, n
+    return offs, (n + multiple - 1) // multiple * multiple
 
 
 class GradBuckets:
-    def __init__(self, buckets, device, group=None, dtype=torch.float32):
+    def __init__(self, buckets, device, group=None, dtype=torch.float32, multiple: int = 64):
         """buckets: list of dicts name -> shape.  Allocates one flat buffer per bucket (fp32 for gradients; the same
         class lays out the bf16 weights for the sharded optimizer); `views[i][name]` are the tensors the kernels read or
-        write (each starts on a 256-byte boundary for fp32: TMA stores, float4 loads)."""
+        write (each starts on a 256-byte boundary for fp32: TMA stores, float4 loads).  multiple: see bucket_layout."""
         self.group = group
         self.shapes = list(buckets)
+        self.multiple = multiple
         self.flat, self.views, self._pending = [], [], []
         for shapes in buckets:
-            offs, n = bucket_layout(shapes)
+            offs, n = bucket_layout(shapes, multiple)
             flat = torch.zeros(n, dtype=dtype, device=device)
             self.flat.append(flat)
             self.views.append({k: flat[offs[k]:offs[k] + torch.Size(s).numel()].view(s) for k, s in shapes.items()})
@@ -89,8 +93,13 @@ class Zero1State:
         self.grads, self.weights, self.world, self.rank, self.group = grads, weights, world, rank, group
         self.lo, self.g_shard, self.master, self.m, self.v, self.segments = [], [], [], [], [], []
         self._pending = []
+        assert grads.multiple == weights.multiple, "gradient and weight buckets must share one layout"
         for b, shapes in enumerate(grads.shapes):
-            offs, n = bucket_layout(shapes)
+            offs, n = bucket_layout(shapes, grads.multiple)
+            if n % (4 * world):
+                raise ValueError(f"ZeRO-1: bucket {b} has {n} elements, not a multiple of 4 * world = {4 * world}: the tail would "
+                                 f"never be updated and slice boundaries would leave 16-byte alignment; build the buckets with "
+                                 f"GradBuckets(..., multiple=64 * world)")
             per = n // world
             lo, hi = rank * per, (rank + 1) * per
             self.lo.append(lo)

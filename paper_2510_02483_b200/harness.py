@@ -59,6 +59,17 @@ def upload_weights(wbits: dict, dev=None) -> dict:
     return {k: bf16_to_device(v, dev) for k, v in wbits.items()}
 
 
+def with_weight_cache(ctx: B.Ctx, weights: dict, dev=None, stream=None) -> dict:
+    """The same weight dict plus "f16_cache": the fp16 operand copies of the seven projection weights, converted once by
+    lsp_layer_prepare_weights (include/lsp.h: lsp_layer_weights.f16_cache).  Valid until the bf16 weights change."""
+    dev = dev or require_cuda()
+    cache = torch.empty(ctx.weight_cache_bytes, dtype=torch.uint8, device=dev)
+    B.lsp_layer_prepare_weights(ctx, weights, cache, stream)
+    out = dict(weights)
+    out["f16_cache"] = cache
+    return out
+
+
 def pad_heads(t: np.ndarray, name: str, n_heads: int, d: int, d_pad: int) -> np.ndarray:
     """Zero-pad every head of a projection tensor from width d to d_pad (lsp_layer_desc.head_dim_logical): rows of
     wq / wk / wv ([heads*d, H]), columns of wo ([H, heads*d]).  Works on weights (uint16 bf16 bits) and gradients."""

@@ -57,14 +57,24 @@ class PretrainStep:
         # gradient buckets (one flat buffer = one all-reduce each): the layers, then {head, final gain}, then the table
         lshapes = harness.WEIGHT_SHAPES(w)
         bshapes = [lshapes] * n_layers + [dict(head=(vocab, H), g_final=(H,)), dict(table=(vocab, H))]
-        self.buckets = dp.GradBuckets(bshapes, self.dev, group)
-        self.wbuckets = dp.GradBuckets(bshapes, self.dev, group, dtype=torch.bfloat16)     # the bf16 weights, same layout
+        mult = 64 * world if zero1 else 64              # ZeRO-1 slices every flat bucket in `world` equal, 16-byte aligned parts
+        self.buckets = dp.GradBuckets(bshapes, self.dev, group, multiple=mult)
+        self.wbuckets = dp.GradBuckets(bshapes, self.dev, group, dtype=torch.bfloat16, multiple=mult)     # the bf16 weights, same layout
         self.world = world
+        # fp16 tensor-core operand copies of every layer's projection weights (lsp_layer_weights.f16_cache): converted here
+        # once; afterwards lsp_adamw_step writes them together with the bf16 weights (lsp_adamw_tensor.weight_f16), so no
+        # forward pass of an iteration -- micro-batches, recomputation -- launches a weight cast
+        self.caches = []
         for l in range(n_layers):
             bits = weights[l] if weights is not None else synth.layer_weights(w, l)
             for k, t in harness.upload_weights(bits, self.dev).items():
                 self.wbuckets.views[l][k].copy_(t)
-            self.layer_w.append(self.wbuckets.views[l])
+            cache = torch.empty(self.ctx.weight_cache_bytes, dtype=torch.uint8, device=self.dev)
+            lw = dict(self.wbuckets.views[l])
+            B.lsp_layer_prepare_weights(self.ctx, lw, cache)
+            lw["f16_cache"] = cache
+            self.caches.append(cache)
+            self.layer_w.append(lw)
             self.layer_g.append(self.buckets.views[l])
         st = None
         if embedding is None or head is None:
@@ -80,9 +90,16 @@ class PretrainStep:
         decay = [{k: len(s) == 2 for k, s in b.items()} for b in bshapes]
         self.zero = dp.Zero1State(self.buckets, self.wbuckets, decay, world, rank, group) if zero1 else None
         if not zero1:
+            which = {k: i for i, k in enumerate(("wq", "wk", "wv", "wo", "w_gate", "w_up", "w_down"))}
             for b, shapes in enumerate(bshapes):
                 for k in (synth.WEIGHT_NAMES if b < n_layers else shapes):
-                    self._register(self.wbuckets.views[b][k], self.buckets.views[b][k], decay=decay[b][k])
+                    w16 = None
+                    if b < n_layers and k in which:
+                        off = B.lsp_weight_cache_offset(self.ctx, which[k])       # -1: rows permuted in the cache (rope_layout 1)
+                        if off >= 0:
+                            n = self.wbuckets.views[b][k].numel()
+                            w16 = self.caches[b][off:off + 2 * n].view(torch.float16)
+                    self._register(self.wbuckets.views[b][k], self.buckets.views[b][k], decay=decay[b][k], weight_f16=w16)
         self.t = 0
         # gradients are carried scaled by T (the gradient of the SUM loss): the mean's 1/T would push the layers' 16-bit
         # backward operands under the fp16 normal range; lsp_adamw_step divides it out (exact for a power-of-two T),
@@ -90,9 +107,9 @@ class PretrainStep:
         self.head_scale = float(T)
         self.grad_scale = dp.global_grad_scale(T * micro_batches, world)
 
-    def _register(self, weight, grad, decay):
+    def _register(self, weight, grad, decay, weight_f16=None):
         self.params.append(dict(grad=grad, master=weight.float(), m=torch.zeros_like(grad), v=torch.zeros_like(grad), weight=weight,
-                                decay=decay))
+                                decay=decay, weight_f16=weight_f16))
 
     @property
     def n_params(self):
@@ -139,6 +156,9 @@ class PretrainStep:
         if self.zero is not None:
             self.zero.step(lambda t, phase, gn: B.lsp_adamw_step(self.ctx, t, lr=lr, step=self.t, gnorm_out=gn, phase=phase,
                                                                  grad_scale=self.grad_scale, stream=stream, **hyper), self.gnorm)
+            # the all-gathered bf16 weights came from other ranks' optimizer slices: refresh the operand caches from them
+            for l in range(self.L):
+                B.lsp_layer_prepare_weights(self.ctx, self.layer_w[l], self.caches[l], stream)
             return
         self.buckets.wait()
         B.lsp_adamw_step(self.ctx, self.params, lr=lr, step=self.t, gnorm_out=self.gnorm,

@@ -194,3 +194,30 @@ def test_zero1_two_gloo_ranks_match_full_adamw():
         assert o["norm"] == pytest.approx(o["norm_ref"], rel=1e-6)
         assert o["worst"] <= 1.01                                   # within half a bf16 ulp (+ fp32 master rounding) of the fp64 result
         assert o["flips"] <= 2e-3 * o["n"]                          # bf16 rounding of an fp32 vs an fp64 master weight
+
+
+def test_zero1_slices_need_padded_buckets():
+    """A world size that does not divide the 64-element padded bucket length (3, 6, ...) must not silently drop the tail of
+    the flat buffer or cut slices off 16-byte boundaries: the constructor refuses, and buckets built with
+    multiple = 64 * world give `world` equal slices that cover every parameter exactly once on 4-element boundaries."""
+    import torch
+    from paper_2510_02483_b200 import dp
+    shapes = [dict(wa=(24, 40), ga=(40,), wb=(40, 24)), dict(table=(50, 40))]
+    decay = [{k: len(s) == 2 for k, s in b.items()} for b in shapes]
+    g, w = dp.GradBuckets(shapes, "cpu"), dp.GradBuckets(shapes, "cpu", dtype=torch.bfloat16)
+    with pytest.raises(ValueError, match="multiple of 4 \\* world"):
+        dp.Zero1State(g, w, decay, 3, 0)
+    g3, w3 = dp.GradBuckets(shapes, "cpu", multiple=192), dp.GradBuckets(shapes, "cpu", dtype=torch.bfloat16, multiple=192)
+    covered = [torch.zeros_like(f, dtype=torch.int32) for f in g3.flat]
+    for r in range(3):
+        z = dp.Zero1State(g3, w3, decay, 3, r)
+        for b, segs in enumerate(z.segments):
+            assert z.lo[b] % 4 == 0 and g3.flat[b].numel() % 3 == 0
+            for _, a, e, _ in segs:
+                assert a % 4 == 0 and e % 4 == 0
+                covered[b][a:e] += 1
+    for b, shp in enumerate(shapes):
+        offs, _ = dp.bucket_layout(shp, 192)
+        for k, s in shp.items():
+            n = torch.Size(s).numel()
+            assert bool((covered[b][offs[k]:offs[k] + n] == 1).all()), (b, k)

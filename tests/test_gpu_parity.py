@@ -168,6 +168,81 @@ def test_layer_bit_reproducible(gpu):
         assert np.array_equal(a[n], b[n]), n
 
 
+@pytest.mark.parametrize("rope_layout", [0, 1])
+@pytest.mark.parametrize("w", [synth.CFG1_TINY, MID], ids=lambda w: w.name)
+def test_layer_weight_cache_is_bit_identical(gpu, w, rope_layout):
+    """lsp_layer_weights.f16_cache (fp16 operand copies made once by lsp_layer_prepare_weights) against the default mode
+    (every forward converts the bf16 weights itself): y, dx and the nine gradients bit for bit, and the cached step
+    launches two kernels fewer (the weight casts of the attention and MLP blocks)."""
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    dev = gpu.require_cuda()
+    ctx = gpu.make_ctx(w, rope_layout=rope_layout)
+    buf = gpu.LayerBuffers(ctx, w, dev)
+    weights = gpu.upload_weights(synth.layer_weights(w), dev)
+    inp = synth.layer_inputs(w)
+    x, dy = gpu.bf16_to_device(inp["x"], dev), gpu.bf16_to_device(inp["dy"], dev)
+
+    def run(wts):
+        n0 = B.lsp_launch_count(ctx)
+        B.lsp_layer_fwd(ctx, x, wts, buf.y, buf.saved, buf.ws)
+        B.lsp_layer_bwd(ctx, x, dy, wts, buf.saved, buf.dx, buf.grads, buf.ws)
+        torch.cuda.synchronize()
+        out = dict(y=buf.y.cpu().numpy(), dx=buf.dx.cpu().numpy())
+        out.update({k: v.cpu().numpy() for k, v in buf.grads.items()})
+        return out, B.lsp_launch_count(ctx) - n0
+
+    plain, n_plain = run(weights)
+    cached_w = gpu.with_weight_cache(ctx, weights, dev)
+    for t in [buf.y, buf.dx] + list(buf.grads.values()):
+        t.fill_(float("nan"))
+    cached, n_cached = run(cached_w)
+    assert n_cached == n_plain - 2
+    for k in plain:
+        assert np.array_equal(plain[k], cached[k]), k
+    assert B.lsp_weight_cache_offset(ctx, 3) > 0 and B.lsp_weight_cache_offset(ctx, 7) == -1
+    assert (B.lsp_weight_cache_offset(ctx, 0) == -1) == (rope_layout == 1)
+    ctx.close()
+
+
+def test_fp16_operand_overflow_is_saturated_and_counted(gpu):
+    """Operand range contract of include/lsp.h: an upstream gradient with |dy| > 65504 (here 1e5-scale entries and one inf)
+    is outside the fp16 operand range.  The conversion must not turn it into a silent inf: it saturates to +-65504 and
+    counts the values it clamped -- every gradient of the backward stays finite, lsp_overflow_count reports the clamped
+    values (each bad element is met twice: in the fp16 copy of dy and in the fp16 copy of da = dy + MLP-branch gradient,
+    whose big entries are dy's), and reset returns the counter to zero."""
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    w = MID
+    dev = gpu.require_cuda()
+    ctx = gpu.make_ctx(w)
+    buf = gpu.LayerBuffers(ctx, w, dev)
+    weights = gpu.upload_weights(synth.layer_weights(w), dev)
+    inp = synth.layer_inputs(w)
+    x = gpu.bf16_to_device(inp["x"], dev)
+    dy = gpu.bf16_to_device(inp["dy"], dev).clone()
+    B.lsp_layer_fwd(ctx, x, weights, buf.y, buf.saved, buf.ws)
+    B.lsp_layer_bwd(ctx, x, dy, weights, buf.saved, buf.dx, buf.grads, buf.ws)
+    assert B.lsp_overflow_count(ctx) == 0                     # N(0,1) inputs and 0.02 N(0,1) weights are in range
+    flat = dy.view(-1)
+    big = torch.arange(0, 4000, 40, device=dev)
+    flat[big] = 1.0e5
+    flat[big + 1] = -2.5e5
+    flat[17] = float("inf")
+    n_bad = int((dy.float().abs() > 65504.0).sum())
+    assert n_bad == 201
+    B.lsp_layer_bwd(ctx, x, dy, weights, buf.saved, buf.dx, buf.grads, buf.ws)
+    torch.cuda.synchronize()
+    n_seen = B.lsp_overflow_count(ctx, reset=True)
+    assert 2 * n_bad <= n_seen <= 2 * n_bad + 8, (n_seen, n_bad)
+    assert B.lsp_overflow_count(ctx) == 0
+    for k, v in buf.grads.items():
+        assert bool(torch.isfinite(v).all()), k
+    # dx = dy + (branch gradients): finite wherever dy itself is finite (the fp32 residual path is not an operand)
+    assert bool(torch.isfinite(buf.dx.view(-1)[torch.isfinite(dy.view(-1).float())]).all())
+    ctx.close()
+
+
 @pytest.mark.parametrize("w", [synth.CFG1_TINY, MID], ids=lambda w: w.name)
 def test_layer_rope_half_split_layout(gpu, w):
     """rope_layout = 1 (pairs (i, i + d/2), the other common RoPE convention) against the oracle's layout-1 path: the
@@ -564,19 +639,159 @@ def test_layer_cfg2_full_size(gpu):
 
 
 @pytest.mark.slow
-def test_layer_cfg4_one_sequence(gpu):
-    """BASELINE.json configs[3] (30B-class layer, MHA 52 heads, FFN 17920) with batch 1 instead of 2: the same kernels,
-    tiles and tails (F = 17920 = 140 x 128), half the oracle time."""
-    _layer_full(gpu, synth.CFG4_30B_LAYER.with_(batch=1))
+def test_layer_cfg4_full_size(gpu):
+    """BASELINE.json configs[3] exactly as bench_configs.py launches it (30B-class layer, MHA 52 heads, hidden 6656,
+    FFN 17920 = 140 x 128, batch 2 x seq 4096): every element of y, dx and the nine gradients against the fp64 oracle
+    (about two minutes of CPU time)."""
+    _layer_full(gpu, synth.CFG4_30B_LAYER)
+
+
+# (batch, kv head) groups whose outputs the oracle recomputes at each sequence length of config 5; fixed here, before
+# any result existed.  The oracle's cost per group grows like S^2 (9 s at S = 16384), the launch has 64 .. 768 groups.
+CFG5_GROUPS = {1024: [(0, 0), (5, 3), (13, 7), (21, 1), (31, 6), (17, 4)], 4096: [(0, 0), (3, 5), (7, 2)],
+               8192: [(0, 4), (3, 7)], 16384: [(1, 5)]}
+
+
+def _cfg5_groups(S):
+    import os
+    if os.environ.get("LSP_FULL_PARITY") == "1":      # every (batch, kv head) group: ~15 minutes of oracle time in all
+        w = [x for x in synth.CFG5_ATTN if x.seq == S][0]
+        return [(b, kv) for b in range(w.batch) for kv in range(w.n_kv_heads)]
+    return CFG5_GROUPS[S]
 
 
 @pytest.mark.slow
 @pytest.mark.parametrize("S", [1024, 4096, 8192, 16384])
-def test_sdpa_cfg5_lengths(gpu, S):
-    """BASELINE.json configs[4] sequence lengths with the 3B group layout (G = 3) on one kv head and one sequence
-    (3 q heads / 1 kv head, batch 1): every element of O, L, dq, dk, dv.  The full 24/8-head, 32768-token launch is
-    the same kernel over more (batch, kv-head) CTAs; its throughput is reported by profiles/."""
-    test_sdpa_fwd_bwd(gpu, 1, S, 3, 1, 128)
+def test_sdpa_cfg5_full_launch(gpu, S):
+    """BASELINE.json configs[4] in the launch bench_configs.py times: 24 q / 8 kv heads of width 128, batch x seq =
+    32768 tokens, (batch, S) = (32, 1024), (8, 4096), (4, 8192), (2, 16384).  The GPU runs the whole launch; the oracle
+    recomputes, element by element, the (batch, kv head) groups listed in CFG5_GROUPS (a group = the kv head's K, V and
+    its 3 query heads: O, L, dq of those heads and dk, dv of the kv head depend on nothing else), because the full
+    launch costs the oracle 15 minutes.  The metric is the north_star one, max|gpu - ref| / rms(ref), over the elements
+    of the checked groups: labelled SAMPLED (groups), every element of each group.  LSP_FULL_PARITY=1 checks all groups."""
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    w = [x for x in synth.CFG5_ATTN if x.seq == S][0]
+    Bz, nq, nkv, d = w.batch, w.n_q_heads, w.n_kv_heads, w.head_dim
+    G = nq // nkv
+    bits = synth.attn_inputs(w)
+    ctx = gpu.make_ctx(w, use_rope=False)
+    dev = torch.device("cuda")
+    t = {k: gpu.bf16_to_device(v) for k, v in bits.items()}
+    o = torch.empty((Bz, S, nq, d), dtype=torch.float32, device=dev)
+    lse = torch.empty((Bz, nq, S), dtype=torch.float32, device=dev)
+    dq = torch.empty_like(o)
+    dk = torch.empty((Bz, S, nkv, d), dtype=torch.float32, device=dev)
+    dv = torch.empty_like(dk)
+    ws = torch.empty(ctx.workspace_bytes, dtype=torch.uint8, device=dev)
+    B.lsp_sdpa_fwd(ctx, t["q"], t["k"], t["v"], o, lse, ws)
+    B.lsp_sdpa_bwd(ctx, t["q"], t["k"], t["v"], o, lse, t["dO"], dq, dk, dv, ws)
+    torch.cuda.synchronize()
+    got_all = dict(O=o.cpu().numpy(), L=lse.cpu().numpy(), dq=dq.cpu().numpy(), dk=dk.cpu().numpy(), dv=dv.cpu().numpy())
+    for n, v in got_all.items():
+        assert np.all(np.isfinite(v)), n                          # the whole launch, not only the checked groups
+    ctx.close()
+    got = {n: [] for n in got_all}
+    ref = {n: [] for n in got_all}
+    for b, kv in _cfg5_groups(S):
+        hs = slice(kv * G, (kv + 1) * G)
+        q64, dO64 = (synth.bf16_bits_to_f64(bits[n][b:b + 1, :, hs]) for n in ("q", "dO"))
+        k64, v64 = (synth.bf16_bits_to_f64(bits[n][b:b + 1, :, kv:kv + 1]) for n in ("k", "v"))
+        O_ref, L_ref = R.sdpa_fwd(q64, k64, v64)
+        dq_ref, dk_ref, dv_ref = R.sdpa_bwd(q64, k64, v64, dO64)
+        for n, r, g in (("O", O_ref, got_all["O"][b:b + 1, :, hs]), ("L", L_ref, got_all["L"][b:b + 1, hs]),
+                        ("dq", dq_ref, got_all["dq"][b:b + 1, :, hs]), ("dk", dk_ref, got_all["dk"][b:b + 1, :, kv:kv + 1]),
+                        ("dv", dv_ref, got_all["dv"][b:b + 1, :, kv:kv + 1])):
+            got[n].append(np.asarray(g, np.float64).reshape(-1))
+            ref[n].append(np.asarray(r, np.float64).reshape(-1))
+    check({n: np.concatenate(v) for n, v in got.items()}, {n: np.concatenate(v) for n, v in ref.items()},
+          ["O", "L", "dq", "dk", "dv"])
+
+
+# ------------------------------------------------------------------------------------------- config 3 at its own size
+def _cfg3_run(gpu, collect):
+    """Embedding gather + 28 x lsp_layer_fwd + 28 x lsp_layer_bwd of BASELINE.json configs[2] (batch 2 x seq 4096, vocab
+    128256, fp32 residual stream); collect(name, layer, device tensor) is called for y, dx0 and every gradient."""
+    import torch
+    w = synth.CFG3_3B_STACK
+    s = synth.stack_inputs(w)
+    run = gpu.StackRunner(w, w.n_layers)
+    ids = torch.from_numpy(s["ids"]).cuda()
+    table = gpu.bf16_to_device(s["embedding"])
+    y = run.forward(ids, table)
+    collect("y", 0, y)
+    dy32 = gpu.bf16_to_device(s["dy"]).float()
+    dx0 = run.backward(dy32, on_layer_grads=lambda l, g: [collect(k, l, v) for k, v in g.items()])
+    collect("dx0", 0, dx0)
+    torch.cuda.synchronize()
+    run.close()
+
+
+@pytest.mark.slow
+def test_stack_cfg3_full_depth_sampled(gpu):
+    """BASELINE.json configs[2] at its own size -- 28 layers, T = 8192, vocab 128256 -- against the fp64 oracle's compact
+    reference tests/golden/cfg3_reference.npz (written by tests/golden/make_cfg3_reference.py from oracle/ alone; the
+    oracle needs 20+ minutes for this config, SURVEY.md 8(d) decision rule).  SAMPLED: per tensor the error is the
+    largest |gpu - ref| over a fixed seeded sample of elements (2^18 of y, dx0; 2^14 of each of the 196 weight
+    gradients) and over the rows of largest reference norm, divided by the reference rms over ALL elements; the 56 gain
+    gradients are compared in full.  Bar: the north_star one, 2e-2.  Every element of every tensor is compared by
+    test_stack_cfg3_full_depth_every_element (LSP_FULL_PARITY=1)."""
+    import os
+    import torch
+    from tests.golden import make_cfg3_reference as M
+    path = os.path.join(os.path.dirname(os.path.abspath(M.__file__)), "cfg3_reference.npz")
+    assert os.path.exists(path), "tests/golden/cfg3_reference.npz is missing: run tests/golden/make_cfg3_reference.py"
+    ref = np.load(path)
+    assert int(ref["n_layers"]) == synth.CFG3_3B_STACK.n_layers
+    errs = {}
+
+    def collect(name, layer, t):
+        if name in ("g_attn", "g_mlp"):
+            key = f"L{layer}/d{name}"
+            g = t.cpu().numpy().astype(np.float64)
+            assert np.all(np.isfinite(g)), key
+            errs[key] = float(np.max(np.abs(g - ref[key + "/full"].astype(np.float64))) / float(ref[key + "/rms"]))
+            return
+        key = name if name in ("y", "dx0") else f"L{layer}/d{name}"
+        assert bool(torch.isfinite(t).all()), key                # every element, on the device
+        idx = M.sample_indices(t.numel(), *M.sample_spec(name, layer))
+        samp = t.reshape(-1)[torch.from_numpy(idx).to(t.device)].cpu().numpy().astype(np.float64)
+        rows = t[torch.from_numpy(ref[key + "/rows"]).to(t.device)].cpu().numpy().astype(np.float64)
+        e = max(np.max(np.abs(samp - ref[key + "/val"].astype(np.float64))), np.max(np.abs(rows - ref[key + "/rowval"].astype(np.float64))))
+        errs[key] = float(e / float(ref[key + "/rms"]))
+
+    _cfg3_run(gpu, collect)
+    assert len(errs) == 2 + 9 * synth.CFG3_3B_STACK.n_layers
+    worst = {}
+    for k, e in errs.items():
+        n = k.split("/")[-1]
+        if e >= worst.get(n, (0.0, ""))[0]:
+            worst[n] = (e, k)
+    print("cfg3 sampled, worst layer per tensor kind: " + "  ".join(f"{n}={e:.2e}@{k.split('/')[0]}" for n, (e, k) in worst.items()))
+    bad = {k: e for k, e in errs.items() if not e <= TOL}
+    assert not bad, f"normalised error above {TOL}: {bad}"
+
+
+@pytest.mark.slow
+def test_stack_cfg3_full_depth_every_element(gpu):
+    """The same launch compared with the oracle run in full on the host cores, every element of y, dx0 and the 28 x 9
+    gradients (about 25 minutes of CPU time on 16 cores): opt-in with LSP_FULL_PARITY=1 -- it does not fit the 1200 s
+    budget of the default `-m gpu` run; its log is committed under profiles/."""
+    import os
+    if os.environ.get("LSP_FULL_PARITY") != "1":
+        pytest.skip("set LSP_FULL_PARITY=1 (about 25 minutes of oracle time)")
+    from tests.golden import make_cfg3_reference as M
+    w = synth.CFG3_3B_STACK
+    got = {}
+    _cfg3_run(gpu, lambda name, layer, t: got.__setitem__((name, layer), t.cpu().numpy()))
+    s = synth.stack_inputs(w)
+    x0_ref = R.embed_fwd(s["ids"], synth.bf16_bits_to_f64(s["embedding"]))
+    y_ref, dx0_ref, g_ref = R.stack_fwd_bwd(x0_ref, synth.bf16_bits_to_f64(s["dy"]), M.LazyWeights(w, w.n_layers), oracle_shape(w))
+    check(dict(y=got[("y", 0)], dx0=got[("dx0", 0)]), dict(y=y_ref, dx0=dx0_ref), ["y", "dx0"])
+    for l in range(w.n_layers):
+        print(f"layer {l}: ", end="")
+        check({"d" + k: got[(k, l)] for k in synth.WEIGHT_NAMES}, {"d" + k: v for k, v in g_ref[l].items()},
+              ["d" + k for k in synth.WEIGHT_NAMES])
 
 
 # ------------------------------------------------------------------------------------------- optimizer step (NEXT #2)
@@ -632,12 +847,59 @@ def test_adamw_step_vs_oracle(gpu):
     ctx.close()
 
 
+def test_adamw_skips_a_step_with_a_non_finite_gradient(gpu):
+    """One inf (or NaN) anywhere in the gradients makes the global norm non-finite: lsp_adamw_step must leave master, m, v
+    and both weight copies untouched (bit for bit) and flag the skip in gnorm_out = {non-finite norm, 0}; the next step,
+    with finite gradients, updates as usual (clip / inf = 0 and inf * 0 = NaN used to be written into the
+    state for good).  Also: weight_f16 receives the fp16 value of the new bf16 weight."""
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    dev = torch.device("cuda")
+    ctx = gpu.make_ctx(synth.CFG1_TINY)
+    gen = torch.Generator(device="cpu").manual_seed(5)
+    shapes = [(260, 64), (512,), (36, 100)]
+    tp = [(torch.randn(s, generator=gen) * 0.02).to(dev) for s in shapes]
+    tm = [(torch.randn(s, generator=gen) * 1e-3).to(dev) for s in shapes]
+    tv = [(torch.rand(s, generator=gen) * 1e-6).to(dev) for s in shapes]
+    tw = [t.to(torch.bfloat16) for t in tp]
+    tw16 = [t.to(torch.bfloat16).to(torch.float16) for t in tp]
+    gn = torch.zeros(2, dtype=torch.float32, device=dev)
+    for bad in (float("inf"), float("nan")):
+        tg = [(torch.randn(s, generator=gen) * 0.1).to(dev) for s in shapes]
+        tg[1][77] = bad
+        before = [x.clone() for x in tp + tm + tv + tw + tw16]
+        tensors = [dict(grad=a, master=b, m=c, v=d, weight=e, weight_f16=f, decay=True) for a, b, c, d, e, f in zip(tg, tp, tm, tv, tw, tw16)]
+        B.lsp_adamw_step(ctx, tensors, lr=1e-3, step=3, gnorm_out=gn)
+        torch.cuda.synchronize()
+        n, c = [float(x) for x in gn.cpu().numpy()]
+        assert not np.isfinite(n) and c == 0.0
+        for a, b in zip(before, tp + tm + tv + tw + tw16):
+            assert torch.equal(a.view(torch.uint8), b.view(torch.uint8))
+    tg = [(torch.randn(s, generator=gen) * 0.1).to(dev) for s in shapes]
+    p_old = [x.clone() for x in tp]
+    tensors = [dict(grad=a, master=b, m=c, v=d, weight=e, weight_f16=f, decay=True) for a, b, c, d, e, f in zip(tg, tp, tm, tv, tw, tw16)]
+    B.lsp_adamw_step(ctx, tensors, lr=1e-3, step=4, gnorm_out=gn)
+    torch.cuda.synchronize()
+    n, c = [float(x) for x in gn.cpu().numpy()]
+    assert np.isfinite(n) and c > 0.0
+    for i in range(len(shapes)):
+        assert not torch.equal(p_old[i], tp[i])
+        assert bool(torch.isfinite(tp[i]).all() and torch.isfinite(tm[i]).all() and torch.isfinite(tv[i]).all())
+        assert torch.equal(tw[i], tp[i].to(torch.bfloat16))
+        assert torch.equal(tw16[i], tw[i].to(torch.float16))          # the fp16 operand copy = the forward's own cast
+    ctx.close()
+
+
 # ------------------------------------------------------------------------------------------- model head + embedding backward (NEXT #1)
-@pytest.mark.parametrize("Bz,S,H,V", [(1, 256, 256, 1000), (2, 192, 384, 4104)])
+@pytest.mark.parametrize("Bz,S,H,V", [(1, 256, 256, 1000), (2, 192, 384, 4104), (1, 4096, 3072, 128256)])
 def test_head_fwd_bwd_vs_oracle(gpu, Bz, S, H, V):
     """lsp_head_fwd_bwd (final RMSNorm + LM head + mean cross-entropy, all gradients) against oracle/head_ref.py.
     Bars: loss and lse 1e-4 absolute-relative (fp16 operands, fp32 accumulation over H terms); gradients at the layer's
-    bar, max|gpu - ref| / rms(ref) <= 2e-2."""
+    bar, max|gpu - ref| / rms(ref) <= 2e-2.  The last case is config 3's own head (H 3072, V 128256: the one-pass
+    cross-entropy kernel where it is timed) at half the config's tokens.  For dw_head the metric is ill-conditioned in
+    V / T: only the T target rows are O(|xn| / T), the other V - T rows are ~1/V of that, so rms(ref) ~ |xn| / sqrt(T V)
+    while the largest error is one fp16 rounding of the target entry of dz, 2^-11 |xn|_max / T: the ratio grows like
+    2^-11 * 4 * sqrt(V / T) -- 3.1e-2 at T = 512 (measured), 1.1e-2 at T = 4096, 7.7e-3 at the config's T = 8192."""
     import torch
     from oracle import head_ref as Hd
     from paper_2510_02483_b200 import binding as B
@@ -662,6 +924,45 @@ def test_head_fwd_bwd_vs_oracle(gpu, Bz, S, H, V):
     assert abs(float(loss.cpu()) - ref["loss"]) <= 1e-4 * abs(ref["loss"])
     assert np.max(np.abs(lse.cpu().numpy() - ref["lse"])) <= 1e-4 * np.max(np.abs(ref["lse"]))
     check(dict(dx=dx.cpu().numpy(), dg_final=dg.cpu().numpy(), dw_head=dw.cpu().numpy()), ref, ["dx", "dg_final", "dw_head"])
+    ctx.close()
+
+
+def test_head_ignored_targets_vs_oracle(gpu):
+    """Reading H-4: targets outside [0, V) (-100, and one >= V) carry no loss; the mean and every gradient run over the
+    counted tokens (oracle/head_ref.py, pinned against torch cross_entropy(ignore_index)).  Also the all-ignored batch:
+    zero loss, zero gradients, nothing non-finite."""
+    import torch
+    from oracle import head_ref as Hd
+    from paper_2510_02483_b200 import binding as B
+    Bz, S, H, V = 2, 192, 384, 4104
+    w = synth.Workload("head", 7, Bz, S, H, 4, 2, 64, 256, 1e-5, 10000.0)
+    T = w.tokens
+    x_bits = synth.normal_bf16(7, 0, "x", (T, H), 1.0)
+    g_bits = synth.normal_bf16(7, 0, "g_attn", (H,), 0.1, offset=1.0)
+    wh_bits = synth.normal_bf16(7, 0, "embedding", (V, H), 0.02)
+    rng = np.random.default_rng([2510, 2483, 7, V, 1])
+    y = rng.integers(0, V, size=T, dtype=np.int32)
+    y[rng.choice(T, size=T // 3, replace=False)] = -100
+    y[S - 1] = -100; y[T - 1] = -100                      # the last token of each sequence, as in a packed batch
+    y[5] = V                                              # out of range: not counted, never used as an index
+    ctx = gpu.make_ctx(w)
+    dev = torch.device("cuda")
+    x = gpu.bf16_to_device(x_bits); g = gpu.bf16_to_device(g_bits); wh = gpu.bf16_to_device(wh_bits)
+    loss = torch.zeros(1, dtype=torch.float32, device=dev); lse = torch.empty(T, dtype=torch.float32, device=dev)
+    dx = torch.empty((T, H), dtype=torch.float32, device=dev); dg = torch.empty(H, dtype=torch.float32, device=dev)
+    dw = torch.empty((V, H), dtype=torch.float32, device=dev)
+    ws = torch.empty(B.lsp_head_workspace_bytes(ctx, V), dtype=torch.uint8, device=dev)
+    B.lsp_head_fwd_bwd(ctx, x, g, wh, torch.from_numpy(y).to(dev), V, loss, lse, dx, dg, dw, ws)
+    torch.cuda.synchronize()
+    ref = Hd.head_loss_fwd_bwd(synth.bf16_bits_to_f64(x_bits), synth.bf16_bits_to_f64(g_bits), synth.bf16_bits_to_f64(wh_bits), y, 1e-5)
+    assert abs(float(loss.cpu()) - ref["loss"]) <= 1e-4 * abs(ref["loss"])
+    assert np.max(np.abs(lse.cpu().numpy() - ref["lse"])) <= 1e-4 * np.max(np.abs(ref["lse"]))
+    got_dx = dx.cpu().numpy()
+    assert not np.any(got_dx[(y < 0) | (y >= V)])                  # ignored rows: exactly zero
+    check(dict(dx=got_dx, dg_final=dg.cpu().numpy(), dw_head=dw.cpu().numpy()), ref, ["dx", "dg_final", "dw_head"])
+    B.lsp_head_fwd_bwd(ctx, x, g, wh, torch.full((T,), -100, dtype=torch.int32, device=dev), V, loss, lse, dx, dg, dw, ws)
+    torch.cuda.synchronize()
+    assert float(loss.cpu()) == 0.0 and not bool(dx.any()) and not bool(dw.any()) and not bool(dg.any())
     ctx.close()
 
 
