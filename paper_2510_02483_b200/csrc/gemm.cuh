@@ -1219,7 +1219,10 @@ cudaError_t launch_gemm_pair(const GemmMaps& maps, GemmShape sh, const Epi& epi,
   const int mblocks = (sh.M + 2 * MT * GEMM_BM - 1) / (2 * MT * GEMM_BM), nblocks = (sh.N + NOUT - 1) / NOUT;
   const int ntiles = mblocks * nblocks;
   if (ntiles == 0) return cudaSuccess;
-  sh.band = gemm_band(2 * MT * mblocks) / (2 * MT);       // ~2048-row bands
+  // ~2048-row bands.  A band height chosen per shape so that a band is a whole number of 74-tile waves (6 or 12 pair tiles
+  // for 12 n-blocks instead of 8) was measured in round 2 (profiles/r2_notes.md): GEMM time of the step 8.04-8.09 ms
+  // against 7.94-8.02 ms with this fixed height on the same machine -- no gain, not kept.
+  sh.band = gemm_band(2 * MT * mblocks) / (2 * MT);
   if (sh.band < 1) sh.band = 1;
   const int pairs = num_sms / 2;
   const int clusters = ntiles < pairs ? ntiles : pairs;

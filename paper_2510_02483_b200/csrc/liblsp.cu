@@ -1234,6 +1234,13 @@ lsp_status lsp_set_packed_sequences(lsp_ctx* ctx, const int32_t* cu_seqlens_host
 
 long long lsp_launch_count(const lsp_ctx* ctx) { return ctx ? ctx->launches : -1; }
 
+#ifdef LSP_ATTN_TRACE
+// debug builds only (not declared in lsp.h): copies the forward attention kernel's clock trace to the host
+int lsp_debug_read_trace(unsigned long long* host, int n) {
+  return cudaMemcpyFromSymbol(host, g_atc_trace, sizeof(unsigned long long) * n) == cudaSuccess ? 0 : -1;
+}
+#endif
+
 lsp_status lsp_timing_enable(lsp_ctx* ctx, int max_records) {
   if (!ctx || max_records < 0) return LSP_EINVAL;
   LSP_ENTER(ctx);

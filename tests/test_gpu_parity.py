@@ -1169,9 +1169,18 @@ def test_layer_step_replays_from_a_cuda_graph(gpu, w):
 
 def test_pretrain_zero1_matches_replicated_optimizer(gpu):
     """PretrainStep(zero1=True) on one rank (its slice is everything; the two-phase lsp_adamw_step with the sum of g^2
-    handed over in between) against the plain path over three iterations: same losses (1e-6), the same bf16 weights in
-    every tensor up to isolated last-bit flips (the norm passes through one extra fp32 rounding), and a slice plan for
-    world = 2 that covers every parameter exactly once with 4-aligned cuts."""
+    handed over in between) against the plain path over three iterations, and a slice plan for world = 2 that covers
+    every parameter exactly once with 4-aligned cuts.
+
+    Bars.  Iteration 1 starts from identical weights and runs identical kernels: the loss is
+    bit-identical, the gradient norm differs by the one extra fp32 rounding of the handed-over sum (1e-6), and the bf16
+    weights differ only where that last bit of the clip coefficient moves a master weight across a bf16 rounding
+    boundary (isolated flips: < 1e-4 of the elements, one bf16 ulp).  From iteration 2 on the two runs are separate
+    trajectories that start from weights differing in those isolated bits, and a training step amplifies a last-bit
+    difference like any other rounding: a perturbed logit flips fp16 roundings of P (2^-11 each) in the attention, the
+    perturbed gradient moves more master weights across bf16 boundaries.  What must still hold is that both stay the
+    SAME training run to working precision: losses within 1e-5, gradient norms within 1e-4, every weight within two
+    bf16 ulps (2^-7 of the largest weight), fewer than 2 % of the weights different."""
     import torch
     from paper_2510_02483_b200 import dp, pretrain
     w = synth.Workload("pretrain_z1", 12, 2, 192, 256, 4, 2, 128, 688, 1e-5, 500000.0, 2, 1000)
@@ -1181,12 +1190,18 @@ def test_pretrain_zero1_matches_replicated_optimizer(gpu):
     for it in range(3):
         losses = [float(r.step(tid, tt, lr=1e-3).cpu()) for r in runs]
         torch.cuda.synchronize()
-        assert abs(losses[0] - losses[1]) <= 1e-6 * abs(losses[0]), (it, losses)
         n0, n1 = float(runs[0].gnorm[0].cpu()), float(runs[1].gnorm[0].cpu())
-        assert abs(n0 - n1) <= 1e-6 * n0
+        flips, worst = 0.0, 0.0
         for fa, fb in zip(runs[0].wbuckets.flat, runs[1].wbuckets.flat):
             a, b = fa.float().cpu().numpy(), fb.float().cpu().numpy()
-            assert np.mean(a != b) < 1e-4 and np.max(np.abs(a - b)) <= 2.0 ** -7 * np.max(np.abs(a))
+            flips = max(flips, float(np.mean(a != b)))
+            worst = max(worst, float(np.max(np.abs(a - b)) / np.max(np.abs(a))))
+        print(f"iteration {it + 1}: loss diff {abs(losses[0] - losses[1]) / abs(losses[0]):.2e}  norm diff {abs(n0 - n1) / n0:.2e}  "
+              f"weights differing {flips:.2e}  largest difference {worst:.2e} of the largest weight")
+        loss_bar, norm_bar, flip_bar = (0.0, 1e-6, 1e-4) if it == 0 else (1e-5, 1e-4, 2e-2)
+        assert abs(losses[0] - losses[1]) <= loss_bar * abs(losses[0]), (it, losses)
+        assert abs(n0 - n1) <= norm_bar * n0, (it, n0, n1)
+        assert flips < flip_bar and worst <= 2.0 ** -7, (it, flips, worst)
     # slice plan of two ranks over the same buckets
     decay = [{k: len(s) == 2 for k, s in b.items()} for b in runs[0].buckets.shapes]
     plans = [dp.Zero1State(runs[0].buckets, runs[0].wbuckets, decay, 2, r) for r in range(2)]
