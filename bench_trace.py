@@ -1,0 +1,103 @@
+#!/usr/bin/env python
+"""clock64 traces of the three tcgen05 attention kernels (forward, dK/dV, dQ) at the attention shape of config 2.
+
+    python bench_trace.py [--blocks N] > profiles/rX_attn_traces.txt
+
+Builds a DEBUG copy of the library with -DLSP_ATTN_TRACE into a temporary directory (the shipped liblsp.so carries no
+trace code), loads it in place of the product library for this process only, runs lsp_sdpa_fwd / lsp_sdpa_bwd on the
+seeded inputs of 4 sequences x 4096 tokens, 24 q / 8 kv heads, and prints, for consecutive key blocks of ONE CTA in its
+steady state, the SM clock at which each pipeline event happened (relative to the first): when a softmax warp saw its
+accumulator, finished its phase, when the MMA warp saw the operand and had issued each MMA group.  The per-block period
+against the tensor cycles of a block (forward 2048 per tile pair, dK/dV 2048, dQ 768) is the kernel's tensor
+utilisation in steady state; the gaps between events say where the rest goes.  A measurement aid:
+it changes no result and is not part of the C ABI of include/lsp.h.
+"""
+from __future__ import annotations
+
+import argparse
+import ctypes as C
+import os
+import subprocess
+import sys
+import tempfile
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def build_traced(tmp):
+    from paper_2510_02483_b200 import build as Bd
+    out = os.path.join(tmp, "liblsp_trace.so")
+    cmd = [os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")] + Bd.NVCC_FLAGS + ["-DLSP_ATTN_TRACE", "-o", out] + Bd.SOURCES
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed:\n" + r.stdout + r.stderr)
+    return out
+
+
+def table(a, names, nblocks):
+    base = min(int(a[0, k]) for k in names if a[0, k])
+    print("block  " + "  ".join(f"{names[k]:>12s}" for k in sorted(names)))
+    for b in range(nblocks):
+        print(f"{b:5d}  " + "  ".join(f"{(int(a[b, k]) - base) if a[b, k] else -1:12d}" for k in sorted(names)))
+    first = sorted(names)[0]
+    per = [(int(a[b + 1, first]) - int(a[b, first])) for b in range(nblocks - 1) if a[b, first] and a[b + 1, first]]
+    per = sorted(p for p in per if p > 0)
+    if per:
+        print(f"median period between blocks: {per[len(per) // 2]} cycles")
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--blocks", type=int, default=24)
+    args = ap.parse_args(argv)
+    import numpy as np
+    import torch
+    from paper_2510_02483_b200 import binding as B
+    from paper_2510_02483_b200 import harness, synth
+    if not torch.cuda.is_available():
+        raise B.LspError("bench_trace.py needs a CUDA device")
+    with tempfile.TemporaryDirectory() as tmp:
+        B.LIB_PATH = build_traced(tmp)                     # this process only; the product library is untouched
+        lib = B.lib()
+        lib.lsp_debug_read_trace.argtypes = [C.c_void_p, C.c_int]
+        lib.lsp_debug_read_trace.restype = C.c_int
+        w = synth.CFG5_ATTN[1].with_(batch=4)              # B 4 x S 4096, 24 q / 8 kv heads: the attention of config 2
+        ctx = harness.make_ctx(w, use_rope=False)
+        dev = torch.device("cuda")
+        t = {k: harness.bf16_to_device(v, dev) for k, v in synth.attn_inputs(w).items()}
+        Bz, S, nq, nkv, d = w.batch, w.seq, w.n_q_heads, w.n_kv_heads, w.head_dim
+        o = torch.empty((Bz, S, nq, d), dtype=torch.float32, device=dev)
+        lse = torch.empty((Bz, nq, S), dtype=torch.float32, device=dev)
+        dq = torch.empty_like(o)
+        dk = torch.empty((Bz, S, nkv, d), dtype=torch.float32, device=dev)
+        dv = torch.empty_like(dk)
+        ws = torch.empty(ctx.workspace_bytes, dtype=torch.uint8, device=dev)
+        buf = (C.c_ulonglong * (64 * 32))()
+
+        def read():
+            assert lib.lsp_debug_read_trace(buf, 64 * 32) == 0
+            return np.array(buf[:], dtype=np.uint64).reshape(64, 32)
+
+        for _ in range(3):
+            B.lsp_sdpa_fwd(ctx, t["q"], t["k"], t["v"], o, lse, ws)
+        torch.cuda.synchronize()
+        print("== attn_fwd_tc_kernel, CTA 3, key blocks 64.. of the CTA (tile 0 | tile 1 | MMA warp); 2048 tensor cycles per block and tile pair")
+        table(read(), {0: "t0 s_full", 1: "t0 loaded", 2: "t0 max", 3: "t0 P part 0", 4: "t0 P part 1", 8: "t1 s_full", 12: "t1 arrive",
+                       16: "mma P0", 17: "mma PV0", 19: "mma S0", 20: "mma P1", 21: "mma PV1", 23: "mma S1"}, args.blocks)
+        for _ in range(3):
+            B.lsp_sdpa_bwd(ctx, t["q"], t["k"], t["v"], o, lse, t["dO"], dq, dk, dv, ws)
+        torch.cuda.synchronize()
+        a = read()
+        print("\n== attn_bwd_dkdv_tc_kernel, CTA 5, blocks 16.. (softmax warp | MMA warp); 2048 tensor cycles per 128 x 128 block")
+        table(a, {2: "dpt_full", 3: "dS arrive", 19: "mma dS", 20: "dK issued", 21: "dPT issued"}, args.blocks)
+        print("\n== attn_bwd_dq_tc_kernel, CTA 7, blocks 96.. (softmax warp | MMA warp); 768 tensor cycles per 128 x 64 block")
+        table(a, {0: "sdp_full", 1: "dS arrive", 16: "mma dS", 17: "dQ issued", 18: "SdP+2 issued"}, args.blocks)
+        ctx.close()
+        del lib
+    return 0
+
+
+if __name__ == "__main__":
+    raise SystemExit(main())

@@ -54,13 +54,17 @@ constexpr float ATC_RESCALE_LOG2 = 8.0f;
 
 // Share of the forward's exponentials computed on the FMA pipe instead of the SFU, in quarters (0 = none ... 4 = all).
 // The 128 x 128 exponentials of a block occupy the SFU (16 results / clk / SM) for 1024 cycles -- exactly the tensor time
-// of the block's two MMAs.  Measured on B200 (profiles/r2_attn_fwd_trace.md): the polynomial costs 8 FP32-pipe pair
+// of the block's two MMAs.  Measured on B200 (profiles/r2_attn_traces.txt, profiles/r2_notes.md): the polynomial costs 8 FP32-pipe pair
 // instructions + 2 IMAD per key pair and FFMA2 / FADD2 issue at 4 cycles per warp instruction, so per block and SM
 // sub-partition the FMA pipe needs 64 (36 f + 8 (1 - f)) cycles against 1024 (1 - f) on the SFU: 0 -> 512 / 1024,
 // 1/4 -> 960 / 768, 1/2 -> 1408 / 512.  One pair in four is the balance point (forward kernel 0.541 / 0.529 / 0.532 /
 // 0.572 ms inside the cfg2 step for 0 / 1 / 2 / 3 quarters).
 #ifndef LSP_ATTN_POLY_EXP
 #define LSP_ATTN_POLY_EXP 1
+#endif
+// the same for the P^T phase of the dK/dV kernel (0 = all on the SFU, 1 = one key pair in four on the FMA pipe)
+#ifndef LSP_ATTN_BWD_POLY_EXP
+#define LSP_ATTN_BWD_POLY_EXP 1
 #endif
 
 // 2^x for a pair of values <= ~2^8 without the SFU: x clamped at -126 (masked keys are -inf; a clamped value ends as
@@ -193,7 +197,7 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
   auto v_full = [&](int s) { return bar_base + 8u * (6 + s); };
   auto v_empty = [&](int s) { return bar_base + 8u * (8 + s); };
   auto s_full = [&](int t) { return bar_base + 8u * (10 + t); };
-  auto p_full = [&](int t) { return bar_base + 8u * (12 + t); };
+  auto p_full = [&](int t, int part) { return bar_base + 8u * ((part ? 28 : 12) + t); };   // P_t, first / second 32 keys of both halves
   auto o_full = [&](int t) { return bar_base + 8u * (14 + t); };
   auto q_empty = [&](int t) { return bar_base + 8u * (16 + t); };
   auto o_free = [&](int t) { return bar_base + 8u * (18 + t); };
@@ -215,7 +219,7 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
       mbar_init(q_full(i), 1); mbar_init(q_empty(i), 1);
       mbar_init(k_full(i), 1); mbar_init(k_empty(i), 1);
       mbar_init(v_full(i), 1); mbar_init(v_empty(i), 1);
-      mbar_init(s_full(i), 1); mbar_init(p_full(i), 8); mbar_init(o_full(i), 1); mbar_init(o_free(i), 8);
+      mbar_init(s_full(i), 1); mbar_init(p_full(i, 0), 8); mbar_init(p_full(i, 1), 8); mbar_init(o_full(i), 1); mbar_init(o_free(i), 8);
     }
     for (int i = 0; i < ATC_ITEM_RING; ++i) mbar_init(item_bar(i), 1);
     fence_barrier_init();
@@ -292,14 +296,18 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
     };
     // P_t: keys [64 h, 64 h + 64) of the block are the 32 columns [64 h, 64 h + 32) of S_t (each column half stays
     // inside the columns its own warp read), so K step kk reads columns 64 (kk / 4) + 8 (kk % 4)
-    auto issue_pv = [&](int t, int vst, bool acc) {
+    // P_t is handed over in two parts (the first / second 32 keys of both column halves = K steps {0,1,4,5} / {2,3,6,7}):
+    // the first half of P V runs while the second half of P is still being exponentiated
+    auto issue_pv = [&](int t, int vst, bool acc, int part) {
       if (leader) {
         const uint64_t va = desc_adv(dv0, vst * ATC_TILE_BYTES);
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk)
+        for (int e = 0; e < 4; ++e) {
+          const int kk = (e >> 1) * 4 + part * 2 + (e & 1);
           umma_f16_ts(tmem_base + 256 + t * 128, tmem_base + t * 128 + (kk >> 2) * 64 + (kk & 3) * 8, desc_adv(va, kk * 2048), idesc_pv,
-                      (acc || kk != 0) ? 1u : 0u);
-        umma_commit(o_full(t));
+                      (acc || part != 0 || e != 0) ? 1u : 0u);
+        }
+        if (part == 1) umma_commit(o_full(t));
       }
     };
     uint32_t kvc = 0;                          // K/V blocks consumed so far (ring position of this item's block 0)
@@ -336,12 +344,15 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
 #pragma unroll
         for (int t = 0; t < 2; ++t) {
           if (j < nt[t]) {
-            mbar_wait(p_full(t), pc[t] & 1u);
+            mbar_wait(p_full(t, 0), pc[t] & 1u);
             if (lane == 0) ATC_TR(pc[t], 16 + 4 * t);
-            ++pc[t];
             if (j == 0 && qc[t] > 0) mbar_wait(o_free(t), (qc[t] - 1u) & 1u);   // previous item's O_t has been read out
             tc_fence_after();
-            issue_pv(t, st, j > 0);
+            issue_pv(t, st, j > 0, 0);
+            mbar_wait(p_full(t, 1), pc[t] & 1u);
+            ++pc[t];
+            tc_fence_after();
+            issue_pv(t, st, j > 0, 1);
             if (lane == 0) ATC_TR(pc[t] - 1, 17 + 4 * t);
           }
           if (j + 1 < nt[t]) {
@@ -477,14 +488,13 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
             pk[i] = pack_f16(a.x, a.y);
           }
           tmem_st16(tS + q * 16, pk);                            // P_t: keys 64 h + 32 q .. + 31 -> 16 columns
+          tmem_st_wait();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(p_full(t, q));
+          if (tr) ATC_TR(cnt, 3 + q + 8 * t);
         }
         l_run += (acc0.x + acc0.y) + (acc1.x + acc1.y);
-        if (tr) ATC_TR(cnt, 3 + 8 * t);
-        tmem_st_wait();
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(p_full(t));
-        if (tr) ATC_TR(cnt, 4 + 8 * t);
       }
 
       // epilogue of this tile: the row sum of both halves (fixed order: half 0 + half 1), then O_t / l -> o32, o16 (through
@@ -698,15 +708,15 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
   auto acc_full = [&]() { return bar_base + 8u; };
   auto st_full = [&]() { return bar_base + 16u; };               // MMA: S^T of the block has landed
   auto dpt_full = [&]() { return bar_base + 24u; };              // MMA: dP^T of the block has landed
-  auto p_full = [&]() { return bar_base + 32u; };                // 8 softmax warps: P^T written
-  auto ds_full = [&]() { return bar_base + 40u; };               // 8 softmax warps: dS^T written
-  auto q_full = [&](int s) { return bar_base + 8u * (6 + s); };
-  auto q_empty = [&](int s) { return bar_base + 8u * (6 + ATC_KV_QST + s); };
-  auto do_full = [&](int s) { return bar_base + 8u * (6 + 2 * ATC_KV_QST + s); };
-  auto do_empty = [&](int s) { return bar_base + 8u * (6 + 2 * ATC_KV_QST + ATC_KV_DST + s); };
-  auto ld_full = [&](int s) { return bar_base + 8u * (6 + 2 * ATC_KV_QST + 2 * ATC_KV_DST + s); };
-  auto ld_empty = [&](int s) { return bar_base + 8u * (8 + 2 * ATC_KV_QST + 2 * ATC_KV_DST + s); };
-  const uint32_t tmem_slot = bar_base + 8u * (10 + 2 * ATC_KV_QST + 2 * ATC_KV_DST);
+  auto p_full = [&](int q) { return bar_base + 32u + 8u * q; };  // 8 softmax warps: P^T of query quarter-pair q written (q = 0, 1)
+  auto ds_full = [&]() { return bar_base + 48u; };               // 8 softmax warps: dS^T written
+  auto q_full = [&](int s) { return bar_base + 8u * (7 + s); };
+  auto q_empty = [&](int s) { return bar_base + 8u * (7 + ATC_KV_QST + s); };
+  auto do_full = [&](int s) { return bar_base + 8u * (7 + 2 * ATC_KV_QST + s); };
+  auto do_empty = [&](int s) { return bar_base + 8u * (7 + 2 * ATC_KV_QST + ATC_KV_DST + s); };
+  auto ld_full = [&](int s) { return bar_base + 8u * (7 + 2 * ATC_KV_QST + 2 * ATC_KV_DST + s); };
+  auto ld_empty = [&](int s) { return bar_base + 8u * (9 + 2 * ATC_KV_QST + 2 * ATC_KV_DST + s); };
+  const uint32_t tmem_slot = bar_base + 8u * (11 + 2 * ATC_KV_QST + 2 * ATC_KV_DST);
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_base));
 
   const int warp = warp_idx_uniform(), lane = threadIdx.x & 31;
@@ -732,7 +742,7 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
   if (threadIdx.x == 0) {
     tma_prefetch_desc(&maps.q); tma_prefetch_desc(&maps.k); tma_prefetch_desc(&maps.v); tma_prefetch_desc(&maps.dO);
     mbar_init(kv_full(), 1); mbar_init(acc_full(), 1); mbar_init(st_full(), 1); mbar_init(dpt_full(), 1);
-    mbar_init(p_full(), 8); mbar_init(ds_full(), 8);
+    mbar_init(p_full(0), 8); mbar_init(p_full(1), 8); mbar_init(ds_full(), 8);
     for (int i = 0; i < ATC_KV_QST; ++i) { mbar_init(q_full(i), 1); mbar_init(q_empty(i), 1); }
     for (int i = 0; i < ATC_KV_DST; ++i) { mbar_init(do_full(i), 1); mbar_init(do_empty(i), 1); }
     for (int i = 0; i < 2; ++i) { mbar_init(ld_full(i), 32); mbar_init(ld_empty(i), 8); }
@@ -823,21 +833,31 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
       const uint32_t ph = it & 1;
       const uint64_t qa = desc_adv(dQm, qs * ATC_TILE_BYTES), da = desc_adv(dDOm, ds * ATC_TILE_BYTES);
       const bool split = split_block(kb + it % per_head);
-      // each MMA group needs two barriers -- the softmax threads' operand and the next block's tile: polled together
-      if (it + 1 < iters) mbar_wait2(p_full(), ph, q_full((it + 1) % ATC_KV_QST), ((it + 1) / ATC_KV_QST) & 1);
-      else mbar_wait(p_full(), ph);
+      // each MMA group needs two barriers -- the softmax threads' operand and the next block's tile: polled together.
+      // P^T arrives in two parts (the first / second 32 queries of both query halves = K steps {0,1,4,5} / {2,3,6,7}): the
+      // first half of dV runs while the second half of P^T is still being exponentiated
+      if (it + 1 < iters) mbar_wait2(p_full(0), ph, q_full((it + 1) % ATC_KV_QST), ((it + 1) / ATC_KV_QST) & 1);
+      else mbar_wait(p_full(0), ph);
       if (lane == 0) ATC_TR2(it, 16);
-      tc_fence_after();
-      if (leader) {
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk)                                // dV += P^T dO
-          umma_f16_ts(tmem_base + 256, tmem_base + opcol(kk), desc_adv(da, kk * 2048), idesc_acc, (it | kk) != 0 ? 1u : 0u);
-        if (split) {
+      for (int part = 0; part < 2; ++part) {
+        if (part == 1) mbar_wait(p_full(1), ph);
+        tc_fence_after();
+        if (leader) {
 #pragma unroll
-          for (int kk = 0; kk < 8; ++kk)                              // ... + (P^T)_lo dO
-            umma_f16_ts(tmem_base + 256, tmem_base + 32 + opcol(kk), desc_adv(da, kk * 2048), idesc_acc, 1u);
+          for (int e = 0; e < 4; ++e) {                               // dV += P^T dO
+            const int kk = (e >> 1) * 4 + part * 2 + (e & 1);
+            umma_f16_ts(tmem_base + 256, tmem_base + opcol(kk), desc_adv(da, kk * 2048), idesc_acc, (it | part | e) != 0 ? 1u : 0u);
+          }
+          if (split) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {                             // ... + (P^T)_lo dO
+              const int kk = (e >> 1) * 4 + part * 2 + (e & 1);
+              umma_f16_ts(tmem_base + 256, tmem_base + 32 + opcol(kk), desc_adv(da, kk * 2048), idesc_acc, 1u);
+            }
+          }
+          if (part == 1) umma_commit(do_empty(ds));                   // dO(it) was last read by these MMAs
         }
-        umma_commit(do_empty(ds));                                    // dO(it) was last read by these MMAs
       }
       if (lane == 0) ATC_TR2(it, 17);
       if (it + 1 < iters) issue_st(it + 1);                           // overwrites P^T(it): behind dV in the tensor queue
@@ -886,47 +906,54 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
         uint32_t sr[2][32];
         tmem_ld32(tST, sr[0]);
         tmem_ld32(tST + 32, sr[1]);
-        tmem_ld_wait();
-        const float4* l4 = reinterpret_cast<const float4*>(sLD_ptr + ls * 256 + col0);
+        tmem_ld_wait();                                                // all 64 columns in registers before any of them is overwritten
+        const float2 c2 = make_float2(c, c);
 #pragma unroll
-        for (int i = 0; i < 16; ++i) {
-          const float4 L = l4[i];
-          pv[4 * i] = ex2_approx(fmaf(__uint_as_float(sr[i >> 3][(4 * i) & 31]), c, -L.x));
-          pv[4 * i + 1] = ex2_approx(fmaf(__uint_as_float(sr[i >> 3][(4 * i + 1) & 31]), c, -L.y));
-          pv[4 * i + 2] = ex2_approx(fmaf(__uint_as_float(sr[i >> 3][(4 * i + 2) & 31]), c, -L.z));
-          pv[4 * i + 3] = ex2_approx(fmaf(__uint_as_float(sr[i >> 3][(4 * i + 3) & 31]), c, -L.w));
+        for (int q = 0; q < 2; ++q) {                                  // two parts of 32 queries, handed over separately
+          const float4* l4 = reinterpret_cast<const float4*>(sLD_ptr + ls * 256 + col0 + 32 * q);
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const float4 L = l4[i];
+            float2 a = ffma2(make_float2(__uint_as_float(sr[q][4 * i]), __uint_as_float(sr[q][4 * i + 1])), c2, make_float2(-L.x, -L.y));
+            float2 b2 = ffma2(make_float2(__uint_as_float(sr[q][4 * i + 2]), __uint_as_float(sr[q][4 * i + 3])), c2, make_float2(-L.z, -L.w));
+            if (LSP_ATTN_BWD_POLY_EXP && (i & 1) == 0) {               // one key pair in four on the FMA pipe (the phase is SFU-bound)
+              a = ex2_poly2(a);
+            } else {
+              a.x = ex2_approx(a.x); a.y = ex2_approx(a.y);
+            }
+            b2.x = ex2_approx(b2.x); b2.y = ex2_approx(b2.y);
+            pv[32 * q + 4 * i] = a.x; pv[32 * q + 4 * i + 1] = a.y; pv[32 * q + 4 * i + 2] = b2.x; pv[32 * q + 4 * i + 3] = b2.y;
+          }
+          if (rel == 0) {                                              // diagonal block: query (col0 + 32 q + i) < key (row) is masked
+#pragma unroll
+            for (int i = 0; i < 32; ++i)
+              if (col0 + 32 * q + i < row) pv[32 * q + i] = 0.f;
+          }
+          if (doc_end) {                                               // packed sequences: queries of later sequences
+            const int qabs = (kb + rel) * 128 + col0 + 32 * q;
+            if (__any_sync(0xffffffffu, qabs + 31 >= dend)) {
+#pragma unroll
+              for (int i = 0; i < 32; ++i)
+                if (qabs + i >= dend) pv[32 * q + i] = 0.f;
+            }
+          }
+          uint32_t pk[16];
+          if (split) {
+            uint32_t pl[16];
+#pragma unroll
+            for (int i = 0; i < 16; ++i) atc_split_pack(pv[32 * q + 2 * i], pv[32 * q + 2 * i + 1], pk[i], pl[i]);
+            tmem_st16(tST + 32 + 16 * q, pl);
+          } else {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) pk[i] = pack_f16(pv[32 * q + 2 * i], pv[32 * q + 2 * i + 1]);
+          }
+          tmem_st16(tST + 16 * q, pk);
+          tmem_st_wait();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(p_full(q));
         }
       }
-      if (rel == 0) {                                                  // diagonal block: query (col0 + i) < key (row) is masked
-#pragma unroll
-        for (int i = 0; i < 64; ++i)
-          if (col0 + i < row) pv[i] = 0.f;
-      }
-      if (doc_end) {                                                   // packed sequences: queries of later sequences
-        const int qabs = (kb + rel) * 128 + col0;
-        if (__any_sync(0xffffffffu, qabs + 63 >= dend)) {
-#pragma unroll
-          for (int i = 0; i < 64; ++i)
-            if (qabs + i >= dend) pv[i] = 0.f;
-        }
-      }
-      {
-        uint32_t pk[32];
-        if (split) {
-          uint32_t pl[32];
-#pragma unroll
-          for (int i = 0; i < 32; ++i) atc_split_pack(pv[2 * i], pv[2 * i + 1], pk[i], pl[i]);
-          tmem_st32(tST + 32, pl);
-        } else {
-#pragma unroll
-          for (int i = 0; i < 32; ++i) pk[i] = pack_f16(pv[2 * i], pv[2 * i + 1]);
-        }
-        tmem_st32(tST, pk);
-      }
-      tmem_st_wait();
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(p_full());
       if (tr) ATC_TR2(it, 1);
       // dS^T = P^T (dP^T - D)
       mbar_wait(dpt_full(), ph);

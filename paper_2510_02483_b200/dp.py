@@ -9,6 +9,10 @@ backward has been enqueued and overlaps the backward of the next layer; `wait()`
 them.  No averaging pass exists: every rank carries its gradients scaled by its local token count T_local (section 13
 of DESIGN.md), the sum over ranks is T_local * world * (gradient of the global mean loss), and that factor is handed to
 lsp_adamw_step as grad_scale (`global_grad_scale`).  The sum runs in fp32 in the order the backend fixes.
+
+UNMEASURED ON HARDWARE: rounds 1 and 2 had one GPU.  No NCCL rank has run this module; "overlaps the backward of the next
+layer" describes how the calls are ordered (the collective is enqueued behind the bucket's backward and runs on the
+backend's stream), not a timing that was taken.  Covered by the world_size-2 gloo tests of tests/test_dp_gloo.py only.
 """
 from __future__ import annotations
 

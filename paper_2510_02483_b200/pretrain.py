@@ -33,6 +33,12 @@ class PretrainStep:
         backward (one shared `saved` buffer instead of n_layers: activation memory / n_layers for one more forward);
         zero1: optimizer state sharded over the `world` replicas (dp.Zero1State), `rank` = this replica."""
         self.dev = dev or harness.require_cuda()
+        if world > 1:
+            # The persistent GEMMs cut the last wave's tiles into K-slices whose consumer CTA pairs wait for producer pairs of
+            # the SAME grid: safe while the whole grid is co-resident, which nothing guarantees once a collective's kernels
+            # hold SMs at the same time (never run on more than one GPU: DESIGN.md section 14).  Data-parallel only until then.
+            import os
+            os.environ.setdefault("LSP_GEMM_STREAMK", "0")
         self.w, self.L, self.V = w, n_layers, vocab
         self.ctx = harness.make_ctx(w, in_dtype=B.LSP_F32)
         self.n_micro = micro_batches

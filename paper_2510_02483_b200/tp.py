@@ -13,6 +13,9 @@ Weight gradients stay local (each rank owns its slice).
 
 One process per GPU with torch.distributed (NCCL over NVLink 5 / NVSwitch); without a process group the all-reduces are
 the identity, and `phases()` lets a test drive several shards one after the other on one GPU and add their partials.
+
+UNMEASURED ON HARDWARE: rounds 1 and 2 had one GPU; the shards' algebra is tested (sequentially, on one GPU), the four
+all-reduces have never run over NCCL and nothing is claimed about their cost.
 """
 from __future__ import annotations
 
