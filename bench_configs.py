@@ -51,6 +51,7 @@ def bench_layer(w, steps, logical_head_dim=0):
     else:
         wl = w
         weights = harness.upload_weights(synth.layer_weights(w), dev)
+    weights = harness.with_weight_cache(ctx, weights, dev)          # unchanged between steps: fp16 operand copies made once (as bench.py)
     inp = synth.layer_inputs(w)
     x, dy = harness.bf16_to_device(inp["x"], dev), harness.bf16_to_device(inp["dy"], dev)
 
@@ -68,7 +69,7 @@ def bench_layer_packed(w, steps, cu):
     dev = harness.require_cuda()
     ctx = harness.make_ctx(w)
     buf = harness.LayerBuffers(ctx, w, dev)
-    weights = harness.upload_weights(synth.layer_weights(w), dev)
+    weights = harness.with_weight_cache(ctx, harness.upload_weights(synth.layer_weights(w), dev), dev)
     inp = synth.layer_inputs(w)
     x, dy = harness.bf16_to_device(inp["x"], dev), harness.bf16_to_device(inp["dy"], dev)
     B.lsp_set_packed_sequences(ctx, cu)
@@ -90,7 +91,7 @@ def bench_layer_fwd_only(w, steps, infer=False):
     dev = harness.require_cuda()
     ctx = harness.make_ctx(w)
     buf = harness.LayerBuffers(ctx, w, dev)
-    weights = harness.upload_weights(synth.layer_weights(w), dev)
+    weights = harness.with_weight_cache(ctx, harness.upload_weights(synth.layer_weights(w), dev), dev)
     x = harness.bf16_to_device(synth.layer_inputs(w)["x"], dev)
     fn = B.lsp_layer_fwd_infer if infer else B.lsp_layer_fwd
     ms = _time(lambda: fn(ctx, x, weights, buf.y, buf.saved, buf.ws), steps)
@@ -101,7 +102,7 @@ def bench_layer_fwd_only(w, steps, infer=False):
 def bench_stack(w, steps):
     """Config 3: embedding gather + n_layers x (fwd) + n_layers x (bwd); every layer has its own seeded weights."""
     dev = harness.require_cuda()
-    run = harness.StackRunner(w, w.n_layers, dev)
+    run = harness.StackRunner(w, w.n_layers, dev, cache_weights=True)
     s = synth.stack_inputs(w)
     ids = torch.from_numpy(s["ids"]).to(dev)
     table = harness.bf16_to_device(s["embedding"], dev)

@@ -118,7 +118,9 @@ class StackRunner:
     The residual stream between layers is fp32 (in_dtype = LSP_F32); every layer keeps its own `saved` bundle, the
     workspace is shared.  Host-side sequencing only -- every step runs in the library's kernels."""
 
-    def __init__(self, w: synth.Workload, n_layers: int, dev=None):
+    def __init__(self, w: synth.Workload, n_layers: int, dev=None, cache_weights: bool = False):
+        """cache_weights: hand every layer its fp16 operand cache (lsp_layer_prepare_weights once, here) -- the weights of
+        the stack do not change between calls, so no forward launches a weight cast."""
         self.dev = dev or require_cuda()
         self.w, self.L = w, n_layers
         self.ctx = make_ctx(w, in_dtype=B.LSP_F32)
@@ -129,6 +131,8 @@ class StackRunner:
         self.xs = [torch.empty((T, H), **f32) for _ in range(n_layers + 1)]
         self.d = [torch.empty((T, H), **f32) for _ in range(2)]
         self.weights = [upload_weights(synth.layer_weights(w, layer), self.dev) for layer in range(n_layers)]
+        if cache_weights:
+            self.weights = [with_weight_cache(self.ctx, wl, self.dev) for wl in self.weights]
         self.grads = {k: torch.empty(s, **f32) for k, s in WEIGHT_SHAPES(w).items()}
 
     def forward(self, ids: torch.Tensor, table: torch.Tensor, stream=None):
