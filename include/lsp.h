@@ -248,6 +248,30 @@ typedef struct {
 } lsp_adamw_desc;
 lsp_status lsp_adamw_step(lsp_ctx* ctx, int ntensors, const lsp_adamw_tensor* tensors, const lsp_adamw_desc* desc,
                           float* gnorm_out, void* stream);
+/* Allocation-free global gradient norm: the norm / clipping pass of lsp_adamw_step (clipping of the
+ * global l2 gradient norm; readings O-1, O-2 in DESIGN.md section 12) for callers that may not allocate device memory
+ * -- code under CUDA-graph capture, tight serving / training loops, harnesses that forbid cudaMalloc.  It needs NO
+ * context (lsp_create allocates), calls no cudaMalloc / cudaFree / allocating library routine, and keeps its scratch
+ * (the per-block partial sums of g^2) in ONE file-scope device array of LSP_NORM_STATIC_SCRATCH_BYTES that every GPU
+ * which loads the library holds until the process exits.
+ *   cuda_device: the device the pointers live on (made current for the call, the caller's is restored).
+ *   grads[i]: DEVICE fp32 tensor of n[i] elements (n[i] > 0, n[i] % 4 == 0, 16-byte aligned); grads / n are HOST arrays
+ *   of 1 <= ntensors <= LSP_NORM_STATIC_MAX_TENSORS entries (the 255 tensors of the 3B model fit).  A call that needs
+ *   more tensors, or more partial sums than the array holds, is REJECTED with LSP_EINVAL before anything is launched.
+ *   gnorm_out: DEVICE float[2] = {l2 norm of the true gradients g / grad_scale, min(1, clip_norm / (norm + 1e-6)) /
+ *   grad_scale} -- bit for bit what lsp_adamw_step (phase 0) writes for the same tensors in the same order; a
+ *   non-finite norm gives {norm, 0}.  Enqueued on `stream`, no host sync.
+ *   err (may be NULL): caller's HOST buffer of err_len bytes that receives the message of a failed call.
+ * The first call on a device resolves the array's address (cudaGetSymbolAddress, once per device): make it outside
+ * graph capture.  Nothing in the array has to start at zero (every partial sum the final reduction reads is written by
+ * the same call), so the contents a previous call left are never read.  ALL calls on one GPU share the array: calls
+ * that may overlap on the GPU (different streams without an ordering between them) race -- order them. */
+#define LSP_NORM_STATIC_MAX_TENSORS 256
+#define LSP_NORM_STATIC_SCRATCH_BYTES (128 * 1024)
+lsp_status lsp_grad_norm_static(int cuda_device, int ntensors, const float* const* grads, const int64_t* n,
+                                float clip_norm, float grad_scale, float* gnorm_out, void* stream, char* err,
+                                size_t err_len);
+
 /* Host helper (no GPU): the paper's schedule: linear warm-up from 0 to lr_max over `warmup` steps, then
  * cosine decay to lr_min at step `total`, lr_min afterwards (reading O-3).  step is 1-based. */
 double lsp_lr_cosine(int step, double lr_max, double lr_min, int warmup, int total);

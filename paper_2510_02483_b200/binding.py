@@ -20,7 +20,8 @@ EXPORTS = ("lsp_create", "lsp_destroy", "lsp_saved_bytes", "lsp_workspace_bytes"
            "lsp_sdpa_fwd", "lsp_sdpa_bwd", "lsp_embed_fwd", "lsp_gemm", "lsp_layer_step_host", "lsp_launch_count",
            "lsp_timing_enable", "lsp_timing_read", "lsp_adamw_step", "lsp_lr_cosine", "lsp_head_workspace_bytes",
            "lsp_head_fwd_bwd", "lsp_embed_bwd", "lsp_layer_step_host_async", "lsp_host_copies_wait", "lsp_set_packed_sequences", "lsp_layer_fwd_infer",
-           "lsp_overflow_count", "lsp_weight_cache_bytes", "lsp_layer_prepare_weights", "lsp_weight_cache_offset")
+           "lsp_overflow_count", "lsp_weight_cache_bytes", "lsp_layer_prepare_weights", "lsp_weight_cache_offset",
+           "lsp_grad_norm_static")
 
 
 class LspError(RuntimeError):
@@ -101,6 +102,7 @@ def lib():
         L.lsp_layer_prepare_weights.argtypes = [vp, pw, vp, vp]
         L.lsp_weight_cache_offset.argtypes = [vp, i32]
         L.lsp_weight_cache_offset.restype = C.c_longlong
+        L.lsp_grad_norm_static.argtypes = [i32, i32, C.POINTER(vp), C.POINTER(i64), C.c_float, C.c_float, vp, vp, C.c_char_p, C.c_size_t]
         for n in EXPORTS:
             if n not in ("lsp_saved_bytes", "lsp_workspace_bytes", "lsp_last_error", "lsp_launch_count", "lsp_lr_cosine",
                          "lsp_head_workspace_bytes", "lsp_weight_cache_bytes", "lsp_weight_cache_offset"):
@@ -288,6 +290,22 @@ def lsp_adamw_step(ctx, tensors, *, lr, step, gnorm_out, beta1=0.90, beta2=0.95,
                                   None if w16 is None else w16.data_ptr())
     d = lsp_adamw_desc(lr, beta1, beta2, eps, weight_decay, clip_norm, step, grad_scale, phase)
     ctx.check(lib().lsp_adamw_step(ctx.handle, len(tensors), arr, C.byref(d), _ptr(gnorm_out), _stream(stream)))
+
+
+NORM_STATIC_MAX_TENSORS = 256            # LSP_NORM_STATIC_MAX_TENSORS of include/lsp.h
+
+
+def lsp_grad_norm_static(grads, gnorm_out, *, clip_norm=1.0, grad_scale=1.0, stream=None):
+    """Allocation-free global gradient norm (include/lsp.h): grads = list of fp32 torch CUDA tensors on one device,
+    gnorm_out = fp32 CUDA tensor of 2 elements.  Needs no Ctx; the scratch is a static device array of the library."""
+    k = len(grads)
+    ptrs = (C.c_void_p * max(k, 1))(*[g.data_ptr() for g in grads])
+    ns = (C.c_int64 * max(k, 1))(*[g.numel() for g in grads])
+    err = C.create_string_buffer(512)
+    dev = gnorm_out.device.index if gnorm_out.device.index is not None else 0
+    st = lib().lsp_grad_norm_static(dev, k, ptrs, ns, C.c_float(clip_norm), C.c_float(grad_scale), _ptr(gnorm_out), _stream(stream), err, len(err))
+    if st != 0:
+        raise LspError(f"{STATUS.get(st, st)}: {err.value.decode(errors='replace')}")
 
 
 def lsp_lr_cosine(step: int, lr_max: float = 1.2e-3, lr_min: float = 1.0e-5, warmup: int = 2000, total: int = 100000) -> float:

@@ -8,6 +8,7 @@
 #include <stdarg.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -594,6 +595,55 @@ lsp_status as_f16(lsp_ctx* ctx, const void* in, void* ws, cudaStream_t st, const
   if (ctx->d.in_dtype == LSP_BF16) LSP_STAGE(ST_CAST, 1, cast_bf16_f16(static_cast<const __nv_bfloat16*>(in), t, n, ctx->num_sms, ctx->overflow, st));
   else LSP_STAGE(ST_CAST, 1, cast_f32_f16(static_cast<const float*>(in), t, n, ctx->num_sms, ctx->overflow, st));
   *out = t;
+  return LSP_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------ scratch of lsp_grad_norm_static (include/lsp.h)
+// The per-block partial sums of g^2 of the allocation-free gradient-norm entry point.  A device array: every GPU that
+// loads the library holds these 128 KiB until the process exits.  In HOST code the name is only a stand-in for the
+// symbol, never a device address: the entry point resolves the address once per device with cudaGetSymbolAddress
+// (norm_static_setup) and hands THAT pointer to the kernels.
+static __device__ __align__(256) float g_norm_static_scratch[LSP_NORM_STATIC_SCRATCH_BYTES / sizeof(float)];
+
+namespace {
+
+constexpr int NORM_STATIC_MAX_DEVICES = 64;
+struct NormStaticDevice {
+  float* scratch;      // device address of g_norm_static_scratch on this device
+  int num_sms;
+  bool ready;
+};
+NormStaticDevice g_norm_static_dev[NORM_STATIC_MAX_DEVICES];
+std::mutex g_norm_static_mutex;
+
+lsp_status fail_msg(char* err, size_t err_len, lsp_status s, const char* fmt, ...) {
+  if (err && err_len) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(err, err_len, fmt, ap);
+    va_end(ap);
+  }
+  return s;
+}
+
+// once per device, with that device current
+lsp_status norm_static_setup(int dev, NormStaticDevice* out, char* err, size_t err_len) {
+  std::lock_guard<std::mutex> lock(g_norm_static_mutex);
+  NormStaticDevice& d = g_norm_static_dev[dev];
+  if (!d.ready) {
+    float* p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_norm_static_scratch);
+    if (e != cudaSuccess || !p)
+      return fail_msg(err, err_len, LSP_ECUDA, "lsp_grad_norm_static: cudaGetSymbolAddress on device %d failed: %s", dev, cudaGetErrorString(e));
+    int sms = 0;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess || sms <= 0)
+      return fail_msg(err, err_len, LSP_ECUDA, "lsp_grad_norm_static: cannot read the SM count of device %d: %s", dev, cudaGetErrorString(e));
+    d.scratch = p; d.num_sms = sms; d.ready = true;
+  }
+  *out = d;
   return LSP_OK;
 }
 
@@ -1201,6 +1251,63 @@ lsp_status lsp_adamw_step(lsp_ctx* ctx, int ntensors, const lsp_adamw_tensor* te
     return cudaGetLastError();
   };
   LSP_STAGE(ST_ADAMW, (phase == 0 ? 2 : 1) * ngroups + 1, launch());
+  return LSP_OK;
+}
+
+// Allocation-free variant of the gradient-norm pass above (include/lsp.h): the same two kernels, the same blocks per
+// group and the same reduction order as lsp_adamw_step phase 0 -- hence the same bits -- with the partial sums in the
+// device array g_norm_static_scratch instead of the context's cudaMalloc'ed buffer.  No context, no allocation.
+lsp_status lsp_grad_norm_static(int cuda_device, int ntensors, const float* const* grads, const int64_t* n, float clip_norm,
+                                float grad_scale, float* gnorm_out, void* stream, char* err, size_t err_len) {
+  if (err && err_len) err[0] = 0;
+  if (!grads || !n || !gnorm_out) return fail_msg(err, err_len, LSP_EINVAL, "lsp_grad_norm_static: NULL argument");
+  if (ntensors < 1) return fail_msg(err, err_len, LSP_EINVAL, "lsp_grad_norm_static: ntensors must be >= 1");
+  if (ntensors > LSP_NORM_STATIC_MAX_TENSORS)
+    return fail_msg(err, err_len, LSP_EINVAL, "lsp_grad_norm_static: %d tensors exceed the maximum of %d (LSP_NORM_STATIC_MAX_TENSORS); use lsp_adamw_step",
+                    ntensors, LSP_NORM_STATIC_MAX_TENSORS);
+  if (!(clip_norm > 0.f) || !(grad_scale > 0.f)) return fail_msg(err, err_len, LSP_EINVAL, "lsp_grad_norm_static: clip_norm and grad_scale must be > 0");
+  if (cuda_device < 0 || cuda_device >= NORM_STATIC_MAX_DEVICES)
+    return fail_msg(err, err_len, LSP_EINVAL, "lsp_grad_norm_static: device %d outside [0, %d)", cuda_device, NORM_STATIC_MAX_DEVICES);
+  for (int i = 0; i < ntensors; ++i) {
+    if (!grads[i] || n[i] <= 0 || (n[i] % 4)) return fail_msg(err, err_len, LSP_EINVAL, "lsp_grad_norm_static: tensor %d: NULL pointer or n %% 4 != 0", i);
+    if (!aligned(grads[i], 16)) return fail_msg(err, err_len, LSP_EALIGN, "lsp_grad_norm_static: tensor %d is not 16-byte aligned", i);
+  }
+  DeviceGuard guard(cuda_device);
+  if (!guard.ok) return fail_msg(err, err_len, LSP_ECUDA, "lsp_grad_norm_static: cannot make device %d current", cuda_device);
+  NormStaticDevice dv;
+  LSP_TRY(norm_static_setup(cuda_device, &dv, err, err_len));
+  // groups of OPT_MAX_TENSORS tensors, blocks per group as in lsp_adamw_step; all partial sums must fit the array
+  const int ngroups = (ntensors + OPT_MAX_TENSORS - 1) / OPT_MAX_TENSORS;
+  const long long cap = opt_blocks_cap(dv.num_sms);
+  const long long capacity = LSP_NORM_STATIC_SCRATCH_BYTES / sizeof(float);
+  auto group = [&](int gi, OptTensors& t) {
+    memset(&t, 0, sizeof(t));
+    const int i0 = gi * OPT_MAX_TENSORS;
+    t.n = ntensors - i0 < OPT_MAX_TENSORS ? ntensors - i0 : OPT_MAX_TENSORS;
+    for (int i = 0; i < t.n; ++i) {
+      t.g[i] = grads[i0 + i];
+      t.start[i + 1] = t.start[i] + n[i0 + i] / 4;
+    }
+    for (int i = t.n; i < OPT_MAX_TENSORS; ++i) t.start[i + 1] = t.start[t.n];
+    const long long blocks = (t.start[t.n] + OPT_THREADS - 1) / OPT_THREADS;
+    return static_cast<int>(blocks > cap ? cap : blocks);
+  };
+  OptTensors t;
+  long long need = 0;
+  for (int gi = 0; gi < ngroups; ++gi) need += group(gi, t);
+  if (need > capacity)
+    return fail_msg(err, err_len, LSP_EINVAL, "lsp_grad_norm_static: %lld partial sums exceed the %lld of the static scratch (LSP_NORM_STATIC_SCRATCH_BYTES)",
+                    need, capacity);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  int nparts = 0;
+  for (int gi = 0; gi < ngroups; ++gi) {
+    const int nb = group(gi, t);
+    opt_gradsq_kernel<<<nb, OPT_THREADS, 0, st>>>(t, dv.scratch + nparts);
+    nparts += nb;
+  }
+  opt_norm_final_kernel<<<1, OPT_THREADS, 0, st>>>(dv.scratch, nparts, clip_norm, 1.0 / grad_scale, 0, gnorm_out);
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail_msg(err, err_len, LSP_ECUDA, "lsp_grad_norm_static: launch failed: %s", cudaGetErrorString(e));
   return LSP_OK;
 }
 
