@@ -1,6 +1,6 @@
 """Device-side timing of every BASELINE.json configuration (bench.py covers the headline config 2 only).
 
-    python bench_configs.py [--steps K] [--only cfg2,fwd,packed,cfg3,cfg4,cfg5,table1,table1_30b,adamw,head]
+    python bench_configs.py [--steps K] [--only cfg2,fwd,packed,cfg3,cfg4,cfg5,table1,table1_30b,adamw,head,gemm]
 
 Prints one JSON line per configuration: ms per fwd+bwd step (CUDA events on the launching stream, after warm-up),
 tokens/s and executed TFLOP/s (causal attention FLOPs, SURVEY.md 8(d) convention).  Inputs are the seeded synthetic
@@ -182,10 +182,83 @@ def bench_head(w, steps):
     return out
 
 
+def gemm_shapes(w):
+    """The 12 GEMMs of one layer step of workload `w` as (stage, lsp_gemm op, M, N, K)."""
+    T, H, F = w.tokens, w.hidden, w.ffn
+    Nq, Nqkv = w.n_q_heads * w.head_dim, (w.n_q_heads + 2 * w.n_kv_heads) * w.head_dim
+    return [("gemm_qkv", 0, T, Nqkv, H), ("gemm_oproj", 0, T, H, Nq), ("gemm_gateup", 0, T, 2 * F, H), ("gemm_down", 0, T, H, F),
+            ("wgrad_down", 2, H, F, T), ("dgrad_down", 1, T, F, H), ("wgrad_gateup", 2, 2 * F, H, T), ("dgrad_gateup", 1, T, H, 2 * F),
+            ("wgrad_oproj", 2, H, Nq, T), ("dgrad_oproj", 1, T, Nq, H), ("wgrad_qkv", 2, Nqkv, H, T), ("dgrad_qkv", 1, T, H, Nqkv)]
+
+
+def bench_gemm_shapes(w, steps):
+    """Every GEMM shape of the layer step, alone: lsp_gemm (the tcgen05 kernel with its plain fp32-store epilogue; fp16 operands
+    as in the layer, and bf16 operands) against cuBLAS through torch (bf16 in / bf16 out, fp16 in / fp16 out, and bf16 in / fp32
+    out where this torch offers out_dtype) on the same N(0,1) data, timed back to back in turns on the same GPU in the same
+    power state (under the pool's power cap the operand FORMAT matters: the clock settles where the board draws its cap).  cuBLAS is the library yardstick of the
+    roofline (MEASURED_PEAKS.json times it at 8192^3 only); the in-step GEMMs carry fused epilogues on top of this."""
+    dev = harness.require_cuda()
+    ctx = harness.make_ctx(synth.CFG1_TINY)
+    rows = []
+    for name, op, M, N, K in gemm_shapes(w):
+        a_shape = (K, M) if op == 2 else (M, K)
+        b_shape = (N, K) if op == 0 else (K, N)
+        a16 = torch.randn(a_shape, dtype=torch.float32, device=dev).to(torch.float16)
+        b16 = torch.randn(b_shape, dtype=torch.float32, device=dev).to(torch.float16)
+        ab, bb = a16.to(torch.bfloat16), b16.to(torch.bfloat16)
+        c32 = torch.empty((M, N), dtype=torch.float32, device=dev)
+        cb = torch.empty((M, N), dtype=torch.bfloat16, device=dev)
+        ta = ab.t() if op == 2 else ab
+        tb = bb.t() if op == 0 else bb
+
+        th = a16.t() if op == 2 else a16
+        tbh = b16.t() if op == 0 else b16
+        ch = torch.empty((M, N), dtype=torch.float16, device=dev)
+
+        def ours():
+            B.lsp_gemm(ctx, op, M, N, K, a16, a_shape[1], B.LSP_F16, b16, b_shape[1], B.LSP_F16, c32, N)
+
+        def ours_bf16():
+            B.lsp_gemm(ctx, op, M, N, K, ab, a_shape[1], B.LSP_BF16, bb, b_shape[1], B.LSP_BF16, c32, N)
+
+        def cublas_bf16():
+            torch.mm(ta, tb, out=cb)
+
+        def cublas_f16():
+            torch.mm(th, tbh, out=ch)
+
+        def cublas_f32():
+            torch.mm(ta, tb, out_dtype=torch.float32, out=c32)
+        try:
+            cublas_f32()
+            have_f32 = True
+        except (TypeError, RuntimeError):
+            have_f32 = False
+        fns = {"ours": ours, "ours_bf16_operands": ours_bf16, "cublas_bf16_out": cublas_bf16, "cublas_f16_in_out": cublas_f16}
+        if have_f32:
+            fns["cublas_f32_out"] = cublas_f32
+        best = {k: 1e9 for k in fns}
+        for _ in range(3):                                   # in turns: the same thermal / power state for all
+            for k, f in fns.items():
+                best[k] = min(best[k], _time(f, steps))
+        fl = 2.0 * M * N * K
+        row = {"config": "gemm_" + w.name, "stage": name, "op": op, "M": M, "N": N, "K": K}
+        for k, v in best.items():
+            row[k + "_ms"] = round(v, 4)
+            row[k + "_tflops"] = round(fl / v / 1e9, 1)
+        rows.append(row)
+        print(json.dumps(row), flush=True)
+        del a16, b16, ab, bb, c32, cb, ch
+        torch.cuda.empty_cache()
+    keys = [k for k in rows[0] if k.endswith("_ms")]
+    print(json.dumps({"config": "gemm_" + w.name, "stage": "sum of the 12", **{k: round(sum(r[k] for r in rows), 4) for k in keys}}), flush=True)
+    ctx.close()
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--only", default="cfg2,fwd,packed,cfg3,cfg4,cfg5,table1,table1_30b,adamw,head")
+    ap.add_argument("--only", default="cfg2,fwd,packed,cfg3,cfg4,cfg5,table1,table1_30b,adamw,head,gemm")
     args = ap.parse_args(argv)
     B.lib()
     only = set(args.only.split(","))
@@ -217,6 +290,8 @@ def main(argv=None):
             print(json.dumps({"config": "adamw_" + w.name, "params": nparam, "ms_per_step": round(ms, 4),
                               "algorithmic_GB_per_s": round(34.0 * nparam / (ms * 1e-3) / 1e9, 1)}), flush=True)
             torch.cuda.empty_cache()
+    if "gemm" in only:
+        bench_gemm_shapes(synth.CFG2_3B_LAYER, max(args.steps, 20))
     if "head" in only:
         w = synth.CFG3_3B_STACK
         r = bench_head(w, min(args.steps, 5))
