@@ -91,9 +91,10 @@ def main(argv=None):
         torch.cuda.synchronize()
         a = read()
         print("\n== attn_bwd_dkdv_tc_kernel, CTA 5, blocks 16.. (softmax warp | MMA warp); 2048 tensor cycles per 128 x 128 block")
-        table(a, {2: "dpt_full", 3: "dS arrive", 19: "mma dS", 20: "dK issued", 21: "dPT issued"}, args.blocks)
+        table(a, {0: "st_full", 1: "P arrive", 2: "dpt_full", 3: "dS arrive", 16: "mma P", 17: "dV issued", 18: "ST+1 issued", 19: "mma dS",
+                  20: "dK issued", 21: "dPT+1 issued"}, args.blocks)
         print("\n== attn_bwd_dq_tc_kernel, CTA 7, blocks 96.. (softmax warp | MMA warp); 768 tensor cycles per 128 x 64 block")
-        table(a, {0: "sdp_full", 1: "dS arrive", 16: "mma dS", 17: "dQ issued", 18: "SdP+2 issued"}, args.blocks)
+        table(a, {8: "sdp_full", 9: "dS arrive", 24: "mma dS", 25: "dQ issued", 26: "SdP+2 issued"}, args.blocks)
         ctx.close()
         del lib
     return 0

@@ -916,12 +916,18 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
             const float4 L = l4[i];
             float2 a = ffma2(make_float2(__uint_as_float(sr[q][4 * i]), __uint_as_float(sr[q][4 * i + 1])), c2, make_float2(-L.x, -L.y));
             float2 b2 = ffma2(make_float2(__uint_as_float(sr[q][4 * i + 2]), __uint_as_float(sr[q][4 * i + 3])), c2, make_float2(-L.z, -L.w));
-            if (LSP_ATTN_BWD_POLY_EXP && (i & 1) == 0) {               // one key pair in four on the FMA pipe (the phase is SFU-bound)
+            // LSP_ATTN_BWD_POLY_EXP quarters of the key pairs on the FMA pipe (the phase is SFU-bound): 1 = a of even i, 2 = every a,
+            // 3 = every a and b2 of even i
+            if (LSP_ATTN_BWD_POLY_EXP >= 2 || (LSP_ATTN_BWD_POLY_EXP == 1 && (i & 1) == 0)) {
               a = ex2_poly2(a);
             } else {
               a.x = ex2_approx(a.x); a.y = ex2_approx(a.y);
             }
-            b2.x = ex2_approx(b2.x); b2.y = ex2_approx(b2.y);
+            if (LSP_ATTN_BWD_POLY_EXP >= 3 && (i & 1) == 0) {
+              b2 = ex2_poly2(b2);
+            } else {
+              b2.x = ex2_approx(b2.x); b2.y = ex2_approx(b2.y);
+            }
             pv[32 * q + 4 * i] = a.x; pv[32 * q + 4 * i + 1] = a.y; pv[32 * q + 4 * i + 2] = b2.x; pv[32 * q + 4 * i + 3] = b2.y;
           }
           if (rel == 0) {                                              // diagonal block: query (col0 + 32 q + i) < key (row) is masked
@@ -1201,7 +1207,7 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
         // (polling kv_full of block g + 2 together with ds_full here was measured: it holds dQ(g) back whenever that tile
         // is still in flight -- 0.88 instead of 0.82 ms; the K / V wait stays behind the dQ issue)
         mbar_wait(ds_full(buf), (g / ATC_DQ_NB) & 1u);
-        if (lane == 0) ATC_TR3(g, 16);
+        if (lane == 0) ATC_TR3(g, 24);
         if (j == 0 && it > 0) mbar_wait(acc_free(), (it - 1u) & 1u); // the previous item's dQ has been read out
         tc_fence_after();
         if (leader) {
@@ -1218,10 +1224,10 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
           }
           umma_commit(kv_empty(st));
         }
-        if (lane == 0) ATC_TR3(g, 17);
+        if (lane == 0) ATC_TR3(g, 25);
         if (j + 2 < iters) {                                         // this block's S / dP buffers are free again (in-order issue)
           issue_sdp(g + 2, true);
-          if (lane == 0) ATC_TR3(g, 18);
+          if (lane == 0) ATC_TR3(g, 26);
           if (j + 3 == iters && leader) umma_commit(qa_free());
         }
       }
@@ -1267,7 +1273,7 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
         const int buf = g % ATC_DQ_NB;
         mbar_wait(sdp_full(buf), (g / ATC_DQ_NB) & 1u);
         const bool tr = quarter == 0 && half == 0 && lane == 0;
-        if (tr) ATC_TR3(g, 0);
+        if (tr) ATC_TR3(g, 8);
         tc_fence_after();
         uint32_t sr[32], dr[32];
         tmem_ld32(tmem_base + lane_off + ATC_DQ_S + buf * 64 + col0, sr);
@@ -1304,7 +1310,7 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(ds_full(buf));
-        if (tr) ATC_TR3(g, 1);
+        if (tr) ATC_TR3(g, 9);
       }
       const uint32_t next = get_item(it + 1);
       if (next < nitems) copy_in(it + 1);

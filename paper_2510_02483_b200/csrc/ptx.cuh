@@ -60,20 +60,6 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
       : "memory");
   return ok != 0;
 }
-// non-blocking test of a phase (mbarrier.test_wait never suspends the thread; try_wait may)
-__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
-  uint32_t ok;
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-      "selp.u32 %0, 1, 0, p;\n"
-      "}\n"
-      : "=r"(ok)
-      : "r"(bar), "r"(parity)
-      : "memory");
-  return ok != 0;
-}
 // Bounded wait: a protocol bug traps (kernel error) instead of hanging the GPU.  The clock is read only every
 // 4096 polls so that a waiting warp costs its scheduler few issue slots (try_wait itself suspends the thread for a
 // hardware-defined interval before returning false).
