@@ -73,6 +73,7 @@ __device__ __forceinline__ void load_tile_async(uint32_t sbase, const __half* g,
 // grid (ceil(S/128), nq, B), 256 threads: warp w owns query rows 16w..16w+15 of the block.
 template <int D>
 __global__ void __launch_bounds__(256, 1) attn_fwd_kernel(const AttnParams p) {
+  pdl_trigger(); pdl_wait();                     // programmatic dependent launch (ptx.cuh): no global access above
   constexpr int BM = 128, BN = 64, NT = 256;
   constexpr int KS = D / 16;            // k-steps over head_dim
   constexpr int ND = D / 8;             // n-tiles over head_dim (O accumulator)
@@ -233,6 +234,7 @@ __global__ void __launch_bounds__(256, 1) attn_fwd_kernel(const AttnParams p) {
 template <int D, bool PARTS4>
 __global__ void attn_dvec_kernel(const __half* dO, long long lddo, const float* o32, long long ldo, float* dvec,
                                  int B, int S, int nq) {
+  pdl_trigger(); pdl_wait();                     // programmatic dependent launch (ptx.cuh): no global access above
   const long long gw = (static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
   const long long total = static_cast<long long>(B) * S * nq;
@@ -287,6 +289,7 @@ __device__ __forceinline__ void store_grad_tile(float (&acc)[D / 8][4], float sc
 // heads of this kv head and the query blocks at/after the diagonal; dK/dV group-sums stay in registers.
 template <int D>
 __global__ void __launch_bounds__(128, 2) attn_bwd_dkdv_kernel(const AttnParams p) {
+  pdl_trigger(); pdl_wait();                     // programmatic dependent launch (ptx.cuh): no global access above
   constexpr int BN = 64, BM = 64, NT = 128;
   constexpr int KS = D / 16, ND = D / 8;
   extern __shared__ __align__(128) uint8_t smem[];
@@ -442,6 +445,7 @@ __global__ void __launch_bounds__(128, 2) attn_bwd_dkdv_kernel(const AttnParams 
 // grid (ceil(S/64), nq, B), 128 threads: warp w owns queries 16w..16w+15; loops over key blocks <= diagonal.
 template <int D>
 __global__ void __launch_bounds__(128, 2) attn_bwd_dq_kernel(const AttnParams p) {
+  pdl_trigger(); pdl_wait();                     // programmatic dependent launch (ptx.cuh): no global access above
   constexpr int BM = 64, BN = 64, NT = 128;
   constexpr int KS = D / 16, ND = D / 8;
   extern __shared__ __align__(128) uint8_t smem[];
@@ -573,8 +577,7 @@ cudaError_t attn_fwd_launch(const AttnParams& p, cudaStream_t st) {
     once.done();
   }
   dim3 grid((p.S + 127) / 128, p.nq, p.B);
-  attn_fwd_kernel<D><<<grid, 256, attn_fwd_smem<D>(), st>>>(p);
-  return cudaGetLastError();
+  return launch_kernel(attn_fwd_kernel<D>, grid, dim3(256), attn_fwd_smem<D>(), st, p);
 }
 template <int D, bool PARTS4>
 cudaError_t attn_dvec_launch(const __half* dO, long long lddo, const float* o32, long long ldo, float* dvec, int B, int S,
@@ -582,8 +585,7 @@ cudaError_t attn_dvec_launch(const __half* dO, long long lddo, const float* o32,
   const long long warps = static_cast<long long>(B) * S * nq;
   const int threads = 256;
   const long long blocks = (warps * 32 + threads - 1) / threads;
-  attn_dvec_kernel<D, PARTS4><<<static_cast<unsigned>(blocks), threads, 0, st>>>(dO, lddo, o32, ldo, dvec, B, S, nq);
-  return cudaGetLastError();
+  return launch_kernel(attn_dvec_kernel<D, PARTS4>, dim3(static_cast<unsigned>(blocks)), dim3(threads), 0, st, dO, lddo, o32, ldo, dvec, B, S, nq);
 }
 template <int D>
 cudaError_t attn_bwd_launch(const AttnParams& p, cudaStream_t st) {
@@ -596,12 +598,10 @@ cudaError_t attn_bwd_launch(const AttnParams& p, cudaStream_t st) {
     once.done();
   }
   dim3 g1((p.S + 63) / 64, p.nkv, p.B);
-  attn_bwd_dkdv_kernel<D><<<g1, 128, attn_dkdv_smem<D>(), st>>>(p);
-  cudaError_t e = cudaGetLastError();
+  cudaError_t e = launch_kernel(attn_bwd_dkdv_kernel<D>, g1, dim3(128), attn_dkdv_smem<D>(), st, p);
   if (e != cudaSuccess) return e;
   dim3 g2((p.S + 63) / 64, p.nq, p.B);
-  attn_bwd_dq_kernel<D><<<g2, 128, attn_dq_smem<D>(), st>>>(p);
-  return cudaGetLastError();
+  return launch_kernel(attn_bwd_dq_kernel<D>, g2, dim3(128), attn_dq_smem<D>(), st, p);
 }
 
 }  // namespace lsp

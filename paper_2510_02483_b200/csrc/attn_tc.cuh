@@ -232,6 +232,8 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
+  pdl_trigger();
+  pdl_wait();                                    // no global access above (programmatic dependent launch, ptx.cuh)
 
   // item `it` of this CTA: published by the producer thread in slot it % ATC_ITEM_RING (slot reuse is safe: the
   // producer can be at most two items ahead of the slowest reader, see the q_empty / o_free dependencies)
@@ -585,9 +587,8 @@ inline cudaError_t attn_fwd_tc_launch(const __half* q, long long ldq, const __ha
   if (p.o16 && !make_map_store(&maps.o16, p.o16, p.nq * ATC_D, p.S, p.B, p.ldo, false)) return cudaErrorInvalidValue;
   const int nitems = ((p.S + 255) / 256) * p.nq * p.B;
   const int grid = nitems < num_sms ? nitems : num_sms;        // persistent: one CTA per SM
-  if (p.doc_start) attn_fwd_tc_kernel<true><<<grid, ATC_FWD_THREADS, ATC_FWD_SMEM, st>>>(maps, p);
-  else attn_fwd_tc_kernel<false><<<grid, ATC_FWD_THREADS, ATC_FWD_SMEM, st>>>(maps, p);
-  return cudaGetLastError();
+  if (p.doc_start) return launch_kernel(attn_fwd_tc_kernel<true>, dim3(grid), dim3(ATC_FWD_THREADS), ATC_FWD_SMEM, st, maps, p);
+  return launch_kernel(attn_fwd_tc_kernel<false>, dim3(grid), dim3(ATC_FWD_THREADS), ATC_FWD_SMEM, st, maps, p);
 }
 
 // =========================================================================================== backward
@@ -753,6 +754,8 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
+  pdl_trigger();
+  pdl_wait();                                    // no global access above (programmatic dependent launch, ptx.cuh)
 
   if (warp == 0) {
     // ===================================================================== producer: TMA tiles + L, D vectors
@@ -1128,6 +1131,8 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
+  pdl_trigger();
+  pdl_wait();                                    // no global access above (programmatic dependent launch, ptx.cuh)
 
   auto get_item = [&](uint32_t it) -> uint32_t {
     mbar_wait(item_bar(it % ATC_ITEM_RING), (it / ATC_ITEM_RING) & 1u);
@@ -1375,9 +1380,8 @@ inline cudaError_t attn_bwd_dkdv_tc_launch(const __half* q, long long ldq, const
       (p.dk16 && !make_map_store(&m1.g16[1], p.dk16, p.nkv * ATC_D, p.S, p.B, p.ldd16, false)))
     return cudaErrorInvalidValue;
   dim3 g1(((p.S + 127) / 128) * p.nkv * p.B, 1, 1);
-  if (p.doc_start) attn_bwd_dkdv_tc_kernel<true><<<g1, ATC_BWD_THREADS, ATC_BWD_SMEM, st>>>(m1, p);
-  else attn_bwd_dkdv_tc_kernel<false><<<g1, ATC_BWD_THREADS, ATC_BWD_SMEM, st>>>(m1, p);
-  return cudaGetLastError();
+  if (p.doc_start) return launch_kernel(attn_bwd_dkdv_tc_kernel<true>, g1, dim3(ATC_BWD_THREADS), ATC_BWD_SMEM, st, m1, p);
+  return launch_kernel(attn_bwd_dkdv_tc_kernel<false>, g1, dim3(ATC_BWD_THREADS), ATC_BWD_SMEM, st, m1, p);
 }
 
 // dQ: Q, dO as 128-row tiles; K, V streamed as 64-row tiles
@@ -1396,9 +1400,8 @@ inline cudaError_t attn_bwd_dq_tc_launch(const __half* q, long long ldq, const _
     return cudaErrorInvalidValue;
   const int nitems = ((p.S + 127) / 128) * p.nq * p.B;
   const int grid = nitems < num_sms ? nitems : num_sms;        // persistent: one CTA per SM
-  if (p.doc_start) attn_bwd_dq_tc_kernel<true><<<grid, ATC_BWD_THREADS, ATC_DQ_SMEM, st>>>(m2, p);
-  else attn_bwd_dq_tc_kernel<false><<<grid, ATC_BWD_THREADS, ATC_DQ_SMEM, st>>>(m2, p);
-  return cudaGetLastError();
+  if (p.doc_start) return launch_kernel(attn_bwd_dq_tc_kernel<true>, dim3(grid), dim3(ATC_BWD_THREADS), ATC_DQ_SMEM, st, m2, p);
+  return launch_kernel(attn_bwd_dq_tc_kernel<false>, dim3(grid), dim3(ATC_BWD_THREADS), ATC_DQ_SMEM, st, m2, p);
 }
 
 }  // namespace lsp

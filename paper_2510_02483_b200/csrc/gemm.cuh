@@ -652,6 +652,8 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, c
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
+  pdl_trigger();
+  pdl_wait();                                    // no global access above (programmatic dependent launch, ptx.cuh)
 
   if (warp == 0) {
     // ===================================================================== TMA producer
@@ -899,6 +901,8 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
   cluster_sync_all();                            // barriers of both CTAs initialised before any remote arrival / TMA
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
+  pdl_trigger();                                 // the next kernel of the stream may be scheduled (it waits for this one to complete)
+  pdl_wait();                                    // everything above ran under the previous kernel's tail; no global access before here
 
   if (warp == 0) {
     // ===================================================================== TMA producer (both CTAs)
@@ -1232,8 +1236,7 @@ cudaError_t launch_gemm_pair(const GemmMaps& maps, GemmShape sh, const Epi& epi,
     const int s = gemm_tail_split(ntiles, clusters, sh.kblocks[0]);
     if (s >= 2) { sh.sk_split = s; sh.sk_partial = sk->partial; sh.sk_flags = sk->flags; sh.sk_epoch = sk->epoch; }
   }
-  kern<<<2 * clusters, GEMM_THREADS, G::SMEM_BYTES, st>>>(maps, sh, epi);
-  return cudaGetLastError();
+  return launch_kernel(kern, dim3(2 * clusters), dim3(GEMM_THREADS), G::SMEM_BYTES, st, maps, sh, epi);
 }
 
 template <int BN, bool A_MN, bool B_MN, bool DUAL, class Epi>
@@ -1253,8 +1256,7 @@ cudaError_t launch_gemm(const GemmMaps& maps, GemmShape sh, const Epi& epi, int 
   sh.band = gemm_band(mblocks);
   sh.sk_split = 0; sh.sk_partial = nullptr; sh.sk_flags = nullptr; sh.sk_epoch = 0;
   const int grid = ntiles < num_sms ? ntiles : num_sms;
-  kern<<<grid, GEMM_THREADS, Cfg::SMEM_BYTES, st>>>(maps, sh, epi);
-  return cudaGetLastError();
+  return launch_kernel(kern, dim3(grid), dim3(GEMM_THREADS), Cfg::SMEM_BYTES, st, maps, sh, epi);
 }
 
 // Generic entry: up to three K-segments (A_s, B_s, K_s); all segments share the operand majors.

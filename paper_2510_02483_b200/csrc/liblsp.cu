@@ -210,10 +210,9 @@ cudaError_t norm_fwd_t(const lsp_ctx* c, const void* x, const void* g, __half* x
   const int H = c->d.hidden, nv = (H / 4 + NORM_THREADS - 1) / NORM_THREADS;
   const XT* xp = static_cast<const XT*>(x);
   const __nv_bfloat16* gp = static_cast<const __nv_bfloat16*>(g);
-#define LSP_NF(NV) case NV: rmsnorm_fwd_kernel<XT, NV><<<c->T, NORM_THREADS, 0, st>>>(xp, gp, xn, rstd, H, c->d.rms_eps); break;
+#define LSP_NF(NV) case NV: return launch_kernel(rmsnorm_fwd_kernel<XT, NV>, dim3(c->T), dim3(NORM_THREADS), 0, st, xp, gp, xn, rstd, H, c->d.rms_eps);
   switch (nv) { LSP_NF(1) LSP_NF(2) LSP_NF(3) LSP_NF(4) LSP_NF(5) LSP_NF(6) LSP_NF(7) LSP_NF(8) default: return cudaErrorInvalidValue; }
 #undef LSP_NF
-  return cudaGetLastError();
 }
 cudaError_t norm_fwd(const lsp_ctx* c, int dt, const void* x, const void* g, __half* xn, float* rstd, cudaStream_t st) {
   return dt == LSP_F32 ? norm_fwd_t<float>(c, x, g, xn, rstd, st) : norm_fwd_t<__nv_bfloat16>(c, x, g, xn, rstd, st);
@@ -235,21 +234,20 @@ cudaError_t norm_bwd_t(const lsp_ctx* c, const void* x, const float* rstd, const
   if (stages > NORMB_MAX_STAGES) stages = NORMB_MAX_STAGES;
   if (stages < 2) return cudaErrorInvalidValue;
   const size_t smem = stages * stage_bytes;
+  cudaError_t launch_err = cudaSuccess;
 #define LSP_NB(NV, GG) case NV: { \
     auto kern = rmsnorm_bwd_kernel<XT, RT, NV, GG>; \
     static DeviceOnce once; \
     if (once.need()) { cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, NORMB_SMEM_BUDGET); if (e != cudaSuccess) return e; once.done(); } \
-    kern<<<nb, NORMB_THREADS, smem, st>>>(xp, rstd, gp, dxn, rp, dx, dx16, dg_part, c->T, H, stages, residual_scale(c->d), c->overflow); } break;
+    launch_err = launch_kernel(kern, dim3(nb), dim3(NORMB_THREADS), smem, st, xp, rstd, gp, dxn, rp, dx, dx16, dg_part, c->T, H, stages, residual_scale(c->d), c->overflow); } break;
   if (G == 2) {
     switch (nv) { LSP_NB(1, 2) LSP_NB(2, 2) LSP_NB(3, 2) LSP_NB(4, 2) LSP_NB(5, 2) LSP_NB(6, 2) LSP_NB(7, 2) LSP_NB(8, 2) default: return cudaErrorInvalidValue; }
   } else {
     switch (nv) { LSP_NB(5, 1) LSP_NB(6, 1) LSP_NB(7, 1) LSP_NB(8, 1) default: return cudaErrorInvalidValue; }
   }
 #undef LSP_NB
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
-  colsum_kernel<<<(H + 31) / 32, 256, 0, st>>>(dg_part, dg, nb * G, H, dg_accumulate);
-  return cudaGetLastError();
+  if (launch_err != cudaSuccess) return launch_err;
+  return launch_kernel(colsum_kernel, dim3((H + 31) / 32), dim3(256), 0, st, static_cast<const float*>(dg_part), dg, nb * G, H, dg_accumulate);
 }
 // x: forward input of the norm (XT = x_dt); dres: incoming residual gradient (RT = r_dt)
 cudaError_t norm_bwd(const lsp_ctx* c, int x_dt, int r_dt, const void* x, const float* rstd, const void* g, const float* dxn,
@@ -266,16 +264,14 @@ cudaError_t cast_f32_f16(const float* in, __half* out, long long n, int sms, uns
   long long blocks = (n8 + 255) / 256;
   if (blocks > sms * 16LL) blocks = sms * 16LL;
   if (blocks < 1) blocks = 1;
-  cast_f32_f16_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(in, out, n8, counter);
-  return cudaGetLastError();
+  return launch_kernel(cast_f32_f16_kernel, dim3(static_cast<unsigned>(blocks)), dim3(256), 0, st, in, out, n8, counter);
 }
 cudaError_t cast_bf16_f16(const __nv_bfloat16* in, __half* out, long long n, int sms, unsigned long long* counter, cudaStream_t st) {
   const long long n8 = n / 8;
   long long blocks = (n8 + 255) / 256;
   if (blocks > sms * 16LL) blocks = sms * 16LL;
   if (blocks < 1) blocks = 1;
-  cast_bf16_f16_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(in, out, n8, counter);
-  return cudaGetLastError();
+  return launch_kernel(cast_bf16_f16_kernel, dim3(static_cast<unsigned>(blocks)), dim3(256), 0, st, in, out, n8, counter);
 }
 
 // up to CAST_MAX_SEGS bf16 -> fp16 weight casts in one launch (element counts are multiples of 8)
@@ -294,8 +290,7 @@ cudaError_t cast_weights(const lsp_ctx* c, int nseg, const void* const* src, __h
   long long blocks = (segs.start[nseg] + 255) / 256;
   if (blocks > c->num_sms * 16LL) blocks = c->num_sms * 16LL;
   if (blocks < 1) blocks = 1;
-  cast_multi_bf16_f16_kernel<<<static_cast<unsigned>(blocks), 256, 0, st>>>(segs);
-  return cudaGetLastError();
+  return launch_kernel(cast_multi_bf16_f16_kernel, dim3(static_cast<unsigned>(blocks)), dim3(256), 0, st, segs);
 }
 
 }  // namespace

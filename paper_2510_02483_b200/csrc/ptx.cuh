@@ -8,8 +8,10 @@
 #include <cuda_fp16.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <stdlib.h>
 
 #include <atomic>
+#include <utility>
 
 namespace lsp {
 
@@ -32,6 +34,35 @@ struct DeviceOnce {
     if (d <= 63) mask.fetch_or(1ull << d, std::memory_order_release);     // setting an attribute twice is harmless
   }
 };
+
+// ------------------------------------------------------------------------------------------- programmatic dependent launch
+// The tensor-core kernels of a step follow one another on one stream.  Launched with the programmatic-stream-serialization
+// attribute, kernel n+1's CTAs are scheduled as kernel n's CTAs leave their SMs (every CTA of n calls pdl_trigger early;
+// n+1's need the whole SM, so they only land where n is done) and run their prologue -- barrier init, TMEM allocation,
+// descriptor prefetch -- under n's tail; pdl_wait() (griddepcontrol.wait: returns when kernel n has COMPLETED and its
+// writes are visible) stands before the first global-memory access of every such kernel, so nothing else changes.
+// Both instructions are no-ops in a kernel launched the ordinary way.  On by default; LSP_PDL=0 in the environment (read once)
+// launches every kernel the ordinary way.  Measured (profiles/r2_notes.md): config 1 (23 launches, launch-bound) 0.198 ->
+// 0.161 ms per step, config 2 -0.2 .. -1 % (inside the spread of the power-capped boxes); results are bit-identical.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+#ifndef LSP_PDL_DEFAULT
+#define LSP_PDL_DEFAULT 1
+#endif
+inline bool pdl_enabled() {
+  static const int v = [] { const char* e = getenv("LSP_PDL"); return e ? atoi(e) : LSP_PDL_DEFAULT; }();
+  return v != 0;
+}
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_kernel(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = pdl_enabled() ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
+}
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
