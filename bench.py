@@ -157,6 +157,20 @@ def time_oracle(w, steps, warmup, sample_seq=SAMPLE_SEQ):
     return S / dt, dt, sample
 
 
+def host_cpu():
+    """(nproc, CPU model string) of the box the oracle is timed on (print both beside the baseline)."""
+    model = "unknown"
+    try:
+        with open("/proc/cpuinfo") as f:
+            for ln in f:
+                if ln.lower().startswith("model name"):
+                    model = ln.split(":", 1)[1].strip()
+                    break
+    except OSError:
+        pass
+    return os.cpu_count() or 0, model
+
+
 def time_oracle_full(w):
     """One step of the WHOLE workload (every sequence, full length) through oracle/lspref.layer_fwd_bwd, as it stands."""
     from oracle import lspref as R
@@ -186,7 +200,8 @@ def run_reference(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "batch": w.batch, "seq": w.seq, "hidden": w.hidden, "n_q_heads": w.n_q_heads,
                        "n_kv_heads": w.n_kv_heads, "head_dim": w.head_dim, "ffn": w.ffn, "sample": sample},
-            "cpu_baseline": {"value": tps, "unit": "tokens/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": tps, "unit": "tokens/s", "cores": cores, "kind": "oracle", "sample": sample,
+                             "nproc": host_cpu()[0], "cpu_model": host_cpu()[1]},
             "e2e": {"value": tps, "unit": "tokens/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -378,7 +393,7 @@ def run_ours(args):
     if renv.is_main and renv.world_size == 1 and not args.no_cpu_baseline:
         tps, dt, sample = time_oracle(w, 3, 1) if args.cpu_baseline_sample else time_oracle_full(w)
         line["cpu_baseline"] = {"value": tps, "unit": "tokens/s", "cores": blas_threads(), "kind": "oracle", "sample": sample,
-                                "s_per_step": dt}
+                                "s_per_step": dt, "nproc": host_cpu()[0], "cpu_model": host_cpu()[1]}
     ctx.close()
     replicas.finalize()
     if renv.is_main:
