@@ -1,7 +1,8 @@
 #!/usr/bin/env python
-"""clock64 traces of the three tcgen05 attention kernels (forward, dK/dV, dQ) at the attention shape of config 2.
+"""clock64 traces of the three tcgen05 attention kernels (forward, dK/dV, dQ) at the attention shape of config 2, and
+(--gemm) the wait counters of the GEMM kernel's MMA warp for the 12 GEMM shapes of the config-2 step.
 
-    python bench_trace.py [--blocks N] > profiles/rX_attn_traces.txt
+    python bench_trace.py [--blocks N] [--gemm] > profiles/rX_attn_traces.txt
 
 Builds a DEBUG copy of the library with -DLSP_ATTN_TRACE into a temporary directory (the shipped liblsp.so carries no
 trace code), loads it in place of the product library for this process only, runs lsp_sdpa_fwd / lsp_sdpa_bwd on the
@@ -29,7 +30,7 @@ if ROOT not in sys.path:
 def build_traced(tmp):
     from paper_2510_02483_b200 import build as Bd
     out = os.path.join(tmp, "liblsp_trace.so")
-    cmd = [os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")] + Bd.NVCC_FLAGS + ["-DLSP_ATTN_TRACE", "-o", out] + Bd.SOURCES
+    cmd = [os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")] + Bd.NVCC_FLAGS + ["-DLSP_ATTN_TRACE", "-DLSP_GEMM_TRACE", "-o", out] + Bd.SOURCES
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError("nvcc failed:\n" + r.stdout + r.stderr)
@@ -48,9 +49,39 @@ def table(a, names, nblocks):
         print(f"median period between blocks: {per[len(per) // 2]} cycles")
 
 
+def gemm_table(lib, B, harness, synth, torch, np):
+    """Per GEMM shape of the cfg2 step (lsp_gemm, plain fp32 store): what the MMA-issuing warp of a CTA pair did -- cycles in its
+    loop, share of them spent waiting for operand stages (it runs ahead of the tensor queue: a large share is normal) and for a
+    free accumulator, and cycles per 64-wide k-block against the 512 tensor cycles a 256 x 256 x 64 pair step takes."""
+    import bench_configs as BC
+    lib.lsp_debug_read_gemm_trace.argtypes = [C.c_void_p, C.c_int]
+    lib.lsp_debug_read_gemm_trace.restype = C.c_int
+    dev = torch.device("cuda")
+    ctx = harness.make_ctx(synth.CFG1_TINY)
+    buf = (C.c_longlong * (128 * 4))()
+    print("\n== gemm_pair_tcgen05_kernel, MMA warp of every CTA pair (mean over the pairs); 512 tensor cycles per k-block")
+    print(f"{'stage':14s} {'M':>6s} {'N':>6s} {'K':>6s} {'ms':>7s} {'loop cycles':>12s} {'wait stages %':>14s} {'wait accum %':>13s} {'k-blocks':>9s} {'cycles/k-block':>15s} {'SM GHz':>7s}")
+    for name, op, M, N, K in BC.gemm_shapes(synth.CFG2_3B_LAYER):
+        a_shape = (K, M) if op == 2 else (M, K)
+        b_shape = (N, K) if op == 0 else (K, N)
+        a = torch.randn(a_shape, device=dev).to(torch.float16)
+        b = torch.randn(b_shape, device=dev).to(torch.float16)
+        c = torch.empty((M, N), dtype=torch.float32, device=dev)
+        ms = BC._time(lambda: B.lsp_gemm(ctx, op, M, N, K, a, a_shape[1], B.LSP_F16, b, b_shape[1], B.LSP_F16, c, N), 20)
+        assert lib.lsp_debug_read_gemm_trace(buf, 128 * 4) == 0
+        t = np.array(buf[:], dtype=np.int64).reshape(128, 4)
+        t = t[t[:, 3] > 0]
+        loop = t[:, 0].astype(float)
+        print(f"{name:14s} {M:6d} {N:6d} {K:6d} {ms:7.3f} {loop.mean():12.0f} {100 * t[:, 1].sum() / loop.sum():14.1f} "
+              f"{100 * t[:, 2].sum() / loop.sum():13.1f} {t[:, 3].mean():9.0f} {(loop / t[:, 3]).mean():15.1f} {loop.max() / ms / 1e6:7.2f}")
+        del a, b, c
+    ctx.close()
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--blocks", type=int, default=24)
+    ap.add_argument("--gemm", action="store_true", help="also print the GEMM kernel's MMA-warp wait counters per shape")
     args = ap.parse_args(argv)
     import numpy as np
     import torch
@@ -96,6 +127,8 @@ def main(argv=None):
         print("\n== attn_bwd_dq_tc_kernel, CTA 7, blocks 96.. (softmax warp | MMA warp); 768 tensor cycles per 128 x 64 block")
         table(a, {8: "sdp_full", 9: "dS arrive", 24: "mma dS", 25: "dQ issued", 26: "SdP+2 issued"}, args.blocks)
         ctx.close()
+        if args.gemm:
+            gemm_table(lib, B, harness, synth, torch, np)
         del lib
     return 0
 

@@ -598,6 +598,11 @@ struct EpiDOutDvec {
   }
 };
 
+#ifdef LSP_GEMM_TRACE
+// debug builds only: per CTA pair {cycles in the MMA loop, cycles waiting for operand stages, cycles waiting for a free
+// accumulator, k-blocks issued} of the last gemm_pair_tcgen05_kernel launch
+__device__ long long g_gemm_trace[128 * 4];
+#endif
 // ------------------------------------------------------------------------------------------- the kernel
 // linear tile id -> (m-block, n-block), banded m-fastest order
 __device__ __forceinline__ void gemm_tile_coord(int tile, int mblocks, int nblocks, int band, int& mb, int& nb) {
@@ -951,14 +956,29 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
       const uint64_t da0 = umma_smem_desc(smem_base, A_LBO, 1024), db0 = umma_smem_desc(smem_base + A_BYTES, B_LBO, 1024);
       int stage = 0; uint32_t phase = 0;
       int acc = 0; uint32_t acc_phase = 0;
+#ifdef LSP_GEMM_TRACE
+      long long tr_t0 = clock64(), tr_full = 0, tr_tempty = 0, tr_kb = 0;
+#endif
       for (int j = 0; j < nitems; ++j) {
         const GemmItem it = work.get(j);
+#ifdef LSP_GEMM_TRACE
+        long long tr_a = clock64();
+#endif
         mbar_wait_cluster(tempty_bar(acc), acc_phase ^ 1u);
+#ifdef LSP_GEMM_TRACE
+        tr_tempty += clock64() - tr_a;
+#endif
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(acc * ACC_COLS);
         const int kb1 = min(it.kb1, kb_total);
         for (int kb = it.kb0; kb < kb1; ++kb) {
+#ifdef LSP_GEMM_TRACE
+          tr_a = clock64();
+#endif
           mbar_wait_cluster(full_bar(stage), phase);
+#ifdef LSP_GEMM_TRACE
+          tr_full += clock64() - tr_a; ++tr_kb;
+#endif
           tc_fence_after();
           if (leader) {
             const uint64_t da = desc_adv(da0, stage * STAGE_BYTES), db = desc_adv(db0, stage * STAGE_BYTES);
@@ -975,6 +995,12 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
         if (leader) umma_commit_pair(tfull_bar(acc), 3);
         if (++acc == NACC) { acc = 0; acc_phase ^= 1u; }
       }
+#ifdef LSP_GEMM_TRACE
+      if (lane == 0) {                           // debug builds only: where the MMA warp of this pair spent its time
+        long long* o = g_gemm_trace + static_cast<long long>(cid) * 4;
+        o[0] = clock64() - tr_t0; o[1] = tr_full; o[2] = tr_tempty; o[3] = tr_kb;
+      }
+#endif
     }
   } else {
     // ===================================================================== epilogue warps (2..9, both CTAs)

@@ -1336,6 +1336,14 @@ lsp_status lsp_set_packed_sequences(lsp_ctx* ctx, const int32_t* cu_seqlens_host
 
 long long lsp_launch_count(const lsp_ctx* ctx) { return ctx ? ctx->launches : -1; }
 
+#ifdef LSP_GEMM_TRACE
+// debug builds only (not declared in lsp.h): copies the last pair-GEMM launch's MMA-warp wait counters to the host
+int lsp_debug_read_gemm_trace(long long* host, int n) {
+  if (!host || n > 128 * 4) return -1;
+  if (cudaDeviceSynchronize() != cudaSuccess) return -1;
+  return cudaMemcpyFromSymbol(host, g_gemm_trace, static_cast<size_t>(n) * sizeof(long long)) == cudaSuccess ? 0 : -1;
+}
+#endif
 #ifdef LSP_ATTN_TRACE
 // debug builds only (not declared in lsp.h): copies the forward attention kernel's clock trace to the host
 int lsp_debug_read_trace(unsigned long long* host, int n) {
