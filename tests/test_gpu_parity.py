@@ -2,6 +2,9 @@
 on the same seeded bf16 inputs.  Bar (BASELINE.json north_star): max|gpu - ref| / rms(ref) <= 2e-2 per tensor;
 bit-exact for the integer-indexed embedding gather.
 """
+import os
+import sys
+
 import numpy as np
 import pytest
 
@@ -10,6 +13,7 @@ from paper_2510_02483_b200 import synth
 from tests.util import TOL, norm_err
 
 pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 @pytest.fixture(scope="module")
@@ -1150,6 +1154,39 @@ def test_pretrain_recompute_is_bit_identical(gpu):
     assert outs[0][0] == outs[1][0]
     for a, b in zip(outs[0][1], outs[1][1]):
         assert np.array_equal(a, b)
+
+
+_PDL_CHILD = r"""
+import hashlib, sys
+sys.path.insert(0, %r)
+from paper_2510_02483_b200 import harness, synth
+w = {"cfg1_tiny": synth.CFG1_TINY, "mid": synth.Workload("mid", 101, 2, 320, 512, 8, 2, 128, 1376, 1e-5, 500000.0),
+     "table1_3b": synth.Workload("table1_3b_small", 6, 1, 1024, 2048, 16, 2, 128, 11008, 1e-5, 10000.0)}[sys.argv[1]]
+h = hashlib.sha256()
+for rep in range(3):                      # three steps back to back: a launch that overtakes its producer would show up
+    out = harness.run_layer(w)
+    for k in sorted(out):
+        h.update(out[k].tobytes())
+print("DIGEST", h.hexdigest())
+"""
+
+
+@pytest.mark.parametrize("name", ["cfg1_tiny", "mid", "table1_3b"])
+def test_programmatic_dependent_launch_is_bit_identical(gpu, name):
+    """Programmatic dependent launch (ptx.cuh: every kernel of the layer path is launched with the programmatic-stream-
+    serialization attribute and waits with griddepcontrol.wait before its first global access) may only move WHEN a kernel
+    starts, never what it reads: y, dx and the nine gradients of three consecutive layer steps are bit-identical with
+    LSP_PDL=0 (ordinary launches) and LSP_PDL=1.  The setting is read once per process, hence the two subprocesses."""
+    import subprocess
+    digests = {}
+    for v in ("0", "1"):
+        env = dict(os.environ, LSP_PDL=v)
+        r = subprocess.run([sys.executable, "-c", _PDL_CHILD % ROOT, name], capture_output=True, text=True, env=env, timeout=600)
+        assert r.returncode == 0, r.stderr[-2000:]
+        line = [l for l in r.stdout.splitlines() if l.startswith("DIGEST ")]
+        assert line, r.stdout[-2000:]
+        digests[v] = line[-1]
+    assert digests["0"] == digests["1"]
 
 
 @pytest.mark.parametrize("w", [synth.CFG1_TINY, MID], ids=lambda w: w.name)
