@@ -380,7 +380,9 @@ def run_ours(args):
                        "n_kv_heads": w.n_kv_heads, "head_dim": w.head_dim, "ffn": w.ffn, "parallelism": f"replicas x{renv.world_size}",
                        "l2": "working set (saved+ws+weights+grads > 3 GB) far exceeds the 126 MB L2; no flush needed",
                        "weights": ("bf16 weights re-converted to fp16 operands inside every forward" if args.recast_weights else
-                                   "unchanged between steps: fp16 operand cache made once before the loop (lsp_layer_prepare_weights)")},
+                                   "unchanged between steps: fp16 operand cache made once before the loop (lsp_layer_prepare_weights)"),
+                       "launch": ("ordinary stream-ordered launches (LSP_PDL=0)" if os.environ.get("LSP_PDL") == "0" else
+                                  "programmatic dependent launch between the kernels of a step (default; LSP_PDL=0 disables)")},
             "tflops": tflops, "flops_per_step": flops,
             "frac_of_nominal_bf16_peak": tflops / renv.world_size / NOMINAL_BF16_TF,
             "frac_of_measured_sustained": tflops / renv.world_size / peaks["bf16_tflops_sustained"],
