@@ -23,6 +23,11 @@
  *  - Errors: every call returns an lsp_status; nothing throws or aborts across the ABI.  On error
  *    lsp_last_error(ctx) returns a ctx-owned message.  There is no CPU fallback.
  *  - Results are bit-reproducible run to run (no floating-point atomics anywhere).
+ *  - Launches: the kernels of a call are enqueued on the caller's stream with programmatic dependent launch between them
+ *    (each kernel waits for its predecessor's completion before its first global-memory access, so ordering is what plain
+ *    stream order gives; capture into CUDA graphs works).  Environment switches, read once per process, tuning aids only --
+ *    none changes a result bit: LSP_PDL=0 (ordinary launches), LSP_GEMM_STREAMK=0 (no split-K tail), LSP_GEMM_BAND=n
+ *    (rasterisation band), LSP_GEMM_PAIR=0 (single-CTA GEMM kernel), LSP_GEMM_MT=2 (512-row pair tiles).
  */
 #ifndef LSP_H_
 #define LSP_H_
