@@ -25,9 +25,10 @@
  *  - Results are bit-reproducible run to run (no floating-point atomics anywhere).
  *  - Launches: the kernels of a call are enqueued on the caller's stream with programmatic dependent launch between them
  *    (each kernel waits for its predecessor's completion before its first global-memory access, so ordering is what plain
- *    stream order gives; capture into CUDA graphs works).  Environment switches, read once per process, tuning aids only --
- *    none changes a result bit: LSP_PDL=0 (ordinary launches), LSP_GEMM_STREAMK=0 (no split-K tail), LSP_GEMM_BAND=n
- *    (rasterisation band), LSP_GEMM_PAIR=0 (single-CTA GEMM kernel), LSP_GEMM_MT=2 (512-row pair tiles).
+ *    stream order gives; capture into CUDA graphs works).  Environment switches, read once per process, tuning aids only:
+ *    LSP_PDL=0 (ordinary launches) and LSP_GEMM_BAND=n (rasterisation band) change no result bit; LSP_GEMM_STREAMK=0 (no
+ *    split-K tail), LSP_GEMM_PAIR=0 (single-CTA GEMM kernel) and LSP_GEMM_MT=2 (512-row pair tiles) change which tiles are
+ *    summed in K-slices, i.e. the fp32 summation order of those tiles (equal to round-off, still reproducible run to run).
  */
 #ifndef LSP_H_
 #define LSP_H_
