@@ -73,7 +73,7 @@ __device__ __forceinline__ void load_tile_async(uint32_t sbase, const __half* g,
 // grid (ceil(S/128), nq, B), 256 threads: warp w owns query rows 16w..16w+15 of the block.
 template <int D>
 __global__ void __launch_bounds__(256, 1) attn_fwd_kernel(const AttnParams p) {
-  pdl_trigger(); pdl_wait();                     // programmatic dependent launch (ptx.cuh): no global access above
+  pdl_wait(); pdl_trigger();                     // programmatic dependent launch (ptx.cuh): no global access above
   constexpr int BM = 128, BN = 64, NT = 256;
   constexpr int KS = D / 16;            // k-steps over head_dim
   constexpr int ND = D / 8;             // n-tiles over head_dim (O accumulator)
@@ -234,7 +234,7 @@ __global__ void __launch_bounds__(256, 1) attn_fwd_kernel(const AttnParams p) {
 template <int D, bool PARTS4>
 __global__ void attn_dvec_kernel(const __half* dO, long long lddo, const float* o32, long long ldo, float* dvec,
                                  int B, int S, int nq) {
-  pdl_trigger(); pdl_wait();                     // programmatic dependent launch (ptx.cuh): no global access above
+  pdl_wait(); pdl_trigger();                     // programmatic dependent launch (ptx.cuh): no global access above
   const long long gw = (static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
   const long long total = static_cast<long long>(B) * S * nq;
@@ -289,7 +289,7 @@ __device__ __forceinline__ void store_grad_tile(float (&acc)[D / 8][4], float sc
 // heads of this kv head and the query blocks at/after the diagonal; dK/dV group-sums stay in registers.
 template <int D>
 __global__ void __launch_bounds__(128, 2) attn_bwd_dkdv_kernel(const AttnParams p) {
-  pdl_trigger(); pdl_wait();                     // programmatic dependent launch (ptx.cuh): no global access above
+  pdl_wait(); pdl_trigger();                     // programmatic dependent launch (ptx.cuh): no global access above
   constexpr int BN = 64, BM = 64, NT = 128;
   constexpr int KS = D / 16, ND = D / 8;
   extern __shared__ __align__(128) uint8_t smem[];
@@ -445,7 +445,7 @@ __global__ void __launch_bounds__(128, 2) attn_bwd_dkdv_kernel(const AttnParams 
 // grid (ceil(S/64), nq, B), 128 threads: warp w owns queries 16w..16w+15; loops over key blocks <= diagonal.
 template <int D>
 __global__ void __launch_bounds__(128, 2) attn_bwd_dq_kernel(const AttnParams p) {
-  pdl_trigger(); pdl_wait();                     // programmatic dependent launch (ptx.cuh): no global access above
+  pdl_wait(); pdl_trigger();                     // programmatic dependent launch (ptx.cuh): no global access above
   constexpr int BM = 64, BN = 64, NT = 128;
   constexpr int KS = D / 16, ND = D / 8;
   extern __shared__ __align__(128) uint8_t smem[];

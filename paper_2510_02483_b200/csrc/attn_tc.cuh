@@ -232,8 +232,8 @@ attn_fwd_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcParams p
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
-  pdl_trigger();
   pdl_wait();                                    // no global access above (programmatic dependent launch, ptx.cuh)
+  pdl_trigger();
 
   // item `it` of this CTA: published by the producer thread in slot it % ATC_ITEM_RING (slot reuse is safe: the
   // producer can be at most two items ahead of the slowest reader, see the q_empty / o_free dependencies)
@@ -754,8 +754,8 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
-  pdl_trigger();
   pdl_wait();                                    // no global access above (programmatic dependent launch, ptx.cuh)
+  pdl_trigger();
 
   if (warp == 0) {
     // ===================================================================== producer: TMA tiles + L, D vectors
@@ -1131,8 +1131,8 @@ attn_bwd_dq_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwdPa
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
-  pdl_trigger();
   pdl_wait();                                    // no global access above (programmatic dependent launch, ptx.cuh)
+  pdl_trigger();
 
   auto get_item = [&](uint32_t it) -> uint32_t {
     mbar_wait(item_bar(it % ATC_ITEM_RING), (it / ATC_ITEM_RING) & 1u);

@@ -657,8 +657,8 @@ gemm_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape sh, c
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
-  pdl_trigger();
   pdl_wait();                                    // no global access above (programmatic dependent launch, ptx.cuh)
+  pdl_trigger();
 
   if (warp == 0) {
     // ===================================================================== TMA producer
@@ -906,8 +906,8 @@ gemm_pair_tcgen05_kernel(const __grid_constant__ GemmMaps maps, const GemmShape 
   cluster_sync_all();                            // barriers of both CTAs initialised before any remote arrival / TMA
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
-  pdl_trigger();                                 // the next kernel of the stream may be scheduled (it waits for this one to complete)
   pdl_wait();                                    // everything above ran under the previous kernel's tail; no global access before here
+  pdl_trigger();                                 // the next kernel of the stream may be scheduled (it waits for this one to complete)
 
   if (warp == 0) {
     // ===================================================================== TMA producer (both CTAs)

@@ -44,7 +44,7 @@ template <typename XT, int NV>
 __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_fwd_kernel(const XT* __restrict__ x, const __nv_bfloat16* __restrict__ g,
                                                                    __half* __restrict__ xn, float* __restrict__ rstd,
                                                                    int H, float eps) {
-  pdl_trigger(); pdl_wait();                     // programmatic dependent launch (ptx.cuh): no global access above
+  pdl_wait(); pdl_trigger();                     // programmatic dependent launch (ptx.cuh): no global access above
   __shared__ float red[NORM_THREADS / 32];
   const long long row = blockIdx.x;
   const XT* xr = x + row * H;
@@ -138,7 +138,7 @@ rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, con
     fence_barrier_init();
   }
   __syncthreads();
-  pdl_trigger(); pdl_wait();                     // programmatic dependent launch (ptx.cuh): no global access above
+  pdl_wait(); pdl_trigger();                     // programmatic dependent launch (ptx.cuh): no global access above
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (warp == NORMB_CONSUMERS / 32) {
@@ -222,7 +222,7 @@ rmsnorm_bwd_kernel(const XT* __restrict__ x, const float* __restrict__ rstd, con
 // dg[col] (+)= sum over CTAs of dg_part[cta][col], fixed order (deterministic).  Block = 32 columns x 8 partial groups.
 __global__ void __launch_bounds__(256) colsum_kernel(const float* __restrict__ part, float* __restrict__ out, int nparts, int H,
                                                      int accumulate) {
-  pdl_trigger(); pdl_wait();                     // programmatic dependent launch (ptx.cuh): no global access above
+  pdl_wait(); pdl_trigger();                     // programmatic dependent launch (ptx.cuh): no global access above
   __shared__ float sm[8][33];
   const int cx = threadIdx.x & 31, gy = threadIdx.x >> 5;
   const int c = blockIdx.x * 32 + cx;
@@ -246,7 +246,7 @@ __global__ void __launch_bounds__(256) colsum_kernel(const float* __restrict__ p
 // context-owned device counter (lsp_overflow_count): out-of-range input is reported, never silent.  Values below 2^-24
 // flush to zero (an absolute error far under the parity bar).
 __global__ void cast_f32_f16_kernel(const float* __restrict__ in, __half* __restrict__ out, long long n8, unsigned long long* counter) {
-  pdl_trigger(); pdl_wait();                     // programmatic dependent launch (ptx.cuh): no global access above
+  pdl_wait(); pdl_trigger();                     // programmatic dependent launch (ptx.cuh): no global access above
   unsigned int bad = 0;
   for (long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i < n8; i += static_cast<long long>(gridDim.x) * blockDim.x) {
     const float4 a = __ldg(reinterpret_cast<const float4*>(in) + 2 * i), b = __ldg(reinterpret_cast<const float4*>(in) + 2 * i + 1);
@@ -256,7 +256,7 @@ __global__ void cast_f32_f16_kernel(const float* __restrict__ in, __half* __rest
   cast_report(bad, counter);
 }
 __global__ void cast_bf16_f16_kernel(const __nv_bfloat16* __restrict__ in, __half* __restrict__ out, long long n8, unsigned long long* counter) {
-  pdl_trigger(); pdl_wait();                     // programmatic dependent launch (ptx.cuh): no global access above
+  pdl_wait(); pdl_trigger();                     // programmatic dependent launch (ptx.cuh): no global access above
   unsigned int bad = 0;
   for (long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; i < n8; i += static_cast<long long>(gridDim.x) * blockDim.x) {
     const uint4 u = __ldg(reinterpret_cast<const uint4*>(in) + i);
@@ -292,7 +292,7 @@ __device__ __forceinline__ long long cast_src_unit(const CastSegs& segs, long lo
 }
 // four independent 16-byte loads in flight per thread (the kernel is latency-bound otherwise: 2.7 TB/s with one)
 __global__ void __launch_bounds__(256) cast_multi_bf16_f16_kernel(const CastSegs segs) {
-  pdl_trigger(); pdl_wait();                     // programmatic dependent launch (ptx.cuh): no global access above
+  pdl_wait(); pdl_trigger();                     // programmatic dependent launch (ptx.cuh): no global access above
   const long long total = segs.start[segs.nseg];
   const long long stride = static_cast<long long>(gridDim.x) * blockDim.x;
   unsigned int bad = 0;

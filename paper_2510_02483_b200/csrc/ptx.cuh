@@ -36,11 +36,13 @@ struct DeviceOnce {
 };
 
 // ------------------------------------------------------------------------------------------- programmatic dependent launch
-// The tensor-core kernels of a step follow one another on one stream.  Launched with the programmatic-stream-serialization
-// attribute, kernel n+1's CTAs are scheduled as kernel n's CTAs leave their SMs (every CTA of n calls pdl_trigger early;
-// n+1's need the whole SM, so they only land where n is done) and run their prologue -- barrier init, TMEM allocation,
-// descriptor prefetch -- under n's tail; pdl_wait() (griddepcontrol.wait: returns when kernel n has COMPLETED and its
-// writes are visible) stands before the first global-memory access of every such kernel, so nothing else changes.
+// The kernels of a step follow one another on one stream.  Launched with the programmatic-stream-serialization attribute,
+// kernel n+1's CTAs are scheduled as kernel n's CTAs leave their SMs (they need the whole SM, so they only land where n
+// is done) and run their prologue -- barrier init, TMEM allocation, descriptor prefetch -- under n's tail.  Every such
+// kernel executes pdl_wait() (griddepcontrol.wait: returns when kernel n has COMPLETED and its writes are visible) before
+// its first global-memory access and pdl_trigger() (griddepcontrol.launch_dependents) right AFTER it: a kernel that has
+// triggered has seen its predecessor complete, so by induction everything older than the immediate predecessor is
+// complete when a kernel starts, and the immediate predecessor when it passes its wait.  Nothing else changes.
 // Both instructions are no-ops in a kernel launched the ordinary way.  On by default; LSP_PDL=0 in the environment (read once)
 // launches every kernel the ordinary way.  Measured (profiles/r2_notes.md): config 1 (23 launches, launch-bound) 0.198 ->
 // 0.161 ms per step, config 2 -0.2 .. -1 % (inside the spread of the power-capped boxes); results are bit-identical.
