@@ -124,6 +124,12 @@ def main(argv=None):
         print("\n== attn_bwd_dkdv_tc_kernel, CTA 5, blocks 16.. (softmax warp | MMA warp); 2048 tensor cycles per 128 x 128 block")
         table(a, {0: "st_full", 1: "P arrive", 2: "dpt_full", 3: "dS arrive", 16: "mma P", 17: "dV issued", 18: "ST+1 issued", 19: "mma dS",
                   20: "dK issued", 21: "dPT+1 issued"}, args.blocks)
+        print("\n== attn_bwd_dkdv_tc_kernel, lifetime of two CTAs (cycles from CTA entry): first S^T landed | last dS^T handed over | accumulators "
+              "complete | stores written | exit   (block iterations)")
+        for row, what in ((62, "heaviest key block (CTA 5)"), (63, "a light key block (CTA 900)")):
+            t0 = int(a[row, 10])
+            if t0:
+                print(f"{what:32s}" + "  ".join(f"{int(a[row, k]) - t0:10d}" for k in range(11, 16)) + f"   ({int(a[row, 22])} iterations)")
         print("\n== attn_bwd_dq_tc_kernel, CTA 7, blocks 96.. (softmax warp | MMA warp); 768 tensor cycles per 128 x 64 block")
         table(a, {8: "sdp_full", 9: "dS arrive", 24: "mma dS", 25: "dQ issued", 26: "SdP+2 issued"}, args.blocks)
         ctx.close()

@@ -169,7 +169,11 @@ __device__ unsigned long long g_atc_trace[64 * 32];
 #define ATC_TR(blk, ev) do { if (blockIdx.x == 3 && (blk) >= 64 && (blk) < 128) g_atc_trace[((blk) - 64) * 32 + (ev)] = clock64(); } while (0)
 #define ATC_TR2(blk, ev) do { if (blockIdx.x == 5 && (blk) >= 16 && (blk) < 80) g_atc_trace[((blk) - 16) * 32 + (ev)] = clock64(); } while (0)
 #define ATC_TR3(blk, ev) do { if (blockIdx.x == 7 && (blk) >= 96 && (blk) < 160) g_atc_trace[((blk) - 96) * 32 + (ev)] = clock64(); } while (0)
+// dK/dV CTA lifetime: events 0..5 (columns 10..15, iterations in column 22) of the heaviest CTA of group 5 (blockIdx 5) in row 62
+// and of a light one (blockIdx 900) in row 63
+#define ATC_TRL(ev) do { if (blockIdx.x == 5 || blockIdx.x == 900) g_atc_trace[(blockIdx.x == 5 ? 62 : 63) * 32 + 10 + (ev)] = clock64(); } while (0)
 #else
+#define ATC_TRL(ev) do { } while (0)
 #define ATC_TR(blk, ev) do { } while (0)
 #define ATC_TR2(blk, ev) do { } while (0)
 #define ATC_TR3(blk, ev) do { } while (0)
@@ -739,6 +743,7 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
     return qs - (doc_start ? doc_start[min(qs + 127, p.S - 1)] : 0) < ATC_SPLIT_ROWS;
   };
   const int iters = per_head * G;
+  if (threadIdx.x == 64) ATC_TRL(0);                              // CTA entered
 
   if (threadIdx.x == 0) {
     tma_prefetch_desc(&maps.q); tma_prefetch_desc(&maps.k); tma_prefetch_desc(&maps.v); tma_prefetch_desc(&maps.dO);
@@ -903,6 +908,7 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
       mbar_wait(st_full(), ph);
       const bool tr = quarter == 0 && half == 0 && lane == 0;
       if (tr) ATC_TR2(it, 0);
+      if (tr && it == 0) ATC_TRL(1);                                   // first S^T landed: the loop starts
       tc_fence_after();
       float pv[64];
       {
@@ -1003,9 +1009,11 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
       __syncwarp();
       if (lane == 0) mbar_arrive(ds_full());
       if (tr) ATC_TR2(it, 3);
+      if (tr && it == iters - 1) ATC_TRL(2);                           // last dS^T handed over
     }
     // epilogue: this warp stores rows [32 quarter, +32), columns [64 half, 64 half + 64) of dV and dK
     mbar_wait(acc_full(), 0);
+    if (quarter == 0 && half == 0 && lane == 0) ATC_TRL(3);           // accumulators complete: stores begin
     tc_fence_after();
     const int key = k0 + row;
     const bool valid = key < p.S;
@@ -1028,11 +1036,18 @@ attn_bwd_dkdv_tc_kernel(const __grid_constant__ AttnTcMaps maps, const AttnTcBwd
       }
     }
     if (lane == 0) tma_store_wait_all<0>();
+    if (quarter == 0 && half == 0 && lane == 0) ATC_TRL(4);           // this warp's stores are written
   }
 
   tc_fence_before();
   __syncthreads();
   if (warp == 1) { tc_fence_after(); tmem_dealloc(tmem_base, 512); }
+#ifdef LSP_ATTN_TRACE
+  if (threadIdx.x == 64 && (blockIdx.x == 5 || blockIdx.x == 900)) {
+    ATC_TRL(5);
+    g_atc_trace[(blockIdx.x == 5 ? 62 : 63) * 32 + 22] = static_cast<unsigned long long>(iters);
+  }
+#endif
 }
 
 // --------------------------------------------------------------------------------------------- dQ
